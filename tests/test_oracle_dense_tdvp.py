@@ -1,0 +1,85 @@
+"""Pins for oracle/dense_tdvp.py (O-D): MPO = Eq. (1), Lanczos exponential, TDVP vs ED."""
+import numpy as np
+import scipy.linalg as sla
+
+from oracle import dense_tdvp as dt
+from oracle import fermi
+
+
+def test_dense_mpo_equals_hamiltonian():
+    L, t_h, U = 4, 1.0, 4.0
+    W = dt.dense_mpo(t_h, U)
+    cur = W[0].transpose(1, 2, 0)
+    for _ in range(1, L):
+        d = cur.shape[0] * 4
+        cur = np.einsum("abw,wvcd->acbdv", cur, W).reshape(d, d, 6)
+    assert np.abs(cur[:, :, 5] - fermi.hamiltonian(L, t_h, U).toarray()).max() < 1e-13
+
+
+def test_lanczos_exp_vs_expm():
+    rng = np.random.default_rng(3)
+    n = 40
+    H = rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n))
+    H = (H + H.conj().T) / 2
+    v = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    ref = sla.expm(-0.05j * H) @ v
+    out = dt.lanczos_exp(lambda x: H @ x, v, 0.05, 12)
+    assert np.linalg.norm(out - ref) / np.linalg.norm(ref) < 1e-12
+    # exact when the Krylov space is the whole space
+    out = dt.lanczos_exp(lambda x: H @ x, v, 1.0, n)
+    assert np.linalg.norm(out - sla.expm(-1j * H) @ v) / np.linalg.norm(v) < 1e-9
+
+
+def test_heff_matches_einsum():
+    rng = np.random.default_rng(5)
+    W = dt.dense_mpo(1.0, 4.0)
+    cl, cr = 3, 5
+    Le = rng.standard_normal((cl, 6, cl)) + 1j * rng.standard_normal((cl, 6, cl))
+    Re = rng.standard_normal((cr, 6, cr)) + 1j * rng.standard_normal((cr, 6, cr))
+    th = rng.standard_normal((cl, 4, 4, cr)) + 1j * rng.standard_normal((cl, 4, 4, cr))
+    ref = np.einsum("xwa,wvps,vuqt,astb,yub->xpqy", Le, W, W, th, Re)
+    assert np.abs(dt.heff2(Le, W, Re, th) - ref).max() < 1e-12
+    A = rng.standard_normal((cl, 4, cr)) + 1j * rng.standard_normal((cl, 4, cr))
+    ref1 = np.einsum("xwa,wvps,asb,yvb->xpy", Le, W, A, Re)
+    assert np.abs(dt.heff1(Le, W, Re, A) - ref1).max() < 1e-12
+    refL = np.einsum("xps,xwa,wvpq,aqc->svc", A.conj().transpose(0, 1, 2), Le, W, A)
+    assert np.abs(dt.update_left(Le, A, W) - refL).max() < 1e-12
+    refR = np.einsum("xpy,wvpq,yvb,cqb->xwc", A.conj(), W, Re, A)
+    assert np.abs(dt.update_right(Re, A, W) - refR).max() < 1e-12
+
+
+def test_truncate_rule():
+    keep, disc = dt.truncate_rule([np.array([3.0, 2.0, 1.0]), np.array([2.5, 0.5])], [1, 2], 4, -1.0)
+    assert keep == [2, 1]                   # order 3.0(1), 2.5(2), 2.0(1) -> dim 4; 1.0 would be 5
+    tot = 9 + 4 + 1 + 2 * (6.25 + 0.25)
+    assert abs(disc - (1 + 0.5) / tot) < 1e-15
+    keep, _ = dt.truncate_rule([np.array([1.0, 1e-15])], [1], 100, -1.0)
+    assert keep == [1]                      # relative 1e-14 floor
+    keep, disc = dt.truncate_rule([np.array([1.0, 0.1, 0.01])], [1], 100, 1e-3)
+    assert keep == [2] and disc < 1e-3      # tail weight 1e-4/1.0101 <= 1e-3 after two
+    keep, _ = dt.truncate_rule([np.array([1.0]), np.array([1.0])], [3, 1], 2, -1.0)
+    assert keep == [1, 0]                   # keeps at least one even above the cap
+
+
+def test_tdvp_vs_ed_and_time_step_order():
+    """Config-1-like check at L=4: two-site TDVP from the Neel state has an O(dt^2) splitting
+    error and conserves norm/energy (E-tol in DESIGN.md)."""
+    L, t_h, U = 4, 1.0, 4.0
+    ed = fermi.ExactEvolution(L, t_h, U)
+    errs = []
+    for dtime in (0.1, 0.05):
+        td = dt.DenseTDVP(L, t_h, U, krylov_dim=10)
+        steps = int(round(1.0 / dtime))
+        err = 0.0
+        for k in range(1, steps + 1):
+            td.step(dtime)
+            o, e = td.observables(), ed.observables(dtime * k)
+            err = max(err, np.abs(o["n_up"] - e["n_up"]).max(), np.abs(o["docc"] - e["docc"]).max())
+            assert abs(o["norm2"] - 1) < 1e-11
+            assert np.abs(o["n_up"] + o["n_dn"] - 1).max() < 1e-11
+        errs.append(err)
+        psi = td.to_state()
+        H = fermi.hamiltonian(L, t_h, U)
+        assert abs(np.vdot(psi, H @ psi).real) < 1e-5           # Neel energy is 0
+    assert errs[1] < 2e-6
+    assert 3.5 < errs[0] / errs[1] < 10.0     # at least second order in dt (measured: 8.0)

@@ -1,0 +1,226 @@
+"""Pins for oracle/symm.py and oracle/symm_tdvp.py (O-S): every reduced object is expanded to
+its dense tensor ("dense embedding with coefficients expanded") and compared with the dense
+contraction of oracle/dense_tdvp.py; plus the numbers the paper prints (W = 4, Table S2)."""
+import numpy as np
+import pytest
+
+import fh_inputs as fi
+from oracle import dense_tdvp as dt
+from oracle import fermi, symm
+from oracle import symm_tdvp as stv
+
+
+def _rand(rng, m, n):
+    return rng.standard_normal((m, n)) + 1j * rng.standard_normal((m, n))
+
+
+@pytest.fixture(scope="module")
+def chain():
+    """Random symmetric MPS on an L=4 chain with all reachable sectors, degeneracies 1..3."""
+    rng = np.random.default_rng(1)
+    L, t_h, U = 4, 1.0, 4.0
+    tabs = fi.reachable_tables(L)
+    dims = [{sec: int(rng.integers(1, 4)) for sec in tabs[k]} for k in range(L + 1)]
+    dims[0] = {(0, 0): 1}
+    dims[L] = {(0, 0): 1}
+    A = [{k: _rand(rng, dims[i][k[0]], dims[i + 1][k[2]]) for k in symm.site_keys(dims[i], dims[i + 1])}
+         for i in range(L)]
+    Ws = [symm.mpo_reduced(i, t_h, U) for i in range(L)]
+    Wd = [symm.embed_mpo(Ws[i], i) for i in range(L)]
+    Ad = [symm.embed_site(A[i], dims[i], dims[i + 1], i) for i in range(L)]
+    Le = [symm.boundary_left()]
+    for i in range(L):
+        Le.append(symm.env_update_left(Le[i], A[i], Ws[i]))
+    Re = [None] * (L + 1)
+    Re[L] = symm.boundary_right()
+    for i in range(L - 1, -1, -1):
+        Re[i] = symm.env_update_right(Re[i + 1], A[i], Ws[i])
+    Ld = [symm.embed_env(Le[0], dims[0], dims[0])]
+    for i in range(L):
+        Ld.append(dt.update_left(Ld[i], Ad[i], Wd[i]))
+    Rd = [None] * (L + 1)
+    Rd[L] = symm.embed_env(Re[L], dims[L], dims[L])
+    for i in range(L - 1, -1, -1):
+        Rd[i] = dt.update_right(Rd[i + 1], Ad[i], Wd[i])
+    return dict(L=L, t_h=t_h, U=U, dims=dims, A=A, Ws=Ws, Wd=Wd, Ad=Ad, Le=Le, Re=Re, Ld=Ld, Rd=Rd, rng=rng)
+
+
+def test_reduced_site_operators_printed_values():
+    """Reading F-2: the non-zero reduced matrix elements."""
+    for eps in (1, -1):
+        o = symm.reduced_site_ops(eps)
+        r2 = np.sqrt(2.0)
+        ref_p = np.zeros((3, 3)); ref_p[0, 2] = -r2; ref_p[2, 1] = eps
+        ref_m = np.zeros((3, 3)); ref_m[1, 2] = -r2; ref_m[2, 0] = -eps
+        ref_pp = np.zeros((3, 3)); ref_pp[0, 2] = -r2; ref_pp[2, 1] = -eps
+        ref_mp = np.zeros((3, 3)); ref_mp[1, 2] = -r2; ref_mp[2, 0] = eps
+        assert np.abs(o["psi_p"] - ref_p).max() < 1e-14 and np.abs(o["psi_m"] - ref_m).max() < 1e-14
+        assert np.abs(o["psi_p_par"] - ref_pp).max() < 1e-14 and np.abs(o["psi_m_par"] - ref_mp).max() < 1e-14
+        assert np.allclose(o["one"], np.eye(3)) and np.allclose(o["p_d"], np.diag([0, 0, 1.0]))
+        assert np.allclose(o["sz"], np.diag([0.5, -0.5, 0]))
+
+
+def test_mpo_embedding_equals_H_sym_and_W4(chain):
+    """Reduced MPO bond dimension W = 4; expanded chain = dense H_sym exactly."""
+    L, Wd = chain["L"], chain["Wd"]
+    assert len(symm.MPOB) == 4
+    cur = Wd[0][0].transpose(1, 2, 0)
+    for i in range(1, L):
+        d = cur.shape[0] * 4
+        cur = np.einsum("abw,wvcd->acbdv", cur, Wd[i]).reshape(d, d, 6)
+    Hs = fermi.hamiltonian(L, chain["t_h"], chain["U"], symmetric=True).toarray()
+    assert np.abs(cur[:, :, 5] - Hs).max() < 1e-13
+    # on half-filled states H_sym = Eq. (1)
+    H = fermi.hamiltonian(L, chain["t_h"], chain["U"]).toarray()
+    sec = fermi.sector_indices(L, L // 2, L // 2)
+    assert np.abs(Hs[np.ix_(sec, sec)] - H[np.ix_(sec, sec)]).max() < 1e-13
+
+
+def test_symmetric_mps_is_a_T0_Sz0_state(chain):
+    L, Ad = chain["L"], chain["Ad"]
+    psi = Ad[0].reshape(4, -1)
+    for i in range(1, L):
+        psi = (psi @ Ad[i].reshape(Ad[i].shape[0], -1)).reshape(-1, Ad[i].shape[2])
+    psi = psi.ravel()
+    Tp, Tm, Tz = fermi.pseudospin(L)
+    _, _, Sz = fermi.spin_ops(L)
+    assert np.linalg.norm(fermi.casimir(Tp, Tm, Tz) @ psi) < 1e-12 * np.linalg.norm(psi)
+    assert np.linalg.norm(Sz @ psi) < 1e-12 * np.linalg.norm(psi)
+    # full contraction: norm and energy
+    Hs = fermi.hamiltonian(L, chain["t_h"], chain["U"], symmetric=True)
+    LL = chain["Le"][L]
+    assert abs(LL[((0, 0), 0, (0, 0))][0, 0] - np.vdot(psi, psi)) < 1e-10 * abs(np.vdot(psi, psi))
+    assert abs(LL[((0, 0), 3, (0, 0))][0, 0] - np.vdot(psi, Hs @ psi)) < 1e-10 * abs(np.vdot(psi, psi))
+
+
+def test_environments_vs_dense(chain):
+    L, dims = chain["L"], chain["dims"]
+    for i in range(L + 1):
+        dl = chain["Ld"][i]
+        dr = chain["Rd"][i]
+        assert np.abs(symm.embed_env(chain["Le"][i], dims[i], dims[i]) - dl).max() < 1e-12 * max(1, np.abs(dl).max())
+        assert np.abs(symm.embed_env(chain["Re"][i], dims[i], dims[i]) - dr).max() < 1e-12 * max(1, np.abs(dr).max())
+
+
+def test_heff2_vs_dense_hermiticity_inner(chain):
+    L, dims, rng = chain["L"], chain["dims"], chain["rng"]
+    for i in range(L - 1):
+        keys = symm.theta_keys(dims[i], dims[i + 2])
+        assert keys == fi.theta_block_keys(dims[i], dims[i + 2])
+        th = {k: _rand(rng, dims[i][k[0]], dims[i + 2][k[4]]) for k in keys}
+        ph = {k: _rand(rng, dims[i][k[0]], dims[i + 2][k[4]]) for k in keys}
+        out = symm.heff2_apply(chain["Le"][i], chain["Re"][i + 2], th, chain["Ws"][i], chain["Ws"][i + 1])
+        thd = symm.embed_theta(th, dims[i], dims[i + 2], i)
+        phd = symm.embed_theta(ph, dims[i], dims[i + 2], i)
+        ref = np.einsum("xwa,wvps,vuqt,astb,yub->xpqy", chain["Ld"][i], chain["Wd"][i], chain["Wd"][i + 1],
+                        thd, chain["Rd"][i + 2])
+        got = symm.embed_theta(out, dims[i], dims[i + 2], i)
+        assert np.linalg.norm(got - ref) < 1e-13 * np.linalg.norm(ref)
+        assert abs(symm.inner(ph, th) - np.vdot(phd, thd)) < 1e-12 * np.linalg.norm(phd) * np.linalg.norm(thd)
+        hph = symm.heff2_apply(chain["Le"][i], chain["Re"][i + 2], ph, chain["Ws"][i], chain["Ws"][i + 1])
+        assert abs(symm.inner(ph, out) - np.conj(symm.inner(th, hph))) < 1e-12 * abs(symm.inner(ph, out))
+
+
+def test_heff1_vs_dense(chain):
+    for i in range(chain["L"]):
+        dims = chain["dims"]
+        assert symm.site_keys(dims[i], dims[i + 1]) == fi.site_block_keys(dims[i], dims[i + 1])
+        out = symm.heff1_apply(chain["Le"][i], chain["Re"][i + 1], chain["A"][i], chain["Ws"][i])
+        ref = np.einsum("xwa,wvps,asb,yvb->xpy", chain["Ld"][i], chain["Wd"][i], chain["Ad"][i], chain["Rd"][i + 1])
+        got = symm.embed_site(out, dims[i], dims[i + 1], i)
+        assert np.linalg.norm(got - ref) < 1e-13 * np.linalg.norm(ref)
+
+
+def test_svd_split_vs_dense_svd(chain):
+    """F-7: singular values of the dense two-site matrix = those of M_c with multiplicity 2j_c+1;
+    nothing dropped -> merge(A1, A2) reconstructs theta; canonical forms F-6."""
+    L, dims, rng = chain["L"], chain["dims"], chain["rng"]
+    i = 1
+    keys = symm.theta_keys(dims[i], dims[i + 2])
+    th = {k: _rand(rng, dims[i][k[0]], dims[i + 2][k[4]]) for k in keys}
+    thd = symm.embed_theta(th, dims[i], dims[i + 2], i)
+    sv = np.linalg.svd(thd.reshape(thd.shape[0] * 4, -1), compute_uv=False)
+    for direction in ("right", "left"):
+        A1, A2, dm, info = symm.svd_split(th, dims[i], dims[i + 2], 10 ** 9, -1.0, direction)
+        mine = np.sort(np.concatenate([np.repeat(s, c[1] + 1) for c, s in info["svals"].items()]))[::-1]
+        n = min(len(sv), len(mine))
+        assert np.abs(sv[:n] - mine[:n]).max() < 1e-12
+        assert (sv[n:] < 1e-12).all() and (mine[n:] < 1e-12).all()
+        th2 = symm.merge(A1, A2)
+        assert max(np.abs(th2[k] - th[k]).max() for k in th) < 1e-12
+        if direction == "right":
+            chk = {}
+            for (a, s, c), x in A1.items():
+                chk[c] = chk.get(c, 0) + x.conj().T @ x
+        else:
+            chk = {}
+            for (c, s, b), x in A2.items():
+                chk[c] = chk.get(c, 0) + (b[1] + 1) / (c[1] + 1) * (x @ x.conj().T)
+        assert max(np.abs(v - np.eye(len(v))).max() for v in chk.values()) < 1e-12
+    # truncation: discarded weight equals the dense discarded weight for the same cut
+    A1, A2, dm, info = symm.svd_split(th, dims[i], dims[i + 2], 6, -1.0, "right")
+    kept_full = symm.chi_full(dm)
+    assert kept_full <= 6
+    allv = sorted(((s, c) for c, ss in info["svals"].items() for s in ss), key=lambda t: -t[0])
+    tot = sum((c[1] + 1) * s * s for s, c in allv)
+    kept_w = sum((c[1] + 1) * info["svals"][c][:k] @ info["svals"][c][:k] for c, k in info["keep"].items())
+    assert abs(info["discarded"] - (tot - kept_w) / tot) < 1e-14
+
+
+def test_task_lists_are_canonical_and_consistent(chain):
+    i, dims = 1, chain["dims"]
+    Lk, Rk = sorted(chain["Le"][i]), sorted(chain["Re"][i + 2])
+    assert Lk == [k for k in symm.env_keys(dims[i], dims[i]) if k in chain["Le"][i]]
+    tk = symm.theta_keys(dims[i], dims[i + 2])
+    st1, st2 = symm.heff2_tasks(Lk, Rk, tk, chain["Ws"][i], chain["Ws"][i + 1])
+    assert list(st1) == sorted(st1) and list(st2) == sorted(st2)
+    for segs in st1.values():
+        ks = [(e[1], e[2], t[1]) for e, t, _ in segs]
+        assert ks == sorted(ks) and all(abs(a) >= symm.ALPHA_ZERO for _, _, a in segs)
+    tup, al = symm.task_tuples(st1, list(st1), Lk, tk)
+    assert tup.dtype == np.int32 and tup.shape == (sum(len(s) for s in st1.values()), 3)
+    assert (np.diff(tup[:, 0]) >= 0).all()
+    f = symm.heff2_flops(st1, st2, dims[i], dims[i + 2])
+    assert f > 0 and f % 8 == 0
+
+
+def test_symmetric_tdvp_equals_dense_tdvp_and_measurements():
+    """O-S driver = O-D to rounding (same m, nothing truncated); H10 formula = dense measurement."""
+    L, t_h, U = 4, 1.0, 4.0
+    s = stv.SymmTDVP(L, t_h, U, krylov_dim=10)
+    d = dt.DenseTDVP(L, t_h, U, krylov_dim=10)
+    ed = fermi.ExactEvolution(L, t_h, U)
+    for k in range(1, 11):
+        s.step(0.05)
+        d.step(0.05)
+        ms, od = s.measure_local(), d.observables()
+        assert np.abs(ms["sz"] - 0.5 * (od["n_up"] - od["n_dn"])).max() < 1e-11
+        assert np.abs(ms["docc"] - od["docc"]).max() < 1e-11
+        assert np.allclose(ms["n"], 1.0)
+    psi = s.to_state()
+    assert abs(abs(np.vdot(psi, d.to_state())) - 1.0) < 1e-10       # same state up to a phase
+    e = ed.observables(0.5)
+    assert np.abs(ms["docc"] - e["docc"]).max() < 2e-6               # time-step error only
+    g = s.measure_global()
+    assert abs(g["norm2"] - 1) < 1e-11 and abs(g["energy"]) < 1e-5
+    assert s.chi() == [1, 4, 16, 4, 1] and s.chi()[1:-1] == d.bond_dims()
+    Tp, Tm, Tz = fermi.pseudospin(L)
+    assert np.linalg.norm(fermi.casimir(Tp, Tm, Tz) @ psi) < 1e-10
+
+
+def test_bookkeeping_table_s2_and_profiles():
+    """Eqs. (8)-(10) PAPER.md:216-223 on Table S2: 32 sectors,
+    chi_SU(2) = 12288, chi ~ 30000, d_max = 1735, parity n + 2j even."""
+    d = fi.table_s2_profile()
+    assert len(d) == 32 and symm.chi_su2(d) == 12288 and symm.d_max(d) == 1735
+    assert symm.chi_full(d) == 30842 and abs(symm.chi_full(d) / 30000 - 1) < 0.05
+    assert all((q + tj) % 2 == 0 for q, tj in d)
+    assert 2.3 < symm.chi_full(d) / symm.chi_su2(d) < 2.6            # "chi ~ 2.4 chi_SU(2)" PAPER.md:233
+    for k in (29, 30, 31):
+        p = fi.gaussian_profile(k, 1024)
+        assert 1024 - 30 <= symm.chi_full(p) <= 1024
+        assert all((q + tj - k) % 2 == 0 for q, tj in p)
+    chain = fi.chain_profiles(256, L=12)
+    assert chain[0] == {(0, 0): 1} and chain[12] == {(0, 0): 1}
+    tabs = fi.reachable_tables(12)
+    assert all(set(chain[k]) <= set(tabs[k]) for k in range(13))
