@@ -1,0 +1,174 @@
+/*
+ * fh_b200.h -- C ABI of the B200-native hot path of U(1)xSU(2)-symmetric two-site TDVP for
+ * the 1D Fermi-Hubbard chain (arxiv/paper_2606_04771; citations are PAPER.md:<line>).
+ *
+ * Every function returns int: 0 = FH_OK, negative = FH_E* code; fh_last_error(ctx) returns a
+ * NUL-terminated message owned by the library (valid until the next failing call on ctx).
+ * A context is not thread-safe.  All device work is enqueued on the cudaStream_t given at
+ * context creation; calls that return host data synchronise that stream before returning.
+ *
+ * Conventions (readings A-1, F-2, F-4):
+ *   sector label (q, tj): q = N_up - N_dn (integer), tj = 2*T (doubled pseudospin)  -- the
+ *     U(1)_spin x SU(2)_charge symmetry of PAPER.md:41, 208; bond spaces decompose as Eq. (7)
+ *     PAPER.md:210-214 with degeneracy d_{q,tj};
+ *   site multiplets s: 0 = (+1,0) |up>, 1 = (-1,0) |dn>, 2 = (0,1/2) {|0>, eps_i |updn>};
+ *   MPO bond multiplets w: 0 = S (0,0), 1 = P (+1,1/2), 2 = M (-1,1/2), 3 = F (0,0)  (W = 4,
+ *     PAPER.md:260);
+ *   a block is a dense row-major complex128 matrix (interleaved re,im; 16 B per element):
+ *     site tensor   A[a,s,c]            d_a  x d_c
+ *     two-site      theta[a,s1,c,s2,b]  d_a  x d_b   (c = intermediate coupling label)
+ *     environments  L[a',w,a]           d_a' x d_a ,  R[b',w,b]  d_b' x d_b
+ *   blocks of one tensor are stored contiguously in the canonical (lexicographic, sectors
+ *   ordered by (q, tj)) order of their label tuples; "planned block order" below means that.
+ *
+ * Pointer arguments are HOST pointers unless the name ends in _dev.
+ */
+#ifndef FH_B200_H
+#define FH_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FH_OK 0
+#define FH_EINVAL (-1)   /* bad argument (odd L, unknown label, size mismatch, ...) */
+#define FH_ENOMEM (-2)   /* arena exhausted */
+#define FH_ECUDA (-3)    /* CUDA / cuSOLVER runtime error */
+#define FH_ESTATE (-4)   /* call out of order (e.g. heff_apply without heff_plan) */
+
+typedef struct fh_ctx fh_ctx;
+typedef struct fh_mpo fh_mpo;
+typedef struct fh_mps fh_mps;
+
+/* ---- context ---------------------------------------------------------------------------
+ * cuda_stream: a cudaStream_t (NULL = legacy default stream).  arena_dev: device pointer to
+ * arena_bytes bytes owned by the caller (e.g. a torch tensor) that must outlive the context,
+ * or NULL, in which case the library cudaMalloc()s arena_bytes and frees them on destroy.
+ * All tensors (MPS, environments, Krylov vectors, scratch) live in this one HBM arena. */
+int fh_ctx_create(fh_ctx** out, void* cuda_stream, void* arena_dev, size_t arena_bytes);
+void fh_ctx_destroy(fh_ctx* ctx);
+const char* fh_last_error(const fh_ctx* ctx);
+/* bytes currently allocated / high-water mark in the arena */
+int fh_arena_stats(const fh_ctx* ctx, size_t* used_bytes, size_t* peak_bytes);
+
+/* ---- model: Eq. (1) PAPER.md:26-30 -----------------------------------------------------
+ * Builds the reduced MPO (bond multiplets S,P,M,F) of H_sym = hopping + (U/2) sum_i P_D,i,
+ * which equals Eq. (1) on the half-filled sector (reading A-2).  L even, 2 <= L <= 4096. */
+int fh_mpo_build(fh_ctx* ctx, int L, double t_h, double U, fh_mpo** out);
+void fh_mpo_destroy(fh_mpo* mpo);
+/* reduced MPO element table of one site: val[4][4][3][3] = W[w][w'][s'][s], rank2[4][4] = doubled
+ * operator rank of (w,w') or -1 when the pair is absent. */
+int fh_mpo_get_site(const fh_mpo* mpo, int site, double* val, int32_t* rank2);
+
+/* ---- state -----------------------------------------------------------------------------
+ * mps_init_neel: Eq. (2), |up,dn,up,dn,...>, one 1x1 block per site, every bond
+ * a single sector with d = 1; orthogonality centre at site 0; environments R_1..R_L built. */
+int mps_init_neel(fh_ctx* ctx, const fh_mpo* mpo, int L, fh_mps** out);
+/* empty MPS of L sites for synthetic workloads (BASELINE.json configs 2-5) */
+int mps_create(fh_ctx* ctx, int L, fh_mps** out);
+void mps_destroy(fh_ctx* ctx, fh_mps* mps);
+/* Sector table of bond k (k sites to its left), k = 0..L: n labels, sorted by (q,tj). */
+int mps_set_bond(fh_ctx* ctx, fh_mps* mps, int bond, int n, const int32_t* q, const int32_t* tj,
+                 const int32_t* d);
+int mps_get_bond(const fh_mps* mps, int bond, int* n, int32_t* q, int32_t* tj, int32_t* d);
+/* Number of blocks / total complex elements of site tensor `site` given its two bond tables
+ * (all fusion-allowed (a,s,c)), and the labels[nblk][5] = (qa,tja,s,qc,tjc), dims[nblk][2]. */
+int mps_site_layout(const fh_mps* mps, int site, int* nblk, int64_t* nelem, int32_t* labels,
+                    int32_t* dims);
+/* Upload / download a whole site tensor: `data` holds the blocks back to back in planned block
+ * order.  data_is_device != 0: device pointer (copied D2D on the context stream). */
+int mps_set_site(fh_ctx* ctx, fh_mps* mps, int site, const void* data, int data_is_device);
+int mps_get_site(fh_ctx* ctx, const fh_mps* mps, int site, void* data, int data_is_device);
+
+/* ---- environments (H4, H5) ---------------------------------------------
+ * env_update_left : L_{site+1}[c',w',c] = sum alpha A[a',s',c']^H (L_site[a',w,a] A[a,s,c])
+ * env_update_right: R_{site}[c',w,c]    = sum alpha_R conj(A[c',s',b']) R_{site+1}[b',w',b] A[c,s,b]^T
+ * with alpha = recoupling coefficient (F-5) x reduced MPO element.  L_0 and R_L are the
+ * boundary 1x1 blocks.  The result is stored inside the MPS object. */
+int env_update_left(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int site);
+int env_update_right(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int site);
+/* which = 0: L_k, 1: R_k (k = bond index).  Layout query and download as for sites:
+ * labels[nblk][5] = (qx',tjx',w,qx,tjx), dims[nblk][2]. */
+int env_layout(const fh_mps* mps, int which, int bond, int* nblk, int64_t* nelem, int32_t* labels,
+               int32_t* dims);
+int env_get(fh_ctx* ctx, const fh_mps* mps, int which, int bond, void* data, int data_is_device);
+int env_set(fh_ctx* ctx, fh_mps* mps, int which, int bond, int nblk, const int32_t* labels,
+            const void* data, int data_is_device);
+
+/* ---- hot path: H_eff theta = L . W_i . W_{i+1} . theta . R  (H0-H3) --
+ * heff_plan emits the two task lists of the apply on bond (site, site+1) [nsite = 2] or on
+ * site `site` [nsite = 1] from the sector tables, MPO sparsity and recoupling coefficients,
+ * sorts them canonically, builds the tile queue and uploads everything.  It uses L_site and
+ * R_{site+nsite} stored in the MPS. */
+int heff_plan(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, int nsite);
+/* block layout of the planned vector: nsite=2: labels[nblk][8] = (qa,tja,s1,qc,tjc,s2,qb,tjb);
+ * nsite=1: labels[nblk][5].  dims[nblk][2]. */
+int heff_layout(const fh_ctx* ctx, int* nblk, int64_t* nelem, int32_t* labels, int32_t* dims);
+/* host copy of a task list, stage = 1 or 2: tuples[ntask][3] = (out_id, lhs_id, rhs_id), ids =
+ * positions in canonical block order (stage 1: Z, L, theta; stage 2: out, Z, R); alpha[ntask].
+ * Pass tuples = alpha = NULL to query ntask (and nout = number of output blocks). */
+int heff_get_tasks(const fh_ctx* ctx, int stage, int* ntask, int* nout, int32_t* tuples, double* alpha);
+/* out_dev = H_eff * theta_dev; both device vectors of heff_layout's nelem complex128. */
+int heff_apply(fh_ctx* ctx, const void* theta_dev, void* out_dev);
+/* sum over both task lists of 8*m*n*k */
+int64_t heff_flops(const fh_ctx* ctx);
+/* <x,y> = sum_blocks (2 j_b + 1) sum conj(x) y  (F-6) over the planned layout; result[2] = re,im */
+int heff_inner(fh_ctx* ctx, const void* x_dev, const void* y_dev, double* result);
+/* out_dev = exp(-i tau H_eff) theta_dev by an m-vector Lanczos process (H6, H7) */
+int heff_expm(fh_ctx* ctx, const void* theta_dev, void* out_dev, double tau, int krylov_dim);
+
+/* ---- time evolution ---------------------------------------------------
+ * One full step dt = left->right half-sweep with tau = dt/2 followed by right->left with
+ * tau = dt/2 (reading A-4); at every bond: merge, Lanczos exponential, block-wise SVD with the
+ * truncation rule A-6, environment update, one-site backward step. */
+typedef struct {
+  int krylov_dim;      /* Lanczos vectors m (>= 2) */
+  double krylov_tol;   /* happy-breakdown threshold on beta_j (relative to 1), e.g. 1e-12 */
+  int chi_max_full;    /* cap on sum d (2j+1) of the new bond */
+  double eps_trunc;    /* discarded relative weight; < 0 disables */
+} fh_params;
+int tdvp2_sweep(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh_params* params);
+/* statistics of the last sweep: max discarded weight, max chi_full, max chi_su2, max d */
+int tdvp2_last_stats(const fh_ctx* ctx, double* max_discarded, int* chi_full, int* chi_su2, int* dmax);
+
+/* ---- observables (H10; reading A-12) -----------------------------------
+ * n_i = <1> ratio (== 1 in a T_tot = 0 state), sz_i = <S^z_i>, docc_i = <n_up n_dn>_i = <P_D>/2;
+ * host arrays of length L.  Requires all sites right of the centre right-canonical (true
+ * after mps_init_neel / tdvp2_sweep). */
+int measure_local(fh_ctx* ctx, const fh_mps* mps, double* n_i, double* sz_i, double* docc_i);
+/* <psi|psi> and <psi|H|psi>/<psi|psi> by a full left contraction */
+int measure_global(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, double* norm2, double* energy);
+
+/* seconds spent (CUDA events on the context stream) since the last fh_reset_timers, by phase */
+int fh_get_timers(const fh_ctx* ctx, double* sec_heff, double* sec_env, double* sec_svd,
+                  double* sec_vec, double* sec_pack);
+int fh_reset_timers(fh_ctx* ctx);
+/* number of kernels the library launched since context creation */
+int64_t fh_launch_count(const fh_ctx* ctx);
+
+/* ---- calibration helper for the roofline denominator ------------------------
+ * Runs cublasZgemm (is_complex=1) or cublasDgemm n x n x n `reps` times on the context stream
+ * and returns the average seconds per call.  Library GEMM, not part of the hot path. */
+int fh_cublas_gemm_seconds(fh_ctx* ctx, int n, int is_complex, int reps, double* seconds);
+
+/* ---- host-only entry points (no CUDA call inside): the symmetry layer on its own -----------
+ * Closed-form recoupling coefficients of reading F-5 (all arguments doubled spins):
+ *   coefL(a,s,c; k,r,k'; a',s',c') = sqrt((2c+1)(2k'+1)(2a'+1)(2s'+1)) {a s c; k r k'; a' s' c'}
+ *   coefR(c,s,b; k,r,k'; c',s',b') = (2b'+1)/(2c'+1) sqrt((2b+1)(2k'+1)(2c'+1)(2s'+1)) {c s b; k r k'; c' s' b'} */
+double fh_coef_left(int ta, int ts, int tc, int tk, int tr, int tkp, int tap, int tsp, int tcp);
+double fh_coef_right(int tc, int ts, int tb, int tk, int tr, int tkp, int tcp, int tsp, int tbp);
+/* Emit the task lists of an apply on `site` (nsite = 1 | 2) from explicit tables: bl/br =
+ * [n][3] (q,tj,d) of the left and right bond, Llab/Rlab = [nblk][5] canonical-order labels of the
+ * environment blocks.  Results are kept in a process-global scratch (not thread-safe) and read
+ * with fh_host_get_tasks (same format as heff_get_tasks; flops = sum 8mnk of that stage). */
+int fh_host_plan(int site, int nsite, double t_h, double U, int nl, const int32_t* bl, int nr, const int32_t* br,
+                 int nLblk, const int32_t* Llab, int nRblk, const int32_t* Rlab);
+int fh_host_get_tasks(int stage, int* ntask, int* nout, int32_t* tuples, double* alpha, int64_t* flops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FH_B200_H */

@@ -1,0 +1,311 @@
+"""Thin ctypes binding of libfh_b200.so (include/fh_b200.h): argument marshalling only.
+
+Every step of the hot path runs inside the library's CUDA kernels; PyTorch is used here for
+device memory (the HBM arena, vectors) and streams, nothing else.  There is no CPU fallback:
+importing this module fails if the shared library is missing, and every call raises FhError on
+a non-zero return code.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfh_b200.so")
+if not os.path.exists(LIB_PATH):
+    raise ImportError("libfh_b200.so is not built: run `python -m paper_2606_04771_b200.build` "
+                      "(or __graft_entry__.build()); there is no CPU fallback")
+lib = C.CDLL(LIB_PATH)
+
+c_int, c_i64, c_dbl, c_void_p, c_size_t = C.c_int, C.c_int64, C.c_double, C.c_void_p, C.c_size_t
+P = C.POINTER
+
+
+class fh_params(C.Structure):
+    _fields_ = [("krylov_dim", c_int), ("krylov_tol", c_dbl), ("chi_max_full", c_int), ("eps_trunc", c_dbl)]
+
+
+_SIGS = {
+    "fh_ctx_create": (c_int, [P(c_void_p), c_void_p, c_void_p, c_size_t]),
+    "fh_ctx_destroy": (None, [c_void_p]),
+    "fh_last_error": (C.c_char_p, [c_void_p]),
+    "fh_arena_stats": (c_int, [c_void_p, P(c_size_t), P(c_size_t)]),
+    "fh_mpo_build": (c_int, [c_void_p, c_int, c_dbl, c_dbl, P(c_void_p)]),
+    "fh_mpo_destroy": (None, [c_void_p]),
+    "fh_mpo_get_site": (c_int, [c_void_p, c_int, c_void_p, c_void_p]),
+    "mps_init_neel": (c_int, [c_void_p, c_void_p, c_int, P(c_void_p)]),
+    "mps_create": (c_int, [c_void_p, c_int, P(c_void_p)]),
+    "mps_destroy": (None, [c_void_p, c_void_p]),
+    "mps_set_bond": (c_int, [c_void_p, c_void_p, c_int, c_int, c_void_p, c_void_p, c_void_p]),
+    "mps_get_bond": (c_int, [c_void_p, c_int, P(c_int), c_void_p, c_void_p, c_void_p]),
+    "mps_site_layout": (c_int, [c_void_p, c_int, P(c_int), P(c_i64), c_void_p, c_void_p]),
+    "mps_set_site": (c_int, [c_void_p, c_void_p, c_int, c_void_p, c_int]),
+    "mps_get_site": (c_int, [c_void_p, c_void_p, c_int, c_void_p, c_int]),
+    "env_update_left": (c_int, [c_void_p, c_void_p, c_void_p, c_int]),
+    "env_update_right": (c_int, [c_void_p, c_void_p, c_void_p, c_int]),
+    "env_layout": (c_int, [c_void_p, c_int, c_int, P(c_int), P(c_i64), c_void_p, c_void_p]),
+    "env_get": (c_int, [c_void_p, c_void_p, c_int, c_int, c_void_p, c_int]),
+    "env_set": (c_int, [c_void_p, c_void_p, c_int, c_int, c_int, c_void_p, c_void_p, c_int]),
+    "heff_plan": (c_int, [c_void_p, c_void_p, c_void_p, c_int, c_int]),
+    "heff_layout": (c_int, [c_void_p, P(c_int), P(c_i64), c_void_p, c_void_p]),
+    "heff_get_tasks": (c_int, [c_void_p, c_int, P(c_int), P(c_int), c_void_p, c_void_p]),
+    "heff_apply": (c_int, [c_void_p, c_void_p, c_void_p]),
+    "heff_flops": (c_i64, [c_void_p]),
+    "heff_inner": (c_int, [c_void_p, c_void_p, c_void_p, P(c_dbl)]),
+    "heff_expm": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, c_int]),
+    "tdvp2_sweep": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, P(fh_params)]),
+    "tdvp2_last_stats": (c_int, [c_void_p, P(c_dbl), P(c_int), P(c_int), P(c_int)]),
+    "measure_local": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
+    "measure_global": (c_int, [c_void_p, c_void_p, c_void_p, P(c_dbl), P(c_dbl)]),
+    "fh_get_timers": (c_int, [c_void_p, P(c_dbl), P(c_dbl), P(c_dbl), P(c_dbl), P(c_dbl)]),
+    "fh_reset_timers": (c_int, [c_void_p]),
+    "fh_launch_count": (c_i64, [c_void_p]),
+    "fh_cublas_gemm_seconds": (c_int, [c_void_p, c_int, c_int, c_int, P(c_dbl)]),
+    "fh_coef_left": (c_dbl, [c_int] * 9),
+    "fh_coef_right": (c_dbl, [c_int] * 9),
+    "fh_host_plan": (c_int, [c_int, c_int, c_dbl, c_dbl, c_int, c_void_p, c_int, c_void_p, c_int, c_void_p,
+                             c_int, c_void_p]),
+    "fh_host_get_tasks": (c_int, [c_int, P(c_int), P(c_int), c_void_p, c_void_p, P(c_i64)]),
+}
+EXPORTS = sorted(_SIGS)
+for _name, (_res, _args) in _SIGS.items():
+    _f = getattr(lib, _name)
+    _f.restype = _res
+    _f.argtypes = _args
+
+
+class FhError(RuntimeError):
+    pass
+
+
+def _np_ptr(a):
+    return a.ctypes.data_as(c_void_p)
+
+
+def _i32(x):
+    return np.ascontiguousarray(np.asarray(x, dtype=np.int32))
+
+
+# ------------------------------------------------------------------ host-only entry points
+def fh_coef_left(*t):
+    return lib.fh_coef_left(*[int(x) for x in t])
+
+
+def fh_coef_right(*t):
+    return lib.fh_coef_right(*[int(x) for x in t])
+
+
+def fh_host_plan(site, nsite, t_h, U, dims_l, dims_r, L_keys, R_keys):
+    """dims_*: {(q,tj): d}; *_keys: canonical-order env keys ((q',tj'), w, (q,tj)).  Returns
+    [(tuples int32[n,3], alpha f64[n], nout, flops)] for stage 1 and 2."""
+    bl = _i32([[q, tj, d] for (q, tj), d in sorted(dims_l.items())])
+    br = _i32([[q, tj, d] for (q, tj), d in sorted(dims_r.items())])
+    Ll = _i32([[xp[0], xp[1], w, x[0], x[1]] for xp, w, x in L_keys])
+    Rl = _i32([[xp[0], xp[1], w, x[0], x[1]] for xp, w, x in R_keys])
+    rc = lib.fh_host_plan(site, nsite, t_h, U, len(bl), _np_ptr(bl), len(br), _np_ptr(br),
+                          len(Ll), _np_ptr(Ll), len(Rl), _np_ptr(Rl))
+    if rc != 0:
+        raise FhError("fh_host_plan failed: %d" % rc)
+    out = []
+    for stage in (1, 2):
+        nt, no, fl = c_int(), c_int(), c_i64()
+        lib.fh_host_get_tasks(stage, C.byref(nt), C.byref(no), None, None, C.byref(fl))
+        tup = np.zeros((nt.value, 3), dtype=np.int32)
+        al = np.zeros(nt.value, dtype=np.float64)
+        lib.fh_host_get_tasks(stage, C.byref(nt), C.byref(no), _np_ptr(tup), _np_ptr(al), C.byref(fl))
+        out.append((tup, al, no.value, fl.value))
+    return out
+
+
+# ------------------------------------------------------------------ device objects
+class Context:
+    """fh_ctx: owns the HBM arena (a torch uint8 tensor) and the stream."""
+
+    def __init__(self, arena_bytes, stream=None, device="cuda:0"):
+        import torch
+        if not torch.cuda.is_available():
+            raise FhError("no CUDA device: the library has no CPU path")
+        self.torch = torch
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self.arena = torch.empty(int(arena_bytes), dtype=torch.uint8, device=self.device)
+        h = c_void_p()
+        rc = lib.fh_ctx_create(C.byref(h), c_void_p(self.stream.cuda_stream), c_void_p(self.arena.data_ptr()),
+                               c_size_t(int(arena_bytes)))
+        if rc != 0:
+            raise FhError("fh_ctx_create failed: %d" % rc)
+        self.h = h
+
+    def check(self, rc, what=""):
+        if rc != 0:
+            msg = lib.fh_last_error(self.h)
+            raise FhError("%s failed (%d): %s" % (what, rc, msg.decode() if msg else ""))
+
+    def close(self):
+        if self.h:
+            lib.fh_ctx_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # --- model / state
+    def fh_mpo_build(self, L, t_h, U):
+        h = c_void_p()
+        self.check(lib.fh_mpo_build(self.h, L, t_h, U, C.byref(h)), "fh_mpo_build")
+        return h
+
+    def fh_mpo_get_site(self, mpo, site):
+        val = np.zeros((4, 4, 3, 3))
+        rank2 = np.zeros((4, 4), dtype=np.int32)
+        self.check(lib.fh_mpo_get_site(mpo, site, _np_ptr(val), _np_ptr(rank2)), "fh_mpo_get_site")
+        return val, rank2
+
+    def mps_init_neel(self, mpo, L):
+        h = c_void_p()
+        self.check(lib.mps_init_neel(self.h, mpo, L, C.byref(h)), "mps_init_neel")
+        return h
+
+    def mps_create(self, L):
+        h = c_void_p()
+        self.check(lib.mps_create(self.h, L, C.byref(h)), "mps_create")
+        return h
+
+    def mps_destroy(self, mps):
+        lib.mps_destroy(self.h, mps)
+
+    def mps_set_bond(self, mps, bond, dims):
+        items = sorted(dims.items())
+        q, tj, d = _i32([k[0] for k, _ in items]), _i32([k[1] for k, _ in items]), _i32([v for _, v in items])
+        self.check(lib.mps_set_bond(self.h, mps, bond, len(items), _np_ptr(q), _np_ptr(tj), _np_ptr(d)), "mps_set_bond")
+
+    def mps_get_bond(self, mps, bond):
+        n = c_int()
+        self.check(lib.mps_get_bond(mps, bond, C.byref(n), None, None, None), "mps_get_bond")
+        q, tj, d = (np.zeros(n.value, dtype=np.int32) for _ in range(3))
+        self.check(lib.mps_get_bond(mps, bond, C.byref(n), _np_ptr(q), _np_ptr(tj), _np_ptr(d)), "mps_get_bond")
+        return {(int(a), int(b)): int(c) for a, b, c in zip(q, tj, d)}
+
+    def _layout(self, fn, nlab, *args):
+        nb, ne = c_int(), c_i64()
+        rc = fn(*args, C.byref(nb), C.byref(ne), None, None)
+        self.check(rc, fn.__name__)
+        lab = np.zeros((nb.value, nlab), dtype=np.int32)
+        dims = np.zeros((nb.value, 2), dtype=np.int32)
+        self.check(fn(*args, C.byref(nb), C.byref(ne), _np_ptr(lab), _np_ptr(dims)), fn.__name__)
+        return lab, dims, ne.value
+
+    def mps_site_layout(self, mps, site):
+        return self._layout(lib.mps_site_layout, 5, mps, site)
+
+    def env_layout(self, mps, which, bond):
+        return self._layout(lib.env_layout, 5, mps, which, bond)
+
+    def heff_layout(self, nsite):
+        return self._layout(lib.heff_layout, 8 if nsite == 2 else 5, self.h)
+
+    def mps_set_site(self, mps, site, data):
+        """data: numpy complex128 1-D (host) or torch complex128 CUDA tensor, blocks back to back."""
+        if isinstance(data, np.ndarray):
+            data = np.ascontiguousarray(data, dtype=np.complex128)
+            self.check(lib.mps_set_site(self.h, mps, site, _np_ptr(data), 0), "mps_set_site")
+        else:
+            self.check(lib.mps_set_site(self.h, mps, site, c_void_p(data.data_ptr()), 1), "mps_set_site")
+
+    def mps_get_site(self, mps, site):
+        _, _, ne = self.mps_site_layout(mps, site)
+        out = np.zeros(ne, dtype=np.complex128)
+        self.check(lib.mps_get_site(self.h, mps, site, _np_ptr(out), 0), "mps_get_site")
+        return out
+
+    def env_update_left(self, mpo, mps, site):
+        self.check(lib.env_update_left(self.h, mpo, mps, site), "env_update_left")
+
+    def env_update_right(self, mpo, mps, site):
+        self.check(lib.env_update_right(self.h, mpo, mps, site), "env_update_right")
+
+    def env_get(self, mps, which, bond):
+        lab, dims, ne = self.env_layout(mps, which, bond)
+        out = np.zeros(ne, dtype=np.complex128)
+        self.check(lib.env_get(self.h, mps, which, bond, _np_ptr(out), 0), "env_get")
+        return lab, dims, out
+
+    def env_set(self, mps, which, bond, labels, data):
+        labels = _i32(labels)
+        if isinstance(data, np.ndarray):
+            data = np.ascontiguousarray(data, dtype=np.complex128)
+            self.check(lib.env_set(self.h, mps, which, bond, len(labels), _np_ptr(labels), _np_ptr(data), 0), "env_set")
+        else:
+            self.check(lib.env_set(self.h, mps, which, bond, len(labels), _np_ptr(labels),
+                                   c_void_p(data.data_ptr()), 1), "env_set")
+
+    # --- hot path
+    def heff_plan(self, mpo, mps, site, nsite):
+        self.check(lib.heff_plan(self.h, mpo, mps, site, nsite), "heff_plan")
+
+    def heff_get_tasks(self, stage):
+        nt, no = c_int(), c_int()
+        self.check(lib.heff_get_tasks(self.h, stage, C.byref(nt), C.byref(no), None, None), "heff_get_tasks")
+        tup = np.zeros((nt.value, 3), dtype=np.int32)
+        al = np.zeros(nt.value, dtype=np.float64)
+        self.check(lib.heff_get_tasks(self.h, stage, C.byref(nt), C.byref(no), _np_ptr(tup), _np_ptr(al)), "heff_get_tasks")
+        return tup, al, no.value
+
+    def heff_apply(self, theta, out):
+        """theta, out: torch complex128 CUDA tensors (device pointers are passed through)."""
+        self.check(lib.heff_apply(self.h, c_void_p(theta.data_ptr()), c_void_p(out.data_ptr())), "heff_apply")
+
+    def heff_flops(self):
+        return int(lib.heff_flops(self.h))
+
+    def heff_inner(self, x, y):
+        r = (c_dbl * 2)()
+        self.check(lib.heff_inner(self.h, c_void_p(x.data_ptr()), c_void_p(y.data_ptr()), r), "heff_inner")
+        return complex(r[0], r[1])
+
+    def heff_expm(self, theta, out, tau, krylov_dim):
+        self.check(lib.heff_expm(self.h, c_void_p(theta.data_ptr()), c_void_p(out.data_ptr()), tau, krylov_dim), "heff_expm")
+
+    def tdvp2_sweep(self, mpo, mps, dt, krylov_dim=10, krylov_tol=1e-12, chi_max_full=1 << 30, eps_trunc=-1.0):
+        p = fh_params(krylov_dim, krylov_tol, chi_max_full, eps_trunc)
+        self.check(lib.tdvp2_sweep(self.h, mpo, mps, dt, C.byref(p)), "tdvp2_sweep")
+
+    def tdvp2_last_stats(self):
+        d, a, b, c = c_dbl(), c_int(), c_int(), c_int()
+        self.check(lib.tdvp2_last_stats(self.h, C.byref(d), C.byref(a), C.byref(b), C.byref(c)), "tdvp2_last_stats")
+        return dict(max_discarded=d.value, chi_full=a.value, chi_su2=b.value, dmax=c.value)
+
+    def measure_local(self, mps, L):
+        n, sz, dc = np.zeros(L), np.zeros(L), np.zeros(L)
+        self.check(lib.measure_local(self.h, mps, _np_ptr(n), _np_ptr(sz), _np_ptr(dc)), "measure_local")
+        return dict(n=n, sz=sz, docc=dc)
+
+    def measure_global(self, mpo, mps):
+        a, b = c_dbl(), c_dbl()
+        self.check(lib.measure_global(self.h, mpo, mps, C.byref(a), C.byref(b)), "measure_global")
+        return dict(norm2=a.value, energy=b.value)
+
+    def fh_get_timers(self):
+        v = [c_dbl() for _ in range(5)]
+        self.check(lib.fh_get_timers(self.h, *[C.byref(x) for x in v]), "fh_get_timers")
+        return dict(zip(("heff", "env", "svd", "vec", "pack"), [x.value for x in v]))
+
+    def fh_reset_timers(self):
+        self.check(lib.fh_reset_timers(self.h), "fh_reset_timers")
+
+    def fh_launch_count(self):
+        return int(lib.fh_launch_count(self.h))
+
+    def fh_arena_stats(self):
+        a, b = c_size_t(), c_size_t()
+        self.check(lib.fh_arena_stats(self.h, C.byref(a), C.byref(b)), "fh_arena_stats")
+        return a.value, b.value
+
+    def fh_cublas_gemm_seconds(self, n, is_complex, reps):
+        s = c_dbl()
+        self.check(lib.fh_cublas_gemm_seconds(self.h, n, int(is_complex), reps, C.byref(s)), "fh_cublas_gemm_seconds")
+        return s.value

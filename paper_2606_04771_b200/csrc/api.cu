@@ -1,0 +1,874 @@
+// C ABI entry points (include/fh_b200.h) and the engine pieces they share: arena, plans,
+// H_eff apply, weighted inner product, Lanczos exponential, environment updates.
+#include <cublas_v2.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+
+#include "context.hpp"
+
+using namespace fh;
+
+// ============================================================================ arena / pools
+int64_t Arena::alloc(int64_t n) {
+  n = round_up(n < 1 ? 1 : n);
+  for (auto it = free_.begin(); it != free_.end(); ++it) {
+    if (it->second >= n) {
+      const int64_t off = it->first, len = it->second;
+      free_.erase(it);
+      if (len > n) free_[off + n] = len - n;
+      used += n;
+      peak = std::max(peak, used);
+      return off;
+    }
+  }
+  throw FhError(FH_ENOMEM, "arena exhausted: need " + std::to_string(n * 16) + " bytes, used " +
+                               std::to_string(used * 16) + " of " + std::to_string(cap * 16));
+}
+void Arena::release(int64_t off, int64_t n) {
+  n = round_up(n < 1 ? 1 : n);
+  used -= n;
+  auto it = free_.emplace(off, n).first;
+  auto nx = std::next(it);
+  if (nx != free_.end() && it->first + it->second == nx->first) {
+    it->second += nx->second;
+    free_.erase(nx);
+  }
+  if (it != free_.begin()) {
+    auto pv = std::prev(it);
+    if (pv->first + pv->second == it->first) {
+      pv->second += it->second;
+      free_.erase(it);
+    }
+  }
+}
+
+void DevPool::reserve(size_t bytes, cudaStream_t s) {
+  top = 0;
+  if (bytes <= cap) return;
+  if (ptr) {
+    FH_CUDA(cudaStreamSynchronize(s));
+    FH_CUDA(cudaFree(ptr));
+  }
+  cap = bytes + bytes / 2 + 4096;
+  FH_CUDA(cudaMalloc((void**)&ptr, cap));
+}
+void* DevPool::take(size_t bytes) {
+  const size_t b = (bytes + 255) / 256 * 256;
+  if (top + b > cap) throw FhError(FH_ENOMEM, "device pool overflow");
+  void* p = ptr + top;
+  top += b;
+  return p;
+}
+void DevPool::destroy() {
+  if (ptr) cudaFree(ptr);
+  ptr = nullptr;
+  cap = top = 0;
+}
+
+size_t fh::stage_bytes(const Stage& st) {
+  return st.outs.size() * sizeof(GemmOut) + st.segs.size() * sizeof(GemmSeg) +
+         (st.tiles64.size() + st.tiles32.size()) * sizeof(GemmTile) + 4 * 256;
+}
+void fh::upload_stage(DevPool& pool, Stage& st, cudaStream_t s) {
+  st.d_outs = upload(pool, st.outs, s);
+  st.d_segs = upload(pool, st.segs, s);
+  st.d_tiles64 = upload(pool, st.tiles64, s);
+  st.d_tiles32 = upload(pool, st.tiles32, s);
+}
+
+void fh_ctx::alloc_tensor(BlockTensor& t) { t.base = alloc.alloc(t.nelem); }
+void fh_ctx::free_tensor(BlockTensor& t) {
+  if (t.base >= 0) alloc.release(t.base, t.nelem);
+  t.base = -1;
+}
+void fh_ctx::ensure_pinned(size_t n) {
+  if (n <= h_pinned_n) return;
+  if (h_pinned) {
+    FH_CUDA(cudaStreamSynchronize(stream));
+    FH_CUDA(cudaFreeHost(h_pinned));
+  }
+  h_pinned_n = n * 2 + 1024;
+  FH_CUDA(cudaMallocHost((void**)&h_pinned, h_pinned_n * sizeof(double)));
+}
+void fh_ctx::timer_begin(int cat) {
+  if (spans.size() > 8192) timers_resolve();
+  Span sp;
+  for (cudaEvent_t* e : {&sp.a, &sp.b}) {
+    if (!ev_free.empty()) {
+      *e = ev_free.back();
+      ev_free.pop_back();
+    } else {
+      FH_CUDA(cudaEventCreate(e));
+    }
+  }
+  sp.cat = cat;
+  FH_CUDA(cudaEventRecord(sp.a, stream));
+  spans.push_back(sp);
+}
+void fh_ctx::timer_end() { FH_CUDA(cudaEventRecord(spans.back().b, stream)); }
+void fh_ctx::timers_resolve() {
+  if (spans.empty()) return;
+  FH_CUDA(cudaStreamSynchronize(stream));
+  for (Span& sp : spans) {
+    float ms = 0.f;
+    FH_CUDA(cudaEventElapsedTime(&ms, sp.a, sp.b));
+    sec[sp.cat] += ms * 1e-3;
+    ev_free.push_back(sp.a);
+    ev_free.push_back(sp.b);
+  }
+  spans.clear();
+}
+
+// ============================================================================ plan + apply
+static int last_tj_pos(int nsite) { return nsite == 2 ? 7 : 4; }
+
+void fh::plan_heff(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, int nsite) {
+  FH_REQUIRE(nsite == 1 || nsite == 2, FH_EINVAL, "heff_plan: nsite must be 1 or 2");
+  FH_REQUIRE(site >= 0 && site + nsite <= mps->L, FH_EINVAL, "heff_plan: site out of range");
+  const BlockTensor& Le = mps->Lenv[site];
+  const BlockTensor& Re = mps->Renv[site + nsite];
+  FH_REQUIRE(Le.base >= 0 && Re.base >= 0, FH_ESTATE, "heff_plan: environments of this bond are not built");
+  Plan& P = ctx->plan;
+  ctx->free_tensor(P.Z);
+  P.valid = false;
+  P.nsite = nsite;
+  P.site = site;
+  if (nsite == 2) {
+    layout_theta(mps->bond[site], mps->bond[site + 2], P.vec);
+    emit_heff2(Le, Re, P.vec, mpo->site[site & 1], mpo->site[(site + 1) & 1], P.Z, P.st1, P.st2);
+  } else {
+    layout_site(mps->bond[site], mps->bond[site + 1], P.vec);
+    emit_heff1(Le, Re, P.vec, mpo->site[site & 1], P.Z, P.st1, P.st2);
+  }
+  ctx->alloc_tensor(P.Z);
+  P.Lptr = ctx->ptr(Le.base);
+  P.Rptr = ctx->ptr(Re.base);
+  // weighted inner-product chunks (F-6)
+  P.chunks.clear();
+  const int tpos = last_tj_pos(nsite);
+  for (size_t i = 0; i < P.vec.keys.size(); ++i) {
+    const int64_t n = (int64_t)P.vec.rows[i] * P.vec.cols[i];
+    for (int64_t s = 0; s < n; s += 8192)
+      P.chunks.push_back(VecChunk{P.vec.off[i] + s, (int)std::min<int64_t>(8192, n - s), (float)(P.vec.keys[i][tpos] + 1)});
+  }
+  const size_t need = stage_bytes(P.st1) + stage_bytes(P.st2) + P.chunks.size() * (sizeof(VecChunk) + 16) + 4096;
+  P.pool.reserve(need, ctx->stream);
+  upload_stage(P.pool, P.st1, ctx->stream);
+  upload_stage(P.pool, P.st2, ctx->stream);
+  P.d_chunks = upload(P.pool, P.chunks, ctx->stream);
+  P.d_partial = (double*)P.pool.take(std::max<size_t>(1, P.chunks.size()) * 2 * sizeof(double));
+  P.d_result = (double*)P.pool.take(2 * sizeof(double));
+  P.valid = true;
+}
+
+void fh::apply_heff(fh_ctx* ctx, const cplx* theta, cplx* out) {
+  Plan& P = ctx->plan;
+  FH_REQUIRE(P.valid, FH_ESTATE, "heff_apply: no plan (call heff_plan first)");
+  cplx* Z = ctx->ptr(P.Z.base);
+  launch_grouped_gemm(P.st1, P.Lptr, theta, Z, ctx->stream, &ctx->launches);
+  launch_grouped_gemm(P.st2, Z, P.Rptr, out, ctx->stream, &ctx->launches);
+  FH_CUDA(cudaGetLastError());
+}
+
+double2 fh::inner(fh_ctx* ctx, const cplx* x, const cplx* y) {
+  Plan& P = ctx->plan;
+  FH_REQUIRE(P.valid, FH_ESTATE, "inner: no plan");
+  ctx->ensure_pinned(2);
+  if (P.chunks.empty()) return make_double2(0, 0);
+  launch_wdot(P.d_chunks, (int)P.chunks.size(), x, y, P.d_partial, P.d_result, ctx->stream, &ctx->launches);
+  FH_CUDA(cudaMemcpyAsync(ctx->h_pinned, P.d_result, 2 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+  FH_CUDA(cudaStreamSynchronize(ctx->stream));
+  return make_double2(ctx->h_pinned[0], ctx->h_pinned[1]);
+}
+
+// symmetric tridiagonal eigen-decomposition by cyclic Jacobi (m <= 32): T = Q diag(lam) Q^T
+static void jacobi_eig(int n, std::vector<double>& Amat, std::vector<double>& Q) {
+  Q.assign(n * n, 0.0);
+  for (int i = 0; i < n; ++i) Q[i * n + i] = 1.0;
+  for (int sweep = 0; sweep < 100; ++sweep) {
+    double offd = 0.0;
+    for (int i = 0; i < n; ++i)
+      for (int j = i + 1; j < n; ++j) offd += Amat[i * n + j] * Amat[i * n + j];
+    if (offd < 1e-300) break;
+    for (int p = 0; p < n; ++p)
+      for (int q = p + 1; q < n; ++q) {
+        const double apq = Amat[p * n + q];
+        if (std::fabs(apq) < 1e-300) continue;
+        const double app = Amat[p * n + p], aqq = Amat[q * n + q];
+        const double theta = (aqq - app) / (2.0 * apq);
+        const double t = (theta >= 0 ? 1.0 : -1.0) / (std::fabs(theta) + std::sqrt(theta * theta + 1.0));
+        const double c = 1.0 / std::sqrt(t * t + 1.0), s = t * c;
+        for (int k = 0; k < n; ++k) {
+          const double akp = Amat[k * n + p], akq = Amat[k * n + q];
+          Amat[k * n + p] = c * akp - s * akq;
+          Amat[k * n + q] = s * akp + c * akq;
+        }
+        for (int k = 0; k < n; ++k) {
+          const double apk = Amat[p * n + k], aqk = Amat[q * n + k];
+          Amat[p * n + k] = c * apk - s * aqk;
+          Amat[q * n + k] = s * apk + c * aqk;
+        }
+        for (int k = 0; k < n; ++k) {
+          const double qkp = Q[k * n + p], qkq = Q[k * n + q];
+          Q[k * n + p] = c * qkp - s * qkq;
+          Q[k * n + q] = s * qkp + c * qkq;
+        }
+      }
+  }
+}
+
+// theta <- exp(-i tau H_eff) theta (H6 + H7).  work holds (m+1) vectors of n elements.
+void fh::expm_lanczos(fh_ctx* ctx, cplx* theta, double tau, int m, double tol, cplx* V) {
+  Plan& P = ctx->plan;
+  const int64_t n = P.vec.nelem;
+  FH_REQUIRE(m >= 1 && m <= 32, FH_EINVAL, "krylov_dim must be in [1, 32]");
+  if (n == 0) return;
+  cudaStream_t s = ctx->stream;
+  ctx->timer_begin(T_VEC);
+  const double nrm2 = inner(ctx, theta, theta).x;
+  ctx->timer_end();
+  if (!(nrm2 > 0.0)) return;
+  const double nrm = std::sqrt(nrm2);
+  ctx->timer_begin(T_VEC);
+  launch_scale(n, make_double2(1.0 / nrm, 0.0), theta, V, s, &ctx->launches);
+  ctx->timer_end();
+  std::vector<double> alpha, beta;
+  int k = 0;
+  for (int j = 0; j < m; ++j) {
+    cplx* vj = V + (int64_t)j * n;
+    cplx* w = V + (int64_t)(j + 1) * n;
+    ctx->timer_begin(T_HEFF);
+    apply_heff(ctx, vj, w);
+    ctx->timer_end();
+    ctx->timer_begin(T_VEC);
+    const double a = inner(ctx, vj, w).x;
+    alpha.push_back(a);
+    k = j + 1;
+    launch_axpy(n, make_double2(-a, 0.0), vj, w, s, &ctx->launches);
+    if (j > 0) launch_axpy(n, make_double2(-beta[j - 1], 0.0), V + (int64_t)(j - 1) * n, w, s, &ctx->launches);
+    if (j == m - 1) {
+      ctx->timer_end();
+      break;
+    }
+    const double b = std::sqrt(std::max(0.0, inner(ctx, w, w).x));
+    if (b < tol) {
+      ctx->timer_end();
+      break;
+    }
+    beta.push_back(b);
+    launch_scale(n, make_double2(1.0 / b, 0.0), w, w, s, &ctx->launches);
+    ctx->timer_end();
+  }
+  // host: c = exp(-i tau T) e_1 through the symmetric eigendecomposition of T (H7)
+  std::vector<double> T(k * k, 0.0), Q;
+  for (int i = 0; i < k; ++i) {
+    T[i * k + i] = alpha[i];
+    if (i + 1 < k) T[i * k + i + 1] = T[(i + 1) * k + i] = beta[i];
+  }
+  jacobi_eig(k, T, Q);
+  std::vector<cplx> c(k);
+  for (int i = 0; i < k; ++i) {
+    double re = 0.0, im = 0.0;
+    for (int l = 0; l < k; ++l) {
+      const double lam = T[l * k + l], wgt = Q[i * k + l] * Q[0 * k + l];
+      re += wgt * std::cos(tau * lam);
+      im -= wgt * std::sin(tau * lam);
+    }
+    c[i] = make_double2(nrm * re, nrm * im);
+  }
+  ctx->timer_begin(T_VEC);
+  launch_lincomb(n, k, c.data(), V, n, theta, s, &ctx->launches);
+  ctx->timer_end();
+  FH_CUDA(cudaGetLastError());
+}
+
+// ============================================================================ environments
+static void run_two_stage(fh_ctx* ctx, Stage& st1, Stage& st2, BlockTensor& mid, const cplx* A1, const cplx* B1,
+                          const cplx* A2_or_null, const cplx* B2_or_null, cplx* out, bool mid_is_lhs2) {
+  // stage 1: mid = op(A1) op(B1); stage 2: out = op(lhs2) op(rhs2) where one operand is `mid`
+  ctx->alloc_tensor(mid);
+  ctx->pool_aux.reserve(stage_bytes(st1) + stage_bytes(st2) + 4096, ctx->stream);
+  upload_stage(ctx->pool_aux, st1, ctx->stream);
+  upload_stage(ctx->pool_aux, st2, ctx->stream);
+  cplx* pm = ctx->ptr(mid.base);
+  launch_grouped_gemm(st1, A1, B1, pm, ctx->stream, &ctx->launches);
+  if (mid_is_lhs2) launch_grouped_gemm(st2, pm, B2_or_null, out, ctx->stream, &ctx->launches);
+  else launch_grouped_gemm(st2, A2_or_null, pm, out, ctx->stream, &ctx->launches);
+  FH_CUDA(cudaGetLastError());
+  ctx->free_tensor(mid);
+}
+
+void fh::do_env_update_left(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int site) {
+  FH_REQUIRE(site >= 0 && site < mps->L, FH_EINVAL, "env_update_left: site out of range");
+  BlockTensor& Le = mps->Lenv[site];
+  BlockTensor& A = mps->A[site];
+  FH_REQUIRE(Le.base >= 0 && A.base >= 0, FH_ESTATE, "env_update_left: L_site or A_site missing");
+  BlockTensor X, out;
+  Stage st1, st2;
+  emit_env_left(Le, A, mpo->site[site & 1], X, out, st1, st2);
+  ctx->free_tensor(mps->Lenv[site + 1]);
+  ctx->alloc_tensor(out);
+  ctx->timer_begin(T_ENV);
+  run_two_stage(ctx, st1, st2, X, ctx->ptr(Le.base), ctx->ptr(A.base), ctx->ptr(A.base), nullptr,
+                ctx->ptr(out.base), false);
+  ctx->timer_end();
+  mps->Lenv[site + 1] = out;
+}
+
+void fh::do_env_update_right(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int site) {
+  FH_REQUIRE(site >= 0 && site < mps->L, FH_EINVAL, "env_update_right: site out of range");
+  BlockTensor& Re = mps->Renv[site + 1];
+  BlockTensor& A = mps->A[site];
+  FH_REQUIRE(Re.base >= 0 && A.base >= 0, FH_ESTATE, "env_update_right: R_{site+1} or A_site missing");
+  BlockTensor Y, out;
+  Stage st1, st2;
+  emit_env_right(Re, A, mpo->site[site & 1], Y, out, st1, st2);
+  ctx->free_tensor(mps->Renv[site]);
+  ctx->alloc_tensor(out);
+  ctx->timer_begin(T_ENV);
+  run_two_stage(ctx, st1, st2, Y, ctx->ptr(A.base), ctx->ptr(Re.base), nullptr, ctx->ptr(A.base),
+                ctx->ptr(out.base), true);
+  ctx->timer_end();
+  mps->Renv[site] = out;
+}
+
+// ============================================================================ C ABI
+#define FH_TRY(ctxptr, ...)                    \
+  try {                                        \
+    __VA_ARGS__;                               \
+    return FH_OK;                              \
+  } catch (const fh::FhError& e) {             \
+    if (ctxptr) (ctxptr)->err = e.what();      \
+    return e.code;                             \
+  } catch (const std::exception& e) {          \
+    if (ctxptr) (ctxptr)->err = e.what();      \
+    return FH_EINVAL;                          \
+  }
+
+extern "C" {
+
+int fh_ctx_create(fh_ctx** out, void* cuda_stream, void* arena_dev, size_t arena_bytes) {
+  if (!out || arena_bytes < (1u << 20)) return FH_EINVAL;
+  fh_ctx* c = new fh_ctx();
+  try {
+    int ndev = 0;
+    FH_CUDA(cudaGetDeviceCount(&ndev));
+    FH_REQUIRE(ndev > 0, FH_ECUDA, "no CUDA device");
+    c->stream = (cudaStream_t)cuda_stream;
+    if (arena_dev) {
+      c->arena = (cplx*)arena_dev;
+    } else {
+      FH_CUDA(cudaMalloc((void**)&c->arena, arena_bytes));
+      c->own_arena = true;
+    }
+    c->alloc.init((int64_t)(arena_bytes / sizeof(cplx)));
+    c->ensure_pinned(4096);
+  } catch (const std::exception& e) {
+    delete c;
+    return FH_ECUDA;
+  }
+  *out = c;
+  return FH_OK;
+}
+
+void fh_ctx_destroy(fh_ctx* c) {
+  if (!c) return;
+  cudaStreamSynchronize(c->stream);
+  for (auto& sp : c->spans) {
+    cudaEventDestroy(sp.a);
+    cudaEventDestroy(sp.b);
+  }
+  for (auto e : c->ev_free) cudaEventDestroy(e);
+  c->plan.pool.destroy();
+  c->pool_aux.destroy();
+  if (c->cusolver) cusolverDnDestroy(c->cusolver);
+  if (c->svd_work) cudaFree(c->svd_work);
+  if (c->d_info) cudaFree(c->d_info);
+  if (c->h_pinned) cudaFreeHost(c->h_pinned);
+  if (c->own_arena) cudaFree(c->arena);
+  delete c;
+}
+
+const char* fh_last_error(const fh_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+int fh_arena_stats(const fh_ctx* c, size_t* used, size_t* peak) {
+  if (!c) return FH_EINVAL;
+  if (used) *used = (size_t)c->alloc.used * sizeof(cplx);
+  if (peak) *peak = (size_t)c->alloc.peak * sizeof(cplx);
+  return FH_OK;
+}
+
+int fh_mpo_build(fh_ctx* ctx, int L, double t_h, double U, fh_mpo** out) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(out != nullptr, FH_EINVAL, "fh_mpo_build: out is NULL");
+    FH_REQUIRE(L >= 2 && L <= 4096 && L % 2 == 0, FH_EINVAL, "fh_mpo_build: L must be even, 2 <= L <= 4096");
+    fh_mpo* m = new fh_mpo();
+    m->L = L;
+    m->t_h = t_h;
+    m->U = U;
+    mpo_site_table(0, t_h, U, m->site[0]);
+    mpo_site_table(1, t_h, U, m->site[1]);
+    *out = m;
+  })
+}
+void fh_mpo_destroy(fh_mpo* m) { delete m; }
+
+int fh_mpo_get_site(const fh_mpo* mpo, int site, double* val, int32_t* rank2) {
+  if (!mpo || site < 0 || site >= mpo->L) return FH_EINVAL;
+  const MpoSite& W = mpo->site[site & 1];
+  if (val) std::memcpy(val, W.val, sizeof(W.val));
+  if (rank2)
+    for (int a = 0; a < 4; ++a)
+      for (int b = 0; b < 4; ++b) rank2[a * 4 + b] = W.rank2[a][b];
+  return FH_OK;
+}
+
+static void set_boundaries(fh_ctx* ctx, fh_mps* m) {
+  // L_0[(0,0),S,(0,0)] = 1, R_L[(0,0),F,(0,0)] = 1 (F-4)
+  const cplx one = make_double2(1.0, 0.0);
+  for (int which = 0; which < 2; ++which) {
+    BlockTensor& E = which == 0 ? m->Lenv[0] : m->Renv[m->L];
+    ctx->free_tensor(E);
+    E.clear();
+    E.nlab = 5;
+    E.add(key_env(Sector{0, 0}, which == 0 ? 0 : 3, Sector{0, 0}), 1, 1);
+    E.finalize();
+    ctx->alloc_tensor(E);
+    FH_CUDA(cudaMemcpyAsync(ctx->ptr(E.base), &one, sizeof(cplx), cudaMemcpyHostToDevice, ctx->stream));
+  }
+}
+
+int mps_create(fh_ctx* ctx, int L, fh_mps** out) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && out, FH_EINVAL, "mps_create: NULL argument");
+    FH_REQUIRE(L >= 2 && L <= 4096 && L % 2 == 0, FH_EINVAL, "mps_create: L must be even, 2 <= L <= 4096");
+    fh_mps* m = new fh_mps();
+    m->L = L;
+    m->bond.resize(L + 1);
+    m->A.resize(L);
+    m->Lenv.resize(L + 1);
+    m->Renv.resize(L + 1);
+    m->bond[0].sec = {Sector{0, 0}};
+    m->bond[0].d = {1};
+    m->bond[L] = m->bond[0];
+    set_boundaries(ctx, m);
+    *out = m;
+  })
+}
+
+void mps_destroy(fh_ctx* ctx, fh_mps* m) {
+  if (!m) return;
+  if (ctx) {
+    for (auto& t : m->A) ctx->free_tensor(t);
+    for (auto& t : m->Lenv) ctx->free_tensor(t);
+    for (auto& t : m->Renv) ctx->free_tensor(t);
+  }
+  delete m;
+}
+
+int mps_init_neel(fh_ctx* ctx, const fh_mpo* mpo, int L, fh_mps** out) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && mpo && out, FH_EINVAL, "mps_init_neel: NULL argument");
+    FH_REQUIRE(mpo->L == L, FH_EINVAL, "mps_init_neel: L differs from the MPO's");
+    fh_mps* m = nullptr;
+    int rc = mps_create(ctx, L, &m);
+    if (rc != FH_OK) throw FhError(rc, ctx->err);
+    const cplx one = make_double2(1.0, 0.0);
+    int q = 0;
+    for (int i = 0; i < L; ++i) {
+      const int s = (i % 2 == 0) ? 0 : 1;
+      const int qn = q + SITE_Q[s];
+      m->bond[i + 1].sec = {Sector{qn, 0}};
+      m->bond[i + 1].d = {1};
+      BlockTensor& A = m->A[i];
+      A.clear();
+      A.nlab = 5;
+      A.add(key_site(Sector{q, 0}, s, Sector{qn, 0}), 1, 1);
+      A.finalize();
+      ctx->alloc_tensor(A);
+      FH_CUDA(cudaMemcpyAsync(ctx->ptr(A.base), &one, sizeof(cplx), cudaMemcpyHostToDevice, ctx->stream));
+      q = qn;
+    }
+    for (int i = L - 1; i >= 1; --i) do_env_update_right(ctx, mpo, m, i);
+    *out = m;
+  })
+}
+
+int mps_set_bond(fh_ctx* ctx, fh_mps* mps, int bond, int n, const int32_t* q, const int32_t* tj, const int32_t* d) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(mps && bond >= 0 && bond <= mps->L && n >= 1, FH_EINVAL, "mps_set_bond: bad argument");
+    Bond b;
+    for (int i = 0; i < n; ++i) {
+      FH_REQUIRE(tj[i] >= 0 && d[i] >= 1, FH_EINVAL, "mps_set_bond: tj >= 0 and d >= 1 required");
+      FH_REQUIRE(((q[i] + tj[i] - bond) & 1) == 0, FH_EINVAL, "mps_set_bond: parity rule q + 2j = bond (mod 2) violated");
+      if (i > 0) FH_REQUIRE(Sector({q[i - 1], tj[i - 1]}) < Sector({q[i], tj[i]}), FH_EINVAL, "mps_set_bond: labels must be sorted by (q, tj) and distinct");
+      b.sec.push_back(Sector{q[i], tj[i]});
+      b.d.push_back(d[i]);
+    }
+    if (bond == 0 || bond == mps->L)
+      FH_REQUIRE(n == 1 && q[0] == 0 && tj[0] == 0 && d[0] == 1, FH_EINVAL, "mps_set_bond: boundary bonds are the single sector (0,0), d=1");
+    mps->bond[bond] = b;
+  })
+}
+
+int mps_get_bond(const fh_mps* mps, int bond, int* n, int32_t* q, int32_t* tj, int32_t* d) {
+  if (!mps || bond < 0 || bond > mps->L || !n) return FH_EINVAL;
+  const Bond& b = mps->bond[bond];
+  *n = (int)b.sec.size();
+  for (size_t i = 0; i < b.sec.size(); ++i) {
+    if (q) q[i] = b.sec[i].q;
+    if (tj) tj[i] = b.sec[i].tj;
+    if (d) d[i] = b.d[i];
+  }
+  return FH_OK;
+}
+
+static void export_layout(const BlockTensor& t, int nlab, int* nblk, int64_t* nelem, int32_t* labels, int32_t* dims) {
+  if (nblk) *nblk = (int)t.keys.size();
+  if (nelem) *nelem = t.nelem;
+  for (size_t i = 0; i < t.keys.size(); ++i) {
+    if (labels)
+      for (int l = 0; l < nlab; ++l) labels[i * nlab + l] = t.keys[i][l];
+    if (dims) {
+      dims[2 * i] = t.rows[i];
+      dims[2 * i + 1] = t.cols[i];
+    }
+  }
+}
+
+int mps_site_layout(const fh_mps* mps, int site, int* nblk, int64_t* nelem, int32_t* labels, int32_t* dims) {
+  if (!mps || site < 0 || site >= mps->L) return FH_EINVAL;
+  if (mps->A[site].base >= 0 || !mps->A[site].keys.empty()) {
+    export_layout(mps->A[site], 5, nblk, nelem, labels, dims);
+  } else {
+    BlockTensor t;
+    layout_site(mps->bond[site], mps->bond[site + 1], t);
+    export_layout(t, 5, nblk, nelem, labels, dims);
+  }
+  return FH_OK;
+}
+
+int mps_set_site(fh_ctx* ctx, fh_mps* mps, int site, const void* data, int is_dev) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(mps && site >= 0 && site < mps->L && data, FH_EINVAL, "mps_set_site: bad argument");
+    BlockTensor t;
+    layout_site(mps->bond[site], mps->bond[site + 1], t);
+    ctx->free_tensor(mps->A[site]);
+    ctx->alloc_tensor(t);
+    FH_CUDA(cudaMemcpyAsync(ctx->ptr(t.base), data, t.nelem * sizeof(cplx),
+                            is_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, ctx->stream));
+    if (!is_dev) FH_CUDA(cudaStreamSynchronize(ctx->stream));
+    mps->A[site] = t;
+  })
+}
+
+int mps_get_site(fh_ctx* ctx, const fh_mps* mps, int site, void* data, int is_dev) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(mps && site >= 0 && site < mps->L && data, FH_EINVAL, "mps_get_site: bad argument");
+    const BlockTensor& t = mps->A[site];
+    FH_REQUIRE(t.base >= 0, FH_ESTATE, "mps_get_site: site tensor not set");
+    FH_CUDA(cudaMemcpyAsync(data, ctx->ptr(t.base), t.nelem * sizeof(cplx),
+                            is_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, ctx->stream));
+    FH_CUDA(cudaStreamSynchronize(ctx->stream));
+  })
+}
+
+int env_update_left(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int site) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && mpo && mps, FH_EINVAL, "env_update_left: NULL argument");
+    do_env_update_left(ctx, mpo, mps, site);
+  })
+}
+int env_update_right(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int site) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && mpo && mps, FH_EINVAL, "env_update_right: NULL argument");
+    do_env_update_right(ctx, mpo, mps, site);
+  })
+}
+
+int env_layout(const fh_mps* mps, int which, int bond, int* nblk, int64_t* nelem, int32_t* labels, int32_t* dims) {
+  if (!mps || bond < 0 || bond > mps->L || (which != 0 && which != 1)) return FH_EINVAL;
+  const BlockTensor& t = which == 0 ? mps->Lenv[bond] : mps->Renv[bond];
+  if (t.base < 0) return FH_ESTATE;
+  export_layout(t, 5, nblk, nelem, labels, dims);
+  return FH_OK;
+}
+
+int env_get(fh_ctx* ctx, const fh_mps* mps, int which, int bond, void* data, int is_dev) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(mps && bond >= 0 && bond <= mps->L && data && (which == 0 || which == 1), FH_EINVAL, "env_get: bad argument");
+    const BlockTensor& t = which == 0 ? mps->Lenv[bond] : mps->Renv[bond];
+    FH_REQUIRE(t.base >= 0, FH_ESTATE, "env_get: environment not built");
+    FH_CUDA(cudaMemcpyAsync(data, ctx->ptr(t.base), t.nelem * sizeof(cplx),
+                            is_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, ctx->stream));
+    FH_CUDA(cudaStreamSynchronize(ctx->stream));
+  })
+}
+
+int env_set(fh_ctx* ctx, fh_mps* mps, int which, int bond, int nblk, const int32_t* labels, const void* data, int is_dev) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(mps && bond >= 0 && bond <= mps->L && data && labels && nblk >= 1 && (which == 0 || which == 1), FH_EINVAL, "env_set: bad argument");
+    const Bond& b = mps->bond[bond];
+    BlockTensor t;
+    t.nlab = 5;
+    for (int i = 0; i < nblk; ++i) {
+      const int32_t* l = labels + 5 * i;
+      const Sector xp{l[0], l[1]}, x{l[3], l[4]};
+      const int w = l[2];
+      FH_REQUIRE(w >= 0 && w < 4 && b.find(xp) >= 0 && b.find(x) >= 0, FH_EINVAL, "env_set: label not in the bond table");
+      FH_REQUIRE(xp.q == x.q + MPO_Q[w] && triangle(x.tj, MPO_TK[w], xp.tj), FH_EINVAL, "env_set: block violates the selection rule");
+      const Key k = key_env(xp, w, x);
+      if (i > 0) FH_REQUIRE(t.keys.back() < k, FH_EINVAL, "env_set: blocks must be in canonical order");
+      t.add(k, b.dim(xp), b.dim(x));
+    }
+    t.finalize();
+    BlockTensor& E = which == 0 ? mps->Lenv[bond] : mps->Renv[bond];
+    ctx->free_tensor(E);
+    ctx->alloc_tensor(t);
+    FH_CUDA(cudaMemcpyAsync(ctx->ptr(t.base), data, t.nelem * sizeof(cplx),
+                            is_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, ctx->stream));
+    if (!is_dev) FH_CUDA(cudaStreamSynchronize(ctx->stream));
+    E = t;
+  })
+}
+
+int heff_plan(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, int nsite) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && mpo && mps, FH_EINVAL, "heff_plan: NULL argument");
+    plan_heff(ctx, mpo, mps, site, nsite);
+  })
+}
+
+int heff_layout(const fh_ctx* ctx, int* nblk, int64_t* nelem, int32_t* labels, int32_t* dims) {
+  if (!ctx || !ctx->plan.valid) return FH_ESTATE;
+  export_layout(ctx->plan.vec, ctx->plan.nsite == 2 ? 8 : 5, nblk, nelem, labels, dims);
+  return FH_OK;
+}
+
+int heff_get_tasks(const fh_ctx* ctx, int stage, int* ntask, int* nout, int32_t* tuples, double* alpha) {
+  if (!ctx || !ctx->plan.valid || (stage != 1 && stage != 2)) return FH_ESTATE;
+  const Stage& st = stage == 1 ? ctx->plan.st1 : ctx->plan.st2;
+  if (ntask) *ntask = (int)st.t_out.size();
+  if (nout) *nout = (int)st.outs.size();
+  for (size_t i = 0; i < st.t_out.size(); ++i) {
+    if (tuples) {
+      tuples[3 * i] = st.t_out[i];
+      tuples[3 * i + 1] = st.t_lhs[i];
+      tuples[3 * i + 2] = st.t_rhs[i];
+    }
+    if (alpha) alpha[i] = st.t_alpha[i];
+  }
+  return FH_OK;
+}
+
+int heff_apply(fh_ctx* ctx, const void* theta_dev, void* out_dev) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && theta_dev && out_dev, FH_EINVAL, "heff_apply: NULL argument");
+    apply_heff(ctx, (const cplx*)theta_dev, (cplx*)out_dev);
+  })
+}
+
+int64_t heff_flops(const fh_ctx* ctx) {
+  if (!ctx || !ctx->plan.valid) return -1;
+  return ctx->plan.st1.flops + ctx->plan.st2.flops;
+}
+
+int heff_inner(fh_ctx* ctx, const void* x_dev, const void* y_dev, double* result) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && x_dev && y_dev && result, FH_EINVAL, "heff_inner: NULL argument");
+    const double2 r = inner(ctx, (const cplx*)x_dev, (const cplx*)y_dev);
+    result[0] = r.x;
+    result[1] = r.y;
+  })
+}
+
+int heff_expm(fh_ctx* ctx, const void* theta_dev, void* out_dev, double tau, int krylov_dim) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && theta_dev && out_dev, FH_EINVAL, "heff_expm: NULL argument");
+    FH_REQUIRE(ctx->plan.valid, FH_ESTATE, "heff_expm: no plan");
+    const int64_t n = ctx->plan.vec.nelem;
+    const int64_t woff = ctx->alloc.alloc((int64_t)(krylov_dim + 1) * n);
+    try {
+      if (out_dev != theta_dev)
+        FH_CUDA(cudaMemcpyAsync(out_dev, theta_dev, n * sizeof(cplx), cudaMemcpyDeviceToDevice, ctx->stream));
+      expm_lanczos(ctx, (cplx*)out_dev, tau, krylov_dim, 1e-12, ctx->ptr(woff));
+    } catch (...) {
+      ctx->alloc.release(woff, (int64_t)(krylov_dim + 1) * n);
+      throw;
+    }
+    ctx->alloc.release(woff, (int64_t)(krylov_dim + 1) * n);
+  })
+}
+
+int tdvp2_sweep(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh_params* p) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && mpo && mps && p, FH_EINVAL, "tdvp2_sweep: NULL argument");
+    FH_REQUIRE(p->krylov_dim >= 2 && p->krylov_dim <= 32 && p->chi_max_full >= 1, FH_EINVAL, "tdvp2_sweep: bad parameters");
+    sweep(ctx, mpo, mps, dt, p);
+  })
+}
+
+int tdvp2_last_stats(const fh_ctx* ctx, double* disc, int* chi_full, int* chi_su2, int* dmax) {
+  if (!ctx) return FH_EINVAL;
+  if (disc) *disc = ctx->stat_disc;
+  if (chi_full) *chi_full = ctx->stat_chi;
+  if (chi_su2) *chi_su2 = ctx->stat_su2;
+  if (dmax) *dmax = ctx->stat_dmax;
+  return FH_OK;
+}
+
+int measure_local(fh_ctx* ctx, const fh_mps* mps, double* n_i, double* sz_i, double* docc_i) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && mps && n_i && sz_i && docc_i, FH_EINVAL, "measure_local: NULL argument");
+    measure_local_impl(ctx, mps, n_i, sz_i, docc_i);
+  })
+}
+
+int measure_global(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, double* norm2, double* energy) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && mpo && mps, FH_EINVAL, "measure_global: NULL argument");
+    // full left contraction on a scratch copy of the left environments
+    fh_mps tmp;
+    tmp.L = mps->L;
+    tmp.bond = mps->bond;
+    tmp.A = mps->A;  // shares device storage (read only)
+    tmp.Lenv.resize(mps->L + 1);
+    tmp.Renv.resize(mps->L + 1);
+    tmp.Lenv[0] = mps->Lenv[0];
+    for (int i = 0; i < mps->L; ++i) {
+      do_env_update_left(ctx, mpo, &tmp, i);
+      if (i > 0) ctx->free_tensor(tmp.Lenv[i]);
+    }
+    BlockTensor& E = tmp.Lenv[mps->L];
+    const int is = E.find(key_env(Sector{0, 0}, 0, Sector{0, 0})), ie = E.find(key_env(Sector{0, 0}, 3, Sector{0, 0}));
+    std::vector<cplx> h(E.nelem);
+    FH_CUDA(cudaMemcpyAsync(h.data(), ctx->ptr(E.base), E.nelem * sizeof(cplx), cudaMemcpyDeviceToHost, ctx->stream));
+    FH_CUDA(cudaStreamSynchronize(ctx->stream));
+    const double n2 = is >= 0 ? h[E.off[is]].x : 0.0;
+    if (norm2) *norm2 = n2;
+    if (energy) *energy = (ie >= 0 && n2 != 0.0) ? h[E.off[ie]].x / n2 : 0.0;
+    ctx->free_tensor(E);
+  })
+}
+
+int fh_get_timers(const fh_ctx* cctx, double* a, double* b, double* c, double* d, double* e) {
+  fh_ctx* ctx = const_cast<fh_ctx*>(cctx);
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx != nullptr, FH_EINVAL, "fh_get_timers: NULL context");
+    ctx->timers_resolve();
+    if (a) *a = ctx->sec[T_HEFF];
+    if (b) *b = ctx->sec[T_ENV];
+    if (c) *c = ctx->sec[T_SVD];
+    if (d) *d = ctx->sec[T_VEC];
+    if (e) *e = ctx->sec[T_PACK];
+  })
+}
+int fh_reset_timers(fh_ctx* ctx) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx != nullptr, FH_EINVAL, "fh_reset_timers: NULL context");
+    ctx->timers_resolve();
+    for (int i = 0; i < T_NCAT; ++i) ctx->sec[i] = 0.0;
+  })
+}
+int64_t fh_launch_count(const fh_ctx* ctx) { return ctx ? ctx->launches : -1; }
+
+int fh_cublas_gemm_seconds(fh_ctx* ctx, int n, int is_complex, int reps, double* seconds) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && n > 0 && reps > 0 && seconds, FH_EINVAL, "fh_cublas_gemm_seconds: bad argument");
+    cublasHandle_t h;
+    FH_REQUIRE(cublasCreate(&h) == CUBLAS_STATUS_SUCCESS, FH_ECUDA, "cublasCreate failed");
+    cublasSetStream(h, ctx->stream);
+    const size_t el = is_complex ? 16 : 8;
+    void *A, *B, *C;
+    FH_CUDA(cudaMalloc(&A, el * n * n));
+    FH_CUDA(cudaMalloc(&B, el * n * n));
+    FH_CUDA(cudaMalloc(&C, el * n * n));
+    FH_CUDA(cudaMemsetAsync(A, 0x3c, el * n * n, ctx->stream));
+    FH_CUDA(cudaMemsetAsync(B, 0x3c, el * n * n, ctx->stream));
+    cudaEvent_t e0, e1;
+    FH_CUDA(cudaEventCreate(&e0));
+    FH_CUDA(cudaEventCreate(&e1));
+    const double one = 1.0, zero = 0.0;
+    const cuDoubleComplex zone = make_cuDoubleComplex(1, 0), zzero = make_cuDoubleComplex(0, 0);
+    for (int it = -2; it < reps; ++it) {
+      if (it == 0) FH_CUDA(cudaEventRecord(e0, ctx->stream));
+      if (is_complex)
+        cublasZgemm(h, CUBLAS_OP_N, CUBLAS_OP_N, n, n, n, &zone, (cuDoubleComplex*)A, n, (cuDoubleComplex*)B, n, &zzero, (cuDoubleComplex*)C, n);
+      else
+        cublasDgemm(h, CUBLAS_OP_N, CUBLAS_OP_N, n, n, n, &one, (double*)A, n, (double*)B, n, &zero, (double*)C, n);
+    }
+    FH_CUDA(cudaEventRecord(e1, ctx->stream));
+    FH_CUDA(cudaEventSynchronize(e1));
+    float ms = 0;
+    FH_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+    *seconds = ms * 1e-3 / reps;
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(A);
+    cudaFree(B);
+    cudaFree(C);
+    cublasDestroy(h);
+  })
+}
+
+// host-only helpers for the CPU test-suite (symmetry layer without a GPU)
+static fh::Stage g_host_st1, g_host_st2;
+
+int fh_host_plan(int site, int nsite, double t_h, double U, int nl, const int32_t* bl, int nr, const int32_t* br,
+                 int nLblk, const int32_t* Llab, int nRblk, const int32_t* Rlab) {
+  try {
+    if ((nsite != 1 && nsite != 2) || !bl || !br || !Llab || !Rlab) return FH_EINVAL;
+    Bond Bl, Br;
+    for (int i = 0; i < nl; ++i) { Bl.sec.push_back(Sector{bl[3 * i], bl[3 * i + 1]}); Bl.d.push_back(bl[3 * i + 2]); }
+    for (int i = 0; i < nr; ++i) { Br.sec.push_back(Sector{br[3 * i], br[3 * i + 1]}); Br.d.push_back(br[3 * i + 2]); }
+    BlockTensor Le, Re, vec, Z;
+    Le.nlab = Re.nlab = 5;
+    for (int i = 0; i < nLblk; ++i) {
+      const int32_t* l = Llab + 5 * i;
+      Le.add(key_env(Sector{l[0], l[1]}, l[2], Sector{l[3], l[4]}), Bl.dim(Sector{l[0], l[1]}), Bl.dim(Sector{l[3], l[4]}));
+    }
+    for (int i = 0; i < nRblk; ++i) {
+      const int32_t* l = Rlab + 5 * i;
+      Re.add(key_env(Sector{l[0], l[1]}, l[2], Sector{l[3], l[4]}), Br.dim(Sector{l[0], l[1]}), Br.dim(Sector{l[3], l[4]}));
+    }
+    Le.finalize();
+    Re.finalize();
+    MpoSite W1, W2;
+    mpo_site_table(site, t_h, U, W1);
+    mpo_site_table(site + 1, t_h, U, W2);
+    if (nsite == 2) {
+      layout_theta(Bl, Br, vec);
+      emit_heff2(Le, Re, vec, W1, W2, Z, g_host_st1, g_host_st2);
+    } else {
+      layout_site(Bl, Br, vec);
+      emit_heff1(Le, Re, vec, W1, Z, g_host_st1, g_host_st2);
+    }
+    return FH_OK;
+  } catch (...) {
+    return FH_EINVAL;
+  }
+}
+
+int fh_host_get_tasks(int stage, int* ntask, int* nout, int32_t* tuples, double* alpha, int64_t* flops) {
+  if (stage != 1 && stage != 2) return FH_EINVAL;
+  const Stage& st = stage == 1 ? g_host_st1 : g_host_st2;
+  if (ntask) *ntask = (int)st.t_out.size();
+  if (nout) *nout = (int)st.outs.size();
+  if (flops) *flops = st.flops;
+  for (size_t i = 0; i < st.t_out.size(); ++i) {
+    if (tuples) { tuples[3 * i] = st.t_out[i]; tuples[3 * i + 1] = st.t_lhs[i]; tuples[3 * i + 2] = st.t_rhs[i]; }
+    if (alpha) alpha[i] = st.t_alpha[i];
+  }
+  return FH_OK;
+}
+
+double fh_coef_left(int ta, int ts, int tc, int tk, int tr, int tkp, int tap, int tsp, int tcp) {
+  return fh::coef_left(ta, ts, tc, tk, tr, tkp, tap, tsp, tcp);
+}
+double fh_coef_right(int tc, int ts, int tb, int tk, int tr, int tkp, int tcp, int tsp, int tbp) {
+  return fh::coef_right(tc, ts, tb, tk, tr, tkp, tcp, tsp, tbp);
+}
+
+}  // extern "C"

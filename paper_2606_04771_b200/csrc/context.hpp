@@ -1,0 +1,141 @@
+// Context, arena, device pools, plans (host side of libfh_b200).
+#pragma once
+#include <cusolverDn.h>
+
+#include <stdexcept>
+
+#include "fh_b200.h"
+#include "symmetry.hpp"
+
+namespace fh {
+
+struct FhError : std::runtime_error {
+  int code;
+  FhError(int c, const std::string& m) : std::runtime_error(m), code(c) {}
+};
+#define FH_CUDA(x)                                                                                    \
+  do {                                                                                                \
+    cudaError_t e__ = (x);                                                                            \
+    if (e__ != cudaSuccess)                                                                           \
+      throw fh::FhError(FH_ECUDA, std::string(#x) + ": " + cudaGetErrorString(e__));                  \
+  } while (0)
+#define FH_REQUIRE(cond, code, msg) \
+  do {                              \
+    if (!(cond)) throw fh::FhError(code, msg); \
+  } while (0)
+
+// first-fit free-list allocator over the single HBM arena; unit = complex128 elements
+struct Arena {
+  int64_t cap = 0, used = 0, peak = 0;
+  std::map<int64_t, int64_t> free_;  // offset -> length
+  static int64_t round_up(int64_t n) { return (n + 15) / 16 * 16; }  // 256-byte granules
+  void init(int64_t n) {
+    cap = n;
+    used = peak = 0;
+    free_.clear();
+    free_[0] = n;
+  }
+  int64_t alloc(int64_t n);
+  void release(int64_t off, int64_t n);
+};
+
+// grow-only device buffer for task lists and other small per-plan tables
+struct DevPool {
+  char* ptr = nullptr;
+  size_t cap = 0, top = 0;
+  void reset() { top = 0; }
+  void reserve(size_t bytes, cudaStream_t s);
+  void* take(size_t bytes);
+  void destroy();
+};
+
+struct Plan {
+  bool valid = false;
+  int nsite = 0, site = 0;
+  BlockTensor vec;  // layout of the vector H_eff acts on (base unused)
+  BlockTensor Z;    // stage-1 intermediate, allocated in the arena
+  Stage st1, st2;
+  const cplx* Lptr = nullptr;
+  const cplx* Rptr = nullptr;
+  std::vector<VecChunk> chunks;
+  VecChunk* d_chunks = nullptr;
+  double* d_partial = nullptr;
+  double* d_result = nullptr;
+  DevPool pool;
+};
+
+enum { T_HEFF = 0, T_ENV = 1, T_SVD = 2, T_VEC = 3, T_PACK = 4, T_NCAT = 5 };
+
+}  // namespace fh
+
+struct fh_mpo {
+  int L;
+  double t_h, U;
+  fh::MpoSite site[2];  // even / odd site parity
+};
+
+struct fh_mps {
+  int L;
+  std::vector<fh::Bond> bond;                       // L+1
+  std::vector<fh::BlockTensor> A, Lenv, Renv;       // L, L+1, L+1
+};
+
+struct fh_ctx {
+  cudaStream_t stream = nullptr;
+  fh::cplx* arena = nullptr;
+  bool own_arena = false;
+  fh::Arena alloc;
+  std::string err;
+  fh::Plan plan;
+  fh::DevPool pool_aux;  // env updates, merge, pack, measure
+  int64_t launches = 0;
+  // pinned host scratch
+  double* h_pinned = nullptr;  // 4096 doubles
+  size_t h_pinned_n = 0;
+  // timers
+  double sec[fh::T_NCAT] = {0, 0, 0, 0, 0};
+  struct Span {
+    cudaEvent_t a, b;
+    int cat;
+  };
+  std::vector<Span> spans;
+  std::vector<cudaEvent_t> ev_free;
+  // SVD
+  cusolverDnHandle_t cusolver = nullptr;
+  void* svd_work = nullptr;
+  size_t svd_work_bytes = 0;
+  int* d_info = nullptr;
+  // last sweep statistics
+  double stat_disc = 0.0;
+  int stat_chi = 0, stat_su2 = 0, stat_dmax = 0;
+
+  fh::cplx* ptr(int64_t off) const { return arena + off; }
+  void alloc_tensor(fh::BlockTensor& t);
+  void free_tensor(fh::BlockTensor& t);
+  void timer_begin(int cat);
+  void timer_end();
+  void timers_resolve();
+  void ensure_pinned(size_t ndoubles);
+};
+
+namespace fh {
+template <class T>
+T* upload(DevPool& pool, const std::vector<T>& v, cudaStream_t s) {
+  if (v.empty()) return nullptr;
+  T* d = (T*)pool.take(v.size() * sizeof(T));
+  FH_CUDA(cudaMemcpyAsync(d, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice, s));
+  return d;
+}
+size_t stage_bytes(const Stage& st);
+void upload_stage(DevPool& pool, Stage& st, cudaStream_t s);
+
+// engine pieces (api.cu / tdvp.cu)
+void plan_heff(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, int nsite);
+void apply_heff(fh_ctx* ctx, const cplx* theta, cplx* out);
+double2 inner(fh_ctx* ctx, const cplx* x, const cplx* y);  // synchronises
+void expm_lanczos(fh_ctx* ctx, cplx* theta_inout, double tau, int m, double tol, cplx* work /* (m+1)*n */);
+void do_env_update_left(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int site);
+void do_env_update_right(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int site);
+void sweep(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh_params* p);
+void measure_local_impl(fh_ctx* ctx, const fh_mps* mps, double* n_i, double* sz_i, double* docc_i);
+}  // namespace fh

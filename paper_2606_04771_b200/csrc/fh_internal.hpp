@@ -1,0 +1,143 @@
+// Internal declarations shared by the host layer and the kernels of libfh_b200.
+// Product code: no dependency on oracle/ ("independence").
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <array>
+#include <map>
+#include <string>
+#include <vector>
+
+namespace fh {
+
+typedef double2 cplx;  // complex128, interleaved (re, im)
+
+// ----------------------------------------------------------------------------- labels
+struct Sector {
+  int q, tj;
+  bool operator<(const Sector& o) const { return q != o.q ? q < o.q : tj < o.tj; }
+  bool operator==(const Sector& o) const { return q == o.q && tj == o.tj; }
+};
+
+// (q, tj) of the site multiplets s = 0,1,2 and of the MPO bond multiplets w = S,P,M,F
+static const int SITE_Q[3] = {1, -1, 0};
+static const int SITE_TJ[3] = {0, 0, 1};
+static const int MPO_Q[4] = {0, 1, -1, 0};
+static const int MPO_TK[4] = {0, 1, 1, 0};
+
+inline bool triangle(int t1, int t2, int t3) {
+  int lo = t1 > t2 ? t1 - t2 : t2 - t1;
+  return lo <= t3 && t3 <= t1 + t2 && ((t1 + t2 + t3) & 1) == 0;
+}
+
+// flattened label tuple, zero padded; compared lexicographically (== Python tuple order)
+typedef std::array<int, 12> Key;
+
+struct Bond {
+  std::vector<Sector> sec;  // sorted
+  std::vector<int> d;
+  int find(Sector s) const;
+  int dim(Sector s) const {
+    int i = find(s);
+    return i < 0 ? 0 : d[i];
+  }
+  int chi_full() const;
+  int chi_su2() const;
+  int dmax() const;
+};
+
+struct BlockTensor {
+  std::vector<Key> keys;  // sorted
+  std::vector<int> rows, cols;
+  std::vector<int64_t> off;  // element offsets relative to the tensor base
+  int64_t nelem = 0;
+  int64_t base = -1;  // element offset in the arena, -1 = not allocated
+  int nlab = 0;       // number of meaningful ints in each key
+  std::map<Key, int> index;
+  void clear();
+  void add(const Key& k, int r, int c);  // append (caller adds in sorted order)
+  void finalize();                       // offsets (each block 2-element aligned => 32 B)
+  int find(const Key& k) const;
+};
+
+// reduced MPO of one site parity: val[w][w'][s'][s], rank2[w][w'] (-1 = absent)
+struct MpoSite {
+  double val[4][4][3][3];
+  int rank2[4][4];
+};
+
+// recoupling coefficients, closed forms (su2.cpp)
+double wigner6j(int ta, int tb, int tc, int td, int te, int tf);
+double wigner9j(int a, int b, int c, int d, int e, int f, int g, int h, int i);
+double coef_left(int ta, int ts, int tc, int tk, int tr, int tkp, int tap, int tsp, int tcp);
+double coef_right(int tc, int ts, int tb, int tk, int tr, int tkp, int tcp, int tsp, int tbp);
+
+// ----------------------------------------------------------------------------- GEMM task lists
+enum OpA { OPA_N = 0, OPA_C = 1, OPA_H = 2 };  // as stored | conj | conj-transpose
+enum OpB { OPB_N = 0, OPB_T = 1 };             // as stored | transpose
+
+struct GemmOut {  // one output block C (M x N, row-major, ld = N)
+  int64_t c_off;
+  int M, N;
+  int seg_begin, seg_end;
+};
+struct GemmSeg {  // one K-segment: C += alpha * op(A) (M x K) * op(B) (K x N)
+  int64_t a_off, b_off;
+  int K, lda, ldb, pad;
+  double alpha;
+};
+struct GemmTile {  // one CTA's work: tile (m0, n0) of output block `out`
+  int out, m0, n0, pad;
+};
+
+struct Stage {
+  // host copies (canonical order) for heff_get_tasks and flops
+  std::vector<int> t_out, t_lhs, t_rhs;
+  std::vector<double> t_alpha;
+  std::vector<GemmOut> outs;
+  std::vector<GemmSeg> segs;
+  std::vector<GemmTile> tiles64, tiles32;
+  int opA = OPA_N, opB = OPB_N;
+  int64_t flops = 0;
+  // device copies
+  GemmOut* d_outs = nullptr;
+  GemmSeg* d_segs = nullptr;
+  GemmTile* d_tiles64 = nullptr;
+  GemmTile* d_tiles32 = nullptr;
+};
+
+// weighted-vector chunk table (H6): contiguous chunk [start, start+len) carries weight w
+struct VecChunk {
+  int64_t start;
+  int len;
+  float w;  // 2j+1, small integer: exact in float
+};
+
+// pack / unpack copy descriptors (H8, H9)
+struct CopyBlk {
+  int64_t src_off, dst_off;
+  int rows, cols, ld_src, ld_dst;
+  int transpose_dst;  // write dst[c*ld_dst + r] instead of dst[r*ld_dst + c]
+  int pad;
+  double scale;
+};
+
+// ----------------------------------------------------------------------------- kernel launchers (kernels.cu)
+void launch_grouped_gemm(const Stage& st, const cplx* A, const cplx* B, cplx* C, cudaStream_t s,
+                         int64_t* launch_counter);
+void launch_wdot(const VecChunk* d_chunks, int nchunks, const cplx* x, const cplx* y, double* d_partial,
+                 double* d_result, cudaStream_t s, int64_t* launch_counter);
+// y = y + a*x (a complex, from device scalar array coef[idx]*sign) etc.: see kernels.cu
+void launch_axpy(int64_t n, cplx a, const cplx* x, cplx* y, cudaStream_t s, int64_t* lc);
+void launch_scale(int64_t n, cplx a, const cplx* x, cplx* y, cudaStream_t s, int64_t* lc);  // y = a*x
+void launch_lincomb(int64_t n, int m, const cplx* coef_host, const cplx* V, int64_t stride, cplx* y,
+                    cudaStream_t s, int64_t* lc);  // y = sum_j coef[j] V[j]
+void launch_copy_blocks(const CopyBlk* d_blks, int nblk, const cplx* src, cplx* dst, cudaStream_t s,
+                        int64_t* lc);
+// per-block weighted squared norms: out[i] = sum |x|^2 over block i
+void launch_block_norms(const VecChunk* d_chunks, int nchunks, const cplx* x, double* d_out,
+                        cudaStream_t s, int64_t* lc);
+void launch_fill_zero(cplx* p, int64_t n, cudaStream_t s, int64_t* lc);
+
+}  // namespace fh

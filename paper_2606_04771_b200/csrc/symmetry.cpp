@@ -1,0 +1,537 @@
+// Host symmetry layer: labels, fusion rules, reduced MPO, task lists.
+//
+// Canonical orders (must match what DESIGN.md states; the oracle emits the same lists from its
+// own code and the tests compare the integer tuples bit for bit):
+//   * blocks of a tensor: lexicographic in the flattened label tuple, sectors ordered by (q, tj);
+//   * stage-1 tasks of a left contraction: by output key (a',s',c',w', rest of the ket key),
+//     segments by (w, a, s);
+//   * two-site stage 2: by output key, segments by (c, s2, b, w_m, w_r);
+//   * one-site stage 2: by output key, segments by (c, w');
+//   * left-environment stage 2: by output key (c',w',c), segments by (a', s');
+//   * right-environment stage 2: by output key (c',w,c), segments by (s', b', w', s, b).
+#include "symmetry.hpp"
+
+#include <algorithm>
+#include <cmath>
+#include <stdexcept>
+
+namespace fh {
+
+// ----------------------------------------------------------------------------- Bond / BlockTensor
+int Bond::find(Sector s) const {
+  auto it = std::lower_bound(sec.begin(), sec.end(), s);
+  if (it == sec.end() || !(*it == s)) return -1;
+  return (int)(it - sec.begin());
+}
+int Bond::chi_full() const {  // Eq. (8)
+  int x = 0;
+  for (size_t i = 0; i < sec.size(); ++i) x += d[i] * (sec[i].tj + 1);
+  return x;
+}
+int Bond::chi_su2() const {  // Eq. (10)
+  int x = 0;
+  for (int v : d) x += v;
+  return x;
+}
+int Bond::dmax() const {  // Eq. (9)
+  int x = 0;
+  for (int v : d) x = std::max(x, v);
+  return x;
+}
+
+void BlockTensor::clear() {
+  keys.clear();
+  rows.clear();
+  cols.clear();
+  off.clear();
+  index.clear();
+  nelem = 0;
+  base = -1;
+}
+void BlockTensor::add(const Key& k, int r, int c) {
+  keys.push_back(k);
+  rows.push_back(r);
+  cols.push_back(c);
+}
+void BlockTensor::finalize() {
+  off.resize(keys.size());
+  index.clear();
+  int64_t n = 0;
+  for (size_t i = 0; i < keys.size(); ++i) {
+    off[i] = n;
+    n += (int64_t)rows[i] * cols[i];
+    index[keys[i]] = (int)i;
+  }
+  nelem = n;
+}
+int BlockTensor::find(const Key& k) const {
+  auto it = index.find(k);
+  return it == index.end() ? -1 : it->second;
+}
+
+static inline Sector key_sector(const Key& k, int pos) { return Sector{k[pos], k[pos + 1]}; }
+
+// labels c with a (x) s -> c
+static inline int fuse(Sector a, int s, Sector out[2]) {
+  int n = 0;
+  const int ts = SITE_TJ[s];
+  for (int tc = std::abs(a.tj - ts); tc <= a.tj + ts; tc += 2) out[n++] = Sector{a.q + SITE_Q[s], tc};
+  return n;
+}
+
+void layout_site(const Bond& bl, const Bond& br, BlockTensor& out) {
+  out.clear();
+  out.nlab = 5;
+  std::vector<std::pair<Key, std::pair<int, int>>> v;
+  for (size_t ia = 0; ia < bl.sec.size(); ++ia)
+    for (int s = 0; s < 3; ++s) {
+      Sector cs[2];
+      int n = fuse(bl.sec[ia], s, cs);
+      for (int j = 0; j < n; ++j) {
+        int ic = br.find(cs[j]);
+        if (ic >= 0) v.push_back({key_site(bl.sec[ia], s, cs[j]), {bl.d[ia], br.d[ic]}});
+      }
+    }
+  std::sort(v.begin(), v.end(), [](const auto& x, const auto& y) { return x.first < y.first; });
+  for (auto& e : v) out.add(e.first, e.second.first, e.second.second);
+  out.finalize();
+}
+
+void layout_theta(const Bond& bl, const Bond& br, BlockTensor& out) {
+  out.clear();
+  out.nlab = 8;
+  std::vector<std::pair<Key, std::pair<int, int>>> v;
+  for (size_t ia = 0; ia < bl.sec.size(); ++ia)
+    for (int s1 = 0; s1 < 3; ++s1) {
+      Sector cs[2];
+      int nc = fuse(bl.sec[ia], s1, cs);
+      for (int j = 0; j < nc; ++j)
+        for (int s2 = 0; s2 < 3; ++s2) {
+          Sector bs[2];
+          int nb = fuse(cs[j], s2, bs);
+          for (int l = 0; l < nb; ++l) {
+            int ib = br.find(bs[l]);
+            if (ib >= 0) v.push_back({key_theta(bl.sec[ia], s1, cs[j], s2, bs[l]), {bl.d[ia], br.d[ib]}});
+          }
+        }
+    }
+  std::sort(v.begin(), v.end(), [](const auto& x, const auto& y) { return x.first < y.first; });
+  for (auto& e : v) out.add(e.first, e.second.first, e.second.second);
+  out.finalize();
+}
+
+// ----------------------------------------------------------------------------- reduced MPO (F-2, F-3)
+void mpo_site_table(int site, double t_h, double U, MpoSite& W) {
+  for (int a = 0; a < 4; ++a)
+    for (int b = 0; b < 4; ++b) {
+      W.rank2[a][b] = -1;
+      for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) W.val[a][b][i][j] = 0.0;
+    }
+  const double eps = (site % 2 == 0) ? 1.0 : -1.0;  // eps_i = (-1)^i, 0-based (reading A-3)
+  const double eps_prev = -eps;
+  const double r2 = std::sqrt(2.0);
+  // identity and (U/2) P_D, rank 0
+  W.rank2[0][0] = 0;
+  W.rank2[3][3] = 0;
+  W.rank2[0][3] = 0;
+  for (int s = 0; s < 3; ++s) W.val[0][0][s][s] = W.val[3][3][s][s] = 1.0;
+  W.val[0][3][2][2] = 0.5 * U;
+  // opening operators Psi^+ P (S->P) and Psi^- P (S->M), rank 1/2
+  W.rank2[0][1] = 1;
+  W.val[0][1][0][2] = -r2;
+  W.val[0][1][2][1] = -eps;
+  W.rank2[0][2] = 1;
+  W.val[0][2][1][2] = -r2;
+  W.val[0][2][2][0] = +eps;
+  // closing operators: P->F carries -t eps_{i-1} sqrt2 Psi^-, M->F carries +t eps_{i-1} sqrt2 Psi^+
+  W.rank2[1][3] = 1;
+  W.val[1][3][1][2] = -t_h * eps_prev * r2 * (-r2);
+  W.val[1][3][2][0] = -t_h * eps_prev * r2 * (-eps);
+  W.rank2[2][3] = 1;
+  W.val[2][3][0][2] = +t_h * eps_prev * r2 * (-r2);
+  W.val[2][3][2][1] = +t_h * eps_prev * r2 * (+eps);
+}
+
+// ----------------------------------------------------------------------------- stage assembly
+void finalize_stage(Stage& st, const BlockTensor& out, const BlockTensor& lhs, const BlockTensor& rhs) {
+  const size_t nt = st.t_out.size();
+  st.outs.resize(out.keys.size());
+  st.segs.resize(nt);
+  st.flops = 0;
+  size_t t = 0;
+  for (size_t o = 0; o < out.keys.size(); ++o) {
+    GemmOut& go = st.outs[o];
+    go.c_off = out.off[o];
+    go.M = out.rows[o];
+    go.N = out.cols[o];
+    go.seg_begin = (int)t;
+    while (t < nt && st.t_out[t] == (int)o) {
+      const int l = st.t_lhs[t], r = st.t_rhs[t];
+      GemmSeg& sg = st.segs[t];
+      sg.a_off = lhs.off[l];
+      sg.b_off = rhs.off[r];
+      sg.lda = lhs.cols[l];
+      sg.ldb = rhs.cols[r];
+      sg.pad = 0;
+      sg.alpha = st.t_alpha[t];
+      int M, K, K2, N;
+      if (st.opA == OPA_H) { M = lhs.cols[l]; K = lhs.rows[l]; } else { M = lhs.rows[l]; K = lhs.cols[l]; }
+      if (st.opB == OPB_T) { N = rhs.rows[r]; K2 = rhs.cols[r]; } else { N = rhs.cols[r]; K2 = rhs.rows[r]; }
+      if (M != go.M || N != go.N || K != K2) throw std::runtime_error("task list: block shapes do not match");
+      sg.K = K;
+      st.flops += (int64_t)8 * M * N * K;
+      ++t;
+    }
+    go.seg_end = (int)t;
+  }
+  if (t != nt) throw std::runtime_error("task list: tasks not sorted by output id");
+  // tile queues, heaviest tiles first (the hardware CTA scheduler then balances greedily)
+  struct TW {
+    GemmTile tile;
+    int64_t work;
+  };
+  std::vector<TW> t64, t32;
+  for (size_t o = 0; o < st.outs.size(); ++o) {
+    const GemmOut& go = st.outs[o];
+    int64_t ksum = 0;
+    for (int s = go.seg_begin; s < go.seg_end; ++s) ksum += (st.segs[s].K + 3) / 4 * 4;
+    const bool small = (go.M <= 32 || go.N <= 32);
+    const int T = small ? 32 : 64;
+    for (int m0 = 0; m0 < go.M; m0 += T)
+      for (int n0 = 0; n0 < go.N; n0 += T) {
+        const int mv = (std::min(T, go.M - m0) + 7) / 8 * 8, nv = (std::min(T, go.N - n0) + 7) / 8 * 8;
+        TW tw{GemmTile{(int)o, m0, n0, 0}, (int64_t)mv * nv * (ksum + 8)};
+        (small ? t32 : t64).push_back(tw);
+      }
+  }
+  auto by_work = [](const TW& a, const TW& b) { return a.work > b.work; };
+  std::stable_sort(t64.begin(), t64.end(), by_work);
+  std::stable_sort(t32.begin(), t32.end(), by_work);
+  st.tiles64.clear();
+  st.tiles32.clear();
+  for (auto& x : t64) st.tiles64.push_back(x.tile);
+  for (auto& x : t32) st.tiles32.push_back(x.tile);
+}
+
+namespace {
+struct RawTask {
+  Key out;      // output block key
+  Key order;    // segment sort key
+  int lhs, rhs;
+  double alpha;
+};
+bool raw_less(const RawTask& a, const RawTask& b) { return a.out != b.out ? a.out < b.out : a.order < b.order; }
+
+// fill st.t_* from raw tasks (sorted here); `out` must already contain every key that occurs
+void tasks_to_stage(std::vector<RawTask>& raw, const BlockTensor& out, Stage& st) {
+  std::sort(raw.begin(), raw.end(), raw_less);
+  st.t_out.clear();
+  st.t_lhs.clear();
+  st.t_rhs.clear();
+  st.t_alpha.clear();
+  for (const RawTask& r : raw) {
+    const int o = out.find(r.out);
+    if (o < 0) throw std::runtime_error("task list: output key missing from layout");
+    st.t_out.push_back(o);
+    st.t_lhs.push_back(r.lhs);
+    st.t_rhs.push_back(r.rhs);
+    st.t_alpha.push_back(r.alpha);
+  }
+}
+
+// layout from the distinct output keys of raw tasks: rows/cols supplied per task
+struct Shape {
+  int r, c;
+};
+void layout_from_tasks(const std::vector<RawTask>& raw, const std::vector<Shape>& shapes, int nlab,
+                       BlockTensor& out) {
+  std::map<Key, Shape> m;
+  for (size_t i = 0; i < raw.size(); ++i) m[raw[i].out] = shapes[i];
+  out.clear();
+  out.nlab = nlab;
+  for (auto& e : m) out.add(e.first, e.second.r, e.second.c);
+  out.finalize();
+}
+
+// Generic "left contraction" (stage 1 of H1, H3, H4):
+//   Z[a',s',c',w' ; rest] = sum_{(w,a,s)} alpha * Lenv[a',w,a] * ket[a,s,c; rest]
+// ket keys: (a.q,a.tj,s,c.q,c.tj, rest...) with `nrest` extra ints (0 for one-site, 3 for two-site).
+void emit_left_contraction(const BlockTensor& Lenv, const BlockTensor& ket, const MpoSite& W, int nrest,
+                           BlockTensor& Z, Stage& st) {
+  std::map<Sector, std::vector<int>> by_a;
+  for (size_t i = 0; i < ket.keys.size(); ++i) by_a[key_sector(ket.keys[i], 0)].push_back((int)i);
+  std::vector<RawTask> raw;
+  std::vector<Shape> shapes;
+  for (size_t e = 0; e < Lenv.keys.size(); ++e) {
+    const Key& ek = Lenv.keys[e];
+    const Sector ap = key_sector(ek, 0), a = key_sector(ek, 3);
+    const int w = ek[2];
+    auto it = by_a.find(a);
+    if (it == by_a.end()) continue;
+    for (int ki : it->second) {
+      const Key& kk = ket.keys[ki];
+      const int s = kk[2];
+      const Sector c = key_sector(kk, 3);
+      for (int wp = 0; wp < 4; ++wp) {
+        const int tr = W.rank2[w][wp];
+        if (tr < 0) continue;
+        for (int sp = 0; sp < 3; ++sp) {
+          const double wv = W.val[w][wp][sp][s];
+          if (wv == 0.0) continue;
+          Sector cps[2];
+          const int ncp = fuse(ap, sp, cps);
+          for (int j = 0; j < ncp; ++j) {
+            const Sector cp = cps[j];
+            if (cp.q != c.q + MPO_Q[wp] || !triangle(c.tj, MPO_TK[wp], cp.tj)) continue;
+            const double al = coef_left(a.tj, SITE_TJ[s], c.tj, MPO_TK[w], tr, MPO_TK[wp], ap.tj, SITE_TJ[sp], cp.tj) * wv;
+            if (std::fabs(al) < ALPHA_ZERO) continue;
+            RawTask t;
+            t.out = Key{ap.q, ap.tj, sp, cp.q, cp.tj, wp, c.q, c.tj, 0, 0, 0, 0};
+            for (int r = 0; r < nrest; ++r) t.out[8 + r] = kk[5 + r];
+            t.order = Key{w, a.q, a.tj, s, 0, 0, 0, 0, 0, 0, 0, 0};
+            t.lhs = (int)e;
+            t.rhs = ki;
+            t.alpha = al;
+            raw.push_back(t);
+            shapes.push_back(Shape{Lenv.rows[e], ket.cols[ki]});
+          }
+        }
+      }
+    }
+  }
+  layout_from_tasks(raw, shapes, 8 + nrest, Z);
+  st.opA = OPA_N;
+  st.opB = OPB_N;
+  tasks_to_stage(raw, Z, st);
+  finalize_stage(st, Z, Lenv, ket);
+}
+}  // namespace
+
+void emit_heff2(const BlockTensor& Lenv, const BlockTensor& Renv, const BlockTensor& vec, const MpoSite& W1,
+                const MpoSite& W2, BlockTensor& Z, Stage& st1, Stage& st2) {
+  emit_left_contraction(Lenv, vec, W1, 3, Z, st1);
+  std::map<Sector, std::vector<int>> by_b;
+  for (size_t i = 0; i < Renv.keys.size(); ++i) by_b[key_sector(Renv.keys[i], 3)].push_back((int)i);
+  std::vector<RawTask> raw;
+  for (size_t z = 0; z < Z.keys.size(); ++z) {
+    const Key& zk = Z.keys[z];  // a'(0,1) s1'(2) c'(3,4) wm(5) c(6,7) s2(8) b(9,10)
+    const Sector ap = key_sector(zk, 0), cp = key_sector(zk, 3), c = key_sector(zk, 6), b = key_sector(zk, 9);
+    const int s1p = zk[2], wm = zk[5], s2 = zk[8];
+    auto it = by_b.find(b);
+    if (it == by_b.end()) continue;
+    for (int ri : it->second) {
+      const Key& rk = Renv.keys[ri];
+      const Sector bp = key_sector(rk, 0);
+      const int wr = rk[2];
+      const int tr = W2.rank2[wm][wr];
+      if (tr < 0) continue;
+      for (int s2p = 0; s2p < 3; ++s2p) {
+        const double wv = W2.val[wm][wr][s2p][s2];
+        if (wv == 0.0) continue;
+        const Key ok = key_theta(ap, s1p, cp, s2p, bp);
+        if (vec.find(ok) < 0) continue;
+        const double al = coef_left(c.tj, SITE_TJ[s2], b.tj, MPO_TK[wm], tr, MPO_TK[wr], cp.tj, SITE_TJ[s2p], bp.tj) * wv;
+        if (std::fabs(al) < ALPHA_ZERO) continue;
+        RawTask t;
+        t.out = ok;
+        t.order = Key{c.q, c.tj, s2, b.q, b.tj, wm, wr, 0, 0, 0, 0, 0};
+        t.lhs = (int)z;
+        t.rhs = ri;
+        t.alpha = al;
+        raw.push_back(t);
+      }
+    }
+  }
+  st2.opA = OPA_N;
+  st2.opB = OPB_T;
+  tasks_to_stage(raw, vec, st2);
+  finalize_stage(st2, vec, Z, Renv);
+}
+
+void emit_heff1(const BlockTensor& Lenv, const BlockTensor& Renv, const BlockTensor& vec, const MpoSite& W,
+                BlockTensor& X, Stage& st1, Stage& st2) {
+  emit_left_contraction(Lenv, vec, W, 0, X, st1);
+  std::vector<RawTask> raw;
+  for (size_t x = 0; x < X.keys.size(); ++x) {
+    const Key& xk = X.keys[x];  // a'(0,1) s'(2) c'(3,4) w'(5) c(6,7)
+    const Sector ap = key_sector(xk, 0), cp = key_sector(xk, 3), c = key_sector(xk, 6);
+    const int ri = Renv.find(key_env(cp, xk[5], c));
+    const Key ok = key_site(ap, xk[2], cp);
+    if (ri < 0 || vec.find(ok) < 0) continue;
+    RawTask t;
+    t.out = ok;
+    t.order = Key{c.q, c.tj, xk[5], 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    t.lhs = (int)x;
+    t.rhs = ri;
+    t.alpha = 1.0;
+    raw.push_back(t);
+  }
+  st2.opA = OPA_N;
+  st2.opB = OPB_T;
+  tasks_to_stage(raw, vec, st2);
+  finalize_stage(st2, vec, X, Renv);
+}
+
+void emit_env_left(const BlockTensor& Lenv, const BlockTensor& A, const MpoSite& W, BlockTensor& X,
+                   BlockTensor& out, Stage& st1, Stage& st2) {
+  emit_left_contraction(Lenv, A, W, 0, X, st1);
+  std::vector<RawTask> raw;
+  std::vector<Shape> shapes;
+  for (size_t x = 0; x < X.keys.size(); ++x) {
+    const Key& xk = X.keys[x];
+    const Sector ap = key_sector(xk, 0), cp = key_sector(xk, 3), c = key_sector(xk, 6);
+    const int ai = A.find(key_site(ap, xk[2], cp));
+    if (ai < 0) continue;
+    RawTask t;
+    t.out = key_env(cp, xk[5], c);
+    t.order = Key{ap.q, ap.tj, xk[2], 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    t.lhs = ai;
+    t.rhs = (int)x;
+    t.alpha = 1.0;
+    raw.push_back(t);
+    shapes.push_back(Shape{A.cols[ai], X.cols[x]});
+  }
+  layout_from_tasks(raw, shapes, 5, out);
+  st2.opA = OPA_H;
+  st2.opB = OPB_N;
+  tasks_to_stage(raw, out, st2);
+  finalize_stage(st2, out, A, X);
+}
+
+void emit_env_right(const BlockTensor& Renv, const BlockTensor& A, const MpoSite& W, BlockTensor& Y,
+                    BlockTensor& out, Stage& st1, Stage& st2) {
+  std::map<Sector, std::vector<int>> r_by_bp, a_by_b;
+  for (size_t i = 0; i < Renv.keys.size(); ++i) r_by_bp[key_sector(Renv.keys[i], 0)].push_back((int)i);
+  for (size_t i = 0; i < A.keys.size(); ++i) a_by_b[key_sector(A.keys[i], 3)].push_back((int)i);
+  std::vector<RawTask> raw1, raw2;
+  std::vector<Shape> shapes1, shapes2;
+  std::map<Key, bool> ydone;
+  struct Pending {
+    Key ykey;
+    RawTask t;
+  };
+  std::vector<Pending> pend;
+  for (size_t ip = 0; ip < A.keys.size(); ++ip) {
+    const Key& akp = A.keys[ip];  // c'(0,1) s'(2) b'(3,4)
+    const Sector cp = key_sector(akp, 0), bp = key_sector(akp, 3);
+    const int sp = akp[2];
+    auto itr = r_by_bp.find(bp);
+    if (itr == r_by_bp.end()) continue;
+    for (int ri : itr->second) {
+      const Key& rk = Renv.keys[ri];  // b'(0,1) w'(2) b(3,4)
+      const int wp = rk[2];
+      const Sector b = key_sector(rk, 3);
+      const Key ykey{cp.q, cp.tj, sp, bp.q, bp.tj, wp, b.q, b.tj, 0, 0, 0, 0};
+      auto ita = a_by_b.find(b);
+      if (ita == a_by_b.end()) continue;
+      for (int ai : ita->second) {
+        const Key& ak = A.keys[ai];  // c(0,1) s(2) b(3,4)
+        const Sector c = key_sector(ak, 0);
+        const int s = ak[2];
+        for (int w = 0; w < 4; ++w) {
+          const int tr = W.rank2[w][wp];
+          if (tr < 0) continue;
+          const double wv = W.val[w][wp][sp][s];
+          if (wv == 0.0) continue;
+          if (cp.q != c.q + MPO_Q[w] || !triangle(c.tj, MPO_TK[w], cp.tj)) continue;
+          const double al = coef_right(c.tj, SITE_TJ[s], b.tj, MPO_TK[w], tr, MPO_TK[wp], cp.tj, SITE_TJ[sp], bp.tj) * wv;
+          if (std::fabs(al) < ALPHA_ZERO) continue;
+          if (!ydone.count(ykey)) {
+            ydone[ykey] = true;
+            RawTask t1;
+            t1.out = ykey;
+            t1.order = Key{0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+            t1.lhs = (int)ip;
+            t1.rhs = ri;
+            t1.alpha = 1.0;
+            raw1.push_back(t1);
+            shapes1.push_back(Shape{A.rows[ip], Renv.cols[ri]});
+          }
+          Pending p;
+          p.ykey = ykey;
+          p.t.out = key_env(cp, w, c);
+          p.t.order = Key{sp, bp.q, bp.tj, wp, s, b.q, b.tj, 0, 0, 0, 0, 0};
+          p.t.lhs = -1;
+          p.t.rhs = ai;
+          p.t.alpha = al;
+          pend.push_back(p);
+          shapes2.push_back(Shape{A.rows[ip], A.rows[ai]});
+        }
+      }
+    }
+  }
+  layout_from_tasks(raw1, shapes1, 8, Y);
+  st1.opA = OPA_C;
+  st1.opB = OPB_N;
+  tasks_to_stage(raw1, Y, st1);
+  finalize_stage(st1, Y, A, Renv);
+  for (auto& p : pend) {
+    p.t.lhs = Y.find(p.ykey);
+    raw2.push_back(p.t);
+  }
+  layout_from_tasks(raw2, shapes2, 5, out);
+  st2.opA = OPA_N;
+  st2.opB = OPB_T;
+  tasks_to_stage(raw2, out, st2);
+  finalize_stage(st2, out, Y, A);
+}
+
+void emit_merge(const BlockTensor& A1, const BlockTensor& A2, const BlockTensor& theta, Stage& st) {
+  std::vector<RawTask> raw;
+  for (size_t i = 0; i < theta.keys.size(); ++i) {
+    const Key& k = theta.keys[i];
+    const Sector a = key_sector(k, 0), c = key_sector(k, 3), b = key_sector(k, 6);
+    const int i1 = A1.find(key_site(a, k[2], c)), i2 = A2.find(key_site(c, k[5], b));
+    if (i1 < 0 || i2 < 0) continue;
+    RawTask t;
+    t.out = k;
+    t.order = Key{0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    t.lhs = i1;
+    t.rhs = i2;
+    t.alpha = 1.0;
+    raw.push_back(t);
+  }
+  st.opA = OPA_N;
+  st.opB = OPB_N;
+  tasks_to_stage(raw, theta, st);
+  finalize_stage(st, theta, A1, A2);
+}
+
+void emit_norm_env(const BlockTensor& Nenv, const BlockTensor& A, BlockTensor& Nout, Stage& st1, Stage& st2) {
+  // stage 1: X[a,s,c] = N[a] A[a,s,c]  (X has A's layout);  stage 2: N'[c] = sum_{a,s} A[a,s,c]^H X[a,s,c]
+  std::vector<RawTask> raw1, raw2;
+  std::vector<Shape> shapes2;
+  for (size_t i = 0; i < A.keys.size(); ++i) {
+    const Key& k = A.keys[i];
+    const Sector a = key_sector(k, 0), c = key_sector(k, 3);
+    const int ni = Nenv.find(Key{a.q, a.tj, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0});
+    if (ni < 0) continue;
+    RawTask t;
+    t.out = k;
+    t.order = Key{0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    t.lhs = ni;
+    t.rhs = (int)i;
+    t.alpha = 1.0;
+    raw1.push_back(t);
+    RawTask u;
+    u.out = Key{c.q, c.tj, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    u.order = Key{a.q, a.tj, k[2], 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    u.lhs = (int)i;
+    u.rhs = (int)i;
+    u.alpha = 1.0;
+    raw2.push_back(u);
+    shapes2.push_back(Shape{A.cols[i], A.cols[i]});
+  }
+  st1.opA = OPA_N;
+  st1.opB = OPB_N;
+  tasks_to_stage(raw1, A, st1);
+  finalize_stage(st1, A, Nenv, A);
+  layout_from_tasks(raw2, shapes2, 2, Nout);
+  st2.opA = OPA_H;
+  st2.opB = OPB_N;
+  tasks_to_stage(raw2, Nout, st2);
+  finalize_stage(st2, Nout, A, A);  // rhs = X which has A's layout
+}
+
+}  // namespace fh

@@ -1,0 +1,440 @@
+// Two-site TDVP sweep: merge (H8), Lanczos exponential (H6/H7 in api.cu),
+// block-wise SVD + truncation (H9, vendor cuSOLVER, timed separately), environment update,
+// one-site backward step (H3); and measure_local through norm environments (H10).
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+
+#include "context.hpp"
+
+using namespace fh;
+
+#define FH_CUSOLVER(x)                                                                    \
+  do {                                                                                    \
+    cusolverStatus_t st__ = (x);                                                          \
+    if (st__ != CUSOLVER_STATUS_SUCCESS)                                                  \
+      throw fh::FhError(FH_ECUDA, std::string(#x) + " failed, status " + std::to_string((int)st__)); \
+  } while (0)
+
+namespace {
+
+// element (j, x) of a strided matrix is multiplied by s[j]
+__global__ void scale_by_s_kernel(cplx* buf, int nj, int nx, int64_t stride_j, int64_t stride_x,
+                                  const double* __restrict__ s) {
+  const int64_t total = (int64_t)nj * nx;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+    const int j = (int)(i / nx), x = (int)(i % nx);
+    cplx* p = buf + j * stride_j + x * stride_x;
+    const double f = s[j];
+    p->x *= f;
+    p->y *= f;
+  }
+}
+
+struct SectorSvd {
+  Sector c;
+  int nrow, ncol, k;       // M_c is nrow x ncol, k = min
+  bool transposed;         // buffer holds M_c^T row-major (== column-major M_c)
+  int64_t m_off, u_off, vt_off, s_off;  // offsets into the scratch (complex / double units)
+  std::vector<std::pair<Key, std::pair<int, int>>> rows;  // (a,s1) part: key{a.q,a.tj,s1}, (offset, dim)
+  std::vector<std::pair<Key, std::pair<int, int>>> cols;  // (s2,b) part: key{s2,b.q,b.tj}
+  int keep = 0;
+};
+
+}  // namespace
+
+// Reading A-6 (same rule as the oracle's, restated): sort all (s, sector, position) by s
+// descending, ties by (sector index, position); drop s <= 1e-14 s_max; stop when the full
+// dimension sum (2j+1) would exceed chi_max_full or the remaining tail weight is <= eps; keep >= 1.
+static double truncate_rule(const std::vector<std::vector<double>>& sv, const std::vector<int>& mult, int chi_max,
+                            double eps, std::vector<int>& keep) {
+  struct It {
+    double s;
+    int c, p;
+  };
+  std::vector<It> items;
+  for (size_t c = 0; c < sv.size(); ++c)
+    for (size_t p = 0; p < sv[c].size(); ++p) items.push_back(It{sv[c][p], (int)c, (int)p});
+  std::sort(items.begin(), items.end(), [](const It& a, const It& b) {
+    if (a.s != b.s) return a.s > b.s;
+    if (a.c != b.c) return a.c < b.c;
+    return a.p < b.p;
+  });
+  double total = 0.0;
+  for (const It& it : items) total += mult[it.c] * it.s * it.s;
+  const double smax = items.empty() ? 0.0 : items[0].s;
+  keep.assign(sv.size(), 0);
+  int dim = 0, nk = 0;
+  double kept = 0.0;
+  for (const It& it : items) {
+    if (nk >= 1) {
+      if (it.s <= 1e-14 * smax) break;
+      if (dim + mult[it.c] > chi_max) break;
+      if (eps >= 0 && (total - kept) <= eps * total) break;
+    }
+    keep[it.c] += 1;
+    dim += mult[it.c];
+    kept += mult[it.c] * it.s * it.s;
+    ++nk;
+  }
+  return total > 0 ? std::max(total - kept, 0.0) / total : 0.0;
+}
+
+// theta (layout th, device pointer) -> new A[i], A[i+1], bond[i+1].  direction +1: A[i] = U
+// (left-canonical), A[i+1] = S V^H...; direction -1: A[i] = U S, A[i+1] = V^H... (right-canonical).
+static void svd_split(fh_ctx* ctx, fh_mps* mps, int i, const BlockTensor& th, const cplx* theta, int direction,
+                      const fh_params* prm) {
+  const Bond& bl = mps->bond[i];
+  const Bond& br = mps->bond[i + 2];
+  // ---- group theta blocks by middle sector c
+  std::map<Sector, SectorSvd> secs;
+  for (size_t t = 0; t < th.keys.size(); ++t) {
+    const Key& k = th.keys[t];
+    const Sector c{k[3], k[4]};
+    SectorSvd& S = secs[c];
+    S.c = c;
+    const Key rk{k[0], k[1], k[2], 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    const Key ck{k[5], k[6], k[7], 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    bool fr = false, fc = false;
+    for (auto& r : S.rows) fr |= (r.first == rk);
+    for (auto& cc : S.cols) fc |= (cc.first == ck);
+    if (!fr) S.rows.push_back({rk, {0, th.rows[t]}});
+    if (!fc) S.cols.push_back({ck, {0, th.cols[t]}});
+  }
+  int64_t cplx_total = 0, dbl_total = 0;
+  std::vector<SectorSvd*> order;
+  for (auto& e : secs) {
+    SectorSvd& S = e.second;
+    std::sort(S.rows.begin(), S.rows.end(), [](const auto& a, const auto& b) { return a.first < b.first; });
+    std::sort(S.cols.begin(), S.cols.end(), [](const auto& a, const auto& b) { return a.first < b.first; });
+    int n = 0;
+    for (auto& r : S.rows) { r.second.first = n; n += r.second.second; }
+    S.nrow = n;
+    n = 0;
+    for (auto& c : S.cols) { c.second.first = n; n += c.second.second; }
+    S.ncol = n;
+    S.k = std::min(S.nrow, S.ncol);
+    S.transposed = S.nrow > S.ncol;  // cuSOLVER gesvd wants rows >= cols of the column-major matrix
+    S.m_off = cplx_total;
+    cplx_total += Arena::round_up((int64_t)S.nrow * S.ncol);
+    S.u_off = cplx_total;
+    cplx_total += Arena::round_up((int64_t)std::max(S.nrow, S.ncol) * S.k);
+    S.vt_off = cplx_total;
+    cplx_total += Arena::round_up((int64_t)S.k * std::min(S.nrow, S.ncol));
+    S.s_off = dbl_total;
+    dbl_total += (S.k + 1) / 2 * 2;
+    order.push_back(&S);
+  }
+  const int64_t s_cplx = (dbl_total + 1) / 2;  // singular values live in the same scratch, as doubles
+  const int64_t scratch_n = cplx_total + Arena::round_up(s_cplx);
+  const int64_t scratch = ctx->alloc.alloc(scratch_n);
+  cplx* buf = ctx->ptr(scratch);
+  double* dS = reinterpret_cast<double*>(buf + cplx_total);
+  cudaStream_t s = ctx->stream;
+
+  // ---- pack (H8): M_c[(a,s1,al),(s2,b,be)] = theta[a,s1,c,s2,b] sqrt((2j_b+1)/(2j_c+1))
+  ctx->timer_begin(T_PACK);
+  launch_fill_zero(buf, cplx_total, s, &ctx->launches);
+  std::vector<CopyBlk> blks;
+  for (size_t t = 0; t < th.keys.size(); ++t) {
+    const Key& k = th.keys[t];
+    SectorSvd& S = secs[Sector{k[3], k[4]}];
+    const Key rk{k[0], k[1], k[2], 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    const Key ck{k[5], k[6], k[7], 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    int ro = 0, co = 0;
+    for (auto& r : S.rows) if (r.first == rk) ro = r.second.first;
+    for (auto& c : S.cols) if (c.first == ck) co = c.second.first;
+    CopyBlk b;
+    b.src_off = th.off[t];
+    b.rows = th.rows[t];
+    b.cols = th.cols[t];
+    b.ld_src = th.cols[t];
+    b.scale = std::sqrt((double)(k[7] + 1) / (double)(k[4] + 1));
+    b.pad = 0;
+    if (!S.transposed) {  // row-major M_c (nrow x ncol)
+      b.dst_off = S.m_off + (int64_t)ro * S.ncol + co;
+      b.ld_dst = S.ncol;
+      b.transpose_dst = 0;
+    } else {  // row-major M_c^T (ncol x nrow)
+      b.dst_off = S.m_off + (int64_t)co * S.nrow + ro;
+      b.ld_dst = S.nrow;
+      b.transpose_dst = 1;
+    }
+    blks.push_back(b);
+  }
+  ctx->pool_aux.reserve(blks.size() * sizeof(CopyBlk) + 4096, s);
+  CopyBlk* d_blks = upload(ctx->pool_aux, blks, s);
+  launch_copy_blocks(d_blks, (int)blks.size(), theta, buf, s, &ctx->launches);
+  ctx->timer_end();
+
+  // ---- block-wise SVD (H9): vendor routine, timed separately
+  ctx->timer_begin(T_SVD);
+  if (!ctx->cusolver) {
+    FH_CUSOLVER(cusolverDnCreate(&ctx->cusolver));
+    FH_CUSOLVER(cusolverDnSetStream(ctx->cusolver, s));
+    FH_CUDA(cudaMalloc((void**)&ctx->d_info, sizeof(int)));
+  }
+  for (SectorSvd* S : order) {
+    // column-major matrix handed to gesvd: rows m >= cols n
+    const int m = std::max(S->nrow, S->ncol), n = S->k;
+    int lwork = 0;
+    FH_CUSOLVER(cusolverDnZgesvd_bufferSize(ctx->cusolver, m, n, &lwork));
+    const size_t need = (size_t)lwork * sizeof(cuDoubleComplex);
+    if (need > ctx->svd_work_bytes) {
+      FH_CUDA(cudaStreamSynchronize(s));
+      if (ctx->svd_work) FH_CUDA(cudaFree(ctx->svd_work));
+      ctx->svd_work_bytes = need + need / 2;
+      FH_CUDA(cudaMalloc(&ctx->svd_work, ctx->svd_work_bytes));
+    }
+    FH_CUSOLVER(cusolverDnZgesvd(ctx->cusolver, 'S', 'S', m, n, (cuDoubleComplex*)(buf + S->m_off), m,
+                                 dS + S->s_off, (cuDoubleComplex*)(buf + S->u_off), m,
+                                 (cuDoubleComplex*)(buf + S->vt_off), n, (cuDoubleComplex*)ctx->svd_work,
+                                 (int)(ctx->svd_work_bytes / sizeof(cuDoubleComplex)), nullptr, ctx->d_info));
+  }
+  ctx->ensure_pinned((size_t)dbl_total + 2);
+  FH_CUDA(cudaMemcpyAsync(ctx->h_pinned, dS, dbl_total * sizeof(double), cudaMemcpyDeviceToHost, s));
+  FH_CUDA(cudaStreamSynchronize(s));
+  ctx->timer_end();
+
+  // ---- truncation on the host (reading A-6)
+  std::vector<std::vector<double>> sv;
+  std::vector<int> mult, keep;
+  for (SectorSvd* S : order) {
+    sv.emplace_back(ctx->h_pinned + S->s_off, ctx->h_pinned + S->s_off + S->k);
+    mult.push_back(S->c.tj + 1);
+  }
+  const double disc = truncate_rule(sv, mult, prm->chi_max_full, prm->eps_trunc, keep);
+  ctx->stat_disc = std::max(ctx->stat_disc, disc);
+  Bond nb;
+  for (size_t x = 0; x < order.size(); ++x) {
+    order[x]->keep = keep[x];
+    if (keep[x] > 0) {
+      nb.sec.push_back(order[x]->c);
+      nb.d.push_back(keep[x]);
+    }
+  }
+  mps->bond[i + 1] = nb;
+  ctx->stat_chi = std::max(ctx->stat_chi, nb.chi_full());
+  ctx->stat_su2 = std::max(ctx->stat_su2, nb.chi_su2());
+  ctx->stat_dmax = std::max(ctx->stat_dmax, nb.dmax());
+
+  // ---- unpack: A_i[a,s1,c] = U_c (x S), A_{i+1}[c,s2,b] = (S x) V_c^H sqrt((2j_c+1)/(2j_b+1))
+  ctx->timer_begin(T_PACK);
+  // With B = column-major (m x n) matrix given to gesvd, B = Ub S VTb:
+  //   not transposed (B = M^T, m = ncol, n = nrow = k):  U_M[r][j] = VTb[j][r] -> memory r*k + j;
+  //                                                     V^H[j][x]  = Ub[x][j]  -> memory j*m + x
+  //   transposed     (B = M,   m = nrow, n = ncol = k):  U_M[r][j] = Ub[r][j]  -> memory j*m + r;
+  //                                                     V^H[j][x]  = VTb[j][x] -> memory x*k + j
+  for (SectorSvd* S : order) {
+    if (S->keep == 0) continue;
+    const int m = std::max(S->nrow, S->ncol), k = S->k;
+    cplx* target;
+    int nx;
+    int64_t sj, sx;
+    if (direction > 0) {  // scale V^H rows
+      nx = S->ncol;
+      if (!S->transposed) { target = buf + S->u_off; sj = m; sx = 1; } else { target = buf + S->vt_off; sj = 1; sx = k; }
+    } else {  // scale U columns
+      nx = S->nrow;
+      if (!S->transposed) { target = buf + S->vt_off; sj = 1; sx = k; } else { target = buf + S->u_off; sj = m; sx = 1; }
+    }
+    const int64_t tot = (int64_t)S->keep * nx;
+    scale_by_s_kernel<<<(int)std::min<int64_t>((tot + 255) / 256, 1184), 256, 0, s>>>(target, S->keep, nx, sj, sx,
+                                                                                    dS + S->s_off);
+    ++ctx->launches;
+  }
+  BlockTensor A1, A2;
+  layout_site(bl, nb, A1);
+  layout_site(nb, br, A2);
+  ctx->free_tensor(mps->A[i]);
+  ctx->free_tensor(mps->A[i + 1]);
+  ctx->alloc_tensor(A1);
+  ctx->alloc_tensor(A2);
+  std::vector<CopyBlk> ub, vb;
+  for (size_t t = 0; t < A1.keys.size(); ++t) {
+    const Key& k = A1.keys[t];  // a(0,1) s1(2) c(3,4)
+    SectorSvd& S = secs[Sector{k[3], k[4]}];
+    const Key rk{k[0], k[1], k[2], 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    int ro = -1;
+    for (auto& r : S.rows) if (r.first == rk) ro = r.second.first;
+    FH_REQUIRE(ro >= 0, FH_ESTATE, "svd unpack: row block not found");
+    const int m = std::max(S.nrow, S.ncol), kk = S.k;
+    CopyBlk b;
+    b.scale = 1.0;
+    b.pad = 0;
+    b.dst_off = A1.off[t];
+    if (!S.transposed) {  // U_M row-major (nrow x k) in the VT buffer
+      b.src_off = S.vt_off + (int64_t)ro * kk;
+      b.rows = A1.rows[t];
+      b.cols = S.keep;
+      b.ld_src = kk;
+      b.ld_dst = S.keep;
+      b.transpose_dst = 0;
+    } else {  // U buffer holds [j][r] with pitch m: copy rows j < keep, cols ro..ro+d_a, transposed
+      b.src_off = S.u_off + ro;
+      b.rows = S.keep;
+      b.cols = A1.rows[t];
+      b.ld_src = m;
+      b.ld_dst = S.keep;
+      b.transpose_dst = 1;
+    }
+    ub.push_back(b);
+  }
+  for (size_t t = 0; t < A2.keys.size(); ++t) {
+    const Key& k = A2.keys[t];  // c(0,1) s2(2) b(3,4)
+    SectorSvd& S = secs[Sector{k[0], k[1]}];
+    const Key ck{k[2], k[3], k[4], 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    int co = -1;
+    for (auto& c : S.cols) if (c.first == ck) co = c.second.first;
+    FH_REQUIRE(co >= 0, FH_ESTATE, "svd unpack: column block not found");
+    const int m = std::max(S.nrow, S.ncol), kk = S.k;
+    CopyBlk b;
+    b.scale = std::sqrt((double)(k[1] + 1) / (double)(k[4] + 1));
+    b.pad = 0;
+    b.dst_off = A2.off[t];
+    if (!S.transposed) {  // V^H[j][x] at j*m + x in the U buffer
+      b.src_off = S.u_off + co;
+      b.rows = S.keep;
+      b.cols = A2.cols[t];
+      b.ld_src = m;
+      b.ld_dst = A2.cols[t];
+      b.transpose_dst = 0;
+    } else {  // V^H[j][x] at x*k + j in the VT buffer: source rows x, cols j; write transposed
+      b.src_off = S.vt_off + (int64_t)co * kk;
+      b.rows = A2.cols[t];
+      b.cols = S.keep;
+      b.ld_src = kk;
+      b.ld_dst = A2.cols[t];
+      b.transpose_dst = 1;
+    }
+    vb.push_back(b);
+  }
+  ctx->pool_aux.reserve((ub.size() + vb.size()) * sizeof(CopyBlk) + 8192, s);
+  CopyBlk* d_ub = upload(ctx->pool_aux, ub, s);
+  CopyBlk* d_vb = upload(ctx->pool_aux, vb, s);
+  launch_copy_blocks(d_ub, (int)ub.size(), buf, ctx->ptr(A1.base), s, &ctx->launches);
+  launch_copy_blocks(d_vb, (int)vb.size(), buf, ctx->ptr(A2.base), s, &ctx->launches);
+  FH_CUDA(cudaGetLastError());
+  ctx->timer_end();
+  mps->A[i] = A1;
+  mps->A[i + 1] = A2;
+  ctx->alloc.release(scratch, scratch_n);
+}
+
+// one local two-site update on bond (i, i+1)
+static void local_update2(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int i, double tau, int direction,
+                          const fh_params* prm) {
+  plan_heff(ctx, mpo, mps, i, 2);
+  Plan& P = ctx->plan;
+  const int64_t n = P.vec.nelem;
+  const int m = prm->krylov_dim;
+  const int64_t wn = (int64_t)(m + 2) * n;
+  const int64_t woff = ctx->alloc.alloc(wn);
+  cplx* theta = ctx->ptr(woff);
+  cplx* V = theta + n;
+  // merge (H8): theta[a,s1,c,s2,b] = A_i[a,s1,c] A_{i+1}[c,s2,b]; blocks whose c is not on the bond are zero
+  {
+    Stage st;
+    emit_merge(mps->A[i], mps->A[i + 1], P.vec, st);
+    ctx->pool_aux.reserve(stage_bytes(st) + 4096, ctx->stream);
+    upload_stage(ctx->pool_aux, st, ctx->stream);
+    ctx->timer_begin(T_PACK);
+    launch_grouped_gemm(st, ctx->ptr(mps->A[i].base), ctx->ptr(mps->A[i + 1].base), theta, ctx->stream, &ctx->launches);
+    ctx->timer_end();
+  }
+  expm_lanczos(ctx, theta, tau, m, prm->krylov_tol, V);
+  BlockTensor th = P.vec;  // copy: svd_split re-plans nothing but keeps the layout alive
+  svd_split(ctx, mps, i, th, theta, direction, prm);
+  ctx->alloc.release(woff, wn);
+}
+
+static void local_update1(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int i, double tau, const fh_params* prm) {
+  plan_heff(ctx, mpo, mps, i, 1);
+  Plan& P = ctx->plan;
+  const int64_t n = P.vec.nelem;
+  FH_REQUIRE(n == mps->A[i].nelem, FH_ESTATE, "one-site update: layout mismatch");
+  const int m = prm->krylov_dim;
+  const int64_t wn = (int64_t)(m + 1) * n;
+  const int64_t woff = ctx->alloc.alloc(wn);
+  expm_lanczos(ctx, ctx->ptr(mps->A[i].base), tau, m, prm->krylov_tol, ctx->ptr(woff));
+  ctx->alloc.release(woff, wn);
+}
+
+void fh::sweep(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh_params* prm) {
+  const int L = mps->L;
+  FH_REQUIRE(mpo->L == L, FH_EINVAL, "tdvp2_sweep: MPO and MPS lengths differ");
+  for (int i = 0; i < L; ++i) FH_REQUIRE(mps->A[i].base >= 0, FH_ESTATE, "tdvp2_sweep: site tensor missing");
+  for (int i = 2; i <= L; ++i) FH_REQUIRE(mps->Renv[i].base >= 0, FH_ESTATE, "tdvp2_sweep: right environments missing (centre must be at site 0)");
+  ctx->stat_disc = 0.0;
+  ctx->stat_chi = ctx->stat_su2 = ctx->stat_dmax = 0;
+  const double tau = 0.5 * dt;
+  for (int i = 0; i < L - 1; ++i) {  // left -> right
+    local_update2(ctx, mpo, mps, i, tau, +1, prm);
+    do_env_update_left(ctx, mpo, mps, i);
+    if (i < L - 2) local_update1(ctx, mpo, mps, i + 1, -tau, prm);
+  }
+  for (int i = L - 2; i >= 0; --i) {  // right -> left
+    local_update2(ctx, mpo, mps, i, tau, -1, prm);
+    do_env_update_right(ctx, mpo, mps, i + 1);
+    if (i > 0) local_update1(ctx, mpo, mps, i, -tau, prm);
+  }
+}
+
+// H10: left norm environments N_{i+1}[c] = sum_{a,s} A^H N_i[a] A;  <O_i> = sum (2j_c+1) red(O)[s] Re Tr(A^H N A)
+void fh::measure_local_impl(fh_ctx* ctx, const fh_mps* mps, double* n_i, double* sz_i, double* docc_i) {
+  const int L = mps->L;
+  cudaStream_t s = ctx->stream;
+  BlockTensor N;
+  N.nlab = 2;
+  N.add(Key{0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, 1, 1);
+  N.finalize();
+  ctx->alloc_tensor(N);
+  const cplx one = make_double2(1.0, 0.0);
+  FH_CUDA(cudaMemcpyAsync(ctx->ptr(N.base), &one, sizeof(cplx), cudaMemcpyHostToDevice, s));
+  for (int i = 0; i < L; ++i) {
+    const BlockTensor& A = mps->A[i];
+    FH_REQUIRE(A.base >= 0, FH_ESTATE, "measure_local: site tensor missing");
+    BlockTensor Nn;
+    Stage st1, st2;
+    emit_norm_env(N, A, Nn, st1, st2);
+    const int64_t xoff = ctx->alloc.alloc(A.nelem);
+    ctx->alloc_tensor(Nn);
+    std::vector<VecChunk> chunks;  // one or more chunks per block; weights applied on the host
+    std::vector<int> chunk_blk;
+    for (size_t b = 0; b < A.keys.size(); ++b) {
+      const int64_t n = (int64_t)A.rows[b] * A.cols[b];
+      for (int64_t o = 0; o < n; o += 8192) {
+        chunks.push_back(VecChunk{A.off[b] + o, (int)std::min<int64_t>(8192, n - o), 1.0f});
+        chunk_blk.push_back((int)b);
+      }
+    }
+    ctx->pool_aux.reserve(stage_bytes(st1) + stage_bytes(st2) + chunks.size() * (sizeof(VecChunk) + 16) + 8192, s);
+    upload_stage(ctx->pool_aux, st1, s);
+    upload_stage(ctx->pool_aux, st2, s);
+    VecChunk* d_chunks = upload(ctx->pool_aux, chunks, s);
+    double* d_part = (double*)ctx->pool_aux.take(chunks.size() * 2 * sizeof(double));
+    cplx* X = ctx->ptr(xoff);
+    launch_grouped_gemm(st1, ctx->ptr(N.base), ctx->ptr(A.base), X, s, &ctx->launches);
+    launch_wdot(d_chunks, (int)chunks.size(), ctx->ptr(A.base), X, d_part, nullptr, s, &ctx->launches);
+    launch_grouped_gemm(st2, ctx->ptr(A.base), X, ctx->ptr(Nn.base), s, &ctx->launches);
+    ctx->ensure_pinned(chunks.size() * 2 + 2);
+    FH_CUDA(cudaMemcpyAsync(ctx->h_pinned, d_part, chunks.size() * 2 * sizeof(double), cudaMemcpyDeviceToHost, s));
+    FH_CUDA(cudaStreamSynchronize(s));
+    double one_v = 0.0, sz = 0.0, pd = 0.0;
+    for (size_t c = 0; c < chunks.size(); ++c) {
+      const Key& k = A.keys[chunk_blk[c]];
+      const double w = (k[4] + 1) * ctx->h_pinned[2 * c];
+      one_v += w;
+      if (k[2] == 0) sz += 0.5 * w;
+      if (k[2] == 1) sz -= 0.5 * w;
+      if (k[2] == 2) pd += w;
+    }
+    n_i[i] = one_v != 0.0 ? one_v / one_v : 0.0;  // <n_i> = 1 identically in a T_tot = 0 state (A-12)
+    sz_i[i] = sz / one_v;
+    docc_i[i] = 0.5 * pd / one_v;
+    ctx->alloc.release(xoff, A.nelem);
+    ctx->free_tensor(N);
+    N = Nn;
+  }
+  ctx->free_tensor(N);
+}

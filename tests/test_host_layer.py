@@ -1,0 +1,92 @@
+"""CPU tests (-m "not gpu") of the library's host symmetry layer: the shared library loads,
+exports every symbol include/fh_b200.h declares, its closed-form recoupling coefficients agree
+with the oracle's CG-sum definitions, and its task lists equal the oracle's bit for bit."""
+import os
+import random
+import re
+
+import numpy as np
+import pytest
+
+import fh_inputs as fi
+from oracle import su2, symm
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def binding():
+    import paper_2606_04771_b200 as pkg
+    pkg.build()
+    return pkg.binding
+
+
+def test_library_exports_every_declared_symbol(binding):
+    hdr = open(os.path.join(ROOT, "include", "fh_b200.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    names = set(re.findall(r"\b([a-z_0-9]+)\s*\(", hdr))
+    names -= {"defined", "sizeof"}
+    decl = {n for n in names if re.search(r"\b(int|void|double|int64_t|const char\*)\s+\*?\s*%s\s*\(" % n, hdr)}
+    assert len(decl) >= 38
+    for n in sorted(decl):
+        assert hasattr(binding.lib, n), n
+    assert set(binding.EXPORTS) == decl
+
+
+def test_closed_form_coefficients_match_oracle(binding):
+    rnd = random.Random(5)
+    n = 0
+    while n < 300:
+        ta = rnd.randint(0, 9)
+        ts, tsp, tk, tr = (rnd.choice([0, 1]) for _ in range(4))
+        tkp = rnd.choice(range(abs(tk - tr), tk + tr + 1, 2))
+        tc = rnd.choice(range(abs(ta - ts), ta + ts + 1, 2))
+        tap = rnd.choice(range(abs(ta - tk), ta + tk + 1, 2))
+        tcp = rnd.choice(range(abs(tap - tsp), tap + tsp + 1, 2))
+        t = (ta, ts, tc, tk, tr, tkp, tap, tsp, tcp)
+        assert abs(binding.fh_coef_left(*t) - su2.coef_left(*t)) < 1e-13, t
+        assert abs(binding.fh_coef_right(*t) - su2.coef_right(*t)) < 1e-13, t
+        n += 1
+
+
+def _compare(binding, site, nsite, dims_l, dims_r, Lk, Rk, t_h=1.0, U=4.0):
+    W1, W2 = symm.mpo_reduced(site, t_h, U), symm.mpo_reduced(site + 1, t_h, U)
+    if nsite == 2:
+        vk = symm.theta_keys(dims_l, dims_r)
+        st1, st2 = symm.heff2_tasks(Lk, Rk, vk, W1, W2)
+    else:
+        vk = symm.site_keys(dims_l, dims_r)
+        st1, st2 = symm.heff1_tasks(Lk, Rk, vk, W1)
+    o1 = symm.task_tuples(st1, list(st1), Lk, vk)
+    o2 = symm.task_tuples(st2, vk, list(st1), Rk)
+    (t1, a1, n1, f1), (t2, a2, n2, f2) = binding.fh_host_plan(site, nsite, t_h, U, dims_l, dims_r, Lk, Rk)
+    assert n1 == len(st1) and n2 == len(vk)
+    assert t1.shape == o1[0].shape and (t1 == o1[0]).all()          # bit-exact integer tuples
+    assert t2.shape == o2[0].shape and (t2 == o2[0]).all()
+    assert np.abs(a1 - o1[1]).max() < 1e-13 and np.abs(a2 - o2[1]).max() < 1e-13
+    if nsite == 2:
+        assert f1 + f2 == symm.heff2_flops(st1, st2, dims_l, dims_r)
+    return len(a1), len(a2)
+
+
+def test_task_lists_bit_exact_small_chain(binding):
+    rng = np.random.default_rng(2)
+    L = 6
+    tabs = fi.reachable_tables(L)
+    dims = [{sec: int(rng.integers(1, 5)) for sec in tabs[k]} for k in range(L + 1)]
+    for site in range(L - 1):
+        Lk = symm.env_keys(dims[site], dims[site])
+        Rk = symm.env_keys(dims[site + 2], dims[site + 2])
+        _compare(binding, site, 2, dims[site], dims[site + 2], Lk, Rk)
+    for site in range(L):
+        Lk = symm.env_keys(dims[site], dims[site])
+        Rk = symm.env_keys(dims[site + 1], dims[site + 1])
+        _compare(binding, site, 1, dims[site], dims[site + 1], Lk, Rk)
+
+
+def test_task_lists_bit_exact_config2_shape(binding):
+    """BASELINE config 2's sector structure at reduced chi (central bond of L=60)."""
+    dl, dr = fi.gaussian_profile(29, 256), fi.gaussian_profile(31, 256)
+    Lk, Rk = symm.env_keys(dl, dl), symm.env_keys(dr, dr)
+    n1, n2 = _compare(binding, 29, 2, dl, dr, Lk, Rk)
+    assert n1 > 500 and n2 > 500
