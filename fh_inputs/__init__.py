@@ -21,3 +21,5 @@ Recipes (BASELINE.json configs 2-5):
 from .profiles import (SITE_LABELS, fuse_labels, gaussian_profile, chain_profiles,  # noqa: F401
                        table_s2_profile, TABLE_S2, reachable_tables, neighbour_profile)
 from .blocks import random_blocks, site_block_keys, theta_block_keys, env_block_keys  # noqa: F401
+from .chain import (SEED, site_tensor, left_canonical, right_canonical, chain_dims,  # noqa: F401
+                    theta_random, canonical_chain)

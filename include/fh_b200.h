@@ -82,6 +82,9 @@ int mps_site_layout(const fh_mps* mps, int site, int* nblk, int64_t* nelem, int3
  * order.  data_is_device != 0: device pointer (copied D2D on the context stream). */
 int mps_set_site(fh_ctx* ctx, fh_mps* mps, int site, const void* data, int data_is_device);
 int mps_get_site(fh_ctx* ctx, const fh_mps* mps, int site, void* data, int data_is_device);
+/* Release the arena storage of one site tensor (streamed environment construction at large chi,
+ * BASELINE.json config 5: a site is uploaded, absorbed into an environment, then dropped). */
+int mps_drop_site(fh_ctx* ctx, fh_mps* mps, int site);
 
 /* ---- environments (H4, H5) ---------------------------------------------
  * env_update_left : L_{site+1}[c',w',c] = sum alpha A[a',s',c']^H (L_site[a',w,a] A[a,s,c])
@@ -113,6 +116,10 @@ int heff_layout(const fh_ctx* ctx, int* nblk, int64_t* nelem, int32_t* labels, i
 int heff_get_tasks(const fh_ctx* ctx, int stage, int* ntask, int* nout, int32_t* tuples, double* alpha);
 /* out_dev = H_eff * theta_dev; both device vectors of heff_layout's nelem complex128. */
 int heff_apply(fh_ctx* ctx, const void* theta_dev, void* out_dev);
+/* Same operation with HOST buffers (pageable or pinned) of heff_layout's nelem complex128:
+ * copies theta to the device, applies, copies the result back and synchronises the stream.
+ * This is the end-to-end entry a caller without device memory uses. */
+int heff_apply_host(fh_ctx* ctx, const void* theta_host, void* out_host);
 /* sum over both task lists of 8*m*n*k */
 int64_t heff_flops(const fh_ctx* ctx);
 /* <x,y> = sum_blocks (2 j_b + 1) sum conj(x) y  (F-6) over the planned layout; result[2] = re,im */

@@ -41,6 +41,8 @@ _SIGS = {
     "mps_site_layout": (c_int, [c_void_p, c_int, P(c_int), P(c_i64), c_void_p, c_void_p]),
     "mps_set_site": (c_int, [c_void_p, c_void_p, c_int, c_void_p, c_int]),
     "mps_get_site": (c_int, [c_void_p, c_void_p, c_int, c_void_p, c_int]),
+    "mps_drop_site": (c_int, [c_void_p, c_void_p, c_int]),
+    "heff_apply_host": (c_int, [c_void_p, c_void_p, c_void_p]),
     "env_update_left": (c_int, [c_void_p, c_void_p, c_void_p, c_int]),
     "env_update_right": (c_int, [c_void_p, c_void_p, c_void_p, c_int]),
     "env_layout": (c_int, [c_void_p, c_int, c_int, P(c_int), P(c_i64), c_void_p, c_void_p]),
@@ -221,6 +223,15 @@ class Context:
         out = np.zeros(ne, dtype=np.complex128)
         self.check(lib.mps_get_site(self.h, mps, site, _np_ptr(out), 0), "mps_get_site")
         return out
+
+    def mps_drop_site(self, mps, site):
+        self.check(lib.mps_drop_site(self.h, mps, site), "mps_drop_site")
+
+    def heff_apply_host(self, theta, out):
+        """theta, out: host buffers (numpy complex128 or pinned torch CPU tensors)."""
+        pi = theta.ctypes.data if isinstance(theta, np.ndarray) else theta.data_ptr()
+        po = out.ctypes.data if isinstance(out, np.ndarray) else out.data_ptr()
+        self.check(lib.heff_apply_host(self.h, c_void_p(pi), c_void_p(po)), "heff_apply_host")
 
     def env_update_left(self, mpo, mps, site):
         self.check(lib.env_update_left(self.h, mpo, mps, site), "env_update_left")

@@ -575,6 +575,14 @@ int mps_get_site(fh_ctx* ctx, const fh_mps* mps, int site, void* data, int is_de
   })
 }
 
+int mps_drop_site(fh_ctx* ctx, fh_mps* mps, int site) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && mps && site >= 0 && site < mps->L, FH_EINVAL, "mps_drop_site: bad argument");
+    ctx->free_tensor(mps->A[site]);
+    mps->A[site].clear();
+  })
+}
+
 int env_update_left(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int site) {
   FH_TRY(ctx, {
     FH_REQUIRE(ctx && mpo && mps, FH_EINVAL, "env_update_left: NULL argument");
@@ -667,6 +675,27 @@ int heff_apply(fh_ctx* ctx, const void* theta_dev, void* out_dev) {
   FH_TRY(ctx, {
     FH_REQUIRE(ctx && theta_dev && out_dev, FH_EINVAL, "heff_apply: NULL argument");
     apply_heff(ctx, (const cplx*)theta_dev, (cplx*)out_dev);
+  })
+}
+
+int heff_apply_host(fh_ctx* ctx, const void* theta_host, void* out_host) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && theta_host && out_host, FH_EINVAL, "heff_apply_host: NULL argument");
+    FH_REQUIRE(ctx->plan.valid, FH_ESTATE, "heff_apply_host: no plan (call heff_plan first)");
+    const int64_t n = ctx->plan.vec.nelem;
+    const int64_t off = ctx->alloc.alloc(2 * n);
+    try {
+      cplx* din = ctx->ptr(off);
+      cplx* dout = din + n;
+      FH_CUDA(cudaMemcpyAsync(din, theta_host, n * sizeof(cplx), cudaMemcpyHostToDevice, ctx->stream));
+      apply_heff(ctx, din, dout);
+      FH_CUDA(cudaMemcpyAsync(out_host, dout, n * sizeof(cplx), cudaMemcpyDeviceToHost, ctx->stream));
+      FH_CUDA(cudaStreamSynchronize(ctx->stream));
+    } catch (...) {
+      ctx->alloc.release(off, 2 * n);
+      throw;
+    }
+    ctx->alloc.release(off, 2 * n);
   })
 }
 

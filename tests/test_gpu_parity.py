@@ -1,0 +1,301 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C-ABI binding, against the CPU
+oracle on the same seeded inputs.  Tolerances (north_star): relative Frobenius error <= 1e-11 per
+heff_apply in FP64; local observables within 1e-8 at matched chi; task tuples bit-exact."""
+import numpy as np
+import pytest
+
+import fh_inputs as fi
+from oracle import symm
+from oracle import symm_tdvp as stv
+from oracle.dense_tdvp import lanczos_exp
+
+from oracle_side import central_bond, env_key, heff2_selected, rel_err
+
+pytestmark = pytest.mark.gpu
+
+TOL_APPLY = 1e-11
+
+
+@pytest.fixture(scope="module")
+def H():
+    import paper_2606_04771_b200 as pkg
+    pkg.build()
+    from paper_2606_04771_b200 import harness
+    return harness
+
+
+@pytest.fixture()
+def ctx(H):
+    c = H.binding.Context(1 << 30)
+    yield c
+    c.close()
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _dev(v):
+    torch = _torch()
+    return torch.from_numpy(np.ascontiguousarray(v)).cuda()
+
+
+def _rand(rng, m, n):
+    return rng.standard_normal((m, n)) + 1j * rng.standard_normal((m, n))
+
+
+def _small_chain(rng, L, dmax):
+    tabs = fi.reachable_tables(L)
+    dims = [{sec: int(rng.integers(1, dmax + 1)) for sec in tabs[k]} for k in range(L + 1)]
+    dims[0] = {(0, 0): 1}
+    dims[L] = {(0, 0): 1}
+    A = [{k: _rand(rng, dims[i][k[0]], dims[i + 1][k[2]]) for k in symm.site_keys(dims[i], dims[i + 1])}
+         for i in range(L)]
+    return dims, A
+
+
+def _apply_gpu(H, ctx, vec_blocks, nsite):
+    lab, dm, ne = ctx.heff_layout(nsite)
+    keyfn = H.theta_key if nsite == 2 else H.site_key
+    x = _dev(H.flatten(vec_blocks, lab, dm, keyfn))
+    y = _torch().empty_like(x)
+    ctx.heff_apply(x, y)
+    return H.unflatten(y.cpu().numpy(), lab, dm, keyfn)
+
+
+# ------------------------------------------------------------------ small chains, every bond
+@pytest.mark.parametrize("L,dmax,seed", [(4, 3, 1), (6, 5, 2), (6, 11, 3)])
+def test_env_and_apply_parity_small_chain(H, ctx, L, dmax, seed):
+    """Ragged tiny blocks (1..11), all reachable sector combinations: environments (H4, H5),
+    two-site apply (H1+H2) on every bond and one-site apply (H3) on every site."""
+    rng = np.random.default_rng(seed)
+    t_h, U = 1.0, 4.0
+    dims, A = _small_chain(rng, L, dmax)
+    W = [symm.mpo_reduced(i, t_h, U) for i in range(L)]
+    Le = [symm.boundary_left()]
+    for i in range(L):
+        Le.append(symm.env_update_left(Le[i], A[i], W[i]))
+    Re = [None] * (L + 1)
+    Re[L] = symm.boundary_right()
+    for i in range(L - 1, -1, -1):
+        Re[i] = symm.env_update_right(Re[i + 1], A[i], W[i])
+
+    mpo = ctx.fh_mpo_build(L, t_h, U)
+    mps = ctx.mps_create(L)
+    for i in range(L):
+        H.set_site(ctx, mps, i, A[i], dims[i], dims[i + 1])
+    for i in range(L):
+        ctx.env_update_left(mpo, mps, i)
+    for i in range(L - 1, -1, -1):
+        ctx.env_update_right(mpo, mps, i)
+    for which, ref in ((0, Le), (1, Re)):
+        for k in range(L + 1):
+            lab, dm, flat = ctx.env_get(mps, which, k)
+            got = H.unflatten(flat, lab, dm, env_key)
+            assert sorted(got) == sorted(ref[k]), (which, k)
+            assert rel_err(got, ref[k], weighted=False) < 1e-12, (which, k)
+    for i in range(L - 1):
+        keys = symm.theta_keys(dims[i], dims[i + 2])
+        th = {k: _rand(rng, dims[i][k[0]], dims[i + 2][k[4]]) for k in keys}
+        ref = symm.heff2_apply(Le[i], Re[i + 2], th, W[i], W[i + 1])
+        ctx.heff_plan(mpo, mps, i, 2)
+        got = _apply_gpu(H, ctx, th, 2)
+        assert rel_err(got, ref) < TOL_APPLY, i
+    for i in range(L):
+        ref = symm.heff1_apply(Le[i], Re[i + 1], A[i], W[i])
+        ctx.heff_plan(mpo, mps, i, 1)
+        got = _apply_gpu(H, ctx, A[i], 1)
+        assert rel_err(got, ref) < TOL_APPLY, i
+    ctx.mps_destroy(mps)
+
+
+# ------------------------------------------------------------------ BASELINE config 2 at full size
+def test_config2_full_size_apply_tasks_and_hermiticity(H, ctx):
+    """configs[1]: L=60 central bond, chi=1024, environments contracted from the random canonical
+    MPS on both sides independently; heff_apply vs O-S <= 1e-11; task tuples bit-exact; flops equal;
+    H_eff Hermitian under the weighted inner product F-6."""
+    chi, L = 1024, 60
+    o = central_bond(chi, L)
+    c = o["centre"]
+    dl, dr = o["dims"][c], o["dims"][c + 2]
+    mpo = ctx.fh_mpo_build(L, 1.0, 4.0)
+    mps, dims = H.build_central_bond(ctx, mpo, chi, L)
+    assert dims[c] == dl and dims[c + 2] == dr
+    for which, k, ref in ((0, c, o["Lenv"]), (1, c + 2, o["Renv"])):
+        lab, dm, flat = ctx.env_get(mps, which, k)
+        got = H.unflatten(flat, lab, dm, env_key)
+        assert sorted(got) == sorted(ref)
+        assert rel_err(got, ref, weighted=False) < 1e-12
+    ctx.heff_plan(mpo, mps, c, 2)
+    # bit-exact task lists (A-14)
+    Lk, Rk = sorted(o["Lenv"]), sorted(o["Renv"])
+    vk = symm.theta_keys(dl, dr)
+    st1, st2 = symm.heff2_tasks(Lk, Rk, vk, o["W"][c], o["W"][c + 1])
+    o1 = symm.task_tuples(st1, list(st1), Lk, vk)
+    o2 = symm.task_tuples(st2, vk, list(st1), Rk)
+    t1, a1, n1 = ctx.heff_get_tasks(1)
+    t2, a2, n2 = ctx.heff_get_tasks(2)
+    assert n1 == len(st1) and n2 == len(vk)
+    assert t1.shape == o1[0].shape and (t1 == o1[0]).all()
+    assert t2.shape == o2[0].shape and (t2 == o2[0]).all()
+    assert np.abs(a1 - o1[1]).max() < 1e-13 and np.abs(a2 - o2[1]).max() < 1e-13
+    assert ctx.heff_flops() == symm.heff2_flops(st1, st2, dl, dr)
+    # apply
+    th = fi.theta_random(fi.SEED, c, dl, dr)
+    ref = symm.heff2_apply(o["Lenv"], o["Renv"], th, o["W"][c], o["W"][c + 1])
+    got = _apply_gpu(H, ctx, th, 2)
+    assert rel_err(got, ref) < TOL_APPLY
+    # host-buffer entry point gives the same bits as the device entry point
+    lab, dm, ne = ctx.heff_layout(2)
+    xin = H.flatten(th, lab, dm, H.theta_key)
+    xout = np.zeros_like(xin)
+    ctx.heff_apply_host(xin, xout)
+    assert np.array_equal(xout, H.flatten(got, lab, dm, H.theta_key))
+    # Hermiticity and inner product
+    ph = fi.theta_random(fi.SEED + 1, c, dl, dr)
+    x, y = _dev(xin), _dev(H.flatten(ph, lab, dm, H.theta_key))
+    hx, hy = _torch().empty_like(x), _torch().empty_like(y)
+    ctx.heff_apply(x, hx)
+    ctx.heff_apply(y, hy)
+    ip = ctx.heff_inner(y, x)
+    assert abs(ip - symm.inner(ph, th)) < 1e-12 * max(1.0, abs(ip))
+    a, b = ctx.heff_inner(y, hx), ctx.heff_inner(x, hy)
+    scale = np.sqrt(abs(ctx.heff_inner(hx, hx)) * abs(ctx.heff_inner(y, y)))
+    assert abs(a - np.conj(b)) < 1e-12 * scale
+    ctx.mps_destroy(mps)
+
+
+# ------------------------------------------------------------------ blocks that span several tiles
+@pytest.mark.parametrize("den", [24, 8])
+def test_apply_parity_table_s2_shape_random_envs(H, ctx, den):
+    """Paper-shaped sectors (Table S2 scaled by 1/den: d_max = 72 / 216, several 64- and 32-tiles
+    with ragged tails) with iid random environments given through env_set."""
+    L, c = 60, 29
+    even = fi.table_s2_profile(1, den)
+    dl, dr = fi.neighbour_profile(even, -1), fi.neighbour_profile(even, +1)
+    Lk, Rk = fi.env_block_keys(dl, dl), fi.env_block_keys(dr, dr)
+    Le = fi.random_blocks(7, 1, Lk, {k: (dl[k[0]], dl[k[2]]) for k in Lk})
+    Re = fi.random_blocks(7, 2, Rk, {k: (dr[k[0]], dr[k[2]]) for k in Rk})
+    th = fi.theta_random(7, c, dl, dr)
+    W1, W2 = symm.mpo_reduced(c, 1.0, 4.0), symm.mpo_reduced(c + 1, 1.0, 4.0)
+    mpo = ctx.fh_mpo_build(L, 1.0, 4.0)
+    mps = ctx.mps_create(L)
+    ctx.mps_set_bond(mps, c, dl)
+    ctx.mps_set_bond(mps, c + 2, dr)
+    for which, bond, keys, E in ((0, c, Lk, Le), (1, c + 2, Rk, Re)):
+        labels = [[k[0][0], k[0][1], k[1], k[2][0], k[2][1]] for k in keys]
+        flat = np.concatenate([E[k].ravel() for k in keys])
+        ctx.env_set(mps, which, bond, labels, flat)
+    ctx.heff_plan(mpo, mps, c, 2)
+    got = _apply_gpu(H, ctx, th, 2)
+    rng = np.random.default_rng(den)
+    keys = sorted(th)
+    if den >= 24:
+        ref = symm.heff2_apply(Le, Re, th, W1, W2)
+        assert rel_err(got, ref) < TOL_APPLY
+    else:
+        big = sorted(keys, key=lambda k: -th[k].size)[:6]
+        pick = big + [keys[i] for i in rng.choice(len(keys), 30, replace=False)]
+        ref = heff2_selected(Le, Re, th, W1, W2, pick)
+        for k in pick:
+            den_ = max(np.linalg.norm(ref[k]), 1e-300)
+            assert np.linalg.norm(got[k] - ref[k]) / den_ < TOL_APPLY, k
+    ctx.mps_destroy(mps)
+
+
+# ------------------------------------------------------------------ Lanczos exponential (H6 + H7)
+def test_expm_parity_central_bond(H, ctx):
+    """exp(-i tau H_eff) theta with m = 10 on the chi = 256 central bond vs the oracle's Lanczos
+    (full re-orthogonalisation) on the sqrt(2j+1)-scaled flat vector; norm conserved."""
+    chi, L, tau, m = 256, 60, 0.025, 10
+    o = central_bond(chi, L)
+    c = o["centre"]
+    dl, dr = o["dims"][c], o["dims"][c + 2]
+    th = fi.theta_random(fi.SEED, c, dl, dr)
+    W1, W2 = o["W"][c], o["W"][c + 1]
+
+    def apply_h(vec):
+        t = stv.unflatten(vec, th)
+        out = symm.heff2_apply(o["Lenv"], o["Renv"], t, W1, W2)
+        return stv.flatten({k: out[k] for k in th})
+
+    ref = stv.unflatten(lanczos_exp(apply_h, stv.flatten(th), tau, m), th)
+    mpo = ctx.fh_mpo_build(L, 1.0, 4.0)
+    mps, _ = H.build_central_bond(ctx, mpo, chi, L)
+    ctx.heff_plan(mpo, mps, c, 2)
+    lab, dm, ne = ctx.heff_layout(2)
+    x = _dev(H.flatten(th, lab, dm, H.theta_key))
+    y = _torch().empty_like(x)
+    ctx.heff_expm(x, y, tau, m)
+    got = H.unflatten(y.cpu().numpy(), lab, dm, H.theta_key)
+    assert rel_err(got, ref) < 1e-10
+    n0, n1 = ctx.heff_inner(x, x).real, ctx.heff_inner(y, y).real
+    assert abs(n1 / n0 - 1.0) < 1e-11
+    ctx.mps_destroy(mps)
+
+
+# ------------------------------------------------------------------ BASELINE config 1 end to end
+def test_config1_neel_quench_L8_vs_oracle(H, ctx):
+    """configs[0]: L=8 Neel quench, t_h=1, U=4, dt=0.05 to t=1.0, chi_max 256 (exact), m=10.
+    GPU tdvp2_sweep + measure_local/global vs the oracle's symmetric TDVP2 driver at matched
+    chi: observables <= 1e-8, sector tables identical, norm and energy conserved."""
+    L, t_h, U, dt, nstep, m = 8, 1.0, 4.0, 0.05, 20, 10
+    ref = stv.SymmTDVP(L, t_h, U, krylov_dim=m, chi_max_full=256, eps_trunc=-1.0)
+    mpo = ctx.fh_mpo_build(L, t_h, U)
+    mps = ctx.mps_init_neel(mpo, L)
+    g0 = ctx.measure_global(mpo, mps)
+    assert abs(g0["norm2"] - 1.0) < 1e-14 and abs(g0["energy"]) < 1e-13   # <Neel|H|Neel> = 0
+    l0 = ctx.measure_local(mps, L)
+    assert np.allclose(l0["sz"], [0.5 if i % 2 == 0 else -0.5 for i in range(L)], atol=1e-14)
+    assert np.allclose(l0["docc"], 0.0, atol=1e-14) and np.allclose(l0["n"], 1.0, atol=1e-14)
+    worst = 0.0
+    for step in range(nstep):
+        ref.step(dt)
+        ctx.tdvp2_sweep(mpo, mps, dt, krylov_dim=m, chi_max_full=256, eps_trunc=-1.0)
+        a, b = ref.measure_local(), ctx.measure_local(mps, L)
+        for key in ("n", "sz", "docc"):
+            worst = max(worst, np.abs(a[key] - b[key]).max())
+        ga, gb = ref.measure_global(), ctx.measure_global(mpo, mps)
+        assert abs(ga["norm2"] - gb["norm2"]) < 1e-10 and abs(ga["energy"] - gb["energy"]) < 1e-9
+        assert abs(gb["norm2"] - 1.0) < 1e-10 and abs(gb["energy"]) < 1e-9
+        for k in range(L + 1):
+            assert ctx.mps_get_bond(mps, k) == ref.dims[k], (step, k)
+    assert worst < 1e-8, worst
+    st = ctx.tdvp2_last_stats()
+    assert st["chi_full"] == max(ref.chi()) and st["max_discarded"] < 1e-20
+    ctx.mps_destroy(mps)
+
+
+# ------------------------------------------------------------------ edge cases and errors
+def test_edge_cases_and_error_codes(H, ctx):
+    B = H.binding
+    with pytest.raises(B.FhError):
+        ctx.fh_mpo_build(7, 1.0, 4.0)                 # odd L
+    with pytest.raises(B.FhError):
+        ctx.fh_mpo_build(0, 1.0, 4.0)                 # empty chain
+    mpo = ctx.fh_mpo_build(2, 1.0, 4.0)
+    x = _torch().zeros(4, dtype=_torch().complex128, device="cuda")
+    with pytest.raises(B.FhError):
+        ctx.heff_apply(x, x.clone())                  # no plan yet
+    # smallest chain: L=2 Neel, one bond, every block 1x1; singlet-sector two-site problem
+    mps = ctx.mps_init_neel(mpo, 2)
+    ctx.heff_plan(mpo, mps, 0, 2)
+    lab, dm, ne = ctx.heff_layout(2)
+    ref = stv.SymmTDVP(2, 1.0, 4.0, krylov_dim=4)
+    th = ref._theta(0)
+    assert ne == sum(v.size for v in th.values())
+    want = symm.heff2_apply(ref.Lenv[0], ref.Renv[2], th, ref.W[0], ref.W[1])
+    got = _apply_gpu(H, ctx, th, 2)
+    assert rel_err(got, want) < TOL_APPLY
+    with pytest.raises(B.FhError):
+        ctx.heff_plan(mpo, mps, 1, 2)                 # bond out of range
+    with pytest.raises(B.FhError):
+        ctx.mps_set_bond(mps, 1, {(0, 0): 1})         # violates the parity rule q + 2j = k (mod 2)
+    ctx.mps_destroy(mps)
+    # arena exhaustion is reported, not fatal
+    small = B.Context(1 << 20)
+    mpo2 = small.fh_mpo_build(60, 1.0, 4.0)
+    with pytest.raises(B.FhError, match="arena"):
+        H.build_central_bond(small, mpo2, 4096, 60)
+    small.close()
