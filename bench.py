@@ -56,7 +56,8 @@ def peaks():
 
 def workload_name(args):
     if args.profile == "gaussian":
-        return "config3 heff_apply: L=60 central bond (29,30), chi=%d, Gaussian sector profile, complex128" % args.chi
+        cfg = {1024: "config 2", 4096: "config 3"}.get(args.chi, "config 2/3 recipe")
+        return "%s heff_apply: L=60 central bond (29,30), chi=%d, Gaussian sector profile, complex128" % (cfg, args.chi)
     return "heff_apply: L=60 central bond, Table S2 profile x %s, complex128" % args.s2_scale
 
 
@@ -106,3 +107,231 @@ class ClockSampler:
         os.unlink(self.f.name)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
                 "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def cpu_oracle_setup(args):
+    """Oracle-side workload (bounded sample): same sector structure and theta; environments are
+    iid random blocks of the right shapes (timing does not depend on their values, and building
+    the canonical chain in pure Python would dominate the run)."""
+    import fh_inputs as fi
+    from oracle import symm
+    L, c = 60, 29
+    dims = fi.chain_dims(args.chi, L, args.profile, s2_scale(args))
+    dl, dr = dims[c], dims[c + 2]
+    Lk, Rk = fi.env_block_keys(dl, dl), fi.env_block_keys(dr, dr)
+    Le = fi.random_blocks(11, 1, Lk, {k: (dl[k[0]], dl[k[2]]) for k in Lk})
+    Re = fi.random_blocks(11, 2, Rk, {k: (dr[k[0]], dr[k[2]]) for k in Rk})
+    th = fi.theta_random(fi.SEED, c, dl, dr)
+    W1, W2 = symm.mpo_reduced(c, 1.0, 4.0), symm.mpo_reduced(c + 1, 1.0, 4.0)
+    st1, st2 = symm.heff2_tasks(sorted(Le), sorted(Re), sorted(th), W1, W2)
+    flops = symm.heff2_flops(st1, st2, dl, dr)
+    # bound the sample to ~2 GFLOP of output blocks (whole apply when it is smaller)
+    budget, sub2, acc = 4e9, {}, 0
+    for k, segs in st2.items():
+        sub2[k] = segs
+        acc += sum(8 * dl[z[0]] * dr[b] * dr[bp] for z, (bp, wr, b), _ in segs)
+        if acc > budget:
+            break
+    whole = len(sub2) == len(st2)
+    need = {seg[0] for segs in sub2.values() for seg in segs}
+    sub1 = st1 if whole else {z: st1[z] for z in need}
+    f1 = sum(8 * dl[ap] * dl[a] * dr[kk[4]] for z, segs in sub1.items() for (ap, w, a), kk, _ in segs)
+    f2 = sum(8 * dl[z[0]] * dr[b] * dr[bp] for segs in sub2.values() for z, (bp, wr, b), _ in segs)
+
+    def step():
+        Z = symm.run_stage(sub1, Le, th)
+        return symm.run_stage(sub2, Z, Re, "n", "t")
+
+    sample = ("whole heff_apply" if whole else "%d of %d output blocks" % (len(sub2), len(st2))) + \
+        " (%.3g of %.3g GFLOP), task lists prebuilt, random environments of the same shapes" % (
+            (f1 + f2) * 1e-9, flops * 1e-9)
+    return step, f1 + f2, sample
+
+
+def cpu_cores():
+    try:
+        from threadpoolctl import threadpool_info
+        n = max([d.get("num_threads", 1) for d in threadpool_info()] or [1])
+    except Exception:
+        n = os.cpu_count() or 1
+    return int(n)
+
+
+def time_oracle(args, steps, warmup):
+    step, flops, sample = cpu_oracle_setup(args)
+    for _ in range(warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        step()
+    dt = (time.perf_counter() - t0) / steps
+    return dict(value=flops / dt * 1e-9, unit="GFLOP/s", cores=cpu_cores(), kind="oracle", sample=sample), dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cb, dt = time_oracle(args, args.steps, args.warmup)
+    out = {"impl": "reference", "metric": "heff_apply_gflops", "value": cb["value"], "unit": "GFLOP/s",
+           "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3,
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "complex128 (f64)",
+           "data": "synthetic", "config": {"workload": workload_name(args), "chi": args.chi, "profile": args.profile},
+           "cpu_baseline": cb,
+           "e2e": {"value": cb["value"], "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_04771_b200 import harness as H     # fails loudly if the CUDA library is missing
+    import fh_inputs as fi
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the library has no CPU path (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    pk = peaks()
+    L, c = 60, 29
+    chi = args.chi
+    # replicas only (north_star: one GPU, no sharding, no collectives): every rank runs the same bond
+    arena = int(min(160e9, max(2 << 30, 64.0 * chi * chi)))
+    ctx = H.binding.Context(arena, device="cuda:%d" % local)
+    mpo = ctx.fh_mpo_build(L, 1.0, 4.0)
+    t_build = time.perf_counter()
+    mps, dims = H.build_central_bond(ctx, mpo, chi, L, profile=args.profile, table_s2_scale=s2_scale(args))
+    ctx.heff_plan(mpo, mps, c, 2)
+    torch.cuda.synchronize()
+    t_build = time.perf_counter() - t_build
+    lab, dm, ne = ctx.heff_layout(2)
+    th = fi.theta_random(fi.SEED, c, dims[c], dims[c + 2])
+    x_host = torch.from_numpy(H.flatten(th, lab, dm, H.theta_key)).pin_memory()
+    y_host = torch.empty_like(x_host).pin_memory()
+    x = x_host.cuda()
+    y = torch.empty_like(x)
+    flops = ctx.heff_flops()
+    t1, _, nz = ctx.heff_get_tasks(1)
+    t2, _, no = ctx.heff_get_tasks(2)
+    flush = None if args.no_flush else torch.empty(256 << 20, dtype=torch.uint8, device=x.device)
+
+    def sync_all():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        ctx.heff_apply(x, y)
+    peak_dmma = ctx.fh_dmma_peak_tflops(5)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    l0 = ctx.fh_launch_count()
+    sync_all()
+    clocks = ClockSampler(local)
+    wall0 = time.perf_counter()
+    for a, b in ev:
+        if flush is not None:
+            flush.zero_()
+        a.record()
+        ctx.heff_apply(x, y)
+        b.record()
+    sync_all()
+    wall = time.perf_counter() - wall0
+    launches = ctx.fh_launch_count() - l0
+    ms = [a.elapsed_time(b) for a, b in ev]
+    t_dev = sum(ms) * 1e-3
+    # L2-warm variant: K applies back to back inside one event pair (what a Lanczos loop sees)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(args.steps):
+        ctx.heff_apply(x, y)
+    b.record()
+    torch.cuda.synchronize()
+    t_warm = a.elapsed_time(b) * 1e-3
+    clk = clocks.stop()
+    # end to end through the host-buffer entry point (pinned host memory, H2D + D2H inside)
+    for _ in range(2):
+        ctx.heff_apply_host(x_host, y_host)
+    sync_all()
+    w0 = time.perf_counter()
+    for _ in range(args.steps):
+        ctx.heff_apply_host(x_host, y_host)
+    torch.cuda.synchronize()
+    t_e2e = time.perf_counter() - w0
+    tt = torch.tensor([t_dev, t_e2e, t_warm], dtype=torch.float64, device=x.device)
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    t_dev, t_e2e, t_warm = [float(v) for v in tt.cpu()]
+    if rank != 0:
+        return
+    gf = world * flops * args.steps / t_dev * 1e-9
+    per_gpu_tf = flops * args.steps / t_dev * 1e-12
+    peak_rule = pk["bf16"] * NOMINAL_FP64_TF / NOMINAL_BF16_TF
+    zbytes = 16 * sum(int(a_) * int(b_) for a_, b_ in dm)
+    out = {
+        "metric": "heff_apply_gflops", "value": gf, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": t_dev / args.steps * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "complex128 (f64)", "data": "synthetic",
+        "config": {"workload": workload_name(args), "chi": chi, "profile": args.profile,
+                   "chi_su2": [sum(dims[k].values()) for k in (c, c + 1, c + 2)],
+                   "d_max": max(max(dims[k].values()) for k in (c, c + 2)), "theta_blocks": len(lab),
+                   "z_blocks": nz, "tasks": [len(t1), len(t2)], "flop_per_apply": flops, "theta_bytes": zbytes,
+                   "l2": "not flushed" if flush is None else "flushed between timed applies (256 MiB write, outside the event pairs)",
+                   "parallelism": "replicas only (one GPU per problem, no collectives)", "setup_seconds": t_build},
+        "value_l2_warm": world * flops * args.steps / t_warm * 1e-9,
+        "roofline": {"kernel": "grouped_zgemm_kernel (stage 1 + stage 2 launches of one apply)", "bound": "tensor",
+                     "achieved": per_gpu_tf, "peak": peak_dmma, "unit": "TFLOP/s", "frac": per_gpu_tf / peak_dmma,
+                     "peak_source": "FP64 DMMA.8x8x4 issue peak measured in this run (fh_dmma_peak_tflops)",
+                     "peak_rule": peak_rule, "frac_rule": per_gpu_tf / peak_rule,
+                     "peak_rule_source": "%s bf16 %.1f TF x nominal fp64/bf16 %g/%g" % (
+                         pk["source"], pk["bf16"], NOMINAL_FP64_TF, NOMINAL_BF16_TF),
+                     "frac_l2_warm": flops * args.steps / t_warm * 1e-12 / peak_dmma, "traffic": None},
+        "e2e": {"value": world * flops * args.steps / t_e2e * 1e-9, "unit": "GFLOP/s",
+                "h2d_bytes_per_step": zbytes, "d2h_bytes_per_step": zbytes, "api": "heff_apply_host (pinned host buffers)"},
+        "gpu_launches": int(launches), "clocks": clk, "wall_seconds_timed_region": wall,
+    }
+    if args.sweep:
+        out["sweep"] = run_sweep(ctx, H, mpo, args)
+    if not args.no_cpu_baseline:
+        cb, _ = time_oracle(args, 3, 1)
+        out["cpu_baseline"] = cb
+    print(json.dumps(out))
+    ctx.close()
+
+
+def run_sweep(ctx, H, mpo, args):
+    """One full tdvp2_sweep(dt=0.05), m=10, over all 59 bonds of the random right-canonical chain
+    at --sweep-chi, with the library's per-phase CUDA-event timers (config 3's second half)."""
+    import torch
+    chi = args.sweep_chi
+    mps, _ = H.build_central_bond(ctx, mpo, chi, 60, centre=0, keep_sites=True,
+                                  profile="gaussian")
+    ctx.fh_reset_timers()
+    torch.cuda.synchronize()
+    l0 = ctx.fh_launch_count()
+    t0 = time.perf_counter()
+    ctx.tdvp2_sweep(mpo, mps, 0.05, krylov_dim=10, chi_max_full=chi, eps_trunc=-1.0)
+    torch.cuda.synchronize()
+    sec = time.perf_counter() - t0
+    tm = ctx.fh_get_timers()
+    st = ctx.tdvp2_last_stats()
+    ctx.mps_destroy(mps)
+    return {"chi": chi, "seconds": sec, "device_seconds_by_phase": tm, "stats": st,
+            "launches": ctx.fh_launch_count() - l0}
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

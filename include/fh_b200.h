@@ -141,6 +141,11 @@ int tdvp2_sweep(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh
 /* statistics of the last sweep: max discarded weight, max chi_full, max chi_su2, max d */
 int tdvp2_last_stats(const fh_ctx* ctx, double* max_discarded, int* chi_full, int* chi_su2, int* dmax);
 
+/* Singular values kept on `bond` by the most recent SVD split there (H9), concatenated sector by
+ * sector in the order of mps_get_bond (d_c values per sector, descending inside a sector).  n = 0
+ * if the bond has not been split yet.  Pass s = NULL to query n.  Gauge-invariant data (A-13). */
+int mps_get_svals(const fh_mps* mps, int bond, int* n, double* s);
+
 /* ---- observables (H10; reading A-12) -----------------------------------
  * n_i = <1> ratio (== 1 in a T_tot = 0 state), sz_i = <S^z_i>, docc_i = <n_up n_dn>_i = <P_D>/2;
  * host arrays of length L.  Requires all sites right of the centre right-canonical (true
@@ -160,6 +165,11 @@ int64_t fh_launch_count(const fh_ctx* ctx);
  * Runs cublasZgemm (is_complex=1) or cublasDgemm n x n x n `reps` times on the context stream
  * and returns the average seconds per call.  Library GEMM, not part of the hot path. */
 int fh_cublas_gemm_seconds(fh_ctx* ctx, int n, int is_complex, int reps, double* seconds);
+
+/* FP64 tensor-pipe issue peak: a register-only loop of DMMA.8x8x4 (mma.sync.m8n8k4.f64) on every
+ * SM; returns the achieved TFLOP/s (2 flops per FMA).  The roofline denominator of the GEMM
+ * kernels, measured on the same device and clocks as the run.  Not part of the hot path. */
+int fh_dmma_peak_tflops(fh_ctx* ctx, int reps, double* tflops);
 
 /* ---- host-only entry points (no CUDA call inside): the symmetry layer on its own -----------
  * Closed-form recoupling coefficients of reading F-5 (all arguments doubled spins):

@@ -56,6 +56,7 @@ class SymmTDVP:
         for i in range(L - 1, 0, -1):
             self.Renv[i] = symm.env_update_right(self.Renv[i + 1], self.A[i], self.W[i])
         self.max_discarded = 0.0
+        self.svals = [None] * (L + 1)     # kept singular values of the last split per bond
 
     # ---- local solvers
     def _evolve2(self, i, theta, tau):
@@ -104,6 +105,7 @@ class SymmTDVP:
                                               self.chi_max, self.eps, "right")
             self.max_discarded = max(self.max_discarded, info["discarded"])
             self.A[i], self.A[i + 1], self.dims[i + 1] = A1, A2, dm
+            self.svals[i + 1] = {c: info["svals"][c][:k] for c, k in info["keep"].items() if k > 0}
             self.Lenv[i + 1] = symm.env_update_left(self.Lenv[i], A1, self.W[i])
             if i < L - 2:
                 self.A[i + 1] = self._evolve1(i + 1, A2, self.Lenv[i + 1], self.Renv[i + 2], -tau)
@@ -113,6 +115,7 @@ class SymmTDVP:
                                               self.chi_max, self.eps, "left")
             self.max_discarded = max(self.max_discarded, info["discarded"])
             self.A[i], self.A[i + 1], self.dims[i + 1] = A1, A2, dm
+            self.svals[i + 1] = {c: info["svals"][c][:k] for c, k in info["keep"].items() if k > 0}
             self.Renv[i + 1] = symm.env_update_right(self.Renv[i + 2], A2, self.W[i + 1])
             if i > 0:
                 self.A[i] = self._evolve1(i, A1, self.Lenv[i], self.Renv[i + 1], -tau)

@@ -41,6 +41,8 @@ _SIGS = {
     "mps_site_layout": (c_int, [c_void_p, c_int, P(c_int), P(c_i64), c_void_p, c_void_p]),
     "mps_set_site": (c_int, [c_void_p, c_void_p, c_int, c_void_p, c_int]),
     "mps_get_site": (c_int, [c_void_p, c_void_p, c_int, c_void_p, c_int]),
+    "mps_get_svals": (c_int, [c_void_p, c_int, P(c_int), c_void_p]),
+    "fh_dmma_peak_tflops": (c_int, [c_void_p, c_int, P(c_dbl)]),
     "mps_drop_site": (c_int, [c_void_p, c_void_p, c_int]),
     "heff_apply_host": (c_int, [c_void_p, c_void_p, c_void_p]),
     "env_update_left": (c_int, [c_void_p, c_void_p, c_void_p, c_int]),
@@ -223,6 +225,23 @@ class Context:
         out = np.zeros(ne, dtype=np.complex128)
         self.check(lib.mps_get_site(self.h, mps, site, _np_ptr(out), 0), "mps_get_site")
         return out
+
+    def mps_get_svals(self, mps, bond):
+        """{(q,tj): kept singular values (descending)} of the last SVD split on `bond`."""
+        n = c_int()
+        self.check(lib.mps_get_svals(mps, bond, C.byref(n), None), "mps_get_svals")
+        s = np.zeros(n.value)
+        self.check(lib.mps_get_svals(mps, bond, C.byref(n), _np_ptr(s)), "mps_get_svals")
+        out, o = {}, 0
+        for sec, d in self.mps_get_bond(mps, bond).items():
+            out[sec] = s[o:o + d]
+            o += d
+        return out if n.value else {}
+
+    def fh_dmma_peak_tflops(self, reps=5):
+        t = c_dbl()
+        self.check(lib.fh_dmma_peak_tflops(self.h, reps, C.byref(t)), "fh_dmma_peak_tflops")
+        return t.value
 
     def mps_drop_site(self, mps, site):
         self.check(lib.mps_drop_site(self.h, mps, site), "mps_drop_site")

@@ -450,6 +450,7 @@ int mps_create(fh_ctx* ctx, int L, fh_mps** out) {
     m->A.resize(L);
     m->Lenv.resize(L + 1);
     m->Renv.resize(L + 1);
+    m->sval.resize(L + 1);
     m->bond[0].sec = {Sector{0, 0}};
     m->bond[0].d = {1};
     m->bond[L] = m->bond[0];
@@ -573,6 +574,14 @@ int mps_get_site(fh_ctx* ctx, const fh_mps* mps, int site, void* data, int is_de
                             is_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, ctx->stream));
     FH_CUDA(cudaStreamSynchronize(ctx->stream));
   })
+}
+
+int mps_get_svals(const fh_mps* mps, int bond, int* n, double* s) {
+  if (!mps || bond < 0 || bond > mps->L || !n) return FH_EINVAL;
+  const std::vector<double>& v = mps->sval[bond];
+  *n = (int)v.size();
+  if (s) std::memcpy(s, v.data(), v.size() * sizeof(double));
+  return FH_OK;
 }
 
 int mps_drop_site(fh_ctx* ctx, fh_mps* mps, int site) {
@@ -839,6 +848,28 @@ int fh_cublas_gemm_seconds(fh_ctx* ctx, int n, int is_complex, int reps, double*
     cudaFree(B);
     cudaFree(C);
     cublasDestroy(h);
+  })
+}
+
+int fh_dmma_peak_tflops(fh_ctx* ctx, int reps, double* tflops) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && reps > 0 && tflops, FH_EINVAL, "fh_dmma_peak_tflops: bad argument");
+    double* scratch = nullptr;
+    FH_CUDA(cudaMalloc((void**)&scratch, (size_t)148 * 4 * 256 * sizeof(double)));
+    cudaEvent_t e0, e1;
+    FH_CUDA(cudaEventCreate(&e0));
+    FH_CUDA(cudaEventCreate(&e1));
+    const double fl = fh::launch_dmma_peak(scratch, ctx->stream, &ctx->launches);  // warm-up
+    FH_CUDA(cudaEventRecord(e0, ctx->stream));
+    for (int r = 0; r < reps; ++r) fh::launch_dmma_peak(scratch, ctx->stream, &ctx->launches);
+    FH_CUDA(cudaEventRecord(e1, ctx->stream));
+    FH_CUDA(cudaEventSynchronize(e1));
+    float ms = 0;
+    FH_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+    *tflops = fl * reps / (ms * 1e-3) * 1e-12;
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(scratch);
   })
 }
 

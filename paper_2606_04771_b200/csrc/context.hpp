@@ -78,6 +78,7 @@ struct fh_mps {
   int L;
   std::vector<fh::Bond> bond;                       // L+1
   std::vector<fh::BlockTensor> A, Lenv, Renv;       // L, L+1, L+1
+  std::vector<std::vector<double>> sval;            // L+1: kept singular values of the last split
 };
 
 struct fh_ctx {

@@ -139,5 +139,7 @@ void launch_copy_blocks(const CopyBlk* d_blks, int nblk, const cplx* src, cplx* 
 void launch_block_norms(const VecChunk* d_chunks, int nchunks, const cplx* x, double* d_out,
                         cudaStream_t s, int64_t* lc);
 void launch_fill_zero(cplx* p, int64_t n, cudaStream_t s, int64_t* lc);
+// calibration: register-only DMMA loop on 148*4 CTAs of 256 threads; returns the flops of one launch
+double launch_dmma_peak(double* scratch, cudaStream_t s, int64_t* lc);
 
 }  // namespace fh

@@ -408,4 +408,29 @@ void launch_copy_blocks(const CopyBlk* d_blks, int nblk, const cplx* src, cplx* 
   ++*lc;
 }
 
+// ------------------------------------------------------------------------------------------
+// calibration: FP64 tensor-pipe issue peak (roofline denominator, not on the hot path)
+// ------------------------------------------------------------------------------------------
+constexpr int PEAK_ITERS = 2048, PEAK_ACC = 8;
+__global__ void __launch_bounds__(256) dmma_peak_kernel(double* out) {
+  double c[PEAK_ACC][2];
+#pragma unroll
+  for (int i = 0; i < PEAK_ACC; ++i) c[i][0] = c[i][1] = threadIdx.x * 1e-9 + i;
+  const double a = 1.0 + threadIdx.x * 1e-7, b = 1.0 - threadIdx.x * 1e-7;
+  for (int it = 0; it < PEAK_ITERS; ++it) {
+#pragma unroll
+    for (int i = 0; i < PEAK_ACC; ++i) dmma884(c[i][0], c[i][1], a, b);
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int i = 0; i < PEAK_ACC; ++i) s += c[i][0] + c[i][1];
+  out[blockIdx.x * 256 + threadIdx.x] = s;
+}
+double launch_dmma_peak(double* scratch, cudaStream_t s, int64_t* lc) {
+  const int ctas = 148 * 4;
+  dmma_peak_kernel<<<ctas, 256, 0, s>>>(scratch);
+  ++*lc;
+  return 2.0 * 256.0 * PEAK_ITERS * PEAK_ACC * 8.0 * ctas;  // 8 warps x 256 FMA per DMMA.8x8x4
+}
+
 }  // namespace fh

@@ -214,6 +214,9 @@ static void svd_split(fh_ctx* ctx, fh_mps* mps, int i, const BlockTensor& th, co
     }
   }
   mps->bond[i + 1] = nb;
+  mps->sval[i + 1].clear();
+  for (size_t x = 0; x < order.size(); ++x)
+    mps->sval[i + 1].insert(mps->sval[i + 1].end(), sv[x].begin(), sv[x].begin() + keep[x]);
   ctx->stat_chi = std::max(ctx->stat_chi, nb.chi_full());
   ctx->stat_su2 = std::max(ctx->stat_su2, nb.chi_su2());
   ctx->stat_dmax = std::max(ctx->stat_dmax, nb.dmax());
