@@ -68,14 +68,11 @@ void DevPool::destroy() {
 }
 
 size_t fh::stage_bytes(const Stage& st) {
-  return st.outs.size() * sizeof(GemmOut) + st.segs.size() * sizeof(GemmSeg) +
-         (st.tiles64.size() + st.tiles32.size()) * sizeof(GemmTile) + 4 * 256;
+  return st.segs.size() * sizeof(GemmSeg) + st.units.size() * sizeof(GemmUnit) + 4 * 256;
 }
 void fh::upload_stage(DevPool& pool, Stage& st, cudaStream_t s) {
-  st.d_outs = upload(pool, st.outs, s);
   st.d_segs = upload(pool, st.segs, s);
-  st.d_tiles64 = upload(pool, st.tiles64, s);
-  st.d_tiles32 = upload(pool, st.tiles32, s);
+  st.d_units = upload(pool, st.units, s);
 }
 
 void fh_ctx::alloc_tensor(BlockTensor& t) { t.base = alloc.alloc(t.nelem); }

@@ -77,18 +77,26 @@ double coef_right(int tc, int ts, int tb, int tk, int tr, int tkp, int tcp, int 
 enum OpA { OPA_N = 0, OPA_C = 1, OPA_H = 2 };  // as stored | conj | conj-transpose
 enum OpB { OPB_N = 0, OPB_T = 1 };             // as stored | transpose
 
-struct GemmOut {  // one output block C (M x N, row-major, ld = N)
+struct GemmOut {  // one output block C (M x N, row-major, leading dimension ldc)
   int64_t c_off;
   int M, N;
   int seg_begin, seg_end;
+  int ldc, steps;  // steps = sum over segments of ceil(K / 4) (DMMA k-steps)
 };
 struct GemmSeg {  // one K-segment: C += alpha * op(A) (M x K) * op(B) (K x N)
-  int64_t a_off, b_off;
-  int K, lda, ldb, pad;
-  double alpha;
+  int64_t a_off, b_off;   // element offsets of the operand blocks
+  int K;
+  int a_sm, a_sk;         // element strides of op(A): (m, k) -> a_off + m * a_sm + k * a_sk
+  int b_sk, b_sn;         // element strides of op(B): (k, n) -> b_off + k * b_sk + n * b_sn
+  int pad;
+  double alpha;           // real recoupling coefficient x MPO scalar
 };
-struct GemmTile {  // one CTA's work: tile (m0, n0) of output block `out`
-  int out, m0, n0, pad;
+// One warp's work: a (8*mt) x (8*nt) sub-tile of output block `out` over the whole K of that
+// block (all its segments).  The output geometry is repeated here so that the kernel needs a
+// single descriptor load per unit.  shape = mt * 16 + nt, mt * nt <= 16, mt, nt <= 8.
+struct GemmUnit {
+  int64_t c_off;
+  int ldc, M, N, seg_begin, seg_end, steps, m0, n0, shape, pad;
 };
 
 struct Stage {
@@ -97,14 +105,13 @@ struct Stage {
   std::vector<double> t_alpha;
   std::vector<GemmOut> outs;
   std::vector<GemmSeg> segs;
-  std::vector<GemmTile> tiles64, tiles32;
+  std::vector<GemmUnit> units;  // sorted by work, heaviest first
   int opA = OPA_N, opB = OPB_N;
   int64_t flops = 0;
+  int64_t dmma_padded = 0;  // DMMA.8x8x4 instructions the unit list issues (incl. ragged-edge padding)
   // device copies
-  GemmOut* d_outs = nullptr;
   GemmSeg* d_segs = nullptr;
-  GemmTile* d_tiles64 = nullptr;
-  GemmTile* d_tiles32 = nullptr;
+  GemmUnit* d_units = nullptr;
 };
 
 // weighted-vector chunk table (H6): contiguous chunk [start, start+len) carries weight w

@@ -1,14 +1,9 @@
-// Hand-written sm_100a kernels of the hot path:
-//   * grouped_zgemm_kernel: segmented grouped complex128 GEMM over a tile queue,
-//       C_o (M x N) = sum_{t in seg(o)} alpha_t * op(A_t) (M x K_t) * op(B_t) (K_t x N)
-//     FP64 tensor-core path: mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4, the only FP64 MMA shape
-//     sm_100a has; tcgen05 has no f64 kind), four real DMMAs per complex product, operands staged
-//     through a multi-stage cp.async (LDGSTS) ring with zero-filled ragged edges, the real
-//     recoupling coefficient alpha fused into the A-fragment load, padding sub-tiles skipped.
-//   * weighted dot / axpy / linear-combination kernels for the Lanczos recurrences (HBM-bound).
-//   * block gather/scatter with scaling for pack/unpack around the block-wise SVD (HBM-bound).
-// Outputs are never shared between CTAs and reductions run in a fixed order: results are
-// run-to-run bit-identical.
+// Hand-written sm_100a kernels of the bandwidth-bound part of the hot path:
+//   * weighted dot / axpy / linear-combination kernels for the Lanczos recurrences;
+//   * block gather/scatter with scaling for pack/unpack around the block-wise SVD;
+//   * the DMMA issue-peak calibration kernel (roofline denominator).
+// The segmented grouped ZGEMM (H1-H5) lives in zgemm.cu.
+// Reductions run in a fixed order: results are run-to-run bit-identical.
 #include "fh_internal.hpp"
 
 namespace fh {
@@ -20,226 +15,6 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
   asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
       : "+d"(c0), "+d"(c1)
       : "d"(a), "d"(b));
-}
-__device__ __forceinline__ void cp_async16(uint32_t smem_addr, const void* gptr, int src_bytes) {
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_addr), "l"(gptr), "r"(src_bytes));
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() {
-  asm volatile("cp.async.wait_group %0;" ::"n"(N));
-}
-
-// ------------------------------------------------------------------------------------------
-// Segmented grouped ZGEMM
-// ------------------------------------------------------------------------------------------
-// Shared-memory tile layouts (BK = 8 complex per pipeline stage):
-//   K-minor (operand stored with k contiguous: A for OPA_N/OPA_C, B for OPB_T):
-//       [BK/4][ROWS][4] complex  -> a fragment load (row = lane/4, k = lane%4) of a quarter
-//       warp touches 128 contiguous bytes: conflict-free without padding.
-//   K-major (operand stored with the m / n index contiguous: A for OPA_H, B for OPB_N):
-//       [BK][COLS + 2] complex   -> row pitch = 32 B mod 128: the 4 k-rows of a quarter warp
-//       land in distinct 32-byte bank groups: conflict-free.
-constexpr int BK = 8;
-
-template <int ROWS, bool KMINOR>
-struct TileLayout {
-  static constexpr int elems = KMINOR ? ROWS * BK : BK * (ROWS + 2);
-  // element index of (row r, k)
-  __device__ static __forceinline__ int at(int r, int k) {
-    return KMINOR ? (((k >> 2) * ROWS + r) << 2) + (k & 3) : k * (ROWS + 2) + r;
-  }
-};
-
-template <int BM, int BN, int WARPS_M, int WARPS_N, int OPA, int OPB, int STAGES>
-__global__ void __launch_bounds__(WARPS_M* WARPS_N * 32)
-    grouped_zgemm_kernel(const GemmTile* __restrict__ tiles, const GemmOut* __restrict__ outs,
-                         const GemmSeg* __restrict__ segs, const cplx* __restrict__ Abase,
-                         const cplx* __restrict__ Bbase, cplx* __restrict__ Cbase) {
-  constexpr int NT = WARPS_M * WARPS_N * 32;
-  constexpr int WM = BM / WARPS_M, WN = BN / WARPS_N;
-  constexpr int MT = WM / 8, NTL = WN / 8;
-  constexpr bool A_KMINOR = (OPA != OPA_H);
-  constexpr bool B_KMINOR = (OPB == OPB_T);
-  typedef TileLayout<BM, A_KMINOR> LA;
-  typedef TileLayout<BN, B_KMINOR> LB;
-  constexpr int STAGE_ELEMS = LA::elems + LB::elems;
-
-  extern __shared__ __align__(128) unsigned char smem_raw[];
-  cplx* smem = reinterpret_cast<cplx*>(smem_raw);
-
-  const GemmTile tile = tiles[blockIdx.x];
-  const GemmOut out = outs[tile.out];
-  const int M = out.M, N = out.N;
-  const int m0 = tile.m0, n0 = tile.n0;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int wm0 = (warp / WARPS_N) * WM, wn0 = (warp % WARPS_N) * WN;
-  const int mrem = M - m0, nrem = N - n0;  // valid rows / cols in this tile (may exceed BM / BN)
-
-  // number of 8x8 sub-tiles of this warp that hold real data (edge skipping, warp-uniform)
-  int mt_valid = (mrem - wm0 + 7) >> 3;
-  mt_valid = mt_valid < 0 ? 0 : (mt_valid > MT ? MT : mt_valid);
-  int nt_valid = (nrem - wn0 + 7) >> 3;
-  nt_valid = nt_valid < 0 ? 0 : (nt_valid > NTL ? NTL : nt_valid);
-
-  double acc_re[MT][NTL][2], acc_im[MT][NTL][2];
-#pragma unroll
-  for (int i = 0; i < MT; ++i)
-#pragma unroll
-    for (int j = 0; j < NTL; ++j) acc_re[i][j][0] = acc_re[i][j][1] = acc_im[i][j][0] = acc_im[i][j][1] = 0.0;
-
-  // ---- chunk iterators: a chunk is BK consecutive k of one segment
-  int ld_seg = out.seg_begin, ld_k0 = 0;
-  int cp_seg = out.seg_begin, cp_k0 = 0;
-  const int seg_end = out.seg_end;
-
-  auto load_chunk = [&](int stage) {
-    if (ld_seg < seg_end) {
-      const GemmSeg sg = segs[ld_seg];
-      cplx* sA = smem + stage * STAGE_ELEMS;
-      cplx* sB = sA + LA::elems;
-      const cplx* gA = Abase + sg.a_off;
-      const cplx* gB = Bbase + sg.b_off;
-      const int kleft = sg.K - ld_k0;
-      // A tile: BM rows x BK
-#pragma unroll
-      for (int idx = tid; idx < BM * BK; idx += NT) {
-        int r, k;
-        if (A_KMINOR) { r = idx / BK; k = idx % BK; } else { k = idx / BM; r = idx % BM; }
-        const bool ok = (r < mrem) && (k < kleft);
-        const cplx* src = gA;
-        if (ok) src = A_KMINOR ? gA + (int64_t)(m0 + r) * sg.lda + (ld_k0 + k)
-                               : gA + (int64_t)(ld_k0 + k) * sg.lda + (m0 + r);
-        cp_async16((uint32_t)__cvta_generic_to_shared(sA + LA::at(r, k)), src, ok ? 16 : 0);
-      }
-      // B tile: BK x BN cols
-#pragma unroll
-      for (int idx = tid; idx < BN * BK; idx += NT) {
-        int c, k;
-        if (B_KMINOR) { c = idx / BK; k = idx % BK; } else { k = idx / BN; c = idx % BN; }
-        const bool ok = (c < nrem) && (k < kleft);
-        const cplx* src = gB;
-        if (ok) src = B_KMINOR ? gB + (int64_t)(n0 + c) * sg.ldb + (ld_k0 + k)
-                               : gB + (int64_t)(ld_k0 + k) * sg.ldb + (n0 + c);
-        cp_async16((uint32_t)__cvta_generic_to_shared(sB + LB::at(c, k)), src, ok ? 16 : 0);
-      }
-      ld_k0 += BK;
-      if (ld_k0 >= sg.K) { ld_k0 = 0; ++ld_seg; }
-    }
-    cp_async_commit();
-  };
-
-#pragma unroll
-  for (int s = 0; s < STAGES - 1; ++s) load_chunk(s);
-
-  int stage = 0;
-  while (cp_seg < seg_end) {
-    cp_async_wait<STAGES - 2>();
-    __syncthreads();
-    {
-      int ld_stage = stage + STAGES - 1;
-      if (ld_stage >= STAGES) ld_stage -= STAGES;
-      load_chunk(ld_stage);
-    }
-    const GemmSeg sg = segs[cp_seg];
-    const double alpha = sg.alpha;
-    const int kvalid = sg.K - cp_k0;  // > 0
-    const int nk4 = kvalid >= BK ? BK / 4 : (kvalid + 3) >> 2;
-    const cplx* sA = smem + stage * STAGE_ELEMS;
-    const cplx* sB = sA + LA::elems;
-    const int fr = lane >> 2, fk = lane & 3;
-#pragma unroll
-    for (int kk = 0; kk < BK / 4; ++kk) {
-      if (kk < nk4) {
-        double a_re[MT], a_im[MT], a_nim[MT];
-#pragma unroll
-        for (int i = 0; i < MT; ++i) {
-          if (i < mt_valid) {
-            const cplx v = sA[LA::at(wm0 + i * 8 + fr, kk * 4 + fk)];
-            a_re[i] = alpha * v.x;
-            const double im = alpha * v.y;
-            a_im[i] = (OPA == OPA_N) ? im : -im;  // conj for OPA_C / OPA_H
-            a_nim[i] = -a_im[i];
-          }
-        }
-#pragma unroll
-        for (int j = 0; j < NTL; ++j) {
-          if (j < nt_valid) {
-            const cplx b = sB[LB::at(wn0 + j * 8 + fr, kk * 4 + fk)];
-#pragma unroll
-            for (int i = 0; i < MT; ++i) {
-              if (i < mt_valid) {
-                dmma884(acc_re[i][j][0], acc_re[i][j][1], a_re[i], b.x);
-                dmma884(acc_im[i][j][0], acc_im[i][j][1], a_re[i], b.y);
-                dmma884(acc_re[i][j][0], acc_re[i][j][1], a_nim[i], b.y);
-                dmma884(acc_im[i][j][0], acc_im[i][j][1], a_im[i], b.x);
-              }
-            }
-          }
-        }
-      }
-    }
-    cp_k0 += BK;
-    if (cp_k0 >= sg.K) { cp_k0 = 0; ++cp_seg; }
-    stage = stage + 1 == STAGES ? 0 : stage + 1;
-  }
-  cp_async_wait<0>();
-
-  // ---- epilogue: thread holds C[row = lane/4][col = (lane%4)*2 + {0,1}] of every sub-tile
-  cplx* gC = Cbase + out.c_off;
-  const int er = lane >> 2, ec = (lane & 3) * 2;
-#pragma unroll
-  for (int i = 0; i < MT; ++i) {
-    const int r = m0 + wm0 + i * 8 + er;
-    if (i < mt_valid && r < M) {
-#pragma unroll
-      for (int j = 0; j < NTL; ++j) {
-        const int c = n0 + wn0 + j * 8 + ec;
-        if (j < nt_valid) {
-          cplx* p = gC + (int64_t)r * N + c;
-          if (c < N) p[0] = make_double2(acc_re[i][j][0], acc_im[i][j][0]);
-          if (c + 1 < N) p[1] = make_double2(acc_re[i][j][1], acc_im[i][j][1]);
-        }
-      }
-    }
-  }
-}
-
-template <int BM, int BN, int WARPS_M, int WARPS_N, int STAGES>
-static void launch_variant(const Stage& st, const GemmTile* d_tiles, int ntiles, const cplx* A, const cplx* B,
-                           cplx* C, cudaStream_t s) {
-  if (ntiles == 0) return;
-  constexpr int NT = WARPS_M * WARPS_N * 32;
-#define FH_LAUNCH(OA, OB)                                                                          \
-  {                                                                                                \
-    constexpr bool AK = (OA != OPA_H);                                                             \
-    constexpr bool BKM = (OB == OPB_T);                                                            \
-    constexpr size_t smem = (size_t)STAGES * (TileLayout<BM, AK>::elems + TileLayout<BN, BKM>::elems) * sizeof(cplx); \
-    auto kern = grouped_zgemm_kernel<BM, BN, WARPS_M, WARPS_N, OA, OB, STAGES>;                    \
-    static bool attr_done = false;                                                                 \
-    if (!attr_done) {                                                                              \
-      cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);          \
-      attr_done = true;                                                                            \
-    }                                                                                              \
-    kern<<<ntiles, NT, smem, s>>>(d_tiles, st.d_outs, st.d_segs, A, B, C);                          \
-  }
-  if (st.opA == OPA_N && st.opB == OPB_N) FH_LAUNCH(OPA_N, OPB_N)
-  else if (st.opA == OPA_N && st.opB == OPB_T) FH_LAUNCH(OPA_N, OPB_T)
-  else if (st.opA == OPA_C && st.opB == OPB_N) FH_LAUNCH(OPA_C, OPB_N)
-  else if (st.opA == OPA_H && st.opB == OPB_N) FH_LAUNCH(OPA_H, OPB_N)
-#undef FH_LAUNCH
-}
-
-void launch_grouped_gemm(const Stage& st, const cplx* A, const cplx* B, cplx* C, cudaStream_t s,
-                         int64_t* lc) {
-  if (!st.tiles64.empty()) {
-    launch_variant<64, 64, 2, 2, 4>(st, st.d_tiles64, (int)st.tiles64.size(), A, B, C, s);
-    ++*lc;
-  }
-  if (!st.tiles32.empty()) {
-    launch_variant<32, 32, 2, 2, 4>(st, st.d_tiles32, (int)st.tiles32.size(), A, B, C, s);
-    ++*lc;
-  }
 }
 
 // ------------------------------------------------------------------------------------------

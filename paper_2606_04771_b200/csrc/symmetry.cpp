@@ -154,6 +154,66 @@ void mpo_site_table(int site, double t_h, double U, MpoSite& W) {
 }
 
 // ----------------------------------------------------------------------------- stage assembly
+// Unit decomposition: every output block is cut into warp units of
+// (8 mt) x (8 nt) elements, mt * nt <= GEMM_MAX_SUBTILES, chosen per block so that (i) only the
+// last row / column of 8x8 sub-tiles is padded, (ii) one unit issues at most ~GEMM_UNIT_DMMA_CAP
+// DMMAs (long-K blocks get smaller units so that there are enough of them to fill 148 SMs), and
+// (iii) the number of operand fragments loaded per DMMA is minimal under (i) and (ii).
+static const int GEMM_MAX_SUBTILES = 16;
+static const int GEMM_MAX_DIM = 8;
+static const int GEMM_UNIT_DMMA_CAP = 3072;
+
+static void emit_units(Stage& st) {
+  struct UW {
+    GemmUnit u;
+    int64_t work;
+  };
+  std::vector<UW> v;
+  st.dmma_padded = 0;
+  for (size_t oi = 0; oi < st.outs.size(); ++oi) {
+    const GemmOut& o = st.outs[oi];
+    if (o.M <= 0 || o.N <= 0) continue;
+    const int M8 = (o.M + 7) / 8, N8 = (o.N + 7) / 8;
+    const int s_t = std::min(GEMM_MAX_SUBTILES, std::max(2, GEMM_UNIT_DMMA_CAP / std::max(1, 4 * o.steps)));
+    int best_h = 1, best_w = 1;
+    long best_cost = -1, best_units = 0;
+    for (int h = 1; h <= std::min(GEMM_MAX_DIM, M8); ++h) {
+      const int g = (M8 + h - 1) / h, hm = (M8 + g - 1) / g;
+      const int wmax = std::min(GEMM_MAX_DIM, s_t / hm);
+      if (wmax < 1) continue;
+      const int nu = (N8 + wmax - 1) / wmax;
+      const long cost = (long)nu * M8 + (long)g * N8, nun = (long)nu * g;  // fragments loaded per k-step
+      if (best_cost < 0 || cost < best_cost || (cost == best_cost && nun < best_units)) {
+        best_cost = cost;
+        best_units = nun;
+        best_h = hm;
+        best_w = wmax;
+      }
+    }
+    const int g = (M8 + best_h - 1) / best_h, nu = (N8 + best_w - 1) / best_w;
+    int m8 = 0;
+    for (int i = 0; i < g; ++i) {
+      const int h = M8 / g + (i < M8 % g ? 1 : 0);
+      int n8 = 0;
+      for (int j = 0; j < nu; ++j) {
+        const int w = N8 / nu + (j < N8 % nu ? 1 : 0);
+        UW x;
+        x.u = GemmUnit{o.c_off, o.ldc, o.M, o.N, o.seg_begin, o.seg_end, o.steps, m8 * 8, n8 * 8, h * 16 + w, 0};
+        x.work = (int64_t)h * w * std::max(1, o.steps);
+        st.dmma_padded += 4 * (int64_t)h * w * o.steps;
+        v.push_back(x);
+        n8 += w;
+      }
+      m8 += h;
+    }
+  }
+  // heaviest first: the hardware CTA scheduler (one unit per one-warp CTA) then balances greedily
+  std::stable_sort(v.begin(), v.end(), [](const UW& a, const UW& b) { return a.work > b.work; });
+  st.units.clear();
+  st.units.reserve(v.size());
+  for (auto& x : v) st.units.push_back(x.u);
+}
+
 void finalize_stage(Stage& st, const BlockTensor& out, const BlockTensor& lhs, const BlockTensor& rhs) {
   const size_t nt = st.t_out.size();
   st.outs.resize(out.keys.size());
@@ -165,53 +225,49 @@ void finalize_stage(Stage& st, const BlockTensor& out, const BlockTensor& lhs, c
     go.c_off = out.off[o];
     go.M = out.rows[o];
     go.N = out.cols[o];
+    go.ldc = out.cols[o];
+    go.steps = 0;
     go.seg_begin = (int)t;
     while (t < nt && st.t_out[t] == (int)o) {
       const int l = st.t_lhs[t], r = st.t_rhs[t];
       GemmSeg& sg = st.segs[t];
       sg.a_off = lhs.off[l];
       sg.b_off = rhs.off[r];
-      sg.lda = lhs.cols[l];
-      sg.ldb = rhs.cols[r];
       sg.pad = 0;
       sg.alpha = st.t_alpha[t];
       int M, K, K2, N;
-      if (st.opA == OPA_H) { M = lhs.cols[l]; K = lhs.rows[l]; } else { M = lhs.rows[l]; K = lhs.cols[l]; }
-      if (st.opB == OPB_T) { N = rhs.rows[r]; K2 = rhs.cols[r]; } else { N = rhs.cols[r]; K2 = rhs.rows[r]; }
+      if (st.opA == OPA_H) {  // stored K x M
+        M = lhs.cols[l];
+        K = lhs.rows[l];
+        sg.a_sm = 1;
+        sg.a_sk = lhs.cols[l];
+      } else {  // stored M x K
+        M = lhs.rows[l];
+        K = lhs.cols[l];
+        sg.a_sm = lhs.cols[l];
+        sg.a_sk = 1;
+      }
+      if (st.opB == OPB_T) {  // stored N x K
+        N = rhs.rows[r];
+        K2 = rhs.cols[r];
+        sg.b_sk = 1;
+        sg.b_sn = rhs.cols[r];
+      } else {  // stored K x N
+        N = rhs.cols[r];
+        K2 = rhs.rows[r];
+        sg.b_sk = rhs.cols[r];
+        sg.b_sn = 1;
+      }
       if (M != go.M || N != go.N || K != K2) throw std::runtime_error("task list: block shapes do not match");
       sg.K = K;
+      go.steps += (K + 3) / 4;
       st.flops += (int64_t)8 * M * N * K;
       ++t;
     }
     go.seg_end = (int)t;
   }
   if (t != nt) throw std::runtime_error("task list: tasks not sorted by output id");
-  // tile queues, heaviest tiles first (the hardware CTA scheduler then balances greedily)
-  struct TW {
-    GemmTile tile;
-    int64_t work;
-  };
-  std::vector<TW> t64, t32;
-  for (size_t o = 0; o < st.outs.size(); ++o) {
-    const GemmOut& go = st.outs[o];
-    int64_t ksum = 0;
-    for (int s = go.seg_begin; s < go.seg_end; ++s) ksum += (st.segs[s].K + 3) / 4 * 4;
-    const bool small = (go.M <= 32 || go.N <= 32);
-    const int T = small ? 32 : 64;
-    for (int m0 = 0; m0 < go.M; m0 += T)
-      for (int n0 = 0; n0 < go.N; n0 += T) {
-        const int mv = (std::min(T, go.M - m0) + 7) / 8 * 8, nv = (std::min(T, go.N - n0) + 7) / 8 * 8;
-        TW tw{GemmTile{(int)o, m0, n0, 0}, (int64_t)mv * nv * (ksum + 8)};
-        (small ? t32 : t64).push_back(tw);
-      }
-  }
-  auto by_work = [](const TW& a, const TW& b) { return a.work > b.work; };
-  std::stable_sort(t64.begin(), t64.end(), by_work);
-  std::stable_sort(t32.begin(), t32.end(), by_work);
-  st.tiles64.clear();
-  st.tiles32.clear();
-  for (auto& x : t64) st.tiles64.push_back(x.tile);
-  for (auto& x : t32) st.tiles32.push_back(x.tile);
+  emit_units(st);
 }
 
 namespace {

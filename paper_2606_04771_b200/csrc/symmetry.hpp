@@ -20,7 +20,7 @@ void layout_theta(const Bond& bl, const Bond& br, BlockTensor& out);
 void mpo_site_table(int site, double t_h, double U, MpoSite& out);
 
 // Task lists.  Each emitter fills the intermediate tensor layout (Z / X / Y), the output layout
-// where it is not given, and the two stages (host task arrays + GemmOut/GemmSeg + tile queues).
+// where it is not given, and the two stages (host task arrays + GemmOut/GemmSeg + warp-unit list).
 // two-site apply (H1 + H2): vec = theta layout (input and output)
 void emit_heff2(const BlockTensor& Lenv, const BlockTensor& Renv, const BlockTensor& vec, const MpoSite& W1,
                 const MpoSite& W2, BlockTensor& Z, Stage& st1, Stage& st2);
@@ -39,7 +39,7 @@ void emit_merge(const BlockTensor& A1, const BlockTensor& A2, const BlockTensor&
 // N layouts use key {q, tj}.
 void emit_norm_env(const BlockTensor& Nenv, const BlockTensor& A, BlockTensor& Nout, Stage& st1, Stage& st2);
 
-// fills outs/segs from the (sorted) task arrays and builds the tile queues
+// fills outs/segs from the (sorted) task arrays and builds the warp-unit list
 void finalize_stage(Stage& st, const BlockTensor& out, const BlockTensor& lhs, const BlockTensor& rhs);
 
 }  // namespace fh
