@@ -354,6 +354,7 @@ int fh_ctx_create(fh_ctx** out, void* cuda_stream, void* arena_dev, size_t arena
     FH_CUDA(cudaGetDeviceCount(&ndev));
     FH_REQUIRE(ndev > 0, FH_ECUDA, "no CUDA device");
     c->stream = (cudaStream_t)cuda_stream;
+    FH_CUDA(cudaGetDevice(&c->device));
     if (arena_dev) {
       c->arena = (cplx*)arena_dev;
     } else {
@@ -380,9 +381,16 @@ void fh_ctx_destroy(fh_ctx* c) {
   for (auto e : c->ev_free) cudaEventDestroy(e);
   c->plan.pool.destroy();
   c->pool_aux.destroy();
-  if (c->cusolver) cusolverDnDestroy(c->cusolver);
-  if (c->svd_work) cudaFree(c->svd_work);
-  if (c->d_info) cudaFree(c->d_info);
+  for (auto& w : c->svd_workers) {
+    if (w.s) cudaStreamSynchronize(w.s);
+    if (w.h) cusolverDnDestroy(w.h);
+    if (w.params) cusolverDnDestroyParams(w.params);
+    if (w.dwork) cudaFree(w.dwork);
+    if (w.d_info) cudaFree(w.d_info);
+    if (w.done) cudaEventDestroy(w.done);
+    if (w.s) cudaStreamDestroy(w.s);
+  }
+  if (c->svd_fork) cudaEventDestroy(c->svd_fork);
   if (c->h_pinned) cudaFreeHost(c->h_pinned);
   if (c->own_arena) cudaFree(c->arena);
   delete c;

@@ -101,11 +101,23 @@ struct fh_ctx {
   };
   std::vector<Span> spans;
   std::vector<cudaEvent_t> ev_free;
-  // SVD
-  cusolverDnHandle_t cusolver = nullptr;
-  void* svd_work = nullptr;
-  size_t svd_work_bytes = 0;
-  int* d_info = nullptr;
+  // SVD (H9): one cuSOLVER handle + stream + workspace per host worker thread; the sector SVDs of a
+  // bond are independent and cuSOLVER's SVD drivers block their calling thread, so concurrency needs
+  // host threads (tdvp.cu, run_sector_svds)
+  struct SvdWorker {
+    cusolverDnHandle_t h = nullptr;
+    cusolverDnParams_t params = nullptr;
+    cudaStream_t s = nullptr;
+    void* dwork = nullptr;
+    size_t dwork_bytes = 0;
+    std::vector<char> hwork;
+    int* d_info = nullptr;
+    cudaEvent_t done = nullptr;
+  };
+  std::vector<SvdWorker> svd_workers;
+  cudaEvent_t svd_fork = nullptr;
+  int device = 0;
+  int64_t svd_count[3] = {0, 0, 0};  // gesvd, gesvdp, gesvdp fallbacks to gesvd
   // last sweep statistics
   double stat_disc = 0.0;
   int stat_chi = 0, stat_su2 = 0, stat_dmax = 0;
