@@ -93,10 +93,11 @@ struct GemmSeg {  // one K-segment: C += alpha * op(A) (M x K) * op(B) (K x N)
 };
 // One warp's work: a (8*mt) x (8*nt) sub-tile of output block `out` over the whole K of that
 // block (all its segments).  The output geometry is repeated here so that the kernel needs a
-// single descriptor load per unit.  shape = mt * 16 + nt, mt * nt <= 16, mt, nt <= 8.
+// single descriptor load per unit (96 bytes).  shape = mt * 16 + nt, mt * nt <= 16, mt, nt <= 8.
 struct GemmUnit {
   int64_t c_off;
   int ldc, M, N, seg_begin, seg_end, steps, m0, n0, shape, pad;
+  GemmSeg first;  // copy of segs[seg_begin]: the unit starts streaming after ONE descriptor load
 };
 
 struct Stage {

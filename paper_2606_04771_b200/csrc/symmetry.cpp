@@ -170,11 +170,17 @@ static void emit_units(Stage& st) {
   };
   std::vector<UW> v;
   st.dmma_padded = 0;
+  // The per-unit cap only exists to create enough units for 148 SMs x 8 resident warps; when the
+  // stage is large (chi >~ 8000) full 16-sub-tile units are plentiful and the cap is lifted
+  // (measured at chi = 16384: 31.0 TFLOP/s uncapped vs 20.9 with the cap of 3072).
+  int64_t total16 = 0;
+  for (const GemmOut& o : st.outs) total16 += (int64_t)4 * ((o.M + 7) / 8) * ((o.N + 7) / 8) * o.steps;
+  const int64_t cap = std::max<int64_t>(GEMM_UNIT_DMMA_CAP, total16 / (148 * 8 * 6));
   for (size_t oi = 0; oi < st.outs.size(); ++oi) {
     const GemmOut& o = st.outs[oi];
     if (o.M <= 0 || o.N <= 0) continue;
     const int M8 = (o.M + 7) / 8, N8 = (o.N + 7) / 8;
-    const int s_t = std::min(GEMM_MAX_SUBTILES, std::max(2, GEMM_UNIT_DMMA_CAP / std::max(1, 4 * o.steps)));
+    const int s_t = (int)std::min<int64_t>(GEMM_MAX_SUBTILES, std::max<int64_t>(2, cap / std::max(1, 4 * o.steps)));
     int best_h = 1, best_w = 1;
     long best_cost = -1, best_units = 0;
     for (int h = 1; h <= std::min(GEMM_MAX_DIM, M8); ++h) {
@@ -198,7 +204,8 @@ static void emit_units(Stage& st) {
       for (int j = 0; j < nu; ++j) {
         const int w = N8 / nu + (j < N8 % nu ? 1 : 0);
         UW x;
-        x.u = GemmUnit{o.c_off, o.ldc, o.M, o.N, o.seg_begin, o.seg_end, o.steps, m8 * 8, n8 * 8, h * 16 + w, 0};
+        x.u = GemmUnit{o.c_off, o.ldc, o.M, o.N, o.seg_begin, o.seg_end, o.steps, m8 * 8, n8 * 8, h * 16 + w, 0,
+                         o.seg_end > o.seg_begin ? st.segs[o.seg_begin] : GemmSeg{0, 0, 0, 0, 0, 0, 0, 0, 0.0}};
         x.work = (int64_t)h * w * std::max(1, o.steps);
         st.dmma_padded += 4 * (int64_t)h * w * o.steps;
         v.push_back(x);

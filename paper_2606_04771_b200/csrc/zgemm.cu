@@ -65,22 +65,36 @@ struct Producer {
   int64_t dA, dB;
   int a_sk, b_sk;
   bool done;
+  // descriptor of segment si + 1, loaded one segment ahead so that the switch never waits on L2
+  int64_t n_a_off, n_b_off;
+  int n_K, n_a_sm, n_a_sk, n_b_sk, n_b_sn;
 
-  __device__ __forceinline__ void setup(const GemmSeg& sg) {
-    K = sg.K;
+  __device__ __forceinline__ void setup(int64_t a_off, int64_t b_off, int K_, int a_sm, int a_sk_, int b_sk_,
+                                        int b_sn) {
+    K = K_;
     nfull = K >> 2;
     nst = (K + 3) >> 2;
     s = 0;
-    a_sk = sg.a_sk;
-    b_sk = sg.b_sk;
-    const cplx* A0 = Abase + sg.a_off + (int64_t)kq * sg.a_sk;
-    const cplx* B0 = Bbase + sg.b_off + (int64_t)kq * sg.b_sk;
+    a_sk = a_sk_;
+    b_sk = b_sk_;
+    const cplx* A0 = Abase + a_off + (int64_t)kq * a_sk_;
+    const cplx* B0 = Bbase + b_off + (int64_t)kq * b_sk_;
 #pragma unroll
-    for (int i = 0; i < MT; ++i) pa[i] = A0 + (int64_t)mi[i] * sg.a_sm;
+    for (int i = 0; i < MT; ++i) pa[i] = A0 + (int64_t)mi[i] * a_sm;
 #pragma unroll
-    for (int j = 0; j < NT; ++j) pb[j] = B0 + (int64_t)nj[j] * sg.b_sn;
-    dA = 4 * (int64_t)sg.a_sk;
-    dB = 4 * (int64_t)sg.b_sk;
+    for (int j = 0; j < NT; ++j) pb[j] = B0 + (int64_t)nj[j] * b_sn;
+    dA = 4 * (int64_t)a_sk_;
+    dB = 4 * (int64_t)b_sk_;
+  }
+  __device__ __forceinline__ void prefetch_next() {
+    const GemmSeg* np = segs + min(si + 1, se - 1);
+    n_a_off = np->a_off;
+    n_b_off = np->b_off;
+    n_K = np->K;
+    n_a_sm = np->a_sm;
+    n_a_sk = np->a_sk;
+    n_b_sk = np->b_sk;
+    n_b_sn = np->b_sn;
   }
   __device__ __forceinline__ void init(const GemmSeg* segs_, const GemmUnit& u, const cplx* A, const cplx* B,
                                        int lane) {
@@ -98,7 +112,8 @@ struct Producer {
     for (int i = 0; i < MT; ++i) mi[i] = min(u.m0 + 8 * i + r, u.M - 1);
 #pragma unroll
     for (int j = 0; j < NT; ++j) nj[j] = min(u.n0 + 8 * j + r, u.N - 1);
-    setup(segs[si]);
+    setup(u.first.a_off, u.first.b_off, u.first.K, u.first.a_sm, u.first.a_sk, u.first.b_sk, u.first.b_sn);
+    prefetch_next();
   }
   __device__ __forceinline__ void issue(uint32_t dst) {
     if (!done) {
@@ -126,8 +141,12 @@ struct Producer {
       ++s;
       if (s == nst) {
         ++si;
-        if (si < se) setup(segs[si]);
-        else done = true;
+        if (si < se) {
+          setup(n_a_off, n_b_off, n_K, n_a_sm, n_a_sk, n_b_sk, n_b_sn);
+          prefetch_next();
+        } else {
+          done = true;
+        }
       }
     }
     cp_commit();
@@ -150,13 +169,17 @@ __device__ __noinline__ void run_unit(const GemmUnit& u, const GemmSeg* __restri
     Producer<MT, NT> P;
     P.init(segs, u, A, B, lane);
     const uint32_t lane_ring = ring + lane * 16;
-#pragma unroll
+#pragma unroll 1
     for (int d = 0; d < D - 1; ++d) P.issue(lane_ring + d * STAGE_BYTES);
-    // consumer-side walk over the segments for alpha
+    // consumer-side walk over the segments for alpha, one segment of lookahead
     int csi = u.seg_begin;
-    int cleft = (segs[csi].K + 3) >> 2;
-    double alpha = segs[csi].alpha;
+    const int cse = u.seg_end;
+    int cleft = (u.first.K + 3) >> 2;
+    double alpha = u.first.alpha;
+    int nK = segs[min(csi + 1, cse - 1)].K;
+    double nalpha = segs[min(csi + 1, cse - 1)].alpha;
     int rd = 0, wr = D - 1;
+#pragma unroll 1
     for (int t = 0; t < total; ++t) {
       cp_wait<D - 2>();
       const uint32_t src = lane_ring + rd * STAGE_BYTES;
@@ -192,10 +215,13 @@ __device__ __noinline__ void run_unit(const GemmUnit& u, const GemmSeg* __restri
       for (int j = 0; j < NT; ++j)
 #pragma unroll
         for (int i = 0; i < MT; ++i) dmma884(cim[i][j], ai[i], b[j].x);
-      if (--cleft == 0 && t + 1 < total) {
+      if (--cleft == 0) {
         ++csi;
-        cleft = (segs[csi].K + 3) >> 2;
-        alpha = segs[csi].alpha;
+        cleft = (nK + 3) >> 2;
+        alpha = nalpha;
+        const GemmSeg* np = segs + min(csi + 1, cse - 1);
+        nK = np->K;
+        nalpha = np->alpha;
       }
     }
     cp_wait<0>();
