@@ -40,8 +40,9 @@ def parse_args():
     ap.add_argument("--s2-scale", default="1/6", help="num/den scale of Table S2 degeneracies")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-flush", action="store_true", help="do not flush L2 between timed applies")
-    ap.add_argument("--sweep", action="store_true", help="also time one full tdvp2_sweep at --sweep-chi")
-    ap.add_argument("--sweep-chi", type=int, default=1024)
+    ap.add_argument("--no-sweep", action="store_true", help="skip the timed tdvp2_sweep (second half of the metric)")
+    ap.add_argument("--sweep", action="store_true", help="(default on) time one full tdvp2_sweep at --sweep-chi")
+    ap.add_argument("--sweep-chi", type=int, default=4096)
     return ap.parse_args()
 
 
@@ -295,7 +296,7 @@ def run_ours(args):
                 "h2d_bytes_per_step": zbytes, "d2h_bytes_per_step": zbytes, "api": "heff_apply_host (pinned host buffers)"},
         "gpu_launches": int(launches), "clocks": clk, "wall_seconds_timed_region": wall,
     }
-    if args.sweep:
+    if not args.no_sweep and world == 1:
         out["sweep"] = run_sweep(ctx, H, mpo, args)
     if not args.no_cpu_baseline:
         cb, _ = time_oracle(args, 3, 1)

@@ -289,6 +289,34 @@ def test_config1_neel_quench_L8_vs_oracle(H, ctx):
     ctx.mps_destroy(mps)
 
 
+def test_config4_L60_U0_quench_vs_closed_form(H, ctx):
+    """configs[3] shape at U=0: L=60 Neel quench, dt=0.05, m=10, eps_trunc=1e-12 (chi grows as the
+    entanglement demands), against the free-fermion closed form O-U0 (oracle/u0.py: single-particle
+    propagator of the open chain) -- a pin of the large-L symmetric code path that does not go
+    through the symmetric oracle.  The residual is the TDVP2 splitting error at dt=0.05 (O(dt^2) per
+    unit time, measured ~1e-6 at L=8 against ED) plus the 1e-12 truncation; n_i = 1 must hold to
+    rounding (reading A-12) and the norm and energy (= 0 for the Neel state at any U) stay put."""
+    from oracle import u0
+    L, t_h, dt, nstep, m = 60, 1.0, 0.05, 8, 10
+    mpo = ctx.fh_mpo_build(L, t_h, 0.0)
+    mps = ctx.mps_init_neel(mpo, L)
+    worst = 0.0
+    for step in range(1, nstep + 1):
+        ctx.tdvp2_sweep(mpo, mps, dt, krylov_dim=m, chi_max_full=4096, eps_trunc=1e-12)
+        got = ctx.measure_local(mps, L)
+        ref = u0.observables(L, t_h, step * dt)
+        assert np.abs(got["n"] - 1.0).max() < 1e-10
+        worst = max(worst, np.abs(got["sz"] - ref["sz"]).max(), np.abs(got["docc"] - ref["docc"]).max())
+        g = ctx.measure_global(mpo, mps)
+        assert abs(g["norm2"] - 1.0) < 1e-8 and abs(g["energy"]) < 1e-7
+    st = ctx.tdvp2_last_stats()
+    print("L=60 U=0: max |obs - closed form| = %.2e, chi reached %d (chi_su2 %d), discarded %.1e"
+          % (worst, st["chi_full"], st["chi_su2"], st["max_discarded"]))
+    assert worst < 2e-5, worst
+    assert st["max_discarded"] < 1e-10
+    ctx.mps_destroy(mps)
+
+
 # ------------------------------------------------------------------ edge cases and errors
 def test_edge_cases_and_error_codes(H, ctx):
     B = H.binding
