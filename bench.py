@@ -27,6 +27,8 @@ NOMINAL_FP64_TF = 40.0      # B200 dense FP64 (tensor = vector) nominal, HGX B20
 NOMINAL_BF16_TF = 2250.0    # guide: 2.25 PFLOP/s dense bf16
 FALLBACK_BF16_TF = 1590.0   # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 FALLBACK_HBM_GBS = 6650.0
+# one ncu --set full capture of the default workload (profiles/r1_heff_apply_ncu.md), bytes per launch
+NCU_DRAM_BYTES_PER_LAUNCH = 0.5 * (16.166144e6 + 1.224448e6 + 36.569344e6 + 0.709632e6)
 
 
 def parse_args():
@@ -202,7 +204,7 @@ def run_ours(args):
     L, c = 60, 29
     chi = args.chi
     # replicas only (north_star: one GPU, no sharding, no collectives): every rank runs the same bond
-    arena = int(min(160e9, max(2 << 30, 64.0 * chi * chi)))
+    arena = int(min(160e9, max(16 << 30, 64.0 * chi * chi)))
     ctx = H.binding.Context(arena, device="cuda:%d" % local)
     mpo = ctx.fh_mpo_build(L, 1.0, 4.0)
     t_build = time.perf_counter()
@@ -291,11 +293,22 @@ def run_ours(args):
                      "peak_rule": peak_rule, "frac_rule": per_gpu_tf / peak_rule,
                      "peak_rule_source": "%s bf16 %.1f TF x nominal fp64/bf16 %g/%g" % (
                          pk["source"], pk["bf16"], NOMINAL_FP64_TF, NOMINAL_BF16_TF),
-                     "frac_l2_warm": flops * args.steps / t_warm * 1e-12 / peak_dmma, "traffic": None},
+                     "frac_l2_warm": flops * args.steps / t_warm * 1e-12 / peak_dmma,
+                     "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (chi == 4096 and args.profile == "gaussian") else None,
+                     "traffic_source": "profiles/r1_heff_apply_ncu.md: dram__bytes_read.sum + dram__bytes_write.sum, mean of the stage-1 and stage-2 launch (17.4 MB and 37.3 MB); algorithmic minimum 55 MB per launch pair / 2"},
         "e2e": {"value": world * flops * args.steps / t_e2e * 1e-9, "unit": "GFLOP/s",
                 "h2d_bytes_per_step": zbytes, "d2h_bytes_per_step": zbytes, "api": "heff_apply_host (pinned host buffers)"},
         "gpu_launches": int(launches), "clocks": clk, "wall_seconds_timed_region": wall,
     }
+    # H6 / H8: the HBM-bound vector and pack kernels, in isolation, on a Krylov basis the size of
+    # chi = 49152's theta (64 Mi elements = 1 GiB per vector: far beyond L2), against the measured copy peak
+    try:
+        nvec = 1 << 26 if arena >= (14 << 30) else 1 << 22
+        g = ctx.fh_vec_kernels_gbs(nvec, m=10, reps=5)
+        out["hbm_kernels"] = {"elements": nvec, "unit": "GB/s", "peak": pk["hbm"], "peak_source": pk["source"],
+                              "achieved": g, "frac": {k: v / pk["hbm"] for k, v in g.items()}}
+    except H.binding.FhError as e:
+        out["hbm_kernels"] = {"error": str(e)}
     if not args.no_sweep and world == 1:
         out["sweep"] = run_sweep(ctx, H, mpo, args)
     if not args.no_cpu_baseline:

@@ -43,6 +43,7 @@ _SIGS = {
     "mps_get_site": (c_int, [c_void_p, c_void_p, c_int, c_void_p, c_int]),
     "mps_get_svals": (c_int, [c_void_p, c_int, P(c_int), c_void_p]),
     "fh_dmma_peak_tflops": (c_int, [c_void_p, c_int, P(c_dbl)]),
+    "fh_vec_kernels_gbs": (c_int, [c_void_p, c_i64, c_int, c_int, P(c_dbl)]),
     "mps_drop_site": (c_int, [c_void_p, c_void_p, c_int]),
     "heff_apply_host": (c_int, [c_void_p, c_void_p, c_void_p]),
     "env_update_left": (c_int, [c_void_p, c_void_p, c_void_p, c_int]),
@@ -242,6 +243,11 @@ class Context:
         t = c_dbl()
         self.check(lib.fh_dmma_peak_tflops(self.h, reps, C.byref(t)), "fh_dmma_peak_tflops")
         return t.value
+
+    def fh_vec_kernels_gbs(self, n_elems, m=10, reps=10):
+        g = (c_dbl * 6)()
+        self.check(lib.fh_vec_kernels_gbs(self.h, int(n_elems), int(m), int(reps), g), "fh_vec_kernels_gbs")
+        return dict(zip(("wdot", "axpy", "scale", "lincomb", "pack", "pack_transposed"), [float(v) for v in g]))
 
     def mps_drop_site(self, mps, site):
         self.check(lib.mps_drop_site(self.h, mps, site), "mps_drop_site")

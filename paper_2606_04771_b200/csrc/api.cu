@@ -878,6 +878,68 @@ int fh_dmma_peak_tflops(fh_ctx* ctx, int reps, double* tflops) {
   })
 }
 
+int fh_vec_kernels_gbs(fh_ctx* ctx, int64_t n, int m, int reps, double* gbs) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && gbs && n >= 65536 && m >= 1 && m <= 32 && reps > 0, FH_EINVAL, "fh_vec_kernels_gbs: bad argument");
+    const int64_t off = ctx->alloc.alloc((int64_t)(m + 3) * n);
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    try {
+      cudaStream_t s = ctx->stream;
+      cplx* V = ctx->ptr(off);
+      cplx* x = V + (int64_t)m * n;
+      cplx* y = x + n;
+      cplx* z = y + n;
+      launch_fill_zero(V, (int64_t)(m + 3) * n, s, &ctx->launches);
+      std::vector<VecChunk> ch;
+      for (int64_t st = 0; st < n; st += 8192) ch.push_back(VecChunk{st, (int)std::min<int64_t>(8192, n - st), 2.0f});
+      const int B = 256;
+      std::vector<CopyBlk> cb, cbt;
+      for (int64_t st = 0; st + (int64_t)B * B <= n; st += (int64_t)B * B) {
+        cb.push_back(CopyBlk{st, st, B, B, B, B, 0, 0, 1.25});
+        cbt.push_back(CopyBlk{st, st, B, B, B, B, 1, 0, 1.25});
+      }
+      ctx->pool_aux.reserve(ch.size() * (sizeof(VecChunk) + 16) + 2 * cb.size() * sizeof(CopyBlk) + 8192, s);
+      VecChunk* d_ch = upload(ctx->pool_aux, ch, s);
+      CopyBlk* d_cb = upload(ctx->pool_aux, cb, s);
+      CopyBlk* d_cbt = upload(ctx->pool_aux, cbt, s);
+      double* d_part = (double*)ctx->pool_aux.take(ch.size() * 2 * sizeof(double));
+      double* d_res = (double*)ctx->pool_aux.take(2 * sizeof(double));
+      FH_CUDA(cudaEventCreate(&e0));
+      FH_CUDA(cudaEventCreate(&e1));
+      std::vector<cplx> coef(m, make_double2(0.5, 0.25));
+      const double nb = (double)cb.size() * B * B;
+      const double bytes[6] = {32.0 * n, 48.0 * n, 32.0 * n, 16.0 * (m + 1) * n, 32.0 * nb, 32.0 * nb};
+      for (int k = 0; k < 6; ++k) {
+        for (int r = -2; r < reps; ++r) {
+          if (r == 0) FH_CUDA(cudaEventRecord(e0, s));
+          switch (k) {
+            case 0: launch_wdot(d_ch, (int)ch.size(), x, y, d_part, d_res, s, &ctx->launches); break;
+            case 1: launch_axpy(n, make_double2(0.5, 0.1), x, y, s, &ctx->launches); break;
+            case 2: launch_scale(n, make_double2(0.5, 0.1), x, z, s, &ctx->launches); break;
+            case 3: launch_lincomb(n, m, coef.data(), V, n, z, s, &ctx->launches); break;
+            case 4: launch_copy_blocks(d_cb, (int)cb.size(), x, z, s, &ctx->launches); break;
+            default: launch_copy_blocks(d_cbt, (int)cbt.size(), x, z, s, &ctx->launches); break;
+          }
+        }
+        FH_CUDA(cudaEventRecord(e1, s));
+        FH_CUDA(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        FH_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+        gbs[k] = bytes[k] * reps / (ms * 1e-3) * 1e-9;
+      }
+      FH_CUDA(cudaGetLastError());
+    } catch (...) {
+      if (e0) cudaEventDestroy(e0);
+      if (e1) cudaEventDestroy(e1);
+      ctx->alloc.release(off, (int64_t)(m + 3) * n);
+      throw;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    ctx->alloc.release(off, (int64_t)(m + 3) * n);
+  })
+}
+
 // host-only helpers for the CPU test-suite (symmetry layer without a GPU)
 static fh::Stage g_host_st1, g_host_st2;
 

@@ -165,14 +165,41 @@ __global__ void __launch_bounds__(256) copy_blocks_kernel(const CopyBlk* __restr
   const CopyBlk b = blks[blockIdx.x];
   const cplx* ps = src + b.src_off;
   cplx* pd = dst + b.dst_off;
-  const int64_t total = (int64_t)b.rows * b.cols;
-  for (int64_t i = (int64_t)blockIdx.y * 256 + threadIdx.x; i < total; i += (int64_t)gridDim.y * 256) {
-    const int r = (int)(i / b.cols), c = (int)(i % b.cols);
-    cplx v = ps[(int64_t)r * b.ld_src + c];
-    v.x *= b.scale;
-    v.y *= b.scale;
-    if (b.transpose_dst) pd[(int64_t)c * b.ld_dst + r] = v;
-    else pd[(int64_t)r * b.ld_dst + c] = v;
+  if (!b.transpose_dst) {
+    const int64_t total = (int64_t)b.rows * b.cols;
+    for (int64_t i = (int64_t)blockIdx.y * 256 + threadIdx.x; i < total; i += (int64_t)gridDim.y * 256) {
+      const int r = (int)(i / b.cols), c = (int)(i % b.cols);
+      cplx v = ps[(int64_t)r * b.ld_src + c];
+      v.x *= b.scale;
+      v.y *= b.scale;
+      pd[(int64_t)r * b.ld_dst + c] = v;
+    }
+    return;
+  }
+  // transposing copy: 32 x 32 tiles through shared memory so that both the reads (rows of src)
+  // and the writes (rows of dst) are contiguous 512-byte runs
+  __shared__ cplx tile[32][33];
+  const int tr = (b.rows + 31) >> 5, tc = (b.cols + 31) >> 5;
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;  // 32 x 8 threads
+  for (int t = blockIdx.y; t < tr * tc; t += gridDim.y) {
+    const int r0 = (t / tc) << 5, c0 = (t % tc) << 5;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const int r = r0 + ty + 8 * k, c = c0 + tx;
+      if (r < b.rows && c < b.cols) {
+        cplx v = ps[(int64_t)r * b.ld_src + c];
+        v.x *= b.scale;
+        v.y *= b.scale;
+        tile[ty + 8 * k][tx] = v;
+      }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const int c = c0 + ty + 8 * k, r = r0 + tx;  // dst row = src column
+      if (r < b.rows && c < b.cols) pd[(int64_t)c * b.ld_dst + r] = tile[tx][ty + 8 * k];
+    }
+    __syncthreads();
   }
 }
 void launch_copy_blocks(const CopyBlk* d_blks, int nblk, const cplx* src, cplx* dst, cudaStream_t s,
