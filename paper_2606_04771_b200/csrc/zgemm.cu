@@ -45,193 +45,173 @@ __device__ __forceinline__ cplx lds_c(uint32_t addr) {
   return v;
 }
 
-constexpr int RING_DEPTH = 3;     // cp.async stages in flight per warp
+constexpr int RING_DEPTH = 4;     // cp.async ring stages per warp (power of two)
 constexpr int MAX_FRAGS = 10;     // mt + nt <= 10 for every shape with mt * nt <= 16, mt, nt <= 8
 constexpr int RING_BYTES = RING_DEPTH * MAX_FRAGS * 512;
 
-// Producer side of one unit: walks the k-steps of all segments and issues the cp.asyncs of one
-// step (mt A fragments + nt B fragments, 16 B per lane each) into a ring stage.
+// One unit = the flattened k-step sequence of all segments of an output block.  Step t is consumed
+// (LDS + 4 mt nt DMMAs) while step t + D - 1 is being copied.  The sequence is cut into chunks inside
+// which neither the consumer nor the producer (D - 1 steps ahead) changes segment and the producer
+// copies only full 4-wide k-steps: the chunk loop carries no bookkeeping at all (per k-step: mt + nt
+// LDGSTS with their pointer updates, mt + nt LDS.128, 2 mt DMUL, one wait, one commit).  Ragged k
+// tails, segment switches and the drain run through the slow path, one step at a time.
 // Fragment layout of DMMA.8x8x4: lane l holds A[row l/4][k l%4] and B[k l%4][col l/4].
-template <int MT, int NT>
-struct Producer {
-  const GemmSeg* segs;
-  const cplx *Abase, *Bbase;
-  int si, se;
-  int s, nfull, nst, K;
-  int mi[MT], nj[NT];
-  int kq;
-  const cplx* pa[MT];
-  const cplx* pb[NT];
-  int64_t dA, dB;
-  int a_sk, b_sk;
-  bool done;
-  // descriptor of segment si + 1, loaded one segment ahead so that the switch never waits on L2
-  int64_t n_a_off, n_b_off;
-  int n_K, n_a_sm, n_a_sk, n_b_sk, n_b_sn;
-
-  __device__ __forceinline__ void setup(int64_t a_off, int64_t b_off, int K_, int a_sm, int a_sk_, int b_sk_,
-                                        int b_sn) {
-    K = K_;
-    nfull = K >> 2;
-    nst = (K + 3) >> 2;
-    s = 0;
-    a_sk = a_sk_;
-    b_sk = b_sk_;
-    const cplx* A0 = Abase + a_off + (int64_t)kq * a_sk_;
-    const cplx* B0 = Bbase + b_off + (int64_t)kq * b_sk_;
-#pragma unroll
-    for (int i = 0; i < MT; ++i) pa[i] = A0 + (int64_t)mi[i] * a_sm;
-#pragma unroll
-    for (int j = 0; j < NT; ++j) pb[j] = B0 + (int64_t)nj[j] * b_sn;
-    dA = 4 * (int64_t)a_sk_;
-    dB = 4 * (int64_t)b_sk_;
+// Rows / columns beyond the block edge re-read the last valid one: they only feed accumulator rows /
+// columns that are never stored.  Lanes with k >= K copy zero bytes and get zeros (cp.async zero fill).
+#define P_SETUP(AOFF, BOFF, KK, ASM, ASK, BSK, BSN)                         \
+  {                                                                         \
+    p_K = (KK);                                                             \
+    p_left = (p_K + 3) >> 2;                                                \
+    p_ask = (ASK);                                                          \
+    p_bsk = (BSK);                                                          \
+    const cplx* A0 = A + (AOFF) + (int64_t)kq * p_ask;                      \
+    const cplx* B0 = B + (BOFF) + (int64_t)kq * p_bsk;                      \
+    const int asm_ = (ASM), bsn_ = (BSN);                                   \
+    _Pragma("unroll") for (int i = 0; i < MT; ++i) pa[i] = A0 + (int64_t)mi[i] * asm_; \
+    _Pragma("unroll") for (int j = 0; j < NT; ++j) pb[j] = B0 + (int64_t)nj[j] * bsn_; \
+    dA = 4 * (int64_t)p_ask;                                                \
+    dB = 4 * (int64_t)p_bsk;                                                \
   }
-  __device__ __forceinline__ void prefetch_next() {
-    const GemmSeg* np = segs + min(si + 1, se - 1);
-    n_a_off = np->a_off;
-    n_b_off = np->b_off;
-    n_K = np->K;
-    n_a_sm = np->a_sm;
-    n_a_sk = np->a_sk;
-    n_b_sk = np->b_sk;
-    n_b_sn = np->b_sn;
+#define P_STEP_SLOW(DST)                                                                         \
+  {                                                                                              \
+    const uint32_t dst_ = (DST);                                                                 \
+    if (p_issued < total) {                                                                      \
+      const int k = 4 * (((p_K + 3) >> 2) - p_left) + kq;                                        \
+      const int back = k < p_K ? 0 : k - (p_K - 1);                                              \
+      const int sz = k < p_K ? 16 : 0;                                                           \
+      _Pragma("unroll") for (int i = 0; i < MT; ++i) {                                           \
+        cp_async16(dst_ + i * 512, pa[i] - (int64_t)back * p_ask, sz);                           \
+        pa[i] += dA;                                                                             \
+      }                                                                                          \
+      _Pragma("unroll") for (int j = 0; j < NT; ++j) {                                           \
+        cp_async16(dst_ + (MT + j) * 512, pb[j] - (int64_t)back * p_bsk, sz);                    \
+        pb[j] += dB;                                                                             \
+      }                                                                                          \
+      ++p_issued;                                                                                \
+      if (--p_left == 0 && p_issued < total) {                                                   \
+        ++p_si;                                                                                  \
+        const GemmSeg* sp = segs + p_si;                                                             \
+        P_SETUP(sp->a_off, sp->b_off, sp->K, sp->a_sm, sp->a_sk, sp->b_sk, sp->b_sn)             \
+      }                                                                                          \
+    }                                                                                            \
+    cp_commit();                                                                                 \
   }
-  __device__ __forceinline__ void init(const GemmSeg* segs_, const GemmUnit& u, const cplx* A, const cplx* B,
-                                       int lane) {
-    segs = segs_;
-    Abase = A;
-    Bbase = B;
-    si = u.seg_begin;
-    se = u.seg_end;
-    kq = lane & 3;
-    done = false;
-    const int r = lane >> 2;
-    // rows / columns beyond the block edge re-read the last valid one: they only feed accumulator
-    // rows / columns that are never stored
-#pragma unroll
-    for (int i = 0; i < MT; ++i) mi[i] = min(u.m0 + 8 * i + r, u.M - 1);
-#pragma unroll
-    for (int j = 0; j < NT; ++j) nj[j] = min(u.n0 + 8 * j + r, u.N - 1);
-    setup(u.first.a_off, u.first.b_off, u.first.K, u.first.a_sm, u.first.a_sk, u.first.b_sk, u.first.b_sn);
-    prefetch_next();
+#define CONSUME(SRC, AL, ALS)                                                                    \
+  {                                                                                              \
+    double ar[MT], ai[MT];                                                                       \
+    cplx b[NT];                                                                                  \
+    _Pragma("unroll") for (int i = 0; i < MT; ++i) {                                             \
+      const cplx v = lds_c((SRC) + i * 512);                                                     \
+      ar[i] = (AL) * v.x;                                                                        \
+      ai[i] = (ALS) * v.y;                                                                       \
+    }                                                                                            \
+    _Pragma("unroll") for (int j = 0; j < NT; ++j) b[j] = lds_c((SRC) + (MT + j) * 512);         \
+    _Pragma("unroll") for (int j = 0; j < NT; ++j)                                               \
+      _Pragma("unroll") for (int i = 0; i < MT; ++i) dmma884(cre[i][j], ar[i], b[j].x);             \
+    _Pragma("unroll") for (int j = 0; j < NT; ++j)                                               \
+      _Pragma("unroll") for (int i = 0; i < MT; ++i) dmma884(cim[i][j], ar[i], b[j].y);             \
+    _Pragma("unroll") for (int j = 0; j < NT; ++j)                                               \
+      _Pragma("unroll") for (int i = 0; i < MT; ++i) dmma884(cre[i][j], -ai[i], b[j].y);            \
+    _Pragma("unroll") for (int j = 0; j < NT; ++j)                                               \
+      _Pragma("unroll") for (int i = 0; i < MT; ++i) dmma884(cim[i][j], ai[i], b[j].x);             \
   }
-  __device__ __forceinline__ void issue(uint32_t dst) {
-    if (!done) {
-      if (s < nfull) {
-#pragma unroll
-        for (int i = 0; i < MT; ++i) {
-          cp_async16(dst + i * 512, pa[i], 16);
-          pa[i] += dA;
-        }
-#pragma unroll
-        for (int j = 0; j < NT; ++j) {
-          cp_async16(dst + (MT + j) * 512, pb[j], 16);
-          pb[j] += dB;
-        }
-      } else {
-        // ragged k tail of the segment: lanes with k >= K copy nothing and get zeros
-        const int k = 4 * nfull + kq;
-        const int back = k < K ? 0 : k - (K - 1);
-        const int sz = k < K ? 16 : 0;
-#pragma unroll
-        for (int i = 0; i < MT; ++i) cp_async16(dst + i * 512, pa[i] - (int64_t)back * a_sk, sz);
-#pragma unroll
-        for (int j = 0; j < NT; ++j) cp_async16(dst + (MT + j) * 512, pb[j] - (int64_t)back * b_sk, sz);
-      }
-      ++s;
-      if (s == nst) {
-        ++si;
-        if (si < se) {
-          setup(n_a_off, n_b_off, n_K, n_a_sm, n_a_sk, n_b_sk, n_b_sn);
-          prefetch_next();
-        } else {
-          done = true;
-        }
-      }
-    }
-    cp_commit();
-  }
-};
 
 template <int MT, int NT>
-__device__ __noinline__ void run_unit(const GemmUnit& u, const GemmSeg* __restrict__ segs,
-                                      const cplx* __restrict__ A, const cplx* __restrict__ B,
-                                      cplx* __restrict__ C, int lane, double conj_sign, uint32_t ring) {
+__device__ __noinline__ void run_unit(const GemmUnit& u, const GemmSeg* __restrict__ segs, const cplx* __restrict__ A,
+                                       const cplx* __restrict__ B, cplx* __restrict__ C, int lane, double conj_sign,
+                                       uint32_t ring) {
   constexpr int D = RING_DEPTH;
-  constexpr int STAGE_BYTES = (MT + NT) * 512;
+  static_assert((D & (D - 1)) == 0, "RING_DEPTH must be a power of two");
+  constexpr int F = MT + NT;
+  constexpr int STAGE_BYTES = F * 512;
   double cre[MT][NT][2], cim[MT][NT][2];
 #pragma unroll
   for (int i = 0; i < MT; ++i)
 #pragma unroll
     for (int j = 0; j < NT; ++j) cre[i][j][0] = cre[i][j][1] = cim[i][j][0] = cim[i][j][1] = 0.0;
   const int total = u.steps;
+  const int kq = lane & 3, r8 = lane >> 2;
+  const uint32_t lane_ring = ring + lane * 16;
   if (total > 0) {
-    Producer<MT, NT> P;
-    P.init(segs, u, A, B, lane);
-    const uint32_t lane_ring = ring + lane * 16;
+    int mi[MT], nj[NT];
+#pragma unroll
+    for (int i = 0; i < MT; ++i) mi[i] = min(u.m0 + 8 * i + r8, u.M - 1);
+#pragma unroll
+    for (int j = 0; j < NT; ++j) nj[j] = min(u.n0 + 8 * j + r8, u.N - 1);
+    // ---- producer state
+    const cplx* pa[MT];
+    const cplx* pb[NT];
+    int64_t dA, dB;
+    int p_si = u.seg_begin, p_left, p_K, p_ask, p_bsk;  // p_left: steps left in the producer's segment
+    const int se = u.seg_end;
+    int p_issued = 0;
+    P_SETUP(u.first.a_off, u.first.b_off, u.first.K, u.first.a_sm, u.first.a_sk, u.first.b_sk, u.first.b_sn)
 #pragma unroll 1
-    for (int d = 0; d < D - 1; ++d) P.issue(lane_ring + d * STAGE_BYTES);
-    // consumer-side walk over the segments for alpha, one segment of lookahead
-    int csi = u.seg_begin;
-    const int cse = u.seg_end;
-    int cleft = (u.first.K + 3) >> 2;
+    for (int d = 0; d < D - 1; ++d) { P_STEP_SLOW(lane_ring + d * STAGE_BYTES) }
+    // ---- consumer state
+    int c_si = u.seg_begin;
+    int c_left = (u.first.K + 3) >> 2;
     double alpha = u.first.alpha;
-    int nK = segs[min(csi + 1, cse - 1)].K;
-    double nalpha = segs[min(csi + 1, cse - 1)].alpha;
-    int rd = 0, wr = D - 1;
-#pragma unroll 1
-    for (int t = 0; t < total; ++t) {
-      cp_wait<D - 2>();
-      const uint32_t src = lane_ring + rd * STAGE_BYTES;
-      double ar[MT], ai[MT];
+    int t = 0;
+    int n_cK = segs[min(c_si + 1, se - 1)].K;
+    double n_alpha = segs[min(c_si + 1, se - 1)].alpha;
+    while (t < total) {
+      // chunk: steps during which the consumer stays in its segment and the producer issues only FULL
+      // steps of its segment (p_left - 1 full steps are guaranteed when the last one may be ragged)
+      const int p_full = (p_issued < total) ? ((p_K & 3) ? p_left - 1 : p_left) : 0;
+      int n = min(c_left, p_full);
       const double als = alpha * conj_sign;
+      if (n > 0) {
+        c_left -= n;
+        p_left -= n;
+        p_issued += n;
+#pragma unroll 1
+        for (; n > 0; --n, ++t) {
+          cp_wait<D - 2>();
+          const uint32_t src = lane_ring + (t & (D - 1)) * STAGE_BYTES;
+          const uint32_t dst = lane_ring + ((t + D - 1) & (D - 1)) * STAGE_BYTES;
 #pragma unroll
-      for (int i = 0; i < MT; ++i) {
-        const cplx v = lds_c(src + i * 512);
-        ar[i] = alpha * v.x;
-        ai[i] = als * v.y;
+          for (int i = 0; i < MT; ++i) {
+            cp_async16(dst + i * 512, pa[i], 16);
+            pa[i] += dA;
+          }
+#pragma unroll
+          for (int j = 0; j < NT; ++j) {
+            cp_async16(dst + (MT + j) * 512, pb[j], 16);
+            pb[j] += dB;
+          }
+          cp_commit();
+          CONSUME(src, alpha, als)
+        }
+        if (p_left == 0 && p_issued < total) {
+          ++p_si;
+          const GemmSeg* sp = segs + p_si;
+          P_SETUP(sp->a_off, sp->b_off, sp->K, sp->a_sm, sp->a_sk, sp->b_sk, sp->b_sn)
+        }
+      } else {
+        // boundary step: slow producer path (ragged tail, segment switch or exhausted), one consumer step
+        cp_wait<D - 2>();
+        const uint32_t src = lane_ring + (t & (D - 1)) * STAGE_BYTES;
+        P_STEP_SLOW(lane_ring + ((t + D - 1) & (D - 1)) * STAGE_BYTES)
+        CONSUME(src, alpha, als)
+        ++t;
+        --c_left;
       }
-      cplx b[NT];
-#pragma unroll
-      for (int j = 0; j < NT; ++j) b[j] = lds_c(src + (MT + j) * 512);
-      P.issue(lane_ring + wr * STAGE_BYTES);
-      rd = rd + 1 == D ? 0 : rd + 1;
-      wr = wr + 1 == D ? 0 : wr + 1;
-      // (ar + i ai)(br + i bi): four real DMMAs per 8x8 sub-tile, ordered so that consecutive
-      // DMMAs never touch the same accumulator
-#pragma unroll
-      for (int j = 0; j < NT; ++j)
-#pragma unroll
-        for (int i = 0; i < MT; ++i) dmma884(cre[i][j], ar[i], b[j].x);
-#pragma unroll
-      for (int j = 0; j < NT; ++j)
-#pragma unroll
-        for (int i = 0; i < MT; ++i) dmma884(cim[i][j], ar[i], b[j].y);
-#pragma unroll
-      for (int j = 0; j < NT; ++j)
-#pragma unroll
-        for (int i = 0; i < MT; ++i) dmma884(cre[i][j], -ai[i], b[j].y);
-#pragma unroll
-      for (int j = 0; j < NT; ++j)
-#pragma unroll
-        for (int i = 0; i < MT; ++i) dmma884(cim[i][j], ai[i], b[j].x);
-      if (--cleft == 0) {
-        ++csi;
-        cleft = (nK + 3) >> 2;
-        alpha = nalpha;
-        const GemmSeg* np = segs + min(csi + 1, cse - 1);
-        nK = np->K;
-        nalpha = np->alpha;
+      if (c_left == 0 && t < total) {
+        ++c_si;
+        c_left = (n_cK + 3) >> 2;
+        alpha = n_alpha;
+        n_cK = segs[min(c_si + 1, se - 1)].K;
+        n_alpha = segs[min(c_si + 1, se - 1)].alpha;
       }
     }
     cp_wait<0>();
   }
-  // epilogue: lane holds C[row lane/4][cols 2 (lane%4), 2 (lane%4) + 1] of every sub-tile
-  const int er = lane >> 2, ec = (lane & 3) * 2;
+  const int ec = kq * 2;
   cplx* gC = C + u.c_off;
 #pragma unroll
   for (int i = 0; i < MT; ++i) {
-    const int r = u.m0 + 8 * i + er;
+    const int r = u.m0 + 8 * i + r8;
     if (r < u.M) {
 #pragma unroll
       for (int j = 0; j < NT; ++j) {
@@ -243,6 +223,7 @@ __device__ __noinline__ void run_unit(const GemmUnit& u, const GemmSeg* __restri
     }
   }
 }
+
 
 #define FH_FOR_SHAPES(X)                                                                                   \
   X(1, 1) X(1, 2) X(1, 3) X(1, 4) X(1, 5) X(1, 6) X(1, 7) X(1, 8) X(2, 1) X(2, 2) X(2, 3) X(2, 4) X(2, 5)  \
