@@ -204,6 +204,59 @@ def test_apply_parity_table_s2_shape_random_envs(H, ctx, den):
     ctx.mps_destroy(mps)
 
 
+@pytest.mark.parametrize("chi,nsample", [(4096, 40), (16384, 12)])
+def test_apply_parity_bench_sizes_sampled_blocks(H, chi, nsample):
+    """BASELINE config 3 (chi = 4096, the workload bench.py times) and config 4's size (chi = 16384) in
+    the launch configuration of the bench (same sector profile, same plan, same unit lists; iid random
+    environments through env_set so that no oracle input comes from the CUDA path).  The oracle computes
+    sampled output blocks one by one (each output block is an independent sum over its own segments):
+    the six largest blocks plus random ones, relative Frobenius error per block <= 1e-11; plus a
+    property that holds at any size and for any environments: H(2 theta) = 2 H(theta) bit for bit
+    (scaling by two commutes with every rounding; it fails if any block or k-range were skipped or
+    visited twice between the two calls)."""
+    L, c = 60, 29
+    dims = fi.chain_dims(chi, L, "gaussian", (1, 1))
+    dl, dr = dims[c], dims[c + 2]
+    Lk, Rk = fi.env_block_keys(dl, dl), fi.env_block_keys(dr, dr)
+    Le = fi.random_blocks(9, 1, Lk, {k: (dl[k[0]], dl[k[2]]) for k in Lk})
+    Re = fi.random_blocks(9, 2, Rk, {k: (dr[k[0]], dr[k[2]]) for k in Rk})
+    th = fi.theta_random(9, c, dl, dr)
+    W1, W2 = symm.mpo_reduced(c, 1.0, 4.0), symm.mpo_reduced(c + 1, 1.0, 4.0)
+    ctx = H.binding.Context(int(max(1 << 30, 48.0 * chi * chi)))
+    try:
+        mpo = ctx.fh_mpo_build(L, 1.0, 4.0)
+        mps = ctx.mps_create(L)
+        ctx.mps_set_bond(mps, c, dl)
+        ctx.mps_set_bond(mps, c + 2, dr)
+        for which, bond, keys, E in ((0, c, Lk, Le), (1, c + 2, Rk, Re)):
+            labels = [[k[0][0], k[0][1], k[1], k[2][0], k[2][1]] for k in keys]
+            flat = np.concatenate([E[k].ravel() for k in keys])
+            ctx.env_set(mps, which, bond, labels, flat)
+        ctx.heff_plan(mpo, mps, c, 2)
+        lab, dm, ne = ctx.heff_layout(2)
+        x = _dev(H.flatten(th, lab, dm, H.theta_key))
+        y = _torch().empty_like(x)
+        ctx.heff_apply(x, y)
+        got = H.unflatten(y.cpu().numpy(), lab, dm, H.theta_key)
+        y2 = _torch().empty_like(x)
+        ctx.heff_apply(2.0 * x, y2)
+        assert bool((y2 == 2.0 * y).all())                      # exact: scaling by 2 commutes with rounding
+        rng = np.random.default_rng(chi)
+        keys = sorted(th)
+        big = sorted(keys, key=lambda k: -th[k].size)[:6]
+        pick = big + [keys[i] for i in rng.choice(len(keys), nsample, replace=False)]
+        ref = heff2_selected(Le, Re, th, W1, W2, pick)
+        worst = 0.0
+        for k in pick:
+            den_ = max(np.linalg.norm(ref[k]), 1e-300)
+            worst = max(worst, np.linalg.norm(got[k] - ref[k]) / den_)
+        print("chi=%d: %d sampled blocks, worst rel. Frobenius error %.2e" % (chi, len(pick), worst))
+        assert worst < TOL_APPLY
+        ctx.mps_destroy(mps)
+    finally:
+        ctx.close()
+
+
 # ------------------------------------------------------------------ Lanczos exponential (H6 + H7)
 def test_expm_parity_central_bond(H, ctx):
     """exp(-i tau H_eff) theta with m = 10 on the chi = 256 central bond vs the oracle's Lanczos
