@@ -28,7 +28,7 @@ NOMINAL_BF16_TF = 2250.0    # guide: 2.25 PFLOP/s dense bf16
 FALLBACK_BF16_TF = 1590.0   # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 FALLBACK_HBM_GBS = 6650.0
 # one ncu --set full capture of the default workload (profiles/r1_heff_apply_ncu.md), bytes per launch
-NCU_DRAM_BYTES_PER_LAUNCH = 0.5 * (16.166144e6 + 1.224448e6 + 36.569344e6 + 0.709632e6)
+NCU_DRAM_BYTES_PER_LAUNCH = 0.5 * (16.202496e6 + 1.256704e6 + 36.604416e6 + 0.501760e6)
 
 
 def parse_args():
@@ -295,7 +295,7 @@ def run_ours(args):
                          pk["source"], pk["bf16"], NOMINAL_FP64_TF, NOMINAL_BF16_TF),
                      "frac_l2_warm": flops * args.steps / t_warm * 1e-12 / peak_dmma,
                      "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (chi == 4096 and args.profile == "gaussian") else None,
-                     "traffic_source": "profiles/r1_heff_apply_ncu.md: dram__bytes_read.sum + dram__bytes_write.sum, mean of the stage-1 and stage-2 launch (17.4 MB and 37.3 MB); algorithmic minimum 55 MB per launch pair / 2"},
+                     "traffic_source": "profiles/r1_heff_apply_ncu.md: dram__bytes_read.sum + dram__bytes_write.sum, mean of the stage-1 and stage-2 launch (17.5 MB and 37.1 MB); algorithmic minimum 55 MB per launch pair / 2"},
         "e2e": {"value": world * flops * args.steps / t_e2e * 1e-9, "unit": "GFLOP/s",
                 "h2d_bytes_per_step": zbytes, "d2h_bytes_per_step": zbytes, "api": "heff_apply_host (pinned host buffers)"},
         "gpu_launches": int(launches), "clocks": clk, "wall_seconds_timed_region": wall,
