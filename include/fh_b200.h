@@ -191,6 +191,11 @@ double fh_coef_right(int tc, int ts, int tb, int tk, int tr, int tkp, int tcp, i
 int fh_host_plan(int site, int nsite, double t_h, double U, int nl, const int32_t* bl, int nr, const int32_t* br,
                  int nLblk, const int32_t* Llab, int nRblk, const int32_t* Rlab);
 int fh_host_get_tasks(int stage, int* ntask, int* nout, int32_t* tuples, double* alpha, int64_t* flops);
+/* Warp-unit list of the same host plan (what the grouped ZGEMM launches): per unit
+ * [out, m0, n0, mt, nt, steps] (int32[nunit][6], launch order = heaviest first) and per output block
+ * [M, N, steps] (int32[nout][3]); dmma_padded = DMMA.8x8x4 instructions the list issues.  Either array
+ * pointer may be NULL to query the counts only. */
+int fh_host_get_units(int stage, int* nunit, int32_t* units, int* nout, int32_t* outs, int64_t* dmma_padded);
 
 #ifdef __cplusplus
 }

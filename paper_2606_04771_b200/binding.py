@@ -71,6 +71,7 @@ _SIGS = {
     "fh_host_plan": (c_int, [c_int, c_int, c_dbl, c_dbl, c_int, c_void_p, c_int, c_void_p, c_int, c_void_p,
                              c_int, c_void_p]),
     "fh_host_get_tasks": (c_int, [c_int, P(c_int), P(c_int), c_void_p, c_void_p, P(c_i64)]),
+    "fh_host_get_units": (c_int, [c_int, P(c_int), c_void_p, P(c_int), c_void_p, P(c_i64)]),
 }
 EXPORTS = sorted(_SIGS)
 for _name, (_res, _args) in _SIGS.items():
@@ -120,6 +121,19 @@ def fh_host_plan(site, nsite, t_h, U, dims_l, dims_r, L_keys, R_keys):
         lib.fh_host_get_tasks(stage, C.byref(nt), C.byref(no), _np_ptr(tup), _np_ptr(al), C.byref(fl))
         out.append((tup, al, no.value, fl.value))
     return out
+
+
+def fh_host_get_units(stage):
+    """Warp-unit list of the last fh_host_plan: (units int32[n,6] = out, m0, n0, mt, nt, steps;
+    outs int32[nout,3] = M, N, steps; dmma_padded)."""
+    nu, no, dp = c_int(), c_int(), c_i64()
+    lib.fh_host_get_units(stage, C.byref(nu), None, C.byref(no), None, C.byref(dp))
+    units = np.zeros((nu.value, 6), dtype=np.int32)
+    outs = np.zeros((no.value, 3), dtype=np.int32)
+    rc = lib.fh_host_get_units(stage, C.byref(nu), _np_ptr(units), C.byref(no), _np_ptr(outs), C.byref(dp))
+    if rc != 0:
+        raise FhError("fh_host_get_units failed: %d" % rc)
+    return units, outs, dp.value
 
 
 # ------------------------------------------------------------------ device objects

@@ -991,6 +991,36 @@ int fh_host_get_tasks(int stage, int* ntask, int* nout, int32_t* tuples, double*
   return FH_OK;
 }
 
+int fh_host_get_units(int stage, int* nunit, int32_t* units, int* nout, int32_t* outs, int64_t* dmma_padded) {
+  if (stage != 1 && stage != 2) return FH_EINVAL;
+  const Stage& st = stage == 1 ? g_host_st1 : g_host_st2;
+  if (nunit) *nunit = (int)st.units.size();
+  if (nout) *nout = (int)st.outs.size();
+  if (dmma_padded) *dmma_padded = st.dmma_padded;
+  if (units) {
+    // recover the output index of a unit from its c_off (outputs have distinct offsets unless empty)
+    std::map<int64_t, int> by_off;
+    for (size_t o = 0; o < st.outs.size(); ++o)
+      if (st.outs[o].M > 0 && st.outs[o].N > 0) by_off[st.outs[o].c_off] = (int)o;
+    for (size_t i = 0; i < st.units.size(); ++i) {
+      const GemmUnit& u = st.units[i];
+      units[6 * i] = by_off.count(u.c_off) ? by_off[u.c_off] : -1;
+      units[6 * i + 1] = u.m0;
+      units[6 * i + 2] = u.n0;
+      units[6 * i + 3] = u.shape >> 4;
+      units[6 * i + 4] = u.shape & 15;
+      units[6 * i + 5] = u.steps;
+    }
+  }
+  if (outs)
+    for (size_t o = 0; o < st.outs.size(); ++o) {
+      outs[3 * o] = st.outs[o].M;
+      outs[3 * o + 1] = st.outs[o].N;
+      outs[3 * o + 2] = st.outs[o].steps;
+    }
+  return FH_OK;
+}
+
 double fh_coef_left(int ta, int ts, int tc, int tk, int tr, int tkp, int tap, int tsp, int tcp) {
   return fh::coef_left(ta, ts, tc, tk, tr, tkp, tap, tsp, tcp);
 }

@@ -90,3 +90,36 @@ def test_task_lists_bit_exact_config2_shape(binding):
     Lk, Rk = symm.env_keys(dl, dl), symm.env_keys(dr, dr)
     n1, n2 = _compare(binding, 29, 2, dl, dr, Lk, Rk)
     assert n1 > 500 and n2 > 500
+
+
+@pytest.mark.parametrize("chi,profile", [(256, "gaussian"), (1024, "gaussian"), (4096, "gaussian"), (0, "table_s2")])
+def test_unit_lists_tile_every_output_exactly_once(binding, chi, profile):
+    """The warp-unit decomposition the grouped ZGEMM launches, checked on the host:
+    every element of every output block is covered by exactly one unit, units have a compiled shape
+    (mt * nt <= 16, mt, nt <= 8), only the last 8-sliver of a block is padded, the launch order is
+    heaviest first, and the padded DMMA count is what the units add up to."""
+    L, c = 60, 29
+    dims = fi.chain_dims(chi, L, profile, (1, 24))
+    dl, dr = dims[c], dims[c + 2]
+    Lk, Rk = sorted(fi.env_block_keys(dl, dl)), sorted(fi.env_block_keys(dr, dr))
+    binding.fh_host_plan(c, 2, 1.0, 4.0, dl, dr, Lk, Rk)
+    for stage in (1, 2):
+        units, outs, padded = binding.fh_host_get_units(stage)
+        assert len(units) > 0 and (units[:, 0] >= 0).all()
+        cover = [np.zeros(((m + 7) // 8, (n + 7) // 8), dtype=np.int32) for m, n, _ in outs]
+        work, total = [], 0
+        for o, m0, n0, mt, nt, steps in units:
+            M, N, st = outs[o]
+            assert 1 <= mt <= 8 and 1 <= nt <= 8 and mt * nt <= 16
+            assert m0 % 8 == 0 and n0 % 8 == 0 and steps == st
+            assert m0 + 8 * mt <= (M + 7) // 8 * 8 and n0 + 8 * nt <= (N + 7) // 8 * 8   # padding < 8
+            cover[o][m0 // 8:m0 // 8 + mt, n0 // 8:n0 // 8 + nt] += 1
+            work.append(mt * nt * max(1, steps))
+            total += 4 * mt * nt * steps
+        for o, cv in enumerate(cover):
+            if outs[o][0] > 0 and outs[o][1] > 0:
+                assert (cv == 1).all(), (stage, o)
+        assert all(a >= b for a, b in zip(work, work[1:]))          # heaviest first
+        assert total == padded
+        exact = sum(int(m) * int(n) for m, n, _ in outs)             # sanity: padded area < 2x exact for these profiles
+        assert sum(int(cv.size) * 64 for cv in cover) < 4 * exact + 64 * len(outs) * 4
