@@ -267,11 +267,22 @@ void finalize_stage(Stage& st, const BlockTensor& out, const BlockTensor& lhs, c
       }
       if (M != go.M || N != go.N || K != K2) throw std::runtime_error("task list: block shapes do not match");
       sg.K = K;
+      // The kernel reads op(A)(m, k) and op(B)(k, n) only for m < M, n < N, k < K (rows, columns and
+      // k positions beyond are clamped to the last valid one), so proving the extreme element of each
+      // operand inside its tensor proves every copy of the kernel in bounds.
+      if (K > 0) {
+        const int64_t a_last = sg.a_off + (int64_t)(M - 1) * sg.a_sm + (int64_t)(K - 1) * sg.a_sk;
+        const int64_t b_last = sg.b_off + (int64_t)(K - 1) * sg.b_sk + (int64_t)(N - 1) * sg.b_sn;
+        if (sg.a_off < 0 || sg.b_off < 0 || a_last >= lhs.nelem || b_last >= rhs.nelem)
+          throw std::runtime_error("task list: operand block exceeds its tensor");
+      }
       go.steps += (K + 3) / 4;
       st.flops += (int64_t)8 * M * N * K;
       ++t;
     }
     go.seg_end = (int)t;
+    if (go.c_off < 0 || go.c_off + (int64_t)(go.M - 1) * go.ldc + go.N > out.nelem)
+      throw std::runtime_error("task list: output block exceeds its tensor");
   }
   if (t != nt) throw std::runtime_error("task list: tasks not sorted by output id");
   emit_units(st);
