@@ -250,3 +250,44 @@ class DenseTDVP:
             n_dn[i] = p[(d == 2) | (d == 3)].sum() / norm2
             docc[i] = p[d == 3].sum() / norm2
         return dict(n_up=n_up, n_dn=n_dn, docc=docc, norm2=norm2)
+
+
+# ------------------------------------------------------------------ one-site TDVP (NEXT-1)
+def heff0(Lenv, Renv, C):
+    """Zero-site effective Hamiltonian on the bond matrix C (chi_l x chi_r):
+    K C = sum_w L[a',w,a] C[a,b] R[b',w,b]  (backward step of one-site TDVP, refs 8, 9 of the paper)."""
+    return np.einsum("xwa,ab,ywb->xy", Lenv, C, Renv, optimize=True)
+
+
+def tdvp1_step(self, dt):
+    """One-site TDVP time step ("switch from the two-site to the one-site TDVP update
+    once chi has saturated"): L->R half-sweep (forward one-site step tau = dt/2, QR, backward
+    zero-site step) then the mirror R->L half-sweep.  Bond dimensions never change.  Starts and ends
+    with the orthogonality centre on site 0, like `step`."""
+    L, W, m = self.L, self.W, self.m
+    tau = dt / 2
+    for i in range(L):                                           # left -> right
+        Le, Re = self.Lenv[i], self.Renv[i + 1]
+        self.A[i] = lanczos_exp(lambda x: heff1(Le, W, Re, x), self.A[i], tau, m)
+        if i < L - 1:
+            cl, _, cr = self.A[i].shape
+            Q, R = np.linalg.qr(self.A[i].reshape(cl * 4, cr))
+            self.A[i] = Q.reshape(cl, 4, -1)
+            self.Lenv[i + 1] = update_left(Le, self.A[i], W)
+            Ln = self.Lenv[i + 1]
+            C = lanczos_exp(lambda x: heff0(Ln, Re, x), R, -tau, m)
+            self.A[i + 1] = np.tensordot(C, self.A[i + 1], axes=(1, 0))
+    for i in range(L - 1, -1, -1):                               # right -> left
+        Le, Re = self.Lenv[i], self.Renv[i + 1]
+        self.A[i] = lanczos_exp(lambda x: heff1(Le, W, Re, x), self.A[i], tau, m)
+        if i > 0:
+            cl, _, cr = self.A[i].shape
+            Q, R = np.linalg.qr(self.A[i].reshape(cl, 4 * cr).T)  # A = R^T Q^T
+            self.A[i] = Q.T.reshape(-1, 4, cr)
+            self.Renv[i] = update_right(Re, self.A[i], W)
+            Rn = self.Renv[i]
+            C = lanczos_exp(lambda x: heff0(Le, Rn, x), R.T, -tau, m)
+            self.A[i - 1] = np.tensordot(self.A[i - 1], C, axes=(2, 0))
+
+
+DenseTDVP.step1 = tdvp1_step

@@ -569,6 +569,96 @@ def svd_split(theta, dims_l, dims_r, chi_max_full, eps_trunc, direction):
     return dict(sorted(A1.items())), dict(sorted(A2.items())), dims_mid, info
 
 
+# ------------------------------------------------------------------ one-site TDVP pieces (NEXT-1)
+def embed_bond(C, dims_bra, dims_ket):
+    """Bond matrix {c: (d'_c x d_c)} (an SU(2) scalar: diagonal in the sector and in m) -> dense."""
+    offb, nb = bond_offsets(dims_bra)
+    offk, nk = bond_offsets(dims_ket)
+    out = np.zeros((nb, nk), dtype=complex)
+    for c, blk in C.items():
+        for tm in ms(c[1]):
+            out[_rows(offb, dims_bra, c, tm), _rows(offk, dims_ket, c, tm)] += blk
+    return out
+
+
+def heff0_tasks(L_keys, R_keys, c_keys):
+    """Zero-site apply: out[c'] = sum_{(c, w)} L[c',w,c] C[c] R[c',w,c]^T.  The recoupling coefficient
+    is 1: with L = L[c',w,c] C(j_c m, k_w mu | j_c' m') and R likewise (F-4), the sum over m and mu of
+    the two Clebsch-Gordan coefficients is delta_{m' n'} (CG orthogonality).  Stage 1: X[c',w,c] =
+    L[c',w,c] C[c]; stage 2: out[c'] = sum X[c',w,c] R[c',w,c]^T, segments ordered by (c, w)."""
+    Rset = set(R_keys)
+    cset = set(c_keys)
+    st1, st2 = {}, {}
+    for (cp, w, c) in L_keys:
+        if c in cset and cp in cset and (cp, w, c) in Rset:
+            st1[(cp, w, c)] = [((cp, w, c), c, 1.0)]
+            st2.setdefault(cp, []).append(((cp, w, c), (cp, w, c), 1.0))
+    for o in st2:
+        st2[o].sort(key=lambda t: (t[0][2], t[0][1]))
+    return dict(sorted(st1.items())), dict(sorted(st2.items()))
+
+
+def heff0_apply(Lenv, Renv, C):
+    st1, st2 = heff0_tasks(sorted(Lenv), sorted(Renv), sorted(C))
+    X = run_stage(st1, Lenv, C)
+    out = run_stage(st2, X, Renv, "n", "t")
+    for c, v in C.items():
+        if c not in out:
+            out[c] = np.zeros_like(v)
+    return out
+
+
+def split_site_right_moving(A, dims_l, dims_r):
+    """A[a,s,c] = Q[a,s,c'] C[c]: per right sector c the stacked rows (a, s, alpha) are decomposed by
+    an SVD, Q = U (left-canonical), C = S V^dagger (k_c x d_c), k_c = min(rows, d_c).  No truncation.
+    Returns (Q, C, new dims of the bond between them)."""
+    by_c = {}
+    for k in sorted(A):
+        by_c.setdefault(k[2], []).append(k)
+    Q, C, dims_new = {}, {}, {}
+    for c, keys in by_c.items():
+        M = np.vstack([A[k] for k in keys])
+        U_, sv, Vh = np.linalg.svd(M, full_matrices=False)
+        dims_new[c] = U_.shape[1]
+        C[c] = sv[:, None] * Vh
+        ro = 0
+        for k in keys:
+            Q[k] = U_[ro:ro + A[k].shape[0]].copy()
+            ro += A[k].shape[0]
+    return dict(sorted(Q.items())), dict(sorted(C.items())), dims_new
+
+
+def split_site_left_moving(A, dims_l, dims_r):
+    """A[a,s,b] = C[a] Q[a',s,b]: per left sector a the blocks are laid side by side with the weight
+    sqrt((2j_b+1)/(2j_a+1)) (F-6: right-canonical means sum_{s,b} (2j_b+1)/(2j_a+1) Q Q^dagger = 1),
+    SVD, C = U S (d_a x k_a), Q = V^dagger with the weight undone."""
+    by_a = {}
+    for k in sorted(A):
+        by_a.setdefault(k[0], []).append(k)
+    Q, C, dims_new = {}, {}, {}
+    for a, keys in by_a.items():
+        M = np.hstack([A[k] * sqrt((k[2][1] + 1) / (a[1] + 1)) for k in keys])
+        U_, sv, Vh = np.linalg.svd(M, full_matrices=False)
+        dims_new[a] = Vh.shape[0]
+        C[a] = U_ * sv[None, :]
+        co = 0
+        for k in keys:
+            n = A[k].shape[1]
+            Q[k] = Vh[:, co:co + n] * sqrt((a[1] + 1) / (k[2][1] + 1))
+            co += n
+    return dict(sorted(Q.items())), dict(sorted(C.items())), dims_new
+
+
+def absorb_left(C, A):
+    """A'[c,s,b] = C[c] A[c,s,b]."""
+    return {k: C[k[0]] @ v for k, v in A.items()}
+
+
+def absorb_right(A, C):
+    """A'[a,s,c] = A[a,s,c] C[c]."""
+    return {k: v @ C[k[2]] for k, v in A.items()}
+
+
 # ------------------------------------------------------------------ integer task tuples (A-14)
 def task_tuples(tasks, out_order, lhs_order, rhs_order):
     """Flatten {out_key: [(k1, k2, alpha)]} to int32 tuples (out_id, lhs_id, rhs_id) + alphas,

@@ -120,6 +120,58 @@ class SymmTDVP:
             if i > 0:
                 self.A[i] = self._evolve1(i, A1, self.Lenv[i], self.Renv[i + 1], -tau)
 
+    # ---- one-site TDVP (NEXT-1)
+    def _evolve0(self, C, Le, Re, tau):
+        """Backward zero-site step on the bond matrix C; weight 2j_c+1 per sector block (F-6)."""
+        st1, st2 = symm.heff0_tasks(sorted(Le), sorted(Re), sorted(C))
+        keys = list(C)
+
+        def flat(x):
+            return np.concatenate([sqrt(c[1] + 1) * x[c].ravel() for c in keys])
+
+        def unflat(vec):
+            out, n = {}, 0
+            for c in keys:
+                out[c] = (vec[n:n + C[c].size] / sqrt(c[1] + 1)).reshape(C[c].shape)
+                n += C[c].size
+            return out
+
+        def apply_h(vec):
+            x = unflat(vec)
+            X = symm.run_stage(st1, Le, x)
+            out = symm.run_stage(st2, X, Re, "n", "t")
+            for c in keys:
+                if c not in out:
+                    out[c] = np.zeros_like(x[c])
+            return flat(out)
+
+        return unflat(lanczos_exp(apply_h, flat(C), tau, self.m))
+
+    def step1(self, dt):
+        """One-site TDVP step: L->R (forward one-site tau = dt/2, split, backward zero-site) then R->L.
+        Starts and ends with the centre on site 0, like `step`; bond dimensions can only shrink (when a
+        sector has fewer stacked rows than columns), never grow."""
+        L = self.L
+        tau = dt / 2
+        for i in range(L):
+            self.A[i] = self._evolve1(i, self.A[i], self.Lenv[i], self.Renv[i + 1], tau)
+            if i < L - 1:
+                Q, C, dn = symm.split_site_right_moving(self.A[i], self.dims[i], self.dims[i + 1])
+                self.A[i] = Q
+                self.Lenv[i + 1] = symm.env_update_left(self.Lenv[i], Q, self.W[i])
+                C = self._evolve0(C, self.Lenv[i + 1], self.Renv[i + 1], -tau)
+                self.dims[i + 1] = dn
+                self.A[i + 1] = symm.absorb_left(C, self.A[i + 1])
+        for i in range(L - 1, -1, -1):
+            self.A[i] = self._evolve1(i, self.A[i], self.Lenv[i], self.Renv[i + 1], tau)
+            if i > 0:
+                Q, C, dn = symm.split_site_left_moving(self.A[i], self.dims[i], self.dims[i + 1])
+                self.A[i] = Q
+                self.Renv[i] = symm.env_update_right(self.Renv[i + 1], Q, self.W[i])
+                C = self._evolve0(C, self.Lenv[i], self.Renv[i], -tau)
+                self.dims[i] = dn
+                self.A[i - 1] = symm.absorb_right(self.A[i - 1], C)
+
     # ---- measurements (H10; reading A-12)
     def measure_local(self):
         """<1>, <S^z_i>, <P_D,i>/2 per site through left norm-environments

@@ -224,3 +224,53 @@ def test_bookkeeping_table_s2_and_profiles():
     assert chain[0] == {(0, 0): 1} and chain[12] == {(0, 0): 1}
     tabs = fi.reachable_tables(12)
     assert all(set(chain[k]) <= set(tabs[k]) for k in range(13))
+
+
+def test_one_site_tdvp_pieces_and_driver_vs_dense():
+    """NEXT-1: (i) the zero-site apply with coefficient 1 equals the dense einsum of the embedded
+    environments and bond matrix; (ii) the one-site splits reproduce the tensor and give canonical
+    factors; (iii) the symmetric TDVP1 driver equals the dense one (itself pinned against ED) through
+    observables, after a two-site phase that grows the bonds."""
+    from oracle import symm_tdvp as stv
+    from oracle import dense_tdvp as dtv
+    L, t_h, U, dt = 6, 1.0, 4.0, 0.05
+    sy = stv.SymmTDVP(L, t_h, U, krylov_dim=12)
+    de = dtv.DenseTDVP(L, t_h, U, krylov_dim=12)
+    for _ in range(3):
+        sy.step(dt)
+        de.step(dt)
+    # (i) zero-site apply on bond 3 with the driver's own environments (left env needs building)
+    Le = symm.boundary_left()
+    for i in range(3):
+        Le = symm.env_update_left(Le, sy.A[i], sy.W[i])
+    Re = sy.Renv[3]
+    d3 = sy.dims[3]
+    rng = np.random.default_rng(4)
+    C = {c: rng.standard_normal((d, d)) + 1j * rng.standard_normal((d, d)) for c, d in d3.items()}
+    got = symm.embed_bond(symm.heff0_apply(Le, Re, C), d3, d3)
+    ref = np.einsum("xwa,ab,ywb->xy", symm.embed_env(Le, d3, d3), symm.embed_bond(C, d3, d3),
+                    symm.embed_env(Re, d3, d3))
+    assert np.abs(got - ref).max() < 1e-12 * max(1.0, np.abs(ref).max())
+    # (ii) splits
+    A = sy.A[2]
+    Q, Cm, dn = symm.split_site_right_moving(A, sy.dims[2], sy.dims[3])
+    back = symm.absorb_right(Q, Cm)
+    assert max(np.abs(back[k] - A[k]).max() for k in A) < 1e-13
+    for c in dn:
+        g = sum(Q[k].conj().T @ Q[k] for k in Q if k[2] == c)
+        assert np.abs(g - np.eye(dn[c])).max() < 1e-12
+    Q, Cm, dn = symm.split_site_left_moving(A, sy.dims[2], sy.dims[3])
+    back = symm.absorb_left(Cm, Q)
+    assert max(np.abs(back[k] - A[k]).max() for k in A) < 1e-13
+    for a in dn:
+        g = sum((k[2][1] + 1) / (a[1] + 1) * Q[k] @ Q[k].conj().T for k in Q if k[0] == a)
+        assert np.abs(g - np.eye(dn[a])).max() < 1e-12
+    # (iii) drivers
+    worst = 0.0
+    for _ in range(4):
+        sy.step1(dt)
+        de.step1(dt)
+        a, b = sy.measure_local(), de.observables()
+        worst = max(worst, np.abs(a["sz"] - 0.5 * (b["n_up"] - b["n_dn"])).max(), np.abs(a["docc"] - b["docc"]).max())
+    assert worst < 1e-9, worst
+    assert abs(sy.measure_global()["norm2"] - b["norm2"]) < 1e-10
