@@ -138,6 +138,14 @@ typedef struct {
   double eps_trunc;    /* discarded relative weight; < 0 disables */
 } fh_params;
 int tdvp2_sweep(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh_params* params);
+/* One full ONE-site TDVP time step dt ("switch from the two-site to the one-site TDVP
+ * update once the bond dimension has saturated"): L->R half-sweep then R->L, tau = dt/2; at every site:
+ * forward one-site Lanczos step, split without truncation (block-wise SVD of the (a,s)-stacked or
+ * (s,b)-side-by-side blocks), environment update, backward ZERO-site step on the bond matrix
+ * (K C = sum_w L C R^T, recoupling coefficient 1), absorption into the next site.  Bond dimensions
+ * never grow.  Preconditions and state on return as tdvp2_sweep (centre on site 0, right environments
+ * built); krylov_dim and krylov_tol of params are used, chi_max_full and eps_trunc are not. */
+int tdvp1_sweep(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh_params* params);
 /* statistics of the last sweep: max discarded weight, max chi_full, max chi_su2, max d */
 int tdvp2_last_stats(const fh_ctx* ctx, double* max_discarded, int* chi_full, int* chi_su2, int* dmax);
 

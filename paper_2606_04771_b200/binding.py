@@ -59,6 +59,7 @@ _SIGS = {
     "heff_inner": (c_int, [c_void_p, c_void_p, c_void_p, P(c_dbl)]),
     "heff_expm": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, c_int]),
     "tdvp2_sweep": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, P(fh_params)]),
+    "tdvp1_sweep": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, P(fh_params)]),
     "tdvp2_last_stats": (c_int, [c_void_p, P(c_dbl), P(c_int), P(c_int), P(c_int)]),
     "measure_local": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
     "measure_global": (c_int, [c_void_p, c_void_p, c_void_p, P(c_dbl), P(c_dbl)]),
@@ -323,6 +324,10 @@ class Context:
     def tdvp2_sweep(self, mpo, mps, dt, krylov_dim=10, krylov_tol=1e-12, chi_max_full=1 << 30, eps_trunc=-1.0):
         p = fh_params(krylov_dim, krylov_tol, chi_max_full, eps_trunc)
         self.check(lib.tdvp2_sweep(self.h, mpo, mps, dt, C.byref(p)), "tdvp2_sweep")
+
+    def tdvp1_sweep(self, mpo, mps, dt, krylov_dim=10, krylov_tol=1e-12):
+        p = fh_params(krylov_dim, krylov_tol, 1 << 30, -1.0)
+        self.check(lib.tdvp1_sweep(self.h, mpo, mps, dt, C.byref(p)), "tdvp1_sweep")
 
     def tdvp2_last_stats(self):
         d, a, b, c = c_dbl(), c_int(), c_int(), c_int()

@@ -119,7 +119,7 @@ void fh_ctx::timers_resolve() {
 }
 
 // ============================================================================ plan + apply
-static int last_tj_pos(int nsite) { return nsite == 2 ? 7 : 4; }
+static int last_tj_pos(int nsite) { return nsite == 2 ? 7 : (nsite == 1 ? 4 : 1); }
 
 void fh::plan_heff(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, int nsite) {
   FH_REQUIRE(nsite == 1 || nsite == 2, FH_EINVAL, "heff_plan: nsite must be 1 or 2");
@@ -750,6 +750,14 @@ int tdvp2_sweep(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh
     FH_REQUIRE(ctx && mpo && mps && p, FH_EINVAL, "tdvp2_sweep: NULL argument");
     FH_REQUIRE(p->krylov_dim >= 2 && p->krylov_dim <= 32 && p->chi_max_full >= 1, FH_EINVAL, "tdvp2_sweep: bad parameters");
     sweep(ctx, mpo, mps, dt, p);
+  })
+}
+
+int tdvp1_sweep(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh_params* p) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && mpo && mps && p, FH_EINVAL, "tdvp1_sweep: NULL argument");
+    FH_REQUIRE(p->krylov_dim >= 2 && p->krylov_dim <= 32, FH_EINVAL, "tdvp1_sweep: bad parameters");
+    sweep1(ctx, mpo, mps, dt, p);
   })
 }
 

@@ -150,5 +150,6 @@ void expm_lanczos(fh_ctx* ctx, cplx* theta_inout, double tau, int m, double tol,
 void do_env_update_left(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int site);
 void do_env_update_right(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int site);
 void sweep(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh_params* p);
+void sweep1(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh_params* p);
 void measure_local_impl(fh_ctx* ctx, const fh_mps* mps, double* n_i, double* sz_i, double* docc_i);
 }  // namespace fh

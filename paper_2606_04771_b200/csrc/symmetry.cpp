@@ -572,6 +572,77 @@ void emit_merge(const BlockTensor& A1, const BlockTensor& A2, const BlockTensor&
   finalize_stage(st, theta, A1, A2);
 }
 
+void emit_heff0(const BlockTensor& Lenv, const BlockTensor& Renv, const BlockTensor& vec, BlockTensor& X,
+                Stage& st1, Stage& st2) {
+  std::vector<RawTask> raw1, raw2;
+  std::vector<Shape> shapes1;
+  struct Pend {
+    Key xkey;
+    RawTask t;
+  };
+  std::vector<Pend> pend;
+  for (size_t e = 0; e < Lenv.keys.size(); ++e) {
+    const Key& ek = Lenv.keys[e];  // c'(0,1) w(2) c(3,4)
+    const Sector cp = key_sector(ek, 0), c = key_sector(ek, 3);
+    const int ci = vec.find(Key{c.q, c.tj, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0});
+    const int cpi = vec.find(Key{cp.q, cp.tj, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0});
+    const int ri = Renv.find(ek);
+    if (ci < 0 || cpi < 0 || ri < 0) continue;
+    RawTask t1;
+    t1.out = ek;
+    t1.order = Key{0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    t1.lhs = (int)e;
+    t1.rhs = ci;
+    t1.alpha = 1.0;
+    raw1.push_back(t1);
+    shapes1.push_back(Shape{Lenv.rows[e], vec.cols[ci]});
+    Pend p;
+    p.xkey = ek;
+    p.t.out = vec.keys[cpi];
+    p.t.order = Key{c.q, c.tj, ek[2], 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    p.t.lhs = -1;
+    p.t.rhs = ri;
+    p.t.alpha = 1.0;
+    pend.push_back(p);
+  }
+  layout_from_tasks(raw1, shapes1, 5, X);
+  st1.opA = OPA_N;
+  st1.opB = OPB_N;
+  tasks_to_stage(raw1, X, st1);
+  finalize_stage(st1, X, Lenv, vec);
+  for (auto& p : pend) {
+    p.t.lhs = X.find(p.xkey);
+    raw2.push_back(p.t);
+  }
+  st2.opA = OPA_N;
+  st2.opB = OPB_T;
+  tasks_to_stage(raw2, vec, st2);
+  finalize_stage(st2, vec, X, Renv);
+}
+
+void emit_absorb(const BlockTensor& C, const BlockTensor& A, const BlockTensor& Anew, bool left, Stage& st) {
+  std::vector<RawTask> raw;
+  for (size_t i = 0; i < Anew.keys.size(); ++i) {
+    const Key& k = Anew.keys[i];  // x(0,1) s(2) y(3,4)
+    const int ai = A.find(k);
+    const Sector sec = left ? key_sector(k, 0) : key_sector(k, 3);
+    const int ci = C.find(Key{sec.q, sec.tj, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0});
+    if (ai < 0 || ci < 0) continue;
+    RawTask t;
+    t.out = k;
+    t.order = Key{0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    t.lhs = left ? ci : ai;
+    t.rhs = left ? ai : ci;
+    t.alpha = 1.0;
+    raw.push_back(t);
+  }
+  st.opA = OPA_N;
+  st.opB = OPB_N;
+  tasks_to_stage(raw, Anew, st);
+  if (left) finalize_stage(st, Anew, C, A);
+  else finalize_stage(st, Anew, A, C);
+}
+
 void emit_norm_env(const BlockTensor& Nenv, const BlockTensor& A, BlockTensor& Nout, Stage& st1, Stage& st2) {
   // stage 1: X[a,s,c] = N[a] A[a,s,c]  (X has A's layout);  stage 2: N'[c] = sum_{a,s} A[a,s,c]^H X[a,s,c]
   std::vector<RawTask> raw1, raw2;

@@ -39,6 +39,14 @@ void emit_merge(const BlockTensor& A1, const BlockTensor& A2, const BlockTensor&
 // N layouts use key {q, tj}.
 void emit_norm_env(const BlockTensor& Nenv, const BlockTensor& A, BlockTensor& Nout, Stage& st1, Stage& st2);
 
+// zero-site apply on a bond matrix C[c] (rows: bra-side dims, cols: ket-side dims), the backward step of
+// one-site TDVP (NEXT-1): X[c',w,c] = L[c',w,c] C[c];  out[c'] = sum_{(c,w)} X[c',w,c] R[c',w,c]^T, coefficient 1
+// (CG orthogonality).  vec = layout of C with keys {q, tj}.
+void emit_heff0(const BlockTensor& Lenv, const BlockTensor& Renv, const BlockTensor& vec, BlockTensor& X,
+                Stage& st1, Stage& st2);
+// A'[c,s,b] = C[c] A[c,s,b] (left = true) or A'[a,s,c] = A[a,s,c] C[c] (left = false); Anew = layout of A'
+void emit_absorb(const BlockTensor& C, const BlockTensor& A, const BlockTensor& Anew, bool left, Stage& st);
+
 // fills outs/segs from the (sorted) task arrays and builds the warp-unit list
 void finalize_stage(Stage& st, const BlockTensor& out, const BlockTensor& lhs, const BlockTensor& rhs);
 

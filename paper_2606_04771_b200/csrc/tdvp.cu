@@ -473,6 +473,272 @@ static void local_update1(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int i, do
   ctx->alloc.release(woff, wn);
 }
 
+// ============================================================================ one-site TDVP (NEXT-1)
+// Plan of the zero-site apply on the bond matrix C (layout Cl, keys {q, tj}) between Lenv and Renv.
+static void plan_zero_site(fh_ctx* ctx, const BlockTensor& Le, const BlockTensor& Re, const BlockTensor& Cl) {
+  Plan& P = ctx->plan;
+  ctx->free_tensor(P.Z);
+  P.valid = false;
+  P.nsite = 0;
+  P.site = -1;
+  P.vec = Cl;
+  P.vec.base = -1;
+  emit_heff0(Le, Re, P.vec, P.Z, P.st1, P.st2);
+  ctx->alloc_tensor(P.Z);
+  P.Lptr = ctx->ptr(Le.base);
+  P.Rptr = ctx->ptr(Re.base);
+  P.chunks.clear();
+  for (size_t i = 0; i < P.vec.keys.size(); ++i) {
+    const int64_t n = (int64_t)P.vec.rows[i] * P.vec.cols[i];
+    for (int64_t st = 0; st < n; st += 8192)
+      P.chunks.push_back(VecChunk{P.vec.off[i] + st, (int)std::min<int64_t>(8192, n - st), (float)(P.vec.keys[i][1] + 1)});
+  }
+  const size_t need = stage_bytes(P.st1) + stage_bytes(P.st2) + P.chunks.size() * (sizeof(VecChunk) + 16) + 4096;
+  P.pool.reserve(need, ctx->stream);
+  upload_stage(P.pool, P.st1, ctx->stream);
+  upload_stage(P.pool, P.st2, ctx->stream);
+  P.d_chunks = upload(P.pool, P.chunks, ctx->stream);
+  P.d_partial = (double*)P.pool.take(std::max<size_t>(1, P.chunks.size()) * 2 * sizeof(double));
+  P.d_result = (double*)P.pool.take(2 * sizeof(double));
+  P.valid = true;
+}
+
+// Split the one-site tensor of site i without truncation (block-wise SVD per fused sector):
+//   direction +1: A_i[a,s,c] = Q[a,s,c] C[c],  Q left-canonical,  C[c] = S V^H (k_c x d_c); bond i+1 gets dims k
+//   direction -1: A_i[a,s,b] = C[a] Q[a,s,b],  Q right-canonical (weights (2j_b+1)/(2j_a+1)), C[a] = U S (d_a x k_a);
+//                 bond i gets dims k
+// C is allocated in the arena (caller frees it).
+static void split_site(fh_ctx* ctx, fh_mps* mps, int i, int direction, BlockTensor& C) {
+  const BlockTensor Aold = mps->A[i];  // copy of the layout (device data stays where it is)
+  const int gpos = direction > 0 ? 3 : 0;  // label position of the sector the blocks are grouped by
+  std::map<Sector, SectorSvd> secs;
+  struct Ref { int blk, ro, co; };
+  std::map<Sector, std::vector<Ref>> refs;
+  for (size_t t = 0; t < Aold.keys.size(); ++t) {
+    const Key& k = Aold.keys[t];
+    const Sector g{k[gpos], k[gpos + 1]};
+    SectorSvd& S = secs[g];
+    S.c = g;
+    std::vector<Ref>& R = refs[g];
+    if (R.empty()) S.nrow = S.ncol = 0;
+    if (direction > 0) {  // stack rows (a, s): keys are already sorted by (a, s) within a fixed c
+      R.push_back(Ref{(int)t, S.nrow, 0});
+      S.nrow += Aold.rows[t];
+      S.ncol = Aold.cols[t];
+    } else {  // side by side (s, b)
+      R.push_back(Ref{(int)t, 0, S.ncol});
+      S.ncol += Aold.cols[t];
+      S.nrow = Aold.rows[t];
+    }
+  }
+  int64_t cplx_total = 0, dbl_total = 0;
+  std::vector<SectorSvd*> order;
+  for (auto& e : secs) {
+    SectorSvd& S = e.second;
+    S.k = std::min(S.nrow, S.ncol);
+    S.keep = S.k;
+    S.transposed = S.nrow > S.ncol;
+    S.m_off = cplx_total;
+    cplx_total += Arena::round_up((int64_t)S.nrow * S.ncol);
+    S.u_off = cplx_total;
+    cplx_total += Arena::round_up((int64_t)std::max(S.nrow, S.ncol) * S.k);
+    S.vt_off = cplx_total;
+    cplx_total += Arena::round_up((int64_t)S.k * S.k);
+    S.s_off = dbl_total;
+    dbl_total += (S.k + 1) / 2 * 2;
+    order.push_back(&S);
+  }
+  const int64_t scratch_n = cplx_total + Arena::round_up((dbl_total + 1) / 2);
+  const int64_t scratch = ctx->alloc.alloc(scratch_n);
+  cplx* buf = ctx->ptr(scratch);
+  double* dS = reinterpret_cast<double*>(buf + cplx_total);
+  cudaStream_t s = ctx->stream;
+  // ---- pack
+  ctx->timer_begin(T_PACK);
+  std::vector<CopyBlk> blks;
+  for (auto& e : refs) {
+    const SectorSvd& S = secs[e.first];
+    for (const Ref& r : e.second) {
+      const Key& k = Aold.keys[r.blk];
+      CopyBlk b;
+      b.src_off = Aold.off[r.blk];
+      b.rows = Aold.rows[r.blk];
+      b.cols = Aold.cols[r.blk];
+      b.ld_src = Aold.cols[r.blk];
+      b.scale = direction > 0 ? 1.0 : std::sqrt((double)(k[4] + 1) / (double)(k[1] + 1));
+      b.pad = 0;
+      if (!S.transposed) {
+        b.dst_off = S.m_off + (int64_t)r.ro * S.ncol + r.co;
+        b.ld_dst = S.ncol;
+        b.transpose_dst = 0;
+      } else {
+        b.dst_off = S.m_off + (int64_t)r.co * S.nrow + r.ro;
+        b.ld_dst = S.nrow;
+        b.transpose_dst = 1;
+      }
+      blks.push_back(b);
+    }
+  }
+  ctx->pool_aux.reserve(blks.size() * sizeof(CopyBlk) + 4096, s);
+  CopyBlk* d_blks = upload(ctx->pool_aux, blks, s);
+  launch_copy_blocks(d_blks, (int)blks.size(), ctx->ptr(Aold.base), buf, s, &ctx->launches);
+  ctx->timer_end();
+  // ---- SVD
+  ctx->timer_begin(T_SVD);
+  run_sector_svds(ctx, order, buf, dS);
+  ctx->timer_end();
+  // ---- new bond, new layouts
+  Bond nb;
+  for (SectorSvd* S : order) {
+    nb.sec.push_back(S->c);
+    nb.d.push_back(S->k);
+  }
+  const int bpos = direction > 0 ? i + 1 : i;
+  mps->bond[bpos] = nb;
+  ctx->stat_chi = std::max(ctx->stat_chi, nb.chi_full());
+  ctx->stat_su2 = std::max(ctx->stat_su2, nb.chi_su2());
+  ctx->stat_dmax = std::max(ctx->stat_dmax, nb.dmax());
+  BlockTensor Q;
+  layout_site(mps->bond[i], mps->bond[i + 1], Q);
+  C.clear();
+  C.nlab = 2;
+  for (SectorSvd* S : order) {
+    if (direction > 0) C.add(Key{S->c.q, S->c.tj, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, S->k, S->ncol);
+    else C.add(Key{S->c.q, S->c.tj, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, S->nrow, S->k);
+  }
+  C.finalize();
+  ctx->alloc_tensor(Q);
+  ctx->alloc_tensor(C);
+  // ---- unpack (index conventions as in svd_split: B = column-major matrix handed to the solver)
+  ctx->timer_begin(T_PACK);
+  std::vector<CopyBlk> qb, cb;
+  for (SectorSvd* S : order) {
+    const int m = std::max(S->nrow, S->ncol), k = S->k;
+    // multiply by the singular values: rows of V^H (direction +1) or columns of U (direction -1)
+    cplx* target;
+    int nx;
+    int64_t sj, sx;
+    if (direction > 0) {
+      nx = S->ncol;
+      if (!S->transposed) { target = buf + S->u_off; sj = m; sx = 1; } else { target = buf + S->vt_off; sj = 1; sx = k; }
+    } else {
+      nx = S->nrow;
+      if (!S->transposed) { target = buf + S->vt_off; sj = 1; sx = k; } else { target = buf + S->u_off; sj = m; sx = 1; }
+    }
+    const int64_t tot = (int64_t)k * nx;
+    scale_by_s_kernel<<<(int)std::min<int64_t>((tot + 255) / 256, 1184), 256, 0, s>>>(target, k, nx, sj, sx, dS + S->s_off);
+    ++ctx->launches;
+    // C block
+    const int ci = C.find(Key{S->c.q, S->c.tj, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0});
+    CopyBlk b;
+    b.scale = 1.0;
+    b.pad = 0;
+    b.dst_off = C.off[ci];
+    if (direction > 0) {  // C = S V^H (k x ncol)
+      if (!S->transposed) { b.src_off = S->u_off; b.rows = k; b.cols = S->ncol; b.ld_src = m; b.ld_dst = S->ncol; b.transpose_dst = 0; }
+      else { b.src_off = S->vt_off; b.rows = S->ncol; b.cols = k; b.ld_src = k; b.ld_dst = S->ncol; b.transpose_dst = 1; }
+    } else {  // C = U S (nrow x k)
+      if (!S->transposed) { b.src_off = S->vt_off; b.rows = S->nrow; b.cols = k; b.ld_src = k; b.ld_dst = k; b.transpose_dst = 0; }
+      else { b.src_off = S->u_off; b.rows = k; b.cols = S->nrow; b.ld_src = m; b.ld_dst = k; b.transpose_dst = 1; }
+    }
+    cb.push_back(b);
+  }
+  for (auto& e : refs) {
+    const SectorSvd& S = secs[e.first];
+    const int m = std::max(S.nrow, S.ncol), k = S.k;
+    for (const Ref& r : e.second) {
+      const Key& key = Aold.keys[r.blk];
+      const int qi = Q.find(key);
+      FH_REQUIRE(qi >= 0, FH_ESTATE, "one-site split: block missing from the new layout");
+      CopyBlk b;
+      b.pad = 0;
+      b.dst_off = Q.off[qi];
+      if (direction > 0) {  // Q rows [ro, ro + d_a) of U_M, all k columns
+        b.scale = 1.0;
+        if (!S.transposed) { b.src_off = S.vt_off + (int64_t)r.ro * k; b.rows = Aold.rows[r.blk]; b.cols = k; b.ld_src = k; b.ld_dst = k; b.transpose_dst = 0; }
+        else { b.src_off = S.u_off + r.ro; b.rows = k; b.cols = Aold.rows[r.blk]; b.ld_src = m; b.ld_dst = k; b.transpose_dst = 1; }
+      } else {  // Q = V^H[:, co : co + d_b] with the weight undone
+        b.scale = std::sqrt((double)(key[1] + 1) / (double)(key[4] + 1));
+        const int db = Aold.cols[r.blk];
+        if (!S.transposed) { b.src_off = S.u_off + r.co; b.rows = k; b.cols = db; b.ld_src = m; b.ld_dst = db; b.transpose_dst = 0; }
+        else { b.src_off = S.vt_off + (int64_t)r.co * k; b.rows = db; b.cols = k; b.ld_src = k; b.ld_dst = db; b.transpose_dst = 1; }
+      }
+      qb.push_back(b);
+    }
+  }
+  ctx->pool_aux.reserve((qb.size() + cb.size()) * sizeof(CopyBlk) + 8192, s);
+  CopyBlk* d_qb = upload(ctx->pool_aux, qb, s);
+  CopyBlk* d_cb = upload(ctx->pool_aux, cb, s);
+  launch_copy_blocks(d_cb, (int)cb.size(), buf, ctx->ptr(C.base), s, &ctx->launches);
+  launch_copy_blocks(d_qb, (int)qb.size(), buf, ctx->ptr(Q.base), s, &ctx->launches);
+  FH_CUDA(cudaGetLastError());
+  ctx->timer_end();
+  ctx->free_tensor(mps->A[i]);
+  mps->A[i] = Q;
+  ctx->alloc.release(scratch, scratch_n);
+}
+
+// A_j <- C A_j (left) or A_j C (right) with the new bond dims already in mps->bond
+static void absorb_bond(fh_ctx* ctx, fh_mps* mps, int j, const BlockTensor& C, bool left) {
+  BlockTensor An;
+  layout_site(mps->bond[j], mps->bond[j + 1], An);
+  Stage st;
+  emit_absorb(C, mps->A[j], An, left, st);
+  ctx->alloc_tensor(An);
+  ctx->pool_aux.reserve(stage_bytes(st) + 4096, ctx->stream);
+  upload_stage(ctx->pool_aux, st, ctx->stream);
+  ctx->timer_begin(T_PACK);
+  if (left) launch_grouped_gemm(st, ctx->ptr(C.base), ctx->ptr(mps->A[j].base), ctx->ptr(An.base), ctx->stream, &ctx->launches);
+  else launch_grouped_gemm(st, ctx->ptr(mps->A[j].base), ctx->ptr(C.base), ctx->ptr(An.base), ctx->stream, &ctx->launches);
+  ctx->timer_end();
+  FH_CUDA(cudaGetLastError());
+  ctx->free_tensor(mps->A[j]);
+  mps->A[j] = An;
+}
+
+static void zero_site_update(fh_ctx* ctx, const BlockTensor& Le, const BlockTensor& Re, BlockTensor& C, double tau,
+                             const fh_params* prm) {
+  plan_zero_site(ctx, Le, Re, C);
+  const int64_t n = C.nelem;
+  const int m = prm->krylov_dim;
+  const int64_t wn = (int64_t)(m + 1) * n;
+  const int64_t woff = ctx->alloc.alloc(wn);
+  expm_lanczos(ctx, ctx->ptr(C.base), tau, m, prm->krylov_tol, ctx->ptr(woff));
+  ctx->alloc.release(woff, wn);
+}
+
+void fh::sweep1(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh_params* prm) {
+  const int L = mps->L;
+  FH_REQUIRE(mpo->L == L, FH_EINVAL, "tdvp1_sweep: MPO and MPS lengths differ");
+  for (int i = 0; i < L; ++i) FH_REQUIRE(mps->A[i].base >= 0, FH_ESTATE, "tdvp1_sweep: site tensor missing");
+  for (int i = 1; i <= L; ++i) FH_REQUIRE(mps->Renv[i].base >= 0, FH_ESTATE, "tdvp1_sweep: right environments missing (centre must be at site 0)");
+  ctx->stat_disc = 0.0;
+  ctx->stat_chi = ctx->stat_su2 = ctx->stat_dmax = 0;
+  const double tau = 0.5 * dt;
+  for (int i = 0; i < L; ++i) {  // left -> right
+    local_update1(ctx, mpo, mps, i, tau, prm);
+    if (i < L - 1) {
+      BlockTensor C;
+      split_site(ctx, mps, i, +1, C);
+      do_env_update_left(ctx, mpo, mps, i);
+      zero_site_update(ctx, mps->Lenv[i + 1], mps->Renv[i + 1], C, -tau, prm);
+      absorb_bond(ctx, mps, i + 1, C, true);
+      ctx->free_tensor(C);
+    }
+  }
+  for (int i = L - 1; i >= 0; --i) {  // right -> left
+    local_update1(ctx, mpo, mps, i, tau, prm);
+    if (i > 0) {
+      BlockTensor C;
+      split_site(ctx, mps, i, -1, C);
+      do_env_update_right(ctx, mpo, mps, i);
+      zero_site_update(ctx, mps->Lenv[i], mps->Renv[i], C, -tau, prm);
+      absorb_bond(ctx, mps, i - 1, C, false);
+      ctx->free_tensor(C);
+    }
+  }
+}
+
 void fh::sweep(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh_params* prm) {
   const int L = mps->L;
   FH_REQUIRE(mpo->L == L, FH_EINVAL, "tdvp2_sweep: MPO and MPS lengths differ");

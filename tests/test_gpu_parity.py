@@ -370,6 +370,36 @@ def test_config4_L60_U0_quench_vs_closed_form(H, ctx):
     ctx.mps_destroy(mps)
 
 
+def test_next1_one_site_tdvp_L8_vs_oracle(H, ctx):
+    """NEXT-1: tdvp1_sweep against the oracle's symmetric one-site driver (itself equal to the dense TDVP1
+    that is pinned against ED).  L = 8 Neel quench: five two-site steps with eps_trunc = 1e-12 grow the
+    bonds, then six one-site steps at frozen bond dimensions; observables <= 1e-8, identical sector
+    tables after every step, norm and energy conserved."""
+    L, t_h, U, dt, m = 8, 1.0, 4.0, 0.05, 10
+    ref = stv.SymmTDVP(L, t_h, U, krylov_dim=m, chi_max_full=256, eps_trunc=1e-12)
+    mpo = ctx.fh_mpo_build(L, t_h, U)
+    mps = ctx.mps_init_neel(mpo, L)
+    for _ in range(5):
+        ref.step(dt)
+        ctx.tdvp2_sweep(mpo, mps, dt, krylov_dim=m, chi_max_full=256, eps_trunc=1e-12)
+    e0 = ctx.measure_global(mpo, mps)["energy"]
+    worst = 0.0
+    for step in range(6):
+        ref.step1(dt)
+        ctx.tdvp1_sweep(mpo, mps, dt, krylov_dim=m)
+        a, b = ref.measure_local(), ctx.measure_local(mps, L)
+        for key in ("n", "sz", "docc"):
+            worst = max(worst, np.abs(a[key] - b[key]).max())
+        ga, gb = ref.measure_global(), ctx.measure_global(mpo, mps)
+        assert abs(ga["norm2"] - gb["norm2"]) < 1e-10 and abs(ga["energy"] - gb["energy"]) < 1e-9
+        assert abs(gb["energy"] - e0) < 1e-7          # TDVP conserves the energy
+        for k in range(1, L):
+            assert ctx.mps_get_bond(mps, k) == ref.dims[k], (step, k)
+    print("TDVP1 L=8: max |obs GPU - oracle| = %.2e" % worst)
+    assert worst < 1e-8, worst
+    ctx.mps_destroy(mps)
+
+
 # ------------------------------------------------------------------ edge cases and errors
 def test_edge_cases_and_error_codes(H, ctx):
     B = H.binding
