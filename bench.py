@@ -351,9 +351,21 @@ def run_sweep(ctx, H, mpo, args):
     sec = time.perf_counter() - t0
     tm = ctx.fh_get_timers()
     st = ctx.tdvp2_last_stats()
+    launches2 = ctx.fh_launch_count() - l0
+    # NEXT-1: the one-site sweep on the same (now chi-saturated) MPS -- the paper's 4-10x lever
+    ctx.fh_reset_timers()
+    torch.cuda.synchronize()
+    l1 = ctx.fh_launch_count()
+    t0 = time.perf_counter()
+    ctx.tdvp1_sweep(mpo, mps, 0.05, krylov_dim=10)
+    torch.cuda.synchronize()
+    sec1 = time.perf_counter() - t0
+    tm1 = ctx.fh_get_timers()
+    st1 = ctx.tdvp2_last_stats()
     ctx.mps_destroy(mps)
-    return {"chi": chi, "seconds": sec, "device_seconds_by_phase": tm, "stats": st,
-            "launches": ctx.fh_launch_count() - l0}
+    return {"chi": chi, "seconds": sec, "device_seconds_by_phase": tm, "stats": st, "launches": launches2,
+            "one_site": {"seconds": sec1, "device_seconds_by_phase": tm1, "chi_full": st1["chi_full"],
+                         "launches": ctx.fh_launch_count() - l1, "speedup_vs_two_site": sec / sec1}}
 
 
 def run_config4(args):
