@@ -192,7 +192,8 @@ int fh_vec_kernels_gbs(fh_ctx* ctx, int64_t n_elems, int m, int reps, double* gb
  *   coefR(c,s,b; k,r,k'; c',s',b') = (2b'+1)/(2c'+1) sqrt((2b+1)(2k'+1)(2c'+1)(2s'+1)) {c s b; k r k'; c' s' b'} */
 double fh_coef_left(int ta, int ts, int tc, int tk, int tr, int tkp, int tap, int tsp, int tcp);
 double fh_coef_right(int tc, int ts, int tb, int tk, int tr, int tkp, int tcp, int tsp, int tbp);
-/* Emit the task lists of an apply on `site` (nsite = 1 | 2) from explicit tables: bl/br =
+/* Emit the task lists of an apply on `site` (nsite = 1 | 2; nsite = 0: the zero-site apply of one-site
+ * TDVP on the bond whose bra-side dims are bl and ket-side dims br) from explicit tables: bl/br =
  * [n][3] (q,tj,d) of the left and right bond, Llab/Rlab = [nblk][5] canonical-order labels of the
  * environment blocks.  Results are kept in a process-global scratch (not thread-safe) and read
  * with fh_host_get_tasks (same format as heff_get_tasks; flops = sum 8mnk of that stage). */

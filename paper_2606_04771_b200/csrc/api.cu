@@ -954,7 +954,7 @@ static fh::Stage g_host_st1, g_host_st2;
 int fh_host_plan(int site, int nsite, double t_h, double U, int nl, const int32_t* bl, int nr, const int32_t* br,
                  int nLblk, const int32_t* Llab, int nRblk, const int32_t* Rlab) {
   try {
-    if ((nsite != 1 && nsite != 2) || !bl || !br || !Llab || !Rlab) return FH_EINVAL;
+    if ((nsite != 0 && nsite != 1 && nsite != 2) || !bl || !br || !Llab || !Rlab) return FH_EINVAL;
     Bond Bl, Br;
     for (int i = 0; i < nl; ++i) { Bl.sec.push_back(Sector{bl[3 * i], bl[3 * i + 1]}); Bl.d.push_back(bl[3 * i + 2]); }
     for (int i = 0; i < nr; ++i) { Br.sec.push_back(Sector{br[3 * i], br[3 * i + 1]}); Br.d.push_back(br[3 * i + 2]); }
@@ -973,7 +973,14 @@ int fh_host_plan(int site, int nsite, double t_h, double U, int nl, const int32_
     MpoSite W1, W2;
     mpo_site_table(site, t_h, U, W1);
     mpo_site_table(site + 1, t_h, U, W2);
-    if (nsite == 2) {
+    if (nsite == 0) {  // zero-site apply on the bond matrix C[c] (d_bl(c) x d_br(c)), NEXT-1
+      vec.nlab = 2;
+      for (size_t i = 0; i < Bl.sec.size(); ++i)
+        if (Br.find(Bl.sec[i]) >= 0)
+          vec.add(Key{Bl.sec[i].q, Bl.sec[i].tj, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, Bl.d[i], Br.dim(Bl.sec[i]));
+      vec.finalize();
+      emit_heff0(Le, Re, vec, Z, g_host_st1, g_host_st2);
+    } else if (nsite == 2) {
       layout_theta(Bl, Br, vec);
       emit_heff2(Le, Re, vec, W1, W2, Z, g_host_st1, g_host_st2);
     } else {

@@ -123,3 +123,24 @@ def test_unit_lists_tile_every_output_exactly_once(binding, chi, profile):
         assert total == padded
         exact = sum(int(m) * int(n) for m, n, _ in outs)             # sanity: padded area < 2x exact for these profiles
         assert sum(int(cv.size) * 64 for cv in cover) < 4 * exact + 64 * len(outs) * 4
+
+
+def test_zero_site_task_lists_match_oracle(binding):
+    """NEXT-1: the zero-site apply K C = sum_w L C R^T.  Integer task tuples of both stages equal the
+    oracle's (oracle/symm.heff0_tasks) bit for bit, all coefficients are exactly 1, flops agree."""
+    dims = fi.chain_dims(256, 60, "gaussian", (1, 1))
+    dl = dims[30]
+    dr = {k: max(1, v - 1) for k, v in dl.items()}          # ket side slightly smaller: rectangular C blocks
+    Lk, Rk = sorted(fi.env_block_keys(dl, dl)), sorted(fi.env_block_keys(dr, dr))
+    ck = sorted(dl)
+    st1, st2 = symm.heff0_tasks(Lk, Rk, ck)
+    o1 = symm.task_tuples(st1, list(st1), Lk, ck)
+    o2 = symm.task_tuples(st2, ck, list(st1), Rk)
+    (t1, a1, n1, f1), (t2, a2, n2, f2) = binding.fh_host_plan(30, 0, 1.0, 4.0, dl, dr, Lk, Rk)
+    assert n1 == len(st1) and n2 == len(ck)
+    assert t1.shape == o1[0].shape and (t1 == o1[0]).all()
+    assert t2.shape == o2[0].shape and (t2 == o2[0]).all()
+    assert (a1 == 1.0).all() and (a2 == 1.0).all()
+    fl = sum(8 * dl[xk[0]] * dl[xk[2]] * dr[xk[2]] for xk in st1) + \
+        sum(8 * dl[o] * dr[seg[0][2]] * dr[o] for o, segs in st2.items() for seg in segs)
+    assert f1 + f2 == fl
