@@ -150,13 +150,14 @@ void fh::plan_heff(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, 
     for (int64_t s = 0; s < n; s += 8192)
       P.chunks.push_back(VecChunk{P.vec.off[i] + s, (int)std::min<int64_t>(8192, n - s), (float)(P.vec.keys[i][tpos] + 1)});
   }
-  const size_t need = stage_bytes(P.st1) + stage_bytes(P.st2) + P.chunks.size() * (sizeof(VecChunk) + 16) + 4096;
+  const size_t need = stage_bytes(P.st1) + stage_bytes(P.st2) + P.chunks.size() * (sizeof(VecChunk) + 16) + 8192;
   P.pool.reserve(need, ctx->stream);
   upload_stage(P.pool, P.st1, ctx->stream);
   upload_stage(P.pool, P.st2, ctx->stream);
   P.d_chunks = upload(P.pool, P.chunks, ctx->stream);
   P.d_partial = (double*)P.pool.take(std::max<size_t>(1, P.chunks.size()) * 2 * sizeof(double));
   P.d_result = (double*)P.pool.take(2 * sizeof(double));
+  P.d_scal = (double*)P.pool.take(256 * sizeof(double));
   P.valid = true;
 }
 
@@ -217,22 +218,24 @@ static void jacobi_eig(int n, std::vector<double>& Amat, std::vector<double>& Q)
 }
 
 // theta <- exp(-i tau H_eff) theta (H6 + H7).  work holds (m+1) vectors of n elements.
+// The recurrence keeps alpha_j, <w,w> and beta_j in device memory (P.d_scal): no host round trip
+// inside the iteration; one copy of 2m+1 scalars at the end, then the m x m tridiagonal problem on the
+// host.  After a happy breakdown (beta_j < tol) the remaining directions are zero vectors and the host
+// truncates the Krylov space at j.
 void fh::expm_lanczos(fh_ctx* ctx, cplx* theta, double tau, int m, double tol, cplx* V) {
   Plan& P = ctx->plan;
   const int64_t n = P.vec.nelem;
   FH_REQUIRE(m >= 1 && m <= 32, FH_EINVAL, "krylov_dim must be in [1, 32]");
-  if (n == 0) return;
+  if (n == 0 || P.chunks.empty()) return;
   cudaStream_t s = ctx->stream;
+  const int nch = (int)P.chunks.size();
+  // device scalars: [0,1] <theta,theta>, then per j: alpha pair at 2 + 4j, <w,w> pair at 4 + 4j; betas after
+  double* d_sc = P.d_scal;
+  double* d_beta = P.d_scal + 2 + 4 * 32;
   ctx->timer_begin(T_VEC);
-  const double nrm2 = inner(ctx, theta, theta).x;
+  launch_wdot(P.d_chunks, nch, theta, theta, P.d_partial, d_sc, s, &ctx->launches);
+  launch_scale_rsqrt_dev(n, d_sc, 0.0, theta, V, nullptr, s, &ctx->launches);
   ctx->timer_end();
-  if (!(nrm2 > 0.0)) return;
-  const double nrm = std::sqrt(nrm2);
-  ctx->timer_begin(T_VEC);
-  launch_scale(n, make_double2(1.0 / nrm, 0.0), theta, V, s, &ctx->launches);
-  ctx->timer_end();
-  std::vector<double> alpha, beta;
-  int k = 0;
   for (int j = 0; j < m; ++j) {
     cplx* vj = V + (int64_t)j * n;
     cplx* w = V + (int64_t)(j + 1) * n;
@@ -240,23 +243,31 @@ void fh::expm_lanczos(fh_ctx* ctx, cplx* theta, double tau, int m, double tol, c
     apply_heff(ctx, vj, w);
     ctx->timer_end();
     ctx->timer_begin(T_VEC);
-    const double a = inner(ctx, vj, w).x;
-    alpha.push_back(a);
-    k = j + 1;
-    launch_axpy(n, make_double2(-a, 0.0), vj, w, s, &ctx->launches);
-    if (j > 0) launch_axpy(n, make_double2(-beta[j - 1], 0.0), V + (int64_t)(j - 1) * n, w, s, &ctx->launches);
-    if (j == m - 1) {
-      ctx->timer_end();
-      break;
+    launch_wdot(P.d_chunks, nch, vj, w, P.d_partial, d_sc + 2 + 4 * j, s, &ctx->launches);
+    launch_axpy_neg_dev(n, d_sc + 2 + 4 * j, vj, w, s, &ctx->launches);
+    if (j > 0) launch_axpy_neg_dev(n, d_beta + (j - 1), V + (int64_t)(j - 1) * n, w, s, &ctx->launches);
+    if (j < m - 1) {
+      launch_wdot(P.d_chunks, nch, w, w, P.d_partial, d_sc + 4 + 4 * j, s, &ctx->launches);
+      launch_scale_rsqrt_dev(n, d_sc + 4 + 4 * j, tol, w, w, d_beta + j, s, &ctx->launches);
     }
-    const double b = std::sqrt(std::max(0.0, inner(ctx, w, w).x));
-    if (b < tol) {
-      ctx->timer_end();
-      break;
-    }
-    beta.push_back(b);
-    launch_scale(n, make_double2(1.0 / b, 0.0), w, w, s, &ctx->launches);
     ctx->timer_end();
+  }
+  const int nsc = 2 + 4 * 32 + 32;
+  ctx->ensure_pinned(nsc);
+  FH_CUDA(cudaMemcpyAsync(ctx->h_pinned, d_sc, nsc * sizeof(double), cudaMemcpyDeviceToHost, s));
+  FH_CUDA(cudaStreamSynchronize(s));
+  const double nrm2 = ctx->h_pinned[0];
+  if (!(nrm2 > 0.0)) return;  // zero vector: theta is untouched (V holds zeros)
+  const double nrm = std::sqrt(nrm2);
+  std::vector<double> alpha, beta;
+  int k = 0;
+  for (int j = 0; j < m; ++j) {
+    alpha.push_back(ctx->h_pinned[2 + 4 * j]);
+    k = j + 1;
+    if (j == m - 1) break;
+    const double bj = ctx->h_pinned[2 + 4 * 32 + j];
+    if (bj < tol) break;
+    beta.push_back(bj);
   }
   // host: c = exp(-i tau T) e_1 through the symmetric eigendecomposition of T (H7)
   std::vector<double> T(k * k, 0.0), Q;

@@ -61,6 +61,7 @@ struct Plan {
   VecChunk* d_chunks = nullptr;
   double* d_partial = nullptr;
   double* d_result = nullptr;
+  double* d_scal = nullptr;  // Lanczos scalars kept on the device (expm_lanczos)
   DevPool pool;
 };
 

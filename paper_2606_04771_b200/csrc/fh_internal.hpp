@@ -139,6 +139,10 @@ void launch_wdot(const VecChunk* d_chunks, int nchunks, const cplx* x, const cpl
 // y = y + a*x (a complex, from device scalar array coef[idx]*sign) etc.: see kernels.cu
 void launch_axpy(int64_t n, cplx a, const cplx* x, cplx* y, cudaStream_t s, int64_t* lc);
 void launch_scale(int64_t n, cplx a, const cplx* x, cplx* y, cudaStream_t s, int64_t* lc);  // y = a*x
+// device-scalar Lanczos helpers: y -= d_coef[0] x;  y = x / sqrt(d_norm2[0]) (0 below tol), d_beta[0] = sqrt(d_norm2[0])
+void launch_axpy_neg_dev(int64_t n, const double* d_coef, const cplx* x, cplx* y, cudaStream_t s, int64_t* lc);
+void launch_scale_rsqrt_dev(int64_t n, const double* d_norm2, double tol, const cplx* x, cplx* y, double* d_beta,
+                            cudaStream_t s, int64_t* lc);
 void launch_lincomb(int64_t n, int m, const cplx* coef_host, const cplx* V, int64_t stride, cplx* y,
                     cudaStream_t s, int64_t* lc);  // y = sum_j coef[j] V[j]
 void launch_copy_blocks(const CopyBlk* d_blks, int nblk, const cplx* src, cplx* dst, cudaStream_t s,

@@ -527,13 +527,14 @@ static void plan_zero_site(fh_ctx* ctx, const BlockTensor& Le, const BlockTensor
     for (int64_t st = 0; st < n; st += 8192)
       P.chunks.push_back(VecChunk{P.vec.off[i] + st, (int)std::min<int64_t>(8192, n - st), (float)(P.vec.keys[i][1] + 1)});
   }
-  const size_t need = stage_bytes(P.st1) + stage_bytes(P.st2) + P.chunks.size() * (sizeof(VecChunk) + 16) + 4096;
+  const size_t need = stage_bytes(P.st1) + stage_bytes(P.st2) + P.chunks.size() * (sizeof(VecChunk) + 16) + 8192;
   P.pool.reserve(need, ctx->stream);
   upload_stage(P.pool, P.st1, ctx->stream);
   upload_stage(P.pool, P.st2, ctx->stream);
   P.d_chunks = upload(P.pool, P.chunks, ctx->stream);
   P.d_partial = (double*)P.pool.take(std::max<size_t>(1, P.chunks.size()) * 2 * sizeof(double));
   P.d_result = (double*)P.pool.take(2 * sizeof(double));
+  P.d_scal = (double*)P.pool.take(256 * sizeof(double));
   P.valid = true;
 }
 
