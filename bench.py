@@ -224,7 +224,8 @@ def run_ours(args):
     L, c = 60, 29
     chi = args.chi
     # replicas only (north_star: one GPU, no sharding, no collectives): every rank runs the same bond
-    arena = int(min(160e9, max(16 << 30, 64.0 * chi * chi)))
+    sweep_need = 0.0 if args.no_sweep else 300.0 * args.sweep_chi * args.sweep_chi
+    arena = int(min(160e9, max(16 << 30, 64.0 * chi * chi, sweep_need)))
     ctx = H.binding.Context(arena, device="cuda:%d" % local)
     mpo = ctx.fh_mpo_build(L, 1.0, 4.0)
     t_build = time.perf_counter()

@@ -392,6 +392,7 @@ void fh_ctx_destroy(fh_ctx* c) {
   for (auto e : c->ev_free) cudaEventDestroy(e);
   c->plan.pool.destroy();
   c->pool_aux.destroy();
+  c->pool_small.destroy();
   for (auto& w : c->svd_workers) {
     if (w.s) cudaStreamSynchronize(w.s);
     if (w.h) cusolverDnDestroy(w.h);

@@ -90,6 +90,7 @@ struct fh_ctx {
   std::string err;
   fh::Plan plan;
   fh::DevPool pool_aux;  // env updates, merge, pack, measure
+  fh::DevPool pool_small;  // descriptors of the small-matrix SVD kernel
   int64_t launches = 0;
   // pinned host scratch
   double* h_pinned = nullptr;  // 4096 doubles

@@ -70,6 +70,121 @@ __global__ void conj_transpose_kernel(const cplx* __restrict__ src, cplx* __rest
   }
 }
 
+// ------------------------------------------------------------------------------------------
+// Small sector matrices (both dimensions <= SMALL_SVD_MAX): one 8-warp CTA per matrix, one launch for all of
+// them -- one-sided (Hestenes) Jacobi SVD in shared memory.  B (m x n, m >= n, column-major) -> U (m x n),
+// s (descending), V^H (n x n), the same conventions as cusolverDnZgesvd('S', 'S').  Column pairs (p, q) are
+// rotated until every |g_p^H g_q| <= 1e-15 |g_p| |g_q|; the singular values are the final column norms
+// (high relative accuracy, also for tiny ones).  At small chi a bond has tens of such matrices and a vendor
+// call per matrix (0.25 ms each, host-blocking) dominated the sweep.
+constexpr int SMALL_SVD_MAX = 64;
+struct SmallSvd {
+  int64_t m_off, u_off, vt_off, s_off;
+  int m, n;
+};
+__device__ __forceinline__ double warp_sum_all(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+constexpr int SMALL_SVD_WARPS = 8;
+__global__ void __launch_bounds__(32 * SMALL_SVD_WARPS) small_svd_kernel(const SmallSvd* __restrict__ descs,
+                                                                         cplx* __restrict__ buf,
+                                                                         double* __restrict__ dS) {
+  extern __shared__ __align__(16) unsigned char smem_svd[];
+  __shared__ int rotated_any;
+  const SmallSvd d = descs[blockIdx.x];
+  const int m = d.m, n = d.n, lane = threadIdx.x & 31, warp = threadIdx.x >> 5, tid = threadIdx.x;
+  constexpr int NT = 32 * SMALL_SVD_WARPS;
+  cplx* G = reinterpret_cast<cplx*>(smem_svd);  // m x n column-major
+  cplx* V = G + (size_t)m * n;                  // n x n column-major
+  double* sig = reinterpret_cast<double*>(V + (size_t)n * n);
+  const cplx* B = buf + d.m_off;
+  for (int i = tid; i < m * n; i += NT) G[i] = B[i];
+  for (int i = tid; i < n * n; i += NT) V[i] = make_double2((i % n) == (i / n) ? 1.0 : 0.0, 0.0);
+  __syncthreads();
+  // round-robin tournament: ne = n rounded up to even players, ne - 1 rounds of ne / 2 disjoint column pairs;
+  // the pairs of a round are independent and go to different warps
+  const int ne = (n + 1) & ~1;
+  for (int sweep = 0; sweep < 40 && n > 1; ++sweep) {
+    if (tid == 0) rotated_any = 0;
+    __syncthreads();
+    for (int r = 0; r < ne - 1; ++r) {
+      for (int k = warp; k < ne / 2; k += SMALL_SVD_WARPS) {
+        int p = (r + k) % (ne - 1);
+        int q = k == 0 ? ne - 1 : (r - k + ne - 1) % (ne - 1);
+        if (p > q) { const int t_ = p; p = q; q = t_; }
+        if (q >= n) continue;  // dummy player of an odd n
+        double a = 0.0, b = 0.0, cr = 0.0, ci = 0.0;
+        for (int i = lane; i < m; i += 32) {
+          const cplx x = G[p * m + i], y = G[q * m + i];
+          a += x.x * x.x + x.y * x.y;
+          b += y.x * y.x + y.y * y.y;
+          cr += x.x * y.x + x.y * y.y;  // conj(x) * y
+          ci += x.x * y.y - x.y * y.x;
+        }
+        a = warp_sum_all(a);
+        b = warp_sum_all(b);
+        cr = warp_sum_all(cr);
+        ci = warp_sum_all(ci);
+        const double c2 = cr * cr + ci * ci;
+        if (c2 <= 1e-30 * a * b || c2 == 0.0) continue;
+        if (lane == 0) rotated_any = 1;
+        const double cabs = sqrt(c2);
+        const double pr = cr / cabs, pi = ci / cabs;  // phase of c
+        const double zeta = (b - a) / (2.0 * cabs);
+        const double t = (zeta >= 0.0 ? 1.0 : -1.0) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
+        const double cs = 1.0 / sqrt(1.0 + t * t), sn = cs * t;
+        // y~ = conj(phase) * y;  x' = cs x - sn y~;  y' = sn x + cs y~
+        for (int i = lane; i < m; i += 32) {
+          const cplx x = G[p * m + i], y = G[q * m + i];
+          const double yr = pr * y.x + pi * y.y, yi = pr * y.y - pi * y.x;
+          G[p * m + i] = make_double2(cs * x.x - sn * yr, cs * x.y - sn * yi);
+          G[q * m + i] = make_double2(sn * x.x + cs * yr, sn * x.y + cs * yi);
+        }
+        for (int i = lane; i < n; i += 32) {
+          const cplx x = V[p * n + i], y = V[q * n + i];
+          const double yr = pr * y.x + pi * y.y, yi = pr * y.y - pi * y.x;
+          V[p * n + i] = make_double2(cs * x.x - sn * yr, cs * x.y - sn * yi);
+          V[q * n + i] = make_double2(sn * x.x + cs * yr, sn * x.y + cs * yi);
+        }
+      }
+      __syncthreads();
+    }
+    if (!rotated_any) break;
+    __syncthreads();
+  }
+  // singular values = column norms; rank by descending value (ties: lower column first)
+  for (int j = warp; j < n; j += SMALL_SVD_WARPS) {
+    double a = 0.0;
+    for (int i = lane; i < m; i += 32) {
+      const cplx x = G[j * m + i];
+      a += x.x * x.x + x.y * x.y;
+    }
+    a = warp_sum_all(a);
+    if (lane == 0) sig[j] = sqrt(a);
+  }
+  __syncthreads();
+  cplx* U = buf + d.u_off;
+  cplx* VT = buf + d.vt_off;
+  double* S = dS + d.s_off;
+  for (int j = warp; j < n; j += SMALL_SVD_WARPS) {
+    const double sj = sig[j];
+    int rank = 0;
+    for (int l = 0; l < n; ++l) rank += (sig[l] > sj || (sig[l] == sj && l < j)) ? 1 : 0;
+    const double inv = sj > 0.0 ? 1.0 / sj : 0.0;
+    if (lane == 0) S[rank] = sj;
+    for (int i = lane; i < m; i += 32) {
+      const cplx x = G[j * m + i];
+      U[(size_t)rank * m + i] = make_double2(x.x * inv, x.y * inv);
+    }
+    for (int i = lane; i < n; i += 32) {  // V^H[rank][i] = conj(V[i][j]), column-major n x n
+      const cplx x = V[j * n + i];
+      VT[(size_t)i * n + rank] = make_double2(x.x, -x.y);
+    }
+  }
+}
+
 void worker_reserve(fh_ctx::SvdWorker& w, size_t bytes) {
   if (bytes <= w.dwork_bytes) return;
   FH_CUDA(cudaStreamSynchronize(w.s));
@@ -163,8 +278,35 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
     FH_CUDA(cudaEventCreateWithFlags(&ctx->svd_fork, cudaEventDisableTiming));
   }
   const int nw = (int)ctx->svd_workers.size();
-  std::vector<int> idx(order.size());
-  for (size_t i = 0; i < idx.size(); ++i) idx[i] = (int)i;
+  std::vector<int> idx;
+  std::vector<SmallSvd> small;
+  size_t small_smem = 0;
+  for (size_t i = 0; i < order.size(); ++i) {
+    const int m = std::max(order[i]->nrow, order[i]->ncol), n = order[i]->k;
+    if (!qr && m <= SMALL_SVD_MAX) {
+      small.push_back(SmallSvd{order[i]->m_off, order[i]->u_off, order[i]->vt_off, order[i]->s_off, m, n});
+      small_smem = std::max(small_smem, ((size_t)m * n + (size_t)n * n) * sizeof(cplx) + (size_t)n * sizeof(double));
+    } else {
+      idx.push_back((int)i);
+    }
+  }
+  if (!small.empty()) {
+    static bool attr_done = false;
+    if (!attr_done) {
+      FH_CUDA(cudaFuncSetAttribute(small_svd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   (int)((2 * SMALL_SVD_MAX * SMALL_SVD_MAX) * sizeof(cplx) + SMALL_SVD_MAX * sizeof(double))));
+      attr_done = true;
+    }
+    const size_t need = small.size() * sizeof(SmallSvd);
+    ctx->pool_small.reserve(need + 256, ctx->stream);
+    SmallSvd* d_small = (SmallSvd*)ctx->pool_small.take(need);
+    FH_CUDA(cudaMemcpyAsync(d_small, small.data(), need, cudaMemcpyHostToDevice, ctx->stream));
+    small_svd_kernel<<<(int)small.size(), 32 * SMALL_SVD_WARPS, small_smem, ctx->stream>>>(d_small, buf, dS);
+    ++ctx->launches;
+    FH_CUDA(cudaGetLastError());
+    FH_CUDA(cudaStreamSynchronize(ctx->stream));  // `small` (pageable host memory) must outlive the copy
+  }
+  if (idx.empty()) return;
   auto cost = [&](int i) {
     const double m = std::max(order[i]->nrow, order[i]->ncol), n = order[i]->k;
     return m * n * n;
