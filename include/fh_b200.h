@@ -126,6 +126,13 @@ int64_t heff_flops(const fh_ctx* ctx);
 int heff_inner(fh_ctx* ctx, const void* x_dev, const void* y_dev, double* result);
 /* out_dev = exp(-i tau H_eff) theta_dev by an m-vector Lanczos process (H6, H7) */
 int heff_expm(fh_ctx* ctx, const void* theta_dev, void* out_dev, double tau, int krylov_dim);
+/* Same with the adaptive stop of reading A-15: at most krylov_dim vectors, stop when the
+ * residual estimate is <= adapt_tol (> 0); *k_used (host, may be NULL) receives the number of vectors used.
+ * One stream synchronisation per Lanczos step. */
+int heff_expm_adaptive(fh_ctx* ctx, const void* theta_dev, void* out_dev, double tau, int krylov_dim,
+                       double adapt_tol, int* k_used);
+/* cumulative since context creation: exponentials evaluated and Krylov vectors (= H_eff applies) they used */
+int fh_krylov_stats(const fh_ctx* ctx, int64_t* n_exponentials, int64_t* n_vectors);
 
 /* ---- time evolution ---------------------------------------------------
  * One full step dt = left->right half-sweep with tau = dt/2 followed by right->left with
@@ -136,6 +143,10 @@ typedef struct {
   double krylov_tol;   /* happy-breakdown threshold on beta_j (relative to 1), e.g. 1e-12 */
   int chi_max_full;    /* cap on sum d (2j+1) of the new bond */
   double eps_trunc;    /* discarded relative weight; < 0 disables */
+  double krylov_adapt_tol; /* > 0: adaptive Krylov dimension (reading A-15): stop after k <= krylov_dim
+                            * vectors once |tau| beta_k |e_k^T exp(-i tau T_k) e_1| <= krylov_adapt_tol (residual of
+                            * the Krylov approximation in y' = -i H y, times the step; relative to |theta|).
+                            * <= 0: always krylov_dim vectors (BASELINE config 3). */
 } fh_params;
 int tdvp2_sweep(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh_params* params);
 /* One full ONE-site TDVP time step dt ("switch from the two-site to the one-site TDVP

@@ -91,13 +91,32 @@ def heff1(Lenv, W, Renv, A):
     return (t @ Rm).reshape(clp, 4, crp)
 
 
-def lanczos_exp(apply_h, v, tau, m, breakdown=1e-12):
-    """exp(-i tau H) v by an m-vector Lanczos process with full re-orthogonalisation (A-5).
+def krylov_residual_estimate(alpha, beta, b_next, tau):
+    """Reading A-15 ("Krylov dimension chosen adaptively (35)").
+
+    After k Lanczos steps y_k(s) = V_k exp(-i s T_k) e_1 solves y' = -i H y up to the residual
+    r_k(s) = y_k' + i H y_k = -i b_k [e_k^T exp(-i s T_k) e_1] v_{k+1}   (H V_k = V_k T_k + b_k v_{k+1} e_k^T),
+    b_k = b_next the norm of the (k+1)-th unnormalised Lanczos vector.  The error of y_k(tau) is bounded by
+    int_0^tau |r_k(s)| ds; the estimate used for stopping is |tau| * |r_k(tau)|.
+    """
+    k = len(alpha)
+    T = np.diag(alpha) + np.diag(beta[:k - 1], 1) + np.diag(beta[:k - 1], -1)
+    lam, Q = np.linalg.eigh(T)
+    u_last = Q[k - 1, :] @ (np.exp(-1j * tau * lam) * Q[0, :])
+    return abs(tau) * b_next * abs(u_last)
+
+
+def lanczos_exp(apply_h, v, tau, m, breakdown=1e-12, adapt_tol=0.0, stats=None):
+    """exp(-i tau H) v by an (at most) m-vector Lanczos process with full re-orthogonalisation (A-5).
 
     T = tridiag(alpha, beta) is exponentiated through its symmetric eigendecomposition.
+    adapt_tol > 0 (A-15): stop after k < m vectors as soon as krylov_residual_estimate <= adapt_tol
+    (relative to |v|, the start vector being normalised).  `stats`, if a list, receives k.
     """
     nrm = np.linalg.norm(v)
     if nrm == 0.0:
+        if stats is not None:
+            stats.append(0)
         return v.copy()
     shape = v.shape
     V = [(v / nrm).ravel()]
@@ -114,9 +133,13 @@ def lanczos_exp(apply_h, v, tau, m, breakdown=1e-12):
         b = np.linalg.norm(w)
         if j == m - 1 or b < breakdown:
             break
+        if adapt_tol > 0.0 and krylov_residual_estimate(alpha, beta, b, tau) <= adapt_tol:
+            break
         beta.append(b)
         V.append(w / b)
     k = len(alpha)
+    if stats is not None:
+        stats.append(k)
     T = np.diag(alpha) + np.diag(beta[:k - 1], 1) + np.diag(beta[:k - 1], -1)
     lam, Q = np.linalg.eigh(T)
     c = Q @ (np.exp(-1j * tau * lam) * Q[0, :])

@@ -42,8 +42,10 @@ def neel_mps(L):
 
 class SymmTDVP:
     def __init__(self, L, t_h, U, krylov_dim=10, chi_max_full=10 ** 9, eps_trunc=-1.0,
-                 A=None, dims=None):
+                 A=None, dims=None, krylov_adapt_tol=0.0):
         self.L, self.m = L, krylov_dim
+        self.adapt_tol = krylov_adapt_tol     # A-15; 0 = fixed m
+        self.krylov_used = []                 # vectors used by every exponential so far
         self.chi_max, self.eps = chi_max_full, eps_trunc
         self.W = [symm.mpo_reduced(i, t_h, U) for i in range(L)]
         if A is None:
@@ -72,7 +74,7 @@ class SymmTDVP:
                     out[k] = np.zeros_like(v)
             return flatten({k: out[k] for k in theta})
 
-        return unflatten(lanczos_exp(apply_h, flatten(theta), tau, self.m), theta)
+        return unflatten(lanczos_exp(apply_h, flatten(theta), tau, self.m, adapt_tol=self.adapt_tol, stats=self.krylov_used), theta)
 
     def _evolve1(self, i, Ac, Le, Re, tau):
         st1, st2 = symm.heff1_tasks(sorted(Le), sorted(Re), sorted(Ac), self.W[i])
@@ -86,7 +88,7 @@ class SymmTDVP:
                     out[k] = np.zeros_like(v)
             return flatten({k: out[k] for k in Ac})
 
-        return unflatten(lanczos_exp(apply_h, flatten(Ac), tau, self.m), Ac)
+        return unflatten(lanczos_exp(apply_h, flatten(Ac), tau, self.m, adapt_tol=self.adapt_tol, stats=self.krylov_used), Ac)
 
     def _theta(self, i):
         dl, dr = self.dims[i], self.dims[i + 2]
@@ -145,7 +147,7 @@ class SymmTDVP:
                     out[c] = np.zeros_like(x[c])
             return flat(out)
 
-        return unflat(lanczos_exp(apply_h, flat(C), tau, self.m))
+        return unflat(lanczos_exp(apply_h, flat(C), tau, self.m, adapt_tol=self.adapt_tol, stats=self.krylov_used))
 
     def step1(self, dt):
         """One-site TDVP step: L->R (forward one-site tau = dt/2, split, backward zero-site) then R->L.

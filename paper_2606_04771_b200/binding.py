@@ -22,7 +22,8 @@ P = C.POINTER
 
 
 class fh_params(C.Structure):
-    _fields_ = [("krylov_dim", c_int), ("krylov_tol", c_dbl), ("chi_max_full", c_int), ("eps_trunc", c_dbl)]
+    _fields_ = [("krylov_dim", c_int), ("krylov_tol", c_dbl), ("chi_max_full", c_int), ("eps_trunc", c_dbl),
+                ("krylov_adapt_tol", c_dbl)]
 
 
 _SIGS = {
@@ -58,6 +59,8 @@ _SIGS = {
     "heff_flops": (c_i64, [c_void_p]),
     "heff_inner": (c_int, [c_void_p, c_void_p, c_void_p, P(c_dbl)]),
     "heff_expm": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, c_int]),
+    "heff_expm_adaptive": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, c_int, c_dbl, P(c_int)]),
+    "fh_krylov_stats": (c_int, [c_void_p, P(C.c_int64), P(C.c_int64)]),
     "tdvp2_sweep": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, P(fh_params)]),
     "tdvp1_sweep": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, P(fh_params)]),
     "tdvp2_last_stats": (c_int, [c_void_p, P(c_dbl), P(c_int), P(c_int), P(c_int)]),
@@ -321,12 +324,24 @@ class Context:
     def heff_expm(self, theta, out, tau, krylov_dim):
         self.check(lib.heff_expm(self.h, c_void_p(theta.data_ptr()), c_void_p(out.data_ptr()), tau, krylov_dim), "heff_expm")
 
-    def tdvp2_sweep(self, mpo, mps, dt, krylov_dim=10, krylov_tol=1e-12, chi_max_full=1 << 30, eps_trunc=-1.0):
-        p = fh_params(krylov_dim, krylov_tol, chi_max_full, eps_trunc)
+    def heff_expm_adaptive(self, theta, out, tau, krylov_dim, adapt_tol):
+        k = c_int(0)
+        self.check(lib.heff_expm_adaptive(self.h, c_void_p(theta.data_ptr()), c_void_p(out.data_ptr()), tau,
+                                          krylov_dim, adapt_tol, C.byref(k)), "heff_expm_adaptive")
+        return k.value
+
+    def fh_krylov_stats(self):
+        a, b = C.c_int64(0), C.c_int64(0)
+        self.check(lib.fh_krylov_stats(self.h, C.byref(a), C.byref(b)), "fh_krylov_stats")
+        return a.value, b.value
+
+    def tdvp2_sweep(self, mpo, mps, dt, krylov_dim=10, krylov_tol=1e-12, chi_max_full=1 << 30, eps_trunc=-1.0,
+                    krylov_adapt_tol=0.0):
+        p = fh_params(krylov_dim, krylov_tol, chi_max_full, eps_trunc, krylov_adapt_tol)
         self.check(lib.tdvp2_sweep(self.h, mpo, mps, dt, C.byref(p)), "tdvp2_sweep")
 
-    def tdvp1_sweep(self, mpo, mps, dt, krylov_dim=10, krylov_tol=1e-12):
-        p = fh_params(krylov_dim, krylov_tol, 1 << 30, -1.0)
+    def tdvp1_sweep(self, mpo, mps, dt, krylov_dim=10, krylov_tol=1e-12, krylov_adapt_tol=0.0):
+        p = fh_params(krylov_dim, krylov_tol, 1 << 30, -1.0, krylov_adapt_tol)
         self.check(lib.tdvp1_sweep(self.h, mpo, mps, dt, C.byref(p)), "tdvp1_sweep")
 
     def tdvp2_last_stats(self):

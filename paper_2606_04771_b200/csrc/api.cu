@@ -217,25 +217,58 @@ static void jacobi_eig(int n, std::vector<double>& Amat, std::vector<double>& Q)
   }
 }
 
+// u = exp(-i tau T_k) e_1 for the k x k tridiagonal T_k(alpha, beta) through its symmetric eigendecomposition (H7)
+static std::vector<cplx> tridiag_exp_col(const std::vector<double>& alpha, const std::vector<double>& beta, int k,
+                                         double tau) {
+  std::vector<double> T(k * k, 0.0), Q;
+  for (int i = 0; i < k; ++i) {
+    T[i * k + i] = alpha[i];
+    if (i + 1 < k) T[i * k + i + 1] = T[(i + 1) * k + i] = beta[i];
+  }
+  jacobi_eig(k, T, Q);
+  std::vector<cplx> u(k);
+  for (int i = 0; i < k; ++i) {
+    double re = 0.0, im = 0.0;
+    for (int l = 0; l < k; ++l) {
+      const double lam = T[l * k + l], wgt = Q[i * k + l] * Q[0 * k + l];
+      re += wgt * std::cos(tau * lam);
+      im -= wgt * std::sin(tau * lam);
+    }
+    u[i] = make_double2(re, im);
+  }
+  return u;
+}
+
 // theta <- exp(-i tau H_eff) theta (H6 + H7).  work holds (m+1) vectors of n elements.
-// The recurrence keeps alpha_j, <w,w> and beta_j in device memory (P.d_scal): no host round trip
-// inside the iteration; one copy of 2m+1 scalars at the end, then the m x m tridiagonal problem on the
-// host.  After a happy breakdown (beta_j < tol) the remaining directions are zero vectors and the host
-// truncates the Krylov space at j.
-void fh::expm_lanczos(fh_ctx* ctx, cplx* theta, double tau, int m, double tol, cplx* V) {
+// The recurrence keeps alpha_j, <w,w> and beta_j in device memory (P.d_scal): with a fixed Krylov
+// dimension (adapt_tol <= 0) there is no host round trip inside the iteration -- one copy of the scalars
+// at the end, then the m x m tridiagonal problem on the host.  After a happy breakdown (beta_j < tol) the
+// remaining directions are zero vectors and the host truncates the Krylov space at j.
+// adapt_tol > 0 (NEXT-2, reading A-15): the scalars are read back after every step and the process stops
+// with k = j + 1 vectors as soon as |tau| beta_j |e_k^T exp(-i tau T_k) e_1| <= adapt_tol (the norm of the
+// ODE residual of the Krylov approximation times the step); one stream synchronisation per step.
+int fh::expm_lanczos(fh_ctx* ctx, cplx* theta, double tau, int m, double tol, cplx* V, double adapt_tol) {
   Plan& P = ctx->plan;
   const int64_t n = P.vec.nelem;
   FH_REQUIRE(m >= 1 && m <= 32, FH_EINVAL, "krylov_dim must be in [1, 32]");
-  if (n == 0 || P.chunks.empty()) return;
+  if (n == 0 || P.chunks.empty()) return 0;
   cudaStream_t s = ctx->stream;
   const int nch = (int)P.chunks.size();
   // device scalars: [0,1] <theta,theta>, then per j: alpha pair at 2 + 4j, <w,w> pair at 4 + 4j; betas after
   double* d_sc = P.d_scal;
   double* d_beta = P.d_scal + 2 + 4 * 32;
+  const int nsc = 2 + 4 * 32 + 32;
+  ctx->ensure_pinned(nsc);
+  auto fetch_scalars = [&]() {
+    FH_CUDA(cudaMemcpyAsync(ctx->h_pinned, d_sc, nsc * sizeof(double), cudaMemcpyDeviceToHost, s));
+    FH_CUDA(cudaStreamSynchronize(s));
+  };
   ctx->timer_begin(T_VEC);
   launch_wdot(P.d_chunks, nch, theta, theta, P.d_partial, d_sc, s, &ctx->launches);
   launch_scale_rsqrt_dev(n, d_sc, 0.0, theta, V, nullptr, s, &ctx->launches);
   ctx->timer_end();
+  std::vector<double> alpha, beta;
+  int k = 0;  // > 0 once the adaptive rule (or a breakdown seen by it) has fixed the dimension
   for (int j = 0; j < m; ++j) {
     cplx* vj = V + (int64_t)j * n;
     cplx* w = V + (int64_t)(j + 1) * n;
@@ -251,45 +284,49 @@ void fh::expm_lanczos(fh_ctx* ctx, cplx* theta, double tau, int m, double tol, c
       launch_scale_rsqrt_dev(n, d_sc + 4 + 4 * j, tol, w, w, d_beta + j, s, &ctx->launches);
     }
     ctx->timer_end();
-  }
-  const int nsc = 2 + 4 * 32 + 32;
-  ctx->ensure_pinned(nsc);
-  FH_CUDA(cudaMemcpyAsync(ctx->h_pinned, d_sc, nsc * sizeof(double), cudaMemcpyDeviceToHost, s));
-  FH_CUDA(cudaStreamSynchronize(s));
-  const double nrm2 = ctx->h_pinned[0];
-  if (!(nrm2 > 0.0)) return;  // zero vector: theta is untouched (V holds zeros)
-  const double nrm = std::sqrt(nrm2);
-  std::vector<double> alpha, beta;
-  int k = 0;
-  for (int j = 0; j < m; ++j) {
-    alpha.push_back(ctx->h_pinned[2 + 4 * j]);
-    k = j + 1;
-    if (j == m - 1) break;
-    const double bj = ctx->h_pinned[2 + 4 * 32 + j];
-    if (bj < tol) break;
-    beta.push_back(bj);
-  }
-  // host: c = exp(-i tau T) e_1 through the symmetric eigendecomposition of T (H7)
-  std::vector<double> T(k * k, 0.0), Q;
-  for (int i = 0; i < k; ++i) {
-    T[i * k + i] = alpha[i];
-    if (i + 1 < k) T[i * k + i + 1] = T[(i + 1) * k + i] = beta[i];
-  }
-  jacobi_eig(k, T, Q);
-  std::vector<cplx> c(k);
-  for (int i = 0; i < k; ++i) {
-    double re = 0.0, im = 0.0;
-    for (int l = 0; l < k; ++l) {
-      const double lam = T[l * k + l], wgt = Q[i * k + l] * Q[0 * k + l];
-      re += wgt * std::cos(tau * lam);
-      im -= wgt * std::sin(tau * lam);
+    if (adapt_tol > 0.0 && j < m - 1) {
+      fetch_scalars();
+      if (!(ctx->h_pinned[0] > 0.0)) return 0;  // zero vector
+      alpha.push_back(ctx->h_pinned[2 + 4 * j]);
+      const double bj = ctx->h_pinned[2 + 4 * 32 + j];
+      if (bj < tol) {
+        k = j + 1;
+        break;
+      }
+      const std::vector<cplx> u = tridiag_exp_col(alpha, beta, j + 1, tau);
+      const double est = std::fabs(tau) * bj * std::hypot(u[j].x, u[j].y);
+      if (est <= adapt_tol) {
+        k = j + 1;
+        break;
+      }
+      beta.push_back(bj);
     }
-    c[i] = make_double2(nrm * re, nrm * im);
   }
+  if (k == 0) {
+    fetch_scalars();
+    alpha.clear();
+    beta.clear();
+    for (int j = 0; j < m; ++j) {
+      alpha.push_back(ctx->h_pinned[2 + 4 * j]);
+      k = j + 1;
+      if (j == m - 1) break;
+      const double bj = ctx->h_pinned[2 + 4 * 32 + j];
+      if (bj < tol) break;
+      beta.push_back(bj);
+    }
+  }
+  const double nrm2 = ctx->h_pinned[0];
+  if (!(nrm2 > 0.0)) return 0;  // zero vector: theta is untouched (V holds zeros)
+  const double nrm = std::sqrt(nrm2);
+  std::vector<cplx> c = tridiag_exp_col(alpha, beta, k, tau);
+  for (auto& ci : c) ci = make_double2(nrm * ci.x, nrm * ci.y);
   ctx->timer_begin(T_VEC);
   launch_lincomb(n, k, c.data(), V, n, theta, s, &ctx->launches);
   ctx->timer_end();
   FH_CUDA(cudaGetLastError());
+  ctx->krylov_calls += 1;
+  ctx->krylov_vectors += k;
+  return k;
 }
 
 // ============================================================================ environments
@@ -739,7 +776,8 @@ int heff_inner(fh_ctx* ctx, const void* x_dev, const void* y_dev, double* result
   })
 }
 
-int heff_expm(fh_ctx* ctx, const void* theta_dev, void* out_dev, double tau, int krylov_dim) {
+static int heff_expm_impl(fh_ctx* ctx, const void* theta_dev, void* out_dev, double tau, int krylov_dim,
+                          double adapt_tol, int* k_used) {
   FH_TRY(ctx, {
     FH_REQUIRE(ctx && theta_dev && out_dev, FH_EINVAL, "heff_expm: NULL argument");
     FH_REQUIRE(ctx->plan.valid, FH_ESTATE, "heff_expm: no plan");
@@ -748,13 +786,34 @@ int heff_expm(fh_ctx* ctx, const void* theta_dev, void* out_dev, double tau, int
     try {
       if (out_dev != theta_dev)
         FH_CUDA(cudaMemcpyAsync(out_dev, theta_dev, n * sizeof(cplx), cudaMemcpyDeviceToDevice, ctx->stream));
-      expm_lanczos(ctx, (cplx*)out_dev, tau, krylov_dim, 1e-12, ctx->ptr(woff));
+      const int k = expm_lanczos(ctx, (cplx*)out_dev, tau, krylov_dim, 1e-12, ctx->ptr(woff), adapt_tol);
+      if (k_used) *k_used = k;
     } catch (...) {
       ctx->alloc.release(woff, (int64_t)(krylov_dim + 1) * n);
       throw;
     }
     ctx->alloc.release(woff, (int64_t)(krylov_dim + 1) * n);
   })
+}
+
+int heff_expm(fh_ctx* ctx, const void* theta_dev, void* out_dev, double tau, int krylov_dim) {
+  return heff_expm_impl(ctx, theta_dev, out_dev, tau, krylov_dim, 0.0, nullptr);
+}
+
+int heff_expm_adaptive(fh_ctx* ctx, const void* theta_dev, void* out_dev, double tau, int krylov_dim,
+                       double adapt_tol, int* k_used) {
+  if (!(adapt_tol > 0.0)) {
+    if (ctx) ctx->err = "heff_expm_adaptive: adapt_tol must be > 0";
+    return FH_EINVAL;
+  }
+  return heff_expm_impl(ctx, theta_dev, out_dev, tau, krylov_dim, adapt_tol, k_used);
+}
+
+int fh_krylov_stats(const fh_ctx* ctx, int64_t* n_exponentials, int64_t* n_vectors) {
+  if (!ctx) return FH_EINVAL;
+  if (n_exponentials) *n_exponentials = ctx->krylov_calls;
+  if (n_vectors) *n_vectors = ctx->krylov_vectors;
+  return FH_OK;
 }
 
 int tdvp2_sweep(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh_params* p) {

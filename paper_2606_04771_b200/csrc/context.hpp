@@ -120,6 +120,7 @@ struct fh_ctx {
   cudaEvent_t svd_fork = nullptr;
   int device = 0;
   int64_t svd_count[3] = {0, 0, 0};  // gesvd, gesvdp, gesvdp fallbacks to gesvd
+  int64_t krylov_calls = 0, krylov_vectors = 0;  // exponentials evaluated / Krylov vectors (= H_eff applies) used
   // last sweep statistics
   double stat_disc = 0.0;
   int stat_chi = 0, stat_su2 = 0, stat_dmax = 0;
@@ -148,7 +149,9 @@ void upload_stage(DevPool& pool, Stage& st, cudaStream_t s);
 void plan_heff(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, int nsite);
 void apply_heff(fh_ctx* ctx, const cplx* theta, cplx* out);
 double2 inner(fh_ctx* ctx, const cplx* x, const cplx* y);  // synchronises
-void expm_lanczos(fh_ctx* ctx, cplx* theta_inout, double tau, int m, double tol, cplx* work /* (m+1)*n */);
+// returns the number of Krylov vectors used; adapt_tol > 0 enables the adaptive stop (reading A-15)
+int expm_lanczos(fh_ctx* ctx, cplx* theta_inout, double tau, int m, double tol, cplx* work /* (m+1)*n */,
+                 double adapt_tol = 0.0);
 void do_env_update_left(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int site);
 void do_env_update_right(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int site);
 void sweep(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh_params* p);

@@ -631,7 +631,7 @@ static void local_update2(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int i, do
     launch_grouped_gemm(st, ctx->ptr(mps->A[i].base), ctx->ptr(mps->A[i + 1].base), theta, ctx->stream, &ctx->launches);
     ctx->timer_end();
   }
-  expm_lanczos(ctx, theta, tau, m, prm->krylov_tol, V);
+  expm_lanczos(ctx, theta, tau, m, prm->krylov_tol, V, prm->krylov_adapt_tol);
   BlockTensor th = P.vec;  // copy: svd_split re-plans nothing but keeps the layout alive
   svd_split(ctx, mps, i, th, theta, direction, prm);
   ctx->alloc.release(woff, wn);
@@ -645,7 +645,7 @@ static void local_update1(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int i, do
   const int m = prm->krylov_dim;
   const int64_t wn = (int64_t)(m + 1) * n;
   const int64_t woff = ctx->alloc.alloc(wn);
-  expm_lanczos(ctx, ctx->ptr(mps->A[i].base), tau, m, prm->krylov_tol, ctx->ptr(woff));
+  expm_lanczos(ctx, ctx->ptr(mps->A[i].base), tau, m, prm->krylov_tol, ctx->ptr(woff), prm->krylov_adapt_tol);
   ctx->alloc.release(woff, wn);
 }
 
@@ -857,7 +857,7 @@ static void zero_site_update(fh_ctx* ctx, const BlockTensor& Le, const BlockTens
   const int m = prm->krylov_dim;
   const int64_t wn = (int64_t)(m + 1) * n;
   const int64_t woff = ctx->alloc.alloc(wn);
-  expm_lanczos(ctx, ctx->ptr(C.base), tau, m, prm->krylov_tol, ctx->ptr(woff));
+  expm_lanczos(ctx, ctx->ptr(C.base), tau, m, prm->krylov_tol, ctx->ptr(woff), prm->krylov_adapt_tol);
   ctx->alloc.release(woff, wn);
 }
 

@@ -400,6 +400,75 @@ def test_next1_one_site_tdvp_L8_vs_oracle(H, ctx):
     ctx.mps_destroy(mps)
 
 
+# ------------------------------------------------------------------ NEXT-2: adaptive Krylov dimension (A-15)
+def test_next2_adaptive_krylov_expm_and_sweeps(H, ctx):
+    """(a) heff_expm_adaptive on the chi = 256 central bond: same number of Krylov vectors as the oracle's
+    adaptive Lanczos for each tolerance, result within 1e-10, fewer vectors for the looser tolerance, and
+    within ~tol of the fixed m = 20 result.  (b) L = 8 quench driven with krylov_adapt_tol = 1e-10 (two-site
+    steps, then one-site steps): observables <= 1e-8 against the oracle running the same rule, and the same
+    total number of H_eff applies."""
+    chi, L, tau, mmax = 256, 60, 0.025, 20
+    o = central_bond(chi, L)
+    c = o["centre"]
+    dl, dr = o["dims"][c], o["dims"][c + 2]
+    th = fi.theta_random(fi.SEED, c, dl, dr)
+    W1, W2 = o["W"][c], o["W"][c + 1]
+
+    def apply_h(vec):
+        t = stv.unflatten(vec, th)
+        out = symm.heff2_apply(o["Lenv"], o["Renv"], t, W1, W2)
+        return stv.flatten({k: out[k] for k in th})
+
+    mpo = ctx.fh_mpo_build(L, 1.0, 4.0)
+    mps, _ = H.build_central_bond(ctx, mpo, chi, L)
+    ctx.heff_plan(mpo, mps, c, 2)
+    lab, dm, ne = ctx.heff_layout(2)
+    x = _dev(H.flatten(th, lab, dm, H.theta_key))
+    y = _torch().empty_like(x)
+    yfix = _torch().empty_like(x)
+    ctx.heff_expm(x, yfix, tau, mmax)
+    nx = float(ctx.heff_inner(x, x).real) ** 0.5
+    used = {}
+    for tol in (1e-4, 1e-8, 1e-12):
+        st = []
+        ref = stv.unflatten(lanczos_exp(apply_h, stv.flatten(th), tau, mmax, adapt_tol=tol, stats=st), th)
+        k = ctx.heff_expm_adaptive(x, y, tau, mmax, tol)
+        assert k == st[0], (tol, k, st)
+        used[tol] = k
+        got = H.unflatten(y.cpu().numpy(), lab, dm, H.theta_key)
+        assert rel_err(got, ref) < 1e-10
+        d = y - yfix
+        assert float(ctx.heff_inner(d, d).real) ** 0.5 / nx < 10 * tol + 1e-12
+    assert used[1e-4] < used[1e-8] < used[1e-12] < mmax
+    print("adaptive Krylov, chi=256 central bond, tau=0.025: k =", used)
+    ctx.mps_destroy(mps)
+
+    L, t_h, U, dt, tol = 8, 1.0, 4.0, 0.05, 1e-10
+    ref = stv.SymmTDVP(L, t_h, U, krylov_dim=mmax, chi_max_full=256, eps_trunc=1e-12, krylov_adapt_tol=tol)
+    mpo = ctx.fh_mpo_build(L, t_h, U)
+    mps = ctx.mps_init_neel(mpo, L)
+    e0, v0 = ctx.fh_krylov_stats()
+    worst = 0.0
+    for step in range(8):
+        if step < 5:
+            ref.step(dt)
+            ctx.tdvp2_sweep(mpo, mps, dt, krylov_dim=mmax, chi_max_full=256, eps_trunc=1e-12, krylov_adapt_tol=tol)
+        else:
+            ref.step1(dt)
+            ctx.tdvp1_sweep(mpo, mps, dt, krylov_dim=mmax, krylov_adapt_tol=tol)
+        a, b = ref.measure_local(), ctx.measure_local(mps, L)
+        for key in ("n", "sz", "docc"):
+            worst = max(worst, np.abs(a[key] - b[key]).max())
+    e1, v1 = ctx.fh_krylov_stats()
+    ku = [k for k in ref.krylov_used if k > 0]
+    print("adaptive TDVP L=8: %d exponentials, %d applies (oracle %d, %d; fixed m would use %d); max obs diff %.2e"
+          % (e1 - e0, v1 - v0, len(ku), sum(ku), mmax * len(ku), worst))
+    assert worst < 1e-8, worst
+    assert e1 - e0 == len(ku) and v1 - v0 == sum(ku)
+    assert sum(ku) < 0.6 * mmax * len(ku)
+    ctx.mps_destroy(mps)
+
+
 # ------------------------------------------------------------------ edge cases and errors
 def test_edge_cases_and_error_codes(H, ctx):
     B = H.binding

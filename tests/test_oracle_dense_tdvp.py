@@ -117,3 +117,84 @@ def test_tdvp1_on_saturated_bonds_vs_ed_and_time_step_order():
     C1 = rng.standard_normal((Le.shape[0], Re.shape[0])) + 1j * rng.standard_normal((Le.shape[0], Re.shape[0]))
     C2 = rng.standard_normal(C1.shape) + 1j * rng.standard_normal(C1.shape)
     assert abs(np.vdot(C1, dt.heff0(Le, Re, C2)) - np.conj(np.vdot(C2, dt.heff0(Le, Re, C1)))) < 1e-10
+
+
+# ---- NEXT-2, reading A-15: adaptive Krylov dimension -------------------------------------------
+def _rand_herm(n, scale, seed):
+    rng = np.random.default_rng(seed)
+    a = rng.normal(size=(n, n)) + 1j * rng.normal(size=(n, n))
+    h = (a + a.conj().T) / 2
+    return h * (scale / np.linalg.norm(h, 2))
+
+
+def test_krylov_residual_is_the_ode_residual():
+    """The stopping estimate is |tau| |r_k(tau)| with r_k = y_k' + i H y_k the residual of the Krylov
+    approximation in y' = -i H y.  Brute force: build V_k, T_k by plain Lanczos here, evaluate the residual
+    vector from its definition and compare its norm with the oracle's estimate / |tau|."""
+    n, k, tau = 60, 5, 0.37
+    H = _rand_herm(n, 3.0, 11)
+    rng = np.random.default_rng(12)
+    v = rng.normal(size=n) + 1j * rng.normal(size=n)
+    v /= np.linalg.norm(v)
+    V = [v]
+    alpha, beta = [], []
+    for j in range(k):
+        w = H @ V[j]
+        alpha.append(np.vdot(V[j], w).real)
+        w = w - alpha[j] * V[j] - (beta[j - 1] * V[j - 1] if j else 0)
+        for u in V:
+            w = w - np.vdot(u, w) * u
+        b = np.linalg.norm(w)
+        if j < k - 1:
+            beta.append(b)
+            V.append(w / b)
+    Vk = np.array(V).T
+    Tk = Vk.conj().T @ H @ Vk
+    u = sla.expm(-1j * tau * Tk)[:, 0]
+    y = Vk @ u
+    ydot = Vk @ (-1j * Tk @ u)
+    r = ydot + 1j * (H @ y)
+    est = dt.krylov_residual_estimate(alpha, beta, b, tau)
+    assert abs(np.linalg.norm(r) - est / tau) < 1e-12 * max(1.0, np.linalg.norm(r))
+
+
+def test_adaptive_krylov_meets_tolerance_and_bounds_error():
+    """error(y_k(tau)) <= int_0^tau |r_k| <= estimate whenever |r_k(s)| is increasing on [0, tau] (true for
+    tau |H| small against k); so the adaptive result is within adapt_tol of expm, and uses fewer vectors for
+    a looser tolerance or a shorter step."""
+    n = 120
+    H = _rand_herm(n, 4.0, 21)
+    rng = np.random.default_rng(22)
+    v = rng.normal(size=n) + 1j * rng.normal(size=n)
+    used = {}
+    for tau in (0.05, 0.2, 0.5):
+        exact = sla.expm(-1j * tau * H) @ v
+        for tol in (1e-4, 1e-8, 1e-12):
+            st = []
+            y = dt.lanczos_exp(lambda x: H @ x, v, tau, 30, adapt_tol=tol, stats=st)
+            err = np.linalg.norm(y - exact) / np.linalg.norm(v)
+            assert err <= tol + 1e-13, (tau, tol, err, st)
+            assert 1 <= st[0] < 30
+            used[(tau, tol)] = st[0]
+    for tau in (0.05, 0.2, 0.5):
+        assert used[(tau, 1e-4)] < used[(tau, 1e-8)] < used[(tau, 1e-12)]
+    for tol in (1e-4, 1e-8, 1e-12):
+        assert used[(0.05, tol)] < used[(0.2, tol)] < used[(0.5, tol)]
+
+
+def test_adaptive_krylov_off_and_cap():
+    """adapt_tol = 0 is the fixed-m process bit for bit; a cap m smaller than the adaptive choice wins."""
+    H = _rand_herm(50, 5.0, 31)
+    rng = np.random.default_rng(32)
+    v = rng.normal(size=50) + 1j * rng.normal(size=50)
+    a = dt.lanczos_exp(lambda x: H @ x, v, 0.3, 8)
+    b = dt.lanczos_exp(lambda x: H @ x, v, 0.3, 8, adapt_tol=0.0)
+    assert np.array_equal(a, b)
+    st = []
+    c = dt.lanczos_exp(lambda x: H @ x, v, 0.3, 4, adapt_tol=1e-14, stats=st)
+    assert st == [4]
+    assert np.array_equal(c, dt.lanczos_exp(lambda x: H @ x, v, 0.3, 4))
+    # a stop at k gives exactly the fixed-k result
+    st = []
+    d = dt.lanczos_exp(lambda x: H @ x, v, 0.3, 30, adapt_tol=1e-6, stats=st)
+    assert np.allclose(d, dt.lanczos_exp(lambda x: H @ x, v, 0.3, st[0]), rtol=0, atol=1e-14)
