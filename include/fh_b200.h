@@ -157,6 +157,13 @@ int tdvp2_sweep(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh
  * never grow.  Preconditions and state on return as tdvp2_sweep (centre on site 0, right environments
  * built); krylov_dim and krylov_tol of params are used, chi_max_full and eps_trunc are not. */
 int tdvp1_sweep(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh_params* params);
+/* The paper's adaptive driver (reading A-16): one full time step dt that is a two-site
+ * step (tdvp2_sweep) until a two-site step has left the full dimension sum_c d_c (2 j_c + 1) of EVERY bond
+ * no larger than before it ("the bond dimension has saturated": capped by chi_max_full in the bulk, exact at
+ * the edges), and a one-site step (tdvp1_sweep) from then on; the flag lives in the fh_mps and is never
+ * cleared.  *nsite_used (host, may be NULL) receives 2 or 1. */
+int tdvp_sweep_auto(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh_params* params,
+                    int* nsite_used);
 /* statistics of the last sweep: max discarded weight, max chi_full, max chi_su2, max d */
 int tdvp2_last_stats(const fh_ctx* ctx, double* max_discarded, int* chi_full, int* chi_su2, int* dmax);
 

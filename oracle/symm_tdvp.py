@@ -220,3 +220,15 @@ class SymmTDVP:
 
     def chi(self):
         return [symm.chi_full(d) for d in self.dims]
+
+    def step_auto(self, dt):
+        """Reading A-16 of PAPER.md:53, 250 ("switch from the two-site to the one-site update once the bond
+        dimension has saturated"): two-site steps until one of them grows no bond's full dimension, one-site
+        steps from then on.  Returns 2 or 1."""
+        if getattr(self, "saturated", False):
+            self.step1(dt)
+            return 1
+        before = self.chi()
+        self.step(dt)
+        self.saturated = all(a <= b for a, b in zip(self.chi(), before))
+        return 2

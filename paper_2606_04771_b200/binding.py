@@ -63,6 +63,7 @@ _SIGS = {
     "fh_krylov_stats": (c_int, [c_void_p, P(C.c_int64), P(C.c_int64)]),
     "tdvp2_sweep": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, P(fh_params)]),
     "tdvp1_sweep": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, P(fh_params)]),
+    "tdvp_sweep_auto": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, P(fh_params), P(c_int)]),
     "tdvp2_last_stats": (c_int, [c_void_p, P(c_dbl), P(c_int), P(c_int), P(c_int)]),
     "measure_local": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
     "measure_global": (c_int, [c_void_p, c_void_p, c_void_p, P(c_dbl), P(c_dbl)]),
@@ -339,6 +340,13 @@ class Context:
                     krylov_adapt_tol=0.0):
         p = fh_params(krylov_dim, krylov_tol, chi_max_full, eps_trunc, krylov_adapt_tol)
         self.check(lib.tdvp2_sweep(self.h, mpo, mps, dt, C.byref(p)), "tdvp2_sweep")
+
+    def tdvp_sweep_auto(self, mpo, mps, dt, krylov_dim=10, krylov_tol=1e-12, chi_max_full=1 << 30, eps_trunc=-1.0,
+                        krylov_adapt_tol=0.0):
+        p = fh_params(krylov_dim, krylov_tol, chi_max_full, eps_trunc, krylov_adapt_tol)
+        n = c_int(0)
+        self.check(lib.tdvp_sweep_auto(self.h, mpo, mps, dt, C.byref(p), C.byref(n)), "tdvp_sweep_auto")
+        return n.value
 
     def tdvp1_sweep(self, mpo, mps, dt, krylov_dim=10, krylov_tol=1e-12, krylov_adapt_tol=0.0):
         p = fh_params(krylov_dim, krylov_tol, 1 << 30, -1.0, krylov_adapt_tol)

@@ -824,6 +824,26 @@ int tdvp2_sweep(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh
   })
 }
 
+int tdvp_sweep_auto(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh_params* p, int* nsite_used) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && mpo && mps && p, FH_EINVAL, "tdvp_sweep_auto: NULL argument");
+    FH_REQUIRE(p->krylov_dim >= 2 && p->krylov_dim <= 32 && p->chi_max_full >= 1, FH_EINVAL,
+               "tdvp_sweep_auto: bad parameters");
+    if (mps->saturated) {
+      if (nsite_used) *nsite_used = 1;
+      sweep1(ctx, mpo, mps, dt, p);
+    } else {
+      if (nsite_used) *nsite_used = 2;
+      std::vector<int> before;
+      for (const auto& b : mps->bond) before.push_back(b.chi_full());
+      sweep(ctx, mpo, mps, dt, p);
+      bool grew = false;
+      for (size_t k = 0; k < mps->bond.size(); ++k) grew = grew || mps->bond[k].chi_full() > before[k];
+      mps->saturated = !grew;
+    }
+  })
+}
+
 int tdvp1_sweep(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh_params* p) {
   FH_TRY(ctx, {
     FH_REQUIRE(ctx && mpo && mps && p, FH_EINVAL, "tdvp1_sweep: NULL argument");

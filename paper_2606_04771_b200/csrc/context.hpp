@@ -80,6 +80,7 @@ struct fh_mps {
   std::vector<fh::Bond> bond;                       // L+1
   std::vector<fh::BlockTensor> A, Lenv, Renv;       // L, L+1, L+1
   std::vector<std::vector<double>> sval;            // L+1: kept singular values of the last split
+  bool saturated = false;                           // tdvp_sweep_auto: a two-site step grew no bond (A-16)
 };
 
 struct fh_ctx {

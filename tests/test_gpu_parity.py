@@ -469,6 +469,29 @@ def test_next2_adaptive_krylov_expm_and_sweeps(H, ctx):
     ctx.mps_destroy(mps)
 
 
+def test_next1_auto_switch_two_site_to_one_site(H, ctx):
+    """tdvp_sweep_auto (reading A-16): L = 8 quench with the bond dimension capped at chi_full = 40; the
+    two-site steps stop growing any bond after the third step, both sides switch to one-site steps there
+    (same 2/1 sequence), observables stay within 1e-8 and the sector tables stay identical."""
+    L, t_h, U, dt, m, cap = 8, 1.0, 4.0, 0.05, 10, 40
+    ref = stv.SymmTDVP(L, t_h, U, krylov_dim=m, chi_max_full=cap, eps_trunc=-1.0)
+    mpo = ctx.fh_mpo_build(L, t_h, U)
+    mps = ctx.mps_init_neel(mpo, L)
+    seq_o, seq_g, worst = [], [], 0.0
+    for step in range(8):
+        seq_o.append(ref.step_auto(dt))
+        seq_g.append(ctx.tdvp_sweep_auto(mpo, mps, dt, krylov_dim=m, chi_max_full=cap, eps_trunc=-1.0))
+        a, b = ref.measure_local(), ctx.measure_local(mps, L)
+        for key in ("n", "sz", "docc"):
+            worst = max(worst, np.abs(a[key] - b[key]).max())
+        for k in range(1, L):
+            assert ctx.mps_get_bond(mps, k) == ref.dims[k], (step, k)
+    print("auto switch: oracle", seq_o, "GPU", seq_g, "max obs diff %.2e" % worst)
+    assert seq_g == seq_o and seq_g[0] == 2 and seq_g[-1] == 1
+    assert worst < 1e-8, worst
+    ctx.mps_destroy(mps)
+
+
 # ------------------------------------------------------------------ edge cases and errors
 def test_edge_cases_and_error_codes(H, ctx):
     B = H.binding

@@ -274,3 +274,30 @@ def test_one_site_tdvp_pieces_and_driver_vs_dense():
         worst = max(worst, np.abs(a["sz"] - 0.5 * (b["n_up"] - b["n_dn"])).max(), np.abs(a["docc"] - b["docc"]).max())
     assert worst < 1e-9, worst
     assert abs(sy.measure_global()["norm2"] - b["norm2"]) < 1e-10
+
+
+def test_auto_switch_reading_A16_vs_ed():
+    """Reading A-16: step_auto takes two-site steps until one of them grows no bond, then one-site steps.
+    L = 4 untruncated: the bonds reach their maximal dimensions (4, 16, 4); the step after that grows nothing
+    and flips the switch; on the saturated manifold one-site TDVP is exact up to the splitting error, so the
+    observables keep following exact diagonalisation.  With a cap the switch comes as soon as the cap binds."""
+    from oracle import symm_tdvp as stv
+    L, t_h, U, dtime = 4, 1.0, 4.0, 0.05
+    s = stv.SymmTDVP(L, t_h, U, krylov_dim=10)
+    ed = fermi.ExactEvolution(L, t_h, U)
+    seq, err = [], 0.0
+    for k in range(1, 21):
+        chi_before = s.chi()
+        n = s.step_auto(dtime)
+        seq.append(n)
+        if n == 1:
+            assert s.chi() == chi_before            # one-site steps never change a bond here
+        o, e = s.measure_local(), ed.observables(dtime * k)
+        err = max(err, np.abs(o["docc"] - e["docc"]).max(), np.abs(0.5 + o["sz"] - e["n_up"]).max())
+    first1 = seq.index(1)
+    assert first1 >= 2 and all(x == 2 for x in seq[:first1]) and all(x == 1 for x in seq[first1:])
+    assert s.chi() == [1, 4, 16, 4, 1]
+    assert err < 5e-6, err                           # splitting error only (dt = 0.05)
+    capped = stv.SymmTDVP(6, t_h, U, krylov_dim=10, chi_max_full=12)
+    seq = [capped.step_auto(dtime) for _ in range(5)]
+    assert seq[0] == 2 and seq[-1] == 1 and max(capped.chi()) <= 12
