@@ -6,6 +6,7 @@
 
 #include <array>
 #include <map>
+#include <unordered_map>
 #include <string>
 #include <vector>
 
@@ -33,6 +34,13 @@ inline bool triangle(int t1, int t2, int t3) {
 
 // flattened label tuple, zero padded; compared lexicographically (== Python tuple order)
 typedef std::array<int, 12> Key;
+struct KeyHash {
+  size_t operator()(const Key& k) const {
+    uint64_t h = 1469598103934665603ull;
+    for (int v : k) h = (h ^ (uint64_t)(uint32_t)v) * 1099511628211ull;
+    return (size_t)(h ^ (h >> 29));
+  }
+};
 
 struct Bond {
   std::vector<Sector> sec;  // sorted
@@ -54,7 +62,7 @@ struct BlockTensor {
   int64_t nelem = 0;
   int64_t base = -1;  // element offset in the arena, -1 = not allocated
   int nlab = 0;       // number of meaningful ints in each key
-  std::map<Key, int> index;
+  std::unordered_map<Key, int, KeyHash> index;
   void clear();
   void add(const Key& k, int r, int c);  // append (caller adds in sorted order)
   void finalize();                       // offsets (each block 2-element aligned => 32 B)

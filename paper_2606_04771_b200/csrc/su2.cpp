@@ -3,6 +3,7 @@
 // All angular momenta are passed doubled (tj = 2j).  On the hot path s, s', k, r, k' are 0 or
 // 1/2, so every sum has at most a few terms and no cancellation to speak of.
 #include <cmath>
+#include <unordered_map>
 
 #include "fh_internal.hpp"
 
@@ -48,7 +49,28 @@ double wigner6j(int ta, int tb, int tc, int td, int te, int tf) {
 }
 
 // {j1 j2 j3; j4 j5 j6; j7 j8 j9} = sum_x (-1)^{2x} (2x+1) {j1 j4 j7; j8 j9 x} {j2 j5 j8; j4 x j6} {j3 j6 j9; x j1 j2}
+static double wigner9j_sum(int j1, int j2, int j3, int j4, int j5, int j6, int j7, int j8, int j9);
+
+// A plan asks for the same few hundred symbols tens of thousands of times (one per task): memoised per
+// thread on the nine doubled arguments (7 bits each); the stored value is the one the sum returns.
 double wigner9j(int j1, int j2, int j3, int j4, int j5, int j6, int j7, int j8, int j9) {
+  const int a[9] = {j1, j2, j3, j4, j5, j6, j7, j8, j9};
+  uint64_t key = 0;
+  bool packable = true;
+  for (int i = 0; i < 9; ++i) {
+    packable = packable && a[i] >= 0 && a[i] < 128;
+    key = (key << 7) | (uint64_t)(a[i] & 127);
+  }
+  if (!packable) return wigner9j_sum(j1, j2, j3, j4, j5, j6, j7, j8, j9);
+  thread_local std::unordered_map<uint64_t, double> memo;
+  auto it = memo.find(key);
+  if (it != memo.end()) return it->second;
+  const double v = wigner9j_sum(j1, j2, j3, j4, j5, j6, j7, j8, j9);
+  if (memo.size() < (1u << 20)) memo.emplace(key, v);
+  return v;
+}
+
+static double wigner9j_sum(int j1, int j2, int j3, int j4, int j5, int j6, int j7, int j8, int j9) {
   if (!triangle(j1, j2, j3) || !triangle(j4, j5, j6) || !triangle(j7, j8, j9) || !triangle(j1, j4, j7) ||
       !triangle(j2, j5, j8) || !triangle(j3, j6, j9))
     return 0.0;

@@ -56,6 +56,7 @@ void BlockTensor::add(const Key& k, int r, int c) {
 void BlockTensor::finalize() {
   off.resize(keys.size());
   index.clear();
+  index.reserve(keys.size() * 2);
   int64_t n = 0;
   for (size_t i = 0; i < keys.size(); ++i) {
     off[i] = n;
@@ -295,19 +296,60 @@ struct RawTask {
   int lhs, rhs;
   double alpha;
 };
-bool raw_less(const RawTask& a, const RawTask& b) { return a.out != b.out ? a.out < b.out : a.order < b.order; }
 
-// fill st.t_* from raw tasks (sorted here); `out` must already contain every key that occurs
+// the first seven ints of an `order` key packed so that integer order == lexicographic order
+// (each field offset by 64 into 8 bits); false if a field does not fit
+static bool pack_order(const Key& k, uint64_t& packed) {
+  packed = 0;
+  for (int i = 0; i < 7; ++i) {
+    const int v = k[i] + 64;
+    if (v < 0 || v > 255) return false;
+    packed = (packed << 8) | (uint64_t)v;
+  }
+  for (int i = 7; i < 12; ++i)
+    if (k[i] != 0) return false;
+  return true;
+}
+
+// fill st.t_* from raw tasks in canonical order (output block, then `order`); `out` must already contain
+// every key that occurs.  The output index of `out` is ascending in the key, so sorting (index, packed
+// order) pairs gives the same sequence as sorting the 96-byte keys themselves.
 void tasks_to_stage(std::vector<RawTask>& raw, const BlockTensor& out, Stage& st) {
-  std::sort(raw.begin(), raw.end(), raw_less);
+  struct Ref {
+    int o;
+    uint64_t ord;
+    int idx;
+  };
+  std::vector<Ref> refs(raw.size());
+  bool packed_ok = true;
+  for (size_t i = 0; i < raw.size(); ++i) {
+    refs[i].o = out.find(raw[i].out);
+    if (refs[i].o < 0) throw std::runtime_error("task list: output key missing from layout");
+    refs[i].idx = (int)i;
+    packed_ok = packed_ok && pack_order(raw[i].order, refs[i].ord);
+  }
+  if (packed_ok) {
+    std::sort(refs.begin(), refs.end(), [](const Ref& a, const Ref& b) {
+      return a.o != b.o ? a.o < b.o : (a.ord != b.ord ? a.ord < b.ord : a.idx < b.idx);
+    });
+  } else {
+    std::sort(refs.begin(), refs.end(), [&](const Ref& a, const Ref& b) {
+      if (a.o != b.o) return a.o < b.o;
+      if (raw[a.idx].order != raw[b.idx].order) return raw[a.idx].order < raw[b.idx].order;
+      return a.idx < b.idx;
+    });
+  }
   st.t_out.clear();
   st.t_lhs.clear();
   st.t_rhs.clear();
   st.t_alpha.clear();
-  for (const RawTask& r : raw) {
-    const int o = out.find(r.out);
-    if (o < 0) throw std::runtime_error("task list: output key missing from layout");
-    st.t_out.push_back(o);
+  st.t_out.reserve(raw.size());
+  st.t_lhs.reserve(raw.size());
+  st.t_rhs.reserve(raw.size());
+  st.t_alpha.reserve(raw.size());
+  for (const Ref& f : refs) {
+    const RawTask& r = raw[f.idx];
+    st.t_out.push_back(f.o);
     st.t_lhs.push_back(r.lhs);
     st.t_rhs.push_back(r.rhs);
     st.t_alpha.push_back(r.alpha);
@@ -320,11 +362,19 @@ struct Shape {
 };
 void layout_from_tasks(const std::vector<RawTask>& raw, const std::vector<Shape>& shapes, int nlab,
                        BlockTensor& out) {
-  std::map<Key, Shape> m;
-  for (size_t i = 0; i < raw.size(); ++i) m[raw[i].out] = shapes[i];
+  std::unordered_map<Key, int, KeyHash> seen;
+  seen.reserve(raw.size());
+  std::vector<std::pair<Key, Shape>> uniq;
+  for (size_t i = 0; i < raw.size(); ++i) {
+    auto ins = seen.emplace(raw[i].out, (int)uniq.size());
+    if (ins.second) uniq.push_back({raw[i].out, shapes[i]});
+    else uniq[ins.first->second].second = shapes[i];
+  }
+  std::sort(uniq.begin(), uniq.end(),
+            [](const std::pair<Key, Shape>& a, const std::pair<Key, Shape>& b) { return a.first < b.first; });
   out.clear();
   out.nlab = nlab;
-  for (auto& e : m) out.add(e.first, e.second.r, e.second.c);
+  for (auto& e : uniq) out.add(e.first, e.second.r, e.second.c);
   out.finalize();
 }
 
@@ -337,6 +387,8 @@ void emit_left_contraction(const BlockTensor& Lenv, const BlockTensor& ket, cons
   for (size_t i = 0; i < ket.keys.size(); ++i) by_a[key_sector(ket.keys[i], 0)].push_back((int)i);
   std::vector<RawTask> raw;
   std::vector<Shape> shapes;
+  raw.reserve(4 * ket.keys.size());
+  shapes.reserve(4 * ket.keys.size());
   for (size_t e = 0; e < Lenv.keys.size(); ++e) {
     const Key& ek = Lenv.keys[e];
     const Sector ap = key_sector(ek, 0), a = key_sector(ek, 3);
@@ -388,6 +440,7 @@ void emit_heff2(const BlockTensor& Lenv, const BlockTensor& Renv, const BlockTen
   std::map<Sector, std::vector<int>> by_b;
   for (size_t i = 0; i < Renv.keys.size(); ++i) by_b[key_sector(Renv.keys[i], 3)].push_back((int)i);
   std::vector<RawTask> raw;
+  raw.reserve(2 * Z.keys.size());
   for (size_t z = 0; z < Z.keys.size(); ++z) {
     const Key& zk = Z.keys[z];  // a'(0,1) s1'(2) c'(3,4) wm(5) c(6,7) s2(8) b(9,10)
     const Sector ap = key_sector(zk, 0), cp = key_sector(zk, 3), c = key_sector(zk, 6), b = key_sector(zk, 9);
