@@ -61,6 +61,7 @@ _SIGS = {
     "heff_expm": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, c_int]),
     "heff_expm_adaptive": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, c_int, c_dbl, P(c_int)]),
     "fh_krylov_stats": (c_int, [c_void_p, P(C.c_int64), P(C.c_int64)]),
+    "fh_factorization_stats": (c_int, [c_void_p, P(C.c_int64)]),
     "tdvp2_sweep": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, P(fh_params)]),
     "tdvp1_sweep": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, P(fh_params)]),
     "tdvp_sweep_auto": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, P(fh_params), P(c_int)]),
@@ -330,6 +331,11 @@ class Context:
         self.check(lib.heff_expm_adaptive(self.h, c_void_p(theta.data_ptr()), c_void_p(out.data_ptr()), tau,
                                           krylov_dim, adapt_tol, C.byref(k)), "heff_expm_adaptive")
         return k.value
+
+    def fh_factorization_stats(self):
+        a = (C.c_int64 * 5)()
+        self.check(lib.fh_factorization_stats(self.h, a), "fh_factorization_stats")
+        return dict(jacobi_kernel=a[0], gesvdp=a[1], gesvd=a[2], gesvdp_rejected=a[3], qr=a[4])
 
     def fh_krylov_stats(self):
         a, b = C.c_int64(0), C.c_int64(0)

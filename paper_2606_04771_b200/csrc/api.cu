@@ -809,6 +809,16 @@ int heff_expm_adaptive(fh_ctx* ctx, const void* theta_dev, void* out_dev, double
   return heff_expm_impl(ctx, theta_dev, out_dev, tau, krylov_dim, adapt_tol, k_used);
 }
 
+int fh_factorization_stats(const fh_ctx* ctx, int64_t counts[5]) {
+  if (!ctx || !counts) return FH_EINVAL;
+  counts[0] = ctx->svd_small;
+  counts[1] = ctx->svd_count[1];
+  counts[2] = ctx->svd_count[0];
+  counts[3] = ctx->svd_count[2];
+  counts[4] = ctx->qr_count;
+  return FH_OK;
+}
+
 int fh_krylov_stats(const fh_ctx* ctx, int64_t* n_exponentials, int64_t* n_vectors) {
   if (!ctx) return FH_EINVAL;
   if (n_exponentials) *n_exponentials = ctx->krylov_calls;

@@ -303,10 +303,12 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
     FH_CUDA(cudaMemcpyAsync(d_small, small.data(), need, cudaMemcpyHostToDevice, ctx->stream));
     small_svd_kernel<<<(int)small.size(), 32 * SMALL_SVD_WARPS, small_smem, ctx->stream>>>(d_small, buf, dS);
     ++ctx->launches;
+    ctx->svd_small += (int64_t)small.size();
     FH_CUDA(cudaGetLastError());
     FH_CUDA(cudaStreamSynchronize(ctx->stream));  // `small` (pageable host memory) must outlive the copy
   }
   if (idx.empty()) return;
+  if (qr) ctx->qr_count += (int64_t)idx.size();
   auto cost = [&](int i) {
     const double m = std::max(order[i]->nrow, order[i]->ncol), n = order[i]->k;
     return m * n * n;

@@ -492,6 +492,55 @@ def test_next1_auto_switch_two_site_to_one_site(H, ctx):
     ctx.mps_destroy(mps)
 
 
+# ------------------------------------------------------------------ larger sectors: vendor SVD / QR routes
+def test_quench_L24_large_sectors_invariants(H, ctx):
+    """The L = 8 cases above keep every sector matrix below 48 columns, i.e. on the library's own Jacobi
+    kernel.  This quench (L = 24, U = 4, dt = 0.05, eps_trunc = 1e-10) grows the bonds to several hundred
+    states so that the gesvdp route (and, in the one-site steps that follow, Householder QR on the worker
+    streams) carries the sweep; the oracle is too slow here, so the checks are what holds at any size:
+    norm and energy conservation (E(0) = 0 for the Neel state; truncation 1e-10 per bond), <n_i> = 1 on every
+    site (T_tot = 0), total S^z = 0, and the inversion x spin-flip symmetry of the Neel quench on an even
+    chain, S^z_i = -S^z_{L-1-i}, docc_i = docc_{L-1-i}."""
+    L, t_h, U, dt, m = 24, 1.0, 4.0, 0.05, 10
+    mpo = ctx.fh_mpo_build(L, t_h, U)
+    mps = ctx.mps_init_neel(mpo, L)
+    f0 = ctx.fh_factorization_stats()
+
+    def check(tag, etol):
+        g = ctx.measure_global(mpo, mps)
+        o = ctx.measure_local(mps, L)
+        assert abs(g["norm2"] - 1.0) < 1e-6, (tag, g)
+        assert abs(g["energy"]) < etol, (tag, g)
+        assert np.abs(o["n"] - 1.0).max() < 1e-9, tag
+        assert abs(o["sz"].sum()) < 1e-9, tag
+        assert np.abs(o["sz"] + o["sz"][::-1]).max() < 1e-6, tag
+        assert np.abs(o["docc"] - o["docc"][::-1]).max() < 1e-6, tag
+        return g, o
+
+    for step in range(36):
+        ctx.tdvp2_sweep(mpo, mps, dt, krylov_dim=m, chi_max_full=4096, eps_trunc=1e-10)
+        if step % 6 == 5:
+            check(("two-site", step), 1e-5)
+    st = ctx.tdvp2_last_stats()
+    g2, o2 = check("end of two-site phase", 1e-5)
+    f1 = ctx.fh_factorization_stats()
+    assert st["chi_full"] > 300 and st["dmax"] >= 24, st
+    assert f1["gesvdp"] - f0["gesvdp"] > 0, f1                       # the vendor route really ran
+    assert f1["jacobi_kernel"] - f0["jacobi_kernel"] > 0, f1
+    dims_before = [ctx.mps_get_bond(mps, k) for k in range(L + 1)]
+    for step in range(4):
+        ctx.tdvp1_sweep(mpo, mps, dt, krylov_dim=m)
+    g1, o1 = check("one-site phase", 1e-5)
+    f2 = ctx.fh_factorization_stats()
+    assert f2["qr"] - f1["qr"] > 0, f2
+    assert [ctx.mps_get_bond(mps, k) for k in range(L + 1)] == dims_before      # one-site steps keep the bonds
+    assert abs(g1["energy"] - g2["energy"]) < 1e-8 and abs(g1["norm2"] - g2["norm2"]) < 1e-9   # no truncation
+    assert 0.02 < o1["docc"].mean() < 0.25 and np.abs(o1["sz"]).max() < 0.5                # the state has moved
+    print("L=24 quench: chi_full %d, d_max %d, factorizations %s, E = %.2e, norm2 - 1 = %.2e"
+          % (st["chi_full"], st["dmax"], f2, g1["energy"], g1["norm2"] - 1.0))
+    ctx.mps_destroy(mps)
+
+
 # ------------------------------------------------------------------ edge cases and errors
 def test_edge_cases_and_error_codes(H, ctx):
     B = H.binding
