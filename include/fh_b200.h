@@ -134,8 +134,9 @@ int heff_expm_adaptive(fh_ctx* ctx, const void* theta_dev, void* out_dev, double
 /* cumulative since context creation, sector matrices factorised (H9 and the one-site splits) by route:
  * counts[0] own shared-memory Jacobi kernel (both dims <= 64), [1] cusolverDnXgesvdp, [2] cusolverDnZgesvd
  * (n < 48, or redo of [3]), [3] gesvdp results rejected because it reported a perturbed spectrum,
- * [4] Householder QR (geqrf + ungqr) of the one-site splits. */
-int fh_factorization_stats(const fh_ctx* ctx, int64_t counts[5]);
+ * [4] Householder QR by cusolverDnZgeqrf + Zungqr (one-site splits that do not fit shared memory), [5] Householder
+ * QR by the library's own shared-memory kernel. */
+int fh_factorization_stats(const fh_ctx* ctx, int64_t counts[6]);
 /* cumulative since context creation: exponentials evaluated and Krylov vectors (= H_eff applies) they used */
 int fh_krylov_stats(const fh_ctx* ctx, int64_t* n_exponentials, int64_t* n_vectors);
 

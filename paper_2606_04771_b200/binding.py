@@ -333,9 +333,9 @@ class Context:
         return k.value
 
     def fh_factorization_stats(self):
-        a = (C.c_int64 * 5)()
+        a = (C.c_int64 * 6)()
         self.check(lib.fh_factorization_stats(self.h, a), "fh_factorization_stats")
-        return dict(jacobi_kernel=a[0], gesvdp=a[1], gesvd=a[2], gesvdp_rejected=a[3], qr=a[4])
+        return dict(jacobi_kernel=a[0], gesvdp=a[1], gesvd=a[2], gesvdp_rejected=a[3], qr=a[4], qr_kernel=a[5])
 
     def fh_krylov_stats(self):
         a, b = C.c_int64(0), C.c_int64(0)

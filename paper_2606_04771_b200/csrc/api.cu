@@ -809,8 +809,9 @@ int heff_expm_adaptive(fh_ctx* ctx, const void* theta_dev, void* out_dev, double
   return heff_expm_impl(ctx, theta_dev, out_dev, tau, krylov_dim, adapt_tol, k_used);
 }
 
-int fh_factorization_stats(const fh_ctx* ctx, int64_t counts[5]) {
+int fh_factorization_stats(const fh_ctx* ctx, int64_t counts[6]) {
   if (!ctx || !counts) return FH_EINVAL;
+  counts[5] = ctx->qr_small;
   counts[0] = ctx->svd_small;
   counts[1] = ctx->svd_count[1];
   counts[2] = ctx->svd_count[0];

@@ -121,6 +121,7 @@ struct fh_ctx {
   cudaEvent_t svd_fork = nullptr;
   int device = 0;
   int64_t svd_count[3] = {0, 0, 0};  // gesvd, gesvdp, gesvdp fallbacks to gesvd
+  int64_t qr_small = 0;  // one-site splits done by small_qr_kernel
   int64_t svd_small = 0, qr_count = 0;  // sector matrices done by small_svd_kernel / by geqrf+ungqr
   int64_t krylov_calls = 0, krylov_vectors = 0;  // exponentials evaluated / Krylov vectors (= H_eff applies) used
   // last sweep statistics

@@ -185,6 +185,139 @@ __global__ void __launch_bounds__(32 * SMALL_SVD_WARPS) small_svd_kernel(const S
   }
 }
 
+// ------------------------------------------------------------------------------------------
+// Small one-site splits (the whole qm x qn sector matrix fits shared memory): Householder QR in one launch for
+// all of them, one 8-warp CTA per matrix.  Same conventions as cusolverDnZgeqrf + Zungqr (LAPACK zlarfg /
+// zung2r: H_j = I - tau_j v v^H with v_0 = 1, real diagonal of R): column-major A (m x n) at m_off is
+// replaced by Q (m x k, k = min(m, n)), R (k x n) goes straight to r_dst like extract_r_kernel writes it.
+struct SmallQr {
+  int64_t m_off;
+  cplx* r_dst;
+  int m, n, r_ld, r_transpose;
+};
+constexpr size_t SMALL_QR_SMEM = 180 * 1024;
+constexpr int SMALL_QR_WARPS = 8;
+constexpr int SMALL_QR_MAXK = 256;
+__global__ void __launch_bounds__(32 * SMALL_QR_WARPS) small_qr_kernel(const SmallQr* __restrict__ descs,
+                                                                       cplx* __restrict__ buf) {
+  extern __shared__ __align__(16) unsigned char smem_qr[];
+  __shared__ cplx tau_s[SMALL_QR_MAXK];
+  const SmallQr d = descs[blockIdx.x];
+  const int m = d.m, n = d.n, k = min(m, n);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, tid = threadIdx.x;
+  constexpr int NT = 32 * SMALL_QR_WARPS;
+  cplx* A = reinterpret_cast<cplx*>(smem_qr);  // m x n column-major
+  cplx* Ag = buf + d.m_off;
+  for (int i = tid; i < m * n; i += NT) A[i] = Ag[i];
+  __syncthreads();
+  // ---- factorisation: H_j^H ... H_0^H A = R
+  for (int j = 0; j < k; ++j) {
+    cplx* x = A + (size_t)j * m;
+    if (warp == 0) {  // zlarfg on x[j..m)
+      double xn2 = 0.0;
+      for (int i = j + 1 + lane; i < m; i += 32) xn2 += x[i].x * x[i].x + x[i].y * x[i].y;
+      xn2 = warp_sum_all(xn2);
+      const cplx alpha = x[j];
+      cplx tau = make_double2(0.0, 0.0);
+      if (xn2 > 0.0 || alpha.y != 0.0) {
+        const double nrm = sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xn2);
+        const double beta = alpha.x >= 0.0 ? -nrm : nrm;
+        tau = make_double2((beta - alpha.x) / beta, -alpha.y / beta);
+        // v[i] = x[i] / (alpha - beta)
+        const double dr = alpha.x - beta, di = alpha.y, dd = dr * dr + di * di;
+        const double ir = dr / dd, ii = -di / dd;
+        for (int i = j + 1 + lane; i < m; i += 32) {
+          const cplx v = x[i];
+          x[i] = make_double2(v.x * ir - v.y * ii, v.x * ii + v.y * ir);
+        }
+        __syncwarp();
+        if (lane == 0) x[j] = make_double2(beta, 0.0);
+      }
+      if (lane == 0) tau_s[j] = tau;
+    }
+    __syncthreads();
+    const cplx tau = tau_s[j];
+    if (tau.x != 0.0 || tau.y != 0.0) {
+      // apply H_j^H = I - conj(tau) v v^H to the trailing columns, one warp per column
+      for (int c = j + 1 + warp; c < n; c += SMALL_QR_WARPS) {
+        cplx* y = A + (size_t)c * m;
+        double wr = 0.0, wi = 0.0;  // w = v^H y, v_j = 1
+        for (int i = j + 1 + lane; i < m; i += 32) {
+          const cplx v = x[i], yy = y[i];
+          wr += v.x * yy.x + v.y * yy.y;
+          wi += v.x * yy.y - v.y * yy.x;
+        }
+        wr = warp_sum_all(wr);
+        wi = warp_sum_all(wi);
+        wr += y[j].x;
+        wi += y[j].y;
+        const double fr = tau.x * wr + tau.y * wi, fi = tau.x * wi - tau.y * wr;  // conj(tau) * w
+        for (int i = j + 1 + lane; i < m; i += 32) {
+          const cplx v = x[i];
+          y[i].x -= fr * v.x - fi * v.y;
+          y[i].y -= fr * v.y + fi * v.x;
+        }
+        __syncwarp();
+        if (lane == 0) {
+          y[j].x -= fr;
+          y[j].y -= fi;
+        }
+      }
+    }
+    __syncthreads();
+  }
+  // ---- R out (upper trapezoid k x n; zeros below the diagonal)
+  for (int i = tid; i < k * n; i += NT) {
+    const int r = i % k, c = i / k;
+    const cplx v = r <= c ? A[(size_t)c * m + r] : make_double2(0.0, 0.0);
+    if (d.r_transpose) d.r_dst[(int64_t)c * d.r_ld + r] = v;
+    else d.r_dst[(int64_t)r * d.r_ld + c] = v;
+  }
+  __syncthreads();
+  // ---- Q = H_0 ... H_{k-1} (first k columns), in place (zung2r)
+  for (int j = k - 1; j >= 0; --j) {
+    cplx* x = A + (size_t)j * m;
+    const cplx tau = tau_s[j];
+    if (tau.x != 0.0 || tau.y != 0.0) {
+      for (int c = j + 1 + warp; c < k; c += SMALL_QR_WARPS) {  // apply H_j = I - tau v v^H from the left
+        cplx* y = A + (size_t)c * m;
+        double wr = 0.0, wi = 0.0;
+        for (int i = j + 1 + lane; i < m; i += 32) {
+          const cplx v = x[i], yy = y[i];
+          wr += v.x * yy.x + v.y * yy.y;
+          wi += v.x * yy.y - v.y * yy.x;
+        }
+        wr = warp_sum_all(wr);
+        wi = warp_sum_all(wi);
+        wr += y[j].x;
+        wi += y[j].y;
+        const double fr = tau.x * wr - tau.y * wi, fi = tau.x * wi + tau.y * wr;  // tau * w
+        for (int i = j + 1 + lane; i < m; i += 32) {
+          const cplx v = x[i];
+          y[i].x -= fr * v.x - fi * v.y;
+          y[i].y -= fr * v.y + fi * v.x;
+        }
+        __syncwarp();
+        if (lane == 0) {
+          y[j].x -= fr;
+          y[j].y -= fi;
+        }
+      }
+    }
+    __syncthreads();
+    // column j itself: -tau v below the diagonal, 1 - tau on it, zeros above
+    for (int i = tid; i < m; i += NT) {
+      cplx v;
+      if (i < j) v = make_double2(0.0, 0.0);
+      else if (i == j) v = make_double2(1.0 - tau.x, -tau.y);
+      else v = make_double2(-(tau.x * x[i].x - tau.y * x[i].y), -(tau.x * x[i].y + tau.y * x[i].x));
+      x[i] = v;
+    }
+    __syncthreads();
+  }
+  for (int i = tid; i < m * k; i += NT) Ag[i] = A[i];
+}
+
 void worker_reserve(fh_ctx::SvdWorker& w, size_t bytes) {
   if (bytes <= w.dwork_bytes) return;
   FH_CUDA(cudaStreamSynchronize(w.s));
@@ -280,15 +413,41 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
   const int nw = (int)ctx->svd_workers.size();
   std::vector<int> idx;
   std::vector<SmallSvd> small;
-  size_t small_smem = 0;
+  std::vector<SmallQr> small_qr;
+  size_t small_smem = 0, small_qr_smem = 0;
+  static const bool use_small_qr = [] {
+    const char* e = std::getenv("FH_SMALL_QR");  // "0" sends every one-site split to cuSOLVER
+    return !(e && e[0] == '0');
+  }();
   for (size_t i = 0; i < order.size(); ++i) {
     const int m = std::max(order[i]->nrow, order[i]->ncol), n = order[i]->k;
     if (!qr && m <= SMALL_SVD_MAX) {
       small.push_back(SmallSvd{order[i]->m_off, order[i]->u_off, order[i]->vt_off, order[i]->s_off, m, n});
       small_smem = std::max(small_smem, ((size_t)m * n + (size_t)n * n) * sizeof(cplx) + (size_t)n * sizeof(double));
+    } else if (qr && use_small_qr && (size_t)order[i]->qm * order[i]->qn * sizeof(cplx) <= SMALL_QR_SMEM &&
+               std::min(order[i]->qm, order[i]->qn) <= SMALL_QR_MAXK) {
+      small_qr.push_back(SmallQr{order[i]->m_off, order[i]->r_dst, order[i]->qm, order[i]->qn, order[i]->r_ld,
+                                 order[i]->r_transpose});
+      small_qr_smem = std::max(small_qr_smem, (size_t)order[i]->qm * order[i]->qn * sizeof(cplx));
     } else {
       idx.push_back((int)i);
     }
+  }
+  if (!small_qr.empty()) {
+    static bool qr_attr_done = false;
+    if (!qr_attr_done) {
+      FH_CUDA(cudaFuncSetAttribute(small_qr_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMALL_QR_SMEM));
+      qr_attr_done = true;
+    }
+    const size_t need = small_qr.size() * sizeof(SmallQr);
+    ctx->pool_small.reserve(need + 256, ctx->stream);
+    SmallQr* d_qr = (SmallQr*)ctx->pool_small.take(need);
+    FH_CUDA(cudaMemcpyAsync(d_qr, small_qr.data(), need, cudaMemcpyHostToDevice, ctx->stream));
+    small_qr_kernel<<<(int)small_qr.size(), 32 * SMALL_QR_WARPS, small_qr_smem, ctx->stream>>>(d_qr, buf);
+    ++ctx->launches;
+    ctx->qr_small += (int64_t)small_qr.size();
+    FH_CUDA(cudaGetLastError());
+    FH_CUDA(cudaStreamSynchronize(ctx->stream));  // `small_qr` (pageable host memory) must outlive the copy
   }
   if (!small.empty()) {
     static bool attr_done = false;
