@@ -132,7 +132,7 @@ int heff_expm(fh_ctx* ctx, const void* theta_dev, void* out_dev, double tau, int
 int heff_expm_adaptive(fh_ctx* ctx, const void* theta_dev, void* out_dev, double tau, int krylov_dim,
                        double adapt_tol, int* k_used);
 /* cumulative since context creation, sector matrices factorised (H9 and the one-site splits) by route:
- * counts[0] own shared-memory Jacobi kernel (both dims <= 64), [1] cusolverDnXgesvdp, [2] cusolverDnZgesvd
+ * counts[0] own shared-memory Jacobi kernel (matrix and V fit 216 KB: up to 82 x 82), [1] cusolverDnXgesvdp, [2] cusolverDnZgesvd
  * (n < 48, or redo of [3]), [3] gesvdp results rejected because it reported a perturbed spectrum,
  * [4] Householder QR by cusolverDnZgeqrf + Zungqr (one-site splits that do not fit shared memory), [5] Householder
  * QR by the library's own shared-memory kernel. */

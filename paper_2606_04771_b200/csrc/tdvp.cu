@@ -71,13 +71,16 @@ __global__ void conj_transpose_kernel(const cplx* __restrict__ src, cplx* __rest
 }
 
 // ------------------------------------------------------------------------------------------
-// Small sector matrices (both dimensions <= SMALL_SVD_MAX): one 8-warp CTA per matrix, one launch for all of
+// Small sector matrices (G and V fit SMALL_SVD_SMEM, i.e. up to 82 x 82): one 8-warp CTA per matrix, one launch for all of
 // them -- one-sided (Hestenes) Jacobi SVD in shared memory.  B (m x n, m >= n, column-major) -> U (m x n),
 // s (descending), V^H (n x n), the same conventions as cusolverDnZgesvd('S', 'S').  Column pairs (p, q) are
 // rotated until every |g_p^H g_q| <= 1e-15 |g_p| |g_q|; the singular values are the final column norms
 // (high relative accuracy, also for tiny ones).  At small chi a bond has tens of such matrices and a vendor
 // call per matrix (0.25 ms each, host-blocking) dominated the sweep.
-constexpr int SMALL_SVD_MAX = 64;
+constexpr size_t SMALL_SVD_SMEM = 216 * 1024;
+static inline size_t small_svd_bytes(int m, int n) {
+  return ((size_t)m * n + (size_t)n * n) * sizeof(cplx) + (size_t)n * sizeof(double);
+}
 struct SmallSvd {
   int64_t m_off, u_off, vt_off, s_off;
   int m, n;
@@ -421,7 +424,7 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
   }();
   for (size_t i = 0; i < order.size(); ++i) {
     const int m = std::max(order[i]->nrow, order[i]->ncol), n = order[i]->k;
-    if (!qr && m <= SMALL_SVD_MAX) {
+    if (!qr && small_svd_bytes(m, n) <= SMALL_SVD_SMEM) {
       small.push_back(SmallSvd{order[i]->m_off, order[i]->u_off, order[i]->vt_off, order[i]->s_off, m, n});
       small_smem = std::max(small_smem, ((size_t)m * n + (size_t)n * n) * sizeof(cplx) + (size_t)n * sizeof(double));
     } else if (qr && use_small_qr && (size_t)order[i]->qm * order[i]->qn * sizeof(cplx) <= SMALL_QR_SMEM &&
@@ -453,7 +456,7 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
     static bool attr_done = false;
     if (!attr_done) {
       FH_CUDA(cudaFuncSetAttribute(small_svd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                   (int)((2 * SMALL_SVD_MAX * SMALL_SVD_MAX) * sizeof(cplx) + SMALL_SVD_MAX * sizeof(double))));
+                                   (int)SMALL_SVD_SMEM));
       attr_done = true;
     }
     const size_t need = small.size() * sizeof(SmallSvd);
