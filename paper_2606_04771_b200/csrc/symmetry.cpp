@@ -170,6 +170,7 @@ static void emit_units(Stage& st) {
     int64_t work;
   };
   std::vector<UW> v;
+  v.reserve(st.outs.size() * 2);
   st.dmma_padded = 0;
   // The per-unit cap only exists to create enough units for 148 SMs x 8 resident warps; when the
   // stage is large (chi >~ 8000) full 16-sub-tile units are plentiful and the cap is lifted
@@ -215,11 +216,14 @@ static void emit_units(Stage& st) {
       m8 += h;
     }
   }
-  // heaviest first: the hardware CTA scheduler (one unit per one-warp CTA) then balances greedily
-  std::stable_sort(v.begin(), v.end(), [](const UW& a, const UW& b) { return a.work > b.work; });
+  // heaviest first: the hardware CTA scheduler (one unit per one-warp CTA) then balances greedily.
+  // (work, emission index) pairs are sorted, not the 96-byte descriptors; equal work keeps emission order.
+  std::vector<std::pair<int64_t, int>> ord(v.size());
+  for (size_t i = 0; i < v.size(); ++i) ord[i] = {-v[i].work, (int)i};
+  std::sort(ord.begin(), ord.end());
   st.units.clear();
   st.units.reserve(v.size());
-  for (auto& x : v) st.units.push_back(x.u);
+  for (auto& o : ord) st.units.push_back(v[o.second].u);
 }
 
 void finalize_stage(Stage& st, const BlockTensor& out, const BlockTensor& lhs, const BlockTensor& rhs) {
