@@ -11,7 +11,8 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libfh_b200.so")
+# FH_B200_LIB selects another build of the same library (unit_timeline.py uses the -DFH_UNIT_TRACE one)
+LIB_PATH = os.environ.get("FH_B200_LIB") or os.path.join(_HERE, "libfh_b200.so")
 if not os.path.exists(LIB_PATH):
     raise ImportError("libfh_b200.so is not built: run `python -m paper_2606_04771_b200.build` "
                       "(or __graft_entry__.build()); there is no CPU fallback")

@@ -19,18 +19,26 @@ def needs_build():
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force=False, verbose=False):
-    if not force and not needs_build():
+TRACE_LIB = os.path.join(HERE, "libfh_b200_trace.so")
+
+
+def build(force=False, verbose=False, trace=False):
+    """trace=True builds libfh_b200_trace.so instead: the same library with -DFH_UNIT_TRACE (every GEMM unit
+    stamps its begin/end time, SM and warp slot; used by unit_timeline.py, never by tests or bench)."""
+    lib = TRACE_LIB if trace else LIB
+    if not trace and not force and not needs_build():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     objs = []
     os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
     procs = []
     for src in SOURCES:
-        obj = os.path.join(HERE, "build", src + ".o")
+        obj = os.path.join(HERE, "build", src + (".trace.o" if trace else ".o"))
         cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
                "-Xcompiler", "-fPIC", "-x", "cu", "-I", os.path.join(ROOT, "include"), "-I", CSRC,
                "-c", os.path.join(CSRC, src), "-o", obj]
+        if trace:
+            cmd.insert(1, "-DFH_UNIT_TRACE")
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         procs.append((src, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
@@ -41,13 +49,13 @@ def build(force=False, verbose=False):
             raise RuntimeError("nvcc failed on %s:\n%s" % (src, out))
         if verbose and out:
             print(out)
-    cmd = [nvcc, "-shared", "-o", LIB] + objs + ["-L/usr/local/cuda/lib64", "-lcusolver", "-lcublas",
+    cmd = [nvcc, "-shared", "-o", lib] + objs + ["-L/usr/local/cuda/lib64", "-lcusolver", "-lcublas",
                                                   "-Xlinker", "-rpath=/usr/local/cuda/lib64"]
     r = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     if r.returncode != 0:
         raise RuntimeError("link failed:\n" + r.stdout)
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, trace="--trace" in sys.argv))
