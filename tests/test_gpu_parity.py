@@ -492,6 +492,26 @@ def test_next1_auto_switch_two_site_to_one_site(H, ctx):
     ctx.mps_destroy(mps)
 
 
+@pytest.mark.parametrize("L", [2, 4, 6])
+def test_tiny_chains_two_site_one_site_auto(H, ctx, L):
+    """Degenerate sizes: the shortest chains (1 x 1 sectors, bonds that reach their exact dimension after one or
+    two steps, QR of matrices with fewer rows than columns).  tdvp_sweep_auto against the oracle's step_auto:
+    same 2/1 sequence, observables to 1e-12, norm and energy conserved."""
+    mpo = ctx.fh_mpo_build(L, 1.0, 4.0)
+    mps = ctx.mps_init_neel(mpo, L)
+    ref = stv.SymmTDVP(L, 1.0, 4.0, krylov_dim=8, chi_max_full=64, eps_trunc=-1.0)
+    worst = 0.0
+    for step in range(6):
+        assert ref.step_auto(0.05) == ctx.tdvp_sweep_auto(mpo, mps, 0.05, krylov_dim=8, chi_max_full=64, eps_trunc=-1.0)
+        a, b = ref.measure_local(), ctx.measure_local(mps, L)
+        for key in ("n", "sz", "docc"):
+            worst = max(worst, np.abs(a[key] - b[key]).max())
+    g = ctx.measure_global(mpo, mps)
+    assert worst < 1e-12 and abs(g["norm2"] - 1.0) < 1e-11 and abs(g["energy"]) < 1e-11, (worst, g)
+    assert getattr(ref, "saturated", False)
+    ctx.mps_destroy(mps)
+
+
 # ------------------------------------------------------------------ larger sectors: vendor SVD / QR routes
 def test_quench_L24_large_sectors_invariants(H, ctx):
     """The L = 8 cases above keep every sector matrix below 48 columns, i.e. on the library's own Jacobi
