@@ -71,7 +71,7 @@ __global__ void conj_transpose_kernel(const cplx* __restrict__ src, cplx* __rest
 }
 
 // ------------------------------------------------------------------------------------------
-// Small sector matrices (G and V fit SMALL_SVD_SMEM, i.e. up to 82 x 82): one 8-warp CTA per matrix, one launch for all of
+// Small sector matrices (G and V fit SMALL_SVD_SMEM, i.e. up to 82 x 82): one CTA of 8 to 32 warps per matrix, one launch for all of
 // them -- one-sided (Hestenes) Jacobi SVD in shared memory.  B (m x n, m >= n, column-major) -> U (m x n),
 // s (descending), V^H (n x n), the same conventions as cusolverDnZgesvd('S', 'S').  Column pairs (p, q) are
 // rotated until every |g_p^H g_q| <= 1e-15 |g_p| |g_q|; the singular values are the final column norms
@@ -90,15 +90,15 @@ __device__ __forceinline__ double warp_sum_all(double v) {
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
   return v;
 }
-constexpr int SMALL_SVD_WARPS = 8;
-__global__ void __launch_bounds__(32 * SMALL_SVD_WARPS) small_svd_kernel(const SmallSvd* __restrict__ descs,
+constexpr int SMALL_SVD_MAX_WARPS = 32;  // the launch picks 8, 16 or 32 warps by the largest matrix of the batch
+__global__ void __launch_bounds__(32 * SMALL_SVD_MAX_WARPS) small_svd_kernel(const SmallSvd* __restrict__ descs,
                                                                          cplx* __restrict__ buf,
                                                                          double* __restrict__ dS) {
   extern __shared__ __align__(16) unsigned char smem_svd[];
   __shared__ int rotated_any;
   const SmallSvd d = descs[blockIdx.x];
   const int m = d.m, n = d.n, lane = threadIdx.x & 31, warp = threadIdx.x >> 5, tid = threadIdx.x;
-  constexpr int NT = 32 * SMALL_SVD_WARPS;
+  const int NT = blockDim.x, SMALL_SVD_WARPS = blockDim.x >> 5;
   cplx* G = reinterpret_cast<cplx*>(smem_svd);  // m x n column-major
   cplx* V = G + (size_t)m * n;                  // n x n column-major
   double* sig = reinterpret_cast<double*>(V + (size_t)n * n);
@@ -463,7 +463,11 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
     ctx->pool_small.reserve(need + 256, ctx->stream);
     SmallSvd* d_small = (SmallSvd*)ctx->pool_small.take(need);
     FH_CUDA(cudaMemcpyAsync(d_small, small.data(), need, cudaMemcpyHostToDevice, ctx->stream));
-    small_svd_kernel<<<(int)small.size(), 32 * SMALL_SVD_WARPS, small_smem, ctx->stream>>>(d_small, buf, dS);
+    // one warp per column pair of a tournament round: n / 2 pairs want up to 32 warps for the largest matrices
+    int nmax = 0;
+    for (const SmallSvd& d : small) nmax = std::max(nmax, d.n);
+    const int warps = nmax <= 16 ? 8 : (nmax <= 32 ? 16 : SMALL_SVD_MAX_WARPS);
+    small_svd_kernel<<<(int)small.size(), 32 * warps, small_smem, ctx->stream>>>(d_small, buf, dS);
     ++ctx->launches;
     ctx->svd_small += (int64_t)small.size();
     FH_CUDA(cudaGetLastError());
