@@ -190,7 +190,7 @@ __global__ void __launch_bounds__(32 * SMALL_SVD_MAX_WARPS) small_svd_kernel(con
 
 // ------------------------------------------------------------------------------------------
 // Small one-site splits (the whole qm x qn sector matrix fits shared memory): Householder QR in one launch for
-// all of them, one 8-warp CTA per matrix.  Same conventions as cusolverDnZgeqrf + Zungqr (LAPACK zlarfg /
+// all of them, one CTA of 8 to 32 warps per matrix.  Same conventions as cusolverDnZgeqrf + Zungqr (LAPACK zlarfg /
 // zung2r: H_j = I - tau_j v v^H with v_0 = 1, real diagonal of R): column-major A (m x n) at m_off is
 // replaced by Q (m x k, k = min(m, n)), R (k x n) goes straight to r_dst like extract_r_kernel writes it.
 struct SmallQr {
@@ -199,16 +199,16 @@ struct SmallQr {
   int m, n, r_ld, r_transpose;
 };
 constexpr size_t SMALL_QR_SMEM = 180 * 1024;
-constexpr int SMALL_QR_WARPS = 8;
+constexpr int SMALL_QR_MAX_WARPS = 32;  // the launch picks 8, 16 or 32 warps by the widest matrix of the batch
 constexpr int SMALL_QR_MAXK = 256;
-__global__ void __launch_bounds__(32 * SMALL_QR_WARPS) small_qr_kernel(const SmallQr* __restrict__ descs,
+__global__ void __launch_bounds__(32 * SMALL_QR_MAX_WARPS) small_qr_kernel(const SmallQr* __restrict__ descs,
                                                                        cplx* __restrict__ buf) {
   extern __shared__ __align__(16) unsigned char smem_qr[];
   __shared__ cplx tau_s[SMALL_QR_MAXK];
   const SmallQr d = descs[blockIdx.x];
   const int m = d.m, n = d.n, k = min(m, n);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, tid = threadIdx.x;
-  constexpr int NT = 32 * SMALL_QR_WARPS;
+  const int NT = blockDim.x, SMALL_QR_WARPS = blockDim.x >> 5;
   cplx* A = reinterpret_cast<cplx*>(smem_qr);  // m x n column-major
   cplx* Ag = buf + d.m_off;
   for (int i = tid; i < m * n; i += NT) A[i] = Ag[i];
@@ -446,7 +446,10 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
     ctx->pool_small.reserve(need + 256, ctx->stream);
     SmallQr* d_qr = (SmallQr*)ctx->pool_small.take(need);
     FH_CUDA(cudaMemcpyAsync(d_qr, small_qr.data(), need, cudaMemcpyHostToDevice, ctx->stream));
-    small_qr_kernel<<<(int)small_qr.size(), 32 * SMALL_QR_WARPS, small_qr_smem, ctx->stream>>>(d_qr, buf);
+    int qn_max = 0;  // one warp per trailing column of a Householder step
+    for (const SmallQr& d : small_qr) qn_max = std::max(qn_max, d.n);
+    const int qr_warps = qn_max <= 16 ? 8 : (qn_max <= 32 ? 16 : SMALL_QR_MAX_WARPS);
+    small_qr_kernel<<<(int)small_qr.size(), 32 * qr_warps, small_qr_smem, ctx->stream>>>(d_qr, buf);
     ++ctx->launches;
     ctx->qr_small += (int64_t)small_qr.size();
     FH_CUDA(cudaGetLastError());
