@@ -204,10 +204,12 @@ int fh_cublas_gemm_seconds(fh_ctx* ctx, int n, int is_complex, int reps, double*
 int fh_dmma_peak_tflops(fh_ctx* ctx, int reps, double* tflops);
 
 /* HBM-bound kernels of the path timed in isolation on n_elems complex128
- * elements taken from the arena (FH_ENOMEM if (m + 3) * n_elems do not fit): gbs[0] weighted dot,
- * gbs[1] axpy, gbs[2] scale, gbs[3] m-vector linear combination, gbs[4] pack (scaled block copy,
- * 256 x 256 blocks), gbs[5] pack with transposition.  GB/s = algorithmic bytes (32 n, 48 n, 32 n,
- * 16 (m+1) n, 32 n, 32 n) / CUDA-event time averaged over reps.  Measurement helper, not on the path. */
+ * elements taken from the arena (FH_ENOMEM if (m + 3) * n_elems do not fit): gbs[0] weighted dot (one launch,
+ * last CTA sums the partials), gbs[1] axpy, gbs[2] scale, gbs[3] m-vector linear combination, gbs[4] pack
+ * (scaled block copy, 256 x 256 blocks), gbs[5] pack with transposition, gbs[6] the Lanczos three-term update
+ * w -= alpha v_j + beta v_{j-1} fused with <w,w>.  GB/s = algorithmic bytes (32 n, 48 n, 32 n, 16 (m+1) n,
+ * 32 n, 32 n, 64 n) / CUDA-event time averaged over reps; gbs has 7 entries.  Measurement helper, not on
+ * the path. */
 int fh_vec_kernels_gbs(fh_ctx* ctx, int64_t n_elems, int m, int reps, double* gbs);
 
 /* ---- host-only entry points (no CUDA call inside): the symmetry layer on its own -----------

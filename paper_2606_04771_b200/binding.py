@@ -266,9 +266,10 @@ class Context:
         return t.value
 
     def fh_vec_kernels_gbs(self, n_elems, m=10, reps=10):
-        g = (c_dbl * 6)()
+        g = (c_dbl * 7)()
         self.check(lib.fh_vec_kernels_gbs(self.h, int(n_elems), int(m), int(reps), g), "fh_vec_kernels_gbs")
-        return dict(zip(("wdot", "axpy", "scale", "lincomb", "pack", "pack_transposed"), [float(v) for v in g]))
+        return dict(zip(("wdot", "axpy", "scale", "lincomb", "pack", "pack_transposed", "lanczos_update"),
+                        [float(v) for v in g]))
 
     def mps_drop_site(self, mps, site):
         self.check(lib.mps_drop_site(self.h, mps, site), "mps_drop_site")

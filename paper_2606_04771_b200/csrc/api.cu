@@ -158,6 +158,8 @@ void fh::plan_heff(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, 
   P.d_partial = (double*)P.pool.take(std::max<size_t>(1, P.chunks.size()) * 2 * sizeof(double));
   P.d_result = (double*)P.pool.take(2 * sizeof(double));
   P.d_scal = (double*)P.pool.take(256 * sizeof(double));
+  P.d_counter = (unsigned*)P.pool.take(sizeof(unsigned));
+  FH_CUDA(cudaMemsetAsync(P.d_counter, 0, sizeof(unsigned), ctx->stream));
   P.valid = true;
 }
 
@@ -264,7 +266,7 @@ int fh::expm_lanczos(fh_ctx* ctx, cplx* theta, double tau, int m, double tol, cp
     FH_CUDA(cudaStreamSynchronize(s));
   };
   ctx->timer_begin(T_VEC);
-  launch_wdot(P.d_chunks, nch, theta, theta, P.d_partial, d_sc, s, &ctx->launches);
+  launch_wdot_fused(P.d_chunks, nch, theta, theta, P.d_partial, d_sc, P.d_counter, s, &ctx->launches);
   launch_scale_rsqrt_dev(n, d_sc, 0.0, theta, V, nullptr, s, &ctx->launches);
   ctx->timer_end();
   std::vector<double> alpha, beta;
@@ -276,13 +278,11 @@ int fh::expm_lanczos(fh_ctx* ctx, cplx* theta, double tau, int m, double tol, cp
     apply_heff(ctx, vj, w);
     ctx->timer_end();
     ctx->timer_begin(T_VEC);
-    launch_wdot(P.d_chunks, nch, vj, w, P.d_partial, d_sc + 2 + 4 * j, s, &ctx->launches);
-    launch_axpy_neg_dev(n, d_sc + 2 + 4 * j, vj, w, s, &ctx->launches);
-    if (j > 0) launch_axpy_neg_dev(n, d_beta + (j - 1), V + (int64_t)(j - 1) * n, w, s, &ctx->launches);
-    if (j < m - 1) {
-      launch_wdot(P.d_chunks, nch, w, w, P.d_partial, d_sc + 4 + 4 * j, s, &ctx->launches);
-      launch_scale_rsqrt_dev(n, d_sc + 4 + 4 * j, tol, w, w, d_beta + j, s, &ctx->launches);
-    }
+    launch_wdot_fused(P.d_chunks, nch, vj, w, P.d_partial, d_sc + 2 + 4 * j, P.d_counter, s, &ctx->launches);
+    launch_lanczos_update(P.d_chunks, nch, d_sc + 2 + 4 * j, j > 0 ? d_beta + (j - 1) : nullptr, vj,
+                          j > 0 ? V + (int64_t)(j - 1) * n : nullptr, w, P.d_partial, d_sc + 4 + 4 * j, P.d_counter, s,
+                          &ctx->launches);
+    if (j < m - 1) launch_scale_rsqrt_dev(n, d_sc + 4 + 4 * j, tol, w, w, d_beta + j, s, &ctx->launches);
     ctx->timer_end();
     if (adapt_tol > 0.0 && j < m - 1) {
       fetch_scalars();
@@ -1013,17 +1013,24 @@ int fh_vec_kernels_gbs(fh_ctx* ctx, int64_t n, int m, int reps, double* gbs) {
       CopyBlk* d_cb = upload(ctx->pool_aux, cb, s);
       CopyBlk* d_cbt = upload(ctx->pool_aux, cbt, s);
       double* d_part = (double*)ctx->pool_aux.take(ch.size() * 2 * sizeof(double));
-      double* d_res = (double*)ctx->pool_aux.take(2 * sizeof(double));
+      double* d_res = (double*)ctx->pool_aux.take(6 * sizeof(double));
+      FH_CUDA(cudaMemsetAsync(d_res, 0, 6 * sizeof(double), s));
+      unsigned* d_cnt = (unsigned*)ctx->pool_aux.take(sizeof(unsigned));
+      FH_CUDA(cudaMemsetAsync(d_cnt, 0, sizeof(unsigned), s));
       FH_CUDA(cudaEventCreate(&e0));
       FH_CUDA(cudaEventCreate(&e1));
       std::vector<cplx> coef(m, make_double2(0.5, 0.25));
       const double nb = (double)cb.size() * B * B;
-      const double bytes[6] = {32.0 * n, 48.0 * n, 32.0 * n, 16.0 * (m + 1) * n, 32.0 * nb, 32.0 * nb};
-      for (int k = 0; k < 6; ++k) {
+      const double bytes[7] = {32.0 * n, 48.0 * n, 32.0 * n, 16.0 * (m + 1) * n, 32.0 * nb, 32.0 * nb, 64.0 * n};
+      for (int k = 0; k < 7; ++k) {
         for (int r = -2; r < reps; ++r) {
           if (r == 0) FH_CUDA(cudaEventRecord(e0, s));
           switch (k) {
-            case 0: launch_wdot(d_ch, (int)ch.size(), x, y, d_part, d_res, s, &ctx->launches); break;
+            case 0: launch_wdot_fused(d_ch, (int)ch.size(), x, y, d_part, d_res, d_cnt, s, &ctx->launches); break;
+            case 6:  // coefficients (d_res[2], d_res[3]) stay zero: the operands do not grow over the repetitions
+              launch_lanczos_update(d_ch, (int)ch.size(), d_res + 2, d_res + 3, x, y, z, d_part, d_res + 4, d_cnt, s,
+                                    &ctx->launches);
+              break;
             case 1: launch_axpy(n, make_double2(0.5, 0.1), x, y, s, &ctx->launches); break;
             case 2: launch_scale(n, make_double2(0.5, 0.1), x, z, s, &ctx->launches); break;
             case 3: launch_lincomb(n, m, coef.data(), V, n, z, s, &ctx->launches); break;

@@ -62,6 +62,7 @@ struct Plan {
   double* d_partial = nullptr;
   double* d_result = nullptr;
   double* d_scal = nullptr;  // Lanczos scalars kept on the device (expm_lanczos)
+  unsigned* d_counter = nullptr;  // retirement counter of the one-launch reductions (zero between launches)
   DevPool pool;
 };
 

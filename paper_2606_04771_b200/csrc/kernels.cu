@@ -73,6 +73,120 @@ __global__ void __launch_bounds__(256) wdot_final_kernel(const double* __restric
   }
 }
 
+// The CTA that retires last (atomicInc on a counter that wraps back to zero) adds the partials in index order
+// with the tree of wdot_final_kernel: one launch instead of two, same bits whichever CTA happens to be last.
+__device__ __forceinline__ void finish_in_last_cta(const double* __restrict__ partial, int n, double* __restrict__ result,
+                                                   unsigned* __restrict__ counter) {
+  __shared__ bool is_last;
+  __shared__ double fre[8], fim[8];
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) is_last = atomicInc(counter, gridDim.x - 1) == gridDim.x - 1;
+  __syncthreads();
+  if (!is_last) return;
+  __threadfence();
+  double re = 0.0, im = 0.0;
+  for (int i = threadIdx.x; i < n; i += 256) {
+    re += __ldcg(partial + 2 * i);
+    im += __ldcg(partial + 2 * i + 1);
+  }
+  re = warp_sum(re);
+  im = warp_sum(im);
+  if ((threadIdx.x & 31) == 0) { fre[threadIdx.x >> 5] = re; fim[threadIdx.x >> 5] = im; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double r = 0.0, m = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { r += fre[i]; m += fim[i]; }
+    result[0] = r;
+    result[1] = m;
+  }
+}
+
+// <x, y> in one launch (partials + last-CTA sum)
+__global__ void __launch_bounds__(256) wdot_fused_kernel(const VecChunk* __restrict__ chunks, const cplx* __restrict__ x,
+                                                         const cplx* __restrict__ y, double* __restrict__ partial,
+                                                         double* __restrict__ result, unsigned* __restrict__ counter) {
+  const VecChunk ch = chunks[blockIdx.x];
+  const cplx* px = x + ch.start;
+  const cplx* py = y + ch.start;
+  double re = 0.0, im = 0.0;
+  for (int i = threadIdx.x; i < ch.len; i += 256) {
+    const cplx a = px[i], b = py[i];
+    re += a.x * b.x + a.y * b.y;
+    im += a.x * b.y - a.y * b.x;
+  }
+  __shared__ double sre[8], sim[8];
+  re = warp_sum(re);
+  im = warp_sum(im);
+  if ((threadIdx.x & 31) == 0) { sre[threadIdx.x >> 5] = re; sim[threadIdx.x >> 5] = im; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double r = 0.0, m = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { r += sre[i]; m += sim[i]; }
+    partial[2 * blockIdx.x] = (double)ch.w * r;
+    partial[2 * blockIdx.x + 1] = (double)ch.w * m;
+  }
+  finish_in_last_cta(partial, gridDim.x, result, counter);
+}
+
+// Lanczos three-term update and the norm of its result in one launch:
+//   w -= alpha[0] v_j (+ beta_prev[0] v_prev);   result = <w, w> (weighted, F-6)
+// The two subtractions keep the order (and rounding) of two axpy_neg_dev_kernel passes.
+__global__ void __launch_bounds__(256) lanczos_update_kernel(const VecChunk* __restrict__ chunks,
+                                                             const double* __restrict__ alpha,
+                                                             const double* __restrict__ beta_prev,
+                                                             const cplx* __restrict__ vj, const cplx* __restrict__ vprev,
+                                                             cplx* __restrict__ w, double* __restrict__ partial,
+                                                             double* __restrict__ result, unsigned* __restrict__ counter) {
+  const VecChunk ch = chunks[blockIdx.x];
+  const double a = -alpha[0];
+  const double b = beta_prev ? -beta_prev[0] : 0.0;
+  const cplx* pv = vj + ch.start;
+  const cplx* pp = vprev ? vprev + ch.start : nullptr;
+  cplx* pw = w + ch.start;
+  double re = 0.0;
+  for (int i = threadIdx.x; i < ch.len; i += 256) {
+    const cplx xv = pv[i];
+    cplx v = pw[i];
+    v.x += a * xv.x;
+    v.y += a * xv.y;
+    if (pp) {
+      const cplx yv = pp[i];
+      v.x += b * yv.x;
+      v.y += b * yv.y;
+    }
+    pw[i] = v;
+    re += v.x * v.x + v.y * v.y;
+  }
+  __shared__ double sre[8];
+  re = warp_sum(re);
+  if ((threadIdx.x & 31) == 0) sre[threadIdx.x >> 5] = re;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double r = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) r += sre[i];
+    partial[2 * blockIdx.x] = (double)ch.w * r;
+    partial[2 * blockIdx.x + 1] = 0.0;
+  }
+  finish_in_last_cta(partial, gridDim.x, result, counter);
+}
+
+void launch_wdot_fused(const VecChunk* d_chunks, int nchunks, const cplx* x, const cplx* y, double* d_partial,
+                       double* d_result, unsigned* d_counter, cudaStream_t s, int64_t* lc) {
+  wdot_fused_kernel<<<nchunks, 256, 0, s>>>(d_chunks, x, y, d_partial, d_result, d_counter);
+  ++*lc;
+}
+void launch_lanczos_update(const VecChunk* d_chunks, int nchunks, const double* d_alpha, const double* d_beta_prev,
+                           const cplx* vj, const cplx* vprev, cplx* w, double* d_partial, double* d_result,
+                           unsigned* d_counter, cudaStream_t s, int64_t* lc) {
+  lanczos_update_kernel<<<nchunks, 256, 0, s>>>(d_chunks, d_alpha, d_beta_prev, vj, vprev, w, d_partial, d_result,
+                                                d_counter);
+  ++*lc;
+}
+
 void launch_wdot(const VecChunk* d_chunks, int nchunks, const cplx* x, const cplx* y, double* d_partial,
                  double* d_result, cudaStream_t s, int64_t* lc) {
   wdot_partial_kernel<<<nchunks, 256, 0, s>>>(d_chunks, x, y, d_partial);

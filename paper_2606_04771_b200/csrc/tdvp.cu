@@ -848,6 +848,8 @@ static void plan_zero_site(fh_ctx* ctx, const BlockTensor& Le, const BlockTensor
   P.d_partial = (double*)P.pool.take(std::max<size_t>(1, P.chunks.size()) * 2 * sizeof(double));
   P.d_result = (double*)P.pool.take(2 * sizeof(double));
   P.d_scal = (double*)P.pool.take(256 * sizeof(double));
+  P.d_counter = (unsigned*)P.pool.take(sizeof(unsigned));
+  FH_CUDA(cudaMemsetAsync(P.d_counter, 0, sizeof(unsigned), ctx->stream));
   P.valid = true;
 }
 
