@@ -148,7 +148,6 @@ void launch_wdot(const VecChunk* d_chunks, int nchunks, const cplx* x, const cpl
 void launch_axpy(int64_t n, cplx a, const cplx* x, cplx* y, cudaStream_t s, int64_t* lc);
 void launch_scale(int64_t n, cplx a, const cplx* x, cplx* y, cudaStream_t s, int64_t* lc);  // y = a*x
 // device-scalar Lanczos helpers: y -= d_coef[0] x;  y = x / sqrt(d_norm2[0]) (0 below tol), d_beta[0] = sqrt(d_norm2[0])
-void launch_axpy_neg_dev(int64_t n, const double* d_coef, const cplx* x, cplx* y, cudaStream_t s, int64_t* lc);
 // one-launch forms for the Lanczos recurrence: d_counter is a zero-initialised unsigned that the kernels leave at zero
 void launch_wdot_fused(const VecChunk* d_chunks, int nchunks, const cplx* x, const cplx* y, double* d_partial,
                        double* d_result, unsigned* d_counter, cudaStream_t s, int64_t* lc);

@@ -133,7 +133,7 @@ __global__ void __launch_bounds__(256) wdot_fused_kernel(const VecChunk* __restr
 
 // Lanczos three-term update and the norm of its result in one launch:
 //   w -= alpha[0] v_j (+ beta_prev[0] v_prev);   result = <w, w> (weighted, F-6)
-// The two subtractions keep the order (and rounding) of two axpy_neg_dev_kernel passes.
+// The two subtractions keep the order (and rounding) of two separate axpy passes (alpha first, then beta).
 __global__ void __launch_bounds__(256) lanczos_update_kernel(const VecChunk* __restrict__ chunks,
                                                              const double* __restrict__ alpha,
                                                              const double* __restrict__ beta_prev,
@@ -222,19 +222,7 @@ __global__ void __launch_bounds__(256) scale_kernel(int64_t n, cplx a, const cpl
   for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < n; i += (int64_t)gridDim.x * 256)
     y[i] = cmul(a, x[i]);
 }
-// Device-scalar variants for the Lanczos recurrence (no host round trip inside the iteration):
-// y -= coef[0] * x with a real coefficient read from device memory
-__global__ void __launch_bounds__(256) axpy_neg_dev_kernel(int64_t n, const double* __restrict__ coef,
-                                                           const cplx* __restrict__ x, cplx* __restrict__ y) {
-  const double a = -coef[0];
-  for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < n; i += (int64_t)gridDim.x * 256) {
-    const cplx xv = x[i];
-    cplx v = y[i];
-    v.x += a * xv.x;
-    v.y += a * xv.y;
-    y[i] = v;
-  }
-}
+// Device-scalar variant for the Lanczos recurrence (no host round trip inside the iteration):
 // y = x / sqrt(norm2[0]); beta_out[0] = sqrt(norm2[0]).  Below tol the direction is dropped (y = 0):
 // the host sees beta < tol afterwards and truncates the Krylov space there (happy breakdown).
 __global__ void __launch_bounds__(256) scale_rsqrt_dev_kernel(int64_t n, const double* __restrict__ norm2, double tol,
@@ -281,11 +269,6 @@ void launch_axpy(int64_t n, cplx a, const cplx* x, cplx* y, cudaStream_t s, int6
 void launch_scale(int64_t n, cplx a, const cplx* x, cplx* y, cudaStream_t s, int64_t* lc) {
   if (n <= 0) return;
   scale_kernel<<<grid_for(n), 256, 0, s>>>(n, a, x, y);
-  ++*lc;
-}
-void launch_axpy_neg_dev(int64_t n, const double* d_coef, const cplx* x, cplx* y, cudaStream_t s, int64_t* lc) {
-  if (n <= 0) return;
-  axpy_neg_dev_kernel<<<grid_for(n), 256, 0, s>>>(n, d_coef, x, y);
   ++*lc;
 }
 void launch_scale_rsqrt_dev(int64_t n, const double* d_norm2, double tol, const cplx* x, cplx* y, double* d_beta,
