@@ -82,6 +82,14 @@ int mps_site_layout(const fh_mps* mps, int site, int* nblk, int64_t* nelem, int3
  * order.  data_is_device != 0: device pointer (copied D2D on the context stream). */
 int mps_set_site(fh_ctx* ctx, fh_mps* mps, int site, const void* data, int data_is_device);
 int mps_get_site(fh_ctx* ctx, const fh_mps* mps, int site, void* data, int data_is_device);
+/* Checkpoint / resume for long runs (the paper's take up to 16 h).  mps_save writes the bond tables
+ * and the site tensors of a state whose orthogonality centre is on site 0 (the state every sweep returns) to a
+ * binary file (host byte order; header "FHMPS01", L, the tdvp_sweep_auto flag, per bond n x (q, 2j, d), per site
+ * the element count and the complex128 blocks in layout order).  mps_load rebuilds the state in this context and
+ * recomputes R_1..R_L with the given MPO, so that tdvp2_sweep / tdvp1_sweep / measure_* continue from it.
+ * FH_EINVAL: file cannot be opened, is truncated, or does not match the MPO's chain length. */
+int mps_save(fh_ctx* ctx, const fh_mps* mps, const char* path);
+int mps_load(fh_ctx* ctx, const fh_mpo* mpo, const char* path, fh_mps** out);
 /* Release the arena storage of one site tensor (streamed environment construction at large chi,
  * BASELINE.json config 5: a site is uploaded, absorbed into an environment, then dropped). */
 int mps_drop_site(fh_ctx* ctx, fh_mps* mps, int site);

@@ -63,6 +63,8 @@ _SIGS = {
     "heff_expm_adaptive": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, c_int, c_dbl, P(c_int)]),
     "fh_krylov_stats": (c_int, [c_void_p, P(C.c_int64), P(C.c_int64)]),
     "fh_factorization_stats": (c_int, [c_void_p, P(C.c_int64)]),
+    "mps_save": (c_int, [c_void_p, c_void_p, C.c_char_p]),
+    "mps_load": (c_int, [c_void_p, c_void_p, C.c_char_p, P(c_void_p)]),
     "tdvp2_sweep": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, P(fh_params)]),
     "tdvp1_sweep": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, P(fh_params)]),
     "tdvp_sweep_auto": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, P(fh_params), P(c_int)]),
@@ -270,6 +272,14 @@ class Context:
         self.check(lib.fh_vec_kernels_gbs(self.h, int(n_elems), int(m), int(reps), g), "fh_vec_kernels_gbs")
         return dict(zip(("wdot", "axpy", "scale", "lincomb", "pack", "pack_transposed", "lanczos_update"),
                         [float(v) for v in g]))
+
+    def mps_save(self, mps, path):
+        self.check(lib.mps_save(self.h, mps, os.fsencode(path)), "mps_save")
+
+    def mps_load(self, mpo, path):
+        h = c_void_p()
+        self.check(lib.mps_load(self.h, mpo, os.fsencode(path), C.byref(h)), "mps_load")
+        return h
 
     def mps_drop_site(self, mps, site):
         self.check(lib.mps_drop_site(self.h, mps, site), "mps_drop_site")

@@ -6,6 +6,8 @@
 #include <cmath>
 #include <cstring>
 
+#include <cstdio>
+
 #include "context.hpp"
 
 using namespace fh;
@@ -549,6 +551,108 @@ int mps_init_neel(fh_ctx* ctx, const fh_mpo* mpo, int L, fh_mps** out) {
     for (int i = L - 1; i >= 1; --i) do_env_update_right(ctx, mpo, m, i);
     *out = m;
   })
+}
+
+// ---- checkpoint / resume: bond tables + site tensors of a state whose centre is on site 0
+namespace {
+struct FileCloser {
+  FILE* f;
+  ~FileCloser() { if (f) std::fclose(f); }
+};
+const char MPS_MAGIC[8] = {'F', 'H', 'M', 'P', 'S', '0', '1', 0};
+}  // namespace
+
+int mps_save(fh_ctx* ctx, const fh_mps* mps, const char* path) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && mps && path, FH_EINVAL, "mps_save: NULL argument");
+    for (int i = 0; i < mps->L; ++i) FH_REQUIRE(mps->A[i].base >= 0, FH_ESTATE, "mps_save: site tensor missing");
+    FileCloser fc{std::fopen(path, "wb")};
+    FH_REQUIRE(fc.f, FH_EINVAL, std::string("mps_save: cannot open ") + path);
+    auto put = [&](const void* p, size_t n) {
+      FH_REQUIRE(std::fwrite(p, 1, n, fc.f) == n, FH_EINVAL, "mps_save: short write");
+    };
+    const int32_t head[2] = {mps->L, mps->saturated ? 1 : 0};
+    put(MPS_MAGIC, 8);
+    put(head, sizeof(head));
+    for (int k = 0; k <= mps->L; ++k) {
+      const Bond& b = mps->bond[k];
+      const int32_t n = (int32_t)b.sec.size();
+      put(&n, 4);
+      for (int32_t i = 0; i < n; ++i) {
+        const int32_t rec[3] = {b.sec[i].q, b.sec[i].tj, b.d[i]};
+        put(rec, sizeof(rec));
+      }
+    }
+    std::vector<cplx> host;
+    for (int i = 0; i < mps->L; ++i) {
+      const BlockTensor& t = mps->A[i];
+      BlockTensor ref;
+      layout_site(mps->bond[i], mps->bond[i + 1], ref);
+      FH_REQUIRE(ref.nelem == t.nelem && ref.keys == t.keys, FH_ESTATE, "mps_save: site tensor not in the bond tables' layout");
+      host.resize((size_t)t.nelem);
+      FH_CUDA(cudaMemcpyAsync(host.data(), ctx->ptr(t.base), t.nelem * sizeof(cplx), cudaMemcpyDeviceToHost, ctx->stream));
+      FH_CUDA(cudaStreamSynchronize(ctx->stream));
+      const int64_t ne = t.nelem;
+      put(&ne, 8);
+      put(host.data(), (size_t)ne * sizeof(cplx));
+    }
+  })
+}
+
+int mps_load(fh_ctx* ctx, const fh_mpo* mpo, const char* path, fh_mps** out) {
+  fh_mps* m = nullptr;
+  const int rc = [&]() -> int {
+    FH_TRY(ctx, {
+      FH_REQUIRE(ctx && mpo && path && out, FH_EINVAL, "mps_load: NULL argument");
+      FileCloser fc{std::fopen(path, "rb")};
+      FH_REQUIRE(fc.f, FH_EINVAL, std::string("mps_load: cannot open ") + path);
+      auto get = [&](void* p, size_t n) {
+        FH_REQUIRE(std::fread(p, 1, n, fc.f) == n, FH_EINVAL, "mps_load: truncated file");
+      };
+      char magic[8];
+      int32_t head[2];
+      get(magic, 8);
+      FH_REQUIRE(std::memcmp(magic, MPS_MAGIC, 8) == 0, FH_EINVAL, "mps_load: not an fh_mps checkpoint");
+      get(head, sizeof(head));
+      FH_REQUIRE(head[0] == mpo->L, FH_EINVAL, "mps_load: chain length differs from the MPO's");
+      int rc2 = mps_create(ctx, head[0], &m);
+      if (rc2 != FH_OK) throw FhError(rc2, ctx->err);
+      m->saturated = head[1] != 0;
+      for (int k = 0; k <= m->L; ++k) {
+        int32_t n = 0;
+        get(&n, 4);
+        FH_REQUIRE(n >= 1 && n <= (1 << 20), FH_EINVAL, "mps_load: bad sector count");
+        Bond b;
+        for (int32_t i = 0; i < n; ++i) {
+          int32_t rec[3];
+          get(rec, sizeof(rec));
+          FH_REQUIRE(rec[1] >= 0 && rec[2] >= 1, FH_EINVAL, "mps_load: bad sector record");
+          if (i > 0) FH_REQUIRE(b.sec.back() < Sector({rec[0], rec[1]}), FH_EINVAL, "mps_load: sector labels not sorted");
+          b.sec.push_back(Sector{rec[0], rec[1]});
+          b.d.push_back(rec[2]);
+        }
+        m->bond[k] = b;
+      }
+      std::vector<cplx> host;
+      for (int i = 0; i < m->L; ++i) {
+        BlockTensor t;
+        layout_site(m->bond[i], m->bond[i + 1], t);
+        int64_t ne = 0;
+        get(&ne, 8);
+        FH_REQUIRE(ne == t.nelem, FH_EINVAL, "mps_load: site tensor size does not match the bond tables");
+        host.resize((size_t)ne);
+        get(host.data(), (size_t)ne * sizeof(cplx));
+        ctx->alloc_tensor(t);
+        m->A[i] = t;
+        FH_CUDA(cudaMemcpyAsync(ctx->ptr(t.base), host.data(), ne * sizeof(cplx), cudaMemcpyHostToDevice, ctx->stream));
+        FH_CUDA(cudaStreamSynchronize(ctx->stream));
+      }
+      for (int i = m->L - 1; i >= 1; --i) do_env_update_right(ctx, mpo, m, i);
+      *out = m;
+    })
+  }();
+  if (rc != FH_OK && m) mps_destroy(ctx, m);
+  return rc;
 }
 
 int mps_set_bond(fh_ctx* ctx, fh_mps* mps, int bond, int n, const int32_t* q, const int32_t* tj, const int32_t* d) {

@@ -512,6 +512,43 @@ def test_tiny_chains_two_site_one_site_auto(H, ctx, L):
     ctx.mps_destroy(mps)
 
 
+def test_checkpoint_resume(H, ctx, tmp_path):
+    """mps_save / mps_load: a run interrupted after three steps and resumed from the file continues exactly like
+    the uninterrupted one (the right environments are recomputed from the same tensors by the same kernels, so
+    the observables agree to rounding), the auto-switch flag travels with the state, bad files are refused."""
+    L, dt, m = 8, 0.05, 10
+    mpo = ctx.fh_mpo_build(L, 1.0, 4.0)
+    mps = ctx.mps_init_neel(mpo, L)
+    kw = dict(krylov_dim=m, chi_max_full=40, eps_trunc=-1.0)
+    for _ in range(4):
+        ctx.tdvp_sweep_auto(mpo, mps, dt, **kw)
+    path = str(tmp_path / "state.fhmps")
+    ctx.mps_save(mps, path)
+    seq_a = [ctx.tdvp_sweep_auto(mpo, mps, dt, **kw) for _ in range(3)]
+    a, ga = ctx.measure_local(mps, L), ctx.measure_global(mpo, mps)
+    mps2 = ctx.mps_load(mpo, path)
+    seq_b = [ctx.tdvp_sweep_auto(mpo, mps2, dt, **kw) for _ in range(3)]
+    b, gb = ctx.measure_local(mps2, L), ctx.measure_global(mpo, mps2)
+    assert seq_a == seq_b and seq_a[-1] == 1          # saturated flag restored: one-site steps after the reload
+    for key in ("n", "sz", "docc"):
+        assert np.abs(a[key] - b[key]).max() < 1e-13, key
+    assert abs(ga["norm2"] - gb["norm2"]) < 1e-13 and abs(ga["energy"] - gb["energy"]) < 1e-12
+    for k in range(L + 1):
+        assert ctx.mps_get_bond(mps, k) == ctx.mps_get_bond(mps2, k)
+    # refused: missing file, truncated file, wrong chain length
+    with pytest.raises(H.binding.FhError):
+        ctx.mps_load(mpo, str(tmp_path / "nope.fhmps"))
+    blob = open(path, "rb").read()
+    open(str(tmp_path / "cut.fhmps"), "wb").write(blob[:len(blob) // 2])
+    with pytest.raises(H.binding.FhError):
+        ctx.mps_load(mpo, str(tmp_path / "cut.fhmps"))
+    mpo6 = ctx.fh_mpo_build(6, 1.0, 4.0)
+    with pytest.raises(H.binding.FhError):
+        ctx.mps_load(mpo6, path)
+    ctx.mps_destroy(mps)
+    ctx.mps_destroy(mps2)
+
+
 # ------------------------------------------------------------------ larger sectors: vendor SVD / QR routes
 def test_quench_L24_large_sectors_invariants(H, ctx):
     """The L = 8 cases above keep every sector matrix below 48 columns, i.e. on the library's own Jacobi
