@@ -145,6 +145,16 @@ int heff_expm_adaptive(fh_ctx* ctx, const void* theta_dev, void* out_dev, double
  * [4] Householder QR by cusolverDnZgeqrf + Zungqr (one-site splits that do not fit shared memory), [5] Householder
  * QR by the library's own shared-memory kernel. */
 int fh_factorization_stats(const fh_ctx* ctx, int64_t counts[6]);
+/* Task-list cache of the one-site sweeps (H0).  One-site TDVP keeps every bond's sector table
+ * (no SVD, bond dimension fixed), so tdvp1_sweep / tdvp_sweep_auto keep the task lists they emit in
+ * host memory owned by the fh_mps and reuse an entry only when the labels and shapes of every tensor the emitter
+ * reads, and the MPO's t_h and U, are identical to those it was emitted for; a two-site sweep empties the cache.
+ * Results do not depend on it (same lists, same launches).  Stats: lookups that reused / re-emitted a list since
+ * the state was created, and the host bytes held now (any pointer may be NULL).  Limit: drops all entries and
+ * caps the host memory of new ones (default 4 GiB; 0 switches the cache off).  Host-only calls; FH_EINVAL on a
+ * NULL state or a negative limit. */
+int fh_plan_cache_stats(const fh_mps* mps, int64_t* hits, int64_t* misses, int64_t* host_bytes);
+int fh_plan_cache_limit(fh_mps* mps, int64_t max_host_bytes);
 /* cumulative since context creation: exponentials evaluated and Krylov vectors (= H_eff applies) they used */
 int fh_krylov_stats(const fh_ctx* ctx, int64_t* n_exponentials, int64_t* n_vectors);
 

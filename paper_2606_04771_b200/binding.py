@@ -63,6 +63,8 @@ _SIGS = {
     "heff_expm_adaptive": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, c_int, c_dbl, P(c_int)]),
     "fh_krylov_stats": (c_int, [c_void_p, P(C.c_int64), P(C.c_int64)]),
     "fh_factorization_stats": (c_int, [c_void_p, P(C.c_int64)]),
+    "fh_plan_cache_stats": (c_int, [c_void_p, P(C.c_int64), P(C.c_int64), P(C.c_int64)]),
+    "fh_plan_cache_limit": (c_int, [c_void_p, C.c_int64]),
     "mps_save": (c_int, [c_void_p, c_void_p, C.c_char_p]),
     "mps_load": (c_int, [c_void_p, c_void_p, C.c_char_p, P(c_void_p)]),
     "tdvp2_sweep": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, P(fh_params)]),
@@ -348,6 +350,14 @@ class Context:
         a = (C.c_int64 * 6)()
         self.check(lib.fh_factorization_stats(self.h, a), "fh_factorization_stats")
         return dict(jacobi_kernel=a[0], gesvdp=a[1], gesvd=a[2], gesvdp_rejected=a[3], qr=a[4], qr_kernel=a[5])
+
+    def fh_plan_cache_stats(self, mps):
+        a, b, c = C.c_int64(0), C.c_int64(0), C.c_int64(0)
+        self.check(lib.fh_plan_cache_stats(mps, C.byref(a), C.byref(b), C.byref(c)), "fh_plan_cache_stats")
+        return dict(hits=a.value, misses=b.value, host_bytes=c.value)
+
+    def fh_plan_cache_limit(self, mps, max_host_bytes):
+        self.check(lib.fh_plan_cache_limit(mps, int(max_host_bytes)), "fh_plan_cache_limit")
 
     def fh_krylov_stats(self):
         a, b = C.c_int64(0), C.c_int64(0)

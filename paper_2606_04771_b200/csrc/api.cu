@@ -120,6 +120,70 @@ void fh_ctx::timers_resolve() {
   spans.clear();
 }
 
+// ============================================================================ task-list cache (one-site sweeps)
+void fh::sig_add(std::vector<int>& sig, const BlockTensor& t) {
+  const size_t n = t.keys.size();
+  sig.push_back(t.nlab);
+  sig.push_back((int)n);
+  const size_t at = sig.size();
+  sig.resize(at + n * 14);
+  int* p = sig.data() + at;
+  for (size_t i = 0; i < n; ++i) {
+    std::memcpy(p, t.keys[i].data(), 12 * sizeof(int));
+    p[12] = t.rows[i];
+    p[13] = t.cols[i];
+    p += 14;
+  }
+}
+void fh::sig_add(std::vector<int>& sig, const Bond& b) {
+  sig.push_back((int)b.sec.size());
+  for (size_t i = 0; i < b.sec.size(); ++i) {
+    sig.push_back(b.sec[i].q);
+    sig.push_back(b.sec[i].tj);
+    sig.push_back(b.d[i]);
+  }
+}
+void fh::sig_add(std::vector<int>& sig, double x) {
+  int w[2];
+  std::memcpy(w, &x, sizeof(double));
+  sig.push_back(w[0]);
+  sig.push_back(w[1]);
+}
+const PlanCacheEntry* PlanCache::find(int kind, int site, const std::vector<int>& sig) {
+  auto it = map.find(kind * 65536 + site);
+  if (it != map.end() && it->second.sig == sig) {
+    ++hits;
+    return &it->second;
+  }
+  ++misses;
+  return nullptr;
+}
+PlanCacheEntry* PlanCache::store(int kind, int site, std::vector<int>&& sig) {
+  auto it = map.find(kind * 65536 + site);
+  if (it != map.end()) {
+    bytes -= std::min(bytes, it->second.bytes);
+    map.erase(it);
+  }
+  if (bytes >= max_bytes) return nullptr;
+  PlanCacheEntry& e = map[kind * 65536 + site];
+  e.sig = std::move(sig);
+  return &e;
+}
+static size_t stage_host_bytes(const Stage& st) {
+  return st.t_out.size() * (3 * sizeof(int) + sizeof(double)) + st.outs.size() * sizeof(GemmOut) +
+         st.segs.size() * sizeof(GemmSeg) + st.units.size() * sizeof(GemmUnit);
+}
+static size_t layout_host_bytes(const BlockTensor& t) { return t.keys.size() * (sizeof(Key) * 2 + 48); }
+void PlanCache::account(PlanCacheEntry* e) {
+  e->bytes = e->sig.size() * sizeof(int) + stage_host_bytes(e->st1) + stage_host_bytes(e->st2) +
+             layout_host_bytes(e->t0) + layout_host_bytes(e->t1) + e->chunks.size() * sizeof(VecChunk);
+  bytes += e->bytes;
+}
+void PlanCache::clear() {
+  map.clear();
+  bytes = 0;
+}
+
 // ============================================================================ plan + apply
 static int last_tj_pos(int nsite) { return nsite == 2 ? 7 : (nsite == 1 ? 4 : 1); }
 
@@ -134,24 +198,54 @@ void fh::plan_heff(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, 
   P.valid = false;
   P.nsite = nsite;
   P.site = site;
-  if (nsite == 2) {
-    layout_theta(mps->bond[site], mps->bond[site + 2], P.vec);
-    emit_heff2(Le, Re, P.vec, mpo->site[site & 1], mpo->site[(site + 1) & 1], P.Z, P.st1, P.st2);
+  const bool use_cache = nsite == 1 && mps->cache.enabled;
+  std::vector<int> sig;
+  const PlanCacheEntry* hit = nullptr;
+  if (use_cache) {
+    sig_add(sig, Le);
+    sig_add(sig, Re);
+    sig_add(sig, mps->bond[site]);
+    sig_add(sig, mps->bond[site + 1]);
+    sig_add(sig, mpo->t_h);
+    sig_add(sig, mpo->U);
+    hit = mps->cache.find(PC_HEFF1, site, sig);
+  }
+  if (hit) {
+    P.vec = hit->t0;
+    P.Z = hit->t1;
+    P.st1 = hit->st1;
+    P.st2 = hit->st2;
+    P.chunks = hit->chunks;
   } else {
-    layout_site(mps->bond[site], mps->bond[site + 1], P.vec);
-    emit_heff1(Le, Re, P.vec, mpo->site[site & 1], P.Z, P.st1, P.st2);
+    if (nsite == 2) {
+      layout_theta(mps->bond[site], mps->bond[site + 2], P.vec);
+      emit_heff2(Le, Re, P.vec, mpo->site[site & 1], mpo->site[(site + 1) & 1], P.Z, P.st1, P.st2);
+    } else {
+      layout_site(mps->bond[site], mps->bond[site + 1], P.vec);
+      emit_heff1(Le, Re, P.vec, mpo->site[site & 1], P.Z, P.st1, P.st2);
+    }
+    // weighted inner-product chunks (F-6)
+    P.chunks.clear();
+    const int tpos = last_tj_pos(nsite);
+    for (size_t i = 0; i < P.vec.keys.size(); ++i) {
+      const int64_t n = (int64_t)P.vec.rows[i] * P.vec.cols[i];
+      for (int64_t s = 0; s < n; s += 8192)
+        P.chunks.push_back(VecChunk{P.vec.off[i] + s, (int)std::min<int64_t>(8192, n - s), (float)(P.vec.keys[i][tpos] + 1)});
+    }
+    if (use_cache) {
+      if (PlanCacheEntry* e = mps->cache.store(PC_HEFF1, site, std::move(sig))) {
+        e->t0 = P.vec;
+        e->t1 = P.Z;
+        e->st1 = P.st1;
+        e->st2 = P.st2;
+        e->chunks = P.chunks;
+        mps->cache.account(e);
+      }
+    }
   }
   ctx->alloc_tensor(P.Z);
   P.Lptr = ctx->ptr(Le.base);
   P.Rptr = ctx->ptr(Re.base);
-  // weighted inner-product chunks (F-6)
-  P.chunks.clear();
-  const int tpos = last_tj_pos(nsite);
-  for (size_t i = 0; i < P.vec.keys.size(); ++i) {
-    const int64_t n = (int64_t)P.vec.rows[i] * P.vec.cols[i];
-    for (int64_t s = 0; s < n; s += 8192)
-      P.chunks.push_back(VecChunk{P.vec.off[i] + s, (int)std::min<int64_t>(8192, n - s), (float)(P.vec.keys[i][tpos] + 1)});
-  }
   const size_t need = stage_bytes(P.st1) + stage_bytes(P.st2) + P.chunks.size() * (sizeof(VecChunk) + 16) + 8192;
   P.pool.reserve(need, ctx->stream);
   upload_stage(P.pool, P.st1, ctx->stream);
@@ -347,6 +441,38 @@ static void run_two_stage(fh_ctx* ctx, Stage& st1, Stage& st2, BlockTensor& mid,
   ctx->free_tensor(mid);
 }
 
+static std::vector<int> env_sig(const BlockTensor& E, const BlockTensor& A, const fh_mpo* mpo) {
+  std::vector<int> sig;
+  sig_add(sig, E);
+  sig_add(sig, A);
+  sig_add(sig, mpo->t_h);
+  sig_add(sig, mpo->U);
+  return sig;
+}
+static bool env_from_cache(fh_mps* mps, int kind, int site, const BlockTensor& E, const BlockTensor& A,
+                           const fh_mpo* mpo, BlockTensor& mid, BlockTensor& out, Stage& st1, Stage& st2) {
+  if (!mps->cache.enabled) return false;
+  const PlanCacheEntry* e = mps->cache.find(kind, site, env_sig(E, A, mpo));
+  if (!e) return false;
+  mid = e->t0;
+  out = e->t1;
+  st1 = e->st1;
+  st2 = e->st2;
+  return true;
+}
+static void env_to_cache(fh_mps* mps, int kind, int site, const BlockTensor& E, const BlockTensor& A,
+                         const fh_mpo* mpo, const BlockTensor& mid, const BlockTensor& out, const Stage& st1,
+                         const Stage& st2) {
+  if (!mps->cache.enabled) return;
+  if (PlanCacheEntry* e = mps->cache.store(kind, site, env_sig(E, A, mpo))) {
+    e->t0 = mid;
+    e->t1 = out;
+    e->st1 = st1;
+    e->st2 = st2;
+    mps->cache.account(e);
+  }
+}
+
 void fh::do_env_update_left(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int site) {
   FH_REQUIRE(site >= 0 && site < mps->L, FH_EINVAL, "env_update_left: site out of range");
   BlockTensor& Le = mps->Lenv[site];
@@ -354,7 +480,10 @@ void fh::do_env_update_left(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int sit
   FH_REQUIRE(Le.base >= 0 && A.base >= 0, FH_ESTATE, "env_update_left: L_site or A_site missing");
   BlockTensor X, out;
   Stage st1, st2;
-  emit_env_left(Le, A, mpo->site[site & 1], X, out, st1, st2);
+  if (!env_from_cache(mps, PC_ENVL, site, Le, A, mpo, X, out, st1, st2)) {
+    emit_env_left(Le, A, mpo->site[site & 1], X, out, st1, st2);
+    env_to_cache(mps, PC_ENVL, site, Le, A, mpo, X, out, st1, st2);
+  }
   ctx->free_tensor(mps->Lenv[site + 1]);
   ctx->alloc_tensor(out);
   ctx->timer_begin(T_ENV);
@@ -371,7 +500,10 @@ void fh::do_env_update_right(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int si
   FH_REQUIRE(Re.base >= 0 && A.base >= 0, FH_ESTATE, "env_update_right: R_{site+1} or A_site missing");
   BlockTensor Y, out;
   Stage st1, st2;
-  emit_env_right(Re, A, mpo->site[site & 1], Y, out, st1, st2);
+  if (!env_from_cache(mps, PC_ENVR, site, Re, A, mpo, Y, out, st1, st2)) {
+    emit_env_right(Re, A, mpo->site[site & 1], Y, out, st1, st2);
+    env_to_cache(mps, PC_ENVR, site, Re, A, mpo, Y, out, st1, st2);
+  }
   ctx->free_tensor(mps->Renv[site]);
   ctx->alloc_tensor(out);
   ctx->timer_begin(T_ENV);
@@ -921,6 +1053,21 @@ int fh_factorization_stats(const fh_ctx* ctx, int64_t counts[6]) {
   counts[2] = ctx->svd_count[0];
   counts[3] = ctx->svd_count[2];
   counts[4] = ctx->qr_count;
+  return FH_OK;
+}
+
+int fh_plan_cache_stats(const fh_mps* mps, int64_t* hits, int64_t* misses, int64_t* host_bytes) {
+  if (!mps) return FH_EINVAL;
+  if (hits) *hits = mps->cache.hits;
+  if (misses) *misses = mps->cache.misses;
+  if (host_bytes) *host_bytes = (int64_t)mps->cache.bytes;
+  return FH_OK;
+}
+
+int fh_plan_cache_limit(fh_mps* mps, int64_t max_host_bytes) {
+  if (!mps || max_host_bytes < 0) return FH_EINVAL;
+  mps->cache.clear();
+  mps->cache.max_bytes = (size_t)max_host_bytes;
   return FH_OK;
 }
 

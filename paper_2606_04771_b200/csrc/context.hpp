@@ -68,6 +68,34 @@ struct Plan {
 
 enum { T_HEFF = 0, T_ENV = 1, T_SVD = 2, T_VEC = 3, T_PACK = 4, T_NCAT = 5 };
 
+// Task-list cache of the one-site sweeps (H0).  One-site TDVP leaves the sector tables of every bond as they
+// are (no SVD, no change of bond dimension), so the task lists of a sweep equal those of the sweep
+// before.  An entry holds what an emitter produced for (kind, site) together with a signature: the flattened
+// labels and block shapes of every input the emitter reads, and the MPO parameters.  A lookup compares the whole
+// signature, so a stale entry (a QR that lowered a rank, a two-site step in between) is re-emitted, never used.
+// Task lists address operands relative to their tensor base; arena offsets may change freely between sweeps.
+enum { PC_HEFF1 = 0, PC_ENVL = 1, PC_ENVR = 2, PC_HEFF0 = 3, PC_ABSORB_L = 4, PC_ABSORB_R = 5, PC_NKIND = 6 };
+struct PlanCacheEntry {
+  std::vector<int> sig;
+  BlockTensor t0, t1;  // layouts the emitter produced (vec and Z; X and out; new A), base = -1
+  Stage st1, st2;
+  std::vector<VecChunk> chunks;
+  size_t bytes = 0;
+};
+struct PlanCache {
+  bool enabled = false;  // set by the one-site sweep for its own duration
+  size_t bytes = 0, max_bytes = (size_t)4 << 30;  // host bytes held / cap (no new entries beyond it)
+  int64_t hits = 0, misses = 0;
+  std::unordered_map<int, PlanCacheEntry> map;  // kind * 65536 + site
+  const PlanCacheEntry* find(int kind, int site, const std::vector<int>& sig);
+  PlanCacheEntry* store(int kind, int site, std::vector<int>&& sig);  // nullptr when over the cap
+  void account(PlanCacheEntry* e);  // call once the entry is filled
+  void clear();
+};
+void sig_add(std::vector<int>& sig, const BlockTensor& t);
+void sig_add(std::vector<int>& sig, const Bond& b);
+void sig_add(std::vector<int>& sig, double x);
+
 }  // namespace fh
 
 struct fh_mpo {
@@ -82,6 +110,7 @@ struct fh_mps {
   std::vector<fh::BlockTensor> A, Lenv, Renv;       // L, L+1, L+1
   std::vector<std::vector<double>> sval;            // L+1: kept singular values of the last split
   bool saturated = false;                           // tdvp_sweep_auto: a two-site step grew no bond (A-16)
+  mutable fh::PlanCache cache;                      // task lists of the one-site sweeps (host memory only)
 };
 
 struct fh_ctx {

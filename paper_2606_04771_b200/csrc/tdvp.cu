@@ -822,7 +822,9 @@ static void local_update1(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int i, do
 
 // ============================================================================ one-site TDVP (NEXT-1)
 // Plan of the zero-site apply on the bond matrix C (layout Cl, keys {q, tj}) between Lenv and Renv.
-static void plan_zero_site(fh_ctx* ctx, const BlockTensor& Le, const BlockTensor& Re, const BlockTensor& Cl) {
+// `bond` = index of the bond C lives on (cache key of the one-site sweeps' task lists, context.hpp).
+static void plan_zero_site(fh_ctx* ctx, fh_mps* mps, int bond, const BlockTensor& Le, const BlockTensor& Re,
+                           const BlockTensor& Cl) {
   Plan& P = ctx->plan;
   ctx->free_tensor(P.Z);
   P.valid = false;
@@ -830,16 +832,40 @@ static void plan_zero_site(fh_ctx* ctx, const BlockTensor& Le, const BlockTensor
   P.site = -1;
   P.vec = Cl;
   P.vec.base = -1;
-  emit_heff0(Le, Re, P.vec, P.Z, P.st1, P.st2);
+  std::vector<int> sig;
+  const PlanCacheEntry* hit = nullptr;
+  if (mps->cache.enabled) {
+    sig_add(sig, Le);
+    sig_add(sig, Re);
+    sig_add(sig, Cl);
+    hit = mps->cache.find(PC_HEFF0, bond, sig);
+  }
+  if (hit) {
+    P.Z = hit->t1;
+    P.st1 = hit->st1;
+    P.st2 = hit->st2;
+    P.chunks = hit->chunks;
+  } else {
+    emit_heff0(Le, Re, P.vec, P.Z, P.st1, P.st2);
+    P.chunks.clear();
+    for (size_t i = 0; i < P.vec.keys.size(); ++i) {
+      const int64_t n = (int64_t)P.vec.rows[i] * P.vec.cols[i];
+      for (int64_t st = 0; st < n; st += 8192)
+        P.chunks.push_back(VecChunk{P.vec.off[i] + st, (int)std::min<int64_t>(8192, n - st), (float)(P.vec.keys[i][1] + 1)});
+    }
+    if (mps->cache.enabled) {
+      if (PlanCacheEntry* e = mps->cache.store(PC_HEFF0, bond, std::move(sig))) {
+        e->t1 = P.Z;
+        e->st1 = P.st1;
+        e->st2 = P.st2;
+        e->chunks = P.chunks;
+        mps->cache.account(e);
+      }
+    }
+  }
   ctx->alloc_tensor(P.Z);
   P.Lptr = ctx->ptr(Le.base);
   P.Rptr = ctx->ptr(Re.base);
-  P.chunks.clear();
-  for (size_t i = 0; i < P.vec.keys.size(); ++i) {
-    const int64_t n = (int64_t)P.vec.rows[i] * P.vec.cols[i];
-    for (int64_t st = 0; st < n; st += 8192)
-      P.chunks.push_back(VecChunk{P.vec.off[i] + st, (int)std::min<int64_t>(8192, n - st), (float)(P.vec.keys[i][1] + 1)});
-  }
   const size_t need = stage_bytes(P.st1) + stage_bytes(P.st2) + P.chunks.size() * (sizeof(VecChunk) + 16) + 8192;
   P.pool.reserve(need, ctx->stream);
   upload_stage(P.pool, P.st1, ctx->stream);
@@ -1008,9 +1034,31 @@ static void split_site(fh_ctx* ctx, fh_mps* mps, int i, int direction, BlockTens
 // A_j <- C A_j (left) or A_j C (right) with the new bond dims already in mps->bond
 static void absorb_bond(fh_ctx* ctx, fh_mps* mps, int j, const BlockTensor& C, bool left) {
   BlockTensor An;
-  layout_site(mps->bond[j], mps->bond[j + 1], An);
   Stage st;
-  emit_absorb(C, mps->A[j], An, left, st);
+  const int kind = left ? PC_ABSORB_L : PC_ABSORB_R;
+  std::vector<int> sig;
+  const PlanCacheEntry* hit = nullptr;
+  if (mps->cache.enabled) {
+    sig_add(sig, C);
+    sig_add(sig, mps->A[j]);
+    sig_add(sig, mps->bond[j]);
+    sig_add(sig, mps->bond[j + 1]);
+    hit = mps->cache.find(kind, j, sig);
+  }
+  if (hit) {
+    An = hit->t0;
+    st = hit->st1;
+  } else {
+    layout_site(mps->bond[j], mps->bond[j + 1], An);
+    emit_absorb(C, mps->A[j], An, left, st);
+    if (mps->cache.enabled) {
+      if (PlanCacheEntry* e = mps->cache.store(kind, j, std::move(sig))) {
+        e->t0 = An;
+        e->st1 = st;
+        mps->cache.account(e);
+      }
+    }
+  }
   ctx->alloc_tensor(An);
   ctx->pool_aux.reserve(stage_bytes(st) + 4096, ctx->stream);
   upload_stage(ctx->pool_aux, st, ctx->stream);
@@ -1023,9 +1071,9 @@ static void absorb_bond(fh_ctx* ctx, fh_mps* mps, int j, const BlockTensor& C, b
   mps->A[j] = An;
 }
 
-static void zero_site_update(fh_ctx* ctx, const BlockTensor& Le, const BlockTensor& Re, BlockTensor& C, double tau,
-                             const fh_params* prm) {
-  plan_zero_site(ctx, Le, Re, C);
+static void zero_site_update(fh_ctx* ctx, fh_mps* mps, int bond, const BlockTensor& Le, const BlockTensor& Re,
+                             BlockTensor& C, double tau, const fh_params* prm) {
+  plan_zero_site(ctx, mps, bond, Le, Re, C);
   const int64_t n = C.nelem;
   const int m = prm->krylov_dim;
   const int64_t wn = (int64_t)(m + 1) * n;
@@ -1042,13 +1090,20 @@ void fh::sweep1(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh
   ctx->stat_disc = 0.0;
   ctx->stat_chi = ctx->stat_su2 = ctx->stat_dmax = 0;
   const double tau = 0.5 * dt;
+  // task lists are kept from one one-site sweep to the next (context.hpp, PlanCache); the guard switches the
+  // cache off again on every exit so that no other entry point ever reads or fills it
+  struct CacheScope {
+    PlanCache& c;
+    explicit CacheScope(PlanCache& cc) : c(cc) { c.enabled = c.max_bytes > 0; }
+    ~CacheScope() { c.enabled = false; }
+  } cache_scope(mps->cache);
   for (int i = 0; i < L; ++i) {  // left -> right
     local_update1(ctx, mpo, mps, i, tau, prm);
     if (i < L - 1) {
       BlockTensor C;
       split_site(ctx, mps, i, +1, C);
       do_env_update_left(ctx, mpo, mps, i);
-      zero_site_update(ctx, mps->Lenv[i + 1], mps->Renv[i + 1], C, -tau, prm);
+      zero_site_update(ctx, mps, i + 1, mps->Lenv[i + 1], mps->Renv[i + 1], C, -tau, prm);
       absorb_bond(ctx, mps, i + 1, C, true);
       ctx->free_tensor(C);
     }
@@ -1059,7 +1114,7 @@ void fh::sweep1(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh
       BlockTensor C;
       split_site(ctx, mps, i, -1, C);
       do_env_update_right(ctx, mpo, mps, i);
-      zero_site_update(ctx, mps->Lenv[i], mps->Renv[i], C, -tau, prm);
+      zero_site_update(ctx, mps, i, mps->Lenv[i], mps->Renv[i], C, -tau, prm);
       absorb_bond(ctx, mps, i - 1, C, false);
       ctx->free_tensor(C);
     }
@@ -1071,6 +1126,7 @@ void fh::sweep(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh_
   FH_REQUIRE(mpo->L == L, FH_EINVAL, "tdvp2_sweep: MPO and MPS lengths differ");
   for (int i = 0; i < L; ++i) FH_REQUIRE(mps->A[i].base >= 0, FH_ESTATE, "tdvp2_sweep: site tensor missing");
   for (int i = 2; i <= L; ++i) FH_REQUIRE(mps->Renv[i].base >= 0, FH_ESTATE, "tdvp2_sweep: right environments missing (centre must be at site 0)");
+  mps->cache.clear();  // a two-site step changes the sector tables: the one-site task lists are stale
   ctx->stat_disc = 0.0;
   ctx->stat_chi = ctx->stat_su2 = ctx->stat_dmax = 0;
   const double tau = 0.5 * dt;

@@ -400,6 +400,50 @@ def test_next1_one_site_tdvp_L8_vs_oracle(H, ctx):
     ctx.mps_destroy(mps)
 
 
+def test_next1_one_site_task_list_cache(H, ctx, tmp_path):
+    """H0 for the one-site sweeps: tdvp1_sweep keeps its task lists from sweep to sweep (one-site TDVP leaves the
+    sector tables alone).  Two copies of the same L = 8 state (via mps_save / mps_load) run four
+    one-site sweeps, one with the cache, one with it switched off: every site tensor must agree bit for bit
+    (same lists, same launches), the cached run re-emits nothing after its first sweep, the uncached run never
+    hits, and a two-site sweep empties the cache."""
+    L, dt, m = 8, 0.05, 8
+    mpo = ctx.fh_mpo_build(L, 1.0, 4.0)
+    mps = ctx.mps_init_neel(mpo, L)
+    for _ in range(4):
+        ctx.tdvp2_sweep(mpo, mps, dt, krylov_dim=m, chi_max_full=60)
+    path = str(tmp_path / "s.fhmps")
+    ctx.mps_save(mps, path)
+    a, b = ctx.mps_load(mpo, path), ctx.mps_load(mpo, path)
+    ctx.fh_plan_cache_limit(b, 0)
+    ctx.tdvp1_sweep(mpo, a, dt, krylov_dim=m)
+    s1 = ctx.fh_plan_cache_stats(a)
+    # within the first sweep the right-to-left half already reuses the one-site and zero-site plans of the first half
+    assert s1["misses"] > 0 and s1["hits"] > 0 and s1["host_bytes"] > 0
+    for _ in range(3):
+        ctx.tdvp1_sweep(mpo, a, dt, krylov_dim=m)
+    s4 = ctx.fh_plan_cache_stats(a)
+    assert s4["misses"] == s1["misses"], (s1, s4)         # nothing re-emitted after the first sweep
+    assert s4["hits"] > s1["hits"] and s4["host_bytes"] == s1["host_bytes"]
+    for _ in range(4):
+        ctx.tdvp1_sweep(mpo, b, dt, krylov_dim=m)
+    sb = ctx.fh_plan_cache_stats(b)
+    assert sb["hits"] == 0 and sb["host_bytes"] == 0
+    for i in range(L):
+        assert np.array_equal(ctx.mps_site_layout(a, i)[0], ctx.mps_site_layout(b, i)[0])
+        assert np.array_equal(ctx.mps_get_site(a, i), ctx.mps_get_site(b, i)), i
+    # a different Hamiltonian on the same state must not reuse the lists (U enters the coefficients)
+    mpo2 = ctx.fh_mpo_build(L, 1.0, 2.0)
+    ctx.fh_plan_cache_limit(b, 1 << 30)
+    ctx.tdvp1_sweep(mpo2, a, dt, krylov_dim=m)
+    ctx.tdvp1_sweep(mpo2, b, dt, krylov_dim=m)
+    for i in range(L):
+        assert np.array_equal(ctx.mps_get_site(a, i), ctx.mps_get_site(b, i)), i
+    ctx.tdvp2_sweep(mpo, a, dt, krylov_dim=m, chi_max_full=60)
+    assert ctx.fh_plan_cache_stats(a)["host_bytes"] == 0
+    for h in (mps, a, b):
+        ctx.mps_destroy(h)
+
+
 # ------------------------------------------------------------------ NEXT-2: adaptive Krylov dimension (A-15)
 def test_next2_adaptive_krylov_expm_and_sweeps(H, ctx):
     """(a) heff_expm_adaptive on the chi = 256 central bond: same number of Krylov vectors as the oracle's
