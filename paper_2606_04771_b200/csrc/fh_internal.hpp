@@ -139,6 +139,34 @@ struct CopyBlk {
   double scale;
 };
 
+// ----------------------------------------------------------------------------- programmatic dependent launch
+// The kernels of the Lanczos loop (grouped ZGEMM stage 1 / stage 2, weighted dot, three-term update, scale) follow
+// one another on one stream, each depending on all of its predecessor.  They are launched with the
+// programmatic-stream-serialisation attribute: every CTA issues griddepcontrol.launch_dependents at its start, so
+// the next grid is set up and its CTAs move into warp slots the draining grid has freed, read their own
+// descriptor (uploaded before either kernel started) and then block in griddepcontrol.wait, which returns only
+// when the predecessor has completed and its writes are visible.  No kernel touches data a predecessor writes,
+// or writes anything, before its wait.  FH_NO_PDL=1 in the environment launches them the plain way (A/B timing).
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+bool pdl_enabled();
+template <class... KArgs, class... Args>
+inline void launch_pdl(void (*kern)(KArgs...), int grid, int block, cudaStream_t s, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)grid);
+  cfg.blockDim = dim3((unsigned)block);
+  cfg.dynamicSmemBytes = 0;
+  cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = pdl_enabled() ? 1 : 0;
+  cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+#endif
+
 // ----------------------------------------------------------------------------- kernel launchers (kernels.cu)
 void launch_grouped_gemm(const Stage& st, const cplx* A, const cplx* B, cplx* C, cudaStream_t s,
                          int64_t* launch_counter);

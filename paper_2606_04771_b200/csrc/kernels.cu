@@ -6,7 +6,17 @@
 // Reductions run in a fixed order: results are run-to-run bit-identical.
 #include "fh_internal.hpp"
 
+#include <cstdlib>
+
 namespace fh {
+
+bool pdl_enabled() {
+  static const bool on = [] {
+    const char* e = std::getenv("FH_NO_PDL");
+    return !(e && e[0] && e[0] != '0');
+  }();
+  return on;
+}
 
 // ------------------------------------------------------------------------------------------
 // PTX wrappers
@@ -107,7 +117,9 @@ __device__ __forceinline__ void finish_in_last_cta(const double* __restrict__ pa
 __global__ void __launch_bounds__(256) wdot_fused_kernel(const VecChunk* __restrict__ chunks, const cplx* __restrict__ x,
                                                          const cplx* __restrict__ y, double* __restrict__ partial,
                                                          double* __restrict__ result, unsigned* __restrict__ counter) {
+  pdl_launch_dependents();
   const VecChunk ch = chunks[blockIdx.x];
+  pdl_wait();
   const cplx* px = x + ch.start;
   const cplx* py = y + ch.start;
   double re = 0.0, im = 0.0;
@@ -140,7 +152,9 @@ __global__ void __launch_bounds__(256) lanczos_update_kernel(const VecChunk* __r
                                                              const cplx* __restrict__ vj, const cplx* __restrict__ vprev,
                                                              cplx* __restrict__ w, double* __restrict__ partial,
                                                              double* __restrict__ result, unsigned* __restrict__ counter) {
+  pdl_launch_dependents();
   const VecChunk ch = chunks[blockIdx.x];
+  pdl_wait();
   const double a = -alpha[0];
   const double b = beta_prev ? -beta_prev[0] : 0.0;
   const cplx* pv = vj + ch.start;
@@ -176,14 +190,14 @@ __global__ void __launch_bounds__(256) lanczos_update_kernel(const VecChunk* __r
 
 void launch_wdot_fused(const VecChunk* d_chunks, int nchunks, const cplx* x, const cplx* y, double* d_partial,
                        double* d_result, unsigned* d_counter, cudaStream_t s, int64_t* lc) {
-  wdot_fused_kernel<<<nchunks, 256, 0, s>>>(d_chunks, x, y, d_partial, d_result, d_counter);
+  launch_pdl(wdot_fused_kernel, nchunks, 256, s, d_chunks, x, y, d_partial, d_result, d_counter);
   ++*lc;
 }
 void launch_lanczos_update(const VecChunk* d_chunks, int nchunks, const double* d_alpha, const double* d_beta_prev,
                            const cplx* vj, const cplx* vprev, cplx* w, double* d_partial, double* d_result,
                            unsigned* d_counter, cudaStream_t s, int64_t* lc) {
-  lanczos_update_kernel<<<nchunks, 256, 0, s>>>(d_chunks, d_alpha, d_beta_prev, vj, vprev, w, d_partial, d_result,
-                                                d_counter);
+  launch_pdl(lanczos_update_kernel, nchunks, 256, s, d_chunks, d_alpha, d_beta_prev, vj, vprev, w, d_partial, d_result,
+             d_counter);
   ++*lc;
 }
 
@@ -228,6 +242,8 @@ __global__ void __launch_bounds__(256) scale_kernel(int64_t n, cplx a, const cpl
 __global__ void __launch_bounds__(256) scale_rsqrt_dev_kernel(int64_t n, const double* __restrict__ norm2, double tol,
                                                               const cplx* __restrict__ x, cplx* __restrict__ y,
                                                               double* __restrict__ beta_out) {
+  pdl_launch_dependents();
+  pdl_wait();
   const double b = sqrt(fmax(norm2[0], 0.0));
   const double f = (b < tol || b == 0.0) ? 0.0 : 1.0 / b;
   if (blockIdx.x == 0 && threadIdx.x == 0 && beta_out) beta_out[0] = b;
@@ -274,7 +290,7 @@ void launch_scale(int64_t n, cplx a, const cplx* x, cplx* y, cudaStream_t s, int
 void launch_scale_rsqrt_dev(int64_t n, const double* d_norm2, double tol, const cplx* x, cplx* y, double* d_beta,
                             cudaStream_t s, int64_t* lc) {
   if (n <= 0) return;
-  scale_rsqrt_dev_kernel<<<grid_for(n), 256, 0, s>>>(n, d_norm2, tol, x, y, d_beta);
+  launch_pdl(scale_rsqrt_dev_kernel, grid_for(n), 256, s, n, d_norm2, tol, x, y, d_beta);
   ++*lc;
 }
 void launch_lincomb(int64_t n, int m, const cplx* coef_host, const cplx* V, int64_t stride, cplx* y,

@@ -247,7 +247,9 @@ __global__ void __launch_bounds__(32) grouped_zgemm_kernel(const GemmUnit* __res
   unsigned long long t_begin = 0;
   if (trace) asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_begin));
 #endif
-  const GemmUnit u = units[ui];
+  pdl_launch_dependents();
+  const GemmUnit u = units[ui];  // uploaded before the predecessor started: readable before the wait
+  pdl_wait();
   const uint32_t ring = (uint32_t)__cvta_generic_to_shared(ring_smem);
   const double cs = conjA ? -1.0 : 1.0;
   switch (u.shape) {
@@ -303,7 +305,8 @@ void launch_grouped_gemm(const Stage& st, const cplx* A, const cplx* B, cplx* C,
   }
   grouped_zgemm_kernel<<<n, 32, 0, s>>>(st.d_units, n, st.d_segs, A, B, C, st.opA != OPA_N ? 1 : 0, tr);
 #else
-  grouped_zgemm_kernel<<<n, 32, 0, s>>>(st.d_units, n, st.d_segs, A, B, C, st.opA != OPA_N ? 1 : 0);
+  launch_pdl(grouped_zgemm_kernel, n, 32, s, (const GemmUnit*)st.d_units, n, (const GemmSeg*)st.d_segs, A, B, C,
+             st.opA != OPA_N ? 1 : 0);
 #endif
   ++*lc;
 }
