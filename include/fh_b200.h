@@ -208,6 +208,11 @@ int measure_global(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, double* no
 int fh_get_timers(const fh_ctx* ctx, double* sec_heff, double* sec_env, double* sec_svd,
                   double* sec_vec, double* sec_pack);
 int fh_reset_timers(fh_ctx* ctx);
+/* on = 0: the library records no phase events any more (fh_get_timers then returns what was accumulated before);
+ * on != 0 (the default at context creation) records them again.  An event record between two kernels of the
+ * Lanczos loop costs about a microsecond of GPU time and keeps the next kernel from being set up while its
+ * predecessor drains, so production runs that do not read the breakdown switch the timers off. */
+int fh_enable_timers(fh_ctx* ctx, int on);
 /* number of kernels the library launched since context creation */
 int64_t fh_launch_count(const fh_ctx* ctx);
 

@@ -75,6 +75,7 @@ _SIGS = {
     "measure_global": (c_int, [c_void_p, c_void_p, c_void_p, P(c_dbl), P(c_dbl)]),
     "fh_get_timers": (c_int, [c_void_p, P(c_dbl), P(c_dbl), P(c_dbl), P(c_dbl), P(c_dbl)]),
     "fh_reset_timers": (c_int, [c_void_p]),
+    "fh_enable_timers": (c_int, [c_void_p, c_int]),
     "fh_launch_count": (c_i64, [c_void_p]),
     "fh_cublas_gemm_seconds": (c_int, [c_void_p, c_int, c_int, c_int, P(c_dbl)]),
     "fh_coef_left": (c_dbl, [c_int] * 9),
@@ -350,6 +351,9 @@ class Context:
         a = (C.c_int64 * 6)()
         self.check(lib.fh_factorization_stats(self.h, a), "fh_factorization_stats")
         return dict(jacobi_kernel=a[0], gesvdp=a[1], gesvd=a[2], gesvdp_rejected=a[3], qr=a[4], qr_kernel=a[5])
+
+    def fh_enable_timers(self, on):
+        self.check(lib.fh_enable_timers(self.h, 1 if on else 0), "fh_enable_timers")
 
     def fh_plan_cache_stats(self, mps):
         a, b, c = C.c_int64(0), C.c_int64(0), C.c_int64(0)

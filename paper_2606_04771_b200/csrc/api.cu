@@ -92,6 +92,8 @@ void fh_ctx::ensure_pinned(size_t n) {
   FH_CUDA(cudaMallocHost((void**)&h_pinned, h_pinned_n * sizeof(double)));
 }
 void fh_ctx::timer_begin(int cat) {
+  span_open = timers_on;
+  if (!timers_on) return;
   if (spans.size() > 8192) timers_resolve();
   Span sp;
   for (cudaEvent_t* e : {&sp.a, &sp.b}) {
@@ -106,7 +108,11 @@ void fh_ctx::timer_begin(int cat) {
   FH_CUDA(cudaEventRecord(sp.a, stream));
   spans.push_back(sp);
 }
-void fh_ctx::timer_end() { FH_CUDA(cudaEventRecord(spans.back().b, stream)); }
+void fh_ctx::timer_end() {
+  if (!span_open) return;
+  span_open = false;
+  FH_CUDA(cudaEventRecord(spans.back().b, stream));
+}
 void fh_ctx::timers_resolve() {
   if (spans.empty()) return;
   FH_CUDA(cudaStreamSynchronize(stream));
@@ -263,8 +269,8 @@ void fh::apply_heff(fh_ctx* ctx, const cplx* theta, cplx* out) {
   Plan& P = ctx->plan;
   FH_REQUIRE(P.valid, FH_ESTATE, "heff_apply: no plan (call heff_plan first)");
   cplx* Z = ctx->ptr(P.Z.base);
-  launch_grouped_gemm(P.st1, P.Lptr, theta, Z, ctx->stream, &ctx->launches);
-  launch_grouped_gemm(P.st2, Z, P.Rptr, out, ctx->stream, &ctx->launches);
+  launch_grouped_gemm(P.st1, P.Lptr, theta, Z, ctx->stream, &ctx->launches, PDL_GEMM_FIRST);
+  launch_grouped_gemm(P.st2, Z, P.Rptr, out, ctx->stream, &ctx->launches, PDL_GEMM_SECOND);
   FH_CUDA(cudaGetLastError());
 }
 
@@ -1174,6 +1180,13 @@ int fh_reset_timers(fh_ctx* ctx) {
     FH_REQUIRE(ctx != nullptr, FH_EINVAL, "fh_reset_timers: NULL context");
     ctx->timers_resolve();
     for (int i = 0; i < T_NCAT; ++i) ctx->sec[i] = 0.0;
+  })
+}
+int fh_enable_timers(fh_ctx* ctx, int on) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx != nullptr, FH_EINVAL, "fh_enable_timers: NULL context");
+    ctx->timers_resolve();
+    ctx->timers_on = on != 0;
   })
 }
 int64_t fh_launch_count(const fh_ctx* ctx) { return ctx ? ctx->launches : -1; }

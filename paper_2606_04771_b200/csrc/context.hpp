@@ -126,7 +126,10 @@ struct fh_ctx {
   // pinned host scratch
   double* h_pinned = nullptr;  // 4096 doubles
   size_t h_pinned_n = 0;
-  // timers
+  // timers (event pairs around every phase; fh_enable_timers(ctx, 0) drops them: an event record between two
+  // kernels costs GPU front-end time and cancels the programmatic dependent launch across it)
+  bool timers_on = true;
+  bool span_open = false;
   double sec[fh::T_NCAT] = {0, 0, 0, 0, 0};
   struct Span {
     cudaEvent_t a, b;

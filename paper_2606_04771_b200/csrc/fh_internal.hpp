@@ -150,9 +150,12 @@ struct CopyBlk {
 #ifdef __CUDACC__
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-bool pdl_enabled();
+// roles of a launch (bit mask; FH_PDL_MASK in the environment overrides which roles carry the attribute)
+enum { PDL_GEMM_FIRST = 1, PDL_GEMM_SECOND = 2, PDL_WDOT = 4, PDL_UPDATE = 8, PDL_SCALE = 16, PDL_GEMM_OTHER = 32 };
+const int PDL_DEFAULT_MASK = PDL_WDOT | PDL_UPDATE | PDL_SCALE;  // measured: see DESIGN.md 6.3
+bool pdl_enabled(int role);
 template <class... KArgs, class... Args>
-inline void launch_pdl(void (*kern)(KArgs...), int grid, int block, cudaStream_t s, Args... args) {
+inline void launch_pdl(int role, void (*kern)(KArgs...), int grid, int block, cudaStream_t s, Args... args) {
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)grid);
   cfg.blockDim = dim3((unsigned)block);
@@ -162,14 +165,14 @@ inline void launch_pdl(void (*kern)(KArgs...), int grid, int block, cudaStream_t
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = at;
-  cfg.numAttrs = pdl_enabled() ? 1 : 0;
+  cfg.numAttrs = pdl_enabled(role) ? 1 : 0;
   cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
 }
 #endif
 
 // ----------------------------------------------------------------------------- kernel launchers (kernels.cu)
 void launch_grouped_gemm(const Stage& st, const cplx* A, const cplx* B, cplx* C, cudaStream_t s,
-                         int64_t* launch_counter);
+                         int64_t* launch_counter, int pdl_role = 32 /* PDL_GEMM_OTHER */);
 void launch_wdot(const VecChunk* d_chunks, int nchunks, const cplx* x, const cplx* y, double* d_partial,
                  double* d_result, cudaStream_t s, int64_t* launch_counter);
 // y = y + a*x (a complex, from device scalar array coef[idx]*sign) etc.: see kernels.cu

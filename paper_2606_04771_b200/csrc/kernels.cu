@@ -10,12 +10,14 @@
 
 namespace fh {
 
-bool pdl_enabled() {
-  static const bool on = [] {
-    const char* e = std::getenv("FH_NO_PDL");
-    return !(e && e[0] && e[0] != '0');
+bool pdl_enabled(int role) {
+  static const int mask = [] {
+    const char* off = std::getenv("FH_NO_PDL");
+    if (off && off[0] && off[0] != '0') return 0;
+    const char* m = std::getenv("FH_PDL_MASK");
+    return m && m[0] ? std::atoi(m) : PDL_DEFAULT_MASK;
   }();
-  return on;
+  return (mask & role) != 0;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -190,13 +192,13 @@ __global__ void __launch_bounds__(256) lanczos_update_kernel(const VecChunk* __r
 
 void launch_wdot_fused(const VecChunk* d_chunks, int nchunks, const cplx* x, const cplx* y, double* d_partial,
                        double* d_result, unsigned* d_counter, cudaStream_t s, int64_t* lc) {
-  launch_pdl(wdot_fused_kernel, nchunks, 256, s, d_chunks, x, y, d_partial, d_result, d_counter);
+  launch_pdl(PDL_WDOT, wdot_fused_kernel, nchunks, 256, s, d_chunks, x, y, d_partial, d_result, d_counter);
   ++*lc;
 }
 void launch_lanczos_update(const VecChunk* d_chunks, int nchunks, const double* d_alpha, const double* d_beta_prev,
                            const cplx* vj, const cplx* vprev, cplx* w, double* d_partial, double* d_result,
                            unsigned* d_counter, cudaStream_t s, int64_t* lc) {
-  launch_pdl(lanczos_update_kernel, nchunks, 256, s, d_chunks, d_alpha, d_beta_prev, vj, vprev, w, d_partial, d_result,
+  launch_pdl(PDL_UPDATE, lanczos_update_kernel, nchunks, 256, s, d_chunks, d_alpha, d_beta_prev, vj, vprev, w, d_partial, d_result,
              d_counter);
   ++*lc;
 }
@@ -290,7 +292,7 @@ void launch_scale(int64_t n, cplx a, const cplx* x, cplx* y, cudaStream_t s, int
 void launch_scale_rsqrt_dev(int64_t n, const double* d_norm2, double tol, const cplx* x, cplx* y, double* d_beta,
                             cudaStream_t s, int64_t* lc) {
   if (n <= 0) return;
-  launch_pdl(scale_rsqrt_dev_kernel, grid_for(n), 256, s, n, d_norm2, tol, x, y, d_beta);
+  launch_pdl(PDL_SCALE, scale_rsqrt_dev_kernel, grid_for(n), 256, s, n, d_norm2, tol, x, y, d_beta);
   ++*lc;
 }
 void launch_lincomb(int64_t n, int m, const cplx* coef_host, const cplx* V, int64_t stride, cplx* y,

@@ -294,7 +294,8 @@ extern "C" void fh_debug_unit_trace(unsigned long long* dev_buf, size_t capacity
 extern "C" size_t fh_debug_unit_trace_used() { return g_trace_used; }
 #endif
 
-void launch_grouped_gemm(const Stage& st, const cplx* A, const cplx* B, cplx* C, cudaStream_t s, int64_t* lc) {
+void launch_grouped_gemm(const Stage& st, const cplx* A, const cplx* B, cplx* C, cudaStream_t s, int64_t* lc,
+                         int pdl_role) {
   const int n = (int)st.units.size();
   if (n == 0) return;
 #ifdef FH_UNIT_TRACE
@@ -305,7 +306,7 @@ void launch_grouped_gemm(const Stage& st, const cplx* A, const cplx* B, cplx* C,
   }
   grouped_zgemm_kernel<<<n, 32, 0, s>>>(st.d_units, n, st.d_segs, A, B, C, st.opA != OPA_N ? 1 : 0, tr);
 #else
-  launch_pdl(grouped_zgemm_kernel, n, 32, s, (const GemmUnit*)st.d_units, n, (const GemmSeg*)st.d_segs, A, B, C,
+  launch_pdl(pdl_role, grouped_zgemm_kernel, n, 32, s, (const GemmUnit*)st.d_units, n, (const GemmSeg*)st.d_segs, A, B, C,
              st.opA != OPA_N ? 1 : 0);
 #endif
   ++*lc;
