@@ -580,6 +580,7 @@ void fh_ctx_destroy(fh_ctx* c) {
     if (w.s) cudaStreamDestroy(w.s);
   }
   if (c->svd_fork) cudaEventDestroy(c->svd_fork);
+  if (c->small_copied) cudaEventDestroy(c->small_copied);
   if (c->h_pinned) cudaFreeHost(c->h_pinned);
   if (c->own_arena) cudaFree(c->arena);
   delete c;

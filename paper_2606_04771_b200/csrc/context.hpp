@@ -152,6 +152,9 @@ struct fh_ctx {
   };
   std::vector<SvdWorker> svd_workers;
   cudaEvent_t svd_fork = nullptr;
+  cudaEvent_t small_copied = nullptr;  // descriptors of the small-matrix kernels have left small_desc_host
+  bool small_copied_armed = false;
+  std::vector<char> small_desc_host;
   int device = 0;
   int64_t svd_count[3] = {0, 0, 0};  // gesvd, gesvdp, gesvdp fallbacks to gesvd
   int64_t qr_small = 0;  // one-site splits done by small_qr_kernel

@@ -393,6 +393,16 @@ void qr_one(fh_ctx::SvdWorker& w, const SectorSvd& S, cplx* buf) {
   FH_CUSOLVER(cusolverDnZungqr(w.h, m, k, k, A, m, tau, (cuDoubleComplex*)w.dwork, lwork, w.d_info));
 }
 
+// Descriptors of the small-matrix kernels go through a host buffer owned by the context (it outlives the
+// asynchronous copy; the event guards its reuse), so their launch needs no stream synchronisation.
+const void* stage_small_desc(fh_ctx* ctx, const void* src, size_t bytes) {
+  if (ctx->small_copied_armed) FH_CUDA(cudaEventSynchronize(ctx->small_copied));
+  ctx->small_copied_armed = true;
+  if (ctx->small_desc_host.size() < bytes) ctx->small_desc_host.resize(bytes + bytes / 2);
+  std::memcpy(ctx->small_desc_host.data(), src, bytes);
+  return ctx->small_desc_host.data();
+}
+
 // All sector SVDs of one bond (H9), heaviest first, pulled by host worker threads from a shared
 // counter; every worker has its own cuSOLVER handle, stream and workspace.  The main stream forks
 // into the worker streams and joins them again through events, so the phase timers on the main
@@ -412,6 +422,7 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
       FH_CUDA(cudaEventCreateWithFlags(&w.done, cudaEventDisableTiming));
     }
     FH_CUDA(cudaEventCreateWithFlags(&ctx->svd_fork, cudaEventDisableTiming));
+    FH_CUDA(cudaEventCreateWithFlags(&ctx->small_copied, cudaEventDisableTiming));
   }
   const int nw = (int)ctx->svd_workers.size();
   std::vector<int> idx;
@@ -436,6 +447,13 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
       idx.push_back((int)i);
     }
   }
+  // The worker streams fork from the main stream HERE, before the launch of the library's own small-matrix
+  // kernel: that kernel (one CTA per matrix, a few tens of SMs) then runs on the main stream while the vendor
+  // routines of the larger matrices run on the worker streams; the main stream joins them at the end.
+  if (!idx.empty()) {
+    FH_CUDA(cudaEventRecord(ctx->svd_fork, ctx->stream));
+    for (auto& w : ctx->svd_workers) FH_CUDA(cudaStreamWaitEvent(w.s, ctx->svd_fork, 0));
+  }
   if (!small_qr.empty()) {
     static bool qr_attr_done = false;
     if (!qr_attr_done) {
@@ -445,7 +463,8 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
     const size_t need = small_qr.size() * sizeof(SmallQr);
     ctx->pool_small.reserve(need + 256, ctx->stream);
     SmallQr* d_qr = (SmallQr*)ctx->pool_small.take(need);
-    FH_CUDA(cudaMemcpyAsync(d_qr, small_qr.data(), need, cudaMemcpyHostToDevice, ctx->stream));
+    FH_CUDA(cudaMemcpyAsync(d_qr, stage_small_desc(ctx, small_qr.data(), need), need, cudaMemcpyHostToDevice, ctx->stream));
+    FH_CUDA(cudaEventRecord(ctx->small_copied, ctx->stream));
     int qn_max = 0;  // one warp per trailing column of a Householder step
     for (const SmallQr& d : small_qr) qn_max = std::max(qn_max, d.n);
     const int qr_warps = qn_max <= 16 ? 8 : (qn_max <= 32 ? 16 : SMALL_QR_MAX_WARPS);
@@ -453,7 +472,6 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
     ++ctx->launches;
     ctx->qr_small += (int64_t)small_qr.size();
     FH_CUDA(cudaGetLastError());
-    FH_CUDA(cudaStreamSynchronize(ctx->stream));  // `small_qr` (pageable host memory) must outlive the copy
   }
   if (!small.empty()) {
     static bool attr_done = false;
@@ -465,7 +483,8 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
     const size_t need = small.size() * sizeof(SmallSvd);
     ctx->pool_small.reserve(need + 256, ctx->stream);
     SmallSvd* d_small = (SmallSvd*)ctx->pool_small.take(need);
-    FH_CUDA(cudaMemcpyAsync(d_small, small.data(), need, cudaMemcpyHostToDevice, ctx->stream));
+    FH_CUDA(cudaMemcpyAsync(d_small, stage_small_desc(ctx, small.data(), need), need, cudaMemcpyHostToDevice, ctx->stream));
+    FH_CUDA(cudaEventRecord(ctx->small_copied, ctx->stream));
     // one warp per column pair of a tournament round: n / 2 pairs want up to 32 warps for the largest matrices
     int nmax = 0;
     for (const SmallSvd& d : small) nmax = std::max(nmax, d.n);
@@ -474,7 +493,6 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
     ++ctx->launches;
     ctx->svd_small += (int64_t)small.size();
     FH_CUDA(cudaGetLastError());
-    FH_CUDA(cudaStreamSynchronize(ctx->stream));  // `small` (pageable host memory) must outlive the copy
   }
   if (idx.empty()) return;
   if (qr) ctx->qr_count += (int64_t)idx.size();
@@ -483,8 +501,6 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
     return m * n * n;
   };
   std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) { return cost(a) > cost(b); });
-  FH_CUDA(cudaEventRecord(ctx->svd_fork, ctx->stream));
-  for (auto& w : ctx->svd_workers) FH_CUDA(cudaStreamWaitEvent(w.s, ctx->svd_fork, 0));
   std::atomic<int> next{0};
   std::vector<std::string> errs(nw);
   std::vector<std::array<int64_t, 3>> counts(nw, std::array<int64_t, 3>{0, 0, 0});
