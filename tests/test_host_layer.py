@@ -144,3 +144,14 @@ def test_zero_site_task_lists_match_oracle(binding):
     fl = sum(8 * dl[xk[0]] * dl[xk[2]] * dr[xk[2]] for xk in st1) + \
         sum(8 * dl[o] * dr[seg[0][2]] * dr[o] for o, segs in st2.items() for seg in segs)
     assert f1 + f2 == fl
+
+
+def test_host_only_entry_points_refuse_null_handles(binding):
+    """fh_plan_cache_stats / fh_plan_cache_limit / fh_enable_timers are host-only calls: without a GPU they can
+    still be reached, and a NULL handle or a negative limit is FH_EINVAL (include/fh_b200.h), never a crash."""
+    import ctypes as C
+    lib = binding.lib
+    a = C.c_int64(7)
+    assert lib.fh_plan_cache_stats(None, C.byref(a), None, None) < 0 and a.value == 7
+    assert lib.fh_plan_cache_limit(None, 0) < 0
+    assert lib.fh_enable_timers(None, 0) < 0
