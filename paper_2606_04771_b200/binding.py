@@ -348,9 +348,10 @@ class Context:
         return k.value
 
     def fh_factorization_stats(self):
-        a = (C.c_int64 * 6)()
+        a = (C.c_int64 * 7)()
         self.check(lib.fh_factorization_stats(self.h, a), "fh_factorization_stats")
-        return dict(jacobi_kernel=a[0], gesvdp=a[1], gesvd=a[2], gesvdp_rejected=a[3], qr=a[4], qr_kernel=a[5])
+        return dict(jacobi_kernel=a[0], gesvdp=a[1], gesvd=a[2], gesvdp_rejected=a[3], qr=a[4], qr_kernel=a[5],
+                    jacobi_mid_kernel=a[6])
 
     def fh_enable_timers(self, on):
         self.check(lib.fh_enable_timers(self.h, 1 if on else 0), "fh_enable_timers")

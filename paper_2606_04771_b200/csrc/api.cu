@@ -581,6 +581,8 @@ void fh_ctx_destroy(fh_ctx* c) {
   }
   if (c->svd_fork) cudaEventDestroy(c->svd_fork);
   if (c->small_copied) cudaEventDestroy(c->small_copied);
+  if (c->svd_side_done) cudaEventDestroy(c->svd_side_done);
+  if (c->svd_side) cudaStreamDestroy(c->svd_side);
   if (c->h_pinned) cudaFreeHost(c->h_pinned);
   if (c->own_arena) cudaFree(c->arena);
   delete c;
@@ -1052,8 +1054,9 @@ int heff_expm_adaptive(fh_ctx* ctx, const void* theta_dev, void* out_dev, double
   return heff_expm_impl(ctx, theta_dev, out_dev, tau, krylov_dim, adapt_tol, k_used);
 }
 
-int fh_factorization_stats(const fh_ctx* ctx, int64_t counts[6]) {
+int fh_factorization_stats(const fh_ctx* ctx, int64_t counts[7]) {
   if (!ctx || !counts) return FH_EINVAL;
+  counts[6] = ctx->svd_mid;
   counts[5] = ctx->qr_small;
   counts[0] = ctx->svd_small;
   counts[1] = ctx->svd_count[1];

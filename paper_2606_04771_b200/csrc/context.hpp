@@ -152,6 +152,9 @@ struct fh_ctx {
   };
   std::vector<SvdWorker> svd_workers;
   cudaEvent_t svd_fork = nullptr;
+  cudaStream_t svd_side = nullptr;       // mid_svd_kernel runs here, beside the main stream and the workers
+  cudaEvent_t svd_side_done = nullptr;
+  int64_t svd_mid = 0;                   // sector matrices factorised by mid_svd_kernel
   cudaEvent_t small_copied = nullptr;  // descriptors of the small-matrix kernels have left small_desc_host
   bool small_copied_armed = false;
   std::vector<char> small_desc_host;

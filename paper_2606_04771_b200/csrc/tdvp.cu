@@ -189,6 +189,112 @@ __global__ void __launch_bounds__(32 * SMALL_SVD_MAX_WARPS) small_svd_kernel(con
 }
 
 // ------------------------------------------------------------------------------------------
+// Mid-size sector matrices (too large for small_svd_kernel, n <= 120 by default, FH_SVD_MID_MAXN): the same one-sided Jacobi, one
+// 32-warp CTA per matrix, working IN PLACE on B in global memory with V in arena scratch.  A matrix of this size
+// (B and V together 0.3-0.7 MB) stays in the L1/L2 of its SM, and all accesses of a column pair come from one
+// warp, with __syncthreads between tournament rounds, so plain loads and stores are coherent.  It is slower per
+// matrix than the vendor routine (about 10 ms against 5 ms) but it is ONE launch for all of them on a side
+// stream, while the vendor drivers, which are bound by their ~800 launches per matrix on the host threads, work
+// through the larger matrices: every matrix moved here shortens the vendor queue of the bond.
+struct MidSvd {
+  int64_t m_off, u_off, vt_off, s_off, v_off;  // v_off relative to the V scratch base
+  int m, n;
+};
+constexpr int MID_SVD_HARD_MAXN = 256;
+__global__ void __launch_bounds__(1024) mid_svd_kernel(const MidSvd* __restrict__ descs, cplx* buf, cplx* vbase,
+                                                       double* __restrict__ dS) {
+  __shared__ int rotated_any;
+  __shared__ double sig[MID_SVD_HARD_MAXN];
+  const MidSvd d = descs[blockIdx.x];
+  const int m = d.m, n = d.n, lane = threadIdx.x & 31, warp = threadIdx.x >> 5, tid = threadIdx.x;
+  const int NT = blockDim.x, NW = blockDim.x >> 5;
+  cplx* G = buf + d.m_off;   // m x n column-major, rotated in place
+  cplx* V = vbase + d.v_off;  // n x n column-major
+  for (int i = tid; i < n * n; i += NT) V[i] = make_double2((i % n) == (i / n) ? 1.0 : 0.0, 0.0);
+  __syncthreads();
+  const int ne = (n + 1) & ~1;
+  for (int sweep = 0; sweep < 40 && n > 1; ++sweep) {
+    if (tid == 0) rotated_any = 0;
+    __syncthreads();
+    for (int r = 0; r < ne - 1; ++r) {
+      for (int k = warp; k < ne / 2; k += NW) {
+        int p = (r + k) % (ne - 1);
+        int q = k == 0 ? ne - 1 : (r - k + ne - 1) % (ne - 1);
+        if (p > q) { const int t_ = p; p = q; q = t_; }
+        if (q >= n) continue;
+        cplx* gp = G + (size_t)p * m;
+        cplx* gq = G + (size_t)q * m;
+        double a = 0.0, b = 0.0, cr = 0.0, ci = 0.0;
+        for (int i = lane; i < m; i += 32) {
+          const cplx x = gp[i], y = gq[i];
+          a += x.x * x.x + x.y * x.y;
+          b += y.x * y.x + y.y * y.y;
+          cr += x.x * y.x + x.y * y.y;
+          ci += x.x * y.y - x.y * y.x;
+        }
+        a = warp_sum_all(a);
+        b = warp_sum_all(b);
+        cr = warp_sum_all(cr);
+        ci = warp_sum_all(ci);
+        const double c2 = cr * cr + ci * ci;
+        if (c2 <= 1e-30 * a * b || c2 == 0.0) continue;
+        if (lane == 0) rotated_any = 1;
+        const double cabs = sqrt(c2);
+        const double pr = cr / cabs, pi = ci / cabs;
+        const double zeta = (b - a) / (2.0 * cabs);
+        const double t = (zeta >= 0.0 ? 1.0 : -1.0) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
+        const double cs = 1.0 / sqrt(1.0 + t * t), sn = cs * t;
+        for (int i = lane; i < m; i += 32) {
+          const cplx x = gp[i], y = gq[i];
+          const double yr = pr * y.x + pi * y.y, yi = pr * y.y - pi * y.x;
+          gp[i] = make_double2(cs * x.x - sn * yr, cs * x.y - sn * yi);
+          gq[i] = make_double2(sn * x.x + cs * yr, sn * x.y + cs * yi);
+        }
+        cplx* vp = V + (size_t)p * n;
+        cplx* vq = V + (size_t)q * n;
+        for (int i = lane; i < n; i += 32) {
+          const cplx x = vp[i], y = vq[i];
+          const double yr = pr * y.x + pi * y.y, yi = pr * y.y - pi * y.x;
+          vp[i] = make_double2(cs * x.x - sn * yr, cs * x.y - sn * yi);
+          vq[i] = make_double2(sn * x.x + cs * yr, sn * x.y + cs * yi);
+        }
+      }
+      __syncthreads();
+    }
+    if (!rotated_any) break;
+    __syncthreads();
+  }
+  for (int j = warp; j < n; j += NW) {
+    double a = 0.0;
+    for (int i = lane; i < m; i += 32) {
+      const cplx x = G[(size_t)j * m + i];
+      a += x.x * x.x + x.y * x.y;
+    }
+    a = warp_sum_all(a);
+    if (lane == 0) sig[j] = sqrt(a);
+  }
+  __syncthreads();
+  cplx* U = buf + d.u_off;
+  cplx* VT = buf + d.vt_off;
+  double* S = dS + d.s_off;
+  for (int j = warp; j < n; j += NW) {
+    const double sj = sig[j];
+    int rank = 0;
+    for (int l = 0; l < n; ++l) rank += (sig[l] > sj || (sig[l] == sj && l < j)) ? 1 : 0;
+    const double inv = sj > 0.0 ? 1.0 / sj : 0.0;
+    if (lane == 0) S[rank] = sj;
+    for (int i = lane; i < m; i += 32) {
+      const cplx x = G[(size_t)j * m + i];
+      U[(size_t)rank * m + i] = make_double2(x.x * inv, x.y * inv);
+    }
+    for (int i = lane; i < n; i += 32) {
+      const cplx x = V[(size_t)j * n + i];
+      VT[(size_t)i * n + rank] = make_double2(x.x, -x.y);
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------
 // Small one-site splits (the whole qm x qn sector matrix fits shared memory): Householder QR in one launch for
 // all of them, one CTA of 8 to 32 warps per matrix.  Same conventions as cusolverDnZgeqrf + Zungqr (LAPACK zlarfg /
 // zung2r: H_j = I - tau_j v v^H with v_0 = 1, real diagonal of R): column-major A (m x n) at m_off is
@@ -423,12 +529,21 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
     }
     FH_CUDA(cudaEventCreateWithFlags(&ctx->svd_fork, cudaEventDisableTiming));
     FH_CUDA(cudaEventCreateWithFlags(&ctx->small_copied, cudaEventDisableTiming));
+    FH_CUDA(cudaStreamCreateWithFlags(&ctx->svd_side, cudaStreamNonBlocking));
+    FH_CUDA(cudaEventCreateWithFlags(&ctx->svd_side_done, cudaEventDisableTiming));
   }
   const int nw = (int)ctx->svd_workers.size();
   std::vector<int> idx;
   std::vector<SmallSvd> small;
+  std::vector<MidSvd> mid;
   std::vector<SmallQr> small_qr;
   size_t small_smem = 0, small_qr_smem = 0;
+  int64_t mid_v_total = 0;
+  // FH_SVD_MID_MAXN (read at every call, so that a test can compare the two routes in one process): 0 sends
+  // every matrix above the shared-memory route to cuSOLVER
+  const char* mid_env = std::getenv("FH_SVD_MID_MAXN");
+  const int mid_maxn = std::max(0, std::min(mid_env && mid_env[0] ? std::atoi(mid_env) : 120, MID_SVD_HARD_MAXN));
+  const double mid_work = 1.5 * mid_maxn * (double)mid_maxn * mid_maxn;  // m n^2 bound: a long thin matrix would make its one CTA the critical path
   static const bool use_small_qr = [] {
     const char* e = std::getenv("FH_SMALL_QR");  // "0" sends every one-site split to cuSOLVER
     return !(e && e[0] == '0');
@@ -438,6 +553,9 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
     if (!qr && small_svd_bytes(m, n) <= SMALL_SVD_SMEM) {
       small.push_back(SmallSvd{order[i]->m_off, order[i]->u_off, order[i]->vt_off, order[i]->s_off, m, n});
       small_smem = std::max(small_smem, ((size_t)m * n + (size_t)n * n) * sizeof(cplx) + (size_t)n * sizeof(double));
+    } else if (!qr && n <= mid_maxn && (double)m * n * n <= mid_work) {
+      mid.push_back(MidSvd{order[i]->m_off, order[i]->u_off, order[i]->vt_off, order[i]->s_off, mid_v_total, m, n});
+      mid_v_total += ((int64_t)n * n + 15) / 16 * 16;
     } else if (qr && use_small_qr && (size_t)order[i]->qm * order[i]->qn * sizeof(cplx) <= SMALL_QR_SMEM &&
                std::min(order[i]->qm, order[i]->qn) <= SMALL_QR_MAXK) {
       small_qr.push_back(SmallQr{order[i]->m_off, order[i]->r_dst, order[i]->qm, order[i]->qn, order[i]->r_ld,
@@ -450,10 +568,42 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
   // The worker streams fork from the main stream HERE, before the launch of the library's own small-matrix
   // kernel: that kernel (one CTA per matrix, a few tens of SMs) then runs on the main stream while the vendor
   // routines of the larger matrices run on the worker streams; the main stream joins them at the end.
-  if (!idx.empty()) {
+  // one reservation for the descriptor tables of this call (reserve() rewinds the pool)
+  ctx->pool_small.reserve(mid.size() * sizeof(MidSvd) + small.size() * sizeof(SmallSvd) +
+                              small_qr.size() * sizeof(SmallQr) + 1024,
+                          ctx->stream);
+  MidSvd* d_mid = nullptr;
+  int64_t mid_v_off = -1;
+  if (!mid.empty()) {
+    // heaviest first: the CTAs of the largest matrices start first
+    std::stable_sort(mid.begin(), mid.end(), [](const MidSvd& a, const MidSvd& b) {
+      return (double)a.m * a.n * a.n > (double)b.m * b.n * b.n;
+    });
+    const size_t need = mid.size() * sizeof(MidSvd);
+    d_mid = (MidSvd*)ctx->pool_small.take(need);
+    FH_CUDA(cudaMemcpyAsync(d_mid, stage_small_desc(ctx, mid.data(), need), need, cudaMemcpyHostToDevice, ctx->stream));
+    FH_CUDA(cudaEventRecord(ctx->small_copied, ctx->stream));
+    mid_v_off = ctx->alloc.alloc(mid_v_total);
+  }
+  if (!idx.empty() || !mid.empty()) {
     FH_CUDA(cudaEventRecord(ctx->svd_fork, ctx->stream));
     for (auto& w : ctx->svd_workers) FH_CUDA(cudaStreamWaitEvent(w.s, ctx->svd_fork, 0));
   }
+  if (!mid.empty()) {
+    FH_CUDA(cudaStreamWaitEvent(ctx->svd_side, ctx->svd_fork, 0));
+    mid_svd_kernel<<<(int)mid.size(), 1024, 0, ctx->svd_side>>>(d_mid, buf, ctx->ptr(mid_v_off), dS);
+    ++ctx->launches;
+    ctx->svd_mid += (int64_t)mid.size();
+    FH_CUDA(cudaGetLastError());
+    FH_CUDA(cudaEventRecord(ctx->svd_side_done, ctx->svd_side));
+  }
+  // joins the side stream and returns the V scratch (stream-ordered: later users of that arena range are
+  // enqueued on the main stream behind the wait)
+  auto join_side = [&]() {
+    if (mid.empty()) return;
+    FH_CUDA(cudaStreamWaitEvent(ctx->stream, ctx->svd_side_done, 0));
+    ctx->alloc.release(mid_v_off, mid_v_total);
+  };
   if (!small_qr.empty()) {
     static bool qr_attr_done = false;
     if (!qr_attr_done) {
@@ -461,7 +611,6 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
       qr_attr_done = true;
     }
     const size_t need = small_qr.size() * sizeof(SmallQr);
-    ctx->pool_small.reserve(need + 256, ctx->stream);
     SmallQr* d_qr = (SmallQr*)ctx->pool_small.take(need);
     FH_CUDA(cudaMemcpyAsync(d_qr, stage_small_desc(ctx, small_qr.data(), need), need, cudaMemcpyHostToDevice, ctx->stream));
     FH_CUDA(cudaEventRecord(ctx->small_copied, ctx->stream));
@@ -481,7 +630,6 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
       attr_done = true;
     }
     const size_t need = small.size() * sizeof(SmallSvd);
-    ctx->pool_small.reserve(need + 256, ctx->stream);
     SmallSvd* d_small = (SmallSvd*)ctx->pool_small.take(need);
     FH_CUDA(cudaMemcpyAsync(d_small, stage_small_desc(ctx, small.data(), need), need, cudaMemcpyHostToDevice, ctx->stream));
     FH_CUDA(cudaEventRecord(ctx->small_copied, ctx->stream));
@@ -494,7 +642,10 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
     ctx->svd_small += (int64_t)small.size();
     FH_CUDA(cudaGetLastError());
   }
-  if (idx.empty()) return;
+  if (idx.empty()) {
+    join_side();
+    return;
+  }
   if (qr) ctx->qr_count += (int64_t)idx.size();
   auto cost = [&](int i) {
     const double m = std::max(order[i]->nrow, order[i]->ncol), n = order[i]->k;
@@ -533,6 +684,7 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
     FH_CUDA(cudaStreamWaitEvent(ctx->stream, ctx->svd_workers[t].done, 0));
     for (int k = 0; k < 3; ++k) ctx->svd_count[k] += counts[t][k];
   }
+  join_side();
 }
 
 }  // namespace

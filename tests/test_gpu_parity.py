@@ -1,6 +1,8 @@
 """GPU parity tests (-m gpu): the CUDA path, called through the C-ABI binding, against the CPU
 oracle on the same seeded inputs.  Tolerances (north_star): relative Frobenius error <= 1e-11 per
 heff_apply in FP64; local observables within 1e-8 at matched chi; task tuples bit-exact."""
+import os
+
 import numpy as np
 import pytest
 
@@ -626,7 +628,8 @@ def test_quench_L24_large_sectors_invariants(H, ctx):
     g2, o2 = check("end of two-site phase", 1e-5)
     f1 = ctx.fh_factorization_stats()
     assert st["chi_full"] > 300 and st["dmax"] >= 24, st
-    assert f1["gesvdp"] - f0["gesvdp"] > 0, f1                       # the vendor route really ran
+    # the routes above the shared-memory kernel really ran (own global-memory Jacobi up to 120 columns, vendor beyond)
+    assert f1["gesvdp"] + f1["jacobi_mid_kernel"] - f0["gesvdp"] - f0["jacobi_mid_kernel"] > 0, f1
     assert f1["jacobi_kernel"] - f0["jacobi_kernel"] > 0, f1
     dims_before = [ctx.mps_get_bond(mps, k) for k in range(L + 1)]
     for step in range(4):
@@ -640,6 +643,50 @@ def test_quench_L24_large_sectors_invariants(H, ctx):
     print("L=24 quench: chi_full %d, d_max %d, factorizations %s, E = %.2e, norm2 - 1 = %.2e"
           % (st["chi_full"], st["dmax"], f2, g1["energy"], g1["norm2"] - 1.0))
     ctx.mps_destroy(mps)
+
+
+def test_mid_size_jacobi_kernel_vs_vendor_svd(H, ctx, tmp_path):
+    """H9: sector matrices above the shared-memory route with at most 120 columns are factorised by the library's
+    own global-memory Jacobi kernel (mid_svd_kernel, on a side stream beside the vendor routines).  The same L = 16
+    state (grown by an untruncated quench until sector matrices of 90-120 columns exist) takes one two-site sweep
+    with that kernel and, from a reloaded copy, one with FH_SVD_MID_MAXN=0 (every such matrix through cusolver's
+    gesvdp / gesvd): both routes must have run, the kept singular values of every bond agree to 1e-11 s_max, the
+    sector tables are identical and the observables agree to 1e-10."""
+    L, dt, m = 16, 0.1, 8
+    mpo = ctx.fh_mpo_build(L, 1.0, 4.0)
+    mps = ctx.mps_init_neel(mpo, L)
+    for _ in range(22):
+        ctx.tdvp2_sweep(mpo, mps, dt, krylov_dim=m, chi_max_full=1200, eps_trunc=1e-12)
+    path = str(tmp_path / "mid.fhmps")
+    ctx.mps_save(mps, path)
+    a, b = ctx.mps_load(mpo, path), ctx.mps_load(mpo, path)
+    f0 = ctx.fh_factorization_stats()
+    ctx.tdvp2_sweep(mpo, a, dt, krylov_dim=m, chi_max_full=1200, eps_trunc=1e-12)
+    f1 = ctx.fh_factorization_stats()
+    os.environ["FH_SVD_MID_MAXN"] = "0"
+    try:
+        ctx.tdvp2_sweep(mpo, b, dt, krylov_dim=m, chi_max_full=1200, eps_trunc=1e-12)
+    finally:
+        del os.environ["FH_SVD_MID_MAXN"]
+    f2 = ctx.fh_factorization_stats()
+    assert f1["jacobi_mid_kernel"] - f0["jacobi_mid_kernel"] > 0, (f0, f1)
+    assert f2["jacobi_mid_kernel"] == f1["jacobi_mid_kernel"]
+    assert f2["gesvdp"] + f2["gesvd"] - f1["gesvdp"] - f1["gesvd"] >= f1["jacobi_mid_kernel"] - f0["jacobi_mid_kernel"]
+    worst = 0.0
+    for k in range(1, L):
+        assert ctx.mps_get_bond(a, k) == ctx.mps_get_bond(b, k), k
+        sa, sb = ctx.mps_get_svals(a, k), ctx.mps_get_svals(b, k)
+        assert sa.keys() == sb.keys()
+        smax = max(v.max() for v in sa.values())
+        for key in sa:
+            worst = max(worst, np.abs(sa[key] - sb[key]).max() / smax)
+    oa, ob = ctx.measure_local(a, L), ctx.measure_local(b, L)
+    dobs = max(np.abs(oa[key] - ob[key]).max() for key in ("n", "sz", "docc"))
+    print("mid-size Jacobi vs vendor: %d matrices, max |ds|/s_max = %.2e, max |obs diff| = %.2e"
+          % (f1["jacobi_mid_kernel"] - f0["jacobi_mid_kernel"], worst, dobs))
+    assert worst < 1e-11 and dobs < 1e-10, (worst, dobs)
+    for h in (mps, a, b):
+        ctx.mps_destroy(h)
 
 
 # ------------------------------------------------------------------ edge cases and errors
