@@ -193,6 +193,47 @@ void PlanCache::clear() {
 // ============================================================================ plan + apply
 static int last_tj_pos(int nsite) { return nsite == 2 ? 7 : (nsite == 1 ? 4 : 1); }
 
+// weighted inner-product chunks (F-6)
+static void fill_chunks(const BlockTensor& vec, int tpos, std::vector<VecChunk>& chunks) {
+  chunks.clear();
+  for (size_t i = 0; i < vec.keys.size(); ++i) {
+    const int64_t n = (int64_t)vec.rows[i] * vec.cols[i];
+    for (int64_t s = 0; s < n; s += 8192)
+      chunks.push_back(VecChunk{vec.off[i] + s, (int)std::min<int64_t>(8192, n - s), (float)(vec.keys[i][tpos] + 1)});
+  }
+}
+// host-only emission of the two-site plan at `site` (no CUDA calls: also runs on the prefetch thread)
+static void emit_plan2(const fh_mpo* mpo, const fh_mps* mps, int site, BlockTensor& vec, BlockTensor& Z, Stage& st1,
+                       Stage& st2, std::vector<VecChunk>& chunks) {
+  layout_theta(mps->bond[site], mps->bond[site + 2], vec);
+  emit_heff2(mps->Lenv[site], mps->Renv[site + 2], vec, mpo->site[site & 1], mpo->site[(site + 1) & 1], Z, st1, st2);
+  fill_chunks(vec, last_tj_pos(2), chunks);
+}
+void fh::prefetch_plan2(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site) {
+  prefetch_cancel(ctx);
+  static const bool off = [] {
+    const char* e = std::getenv("FH_NO_PREFETCH");  // A/B timing: emit every plan on the calling thread
+    return e && e[0] && e[0] != '0';
+  }();
+  if (off) return;
+  if (site < 0 || site + 2 > mps->L || mps->Lenv[site].base < 0 || mps->Renv[site + 2].base < 0) return;
+  PlanEmit* e = &ctx->prefetch;
+  e->site = site;
+  ctx->prefetch_job = std::async(std::launch::async, [mpo, mps, site, e]() {
+    e->Z.base = -1;
+    emit_plan2(mpo, mps, site, e->vec, e->Z, e->st1, e->st2, e->chunks);
+  });
+  ctx->prefetch_pending = true;
+}
+void fh::prefetch_cancel(fh_ctx* ctx) {
+  if (!ctx->prefetch_pending) return;
+  ctx->prefetch_pending = false;
+  try {
+    ctx->prefetch_job.get();
+  } catch (...) {
+  }
+}
+
 void fh::plan_heff(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, int nsite) {
   FH_REQUIRE(nsite == 1 || nsite == 2, FH_EINVAL, "heff_plan: nsite must be 1 or 2");
   FH_REQUIRE(site >= 0 && site + nsite <= mps->L, FH_EINVAL, "heff_plan: site out of range");
@@ -216,7 +257,22 @@ void fh::plan_heff(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, 
     sig_add(sig, mpo->U);
     hit = mps->cache.find(PC_HEFF1, site, sig);
   }
-  if (hit) {
+  bool prefetched = false;
+  if (nsite == 2 && ctx->prefetch_pending) {
+    ctx->prefetch_pending = false;
+    ctx->prefetch_job.get();  // rethrows what the emitter threw
+    if (ctx->prefetch.site == site) {
+      P.vec = std::move(ctx->prefetch.vec);
+      P.Z = std::move(ctx->prefetch.Z);
+      P.st1 = std::move(ctx->prefetch.st1);
+      P.st2 = std::move(ctx->prefetch.st2);
+      P.chunks = std::move(ctx->prefetch.chunks);
+      prefetched = true;
+      ++ctx->prefetch_used;
+    }
+  }
+  if (prefetched) {
+  } else if (hit) {
     P.vec = hit->t0;
     P.Z = hit->t1;
     P.st1 = hit->st1;
@@ -224,19 +280,11 @@ void fh::plan_heff(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, 
     P.chunks = hit->chunks;
   } else {
     if (nsite == 2) {
-      layout_theta(mps->bond[site], mps->bond[site + 2], P.vec);
-      emit_heff2(Le, Re, P.vec, mpo->site[site & 1], mpo->site[(site + 1) & 1], P.Z, P.st1, P.st2);
+      emit_plan2(mpo, mps, site, P.vec, P.Z, P.st1, P.st2, P.chunks);
     } else {
       layout_site(mps->bond[site], mps->bond[site + 1], P.vec);
       emit_heff1(Le, Re, P.vec, mpo->site[site & 1], P.Z, P.st1, P.st2);
-    }
-    // weighted inner-product chunks (F-6)
-    P.chunks.clear();
-    const int tpos = last_tj_pos(nsite);
-    for (size_t i = 0; i < P.vec.keys.size(); ++i) {
-      const int64_t n = (int64_t)P.vec.rows[i] * P.vec.cols[i];
-      for (int64_t s = 0; s < n; s += 8192)
-        P.chunks.push_back(VecChunk{P.vec.off[i] + s, (int)std::min<int64_t>(8192, n - s), (float)(P.vec.keys[i][tpos] + 1)});
+      fill_chunks(P.vec, last_tj_pos(nsite), P.chunks);
     }
     if (use_cache) {
       if (PlanCacheEntry* e = mps->cache.store(PC_HEFF1, site, std::move(sig))) {
@@ -561,6 +609,7 @@ int fh_ctx_create(fh_ctx** out, void* cuda_stream, void* arena_dev, size_t arena
 
 void fh_ctx_destroy(fh_ctx* c) {
   if (!c) return;
+  fh::prefetch_cancel(c);
   cudaStreamSynchronize(c->stream);
   for (auto& sp : c->spans) {
     cudaEventDestroy(sp.a);

@@ -2,6 +2,7 @@
 #pragma once
 #include <cusolverDn.h>
 
+#include <future>
 #include <stdexcept>
 
 #include "fh_b200.h"
@@ -66,6 +67,16 @@ struct Plan {
   DevPool pool;
 };
 
+// What the emitter produces for one two-site plan; filled by a second host thread while the main thread runs
+// the backward one-site step of the bond before (tdvp.cu, sweep): the emission of the next plan needs only the
+// bond tables and environment layouts, which are final once the environment update has been emitted.
+struct PlanEmit {
+  int site = -1;
+  BlockTensor vec, Z;
+  Stage st1, st2;
+  std::vector<VecChunk> chunks;
+};
+
 enum { T_HEFF = 0, T_ENV = 1, T_SVD = 2, T_VEC = 3, T_PACK = 4, T_NCAT = 5 };
 
 // Task-list cache of the one-site sweeps (H0).  One-site TDVP leaves the sector tables of every bond as they
@@ -120,6 +131,10 @@ struct fh_ctx {
   fh::Arena alloc;
   std::string err;
   fh::Plan plan;
+  fh::PlanEmit prefetch;           // next two-site plan, emitted ahead (see PlanEmit)
+  std::future<void> prefetch_job;
+  bool prefetch_pending = false;
+  int64_t prefetch_used = 0;
   fh::DevPool pool_aux;  // env updates, merge, pack, measure
   fh::DevPool pool_small;  // descriptors of the small-matrix SVD kernel
   int64_t launches = 0;
@@ -189,6 +204,11 @@ void upload_stage(DevPool& pool, Stage& st, cudaStream_t s);
 
 // engine pieces (api.cu / tdvp.cu)
 void plan_heff(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, int nsite);
+// starts the emission of the two-site plan at `site` on another host thread (no CUDA calls there); the next
+// plan_heff(site, 2) takes it over.  The caller must not change the bond tables or environment layouts the
+// plan reads before that; prefetch_cancel waits for a job still in flight and drops its result.
+void prefetch_plan2(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site);
+void prefetch_cancel(fh_ctx* ctx);
 void apply_heff(fh_ctx* ctx, const cplx* theta, cplx* out);
 double2 inner(fh_ctx* ctx, const cplx* x, const cplx* y);  // synchronises
 // returns the number of Krylov vectors used; adapt_tol > 0 enables the adaptive stop (reading A-15)

@@ -1298,16 +1298,30 @@ void fh::sweep(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh_
   ctx->stat_disc = 0.0;
   ctx->stat_chi = ctx->stat_su2 = ctx->stat_dmax = 0;
   const double tau = 0.5 * dt;
-  for (int i = 0; i < L - 1; ++i) {  // left -> right
-    local_update2(ctx, mpo, mps, i, tau, +1, prm);
-    do_env_update_left(ctx, mpo, mps, i);
-    if (i < L - 2) local_update1(ctx, mpo, mps, i + 1, -tau, prm);
+  // The task lists of the next two-site plan are emitted on a second host thread while this one runs the
+  // backward one-site step: after the environment update every table and layout that plan reads is final.
+  try {
+    for (int i = 0; i < L - 1; ++i) {  // left -> right
+      local_update2(ctx, mpo, mps, i, tau, +1, prm);
+      do_env_update_left(ctx, mpo, mps, i);
+      if (i < L - 2) {
+        prefetch_plan2(ctx, mpo, mps, i + 1);
+        local_update1(ctx, mpo, mps, i + 1, -tau, prm);
+      }
+    }
+    for (int i = L - 2; i >= 0; --i) {  // right -> left
+      local_update2(ctx, mpo, mps, i, tau, -1, prm);
+      do_env_update_right(ctx, mpo, mps, i + 1);
+      if (i > 0) {
+        prefetch_plan2(ctx, mpo, mps, i - 1);
+        local_update1(ctx, mpo, mps, i, -tau, prm);
+      }
+    }
+  } catch (...) {
+    prefetch_cancel(ctx);  // the job reads the state: it must be over before the caller may destroy it
+    throw;
   }
-  for (int i = L - 2; i >= 0; --i) {  // right -> left
-    local_update2(ctx, mpo, mps, i, tau, -1, prm);
-    do_env_update_right(ctx, mpo, mps, i + 1);
-    if (i > 0) local_update1(ctx, mpo, mps, i, -tau, prm);
-  }
+  prefetch_cancel(ctx);
 }
 
 // H10: left norm environments N_{i+1}[c] = sum_{a,s} A^H N_i[a] A;  <O_i> = sum (2j_c+1) red(O)[s] Re Tr(A^H N A)
