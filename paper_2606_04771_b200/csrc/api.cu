@@ -406,15 +406,28 @@ int fh::expm_lanczos(fh_ctx* ctx, cplx* theta, double tau, int m, double tol, cp
   if (n == 0 || P.chunks.empty()) return 0;
   cudaStream_t s = ctx->stream;
   const int nch = (int)P.chunks.size();
-  // device scalars: [0,1] <theta,theta>, then per j: alpha pair at 2 + 4j, <w,w> pair at 4 + 4j; betas after
+  // device scalars: [0,1] <theta,theta>, then per j: a_raw_j = <u_j, H u_j> at 2 + 4j, <u_{j+1}, u_{j+1}> at 4 + 4j.
+  // The Krylov vectors are kept unnormalised, u_j = b_j v_j with b_0 = 1 and b_j = beta_{j-1} (kernels.cu,
+  // lanczos_update_kernel): alpha_j = a_raw_j / b_j^2, beta_j = sqrt(<u_{j+1}, u_{j+1}>), and the final linear
+  // combination takes c_j / b_j.
   double* d_sc = P.d_scal;
-  double* d_beta = P.d_scal + 2 + 4 * 32;
   const int nsc = 2 + 4 * 32 + 32;
   ctx->ensure_pinned(nsc);
   auto fetch_scalars = [&]() {
     FH_CUDA(cudaMemcpyAsync(ctx->h_pinned, d_sc, nsc * sizeof(double), cudaMemcpyDeviceToHost, s));
     FH_CUDA(cudaStreamSynchronize(s));
   };
+  // reciprocal of b_j as the kernel takes it (0 below tol) from the fetched scalars
+  auto recip_b = [&](int j) {
+    if (j == 0) return 1.0;
+    const double b = std::sqrt(std::max(ctx->h_pinned[4 + 4 * (j - 1)], 0.0));
+    return (b < tol || b == 0.0) ? 0.0 : 1.0 / b;
+  };
+  auto alpha_of = [&](int j) {
+    const double f = recip_b(j);
+    return ctx->h_pinned[2 + 4 * j] * f * f;
+  };
+  auto beta_of = [&](int j) { return std::sqrt(std::max(ctx->h_pinned[4 + 4 * j], 0.0)); };
   ctx->timer_begin(T_VEC);
   launch_wdot_fused(P.d_chunks, nch, theta, theta, P.d_partial, d_sc, P.d_counter, s, &ctx->launches);
   launch_scale_rsqrt_dev(n, d_sc, 0.0, theta, V, nullptr, s, &ctx->launches);
@@ -429,16 +442,15 @@ int fh::expm_lanczos(fh_ctx* ctx, cplx* theta, double tau, int m, double tol, cp
     ctx->timer_end();
     ctx->timer_begin(T_VEC);
     launch_wdot_fused(P.d_chunks, nch, vj, w, P.d_partial, d_sc + 2 + 4 * j, P.d_counter, s, &ctx->launches);
-    launch_lanczos_update(P.d_chunks, nch, d_sc + 2 + 4 * j, j > 0 ? d_beta + (j - 1) : nullptr, vj,
-                          j > 0 ? V + (int64_t)(j - 1) * n : nullptr, w, P.d_partial, d_sc + 4 + 4 * j, P.d_counter, s,
-                          &ctx->launches);
-    if (j < m - 1) launch_scale_rsqrt_dev(n, d_sc + 4 + 4 * j, tol, w, w, d_beta + j, s, &ctx->launches);
+    launch_lanczos_update(P.d_chunks, nch, d_sc + 2 + 4 * j, j > 0 ? d_sc + 4 + 4 * (j - 1) : nullptr,
+                          j > 1 ? d_sc + 4 + 4 * (j - 2) : nullptr, tol, vj, j > 0 ? V + (int64_t)(j - 1) * n : nullptr, w,
+                          P.d_partial, d_sc + 4 + 4 * j, P.d_counter, s, &ctx->launches);
     ctx->timer_end();
     if (adapt_tol > 0.0 && j < m - 1) {
       fetch_scalars();
       if (!(ctx->h_pinned[0] > 0.0)) return 0;  // zero vector
-      alpha.push_back(ctx->h_pinned[2 + 4 * j]);
-      const double bj = ctx->h_pinned[2 + 4 * 32 + j];
+      alpha.push_back(alpha_of(j));
+      const double bj = beta_of(j);
       if (bj < tol) {
         k = j + 1;
         break;
@@ -457,10 +469,10 @@ int fh::expm_lanczos(fh_ctx* ctx, cplx* theta, double tau, int m, double tol, cp
     alpha.clear();
     beta.clear();
     for (int j = 0; j < m; ++j) {
-      alpha.push_back(ctx->h_pinned[2 + 4 * j]);
+      alpha.push_back(alpha_of(j));
       k = j + 1;
       if (j == m - 1) break;
-      const double bj = ctx->h_pinned[2 + 4 * 32 + j];
+      const double bj = beta_of(j);
       if (bj < tol) break;
       beta.push_back(bj);
     }
@@ -469,7 +481,10 @@ int fh::expm_lanczos(fh_ctx* ctx, cplx* theta, double tau, int m, double tol, cp
   if (!(nrm2 > 0.0)) return 0;  // zero vector: theta is untouched (V holds zeros)
   const double nrm = std::sqrt(nrm2);
   std::vector<cplx> c = tridiag_exp_col(alpha, beta, k, tau);
-  for (auto& ci : c) ci = make_double2(nrm * ci.x, nrm * ci.y);
+  for (int j = 0; j < k; ++j) {  // v_j = u_j / b_j
+    const double g = nrm * recip_b(j);
+    c[j] = make_double2(g * c[j].x, g * c[j].y);
+  }
   ctx->timer_begin(T_VEC);
   launch_lincomb(n, k, c.data(), V, n, theta, s, &ctx->launches);
   ctx->timer_end();
@@ -1345,8 +1360,8 @@ int fh_vec_kernels_gbs(fh_ctx* ctx, int64_t n, int m, int reps, double* gbs) {
           switch (k) {
             case 0: launch_wdot_fused(d_ch, (int)ch.size(), x, y, d_part, d_res, d_cnt, s, &ctx->launches); break;
             case 6:  // coefficients (d_res[2], d_res[3]) stay zero: the operands do not grow over the repetitions
-              launch_lanczos_update(d_ch, (int)ch.size(), d_res + 2, d_res + 3, x, y, z, d_part, d_res + 4, d_cnt, s,
-                                    &ctx->launches);
+              launch_lanczos_update(d_ch, (int)ch.size(), d_res + 2, d_res + 3, nullptr, 0.0, x, y, z, d_part, d_res + 4,
+                                    d_cnt, s, &ctx->launches);
               break;
             case 1: launch_axpy(n, make_double2(0.5, 0.1), x, y, s, &ctx->launches); break;
             case 2: launch_scale(n, make_double2(0.5, 0.1), x, z, s, &ctx->launches); break;

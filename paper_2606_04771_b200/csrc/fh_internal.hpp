@@ -182,9 +182,9 @@ void launch_scale(int64_t n, cplx a, const cplx* x, cplx* y, cudaStream_t s, int
 // one-launch forms for the Lanczos recurrence: d_counter is a zero-initialised unsigned that the kernels leave at zero
 void launch_wdot_fused(const VecChunk* d_chunks, int nchunks, const cplx* x, const cplx* y, double* d_partial,
                        double* d_result, unsigned* d_counter, cudaStream_t s, int64_t* lc);
-void launch_lanczos_update(const VecChunk* d_chunks, int nchunks, const double* d_alpha, const double* d_beta_prev,
-                           const cplx* vj, const cplx* vprev, cplx* w, double* d_partial, double* d_result,
-                           unsigned* d_counter, cudaStream_t s, int64_t* lc);
+void launch_lanczos_update(const VecChunk* d_chunks, int nchunks, const double* d_a_raw, const double* d_bj2,
+                           const double* d_bjm2, double tol, const cplx* vj, const cplx* vprev, cplx* w,
+                           double* d_partial, double* d_result, unsigned* d_counter, cudaStream_t s, int64_t* lc);
 void launch_scale_rsqrt_dev(int64_t n, const double* d_norm2, double tol, const cplx* x, cplx* y, double* d_beta,
                             cudaStream_t s, int64_t* lc);
 void launch_lincomb(int64_t n, int m, const cplx* coef_host, const cplx* V, int64_t stride, cplx* y,

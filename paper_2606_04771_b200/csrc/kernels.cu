@@ -145,20 +145,38 @@ __global__ void __launch_bounds__(256) wdot_fused_kernel(const VecChunk* __restr
   finish_in_last_cta(partial, gridDim.x, result, counter);
 }
 
-// Lanczos three-term update and the norm of its result in one launch:
-//   w -= alpha[0] v_j (+ beta_prev[0] v_prev);   result = <w, w> (weighted, F-6)
-// The two subtractions keep the order (and rounding) of two separate axpy passes (alpha first, then beta).
+// Lanczos three-term update on UNNORMALISED Krylov vectors, and the norm of its result, in one launch.
+// The recurrence keeps u_j = b_j v_j (b_0 = 1, b_j = beta_{j-1} = |u_j|) instead of v_j, so that no separate
+// normalisation pass is needed:  with w = H u_j and a_raw = <u_j, w>,
+//   alpha_j = a_raw / b_j^2,   u_{j+1} = (w - alpha_j u_j) / b_j - (b_j / b_{j-1}) u_{j-1},   result = <u_{j+1}, u_{j+1}>
+// (= beta_j^2).  b_j^2 and b_{j-1}^2 are the results of the two previous updates (NULL = 1).  A norm below tol
+// (happy breakdown) makes its reciprocal 0, as the normalisation pass did: everything stays finite and the host
+// truncates the Krylov space there.
 __global__ void __launch_bounds__(256) lanczos_update_kernel(const VecChunk* __restrict__ chunks,
-                                                             const double* __restrict__ alpha,
-                                                             const double* __restrict__ beta_prev,
+                                                             const double* __restrict__ a_raw,
+                                                             const double* __restrict__ bj2,
+                                                             const double* __restrict__ bjm2, double tol,
                                                              const cplx* __restrict__ vj, const cplx* __restrict__ vprev,
                                                              cplx* __restrict__ w, double* __restrict__ partial,
                                                              double* __restrict__ result, unsigned* __restrict__ counter) {
   pdl_launch_dependents();
   const VecChunk ch = chunks[blockIdx.x];
   pdl_wait();
-  const double a = -alpha[0];
-  const double b = beta_prev ? -beta_prev[0] : 0.0;
+  double bj = 1.0, f = 1.0;
+  if (bj2) {
+    bj = sqrt(fmax(bj2[0], 0.0));
+    f = (bj < tol || bj == 0.0) ? 0.0 : 1.0 / bj;
+  }
+  const double a = -(a_raw[0] * f * f) * f;
+  double b = 0.0;
+  if (vprev) {
+    double fm = 1.0;
+    if (bjm2) {
+      const double bm = sqrt(fmax(bjm2[0], 0.0));
+      fm = (bm < tol || bm == 0.0) ? 0.0 : 1.0 / bm;
+    }
+    b = -bj * fm;
+  }
   const cplx* pv = vj + ch.start;
   const cplx* pp = vprev ? vprev + ch.start : nullptr;
   cplx* pw = w + ch.start;
@@ -166,8 +184,8 @@ __global__ void __launch_bounds__(256) lanczos_update_kernel(const VecChunk* __r
   for (int i = threadIdx.x; i < ch.len; i += 256) {
     const cplx xv = pv[i];
     cplx v = pw[i];
-    v.x += a * xv.x;
-    v.y += a * xv.y;
+    v.x = f * v.x + a * xv.x;
+    v.y = f * v.y + a * xv.y;
     if (pp) {
       const cplx yv = pp[i];
       v.x += b * yv.x;
@@ -195,11 +213,11 @@ void launch_wdot_fused(const VecChunk* d_chunks, int nchunks, const cplx* x, con
   launch_pdl(PDL_WDOT, wdot_fused_kernel, nchunks, 256, s, d_chunks, x, y, d_partial, d_result, d_counter);
   ++*lc;
 }
-void launch_lanczos_update(const VecChunk* d_chunks, int nchunks, const double* d_alpha, const double* d_beta_prev,
-                           const cplx* vj, const cplx* vprev, cplx* w, double* d_partial, double* d_result,
-                           unsigned* d_counter, cudaStream_t s, int64_t* lc) {
-  launch_pdl(PDL_UPDATE, lanczos_update_kernel, nchunks, 256, s, d_chunks, d_alpha, d_beta_prev, vj, vprev, w, d_partial, d_result,
-             d_counter);
+void launch_lanczos_update(const VecChunk* d_chunks, int nchunks, const double* d_a_raw, const double* d_bj2,
+                           const double* d_bjm2, double tol, const cplx* vj, const cplx* vprev, cplx* w,
+                           double* d_partial, double* d_result, unsigned* d_counter, cudaStream_t s, int64_t* lc) {
+  launch_pdl(PDL_UPDATE, lanczos_update_kernel, nchunks, 256, s, d_chunks, d_a_raw, d_bj2, d_bjm2, tol, vj, vprev, w,
+             d_partial, d_result, d_counter);
   ++*lc;
 }
 
