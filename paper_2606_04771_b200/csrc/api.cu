@@ -196,10 +196,11 @@ static int last_tj_pos(int nsite) { return nsite == 2 ? 7 : (nsite == 1 ? 4 : 1)
 // weighted inner-product chunks (F-6)
 static void fill_chunks(const BlockTensor& vec, int tpos, std::vector<VecChunk>& chunks) {
   chunks.clear();
+  const int cl = vec_chunk_len(vec.nelem);
   for (size_t i = 0; i < vec.keys.size(); ++i) {
     const int64_t n = (int64_t)vec.rows[i] * vec.cols[i];
-    for (int64_t s = 0; s < n; s += 8192)
-      chunks.push_back(VecChunk{vec.off[i] + s, (int)std::min<int64_t>(8192, n - s), (float)(vec.keys[i][tpos] + 1)});
+    for (int64_t s = 0; s < n; s += cl)
+      chunks.push_back(VecChunk{vec.off[i] + s, (int)std::min<int64_t>(cl, n - s), (float)(vec.keys[i][tpos] + 1)});
   }
 }
 // host-only emission of the two-site plan at `site` (no CUDA calls: also runs on the prefetch thread)

@@ -3,6 +3,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdlib.h>
 
 #include <array>
 #include <map>
@@ -129,6 +130,19 @@ struct VecChunk {
   int len;
   float w;  // 2j+1, small integer: exact in float
 };
+
+// Chunk length of the Lanczos vectors.  A chunk is one 256-thread CTA; a long chunk is a long chain of L2 round
+// trips per thread (8192 elements = 32 loads), which is what a vector kernel on an L2-resident vector of a few
+// MB waits for, so vectors up to 1 Mi elements get 1024-element chunks, up to 4 Mi 2048; HBM-sized vectors keep 8192 (fewer CTAs
+// and partials).  One-site sweep at chi = 4096: 0.393 / 0.375 / 0.369 / 0.362 / 0.358 s with 8192 / 4096 / 2048 / 1024 / 512.
+inline int vec_chunk_len(int64_t nelem) {
+  static const int forced = [] {
+    const char* e = getenv("FH_VEC_CHUNK");  // A/B timing only
+    return e && e[0] ? atoi(e) : 0;
+  }();
+  if (forced >= 256) return forced;
+  return nelem > ((int64_t)4 << 20) ? 8192 : (nelem > ((int64_t)1 << 20) ? 2048 : 1024);
+}
 
 // pack / unpack copy descriptors (H8, H9)
 struct CopyBlk {

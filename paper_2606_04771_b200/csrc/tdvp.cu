@@ -1016,10 +1016,11 @@ static void plan_zero_site(fh_ctx* ctx, fh_mps* mps, int bond, const BlockTensor
   } else {
     emit_heff0(Le, Re, P.vec, P.Z, P.st1, P.st2);
     P.chunks.clear();
+    const int cl = vec_chunk_len(P.vec.nelem);
     for (size_t i = 0; i < P.vec.keys.size(); ++i) {
       const int64_t n = (int64_t)P.vec.rows[i] * P.vec.cols[i];
-      for (int64_t st = 0; st < n; st += 8192)
-        P.chunks.push_back(VecChunk{P.vec.off[i] + st, (int)std::min<int64_t>(8192, n - st), (float)(P.vec.keys[i][1] + 1)});
+      for (int64_t st = 0; st < n; st += cl)
+        P.chunks.push_back(VecChunk{P.vec.off[i] + st, (int)std::min<int64_t>(cl, n - st), (float)(P.vec.keys[i][1] + 1)});
     }
     if (mps->cache.enabled) {
       if (PlanCacheEntry* e = mps->cache.store(PC_HEFF0, bond, std::move(sig))) {
