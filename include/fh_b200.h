@@ -144,7 +144,7 @@ int heff_expm_adaptive(fh_ctx* ctx, const void* theta_dev, void* out_dev, double
  * (n < 48, or redo of [3]), [3] gesvdp results rejected because it reported a perturbed spectrum,
  * [4] Householder QR by cusolverDnZgeqrf + Zungqr (one-site splits that do not fit shared memory), [5] Householder
  * QR by the library's own shared-memory kernel, [6] own global-memory Jacobi kernel (matrices above the
- * shared-memory route with at most 120 columns; it runs on a side stream beside the vendor routines). */
+ * shared-memory route with at most 128 columns; it runs on a side stream beside the vendor routines). */
 int fh_factorization_stats(const fh_ctx* ctx, int64_t counts[7]);
 /* Task-list cache of the one-site sweeps (H0).  One-site TDVP keeps every bond's sector table
  * (no SVD, bond dimension fixed), so tdvp1_sweep / tdvp_sweep_auto keep the task lists they emit in

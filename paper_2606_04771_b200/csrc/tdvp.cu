@@ -189,7 +189,7 @@ __global__ void __launch_bounds__(32 * SMALL_SVD_MAX_WARPS) small_svd_kernel(con
 }
 
 // ------------------------------------------------------------------------------------------
-// Mid-size sector matrices (too large for small_svd_kernel, n <= 120 by default, FH_SVD_MID_MAXN): the same one-sided Jacobi, one
+// Mid-size sector matrices (too large for small_svd_kernel, n <= 128 by default, FH_SVD_MID_MAXN): the same one-sided Jacobi, one
 // 32-warp CTA per matrix, working IN PLACE on B in global memory with V in arena scratch.  A matrix of this size
 // (B and V together 0.3-0.7 MB) stays in the L1/L2 of its SM, and all accesses of a column pair come from one
 // warp, with __syncthreads between tournament rounds, so plain loads and stores are coherent.  It is slower per
@@ -542,7 +542,9 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
   // FH_SVD_MID_MAXN (read at every call, so that a test can compare the two routes in one process): 0 sends
   // every matrix above the shared-memory route to cuSOLVER
   const char* mid_env = std::getenv("FH_SVD_MID_MAXN");
-  const int mid_maxn = std::max(0, std::min(mid_env && mid_env[0] ? std::atoi(mid_env) : 120, MID_SVD_HARD_MAXN));
+  // default 128: 64 column pairs per tournament round = two per warp of the 32-warp CTA
+  const int mid_req = mid_env && mid_env[0] ? std::atoi(mid_env) : 128;
+  const int mid_maxn = std::max(0, std::min(mid_req, MID_SVD_HARD_MAXN));
   const double mid_work = 1.5 * mid_maxn * (double)mid_maxn * mid_maxn;  // m n^2 bound: a long thin matrix would make its one CTA the critical path
   static const bool use_small_qr = [] {
     const char* e = std::getenv("FH_SMALL_QR");  // "0" sends every one-site split to cuSOLVER

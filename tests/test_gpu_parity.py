@@ -636,7 +636,7 @@ def test_quench_L24_large_sectors_invariants(H, ctx):
     g2, o2 = check("end of two-site phase", 1e-5)
     f1 = ctx.fh_factorization_stats()
     assert st["chi_full"] > 300 and st["dmax"] >= 24, st
-    # the routes above the shared-memory kernel really ran (own global-memory Jacobi up to 120 columns, vendor beyond)
+    # the routes above the shared-memory kernel really ran (own global-memory Jacobi up to 128 columns, vendor beyond)
     assert f1["gesvdp"] + f1["jacobi_mid_kernel"] - f0["gesvdp"] - f0["jacobi_mid_kernel"] > 0, f1
     assert f1["jacobi_kernel"] - f0["jacobi_kernel"] > 0, f1
     dims_before = [ctx.mps_get_bond(mps, k) for k in range(L + 1)]
@@ -654,9 +654,9 @@ def test_quench_L24_large_sectors_invariants(H, ctx):
 
 
 def test_mid_size_jacobi_kernel_vs_vendor_svd(H, ctx, tmp_path):
-    """H9: sector matrices above the shared-memory route with at most 120 columns are factorised by the library's
+    """H9: sector matrices above the shared-memory route with at most 128 columns are factorised by the library's
     own global-memory Jacobi kernel (mid_svd_kernel, on a side stream beside the vendor routines).  The same L = 16
-    state (grown by an untruncated quench until sector matrices of 90-120 columns exist) takes one two-site sweep
+    state (grown by an untruncated quench until sector matrices of 90-128 columns exist) takes one two-site sweep
     with that kernel and, from a reloaded copy, one with FH_SVD_MID_MAXN=0 (every such matrix through cusolver's
     gesvdp / gesvd): both routes must have run, the kept singular values of every bond agree to 1e-11 s_max, the
     sector tables are identical and the observables agree to 1e-10."""
