@@ -180,12 +180,13 @@ static void emit_units(Stage& st) {
   // Small stages (one-site and zero-site applies, environment updates at chi = 4096: well under a million DMMAs)
   // want smaller units still: a unit should not be longer than the fair share of one of the 1184 warp slots,
   // else the stage lasts as long as its few heaviest units (one-site apply at chi = 4096: 82 -> 71 us with the
-  // cap lowered from 3072 to 1024, while the two-site apply, 4.1e6 DMMAs per stage, is fastest at 3072).
+  // cap lowered from 3072 to 1024, the chi = 1024 apply 61 -> 32 us with 256, while the two-site apply at chi = 4096,
+  // 4.1e6 DMMAs per stage, is fastest at 3072).
   static const int64_t cap_floor = [] {
     const char* e = getenv("FH_UNIT_CAP_FLOOR");  // A/B timing only
-    return (int64_t)(e && e[0] ? atoi(e) : 1024);
+    return (int64_t)(e && e[0] ? atoi(e) : 256);
   }();
-  const int64_t fair = total16 / (148 * 8);
+  const int64_t fair = 2 * (total16 / (148 * 8));  // twice the even share: measured best at chi = 1024, 4096 (one- and two-site)
   const int64_t base_cap = std::min<int64_t>(GEMM_UNIT_DMMA_CAP, std::max<int64_t>(cap_floor, fair));
   const int64_t cap = std::max<int64_t>(base_cap, total16 / (148 * 8 * 6));
   for (size_t oi = 0; oi < st.outs.size(); ++oi) {
