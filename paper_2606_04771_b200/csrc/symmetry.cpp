@@ -187,7 +187,12 @@ static void emit_units(Stage& st) {
     return (int64_t)(e && e[0] ? atoi(e) : 256);
   }();
   const int64_t fair = 2 * (total16 / (148 * 8));  // twice the even share: measured best at chi = 1024, 4096 (one- and two-site)
-  const int64_t base_cap = std::min<int64_t>(GEMM_UNIT_DMMA_CAP, std::max<int64_t>(cap_floor, fair));
+  static const int64_t forced_cap = [] {
+    const char* e = getenv("FH_UNIT_CAP");  // A/B timing only: a fixed base cap instead of the fair-share rule
+    return (int64_t)(e && e[0] ? atoi(e) : 0);
+  }();
+  const int64_t base_cap =
+      forced_cap > 0 ? forced_cap : std::min<int64_t>(GEMM_UNIT_DMMA_CAP, std::max<int64_t>(cap_floor, fair));
   const int64_t cap = std::max<int64_t>(base_cap, total16 / (148 * 8 * 6));
   for (size_t oi = 0; oi < st.outs.size(); ++oi) {
     const GemmOut& o = st.outs[oi];
