@@ -240,7 +240,8 @@ def run_ours(args):
     th = fi.theta_random(fi.SEED, c, dims[c], dims[c + 2])
     x_host = torch.from_numpy(H.flatten(th, lab, dm, H.theta_key)).pin_memory()
     y_host = torch.empty_like(x_host).pin_memory()
-    x = x_host.cuda()
+    x = torch.empty_like(x_host, device="cuda:%d" % local)
+    ctx.heff_import(x_host.cuda(), x)       # interchange format -> the library's planned layout, once
     y = torch.empty_like(x)
     flops = ctx.heff_flops()
     t1, _, nz = ctx.heff_get_tasks(1)

@@ -20,6 +20,7 @@
  *     environments  L[a',w,a]           d_a' x d_a ,  R[b',w,b]  d_b' x d_b
  *   blocks of one tensor are stored contiguously in the canonical (lexicographic, sectors
  *   ordered by (q, tj)) order of their label tuples; "planned block order" below means that.
+ *   (The vectors heff_apply works on have a layout of their own: see heff_import / heff_export.)
  *
  * Pointer arguments are HOST pointers unless the name ends in _dev.
  */
@@ -115,22 +116,34 @@ int env_set(fh_ctx* ctx, fh_mps* mps, int which, int bond, int nblk, const int32
  * sorts them canonically, builds the tile queue and uploads everything.  It uses L_site and
  * R_{site+nsite} stored in the MPS. */
 int heff_plan(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, int nsite);
-/* block layout of the planned vector: nsite=2: labels[nblk][8] = (qa,tja,s1,qc,tjc,s2,qb,tjb);
- * nsite=1: labels[nblk][5].  dims[nblk][2]. */
+/* Interchange format of the vector H_eff acts on: nsite=2: labels[nblk][8] = (qa,tja,s1,qc,tjc,s2,qb,tjb);
+ * nsite=1: labels[nblk][5].  dims[nblk][2].  The blocks in this (canonical) order, each dense row-major, one
+ * after the other, plain tensor entries: nelem complex128 in all. */
 int heff_layout(const fh_ctx* ctx, int* nblk, int64_t* nelem, int32_t* labels, int32_t* dims);
 /* host copy of a task list, stage = 1 or 2: tuples[ntask][3] = (out_id, lhs_id, rhs_id), ids =
  * positions in canonical block order (stage 1: Z, L, theta; stage 2: out, Z, R); alpha[ntask].
- * Pass tuples = alpha = NULL to query ntask (and nout = number of output blocks). */
+ * Pass tuples = alpha = NULL to query ntask (and nout = number of output blocks).  An intermediate block
+ * that no stage-2 task reads is not part of the lists (reading A-17). */
 int heff_get_tasks(const fh_ctx* ctx, int stage, int* ntask, int* nout, int32_t* tuples, double* alpha);
-/* out_dev = H_eff * theta_dev; both device vectors of heff_layout's nelem complex128. */
+/* Planned vectors.  heff_apply / heff_inner / heff_expm work on device vectors of heff_layout's nelem
+ * complex128 in the library's PLANNED layout, which is opaque: for nsite = 2 the blocks that share the middle
+ * label c form one row-major matrix theta_c[(a,s1,alpha),(s2,b,beta)] (the matrix the SVD split factorises,
+ * PAPER.md:250; a whole row panel is then one GEMM operand) and every entry carries the factor sqrt(2 j_b + 1),
+ * which turns the multiplet-weighted inner product F-6 into the plain Euclidean one; for nsite = 1 it equals
+ * the interchange format.  heff_import / heff_export convert on the device (one scaled block-copy kernel,
+ * H8 type); source and destination must not overlap. */
+int heff_import(fh_ctx* ctx, const void* blocks_dev, void* vec_dev);
+int heff_export(fh_ctx* ctx, const void* vec_dev, void* blocks_dev);
+/* out_dev = H_eff * theta_dev; both planned device vectors. */
 int heff_apply(fh_ctx* ctx, const void* theta_dev, void* out_dev);
-/* Same operation with HOST buffers (pageable or pinned) of heff_layout's nelem complex128:
- * copies theta to the device, applies, copies the result back and synchronises the stream.
- * This is the end-to-end entry a caller without device memory uses. */
+/* Same operation with HOST buffers (pageable or pinned) of heff_layout's nelem complex128 in the INTERCHANGE
+ * format: copies theta to the device, imports, applies, exports, copies the result back and synchronises
+ * the stream.  This is the end-to-end entry a caller without device memory uses. */
 int heff_apply_host(fh_ctx* ctx, const void* theta_host, void* out_host);
 /* sum over both task lists of 8*m*n*k */
 int64_t heff_flops(const fh_ctx* ctx);
-/* <x,y> = sum_blocks (2 j_b + 1) sum conj(x) y  (F-6) over the planned layout; result[2] = re,im */
+/* <x,y> of two planned vectors = sum_blocks (2 j_b + 1) sum conj(x) y of the tensors they hold (F-6);
+ * result[2] = re,im */
 int heff_inner(fh_ctx* ctx, const void* x_dev, const void* y_dev, double* result);
 /* out_dev = exp(-i tau H_eff) theta_dev by an m-vector Lanczos process (H6, H7) */
 int heff_expm(fh_ctx* ctx, const void* theta_dev, void* out_dev, double tau, int krylov_dim);

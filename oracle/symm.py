@@ -358,6 +358,11 @@ def heff2_tasks(L_keys, R_keys, th_keys, W1, W2):
                 st2.setdefault(okey, []).append((zkey, rk, al))
     for o in st2:
         st2[o].sort(key=lambda t: (t[0][4], t[0][5], t[0][6], t[0][3], t[1][1]))
+    # Reading A-17: an intermediate block Z[a',s1',c',w_m; c,s2,b] that no term of H2 reads
+    # (W_{i+1}[w_m, w_r; s2', s2] vanishes for every (w_r, s2'), e.g. w_m = P with s2 = down) contributes
+    # nothing to H_eff theta; it is not formed and its tasks are not part of the list (nor of the flop count).
+    used = {seg[0] for segs in st2.values() for seg in segs}
+    st1 = {z: segs for z, segs in st1.items() if z in used}
     return st1, dict(sorted(st2.items()))
 
 

@@ -57,6 +57,8 @@ _SIGS = {
     "heff_layout": (c_int, [c_void_p, P(c_int), P(c_i64), c_void_p, c_void_p]),
     "heff_get_tasks": (c_int, [c_void_p, c_int, P(c_int), P(c_int), c_void_p, c_void_p]),
     "heff_apply": (c_int, [c_void_p, c_void_p, c_void_p]),
+    "heff_import": (c_int, [c_void_p, c_void_p, c_void_p]),
+    "heff_export": (c_int, [c_void_p, c_void_p, c_void_p]),
     "heff_flops": (c_i64, [c_void_p]),
     "heff_inner": (c_int, [c_void_p, c_void_p, c_void_p, P(c_dbl)]),
     "heff_expm": (c_int, [c_void_p, c_void_p, c_void_p, c_dbl, c_int]),
@@ -329,6 +331,14 @@ class Context:
     def heff_apply(self, theta, out):
         """theta, out: torch complex128 CUDA tensors (device pointers are passed through)."""
         self.check(lib.heff_apply(self.h, c_void_p(theta.data_ptr()), c_void_p(out.data_ptr())), "heff_apply")
+
+    def heff_import(self, blocks, vec):
+        """interchange format (blocks back to back, heff_layout order) -> planned layout; CUDA tensors."""
+        self.check(lib.heff_import(self.h, c_void_p(blocks.data_ptr()), c_void_p(vec.data_ptr())), "heff_import")
+
+    def heff_export(self, vec, blocks):
+        """planned layout -> interchange format; CUDA tensors."""
+        self.check(lib.heff_export(self.h, c_void_p(vec.data_ptr()), c_void_p(blocks.data_ptr())), "heff_export")
 
     def heff_flops(self):
         return int(lib.heff_flops(self.h))

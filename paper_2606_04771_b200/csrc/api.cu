@@ -197,6 +197,11 @@ static int last_tj_pos(int nsite) { return nsite == 2 ? 7 : (nsite == 1 ? 4 : 1)
 static void fill_chunks(const BlockTensor& vec, int tpos, std::vector<VecChunk>& chunks) {
   chunks.clear();
   const int cl = vec_chunk_len(vec.nelem);
+  if (tpos < 0) {  // two-site vector: held as sqrt(2 j_b + 1) theta, so F-6 is the plain Euclidean product
+    for (int64_t s = 0; s < vec.nelem; s += cl)
+      chunks.push_back(VecChunk{s, (int)std::min<int64_t>(cl, vec.nelem - s), 1.0f});
+    return;
+  }
   for (size_t i = 0; i < vec.keys.size(); ++i) {
     const int64_t n = (int64_t)vec.rows[i] * vec.cols[i];
     for (int64_t s = 0; s < n; s += cl)
@@ -208,7 +213,7 @@ static void emit_plan2(const fh_mpo* mpo, const fh_mps* mps, int site, BlockTens
                        Stage& st2, std::vector<VecChunk>& chunks) {
   layout_theta(mps->bond[site], mps->bond[site + 2], vec);
   emit_heff2(mps->Lenv[site], mps->Renv[site + 2], vec, mpo->site[site & 1], mpo->site[(site + 1) & 1], Z, st1, st2);
-  fill_chunks(vec, last_tj_pos(2), chunks);
+  fill_chunks(vec, -1, chunks);
 }
 void fh::prefetch_plan2(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site) {
   prefetch_cancel(ctx);
@@ -244,6 +249,7 @@ void fh::plan_heff(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, 
   Plan& P = ctx->plan;
   ctx->free_tensor(P.Z);
   P.valid = false;
+  P.io_ready = false;
   P.nsite = nsite;
   P.site = site;
   const bool use_cache = nsite == 1 && mps->cache.enabled;
@@ -312,6 +318,58 @@ void fh::plan_heff(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, 
   P.d_counter = (unsigned*)P.pool.take(sizeof(unsigned));
   FH_CUDA(cudaMemsetAsync(P.d_counter, 0, sizeof(unsigned), ctx->stream));
   P.valid = true;
+}
+
+// Interchange format <-> planned layout (H8-type scaled block copies).  The interchange format is what
+// heff_layout describes: the blocks in canonical key order, each dense row-major, one after the other, plain
+// tensor entries.  The planned layout is the library's own (two-site: fused per middle label, entries
+// multiplied by sqrt(2 j_b + 1); one-site: identical to the interchange format).
+static void ensure_io(fh_ctx* ctx) {
+  Plan& P = ctx->plan;
+  if (P.io_ready) return;
+  std::vector<CopyBlk> imp(P.vec.keys.size()), exp_(P.vec.keys.size());
+  int64_t canon = 0;
+  for (size_t i = 0; i < P.vec.keys.size(); ++i) {
+    const double w = P.nsite == 2 ? std::sqrt((double)(P.vec.keys[i][7] + 1)) : 1.0;
+    CopyBlk b;
+    b.rows = P.vec.rows[i];
+    b.cols = P.vec.cols[i];
+    b.transpose_dst = 0;
+    b.pad = 0;
+    b.src_off = canon;
+    b.dst_off = P.vec.off[i];
+    b.ld_src = P.vec.cols[i];
+    b.ld_dst = P.vec.ld[i];
+    b.scale = w;
+    imp[i] = b;
+    b.src_off = P.vec.off[i];
+    b.dst_off = canon;
+    b.ld_src = P.vec.ld[i];
+    b.ld_dst = P.vec.cols[i];
+    b.scale = 1.0 / w;
+    exp_[i] = b;
+    canon += (int64_t)P.vec.rows[i] * P.vec.cols[i];
+  }
+  FH_REQUIRE(canon == P.vec.nelem, FH_ESTATE, "planned layout and interchange format differ in size");
+  P.n_io = (int)imp.size();
+  P.io_pool.reset();
+  P.io_pool.reserve(2 * imp.size() * sizeof(CopyBlk) + 4096, ctx->stream);
+  P.d_import = upload(P.io_pool, imp, ctx->stream);
+  P.d_export = upload(P.io_pool, exp_, ctx->stream);
+  FH_CUDA(cudaStreamSynchronize(ctx->stream));  // imp / exp_ are stack-owned
+  P.io_ready = true;
+}
+void fh::vec_import(fh_ctx* ctx, const cplx* blocks, cplx* vec) {
+  FH_REQUIRE(ctx->plan.valid, FH_ESTATE, "heff_import: no plan (call heff_plan first)");
+  ensure_io(ctx);
+  launch_copy_blocks(ctx->plan.d_import, ctx->plan.n_io, blocks, vec, ctx->stream, &ctx->launches);
+  FH_CUDA(cudaGetLastError());
+}
+void fh::vec_export(fh_ctx* ctx, const cplx* vec, cplx* blocks) {
+  FH_REQUIRE(ctx->plan.valid, FH_ESTATE, "heff_export: no plan (call heff_plan first)");
+  ensure_io(ctx);
+  launch_copy_blocks(ctx->plan.d_export, ctx->plan.n_io, vec, blocks, ctx->stream, &ctx->launches);
+  FH_CUDA(cudaGetLastError());
 }
 
 void fh::apply_heff(fh_ctx* ctx, const cplx* theta, cplx* out) {
@@ -633,6 +691,7 @@ void fh_ctx_destroy(fh_ctx* c) {
   }
   for (auto e : c->ev_free) cudaEventDestroy(e);
   c->plan.pool.destroy();
+  c->plan.io_pool.destroy();
   c->pool_aux.destroy();
   c->pool_small.destroy();
   for (auto& w : c->svd_workers) {
@@ -1051,24 +1110,41 @@ int heff_apply(fh_ctx* ctx, const void* theta_dev, void* out_dev) {
   })
 }
 
+int heff_import(fh_ctx* ctx, const void* blocks_dev, void* vec_dev) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && blocks_dev && vec_dev && blocks_dev != vec_dev, FH_EINVAL, "heff_import: bad argument");
+    vec_import(ctx, (const cplx*)blocks_dev, (cplx*)vec_dev);
+  })
+}
+
+int heff_export(fh_ctx* ctx, const void* vec_dev, void* blocks_dev) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && blocks_dev && vec_dev && blocks_dev != vec_dev, FH_EINVAL, "heff_export: bad argument");
+    vec_export(ctx, (const cplx*)vec_dev, (cplx*)blocks_dev);
+  })
+}
+
 int heff_apply_host(fh_ctx* ctx, const void* theta_host, void* out_host) {
   FH_TRY(ctx, {
     FH_REQUIRE(ctx && theta_host && out_host, FH_EINVAL, "heff_apply_host: NULL argument");
     FH_REQUIRE(ctx->plan.valid, FH_ESTATE, "heff_apply_host: no plan (call heff_plan first)");
     const int64_t n = ctx->plan.vec.nelem;
-    const int64_t off = ctx->alloc.alloc(2 * n);
+    const int64_t off = ctx->alloc.alloc(3 * n);
     try {
-      cplx* din = ctx->ptr(off);
+      cplx* io = ctx->ptr(off);
+      cplx* din = io + n;
       cplx* dout = din + n;
-      FH_CUDA(cudaMemcpyAsync(din, theta_host, n * sizeof(cplx), cudaMemcpyHostToDevice, ctx->stream));
+      FH_CUDA(cudaMemcpyAsync(io, theta_host, n * sizeof(cplx), cudaMemcpyHostToDevice, ctx->stream));
+      vec_import(ctx, io, din);
       apply_heff(ctx, din, dout);
-      FH_CUDA(cudaMemcpyAsync(out_host, dout, n * sizeof(cplx), cudaMemcpyDeviceToHost, ctx->stream));
+      vec_export(ctx, dout, io);
+      FH_CUDA(cudaMemcpyAsync(out_host, io, n * sizeof(cplx), cudaMemcpyDeviceToHost, ctx->stream));
       FH_CUDA(cudaStreamSynchronize(ctx->stream));
     } catch (...) {
-      ctx->alloc.release(off, 2 * n);
+      ctx->alloc.release(off, 3 * n);
       throw;
     }
-    ctx->alloc.release(off, 2 * n);
+    ctx->alloc.release(off, 3 * n);
   })
 }
 
@@ -1451,14 +1527,14 @@ int fh_host_get_tasks(int stage, int* ntask, int* nout, int32_t* tuples, double*
 int fh_host_get_units(int stage, int* nunit, int32_t* units, int* nout, int32_t* outs, int64_t* dmma_padded) {
   if (stage != 1 && stage != 2) return FH_EINVAL;
   const Stage& st = stage == 1 ? g_host_st1 : g_host_st2;
+  // the outputs the units tile: blocks merged with their compatible neighbours in a row panel (Stage::mouts)
   if (nunit) *nunit = (int)st.units.size();
-  if (nout) *nout = (int)st.outs.size();
+  if (nout) *nout = (int)st.mouts.size();
   if (dmma_padded) *dmma_padded = st.dmma_padded;
   if (units) {
-    // recover the output index of a unit from its c_off (outputs have distinct offsets unless empty)
+    // recover the output index of a unit from its c_off (merged outputs have distinct offsets)
     std::map<int64_t, int> by_off;
-    for (size_t o = 0; o < st.outs.size(); ++o)
-      if (st.outs[o].M > 0 && st.outs[o].N > 0) by_off[st.outs[o].c_off] = (int)o;
+    for (size_t o = 0; o < st.mouts.size(); ++o) by_off[st.mouts[o].c_off] = (int)o;
     for (size_t i = 0; i < st.units.size(); ++i) {
       const GemmUnit& u = st.units[i];
       units[6 * i] = by_off.count(u.c_off) ? by_off[u.c_off] : -1;
@@ -1470,10 +1546,10 @@ int fh_host_get_units(int stage, int* nunit, int32_t* units, int* nout, int32_t*
     }
   }
   if (outs)
-    for (size_t o = 0; o < st.outs.size(); ++o) {
-      outs[3 * o] = st.outs[o].M;
-      outs[3 * o + 1] = st.outs[o].N;
-      outs[3 * o + 2] = st.outs[o].steps;
+    for (size_t o = 0; o < st.mouts.size(); ++o) {
+      outs[3 * o] = st.mouts[o].M;
+      outs[3 * o + 1] = st.mouts[o].N;
+      outs[3 * o + 2] = st.mouts[o].steps;
     }
   return FH_OK;
 }

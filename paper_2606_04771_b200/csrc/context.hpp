@@ -65,6 +65,12 @@ struct Plan {
   double* d_scal = nullptr;  // Lanczos scalars kept on the device (expm_lanczos)
   unsigned* d_counter = nullptr;  // retirement counter of the one-launch reductions (zero between launches)
   DevPool pool;
+  // interchange format <-> planned layout (heff_import / heff_export), built on first use per plan
+  bool io_ready = false;
+  int n_io = 0;
+  CopyBlk* d_import = nullptr;
+  CopyBlk* d_export = nullptr;
+  DevPool io_pool;
 };
 
 // What the emitter produces for one two-site plan; filled by a second host thread while the main thread runs
@@ -210,6 +216,8 @@ void plan_heff(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, int 
 void prefetch_plan2(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site);
 void prefetch_cancel(fh_ctx* ctx);
 void apply_heff(fh_ctx* ctx, const cplx* theta, cplx* out);
+void vec_import(fh_ctx* ctx, const cplx* blocks, cplx* vec);  // interchange format -> planned layout
+void vec_export(fh_ctx* ctx, const cplx* vec, cplx* blocks);  // planned layout -> interchange format
 double2 inner(fh_ctx* ctx, const cplx* x, const cplx* y);  // synchronises
 // returns the number of Krylov vectors used; adapt_tol > 0 enables the adaptive stop (reading A-15)
 int expm_lanczos(fh_ctx* ctx, cplx* theta_inout, double tau, int m, double tol, cplx* work /* (m+1)*n */,

@@ -60,13 +60,21 @@ struct BlockTensor {
   std::vector<Key> keys;  // sorted
   std::vector<int> rows, cols;
   std::vector<int64_t> off;  // element offsets relative to the tensor base
+  // Leading dimension and first column of every block inside its row panel.  Blocks are dense row-major;
+  // in the plain layout (finalize) each block is contiguous (ld = cols, col0 = 0).  The fused layouts of
+  // the two-site vector and of its stage-1 intermediate (finalize_panels) put the blocks that share a
+  // row-panel side by side in one matrix, so that a GEMM over several of them is ONE wider GEMM.
+  std::vector<int> ld, col0;
   int64_t nelem = 0;
   int64_t base = -1;  // element offset in the arena, -1 = not allocated
   int nlab = 0;       // number of meaningful ints in each key
   std::unordered_map<Key, int, KeyHash> index;
   void clear();
   void add(const Key& k, int r, int c);  // append (caller adds in sorted order)
-  void finalize();                       // offsets (each block 2-element aligned => 32 B)
+  void finalize();                       // plain layout: blocks contiguous, one after the other, in key order
+  // fused layout: block i lies in panel `panel[i]` (panels numbered in memory order; all blocks of a panel
+  // have the same row count) at column position `order[i]` within the panel (ranks need not be dense)
+  void finalize_panels(const std::vector<int>& panel, const std::vector<int>& order);
   int find(const Key& k) const;
 };
 
@@ -91,6 +99,7 @@ struct GemmOut {  // one output block C (M x N, row-major, leading dimension ldc
   int M, N;
   int seg_begin, seg_end;
   int ldc, steps;  // steps = sum over segments of ceil(K / 4) (DMMA k-steps)
+  int col0;        // first column inside its row panel (0 for a contiguous block)
 };
 struct GemmSeg {  // one K-segment: C += alpha * op(A) (M x K) * op(B) (K x N)
   int64_t a_off, b_off;   // element offsets of the operand blocks
@@ -113,7 +122,9 @@ struct Stage {
   // host copies (canonical order) for heff_get_tasks and flops
   std::vector<int> t_out, t_lhs, t_rhs;
   std::vector<double> t_alpha;
-  std::vector<GemmOut> outs;
+  std::vector<double> t_scale;  // optional factor on alpha that is NOT part of the canonical list (vector gauge)
+  std::vector<GemmOut> outs;    // one per output block, canonical order
+  std::vector<GemmOut> mouts;   // outs with compatible neighbours in a row panel merged: what the units tile
   std::vector<GemmSeg> segs;
   std::vector<GemmUnit> units;  // sorted by work, heaviest first
   int opA = OPA_N, opB = OPB_N;

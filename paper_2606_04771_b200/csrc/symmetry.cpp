@@ -44,6 +44,8 @@ void BlockTensor::clear() {
   rows.clear();
   cols.clear();
   off.clear();
+  ld.clear();
+  col0.clear();
   index.clear();
   nelem = 0;
   base = -1;
@@ -55,6 +57,8 @@ void BlockTensor::add(const Key& k, int r, int c) {
 }
 void BlockTensor::finalize() {
   off.resize(keys.size());
+  ld = cols;
+  col0.assign(keys.size(), 0);
   index.clear();
   index.reserve(keys.size() * 2);
   int64_t n = 0;
@@ -64,6 +68,37 @@ void BlockTensor::finalize() {
     index[keys[i]] = (int)i;
   }
   nelem = n;
+}
+void BlockTensor::finalize_panels(const std::vector<int>& panel, const std::vector<int>& order) {
+  const size_t n = keys.size();
+  off.assign(n, 0);
+  ld.assign(n, 0);
+  col0.assign(n, 0);
+  int np = 0;
+  for (int p : panel) np = std::max(np, p + 1);
+  std::vector<std::vector<int>> mem(np);
+  for (size_t i = 0; i < n; ++i) mem[panel[i]].push_back((int)i);
+  int64_t base_ = 0;
+  for (int p = 0; p < np; ++p) {
+    std::vector<int>& m = mem[p];
+    if (m.empty()) continue;
+    std::sort(m.begin(), m.end(), [&](int a, int b) { return order[a] != order[b] ? order[a] < order[b] : a < b; });
+    int w = 0;
+    for (int i : m) {
+      if (rows[i] != rows[m[0]]) throw std::runtime_error("fused layout: blocks of a panel differ in row count");
+      col0[i] = w;
+      w += cols[i];
+    }
+    for (int i : m) {
+      ld[i] = w;
+      off[i] = base_ + col0[i];
+    }
+    base_ += (int64_t)rows[m[0]] * w;
+  }
+  nelem = base_;
+  index.clear();
+  index.reserve(n * 2);
+  for (size_t i = 0; i < n; ++i) index[keys[i]] = (int)i;
 }
 int BlockTensor::find(const Key& k) const {
   auto it = index.find(k);
@@ -78,6 +113,12 @@ static inline int fuse(Sector a, int s, Sector out[2]) {
   const int ts = SITE_TJ[s];
   for (int tc = std::abs(a.tj - ts); tc <= a.tj + ts; tc += 2) out[n++] = Sector{a.q + SITE_Q[s], tc};
   return n;
+}
+
+// column rank of the (s2, b) group inside a fused row panel: s2 in the order 0, 2, 1, then b by (q, tj)
+static inline int theta_col_rank(int s2, int bq, int btj) {
+  static const int perm[3] = {0, 2, 1};
+  return (perm[s2] << 22) + ((bq + 1024) << 11) + btj;
 }
 
 void layout_site(const Bond& bl, const Bond& br, BlockTensor& out) {
@@ -118,7 +159,26 @@ void layout_theta(const Bond& bl, const Bond& br, BlockTensor& out) {
     }
   std::sort(v.begin(), v.end(), [](const auto& x, const auto& y) { return x.first < y.first; });
   for (auto& e : v) out.add(e.first, e.second.first, e.second.second);
-  out.finalize();
+  // Fused layout: for every middle label c the blocks form ONE row-major matrix
+  // theta_c[(a,s1,alpha), (s2,b,beta)] -- the matrix M_c of the SVD split (H8) -- with row groups in (a,s1)
+  // order; column groups ordered s2 = 0, 2, 1 (then b), so that the columns the stage-1 intermediates of
+  // w_m = P (s2 in {0,2}) and w_m = M (s2 in {2,1}) need are contiguous.  A row group is a "panel".
+  const size_t n = out.keys.size();
+  std::vector<std::array<int, 5>> pk(n);  // (c.q, c.tj, a.q, a.tj, s1)
+  for (size_t i = 0; i < n; ++i) {
+    const Key& k = out.keys[i];
+    pk[i] = {k[3], k[4], k[0], k[1], k[2]};
+  }
+  std::vector<std::array<int, 5>> uniq(pk);
+  std::sort(uniq.begin(), uniq.end());
+  uniq.erase(std::unique(uniq.begin(), uniq.end()), uniq.end());
+  std::vector<int> panel(n), order(n);
+  for (size_t i = 0; i < n; ++i) {
+    const Key& k = out.keys[i];
+    panel[i] = (int)(std::lower_bound(uniq.begin(), uniq.end(), pk[i]) - uniq.begin());
+    order[i] = theta_col_rank(k[5], k[6], k[7]);
+  }
+  out.finalize_panels(panel, order);
 }
 
 // ----------------------------------------------------------------------------- reduced MPO (F-2, F-3)
@@ -170,13 +230,13 @@ static void emit_units(Stage& st) {
     int64_t work;
   };
   std::vector<UW> v;
-  v.reserve(st.outs.size() * 2);
+  v.reserve(st.mouts.size() * 2);
   st.dmma_padded = 0;
   // The per-unit cap only exists to create enough units for 148 SMs x 8 resident warps; when the
   // stage is large (chi >~ 8000) full 16-sub-tile units are plentiful and the cap is lifted
   // (measured at chi = 16384: 31.0 TFLOP/s uncapped vs 20.9 with the cap of 3072).
   int64_t total16 = 0;
-  for (const GemmOut& o : st.outs) total16 += (int64_t)4 * ((o.M + 7) / 8) * ((o.N + 7) / 8) * o.steps;
+  for (const GemmOut& o : st.mouts) total16 += (int64_t)4 * ((o.M + 7) / 8) * ((o.N + 7) / 8) * o.steps;
   // Small stages (one-site and zero-site applies, environment updates at chi = 4096: well under a million DMMAs)
   // want smaller units still: a unit should not be longer than the fair share of one of the 1184 warp slots,
   // else the stage lasts as long as its few heaviest units (one-site apply at chi = 4096: 82 -> 71 us with the
@@ -194,8 +254,8 @@ static void emit_units(Stage& st) {
   const int64_t base_cap =
       forced_cap > 0 ? forced_cap : std::min<int64_t>(GEMM_UNIT_DMMA_CAP, std::max<int64_t>(cap_floor, fair));
   const int64_t cap = std::max<int64_t>(base_cap, total16 / (148 * 8 * 6));
-  for (size_t oi = 0; oi < st.outs.size(); ++oi) {
-    const GemmOut& o = st.outs[oi];
+  for (size_t oi = 0; oi < st.mouts.size(); ++oi) {
+    const GemmOut& o = st.mouts[oi];
     if (o.M <= 0 || o.N <= 0) continue;
     const int M8 = (o.M + 7) / 8, N8 = (o.N + 7) / 8;
     const int s_t = (int)std::min<int64_t>(GEMM_MAX_SUBTILES, std::max<int64_t>(2, cap / std::max(1, 4 * o.steps)));
@@ -242,18 +302,84 @@ static void emit_units(Stage& st) {
   for (auto& o : ord) st.units.push_back(v[o.second].u);
 }
 
+// Outputs that lie side by side in one row panel (N direction) or one below the other (M direction) and
+// whose segment lists describe the same GEMM on adjacent operand columns / rows are ONE wider / taller GEMM:
+// the merged output keeps the segment list of its first member (the kernel addresses operands by offset and
+// stride only, so columns n >= N_first simply run on into the neighbour block).  The canonical per-block
+// lists (outs, segs, t_*) are untouched; only the unit decomposition uses mouts.
+static void merge_outs(Stage& st, int64_t lhs_nelem, int64_t rhs_nelem) {
+  st.mouts.clear();
+  st.mouts.reserve(st.outs.size());
+  for (const GemmOut& o : st.outs)
+    if (o.M > 0 && o.N > 0) st.mouts.push_back(o);
+  for (int dir = 0; dir < 2; ++dir) {  // 0: N direction, 1: M direction
+    std::vector<GemmOut>& v = st.mouts;
+    std::unordered_map<int64_t, int> by_off;
+    by_off.reserve(v.size() * 2);
+    for (size_t i = 0; i < v.size(); ++i) by_off[v[i].c_off] = (int)i;
+    std::vector<int> ord(v.size());
+    for (size_t i = 0; i < v.size(); ++i) ord[i] = (int)i;
+    std::sort(ord.begin(), ord.end(), [&](int a, int b) { return v[a].c_off < v[b].c_off; });
+    std::vector<char> dead(v.size(), 0);
+    for (int i : ord) {
+      if (dead[i]) continue;
+      GemmOut& o = v[i];
+      for (;;) {
+        const int64_t next = dir == 0 ? o.c_off + o.N : o.c_off + (int64_t)o.M * o.ldc;
+        auto it = by_off.find(next);
+        if (it == by_off.end()) break;
+        const int j = it->second;
+        if (j == i || dead[j]) break;
+        const GemmOut& p = v[j];
+        const int ns = o.seg_end - o.seg_begin;
+        if (p.ldc != o.ldc || p.seg_end - p.seg_begin != ns || ns == 0) break;
+        if (dir == 0 ? (p.M != o.M || p.col0 != o.col0 + o.N) : (p.N != o.N || p.col0 != o.col0)) break;
+        bool ok = true;
+        for (int t = 0; t < ns && ok; ++t) {
+          const GemmSeg& a = st.segs[o.seg_begin + t];
+          const GemmSeg& b = st.segs[p.seg_begin + t];
+          ok = a.K == b.K && a.alpha == b.alpha && a.a_sm == b.a_sm && a.a_sk == b.a_sk && a.b_sk == b.b_sk &&
+               a.b_sn == b.b_sn;
+          if (dir == 0) ok = ok && a.a_off == b.a_off && b.b_off == a.b_off + (int64_t)o.N * a.b_sn;
+          else ok = ok && b.b_off == a.b_off && b.a_off == a.a_off + (int64_t)o.M * a.a_sm;
+        }
+        if (!ok) break;
+        if (dir == 0) o.N += p.N;
+        else o.M += p.M;
+        dead[j] = 1;
+      }
+    }
+    std::vector<GemmOut> kept;
+    kept.reserve(v.size());
+    for (size_t i = 0; i < v.size(); ++i)
+      if (!dead[i]) kept.push_back(v[i]);
+    v.swap(kept);
+  }
+  // every merged GEMM stays inside its operand tensors (same proof as for the single blocks)
+  for (const GemmOut& o : st.mouts)
+    for (int t = o.seg_begin; t < o.seg_end; ++t) {
+      const GemmSeg& sg = st.segs[t];
+      if (sg.K <= 0) continue;
+      const int64_t a_last = sg.a_off + (int64_t)(o.M - 1) * sg.a_sm + (int64_t)(sg.K - 1) * sg.a_sk;
+      const int64_t b_last = sg.b_off + (int64_t)(sg.K - 1) * sg.b_sk + (int64_t)(o.N - 1) * sg.b_sn;
+      if (a_last >= lhs_nelem || b_last >= rhs_nelem) throw std::runtime_error("task list: merged operand exceeds its tensor");
+    }
+}
+
 void finalize_stage(Stage& st, const BlockTensor& out, const BlockTensor& lhs, const BlockTensor& rhs) {
   const size_t nt = st.t_out.size();
   st.outs.resize(out.keys.size());
   st.segs.resize(nt);
   st.flops = 0;
+  const bool scaled = st.t_scale.size() == nt && nt > 0;
   size_t t = 0;
   for (size_t o = 0; o < out.keys.size(); ++o) {
     GemmOut& go = st.outs[o];
     go.c_off = out.off[o];
     go.M = out.rows[o];
     go.N = out.cols[o];
-    go.ldc = out.cols[o];
+    go.ldc = out.ld[o];
+    go.col0 = out.col0[o];
     go.steps = 0;
     go.seg_begin = (int)t;
     while (t < nt && st.t_out[t] == (int)o) {
@@ -262,28 +388,28 @@ void finalize_stage(Stage& st, const BlockTensor& out, const BlockTensor& lhs, c
       sg.a_off = lhs.off[l];
       sg.b_off = rhs.off[r];
       sg.pad = 0;
-      sg.alpha = st.t_alpha[t];
+      sg.alpha = scaled ? st.t_alpha[t] * st.t_scale[t] : st.t_alpha[t];
       int M, K, K2, N;
       if (st.opA == OPA_H) {  // stored K x M
         M = lhs.cols[l];
         K = lhs.rows[l];
         sg.a_sm = 1;
-        sg.a_sk = lhs.cols[l];
+        sg.a_sk = lhs.ld[l];
       } else {  // stored M x K
         M = lhs.rows[l];
         K = lhs.cols[l];
-        sg.a_sm = lhs.cols[l];
+        sg.a_sm = lhs.ld[l];
         sg.a_sk = 1;
       }
       if (st.opB == OPB_T) {  // stored N x K
         N = rhs.rows[r];
         K2 = rhs.cols[r];
         sg.b_sk = 1;
-        sg.b_sn = rhs.cols[r];
+        sg.b_sn = rhs.ld[r];
       } else {  // stored K x N
         N = rhs.cols[r];
         K2 = rhs.rows[r];
-        sg.b_sk = rhs.cols[r];
+        sg.b_sk = rhs.ld[r];
         sg.b_sn = 1;
       }
       if (M != go.M || N != go.N || K != K2) throw std::runtime_error("task list: block shapes do not match");
@@ -306,6 +432,7 @@ void finalize_stage(Stage& st, const BlockTensor& out, const BlockTensor& lhs, c
       throw std::runtime_error("task list: output block exceeds its tensor");
   }
   if (t != nt) throw std::runtime_error("task list: tasks not sorted by output id");
+  merge_outs(st, lhs.nelem, rhs.nelem);
   emit_units(st);
 }
 
@@ -315,6 +442,7 @@ struct RawTask {
   Key order;    // segment sort key
   int lhs, rhs;
   double alpha;
+  double scale = 1.0;  // factor on alpha outside the canonical list (weights of the vector gauge)
 };
 
 // the first seven ints of an `order` key packed so that integer order == lexicographic order
@@ -367,12 +495,17 @@ void tasks_to_stage(std::vector<RawTask>& raw, const BlockTensor& out, Stage& st
   st.t_lhs.reserve(raw.size());
   st.t_rhs.reserve(raw.size());
   st.t_alpha.reserve(raw.size());
+  st.t_scale.clear();
+  bool any_scale = false;
+  for (const RawTask& r : raw) any_scale = any_scale || r.scale != 1.0;
+  if (any_scale) st.t_scale.reserve(raw.size());
   for (const Ref& f : refs) {
     const RawTask& r = raw[f.idx];
     st.t_out.push_back(f.o);
     st.t_lhs.push_back(r.lhs);
     st.t_rhs.push_back(r.rhs);
     st.t_alpha.push_back(r.alpha);
+    if (any_scale) st.t_scale.push_back(r.scale);
   }
 }
 
@@ -401,12 +534,12 @@ void layout_from_tasks(const std::vector<RawTask>& raw, const std::vector<Shape>
 // Generic "left contraction" (stage 1 of H1, H3, H4):
 //   Z[a',s',c',w' ; rest] = sum_{(w,a,s)} alpha * Lenv[a',w,a] * ket[a,s,c; rest]
 // ket keys: (a.q,a.tj,s,c.q,c.tj, rest...) with `nrest` extra ints (0 for one-site, 3 for two-site).
-void emit_left_contraction(const BlockTensor& Lenv, const BlockTensor& ket, const MpoSite& W, int nrest,
-                           BlockTensor& Z, Stage& st) {
+void left_contraction_tasks(const BlockTensor& Lenv, const BlockTensor& ket, const MpoSite& W, int nrest,
+                            std::vector<RawTask>& raw, std::vector<Shape>& shapes) {
   std::map<Sector, std::vector<int>> by_a;
   for (size_t i = 0; i < ket.keys.size(); ++i) by_a[key_sector(ket.keys[i], 0)].push_back((int)i);
-  std::vector<RawTask> raw;
-  std::vector<Shape> shapes;
+  raw.clear();
+  shapes.clear();
   raw.reserve(4 * ket.keys.size());
   shapes.reserve(4 * ket.keys.size());
   for (size_t e = 0; e < Lenv.keys.size(); ++e) {
@@ -446,6 +579,12 @@ void emit_left_contraction(const BlockTensor& Lenv, const BlockTensor& ket, cons
       }
     }
   }
+}
+void emit_left_contraction(const BlockTensor& Lenv, const BlockTensor& ket, const MpoSite& W, int nrest,
+                           BlockTensor& Z, Stage& st) {
+  std::vector<RawTask> raw;
+  std::vector<Shape> shapes;
+  left_contraction_tasks(Lenv, ket, W, nrest, raw, shapes);
   layout_from_tasks(raw, shapes, 8 + nrest, Z);
   st.opA = OPA_N;
   st.opB = OPB_N;
@@ -454,15 +593,25 @@ void emit_left_contraction(const BlockTensor& Lenv, const BlockTensor& ket, cons
 }
 }  // namespace
 
+// Two-site apply.  The vector is held in the gauge theta~[..b] = sqrt(2 j_b + 1) theta[..b], in
+// which the F-6 inner product is the plain Euclidean one: the stage-2 coefficient of an output block b' fed
+// from a column block b carries the extra factor sqrt((2 j_b' + 1) / (2 j_b + 1)) in t_scale, outside the
+// canonical alpha the tests compare with the oracle.
 void emit_heff2(const BlockTensor& Lenv, const BlockTensor& Renv, const BlockTensor& vec, const MpoSite& W1,
                 const MpoSite& W2, BlockTensor& Z, Stage& st1, Stage& st2) {
-  emit_left_contraction(Lenv, vec, W1, 3, Z, st1);
+  std::vector<RawTask> raw1;
+  std::vector<Shape> shapes1;
+  left_contraction_tasks(Lenv, vec, W1, 3, raw1, shapes1);
+  BlockTensor Zall;
+  layout_from_tasks(raw1, shapes1, 11, Zall);
   std::map<Sector, std::vector<int>> by_b;
   for (size_t i = 0; i < Renv.keys.size(); ++i) by_b[key_sector(Renv.keys[i], 3)].push_back((int)i);
   std::vector<RawTask> raw;
-  raw.reserve(2 * Z.keys.size());
-  for (size_t z = 0; z < Z.keys.size(); ++z) {
-    const Key& zk = Z.keys[z];  // a'(0,1) s1'(2) c'(3,4) wm(5) c(6,7) s2(8) b(9,10)
+  std::vector<int> raw_z;  // index into Zall of each stage-2 task's intermediate
+  raw.reserve(2 * Zall.keys.size());
+  std::vector<char> used(Zall.keys.size(), 0);
+  for (size_t z = 0; z < Zall.keys.size(); ++z) {
+    const Key& zk = Zall.keys[z];  // a'(0,1) s1'(2) c'(3,4) wm(5) c(6,7) s2(8) b(9,10)
     const Sector ap = key_sector(zk, 0), cp = key_sector(zk, 3), c = key_sector(zk, 6), b = key_sector(zk, 9);
     const int s1p = zk[2], wm = zk[5], s2 = zk[8];
     auto it = by_b.find(b);
@@ -483,12 +632,56 @@ void emit_heff2(const BlockTensor& Lenv, const BlockTensor& Renv, const BlockTen
         RawTask t;
         t.out = ok;
         t.order = Key{c.q, c.tj, s2, b.q, b.tj, wm, wr, 0, 0, 0, 0, 0};
-        t.lhs = (int)z;
+        t.lhs = -1;
         t.rhs = ri;
         t.alpha = al;
+        t.scale = std::sqrt((double)(bp.tj + 1) / (double)(b.tj + 1));
         raw.push_back(t);
+        raw_z.push_back((int)z);
+        used[z] = 1;
       }
     }
+  }
+  // reading A-17: an intermediate block that no stage-2 task reads is not formed (no task, no storage, no flops)
+  {
+    std::vector<RawTask> keep1;
+    std::vector<Shape> keeps;
+    keep1.reserve(raw1.size());
+    keeps.reserve(raw1.size());
+    for (size_t i = 0; i < raw1.size(); ++i) {
+      const int z = Zall.find(raw1[i].out);
+      if (z >= 0 && used[z]) {
+        keep1.push_back(raw1[i]);
+        keeps.push_back(shapes1[i]);
+      }
+    }
+    raw1.swap(keep1);
+    shapes1.swap(keeps);
+  }
+  layout_from_tasks(raw1, shapes1, 11, Z);
+  // fused layout of Z: the blocks Z[a',s1',c',w_m; c, (s2,b)] of one (a',s1',c',w_m,c) lie side by side in the
+  // column order of the vector, so that stage 1 forms each such row panel with ONE GEMM per segment
+  {
+    const size_t n = Z.keys.size();
+    std::vector<int> panel(n), order(n);
+    int np = -1;
+    for (size_t i = 0; i < n; ++i) {
+      const Key& k = Z.keys[i];
+      bool same = i > 0;
+      for (int x = 0; same && x < 8; ++x) same = k[x] == Z.keys[i - 1][x];
+      if (!same) ++np;
+      panel[i] = np;
+      order[i] = theta_col_rank(k[8], k[9], k[10]);
+    }
+    Z.finalize_panels(panel, order);
+  }
+  st1.opA = OPA_N;
+  st1.opB = OPB_N;
+  tasks_to_stage(raw1, Z, st1);
+  finalize_stage(st1, Z, Lenv, vec);
+  for (size_t i = 0; i < raw.size(); ++i) {
+    raw[i].lhs = Z.find(Zall.keys[raw_z[i]]);
+    if (raw[i].lhs < 0) throw std::runtime_error("two-site task list: intermediate block missing");
   }
   st2.opA = OPA_N;
   st2.opB = OPB_T;
@@ -637,6 +830,7 @@ void emit_merge(const BlockTensor& A1, const BlockTensor& A2, const BlockTensor&
     t.lhs = i1;
     t.rhs = i2;
     t.alpha = 1.0;
+    t.scale = std::sqrt((double)(k[7] + 1));  // the two-site vector lives in the gauge sqrt(2 j_b + 1) theta
     raw.push_back(t);
   }
   st.opA = OPA_N;

@@ -780,7 +780,8 @@ static void svd_split(fh_ctx* ctx, fh_mps* mps, int i, const BlockTensor& th, co
   double* dS = reinterpret_cast<double*>(buf + cplx_total);
   cudaStream_t s = ctx->stream;
 
-  // ---- pack (H8): M_c[(a,s1,al),(s2,b,be)] = theta[a,s1,c,s2,b] sqrt((2j_b+1)/(2j_c+1))
+  // ---- pack (H8): M_c[(a,s1,al),(s2,b,be)] = theta[a,s1,c,s2,b] sqrt((2j_b+1)/(2j_c+1)); the vector already
+  //      carries the sqrt(2j_b+1), so the copy only divides by sqrt(2j_c+1)
   ctx->timer_begin(T_PACK);
   launch_fill_zero(buf, cplx_total, s, &ctx->launches);
   std::vector<CopyBlk> blks;
@@ -796,8 +797,8 @@ static void svd_split(fh_ctx* ctx, fh_mps* mps, int i, const BlockTensor& th, co
     b.src_off = th.off[t];
     b.rows = th.rows[t];
     b.cols = th.cols[t];
-    b.ld_src = th.cols[t];
-    b.scale = std::sqrt((double)(k[7] + 1) / (double)(k[4] + 1));
+    b.ld_src = th.ld[t];
+    b.scale = 1.0 / std::sqrt((double)(k[4] + 1));  // theta is held as sqrt(2 j_b + 1) theta
     b.pad = 0;
     if (!S.transposed) {  // row-major M_c (nrow x ncol)
       b.dst_off = S.m_off + (int64_t)ro * S.ncol + co;
@@ -998,6 +999,7 @@ static void plan_zero_site(fh_ctx* ctx, fh_mps* mps, int bond, const BlockTensor
   Plan& P = ctx->plan;
   ctx->free_tensor(P.Z);
   P.valid = false;
+  P.io_ready = false;
   P.nsite = 0;
   P.site = -1;
   P.vec = Cl;

@@ -69,8 +69,26 @@ def build_central_bond(ctx, mpo, chi, L=60, seed=fi.SEED, profile="gaussian", ta
     return mps, dims
 
 
+def to_planned(ctx, flat):
+    """Host vector in the interchange format (blocks back to back in heff_layout order) -> device vector
+    in the library's planned layout, converted by the library's own kernel (heff_import)."""
+    import torch
+    blocks = torch.from_numpy(np.ascontiguousarray(flat, dtype=np.complex128)).to(ctx.device)
+    vec = torch.empty_like(blocks)
+    ctx.heff_import(blocks, vec)
+    return vec
+
+
+def from_planned(ctx, vec):
+    """Planned device vector -> host numpy vector in the interchange format (heff_export)."""
+    import torch
+    blocks = torch.empty_like(vec)
+    ctx.heff_export(vec, blocks)
+    return blocks.cpu().numpy()
+
+
 def theta_vector(ctx, site, dims_l, dims_r, seed=fi.SEED):
-    """Random two-site vector in the planned layout of the current plan (host numpy)."""
+    """Random two-site vector in the interchange format of the current plan (host numpy)."""
     lab, dm, ne = ctx.heff_layout(2)
     th = fi.theta_random(seed, site, dims_l, dims_r)
     v = flatten(th, lab, dm, theta_key)
@@ -79,4 +97,4 @@ def theta_vector(ctx, site, dims_l, dims_r, seed=fi.SEED):
 
 
 __all__ = ["binding", "site_key", "theta_key", "flatten", "unflatten", "set_site", "build_central_bond",
-           "theta_vector"]
+           "theta_vector", "to_planned", "from_planned"]

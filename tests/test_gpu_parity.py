@@ -60,10 +60,10 @@ def _small_chain(rng, L, dmax):
 def _apply_gpu(H, ctx, vec_blocks, nsite):
     lab, dm, ne = ctx.heff_layout(nsite)
     keyfn = H.theta_key if nsite == 2 else H.site_key
-    x = _dev(H.flatten(vec_blocks, lab, dm, keyfn))
+    x = H.to_planned(ctx, H.flatten(vec_blocks, lab, dm, keyfn))
     y = _torch().empty_like(x)
     ctx.heff_apply(x, y)
-    return H.unflatten(y.cpu().numpy(), lab, dm, keyfn)
+    return H.unflatten(H.from_planned(ctx, y), lab, dm, keyfn)
 
 
 # ------------------------------------------------------------------ small chains, every bond
@@ -156,7 +156,7 @@ def test_config2_full_size_apply_tasks_and_hermiticity(H, ctx):
     assert np.array_equal(xout, H.flatten(got, lab, dm, H.theta_key))
     # Hermiticity and inner product
     ph = fi.theta_random(fi.SEED + 1, c, dl, dr)
-    x, y = _dev(xin), _dev(H.flatten(ph, lab, dm, H.theta_key))
+    x, y = H.to_planned(ctx, xin), H.to_planned(ctx, H.flatten(ph, lab, dm, H.theta_key))
     hx, hy = _torch().empty_like(x), _torch().empty_like(y)
     ctx.heff_apply(x, hx)
     ctx.heff_apply(y, hy)
@@ -236,10 +236,10 @@ def test_apply_parity_bench_sizes_sampled_blocks(H, chi, nsample):
             ctx.env_set(mps, which, bond, labels, flat)
         ctx.heff_plan(mpo, mps, c, 2)
         lab, dm, ne = ctx.heff_layout(2)
-        x = _dev(H.flatten(th, lab, dm, H.theta_key))
+        x = H.to_planned(ctx, H.flatten(th, lab, dm, H.theta_key))
         y = _torch().empty_like(x)
         ctx.heff_apply(x, y)
-        got = H.unflatten(y.cpu().numpy(), lab, dm, H.theta_key)
+        got = H.unflatten(H.from_planned(ctx, y), lab, dm, H.theta_key)
         y2 = _torch().empty_like(x)
         ctx.heff_apply(2.0 * x, y2)
         assert bool((y2 == 2.0 * y).all())                      # exact: scaling by 2 commutes with rounding
@@ -280,10 +280,10 @@ def test_expm_parity_central_bond(H, ctx):
     mps, _ = H.build_central_bond(ctx, mpo, chi, L)
     ctx.heff_plan(mpo, mps, c, 2)
     lab, dm, ne = ctx.heff_layout(2)
-    x = _dev(H.flatten(th, lab, dm, H.theta_key))
+    x = H.to_planned(ctx, H.flatten(th, lab, dm, H.theta_key))
     y = _torch().empty_like(x)
     ctx.heff_expm(x, y, tau, m)
-    got = H.unflatten(y.cpu().numpy(), lab, dm, H.theta_key)
+    got = H.unflatten(H.from_planned(ctx, y), lab, dm, H.theta_key)
     assert rel_err(got, ref) < 1e-10
     n0, n1 = ctx.heff_inner(x, x).real, ctx.heff_inner(y, y).real
     assert abs(n1 / n0 - 1.0) < 1e-11
@@ -477,7 +477,7 @@ def test_next2_adaptive_krylov_expm_and_sweeps(H, ctx):
     mps, _ = H.build_central_bond(ctx, mpo, chi, L)
     ctx.heff_plan(mpo, mps, c, 2)
     lab, dm, ne = ctx.heff_layout(2)
-    x = _dev(H.flatten(th, lab, dm, H.theta_key))
+    x = H.to_planned(ctx, H.flatten(th, lab, dm, H.theta_key))
     y = _torch().empty_like(x)
     yfix = _torch().empty_like(x)
     ctx.heff_expm(x, yfix, tau, mmax)
@@ -489,7 +489,7 @@ def test_next2_adaptive_krylov_expm_and_sweeps(H, ctx):
         k = ctx.heff_expm_adaptive(x, y, tau, mmax, tol)
         assert k == st[0], (tol, k, st)
         used[tol] = k
-        got = H.unflatten(y.cpu().numpy(), lab, dm, H.theta_key)
+        got = H.unflatten(H.from_planned(ctx, y), lab, dm, H.theta_key)
         assert rel_err(got, ref) < 1e-10
         d = y - yfix
         assert float(ctx.heff_inner(d, d).real) ** 0.5 / nx < 10 * tol + 1e-12

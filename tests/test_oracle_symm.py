@@ -14,13 +14,14 @@ def _rand(rng, m, n):
     return rng.standard_normal((m, n)) + 1j * rng.standard_normal((m, n))
 
 
-@pytest.fixture(scope="module")
-def chain():
-    """Random symmetric MPS on an L=4 chain with all reachable sectors, degeneracies 1..3."""
-    rng = np.random.default_rng(1)
-    L, t_h, U = 4, 1.0, 4.0
+@pytest.fixture(scope="module", params=[4, 6])
+def chain(request):
+    """Random symmetric MPS with all reachable sectors: L=4 (2j <= 2, degeneracies 1..3) and L=6 (2j <= 3, so
+    that every branch of the recoupling coefficients with j >= 3/2 is embedded too; degeneracies 1..2)."""
+    L, t_h, U = request.param, 1.0, 4.0
+    rng = np.random.default_rng(1 if L == 4 else 6)
     tabs = fi.reachable_tables(L)
-    dims = [{sec: int(rng.integers(1, 4)) for sec in tabs[k]} for k in range(L + 1)]
+    dims = [{sec: int(rng.integers(1, 4 if L == 4 else 3)) for sec in tabs[k]} for k in range(L + 1)]
     dims[0] = {(0, 0): 1}
     dims[L] = {(0, 0): 1}
     A = [{k: _rand(rng, dims[i][k[0]], dims[i + 1][k[2]]) for k in symm.site_keys(dims[i], dims[i + 1])}
@@ -112,8 +113,11 @@ def test_heff2_vs_dense_hermiticity_inner(chain):
         out = symm.heff2_apply(chain["Le"][i], chain["Re"][i + 2], th, chain["Ws"][i], chain["Ws"][i + 1])
         thd = symm.embed_theta(th, dims[i], dims[i + 2], i)
         phd = symm.embed_theta(ph, dims[i], dims[i + 2], i)
-        ref = np.einsum("xwa,wvps,vuqt,astb,yub->xpqy", chain["Ld"][i], chain["Wd"][i], chain["Wd"][i + 1],
-                        thd, chain["Rd"][i + 2])
+        # H_eff theta = L . W_i . W_{i+1} . theta . R, one pairwise contraction at a time
+        t1 = np.einsum("xwa,astb->xwstb", chain["Ld"][i], thd)
+        t2 = np.einsum("wvps,xwstb->xvptb", chain["Wd"][i], t1)
+        t3 = np.einsum("vuqt,xvptb->xpqub", chain["Wd"][i + 1], t2)
+        ref = np.einsum("xpqub,yub->xpqy", t3, chain["Rd"][i + 2])
         got = symm.embed_theta(out, dims[i], dims[i + 2], i)
         assert np.linalg.norm(got - ref) < 1e-13 * np.linalg.norm(ref)
         assert abs(symm.inner(ph, th) - np.vdot(phd, thd)) < 1e-12 * np.linalg.norm(phd) * np.linalg.norm(thd)
@@ -126,7 +130,9 @@ def test_heff1_vs_dense(chain):
         dims = chain["dims"]
         assert symm.site_keys(dims[i], dims[i + 1]) == fi.site_block_keys(dims[i], dims[i + 1])
         out = symm.heff1_apply(chain["Le"][i], chain["Re"][i + 1], chain["A"][i], chain["Ws"][i])
-        ref = np.einsum("xwa,wvps,asb,yvb->xpy", chain["Ld"][i], chain["Wd"][i], chain["Ad"][i], chain["Rd"][i + 1])
+        t1 = np.einsum("xwa,asb->xwsb", chain["Ld"][i], chain["Ad"][i])
+        t2 = np.einsum("wvps,xwsb->xvpb", chain["Wd"][i], t1)
+        ref = np.einsum("xvpb,yvb->xpy", t2, chain["Rd"][i + 1])
         got = symm.embed_site(out, dims[i], dims[i + 1], i)
         assert np.linalg.norm(got - ref) < 1e-13 * np.linalg.norm(ref)
 
@@ -182,6 +188,50 @@ def test_task_lists_are_canonical_and_consistent(chain):
     assert (np.diff(tup[:, 0]) >= 0).all()
     f = symm.heff2_flops(st1, st2, dims[i], dims[i + 2])
     assert f > 0 and f % 8 == 0
+    # reading A-17: every intermediate block of the list is read by stage 2
+    assert {seg[0] for segs in st2.values() for seg in segs} == set(st1)
+
+
+class _Counting(np.ndarray):
+    """ndarray that counts 8 m n k for every complex matrix product it takes part in."""
+    flops = 0
+
+    def __matmul__(self, other):
+        a, b = np.asarray(self), np.asarray(other)
+        _Counting.flops += 8 * a.shape[0] * a.shape[1] * b.shape[1]
+        return (a @ b).view(_Counting)
+
+    def __rmatmul__(self, other):
+        a, b = np.asarray(other), np.asarray(self)
+        _Counting.flops += 8 * a.shape[0] * a.shape[1] * b.shape[1]
+        return (a @ b).view(_Counting)
+
+
+def test_heff2_flops_hand_worked_and_counted(chain):
+    """Pins of heff2_flops (the numerator of the headline GFLOP/s).
+    (a) Hand-worked: the only bond of an L=2 chain, boundary environments L[(0,0),S,(0,0)] (2 x 2) and
+    R[(0,0),F,(0,0)] (3 x 3), bond degeneracies d_l = 2, d_r = 3.  theta has the three blocks (s1,s2) = (up,dn),
+    (dn,up), (pair,pair).  H = hopping + (U/2)(P_D,0 + P_D,1) has six non-zero reduced elements between them:
+    P_D on site 0 (w_m = F) and on site 1 (w_m = S) on the pair block, and the four hopping terms pair<->(up,dn),
+    pair<->(dn,up) (w_m = P, M).  Each is one stage-1 task (8 * 2*2*3) and one stage-2 task (8 * 2*3*3).
+    (b) Counted: the products the oracle's own heff2_apply executes, counted by an instrumented ndarray."""
+    dl, dr = {(0, 0): 2}, {(0, 0): 3}
+    Lk, Rk = [((0, 0), 0, (0, 0))], [((0, 0), 3, (0, 0))]
+    tk = symm.theta_keys(dl, dr)
+    assert len(tk) == 3
+    st1, st2 = symm.heff2_tasks(Lk, Rk, tk, symm.mpo_reduced(0, 1.0, 4.0), symm.mpo_reduced(1, 1.0, 4.0))
+    assert sum(len(v) for v in st1.values()) == 6 and sum(len(v) for v in st2.values()) == 6
+    assert symm.heff2_flops(st1, st2, dl, dr) == 8 * (6 * 2 * 2 * 3 + 6 * 2 * 3 * 3) == 1440
+    dims, rng = chain["dims"], chain["rng"]
+    for i in range(chain["L"] - 1):
+        Le = {k: v.view(_Counting) for k, v in chain["Le"][i].items()}
+        Re = {k: v.view(_Counting) for k, v in chain["Re"][i + 2].items()}
+        th = {k: _rand(rng, dims[i][k[0]], dims[i + 2][k[4]]).view(_Counting)
+              for k in symm.theta_keys(dims[i], dims[i + 2])}
+        _Counting.flops = 0
+        symm.heff2_apply(Le, Re, th, chain["Ws"][i], chain["Ws"][i + 1])
+        st1, st2 = symm.heff2_tasks(sorted(Le), sorted(Re), sorted(th), chain["Ws"][i], chain["Ws"][i + 1])
+        assert _Counting.flops == symm.heff2_flops(st1, st2, dims[i], dims[i + 2]) > 0
 
 
 def test_symmetric_tdvp_equals_dense_tdvp_and_measurements():
