@@ -52,6 +52,20 @@ typedef struct fh_mps fh_mps;
 int fh_ctx_create(fh_ctx** out, void* cuda_stream, void* arena_dev, size_t arena_bytes);
 void fh_ctx_destroy(fh_ctx* ctx);
 const char* fh_last_error(const fh_ctx* ctx);
+/* Options of a context (host-only; FH_EINVAL on a NULL context, an unknown key or a value out of range).
+ *   FH_OPT_GEMM_PATH     which form of the grouped ZGEMM heff_apply uses for two-site plans: 0 = the library
+ *                        chooses by the size of the plan (default), 1 = one warp-unit per one-warp CTA, two
+ *                        launches (csrc/zgemm.cu), 2 = warp-specialised persistent kernel, both stages in one
+ *                        launch (csrc/zgemm_ws.cu).  Same results to rounding (the k-split tiles of form 2 add
+ *                        partial sums in another, fixed, order).
+ *   FH_OPT_SVD_MID_MAXN  widest sector matrix (columns) the library's own global-memory Jacobi kernel takes
+ *                        instead of the vendor SVD, 0 .. 256 (default 128; 0 = none).
+ *   FH_OPT_SVD_THREADS   host threads that drive the vendor SVD / QR routines, 1 .. 12 (default: cores - 1,
+ *                        at most 12); takes effect before the first factorisation of the context. */
+#define FH_OPT_GEMM_PATH 1
+#define FH_OPT_SVD_MID_MAXN 2
+#define FH_OPT_SVD_THREADS 3
+int fh_set_option(fh_ctx* ctx, int key, int value);
 /* bytes currently allocated / high-water mark in the arena */
 int fh_arena_stats(const fh_ctx* ctx, size_t* used_bytes, size_t* peak_bytes);
 

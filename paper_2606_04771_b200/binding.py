@@ -11,8 +11,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-# FH_B200_LIB selects another build of the same library (unit_timeline.py uses the -DFH_UNIT_TRACE one)
-LIB_PATH = os.environ.get("FH_B200_LIB") or os.path.join(_HERE, "libfh_b200.so")
+LIB_PATH = os.path.join(_HERE, "libfh_b200.so")
 if not os.path.exists(LIB_PATH):
     raise ImportError("libfh_b200.so is not built: run `python -m paper_2606_04771_b200.build` "
                       "(or __graft_entry__.build()); there is no CPU fallback")
@@ -32,6 +31,7 @@ _SIGS = {
     "fh_ctx_destroy": (None, [c_void_p]),
     "fh_last_error": (C.c_char_p, [c_void_p]),
     "fh_arena_stats": (c_int, [c_void_p, P(c_size_t), P(c_size_t)]),
+    "fh_set_option": (c_int, [c_void_p, c_int, c_int]),
     "fh_mpo_build": (c_int, [c_void_p, c_int, c_dbl, c_dbl, P(c_void_p)]),
     "fh_mpo_destroy": (None, [c_void_p]),
     "fh_mpo_get_site": (c_int, [c_void_p, c_int, c_void_p, c_void_p]),
@@ -420,6 +420,11 @@ class Context:
 
     def fh_launch_count(self):
         return int(lib.fh_launch_count(self.h))
+
+    OPT_GEMM_PATH, OPT_SVD_MID_MAXN, OPT_SVD_THREADS = 1, 2, 3
+
+    def fh_set_option(self, key, value):
+        self.check(lib.fh_set_option(self.h, int(key), int(value)), "fh_set_option")
 
     def fh_arena_stats(self):
         a, b = c_size_t(), c_size_t()

@@ -70,11 +70,22 @@ void DevPool::destroy() {
 }
 
 size_t fh::stage_bytes(const Stage& st) {
-  return st.segs.size() * sizeof(GemmSeg) + st.units.size() * sizeof(GemmUnit) + 4 * 256;
+  return st.segs.size() * sizeof(GemmSeg) + st.units.size() * sizeof(GemmUnit) + st.tiles.size() * sizeof(WsTile) + 6 * 256;
+}
+size_t fh::pair_bytes(const WsPair& pr) {
+  return pr.tiles.size() * sizeof(WsTile) + pr.segs.size() * sizeof(GemmSeg) + pr.dep_id.size() * 8 +
+         (size_t)(pr.n_slots + pr.n_dep_counters) * sizeof(unsigned) + 8 * 256;
+}
+void fh::upload_pair(DevPool& pool, WsPair& pr, cudaStream_t s) {
+  pr.d_tiles = upload(pool, pr.tiles, s);
+  pr.d_segs = upload(pool, pr.segs, s);
+  pr.d_dep_id = upload(pool, pr.dep_id, s);
+  pr.d_dep_target = upload(pool, pr.dep_target, s);
 }
 void fh::upload_stage(DevPool& pool, Stage& st, cudaStream_t s) {
   st.d_segs = upload(pool, st.segs, s);
   st.d_units = upload(pool, st.units, s);
+  st.d_tiles = upload(pool, st.tiles, s);
 }
 
 void fh_ctx::alloc_tensor(BlockTensor& t) { t.base = alloc.alloc(t.nelem); }
@@ -217,11 +228,6 @@ static void emit_plan2(const fh_mpo* mpo, const fh_mps* mps, int site, BlockTens
 }
 void fh::prefetch_plan2(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site) {
   prefetch_cancel(ctx);
-  static const bool off = [] {
-    const char* e = std::getenv("FH_NO_PREFETCH");  // A/B timing: emit every plan on the calling thread
-    return e && e[0] && e[0] != '0';
-  }();
-  if (off) return;
   if (site < 0 || site + 2 > mps->L || mps->Lenv[site].base < 0 || mps->Renv[site + 2].base < 0) return;
   PlanEmit* e = &ctx->prefetch;
   e->site = site;
@@ -248,6 +254,8 @@ void fh::plan_heff(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, 
   FH_REQUIRE(Le.base >= 0 && Re.base >= 0, FH_ESTATE, "heff_plan: environments of this bond are not built");
   Plan& P = ctx->plan;
   ctx->free_tensor(P.Z);
+  if (P.ws_scratch >= 0) ctx->alloc.release(P.ws_scratch, P.ws_scratch_n);
+  P.ws_scratch = -1;
   P.valid = false;
   P.io_ready = false;
   P.nsite = nsite;
@@ -305,9 +313,13 @@ void fh::plan_heff(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, 
     }
   }
   ctx->alloc_tensor(P.Z);
+  P.ws_scratch_n = (int64_t)(P.st1.n_slots + P.st2.n_slots) * WS_SLOT_ELEMS;
+  if (P.ws_scratch_n > 0) P.ws_scratch = ctx->alloc.alloc(P.ws_scratch_n);
   P.Lptr = ctx->ptr(Le.base);
   P.Rptr = ctx->ptr(Re.base);
-  const size_t need = stage_bytes(P.st1) + stage_bytes(P.st2) + P.chunks.size() * (sizeof(VecChunk) + 16) + 8192;
+  link_stages(P.st1, P.st2, 0, P.pair);  // stage 2 reads the intermediate as its left operand
+  const size_t need = stage_bytes(P.st1) + stage_bytes(P.st2) + pair_bytes(P.pair) +
+                      P.chunks.size() * (sizeof(VecChunk) + 16) + 8192;
   P.pool.reserve(need, ctx->stream);
   upload_stage(P.pool, P.st1, ctx->stream);
   upload_stage(P.pool, P.st2, ctx->stream);
@@ -317,6 +329,15 @@ void fh::plan_heff(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, 
   P.d_scal = (double*)P.pool.take(256 * sizeof(double));
   P.d_counter = (unsigned*)P.pool.take(sizeof(unsigned));
   FH_CUDA(cudaMemsetAsync(P.d_counter, 0, sizeof(unsigned), ctx->stream));
+  upload_pair(P.pool, P.pair, ctx->stream);
+  {
+    const size_t nf = (size_t)P.pair.n_slots + 1, nd = (size_t)P.pair.n_dep_counters + 1;
+    P.d_ws_flags = (unsigned*)P.pool.take(nf * sizeof(unsigned));
+    P.d_ws_dep = (unsigned*)P.pool.take(nd * sizeof(unsigned));
+    FH_CUDA(cudaMemsetAsync(P.d_ws_flags, 0, nf * sizeof(unsigned), ctx->stream));
+    FH_CUDA(cudaMemsetAsync(P.d_ws_dep, 0, nd * sizeof(unsigned), ctx->stream));
+  }
+  P.ws_epoch = 0;
   P.valid = true;
 }
 
@@ -376,8 +397,21 @@ void fh::apply_heff(fh_ctx* ctx, const cplx* theta, cplx* out) {
   Plan& P = ctx->plan;
   FH_REQUIRE(P.valid, FH_ESTATE, "heff_apply: no plan (call heff_plan first)");
   cplx* Z = ctx->ptr(P.Z.base);
-  launch_grouped_gemm(P.st1, P.Lptr, theta, Z, ctx->stream, &ctx->launches, PDL_GEMM_FIRST);
-  launch_grouped_gemm(P.st2, Z, P.Rptr, out, ctx->stream, &ctx->launches, PDL_GEMM_SECOND);
+  // Which form: measured on the Gaussian and Table-S2 profiles the warp-specialised single
+  // launch wins from about 1e7 padded DMMAs per apply upwards (chi ~ 5000 - 12000: +5 ... +10 %), ties above and
+  // at chi = 4096, and loses below (its start-up is longer than that of 148 x 8 one-warp CTAs).
+  const int64_t dmma = P.st1.dmma_padded + P.st2.dmma_padded;
+  const bool use_ws = P.nsite == 2 && !P.pair.tiles.empty() &&
+                      (ctx->opt_gemm_path == 2 || (ctx->opt_gemm_path == 0 && dmma >= 10000000 && dmma < 400000000));
+  if (use_ws) {
+    ++P.ws_epoch;
+    cplx* sc = P.ws_scratch >= 0 ? ctx->ptr(P.ws_scratch) : nullptr;
+    launch_grouped_gemm_ws_pair(P.pair, P.Lptr, theta, Z, Z, P.Rptr, out, ctx->d_ws_counters, ctx->num_sms, sc,
+                                P.d_ws_flags, P.d_ws_dep, P.ws_epoch, ctx->stream, &ctx->launches);
+  } else {
+    launch_grouped_gemm(P.st1, P.Lptr, theta, Z, ctx->stream, &ctx->launches, PDL_GEMM_FIRST);
+    launch_grouped_gemm(P.st2, Z, P.Rptr, out, ctx->stream, &ctx->launches, PDL_GEMM_SECOND);
+  }
   FH_CUDA(cudaGetLastError());
 }
 
@@ -673,6 +707,13 @@ int fh_ctx_create(fh_ctx** out, void* cuda_stream, void* arena_dev, size_t arena
     }
     c->alloc.init((int64_t)(arena_bytes / sizeof(cplx)));
     c->ensure_pinned(4096);
+    FH_CUDA(cudaMalloc((void**)&c->d_ws_counters, 64));
+    FH_CUDA(cudaMemset(c->d_ws_counters, 0, 64));
+    {
+      cudaDeviceProp prop;
+      FH_CUDA(cudaGetDeviceProperties(&prop, c->device));
+      c->num_sms = prop.multiProcessorCount;
+    }
   } catch (const std::exception& e) {
     delete c;
     return FH_ECUDA;
@@ -692,6 +733,7 @@ void fh_ctx_destroy(fh_ctx* c) {
   for (auto e : c->ev_free) cudaEventDestroy(e);
   c->plan.pool.destroy();
   c->plan.io_pool.destroy();
+  if (c->d_ws_counters) cudaFree(c->d_ws_counters);
   c->pool_aux.destroy();
   c->pool_small.destroy();
   for (auto& w : c->svd_workers) {
@@ -713,6 +755,26 @@ void fh_ctx_destroy(fh_ctx* c) {
 }
 
 const char* fh_last_error(const fh_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+int fh_set_option(fh_ctx* c, int key, int value) {
+  if (!c) return FH_EINVAL;
+  switch (key) {
+    case FH_OPT_GEMM_PATH:
+      if (value < 0 || value > 2) return FH_EINVAL;
+      c->opt_gemm_path = value;
+      return FH_OK;
+    case FH_OPT_SVD_MID_MAXN:
+      if (value < 0 || value > 256) return FH_EINVAL;
+      c->opt_svd_mid_maxn = value;
+      return FH_OK;
+    case FH_OPT_SVD_THREADS:
+      if (value < 1 || value > 12) return FH_EINVAL;
+      c->opt_svd_threads = value;
+      return FH_OK;
+    default:
+      return FH_EINVAL;
+  }
+}
 
 int fh_arena_stats(const fh_ctx* c, size_t* used, size_t* peak) {
   if (!c) return FH_EINVAL;

@@ -65,6 +65,12 @@ struct Plan {
   double* d_scal = nullptr;  // Lanczos scalars kept on the device (expm_lanczos)
   unsigned* d_counter = nullptr;  // retirement counter of the one-launch reductions (zero between launches)
   DevPool pool;
+  // k-split tiles of the warp-specialised GEMM: scratch slots in the arena, arrival counters, launch number
+  int64_t ws_scratch = -1, ws_scratch_n = 0;  // arena offset / elements
+  unsigned* d_ws_flags = nullptr;   // one counter per scratch slot (both stages)
+  unsigned* d_ws_dep = nullptr;     // one counter per stage-1 output panel (cross-stage dependencies)
+  unsigned ws_epoch = 0;
+  WsPair pair;                      // joint tile queue of the two stages: one launch per apply
   // interchange format <-> planned layout (heff_import / heff_export), built on first use per plan
   bool io_ready = false;
   int n_io = 0;
@@ -180,6 +186,11 @@ struct fh_ctx {
   bool small_copied_armed = false;
   std::vector<char> small_desc_host;
   int device = 0;
+  int opt_gemm_path = 0;      // fh_set_option: 0 auto, 1 warp units, 2 warp-specialised
+  int opt_svd_mid_maxn = 128;
+  int opt_svd_threads = 0;    // 0 = default
+  int num_sms = 148;
+  unsigned* d_ws_counters = nullptr;  // tile-queue head and retired-CTA count of the warp-specialised GEMM (zero between launches)
   int64_t svd_count[3] = {0, 0, 0};  // gesvd, gesvdp, gesvdp fallbacks to gesvd
   int64_t qr_small = 0;  // one-site splits done by small_qr_kernel
   int64_t svd_small = 0, qr_count = 0;  // sector matrices done by small_svd_kernel / by geqrf+ungqr
@@ -207,6 +218,8 @@ T* upload(DevPool& pool, const std::vector<T>& v, cudaStream_t s) {
 }
 size_t stage_bytes(const Stage& st);
 void upload_stage(DevPool& pool, Stage& st, cudaStream_t s);
+size_t pair_bytes(const WsPair& pr);
+void upload_pair(DevPool& pool, WsPair& pr, cudaStream_t s);
 
 // engine pieces (api.cu / tdvp.cu)
 void plan_heff(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, int nsite);

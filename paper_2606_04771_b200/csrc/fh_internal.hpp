@@ -118,6 +118,26 @@ struct GemmUnit {
   GemmSeg first;  // copy of segs[seg_begin]: the unit starts streaming after ONE descriptor load
 };
 
+// One tile of the warp-specialised kernel (zgemm_ws.cu): an (8 h) x (8 w) part (h, w <= 8) of output block
+// `c_off`, worked on by a group of 2 x 2 consumer warps.  A tile covers the k range from k_begin inside segment
+// seg_begin to k_end inside segment seg_end - 1 (both multiples of 16 or a segment end); a heavy tile is split
+// along k into parts: kind 1 = a part that leaves its accumulators in scratch slot `slot`, kind 0 = the part
+// that finally adds the `nparts` partial results of slots slot .. slot + nparts - 1 (in that order) and stores
+// the block.  128 bytes; the first segment is repeated inside so that ONE load gives a producer everything it
+// needs to start streaming.
+struct WsTile {
+  int64_t c_off;
+  int ldc, M, N, m0, n0, h, w, seg_begin, seg_end, steps;
+  GemmSeg first;
+  int k_begin, k_end, kind, slot, nparts;
+  // two stages in one launch (stage 2 reads what stage 1 writes): `stage` selects the operand set; a tile of
+  // stage 1 that stores its block raises counter `sig` of its output panel when done; a tile of stage 2 may
+  // start once the counters dep_id[dep_begin .. dep_begin + dep_count) have reached their targets
+  int stage_sig;   // stage | (sig + 1) << 1
+  int dep_begin, dep_count;
+};
+static_assert(sizeof(WsTile) == 128, "WsTile is one 128-byte line");
+
 struct Stage {
   // host copies (canonical order) for heff_get_tasks and flops
   std::vector<int> t_out, t_lhs, t_rhs;
@@ -127,12 +147,17 @@ struct Stage {
   std::vector<GemmOut> mouts;   // outs with compatible neighbours in a row panel merged: what the units tile
   std::vector<GemmSeg> segs;
   std::vector<GemmUnit> units;  // sorted by work, heaviest first
+  std::vector<WsTile> tiles;    // the same outputs cut into tiles for the warp-specialised kernel, heaviest first
+  int n_slots = 0;              // scratch slots (WS_SLOT_ELEMS complex each) the k-split tiles of this stage need
+  std::vector<int> out_mout;    // output block -> index into mouts (-1: empty block)
+  std::vector<int> mout_tiles;  // per merged output: number of tiles that store (part of) it
   int opA = OPA_N, opB = OPB_N;
   int64_t flops = 0;
   int64_t dmma_padded = 0;  // DMMA.8x8x4 instructions the unit list issues (incl. ragged-edge padding)
   // device copies
   GemmSeg* d_segs = nullptr;
   GemmUnit* d_units = nullptr;
+  WsTile* d_tiles = nullptr;
 };
 
 // weighted-vector chunk table (H6): contiguous chunk [start, start+len) carries weight w
@@ -147,11 +172,6 @@ struct VecChunk {
 // MB waits for, so vectors up to 1 Mi elements get 1024-element chunks, up to 4 Mi 2048; HBM-sized vectors keep 8192 (fewer CTAs
 // and partials).  One-site sweep at chi = 4096: 0.393 / 0.375 / 0.369 / 0.362 / 0.358 s with 8192 / 4096 / 2048 / 1024 / 512.
 inline int vec_chunk_len(int64_t nelem) {
-  static const int forced = [] {
-    const char* e = getenv("FH_VEC_CHUNK");  // A/B timing only
-    return e && e[0] ? atoi(e) : 0;
-  }();
-  if (forced >= 256) return forced;
   return nelem > ((int64_t)4 << 20) ? 8192 : (nelem > ((int64_t)1 << 20) ? 2048 : 1024);
 }
 
@@ -198,6 +218,34 @@ inline void launch_pdl(int role, void (*kern)(KArgs...), int grid, int block, cu
 // ----------------------------------------------------------------------------- kernel launchers (kernels.cu)
 void launch_grouped_gemm(const Stage& st, const cplx* A, const cplx* B, cplx* C, cudaStream_t s,
                          int64_t* launch_counter, int pdl_role = 32 /* PDL_GEMM_OTHER */);
+// warp-specialised persistent form (zgemm_ws.cu): d_counters = two zero-initialised unsigned (tile queue head,
+// retired CTAs) that the kernel leaves at zero; grid = number of persistent CTAs (one per SM)
+const int WS_SLOT_ELEMS = 4096;  // accumulators of one tile: 4 warps x 16 sub-tiles x 2 x 32 lanes
+// scratch: n_slots * WS_SLOT_ELEMS elements; flags: n_slots counters, zero before the first launch, which the
+// parts of launch number `epoch` (1, 2, ...) raise to 4 * epoch
+void launch_grouped_gemm_ws(const Stage& st, const cplx* A, const cplx* B, cplx* C, unsigned* d_counters, int grid,
+                            cplx* scratch, unsigned* flags, unsigned epoch, cudaStream_t s, int64_t* launch_counter);
+// Two dependent stages (stage 2 reads C1 as its A or B operand) in ONE launch: tile queue = stage-1 tiles then
+// stage-2 tiles; a stage-2 tile starts when the stage-1 panels it reads are complete (device counters).
+struct WsPair {
+  std::vector<WsTile> tiles;      // stage-1 tiles, then stage-2 tiles (segment indices into the joint array)
+  std::vector<GemmSeg> segs;      // stage-1 segments, then stage-2 segments
+  std::vector<int> dep_id;        // flattened dependency lists of the stage-2 tiles: stage-1 merged-output ids
+  std::vector<unsigned> dep_target;  // arrivals per launch that complete that output (4 warps x its tiles)
+  int n_dep_counters = 0;         // = number of stage-1 merged outputs
+  int n_slots = 0;
+  int conj1 = 0, conj2 = 0;
+  WsTile* d_tiles = nullptr;
+  GemmSeg* d_segs = nullptr;
+  int* d_dep_id = nullptr;
+  unsigned* d_dep_target = nullptr;
+};
+// which operand of stage 2 is stage 1's result: 0 = A (lhs), 1 = B (rhs)
+void link_stages(const Stage& st1, const Stage& st2, int mid_is_rhs2, WsPair& out);
+void launch_grouped_gemm_ws_pair(const WsPair& pr, const cplx* A1, const cplx* B1, cplx* C1, const cplx* A2, const cplx* B2,
+                                 cplx* C2, unsigned* d_counters, int grid, cplx* scratch, unsigned* flags,
+                                 unsigned* dep_counters, unsigned epoch, cudaStream_t s, int64_t* launch_counter);
+int ws_smem_bytes();
 void launch_wdot(const VecChunk* d_chunks, int nchunks, const cplx* x, const cplx* y, double* d_partial,
                  double* d_result, cudaStream_t s, int64_t* launch_counter);
 // y = y + a*x (a complex, from device scalar array coef[idx]*sign) etc.: see kernels.cu

@@ -10,15 +10,7 @@
 
 namespace fh {
 
-bool pdl_enabled(int role) {
-  static const int mask = [] {
-    const char* off = std::getenv("FH_NO_PDL");
-    if (off && off[0] && off[0] != '0') return 0;
-    const char* m = std::getenv("FH_PDL_MASK");
-    return m && m[0] ? std::atoi(m) : PDL_DEFAULT_MASK;
-  }();
-  return (mask & role) != 0;
-}
+bool pdl_enabled(int role) { return (PDL_DEFAULT_MASK & role) != 0; }
 
 // ------------------------------------------------------------------------------------------
 // PTX wrappers

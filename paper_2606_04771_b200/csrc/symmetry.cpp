@@ -242,17 +242,9 @@ static void emit_units(Stage& st) {
   // else the stage lasts as long as its few heaviest units (one-site apply at chi = 4096: 82 -> 71 us with the
   // cap lowered from 3072 to 1024, the chi = 1024 apply 61 -> 32 us with 256, while the two-site apply at chi = 4096,
   // 4.1e6 DMMAs per stage, is fastest at 3072).
-  static const int64_t cap_floor = [] {
-    const char* e = getenv("FH_UNIT_CAP_FLOOR");  // A/B timing only
-    return (int64_t)(e && e[0] ? atoi(e) : 256);
-  }();
+  const int64_t cap_floor = 256;
   const int64_t fair = 2 * (total16 / (148 * 8));  // twice the even share: measured best at chi = 1024, 4096 (one- and two-site)
-  static const int64_t forced_cap = [] {
-    const char* e = getenv("FH_UNIT_CAP");  // A/B timing only: a fixed base cap instead of the fair-share rule
-    return (int64_t)(e && e[0] ? atoi(e) : 0);
-  }();
-  const int64_t base_cap =
-      forced_cap > 0 ? forced_cap : std::min<int64_t>(GEMM_UNIT_DMMA_CAP, std::max<int64_t>(cap_floor, fair));
+  const int64_t base_cap = std::min<int64_t>(GEMM_UNIT_DMMA_CAP, std::max<int64_t>(cap_floor, fair));
   const int64_t cap = std::max<int64_t>(base_cap, total16 / (148 * 8 * 6));
   for (size_t oi = 0; oi < st.mouts.size(); ++oi) {
     const GemmOut& o = st.mouts[oi];
@@ -302,6 +294,129 @@ static void emit_units(Stage& st) {
   for (auto& o : ord) st.units.push_back(v[o.second].u);
 }
 
+// Tile decomposition for the warp-specialised kernel (zgemm_ws.cu).  Every (merged) output is cut into a grid
+// of tiles of h x w sub-tiles of 8 x 8 (h, w <= 8; a group of 2 x 2 warps takes one tile, every warp at most
+// 4 x 4 sub-tiles), as evenly as the sub-tile counts allow -- tile SHAPES stay as large as the block allows,
+// because a warp's efficiency rests on its register tile.  Balance comes from splitting along k instead: a
+// tile heavier than the cap (a fraction of the even share of one of the 2 x 148 groups) is cut into parts at
+// chunk boundaries (16 k); all parts but the one that starts at k = 0 leave their accumulators in a scratch
+// slot, and that one adds them in slot order and stores the block (fixed order: deterministic).  In the queue
+// the parts of a tile come before its finishing part, so a finisher never waits for work not yet handed out.
+static void emit_tiles(Stage& st) {
+  st.tiles.clear();
+  st.n_slots = 0;
+  st.mout_tiles.assign(st.mouts.size(), 0);
+  int64_t total = 0;
+  for (const GemmOut& o : st.mouts) total += (int64_t)4 * ((o.M + 7) / 8) * ((o.N + 7) / 8) * std::max(1, o.steps);
+  // cap = the even share of one group: measured at chi = 4096 / 8192, smaller caps (more, k-split tiles) cost
+  // more in partial-sum traffic and tile switches than they gain in balance
+  const int64_t cap = std::max<int64_t>(2048, total / 296);
+  struct TW {
+    WsTile t;
+    int64_t key;  // sort key: work of the heaviest part of the (split) tile
+    int uid, rank;
+  };
+  std::vector<TW> v;
+  int uid = 0;
+  std::vector<int> cseg, ck;  // chunk -> (segment, k offset)
+  for (const GemmOut& o : st.mouts) {
+    if (o.M <= 0 || o.N <= 0) continue;
+    const int M8 = (o.M + 7) / 8, N8 = (o.N + 7) / 8;
+    const int gh = (M8 + 7) / 8, gw = (N8 + 7) / 8;
+    cseg.clear();
+    ck.clear();
+    for (int sgi = o.seg_begin; sgi < o.seg_end; ++sgi)
+      for (int k = 0; k < st.segs[sgi].K; k += 16) {
+        cseg.push_back(sgi);
+        ck.push_back(k);
+      }
+    const int nch = (int)cseg.size();
+    int m8 = 0;
+    for (int i = 0; i < gh; ++i) {
+      const int h = M8 / gh + (i < M8 % gh ? 1 : 0);
+      int n8 = 0;
+      for (int j = 0; j < gw; ++j) {
+        const int w = N8 / gw + (j < N8 % gw ? 1 : 0);
+        if (h > 0 && w > 0) {
+          const int64_t work = (int64_t)4 * h * w * std::max(1, o.steps);
+          int P = (int)std::min<int64_t>(8, (work + cap - 1) / cap);
+          P = std::max(1, std::min(P, nch / 2));  // at least two chunks per part
+          WsTile base = WsTile{o.c_off, o.ldc, o.M, o.N, m8 * 8, n8 * 8, h, w, o.seg_begin, o.seg_end, o.steps,
+                               o.seg_end > o.seg_begin ? st.segs[o.seg_begin] : GemmSeg{0, 0, 0, 0, 0, 0, 0, 0, 0.0},
+                               0, 1 << 30, 0, 0, 0, 0, 0, 0};
+          base.stage_sig = ((int)(&o - &st.mouts[0]) + 1) << 1;  // stage bit set by link_stages
+          const int slot0 = st.n_slots;
+          int64_t key = 0;
+          std::vector<TW> parts;
+          for (int p = 0; p < P; ++p) {
+            const int cb = (int)((int64_t)nch * p / P), ce = (int)((int64_t)nch * (p + 1) / P);
+            TW x;
+            x.t = base;
+            int steps = o.steps;
+            if (P > 1) {
+              x.t.seg_begin = cseg[cb];
+              x.t.k_begin = ck[cb];
+              x.t.seg_end = cseg[ce - 1] + 1;
+              x.t.k_end = ck[ce - 1] + 16;  // clipped to the segment's K by the producer
+              x.t.first = st.segs[x.t.seg_begin];
+              steps = 0;
+              for (int c = cb; c < ce; ++c) steps += (std::min(16, st.segs[cseg[c]].K - ck[c]) + 3) / 4;
+              x.t.steps = steps;
+              if (p == 0) {
+                x.t.kind = 0;
+                x.t.slot = slot0;
+                x.t.nparts = P - 1;
+              } else {
+                x.t.kind = 1;
+                x.t.slot = slot0 + p - 1;
+                x.t.nparts = 0;
+              }
+            }
+            x.t.nparts |= std::max(1, ce - cb) << 8;  // chunks of this part (a block without segments has one)
+            // arrangement of the group's four warps on the tile: the one whose largest part is smallest
+            // (0: 2 x 2 quadrants, 1: four column strips, 2: four row strips; a part is at most 16 sub-tiles)
+            const int part22 = ((h + 1) / 2) * ((w + 1) / 2);
+            const int partc = h * ((w + 3) / 4), partr = ((h + 3) / 4) * w;
+            int arr = 0, part = part22;
+            if ((w + 3) / 4 <= 2 && partc < part) {
+              arr = 1;
+              part = partc;
+            }
+            if ((h + 3) / 4 <= 2 && partr < part) {
+              arr = 2;
+              part = partr;
+            }
+            x.t.kind |= arr << 2;
+            // a tile lasts as long as its largest part
+            key = std::max<int64_t>(key, (int64_t)part * std::max(1, steps));
+            x.uid = uid;
+            x.rank = p == 0 ? P : p;  // the finishing part (p = 0) goes last
+            parts.push_back(x);
+          }
+          if (P > 1) st.n_slots += P - 1;
+          ++st.mout_tiles[&o - &st.mouts[0]];  // one storing tile (the finishing part of a split one)
+          for (TW& x : parts) {
+            x.key = key;
+            v.push_back(x);
+          }
+          ++uid;
+        }
+        n8 += w;
+      }
+      m8 += h;
+    }
+  }
+  std::vector<int> ord(v.size());
+  for (size_t i = 0; i < v.size(); ++i) ord[i] = (int)i;
+  std::sort(ord.begin(), ord.end(), [&](int a, int b) {
+    if (v[a].key != v[b].key) return v[a].key > v[b].key;
+    if (v[a].uid != v[b].uid) return v[a].uid < v[b].uid;
+    return v[a].rank < v[b].rank;
+  });
+  st.tiles.reserve(v.size());
+  for (int i : ord) st.tiles.push_back(v[i].t);
+}
+
 // Outputs that lie side by side in one row panel (N direction) or one below the other (M direction) and
 // whose segment lists describe the same GEMM on adjacent operand columns / rows are ONE wider / taller GEMM:
 // the merged output keeps the segment list of its first member (the kernel addresses operands by offset and
@@ -310,8 +425,14 @@ static void emit_units(Stage& st) {
 static void merge_outs(Stage& st, int64_t lhs_nelem, int64_t rhs_nelem) {
   st.mouts.clear();
   st.mouts.reserve(st.outs.size());
-  for (const GemmOut& o : st.outs)
-    if (o.M > 0 && o.N > 0) st.mouts.push_back(o);
+  std::vector<std::vector<int>> members;  // original output blocks of every entry of mouts
+  for (size_t oi = 0; oi < st.outs.size(); ++oi) {
+    const GemmOut& o = st.outs[oi];
+    if (o.M > 0 && o.N > 0) {
+      st.mouts.push_back(o);
+      members.push_back(std::vector<int>(1, (int)oi));
+    }
+  }
   for (int dir = 0; dir < 2; ++dir) {  // 0: N direction, 1: M direction
     std::vector<GemmOut>& v = st.mouts;
     std::unordered_map<int64_t, int> by_off;
@@ -346,15 +467,24 @@ static void merge_outs(Stage& st, int64_t lhs_nelem, int64_t rhs_nelem) {
         if (!ok) break;
         if (dir == 0) o.N += p.N;
         else o.M += p.M;
+        members[i].insert(members[i].end(), members[j].begin(), members[j].end());
         dead[j] = 1;
       }
     }
     std::vector<GemmOut> kept;
+    std::vector<std::vector<int>> keptm;
     kept.reserve(v.size());
     for (size_t i = 0; i < v.size(); ++i)
-      if (!dead[i]) kept.push_back(v[i]);
+      if (!dead[i]) {
+        kept.push_back(v[i]);
+        keptm.push_back(std::move(members[i]));
+      }
     v.swap(kept);
+    members.swap(keptm);
   }
+  st.out_mout.assign(st.outs.size(), -1);
+  for (size_t m = 0; m < members.size(); ++m)
+    for (int oi : members[m]) st.out_mout[oi] = (int)m;
   // every merged GEMM stays inside its operand tensors (same proof as for the single blocks)
   for (const GemmOut& o : st.mouts)
     for (int t = o.seg_begin; t < o.seg_end; ++t) {
@@ -364,6 +494,58 @@ static void merge_outs(Stage& st, int64_t lhs_nelem, int64_t rhs_nelem) {
       const int64_t b_last = sg.b_off + (int64_t)(sg.K - 1) * sg.b_sk + (int64_t)(o.N - 1) * sg.b_sn;
       if (a_last >= lhs_nelem || b_last >= rhs_nelem) throw std::runtime_error("task list: merged operand exceeds its tensor");
     }
+}
+
+// Joint tile queue of two dependent stages for ONE launch of the warp-specialised kernel (WsPair): stage-1 tiles
+// (heaviest first), then stage-2 tiles (heaviest first).  A stage-2 tile lists the stage-1 merged outputs that
+// hold the blocks its segments read (as lhs, or as rhs when mid_is_rhs2); it may start once each of them has
+// collected 4 arrivals (the four warps of a group) per storing tile.
+void link_stages(const Stage& st1, const Stage& st2, int mid_is_rhs2, WsPair& pr) {
+  pr.tiles.clear();
+  pr.segs = st1.segs;
+  pr.segs.insert(pr.segs.end(), st2.segs.begin(), st2.segs.end());
+  pr.dep_id.clear();
+  pr.dep_target.clear();
+  pr.n_dep_counters = (int)st1.mouts.size();
+  pr.n_slots = st1.n_slots + st2.n_slots;
+  pr.conj1 = st1.opA != OPA_N;
+  pr.conj2 = st2.opA != OPA_N;
+  pr.tiles.reserve(st1.tiles.size() + st2.tiles.size());
+  for (const WsTile& t : st1.tiles) pr.tiles.push_back(t);  // stage bit 0, sig as emitted
+  // dependency list of every stage-2 merged output
+  const int nseg1 = (int)st1.segs.size();
+  std::vector<int> dbeg(st2.mouts.size(), 0), dcnt(st2.mouts.size(), 0);
+  std::vector<std::vector<int>> deps(st2.mouts.size());
+  for (size_t o = 0; o < st2.outs.size(); ++o) {
+    const int m = st2.out_mout[o];
+    if (m < 0) continue;
+    for (int t = st2.outs[o].seg_begin; t < st2.outs[o].seg_end; ++t) {
+      const int z = mid_is_rhs2 ? st2.t_rhs[t] : st2.t_lhs[t];
+      const int zm = st1.out_mout[z];
+      if (zm >= 0) deps[m].push_back(zm);
+    }
+  }
+  for (size_t m = 0; m < deps.size(); ++m) {
+    std::sort(deps[m].begin(), deps[m].end());
+    deps[m].erase(std::unique(deps[m].begin(), deps[m].end()), deps[m].end());
+    dbeg[m] = (int)pr.dep_id.size();
+    dcnt[m] = (int)deps[m].size();
+    for (int zm : deps[m]) {
+      pr.dep_id.push_back(zm);
+      pr.dep_target.push_back(4u * (unsigned)st1.mout_tiles[zm]);
+    }
+  }
+  for (const WsTile& t0 : st2.tiles) {
+    WsTile t = t0;
+    const int m = (t.stage_sig >> 1) - 1;
+    t.stage_sig = 1;  // stage 2, nothing to signal
+    t.seg_begin += nseg1;
+    t.seg_end += nseg1;
+    t.slot += st1.n_slots;
+    t.dep_begin = dbeg[m];
+    t.dep_count = dcnt[m];
+    pr.tiles.push_back(t);
+  }
 }
 
 void finalize_stage(Stage& st, const BlockTensor& out, const BlockTensor& lhs, const BlockTensor& rhs) {
@@ -434,6 +616,7 @@ void finalize_stage(Stage& st, const BlockTensor& out, const BlockTensor& lhs, c
   if (t != nt) throw std::runtime_error("task list: tasks not sorted by output id");
   merge_outs(st, lhs.nelem, rhs.nelem);
   emit_units(st);
+  emit_tiles(st);
 }
 
 namespace {

@@ -516,7 +516,7 @@ const void* stage_small_desc(fh_ctx* ctx, const void* src, size_t bytes) {
 void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* buf, double* dS, bool qr = false) {
   if (ctx->svd_workers.empty()) {
     int nw = (int)std::thread::hardware_concurrency() - 1;
-    if (const char* e = std::getenv("FH_SVD_THREADS")) nw = std::atoi(e);
+    if (ctx->opt_svd_threads > 0) nw = ctx->opt_svd_threads;
     nw = std::max(1, std::min(nw, 12));
     ctx->svd_workers.resize(nw);
     for (auto& w : ctx->svd_workers) {
@@ -539,17 +539,11 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
   std::vector<SmallQr> small_qr;
   size_t small_smem = 0, small_qr_smem = 0;
   int64_t mid_v_total = 0;
-  // FH_SVD_MID_MAXN (read at every call, so that a test can compare the two routes in one process): 0 sends
-  // every matrix above the shared-memory route to cuSOLVER
-  const char* mid_env = std::getenv("FH_SVD_MID_MAXN");
+  // fh_set_option(FH_OPT_SVD_MID_MAXN): 0 sends every matrix above the shared-memory route to cuSOLVER;
   // default 128: 64 column pairs per tournament round = two per warp of the 32-warp CTA
-  const int mid_req = mid_env && mid_env[0] ? std::atoi(mid_env) : 128;
-  const int mid_maxn = std::max(0, std::min(mid_req, MID_SVD_HARD_MAXN));
+  const int mid_maxn = std::max(0, std::min(ctx->opt_svd_mid_maxn, MID_SVD_HARD_MAXN));
   const double mid_work = 1.5 * mid_maxn * (double)mid_maxn * mid_maxn;  // m n^2 bound: a long thin matrix would make its one CTA the critical path
-  static const bool use_small_qr = [] {
-    const char* e = std::getenv("FH_SMALL_QR");  // "0" sends every one-site split to cuSOLVER
-    return !(e && e[0] == '0');
-  }();
+  const bool use_small_qr = true;
   for (size_t i = 0; i < order.size(); ++i) {
     const int m = std::max(order[i]->nrow, order[i]->ncol), n = order[i]->k;
     if (!qr && small_svd_bytes(m, n) <= SMALL_SVD_SMEM) {
@@ -998,6 +992,8 @@ static void plan_zero_site(fh_ctx* ctx, fh_mps* mps, int bond, const BlockTensor
                            const BlockTensor& Cl) {
   Plan& P = ctx->plan;
   ctx->free_tensor(P.Z);
+  if (P.ws_scratch >= 0) ctx->alloc.release(P.ws_scratch, P.ws_scratch_n);
+  P.ws_scratch = -1;
   P.valid = false;
   P.io_ready = false;
   P.nsite = 0;
@@ -1037,9 +1033,13 @@ static void plan_zero_site(fh_ctx* ctx, fh_mps* mps, int bond, const BlockTensor
     }
   }
   ctx->alloc_tensor(P.Z);
+  P.ws_scratch_n = (int64_t)(P.st1.n_slots + P.st2.n_slots) * WS_SLOT_ELEMS;
+  if (P.ws_scratch_n > 0) P.ws_scratch = ctx->alloc.alloc(P.ws_scratch_n);
   P.Lptr = ctx->ptr(Le.base);
   P.Rptr = ctx->ptr(Re.base);
-  const size_t need = stage_bytes(P.st1) + stage_bytes(P.st2) + P.chunks.size() * (sizeof(VecChunk) + 16) + 8192;
+  link_stages(P.st1, P.st2, 0, P.pair);  // stage 2 reads the intermediate as its left operand
+  const size_t need = stage_bytes(P.st1) + stage_bytes(P.st2) + pair_bytes(P.pair) +
+                      P.chunks.size() * (sizeof(VecChunk) + 16) + 8192;
   P.pool.reserve(need, ctx->stream);
   upload_stage(P.pool, P.st1, ctx->stream);
   upload_stage(P.pool, P.st2, ctx->stream);
@@ -1049,6 +1049,15 @@ static void plan_zero_site(fh_ctx* ctx, fh_mps* mps, int bond, const BlockTensor
   P.d_scal = (double*)P.pool.take(256 * sizeof(double));
   P.d_counter = (unsigned*)P.pool.take(sizeof(unsigned));
   FH_CUDA(cudaMemsetAsync(P.d_counter, 0, sizeof(unsigned), ctx->stream));
+  upload_pair(P.pool, P.pair, ctx->stream);
+  {
+    const size_t nf = (size_t)P.pair.n_slots + 1, nd = (size_t)P.pair.n_dep_counters + 1;
+    P.d_ws_flags = (unsigned*)P.pool.take(nf * sizeof(unsigned));
+    P.d_ws_dep = (unsigned*)P.pool.take(nd * sizeof(unsigned));
+    FH_CUDA(cudaMemsetAsync(P.d_ws_flags, 0, nf * sizeof(unsigned), ctx->stream));
+    FH_CUDA(cudaMemsetAsync(P.d_ws_dep, 0, nd * sizeof(unsigned), ctx->stream));
+  }
+  P.ws_epoch = 0;
   P.valid = true;
 }
 

@@ -206,9 +206,76 @@ def test_apply_parity_table_s2_shape_random_envs(H, ctx, den):
     ctx.mps_destroy(mps)
 
 
-@pytest.mark.parametrize("chi,nsample", [(4096, 40), (16384, 12)])
+def _per_block_worst(got, ref):
+    worst = 0.0
+    for k, v in ref.items():
+        worst = max(worst, np.linalg.norm(got[k] - v) / max(np.linalg.norm(v), 1e-300))
+    return worst
+
+
+@pytest.mark.parametrize("chi,path", [(4096, 1), (4096, 2), (1024, 2)])
+def test_config3_full_size_all_blocks_both_gemm_forms(H, chi, path):
+    """BASELINE config 3 (chi = 4096: the workload and plan bench.py times) and config 2 (chi = 1024), complete:
+    the environments L_29, R_31 are contracted on both sides independently from the seeded canonical chain (29
+    chained H4 / H5 updates at full block size: blocks that span several units / tiles), then ALL output blocks of
+    the two-site apply (H1 + H2), of the one-site apply on site 30 (H3) and of one more right-environment update
+    (H5) are compared with the oracle, per block and globally, relative Frobenius <= 1e-11.  `path` forces the
+    form of the grouped ZGEMM heff_apply uses (fh_set_option): 1 = warp units, two launches; 2 = warp-specialised
+    single launch with cross-stage dependency counters and k-split tiles."""
+    L, c = 60, 29
+    o = central_bond(chi, L)
+    dims, W = o["dims"], o["W"]
+    ctx = H.binding.Context(int(max(1 << 30, 64.0 * chi * chi)))
+    try:
+        ctx.fh_set_option(ctx.OPT_GEMM_PATH, path)
+        mpo = ctx.fh_mpo_build(L, 1.0, 4.0)
+        mps, gdims = H.build_central_bond(ctx, mpo, chi, L)
+        assert [gdims[k] for k in (c, c + 1, c + 2)] == [dims[k] for k in (c, c + 1, c + 2)]
+        for which, bond, ref in ((0, c, o["Lenv"]), (1, c + 2, o["Renv"])):
+            lab, dm, flat = ctx.env_get(mps, which, bond)
+            got = H.unflatten(flat, lab, dm, env_key)
+            assert sorted(got) == sorted(ref)
+            assert rel_err(got, ref, weighted=False) < 1e-11 and _per_block_worst(got, ref) < 1e-10
+        # two-site apply, every block
+        th = fi.theta_random(fi.SEED, c, dims[c], dims[c + 2])
+        ref = symm.heff2_apply(o["Lenv"], o["Renv"], th, W[c], W[c + 1])
+        ctx.heff_plan(mpo, mps, c, 2)
+        assert ctx.heff_flops() == symm.heff2_flops(*symm.heff2_tasks(sorted(o["Lenv"]), sorted(o["Renv"]), sorted(th),
+                                                                       W[c], W[c + 1]), dims[c], dims[c + 2])
+        lab, dm, ne = ctx.heff_layout(2)
+        x = H.to_planned(ctx, H.flatten(th, lab, dm, H.theta_key))
+        y, y2 = _torch().empty_like(x), _torch().empty_like(x)
+        ctx.heff_apply(x, y)
+        ctx.heff_apply(2.0 * x, y2)
+        assert bool((y2 == 2.0 * y).all())                      # exact: scaling by 2 commutes with rounding
+        got = H.unflatten(H.from_planned(ctx, y), lab, dm, H.theta_key)
+        assert len(got) == len(ref) == len(lab)
+        e2, w2 = rel_err(got, ref), _per_block_worst(got, ref)
+        # one more right-environment update (site 30) and the one-site apply on site 30
+        Re30 = symm.env_update_right(o["Renv"], o["A"][c + 1], W[c + 1])
+        ctx.env_update_right(mpo, mps, c + 1)
+        lab, dm, flat = ctx.env_get(mps, 1, c + 1)
+        gotR = H.unflatten(flat, lab, dm, env_key)
+        eR = rel_err(gotR, Re30, weighted=False)
+        Le30 = symm.env_update_left(o["Lenv"], o["A"][c], W[c])
+        ctx.env_update_left(mpo, mps, c)
+        lab, dm, flat = ctx.env_get(mps, 0, c + 1)
+        eL = rel_err(H.unflatten(flat, lab, dm, env_key), Le30, weighted=False)
+        ref1 = symm.heff1_apply(o["Lenv"], Re30, o["A"][c], W[c])
+        ctx.heff_plan(mpo, mps, c, 1)
+        got1 = _apply_gpu(H, ctx, o["A"][c], 1)
+        e1, w1 = rel_err(got1, ref1), _per_block_worst(got1, ref1)
+        print("chi=%d path %d: two-site %d blocks global %.2e worst block %.2e; one-site %d blocks %.2e / %.2e; "
+              "env updates %.2e %.2e" % (chi, path, len(ref), e2, w2, len(ref1), e1, w1, eL, eR))
+        assert e2 < TOL_APPLY and w2 < TOL_APPLY and e1 < TOL_APPLY and w1 < TOL_APPLY and eL < 1e-11 and eR < 1e-11
+        ctx.mps_destroy(mps)
+    finally:
+        ctx.close()
+
+
+@pytest.mark.parametrize("chi,nsample", [(16384, 12)])
 def test_apply_parity_bench_sizes_sampled_blocks(H, chi, nsample):
-    """BASELINE config 3 (chi = 4096, the workload bench.py times) and config 4's size (chi = 16384) in
+    """Config 4's size (chi = 16384; chi = 4096 and 1024 are compared block by block in the test above) in
     the launch configuration of the bench (same sector profile, same plan, same unit lists; iid random
     environments through env_set so that no oracle input comes from the CUDA path).  The oracle computes
     sampled output blocks one by one (each output block is an independent sum over its own segments):
@@ -657,7 +724,7 @@ def test_mid_size_jacobi_kernel_vs_vendor_svd(H, ctx, tmp_path):
     """H9: sector matrices above the shared-memory route with at most 128 columns are factorised by the library's
     own global-memory Jacobi kernel (mid_svd_kernel, on a side stream beside the vendor routines).  The same L = 16
     state (grown by an untruncated quench until sector matrices of 90-128 columns exist) takes one two-site sweep
-    with that kernel and, from a reloaded copy, one with FH_SVD_MID_MAXN=0 (every such matrix through cusolver's
+    with that kernel and, from a reloaded copy, one with fh_set_option(FH_OPT_SVD_MID_MAXN, 0) (every such matrix through cusolver's
     gesvdp / gesvd): both routes must have run, the kept singular values of every bond agree to 1e-11 s_max, the
     sector tables are identical and the observables agree to 1e-10."""
     L, dt, m = 16, 0.1, 8
@@ -671,11 +738,11 @@ def test_mid_size_jacobi_kernel_vs_vendor_svd(H, ctx, tmp_path):
     f0 = ctx.fh_factorization_stats()
     ctx.tdvp2_sweep(mpo, a, dt, krylov_dim=m, chi_max_full=1200, eps_trunc=1e-12)
     f1 = ctx.fh_factorization_stats()
-    os.environ["FH_SVD_MID_MAXN"] = "0"
+    ctx.fh_set_option(ctx.OPT_SVD_MID_MAXN, 0)
     try:
         ctx.tdvp2_sweep(mpo, b, dt, krylov_dim=m, chi_max_full=1200, eps_trunc=1e-12)
     finally:
-        del os.environ["FH_SVD_MID_MAXN"]
+        ctx.fh_set_option(ctx.OPT_SVD_MID_MAXN, 128)
     f2 = ctx.fh_factorization_stats()
     assert f1["jacobi_mid_kernel"] - f0["jacobi_mid_kernel"] > 0, (f0, f1)
     assert f2["jacobi_mid_kernel"] == f1["jacobi_mid_kernel"]
