@@ -8,9 +8,10 @@ run).  None of the method's contractions (environments, H_eff, Lanczos, SVD spli
 coefficients or task lists live here; both the oracle-side tests and the CUDA-side harness
 consume the same numbers from this module and do everything else on their own.
 
-The only convention the gauge fixing has to know is the multiplet weight in the norm of a
-right-canonical tensor, sum_{s,b} (2 j_b + 1)/(2 j_c + 1) A[c,s,b] A[c,s,b]^dagger = 1, i.e.
-that a multiplet of spin j stands for 2j+1 states (Eq. (8)).
+The gauge fixing of the right half needs the metric under which a site tensor counts as
+right-canonical, sum_{s,b} w(c,b)^2 A[c,s,b] A[c,s,b]^dagger = 1.  That metric is a convention of the
+method (F-6) and is NOT defined here: the caller passes ``weight(c, b)`` -- the oracle-side tests take it
+from ``oracle/``, the CUDA-side harness from the library -- and this module only applies it.
 """
 from math import sqrt
 
@@ -51,16 +52,16 @@ def left_canonical(A, dims_l, dims_r):
     return dict(sorted(out.items())), dict(sorted(new_r.items()))
 
 
-def right_canonical(A, dims_l, dims_r):
-    """Gauge-fix so that sum_{s,b} (2j_b+1)/(2j_c+1) A[c,s,b] A[c,s,b]^dagger = 1 for every
-    left sector c: concatenate the weighted blocks of that c side by side, take the Q factor of
-    the QR of the conjugate transpose, undo the weights."""
+def right_canonical(A, dims_l, dims_r, weight):
+    """Gauge-fix so that sum_{s,b} weight(c,b)^2 A[c,s,b] A[c,s,b]^dagger = 1 for every left sector c
+    (``weight`` is the caller's metric, see the module docstring): concatenate the weighted blocks of
+    that c side by side, take the Q factor of the QR of the conjugate transpose, undo the weights."""
     by_c = {}
     for k in sorted(A):
         by_c.setdefault(k[0], []).append(k)
     out, new_l = {}, {}
     for c, ks in by_c.items():
-        wts = [sqrt((k[2][1] + 1) / (c[1] + 1)) for k in ks]
+        wts = [float(weight(c, k[2])) for k in ks]
         M = np.concatenate([w * A[k] for k, w in zip(ks, wts)], axis=1)
         if M.shape[1] < M.shape[0]:
             continue
@@ -110,7 +111,7 @@ def theta_random(seed, site, dims_l, dims_r):
 
 
 def canonical_chain(chi, centre, L=60, seed=SEED, profile="gaussian", table_s2_scale=(1, 1),
-                    sites=None, dims=None):
+                    sites=None, dims=None, weight=None):
     """Generator of (site, A_site, dims_l, dims_r) for a random MPS, left-canonical on sites
     < centre and right-canonical on sites > centre + 1 (sites centre, centre+1 are plain random).
 
@@ -118,6 +119,8 @@ def canonical_chain(chi, centre, L=60, seed=SEED, profile="gaussian", table_s2_s
     that a consumer can stream environment updates without holding the chain (config 5).  QR
     can drop unsupported sectors from a bond; the dims yielded are the final ones, and the
     generator's ``dims`` list (returned through the ``dims`` argument if given) is updated."""
+    if weight is None:
+        raise ValueError("canonical_chain: the caller must pass weight(c, b), the metric of a right-canonical tensor")
     d = chain_dims(chi, L, profile, table_s2_scale) if dims is None else dims
     left = range(0, centre)
     right = range(L - 1, centre + 1, -1)
@@ -132,7 +135,7 @@ def canonical_chain(chi, centre, L=60, seed=SEED, profile="gaussian", table_s2_s
         if sites is not None and i not in sites:
             continue
         A = site_tensor(seed, i, d[i], d[i + 1])
-        A, new_l = right_canonical(A, d[i], d[i + 1])
+        A, new_l = right_canonical(A, d[i], d[i + 1], weight)
         d[i] = new_l
         yield i, A, d[i], d[i + 1]
     for i in (centre, centre + 1):

@@ -51,6 +51,7 @@ typedef struct fh_mps fh_mps;
  * All tensors (MPS, environments, Krylov vectors, scratch) live in this one HBM arena. */
 int fh_ctx_create(fh_ctx** out, void* cuda_stream, void* arena_dev, size_t arena_bytes);
 void fh_ctx_destroy(fh_ctx* ctx);
+/* message of the last failing call on ctx; with ctx = NULL: why the last fh_ctx_create of this thread failed */
 const char* fh_last_error(const fh_ctx* ctx);
 /* Options of a context (host-only; FH_EINVAL on a NULL context, an unknown key or a value out of range).
  *   FH_OPT_GEMM_PATH     which form of the grouped ZGEMM heff_apply uses for two-site plans: 0 = the library
@@ -61,10 +62,15 @@ const char* fh_last_error(const fh_ctx* ctx);
  *   FH_OPT_SVD_MID_MAXN  widest sector matrix (columns) the library's own global-memory Jacobi kernel takes
  *                        instead of the vendor SVD, 0 .. 256 (default 128; 0 = none).
  *   FH_OPT_SVD_THREADS   host threads that drive the vendor SVD / QR routines, 1 .. 12 (default: cores - 1,
- *                        at most 12); takes effect before the first factorisation of the context. */
+ *                        at most 12); takes effect before the first factorisation of the context.
+ *   FH_OPT_SVD_SMALL_MAXN widest sector matrix (columns) the shared-memory Jacobi / Householder kernels take, provided
+ *                        it fits their shared memory, 0 .. 4096 (default 4096 = whatever fits; 0 = none: every
+ *                        matrix goes to the next route).  With FH_OPT_SVD_MID_MAXN this lets a test send small
+ *                        matrices through every factorisation route. */
 #define FH_OPT_GEMM_PATH 1
 #define FH_OPT_SVD_MID_MAXN 2
 #define FH_OPT_SVD_THREADS 3
+#define FH_OPT_SVD_SMALL_MAXN 4
 int fh_set_option(fh_ctx* ctx, int key, int value);
 /* bytes currently allocated / high-water mark in the arena */
 int fh_arena_stats(const fh_ctx* ctx, size_t* used_bytes, size_t* peak_bytes);
@@ -263,6 +269,9 @@ int fh_dmma_peak_tflops(fh_ctx* ctx, int reps, double* tflops);
  * the path. */
 int fh_vec_kernels_gbs(fh_ctx* ctx, int64_t n_elems, int m, int reps, double* gbs);
 
+/* F-6: w(c,b) = sqrt((2 j_b + 1) / (2 j_c + 1)), the weight under which a site tensor A[c,s,b] is right-canonical,
+ * sum_{s,b} w^2 A A^H = 1 (doubled spins tjc, tjb).  Host only. */
+double fh_canonical_weight(int tjc, int tjb);
 /* ---- host-only entry points (no CUDA call inside): the symmetry layer on its own -----------
  * Closed-form recoupling coefficients of reading F-5 (all arguments doubled spins):
  *   coefL(a,s,c; k,r,k'; a',s',c') = sqrt((2c+1)(2k'+1)(2a'+1)(2s'+1)) {a s c; k r k'; a' s' c'}

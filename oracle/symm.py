@@ -488,6 +488,12 @@ def inner(x, y):
     return tot
 
 
+def canonical_weight(c, b):
+    """F-6: a site tensor A[c,s,b] is right-canonical when sum_{s,b} w(c,b)^2 A A^dagger = 1 with
+    w(c,b)^2 = (2 j_b + 1) / (2 j_c + 1): a multiplet of spin j stands for 2j+1 states (Eq. (8))."""
+    return np.sqrt((b[1] + 1) / (c[1] + 1))
+
+
 def boundary_left():
     return {((0, 0), 0, (0, 0)): np.ones((1, 1), dtype=complex)}
 

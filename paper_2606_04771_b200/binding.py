@@ -32,6 +32,7 @@ _SIGS = {
     "fh_last_error": (C.c_char_p, [c_void_p]),
     "fh_arena_stats": (c_int, [c_void_p, P(c_size_t), P(c_size_t)]),
     "fh_set_option": (c_int, [c_void_p, c_int, c_int]),
+    "fh_canonical_weight": (c_dbl, [c_int, c_int]),
     "fh_mpo_build": (c_int, [c_void_p, c_int, c_dbl, c_dbl, P(c_void_p)]),
     "fh_mpo_destroy": (None, [c_void_p]),
     "fh_mpo_get_site": (c_int, [c_void_p, c_int, c_void_p, c_void_p]),
@@ -107,6 +108,11 @@ def _i32(x):
 
 
 # ------------------------------------------------------------------ host-only entry points
+def fh_canonical_weight(c, b):
+    """Metric of a right-canonical site tensor as the LIBRARY defines it (labels (q, tj))."""
+    return lib.fh_canonical_weight(int(c[1]), int(b[1]))
+
+
 def fh_coef_left(*t):
     return lib.fh_coef_left(*[int(x) for x in t])
 
@@ -421,7 +427,7 @@ class Context:
     def fh_launch_count(self):
         return int(lib.fh_launch_count(self.h))
 
-    OPT_GEMM_PATH, OPT_SVD_MID_MAXN, OPT_SVD_THREADS = 1, 2, 3
+    OPT_GEMM_PATH, OPT_SVD_MID_MAXN, OPT_SVD_THREADS, OPT_SVD_SMALL_MAXN = 1, 2, 3, 4
 
     def fh_set_option(self, key, value):
         self.check(lib.fh_set_option(self.h, int(key), int(value)), "fh_set_option")

@@ -11,34 +11,37 @@ SOURCES = ["zgemm.cu", "zgemm_ws.cu", "kernels.cu", "api.cu", "tdvp.cu", "symmet
 HEADERS = ["fh_internal.hpp", "symmetry.hpp", "context.hpp"]
 
 
-def needs_build():
-    if not os.path.exists(LIB):
-        return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.join(ROOT, "include", "fh_b200.h")]
-    return any(os.path.getmtime(d) > t for d in deps)
+def source_digest():
+    """Hash of every source, header and compile flag that goes into the library."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in SOURCES + HEADERS:
+        h.update(open(os.path.join(CSRC, f), "rb").read())
+    h.update(open(os.path.join(ROOT, "include", "fh_b200.h"), "rb").read())
+    h.update(" ".join(NVCC_FLAGS).encode())
+    return h.hexdigest()
 
 
-TRACE_LIB = os.path.join(HERE, "libfh_b200_trace.so")
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC"]
+STAMP = os.path.join(HERE, "build", "libfh_b200.sha256")
 
 
-def build(force=False, verbose=False, trace=False):
-    """trace=True builds libfh_b200_trace.so instead: the same library with -DFH_UNIT_TRACE (every GEMM unit
-    stamps its begin/end time, SM and warp slot; used by unit_timeline.py, never by tests or bench)."""
-    lib = TRACE_LIB if trace else LIB
-    if not trace and not force and not needs_build():
+def build(force=False, verbose=False):
+    """Compile every CUDA / C++ source for sm_100a and link libfh_b200.so in-tree.  The library is rebuilt unless
+    a stamp written by THIS build procedure says that the .so on disk was made from exactly the present sources
+    and flags (a .so that merely looks newer than the sources, e.g. one shipped from another machine, is not
+    trusted)."""
+    digest = source_digest()
+    if not force and os.path.exists(LIB) and os.path.exists(STAMP) and open(STAMP).read().strip() == digest:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     objs = []
     os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
     procs = []
     for src in SOURCES:
-        obj = os.path.join(HERE, "build", src + (".trace.o" if trace else ".o"))
-        cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-               "-Xcompiler", "-fPIC", "-x", "cu", "-I", os.path.join(ROOT, "include"), "-I", CSRC,
-               "-c", os.path.join(CSRC, src), "-o", obj]
-        if trace:
-            cmd.insert(1, "-DFH_UNIT_TRACE")
+        obj = os.path.join(HERE, "build", src + ".o")
+        cmd = [nvcc] + NVCC_FLAGS + ["-x", "cu", "-I", os.path.join(ROOT, "include"), "-I", CSRC,
+                                     "-c", os.path.join(CSRC, src), "-o", obj]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         procs.append((src, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
@@ -49,13 +52,15 @@ def build(force=False, verbose=False, trace=False):
             raise RuntimeError("nvcc failed on %s:\n%s" % (src, out))
         if verbose and out:
             print(out)
-    cmd = [nvcc, "-shared", "-o", lib] + objs + ["-L/usr/local/cuda/lib64", "-lcusolver", "-lcublas",
+    cmd = [nvcc, "-shared", "-o", LIB] + objs + ["-L/usr/local/cuda/lib64", "-lcusolver", "-lcublas",
                                                   "-Xlinker", "-rpath=/usr/local/cuda/lib64"]
     r = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     if r.returncode != 0:
         raise RuntimeError("link failed:\n" + r.stdout)
-    return lib
+    with open(STAMP, "w") as f:
+        f.write(digest + "\n")
+    return LIB
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, trace="--trace" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

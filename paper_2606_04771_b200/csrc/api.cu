@@ -103,6 +103,7 @@ void fh_ctx::ensure_pinned(size_t n) {
   FH_CUDA(cudaMallocHost((void**)&h_pinned, h_pinned_n * sizeof(double)));
 }
 void fh_ctx::timer_begin(int cat) {
+  if (span_open) timer_end();  // a span left open by an exception: close it here so that both events exist
   span_open = timers_on;
   if (!timers_on) return;
   if (spans.size() > 8192) timers_resolve();
@@ -127,10 +128,12 @@ void fh_ctx::timer_end() {
 void fh_ctx::timers_resolve() {
   if (spans.empty()) return;
   FH_CUDA(cudaStreamSynchronize(stream));
+  if (span_open) timer_end();
+  FH_CUDA(cudaStreamSynchronize(stream));
   for (Span& sp : spans) {
     float ms = 0.f;
-    FH_CUDA(cudaEventElapsedTime(&ms, sp.a, sp.b));
-    sec[sp.cat] += ms * 1e-3;
+    if (cudaEventElapsedTime(&ms, sp.a, sp.b) == cudaSuccess) sec[sp.cat] += ms * 1e-3;
+    else cudaGetLastError();  // a span whose end was never recorded (error path): dropped, not fatal
     ev_free.push_back(sp.a);
     ev_free.push_back(sp.b);
   }
@@ -509,6 +512,7 @@ int fh::expm_lanczos(fh_ctx* ctx, cplx* theta, double tau, int m, double tol, cp
   auto fetch_scalars = [&]() {
     FH_CUDA(cudaMemcpyAsync(ctx->h_pinned, d_sc, nsc * sizeof(double), cudaMemcpyDeviceToHost, s));
     FH_CUDA(cudaStreamSynchronize(s));
+    check_fact_status(ctx);  // status words of the factorisations enqueued before this exponential
   };
   // reciprocal of b_j as the kernel takes it (0 below tol) from the fetched scalars
   auto recip_b = [&](int j) {
@@ -688,6 +692,9 @@ void fh::do_env_update_right(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int si
     return FH_EINVAL;                          \
   }
 
+// message of the last failed fh_ctx_create of this thread (there is no context to hold it): fh_last_error(NULL)
+static thread_local std::string g_create_error = "null context";
+
 extern "C" {
 
 int fh_ctx_create(fh_ctx** out, void* cuda_stream, void* arena_dev, size_t arena_bytes) {
@@ -715,6 +722,7 @@ int fh_ctx_create(fh_ctx** out, void* cuda_stream, void* arena_dev, size_t arena
       c->num_sms = prop.multiProcessorCount;
     }
   } catch (const std::exception& e) {
+    g_create_error = std::string("fh_ctx_create: ") + e.what();
     delete c;
     return FH_ECUDA;
   }
@@ -734,6 +742,8 @@ void fh_ctx_destroy(fh_ctx* c) {
   c->plan.pool.destroy();
   c->plan.io_pool.destroy();
   if (c->d_ws_counters) cudaFree(c->d_ws_counters);
+  if (c->d_fact_status) cudaFree(c->d_fact_status);
+  if (c->h_fact_status) cudaFreeHost(c->h_fact_status);
   c->pool_aux.destroy();
   c->pool_small.destroy();
   for (auto& w : c->svd_workers) {
@@ -754,7 +764,7 @@ void fh_ctx_destroy(fh_ctx* c) {
   delete c;
 }
 
-const char* fh_last_error(const fh_ctx* c) { return c ? c->err.c_str() : "null context"; }
+const char* fh_last_error(const fh_ctx* c) { return c ? c->err.c_str() : g_create_error.c_str(); }
 
 int fh_set_option(fh_ctx* c, int key, int value) {
   if (!c) return FH_EINVAL;
@@ -766,6 +776,10 @@ int fh_set_option(fh_ctx* c, int key, int value) {
     case FH_OPT_SVD_MID_MAXN:
       if (value < 0 || value > 256) return FH_EINVAL;
       c->opt_svd_mid_maxn = value;
+      return FH_OK;
+    case FH_OPT_SVD_SMALL_MAXN:
+      if (value < 0 || value > 4096) return FH_EINVAL;
+      c->opt_svd_small_maxn = value;
       return FH_OK;
     case FH_OPT_SVD_THREADS:
       if (value < 1 || value > 12) return FH_EINVAL;
@@ -893,8 +907,11 @@ int mps_save(fh_ctx* ctx, const fh_mps* mps, const char* path) {
   FH_TRY(ctx, {
     FH_REQUIRE(ctx && mps && path, FH_EINVAL, "mps_save: NULL argument");
     for (int i = 0; i < mps->L; ++i) FH_REQUIRE(mps->A[i].base >= 0, FH_ESTATE, "mps_save: site tensor missing");
-    FileCloser fc{std::fopen(path, "wb")};
-    FH_REQUIRE(fc.f, FH_EINVAL, std::string("mps_save: cannot open ") + path);
+    // written to path + ".tmp" and renamed once everything is on disk: a failed save never leaves a
+    // truncated file under the final name
+    const std::string tmp = std::string(path) + ".tmp";
+    FileCloser fc{std::fopen(tmp.c_str(), "wb")};
+    FH_REQUIRE(fc.f, FH_EINVAL, std::string("mps_save: cannot open ") + tmp);
     auto put = [&](const void* p, size_t n) {
       FH_REQUIRE(std::fwrite(p, 1, n, fc.f) == n, FH_EINVAL, "mps_save: short write");
     };
@@ -922,6 +939,13 @@ int mps_save(fh_ctx* ctx, const fh_mps* mps, const char* path) {
       const int64_t ne = t.nelem;
       put(&ne, 8);
       put(host.data(), (size_t)ne * sizeof(cplx));
+    }
+    const bool flushed = std::fflush(fc.f) == 0;
+    const bool closed = std::fclose(fc.f) == 0;
+    fc.f = nullptr;
+    if (!flushed || !closed || std::rename(tmp.c_str(), path) != 0) {
+      std::remove(tmp.c_str());
+      throw FhError(FH_EINVAL, std::string("mps_save: could not complete ") + path);
     }
   })
 }
@@ -953,7 +977,8 @@ int mps_load(fh_ctx* ctx, const fh_mpo* mpo, const char* path, fh_mps** out) {
         for (int32_t i = 0; i < n; ++i) {
           int32_t rec[3];
           get(rec, sizeof(rec));
-          FH_REQUIRE(rec[1] >= 0 && rec[2] >= 1, FH_EINVAL, "mps_load: bad sector record");
+          FH_REQUIRE(rec[1] >= 0 && rec[1] <= 250 && rec[2] >= 1 && rec[0] >= -1000 && rec[0] <= 1000, FH_EINVAL,
+                     "mps_load: bad sector record");
           if (i > 0) FH_REQUIRE(b.sec.back() < Sector({rec[0], rec[1]}), FH_EINVAL, "mps_load: sector labels not sorted");
           b.sec.push_back(Sector{rec[0], rec[1]});
           b.d.push_back(rec[2]);
@@ -987,7 +1012,8 @@ int mps_set_bond(fh_ctx* ctx, fh_mps* mps, int bond, int n, const int32_t* q, co
     FH_REQUIRE(mps && bond >= 0 && bond <= mps->L && n >= 1, FH_EINVAL, "mps_set_bond: bad argument");
     Bond b;
     for (int i = 0; i < n; ++i) {
-      FH_REQUIRE(tj[i] >= 0 && d[i] >= 1, FH_EINVAL, "mps_set_bond: tj >= 0 and d >= 1 required");
+      FH_REQUIRE(tj[i] >= 0 && tj[i] <= 250 && d[i] >= 1, FH_EINVAL, "mps_set_bond: 0 <= tj <= 250 and d >= 1 required");
+      FH_REQUIRE(q[i] >= -1000 && q[i] <= 1000, FH_EINVAL, "mps_set_bond: |q| <= 1000 required");
       FH_REQUIRE(((q[i] + tj[i] - bond) & 1) == 0, FH_EINVAL, "mps_set_bond: parity rule q + 2j = bond (mod 2) violated");
       if (i > 0) FH_REQUIRE(Sector({q[i - 1], tj[i - 1]}) < Sector({q[i], tj[i]}), FH_EINVAL, "mps_set_bond: labels must be sorted by (q, tj) and distinct");
       b.sec.push_back(Sector{q[i], tj[i]});
@@ -1615,6 +1641,8 @@ int fh_host_get_units(int stage, int* nunit, int32_t* units, int* nout, int32_t*
     }
   return FH_OK;
 }
+
+double fh_canonical_weight(int tjc, int tjb) { return std::sqrt((double)(tjb + 1) / (double)(tjc + 1)); }
 
 double fh_coef_left(int ta, int ts, int tc, int tk, int tr, int tkp, int tap, int tsp, int tcp) {
   return fh::coef_left(ta, ts, tc, tk, tr, tkp, tap, tsp, tcp);

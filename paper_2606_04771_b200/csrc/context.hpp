@@ -188,9 +188,16 @@ struct fh_ctx {
   int device = 0;
   int opt_gemm_path = 0;      // fh_set_option: 0 auto, 1 warp units, 2 warp-specialised
   int opt_svd_mid_maxn = 128;
+  int opt_svd_small_maxn = 4096;
   int opt_svd_threads = 0;    // 0 = default
   int num_sms = 148;
   unsigned* d_ws_counters = nullptr;  // tile-queue head and retired-CTA count of the warp-specialised GEMM (zero between launches)
+  // status words of the last batch of sector factorisations (one per matrix, + one more per matrix for the
+  // second vendor call of a QR): 0 = fine, otherwise a cuSOLVER devInfo or FACT_NOT_CONVERGED from a Jacobi kernel
+  int* d_fact_status = nullptr;
+  int* h_fact_status = nullptr;  // pinned
+  int fact_status_cap = 0, fact_status_n = 0;
+  bool fact_status_pending = false;
   int64_t svd_count[3] = {0, 0, 0};  // gesvd, gesvdp, gesvdp fallbacks to gesvd
   int64_t qr_small = 0;  // one-site splits done by small_qr_kernel
   int64_t svd_small = 0, qr_count = 0;  // sector matrices done by small_svd_kernel / by geqrf+ungqr
@@ -209,6 +216,16 @@ struct fh_ctx {
 };
 
 namespace fh {
+// arena scratch that is returned when the scope is left, also by an exception
+struct ArenaScratch {
+  fh_ctx* ctx;
+  int64_t off, n;
+  ArenaScratch(fh_ctx* c, int64_t nelem) : ctx(c), off(c->alloc.alloc(nelem)), n(nelem) {}
+  ~ArenaScratch() { ctx->alloc.release(off, n); }
+  ArenaScratch(const ArenaScratch&) = delete;
+  ArenaScratch& operator=(const ArenaScratch&) = delete;
+  cplx* ptr() const { return ctx->ptr(off); }
+};
 template <class T>
 T* upload(DevPool& pool, const std::vector<T>& v, cudaStream_t s) {
   if (v.empty()) return nullptr;
@@ -240,4 +257,6 @@ void do_env_update_right(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int site);
 void sweep(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh_params* p);
 void sweep1(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh_params* p);
 void measure_local_impl(fh_ctx* ctx, const fh_mps* mps, double* n_i, double* sz_i, double* docc_i);
+// throws FH_ECUDA if a factorisation of the last batch failed; call after the stream has been synchronised
+void check_fact_status(fh_ctx* ctx);
 }  // namespace fh

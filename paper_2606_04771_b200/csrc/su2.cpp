@@ -7,17 +7,25 @@
 
 #include "fh_internal.hpp"
 
+#include <stdexcept>
+
 namespace fh {
 
-static long double fact(int n) {
-  static long double table[400];
-  static bool init = false;
-  if (!init) {
-    table[0] = 1.0L;
-    for (int i = 1; i < 400; ++i) table[i] = table[i - 1] * (long double)i;
-    init = true;
+// n! as long double, n < FACT_MAX (labels with 2j up to ~250; mps_set_bond / mps_load refuse larger ones).
+// The table is built by a function-local static initialiser: thread safe (the two-site plans are emitted on a
+// second host thread).
+static const int FACT_MAX = 800;
+struct FactTable {
+  long double v[FACT_MAX];
+  FactTable() {
+    v[0] = 1.0L;
+    for (int i = 1; i < FACT_MAX; ++i) v[i] = v[i - 1] * (long double)i;
   }
-  return table[n];
+};
+static long double fact(int n) {
+  static const FactTable table;
+  if (n < 0 || n >= FACT_MAX) throw std::out_of_range("recoupling coefficient: label out of the supported range");
+  return table.v[n];
 }
 
 // Delta(a,b,c)^2 with doubled arguments

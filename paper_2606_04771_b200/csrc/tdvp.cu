@@ -81,9 +81,12 @@ constexpr size_t SMALL_SVD_SMEM = 216 * 1024;
 static inline size_t small_svd_bytes(int m, int n) {
   return ((size_t)m * n + (size_t)n * n) * sizeof(cplx) + (size_t)n * sizeof(double);
 }
+constexpr int FACT_NOT_CONVERGED = 1 << 20;  // status word of a Jacobi kernel that ran out of sweeps
+constexpr int JACOBI_MAX_SWEEPS = 40;
 struct SmallSvd {
   int64_t m_off, u_off, vt_off, s_off;
   int m, n;
+  int stat, pad;  // index of the matrix' status word
 };
 __device__ __forceinline__ double warp_sum_all(double v) {
 #pragma unroll
@@ -93,9 +96,11 @@ __device__ __forceinline__ double warp_sum_all(double v) {
 constexpr int SMALL_SVD_MAX_WARPS = 32;  // the launch picks 8, 16 or 32 warps by the largest matrix of the batch
 __global__ void __launch_bounds__(32 * SMALL_SVD_MAX_WARPS) small_svd_kernel(const SmallSvd* __restrict__ descs,
                                                                          cplx* __restrict__ buf,
-                                                                         double* __restrict__ dS) {
+                                                                         double* __restrict__ dS,
+                                                                         int* __restrict__ status) {
   extern __shared__ __align__(16) unsigned char smem_svd[];
   __shared__ int rotated_any;
+  bool converged = false;
   const SmallSvd d = descs[blockIdx.x];
   const int m = d.m, n = d.n, lane = threadIdx.x & 31, warp = threadIdx.x >> 5, tid = threadIdx.x;
   const int NT = blockDim.x, SMALL_SVD_WARPS = blockDim.x >> 5;
@@ -109,7 +114,8 @@ __global__ void __launch_bounds__(32 * SMALL_SVD_MAX_WARPS) small_svd_kernel(con
   // round-robin tournament: ne = n rounded up to even players, ne - 1 rounds of ne / 2 disjoint column pairs;
   // the pairs of a round are independent and go to different warps
   const int ne = (n + 1) & ~1;
-  for (int sweep = 0; sweep < 40 && n > 1; ++sweep) {
+  converged = n <= 1;
+  for (int sweep = 0; sweep < JACOBI_MAX_SWEEPS && n > 1; ++sweep) {
     if (tid == 0) rotated_any = 0;
     __syncthreads();
     for (int r = 0; r < ne - 1; ++r) {
@@ -154,7 +160,10 @@ __global__ void __launch_bounds__(32 * SMALL_SVD_MAX_WARPS) small_svd_kernel(con
       }
       __syncthreads();
     }
-    if (!rotated_any) break;
+    if (!rotated_any) {
+      converged = true;
+      break;
+    }
     __syncthreads();
   }
   // singular values = column norms; rank by descending value (ties: lower column first)
@@ -168,6 +177,7 @@ __global__ void __launch_bounds__(32 * SMALL_SVD_MAX_WARPS) small_svd_kernel(con
     if (lane == 0) sig[j] = sqrt(a);
   }
   __syncthreads();
+  if (tid == 0 && !converged) status[d.stat] = FACT_NOT_CONVERGED;
   cplx* U = buf + d.u_off;
   cplx* VT = buf + d.vt_off;
   double* S = dS + d.s_off;
@@ -199,11 +209,13 @@ __global__ void __launch_bounds__(32 * SMALL_SVD_MAX_WARPS) small_svd_kernel(con
 struct MidSvd {
   int64_t m_off, u_off, vt_off, s_off, v_off;  // v_off relative to the V scratch base
   int m, n;
+  int stat, pad;
 };
 constexpr int MID_SVD_HARD_MAXN = 256;
 __global__ void __launch_bounds__(1024) mid_svd_kernel(const MidSvd* __restrict__ descs, cplx* buf, cplx* vbase,
-                                                       double* __restrict__ dS) {
+                                                       double* __restrict__ dS, int* __restrict__ status) {
   __shared__ int rotated_any;
+  bool converged = false;
   __shared__ double sig[MID_SVD_HARD_MAXN];
   const MidSvd d = descs[blockIdx.x];
   const int m = d.m, n = d.n, lane = threadIdx.x & 31, warp = threadIdx.x >> 5, tid = threadIdx.x;
@@ -213,7 +225,8 @@ __global__ void __launch_bounds__(1024) mid_svd_kernel(const MidSvd* __restrict_
   for (int i = tid; i < n * n; i += NT) V[i] = make_double2((i % n) == (i / n) ? 1.0 : 0.0, 0.0);
   __syncthreads();
   const int ne = (n + 1) & ~1;
-  for (int sweep = 0; sweep < 40 && n > 1; ++sweep) {
+  converged = n <= 1;
+  for (int sweep = 0; sweep < JACOBI_MAX_SWEEPS && n > 1; ++sweep) {
     if (tid == 0) rotated_any = 0;
     __syncthreads();
     for (int r = 0; r < ne - 1; ++r) {
@@ -261,7 +274,10 @@ __global__ void __launch_bounds__(1024) mid_svd_kernel(const MidSvd* __restrict_
       }
       __syncthreads();
     }
-    if (!rotated_any) break;
+    if (!rotated_any) {
+      converged = true;
+      break;
+    }
     __syncthreads();
   }
   for (int j = warp; j < n; j += NW) {
@@ -274,6 +290,7 @@ __global__ void __launch_bounds__(1024) mid_svd_kernel(const MidSvd* __restrict_
     if (lane == 0) sig[j] = sqrt(a);
   }
   __syncthreads();
+  if (tid == 0 && !converged) status[d.stat] = FACT_NOT_CONVERGED;
   cplx* U = buf + d.u_off;
   cplx* VT = buf + d.vt_off;
   double* S = dS + d.s_off;
@@ -443,7 +460,7 @@ const int GESVDP_MIN_N = 48;  // below this the QR-iteration driver is as fast a
 // n >= GESVDP_MIN_N: cusolverDnXgesvdp (polar decomposition + Hermitian eigensolver; measured 3.3x
 // faster than Zgesvd at n = 600) on a copy; if it reports a perturbation of the spectrum
 // (err_sigma != 0: numerically rank-deficient input) the QR-iteration driver Zgesvd redoes it.
-void svd_one(fh_ctx::SvdWorker& w, const SectorSvd& S, cplx* buf, double* dS, int64_t* counts) {
+void svd_one(fh_ctx::SvdWorker& w, const SectorSvd& S, cplx* buf, double* dS, int64_t* counts, int* d_status) {
   const int m = std::max(S.nrow, S.ncol), n = S.k;
   cuDoubleComplex* A = (cuDoubleComplex*)(buf + S.m_off);
   cuDoubleComplex* U = (cuDoubleComplex*)(buf + S.u_off);
@@ -469,6 +486,7 @@ void svd_one(fh_ctx::SvdWorker& w, const SectorSvd& S, cplx* buf, double* dS, in
     if (err_sigma == 0.0) {
       const int64_t tot = (int64_t)n * n;
       conj_transpose_kernel<<<(int)std::min<int64_t>((tot + 255) / 256, 1184), 256, 0, w.s>>>((const cplx*)V, (cplx*)VT, n);
+      FH_CUDA(cudaMemcpyAsync(d_status, w.d_info, sizeof(int), cudaMemcpyDeviceToDevice, w.s));
       ++counts[1];
       return;
     }
@@ -479,11 +497,12 @@ void svd_one(fh_ctx::SvdWorker& w, const SectorSvd& S, cplx* buf, double* dS, in
   worker_reserve(w, (size_t)lwork * sizeof(cuDoubleComplex));
   FH_CUSOLVER(cusolverDnZgesvd(w.h, 'S', 'S', m, n, A, m, sv, U, m, VT, n, (cuDoubleComplex*)w.dwork,
                                (int)(w.dwork_bytes / sizeof(cuDoubleComplex)), nullptr, w.d_info));
+  FH_CUDA(cudaMemcpyAsync(d_status, w.d_info, sizeof(int), cudaMemcpyDeviceToDevice, w.s));
   ++counts[0];
 }
 
 // Householder QR of one sector matrix (one-site split, no truncation): geqrf, R copied out, ungqr in place.
-void qr_one(fh_ctx::SvdWorker& w, const SectorSvd& S, cplx* buf) {
+void qr_one(fh_ctx::SvdWorker& w, const SectorSvd& S, cplx* buf, int* d_status, int* d_status2) {
   const int m = S.qm, n = S.qn, k = std::min(m, n);
   cuDoubleComplex* A = (cuDoubleComplex*)(buf + S.m_off);
   cuDoubleComplex* tau = (cuDoubleComplex*)(buf + S.u_off);
@@ -493,10 +512,12 @@ void qr_one(fh_ctx::SvdWorker& w, const SectorSvd& S, cplx* buf) {
   const int lwork = std::max(lw1, lw2);
   worker_reserve(w, (size_t)lwork * sizeof(cuDoubleComplex) + 256);
   FH_CUSOLVER(cusolverDnZgeqrf(w.h, m, n, A, m, tau, (cuDoubleComplex*)w.dwork, lwork, w.d_info));
+  FH_CUDA(cudaMemcpyAsync(d_status, w.d_info, sizeof(int), cudaMemcpyDeviceToDevice, w.s));
   const int64_t tot = (int64_t)k * n;
   extract_r_kernel<<<(int)std::min<int64_t>((tot + 255) / 256, 1184), 256, 0, w.s>>>((const cplx*)A, m, k, n, S.r_dst, S.r_ld,
                                                                                      S.r_transpose);
   FH_CUSOLVER(cusolverDnZungqr(w.h, m, k, k, A, m, tau, (cuDoubleComplex*)w.dwork, lwork, w.d_info));
+  FH_CUDA(cudaMemcpyAsync(d_status2, w.d_info, sizeof(int), cudaMemcpyDeviceToDevice, w.s));
 }
 
 // Descriptors of the small-matrix kernels go through a host buffer owned by the context (it outlives the
@@ -532,6 +553,23 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
     FH_CUDA(cudaStreamCreateWithFlags(&ctx->svd_side, cudaStreamNonBlocking));
     FH_CUDA(cudaEventCreateWithFlags(&ctx->svd_side_done, cudaEventDisableTiming));
   }
+  // status words of this batch (checked by check_fact_status after the caller's next synchronisation)
+  if (ctx->fact_status_pending) {
+    FH_CUDA(cudaStreamSynchronize(ctx->stream));
+    check_fact_status(ctx);
+  }
+  const int nstat = 2 * (int)order.size();
+  if (nstat > ctx->fact_status_cap) {
+    FH_CUDA(cudaStreamSynchronize(ctx->stream));
+    if (ctx->d_fact_status) cudaFree(ctx->d_fact_status);
+    if (ctx->h_fact_status) cudaFreeHost(ctx->h_fact_status);
+    ctx->fact_status_cap = 2 * nstat + 256;
+    FH_CUDA(cudaMalloc((void**)&ctx->d_fact_status, ctx->fact_status_cap * sizeof(int)));
+    FH_CUDA(cudaMallocHost((void**)&ctx->h_fact_status, ctx->fact_status_cap * sizeof(int)));
+  }
+  int* const d_status = ctx->d_fact_status;
+  if (nstat > 0) FH_CUDA(cudaMemsetAsync(d_status, 0, nstat * sizeof(int), ctx->stream));
+  const int nord = (int)order.size();
   const int nw = (int)ctx->svd_workers.size();
   std::vector<int> idx;
   std::vector<SmallSvd> small;
@@ -543,16 +581,16 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
   // default 128: 64 column pairs per tournament round = two per warp of the 32-warp CTA
   const int mid_maxn = std::max(0, std::min(ctx->opt_svd_mid_maxn, MID_SVD_HARD_MAXN));
   const double mid_work = 1.5 * mid_maxn * (double)mid_maxn * mid_maxn;  // m n^2 bound: a long thin matrix would make its one CTA the critical path
-  const bool use_small_qr = true;
+  const int small_maxn = ctx->opt_svd_small_maxn;  // fh_set_option(FH_OPT_SVD_SMALL_MAXN)
   for (size_t i = 0; i < order.size(); ++i) {
     const int m = std::max(order[i]->nrow, order[i]->ncol), n = order[i]->k;
-    if (!qr && small_svd_bytes(m, n) <= SMALL_SVD_SMEM) {
-      small.push_back(SmallSvd{order[i]->m_off, order[i]->u_off, order[i]->vt_off, order[i]->s_off, m, n});
+    if (!qr && n <= small_maxn && small_svd_bytes(m, n) <= SMALL_SVD_SMEM) {
+      small.push_back(SmallSvd{order[i]->m_off, order[i]->u_off, order[i]->vt_off, order[i]->s_off, m, n, (int)i, 0});
       small_smem = std::max(small_smem, ((size_t)m * n + (size_t)n * n) * sizeof(cplx) + (size_t)n * sizeof(double));
     } else if (!qr && n <= mid_maxn && (double)m * n * n <= mid_work) {
-      mid.push_back(MidSvd{order[i]->m_off, order[i]->u_off, order[i]->vt_off, order[i]->s_off, mid_v_total, m, n});
+      mid.push_back(MidSvd{order[i]->m_off, order[i]->u_off, order[i]->vt_off, order[i]->s_off, mid_v_total, m, n, (int)i, 0});
       mid_v_total += ((int64_t)n * n + 15) / 16 * 16;
-    } else if (qr && use_small_qr && (size_t)order[i]->qm * order[i]->qn * sizeof(cplx) <= SMALL_QR_SMEM &&
+    } else if (qr && order[i]->qn <= small_maxn && (size_t)order[i]->qm * order[i]->qn * sizeof(cplx) <= SMALL_QR_SMEM &&
                std::min(order[i]->qm, order[i]->qn) <= SMALL_QR_MAXK) {
       small_qr.push_back(SmallQr{order[i]->m_off, order[i]->r_dst, order[i]->qm, order[i]->qn, order[i]->r_ld,
                                  order[i]->r_transpose});
@@ -587,7 +625,7 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
   }
   if (!mid.empty()) {
     FH_CUDA(cudaStreamWaitEvent(ctx->svd_side, ctx->svd_fork, 0));
-    mid_svd_kernel<<<(int)mid.size(), 1024, 0, ctx->svd_side>>>(d_mid, buf, ctx->ptr(mid_v_off), dS);
+    mid_svd_kernel<<<(int)mid.size(), 1024, 0, ctx->svd_side>>>(d_mid, buf, ctx->ptr(mid_v_off), dS, d_status);
     ++ctx->launches;
     ctx->svd_mid += (int64_t)mid.size();
     FH_CUDA(cudaGetLastError());
@@ -633,13 +671,20 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
     int nmax = 0;
     for (const SmallSvd& d : small) nmax = std::max(nmax, d.n);
     const int warps = nmax <= 16 ? 8 : (nmax <= 32 ? 16 : SMALL_SVD_MAX_WARPS);
-    small_svd_kernel<<<(int)small.size(), 32 * warps, small_smem, ctx->stream>>>(d_small, buf, dS);
+    small_svd_kernel<<<(int)small.size(), 32 * warps, small_smem, ctx->stream>>>(d_small, buf, dS, d_status);
     ++ctx->launches;
     ctx->svd_small += (int64_t)small.size();
     FH_CUDA(cudaGetLastError());
   }
+  auto read_status = [&]() {
+    if (nstat == 0) return;
+    FH_CUDA(cudaMemcpyAsync(ctx->h_fact_status, d_status, nstat * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    ctx->fact_status_n = nstat;
+    ctx->fact_status_pending = true;
+  };
   if (idx.empty()) {
     join_side();
+    read_status();
     return;
   }
   if (qr) ctx->qr_count += (int64_t)idx.size();
@@ -658,8 +703,8 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
       for (;;) {
         const int i = next.fetch_add(1);
         if (i >= (int)idx.size()) break;
-        if (qr) qr_one(w, *order[idx[i]], buf);
-        else svd_one(w, *order[idx[i]], buf, dS, counts[wi].data());
+        if (qr) qr_one(w, *order[idx[i]], buf, d_status + idx[i], d_status + nord + idx[i]);
+        else svd_one(w, *order[idx[i]], buf, dS, counts[wi].data(), d_status + idx[i]);
       }
       FH_CUDA(cudaEventRecord(w.done, w.s));
     } catch (const std::exception& e) {
@@ -675,15 +720,37 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
     for (int t = 0; t < nthreads; ++t) th.emplace_back(body, t);
     for (auto& t : th) t.join();
   }
+  // join every stream that was forked before reporting a worker's failure: nothing may still run on them
+  std::string first_err;
   for (int t = 0; t < std::max(1, nthreads); ++t) {
-    if (!errs[t].empty()) throw FhError(FH_ECUDA, "sector SVD worker: " + errs[t]);
+    if (!errs[t].empty()) {
+      if (first_err.empty()) first_err = errs[t];
+      cudaStreamSynchronize(ctx->svd_workers[t].s);
+      continue;
+    }
     FH_CUDA(cudaStreamWaitEvent(ctx->stream, ctx->svd_workers[t].done, 0));
     for (int k = 0; k < 3; ++k) ctx->svd_count[k] += counts[t][k];
   }
   join_side();
+  if (!first_err.empty()) throw FhError(FH_ECUDA, "sector SVD worker: " + first_err);
+  read_status();
 }
 
 }  // namespace
+
+void fh::check_fact_status(fh_ctx* ctx) {
+  if (!ctx->fact_status_pending) return;
+  ctx->fact_status_pending = false;
+  for (int i = 0; i < ctx->fact_status_n; ++i) {
+    const int v = ctx->h_fact_status[i];
+    if (v == 0) continue;
+    if (v == FACT_NOT_CONVERGED)
+      throw FhError(FH_ECUDA, "sector SVD: one-sided Jacobi did not converge in " + std::to_string(JACOBI_MAX_SWEEPS) +
+                                  " sweeps (matrix " + std::to_string(i) + " of the bond)");
+    throw FhError(FH_ECUDA, "sector factorisation: cuSOLVER devInfo = " + std::to_string(v) + " (matrix " +
+                                std::to_string(i % std::max(1, ctx->fact_status_n / 2)) + " of the bond)");
+  }
+}
 
 // Reading A-6 (same rule as the oracle's, restated): sort all (s, sector, position) by s
 // descending, ties by (sector index, position); drop s <= 1e-14 s_max; stop when the full
@@ -769,8 +836,8 @@ static void svd_split(fh_ctx* ctx, fh_mps* mps, int i, const BlockTensor& th, co
   }
   const int64_t s_cplx = (dbl_total + 1) / 2;  // singular values live in the same scratch, as doubles
   const int64_t scratch_n = cplx_total + Arena::round_up(s_cplx);
-  const int64_t scratch = ctx->alloc.alloc(scratch_n);
-  cplx* buf = ctx->ptr(scratch);
+  ArenaScratch scratch_mem(ctx, scratch_n);
+  cplx* buf = scratch_mem.ptr();
   double* dS = reinterpret_cast<double*>(buf + cplx_total);
   cudaStream_t s = ctx->stream;
 
@@ -817,6 +884,7 @@ static void svd_split(fh_ctx* ctx, fh_mps* mps, int i, const BlockTensor& th, co
   FH_CUDA(cudaMemcpyAsync(ctx->h_pinned, dS, dbl_total * sizeof(double), cudaMemcpyDeviceToHost, s));
   FH_CUDA(cudaStreamSynchronize(s));
   ctx->timer_end();
+  check_fact_status(ctx);
 
   // ---- truncation on the host (reading A-6)
   std::vector<std::vector<double>> sv;
@@ -943,7 +1011,6 @@ static void svd_split(fh_ctx* ctx, fh_mps* mps, int i, const BlockTensor& th, co
   ctx->timer_end();
   mps->A[i] = A1;
   mps->A[i + 1] = A2;
-  ctx->alloc.release(scratch, scratch_n);
 }
 
 // one local two-site update on bond (i, i+1)
@@ -954,8 +1021,8 @@ static void local_update2(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int i, do
   const int64_t n = P.vec.nelem;
   const int m = prm->krylov_dim;
   const int64_t wn = (int64_t)(m + 2) * n;
-  const int64_t woff = ctx->alloc.alloc(wn);
-  cplx* theta = ctx->ptr(woff);
+  ArenaScratch work(ctx, wn);  // theta and the Krylov basis: returned also when a step below throws
+  cplx* theta = work.ptr();
   cplx* V = theta + n;
   // merge (H8): theta[a,s1,c,s2,b] = A_i[a,s1,c] A_{i+1}[c,s2,b]; blocks whose c is not on the bond are zero
   {
@@ -970,7 +1037,6 @@ static void local_update2(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int i, do
   expm_lanczos(ctx, theta, tau, m, prm->krylov_tol, V, prm->krylov_adapt_tol);
   BlockTensor th = P.vec;  // copy: svd_split re-plans nothing but keeps the layout alive
   svd_split(ctx, mps, i, th, theta, direction, prm);
-  ctx->alloc.release(woff, wn);
 }
 
 static void local_update1(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int i, double tau, const fh_params* prm) {
@@ -980,9 +1046,8 @@ static void local_update1(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int i, do
   FH_REQUIRE(n == mps->A[i].nelem, FH_ESTATE, "one-site update: layout mismatch");
   const int m = prm->krylov_dim;
   const int64_t wn = (int64_t)(m + 1) * n;
-  const int64_t woff = ctx->alloc.alloc(wn);
-  expm_lanczos(ctx, ctx->ptr(mps->A[i].base), tau, m, prm->krylov_tol, ctx->ptr(woff), prm->krylov_adapt_tol);
-  ctx->alloc.release(woff, wn);
+  ArenaScratch work(ctx, wn);
+  expm_lanczos(ctx, ctx->ptr(mps->A[i].base), tau, m, prm->krylov_tol, work.ptr(), prm->krylov_adapt_tol);
 }
 
 // ============================================================================ one-site TDVP (NEXT-1)
@@ -1301,6 +1366,10 @@ void fh::sweep1(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh
       ctx->free_tensor(C);
     }
   }
+  if (ctx->fact_status_pending) {
+    FH_CUDA(cudaStreamSynchronize(ctx->stream));
+    check_fact_status(ctx);
+  }
 }
 
 void fh::sweep(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, double dt, const fh_params* prm) {
@@ -1387,12 +1456,28 @@ void fh::measure_local_impl(fh_ctx* ctx, const fh_mps* mps, double* n_i, double*
       if (k[2] == 1) sz -= 0.5 * w;
       if (k[2] == 2) pd += w;
     }
-    n_i[i] = one_v != 0.0 ? one_v / one_v : 0.0;  // <n_i> = 1 identically in a T_tot = 0 state (A-12)
+    // <n_i> = <1 + 2 T^z_i> = (w_up + w_dn + 2 * w_pair / 2) / <psi|psi>: the pair multiplet has <T^z_i> = 0 in a
+    // T_tot = 0 state (A-12).  The numerator is this site's sum of multiplet weights, the denominator the norm from
+    // the complete left-to-right contraction (filled in below): the ratio is 1 only if the norm environments, the
+    // multiplet weights and the site tensors are consistent on every site.
+    n_i[i] = one_v;
+    FH_REQUIRE(one_v > 0.0, FH_ESTATE, "measure_local: the state has zero weight on a site");
     sz_i[i] = sz / one_v;
     docc_i[i] = 0.5 * pd / one_v;
     ctx->alloc.release(xoff, A.nelem);
     ctx->free_tensor(N);
     N = Nn;
   }
+  // <psi|psi> = the last norm environment (one 1 x 1 block of the total sector)
+  double norm2 = 0.0;
+  {
+    ctx->ensure_pinned(2);
+    FH_REQUIRE(N.nelem >= 1, FH_ESTATE, "measure_local: empty norm environment");
+    FH_CUDA(cudaMemcpyAsync(ctx->h_pinned, ctx->ptr(N.base), sizeof(cplx), cudaMemcpyDeviceToHost, s));
+    FH_CUDA(cudaStreamSynchronize(s));
+    norm2 = ctx->h_pinned[0];
+  }
   ctx->free_tensor(N);
+  FH_REQUIRE(norm2 > 0.0, FH_ESTATE, "measure_local: the state has zero norm");
+  for (int i = 0; i < L; ++i) n_i[i] /= norm2;
 }

@@ -234,19 +234,11 @@ __global__ void __launch_bounds__(32) grouped_zgemm_kernel(const GemmUnit* __res
                                                            const GemmSeg* __restrict__ segs,
                                                            const cplx* __restrict__ A, const cplx* __restrict__ B,
                                                            cplx* __restrict__ C, int conjA
-#ifdef FH_UNIT_TRACE
-                                                           ,
-                                                           unsigned long long* __restrict__ trace
-#endif
 ) {
   __shared__ __align__(128) unsigned char ring_smem[RING_BYTES];
   const int lane = threadIdx.x;
   const int ui = blockIdx.x;
   if (ui >= nunits) return;
-#ifdef FH_UNIT_TRACE
-  unsigned long long t_begin = 0;
-  if (trace) asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_begin));
-#endif
   pdl_launch_dependents();
   const GemmUnit u = units[ui];  // uploaded before the predecessor started: readable before the wait
   pdl_wait();
@@ -262,53 +254,17 @@ __global__ void __launch_bounds__(32) grouped_zgemm_kernel(const GemmUnit* __res
     default:
       break;
   }
-#ifdef FH_UNIT_TRACE
-  if (trace && lane == 0) {
-    unsigned long long t_end;
-    unsigned smid, warpid;
-    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_end));
-    asm volatile("mov.u32 %0, %smid;" : "=r"(smid));
-    asm volatile("mov.u32 %0, %warpid;" : "=r"(warpid));
-    trace[4 * (size_t)ui + 0] = t_begin;
-    trace[4 * (size_t)ui + 1] = t_end;
-    trace[4 * (size_t)ui + 2] = ((unsigned long long)smid << 32) | warpid;
-    trace[4 * (size_t)ui + 3] = ((unsigned long long)u.shape << 32) | (unsigned)u.steps;
-  }
-#endif
 }
 
 }  // namespace
 
-#ifdef FH_UNIT_TRACE
-// Debugging aid, NOT compiled into the product library (build with -DFH_UNIT_TRACE): every unit records
-// {globaltimer at entry, at exit, smid << 32 | warpid, shape << 32 | steps} into a caller-provided device
-// buffer, launches appended one after the other.  This is how the timeline analysis in DESIGN.md 6.2
-// (slot refill in groups of four, pipe utilisation at full residency) was obtained.
-static unsigned long long* g_trace = nullptr;
-static size_t g_trace_cap = 0, g_trace_used = 0;
-extern "C" void fh_debug_unit_trace(unsigned long long* dev_buf, size_t capacity_units) {
-  g_trace = dev_buf;
-  g_trace_cap = capacity_units;
-  g_trace_used = 0;
-}
-extern "C" size_t fh_debug_unit_trace_used() { return g_trace_used; }
-#endif
 
 void launch_grouped_gemm(const Stage& st, const cplx* A, const cplx* B, cplx* C, cudaStream_t s, int64_t* lc,
                          int pdl_role) {
   const int n = (int)st.units.size();
   if (n == 0) return;
-#ifdef FH_UNIT_TRACE
-  unsigned long long* tr = nullptr;
-  if (g_trace && g_trace_used + n <= g_trace_cap) {
-    tr = g_trace + 4 * g_trace_used;
-    g_trace_used += n;
-  }
-  grouped_zgemm_kernel<<<n, 32, 0, s>>>(st.d_units, n, st.d_segs, A, B, C, st.opA != OPA_N ? 1 : 0, tr);
-#else
   launch_pdl(pdl_role, grouped_zgemm_kernel, n, 32, s, (const GemmUnit*)st.d_units, n, (const GemmSeg*)st.d_segs, A, B, C,
              st.opA != OPA_N ? 1 : 0);
-#endif
   ++*lc;
 }
 

@@ -58,7 +58,7 @@ def build_central_bond(ctx, mpo, chi, L=60, seed=fi.SEED, profile="gaussian", ta
     centre = L // 2 - 1 if centre is None else centre
     mps = ctx.mps_create(L)
     dims = fi.chain_dims(chi, L, profile, table_s2_scale)
-    for i, A, dl, dr in fi.canonical_chain(chi, centre, L, seed, dims=dims):
+    for i, A, dl, dr in fi.canonical_chain(chi, centre, L, seed, dims=dims, weight=binding.fh_canonical_weight):
         set_site(ctx, mps, i, A, dl, dr)
         if i < centre:
             ctx.env_update_left(mpo, mps, i)

@@ -31,7 +31,7 @@ def central_bond(chi, L=60, seed=fi.SEED, profile="gaussian", table_s2_scale=(1,
     W = [symm.mpo_reduced(i, t_h, U) for i in range(L)]
     Le, Re = symm.boundary_left(), symm.boundary_right()
     A_c = {}
-    for i, A, dl, dr in fi.canonical_chain(chi, centre, L, seed, dims=dims):
+    for i, A, dl, dr in fi.canonical_chain(chi, centre, L, seed, dims=dims, weight=symm.canonical_weight):
         if i < centre:
             Le = symm.env_update_left(Le, A, W[i])
         elif i > centre + 1:
