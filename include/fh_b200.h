@@ -260,6 +260,28 @@ int fh_cublas_gemm_seconds(fh_ctx* ctx, int n, int is_complex, int reps, double*
  * kernels, measured on the same device and clocks as the run.  Not part of the hot path. */
 int fh_dmma_peak_tflops(fh_ctx* ctx, int reps, double* tflops);
 
+/* ---- Lanczos vector kernels and scaled block copy on caller data (H6, H8) ---------------------------------
+ * The kernels expm_lanczos and the pack / unpack steps launch, callable on their own.  A vector of n complex128
+ * is a sequence of nblk contiguous blocks of blk_len[b] elements with the integer weight blk_weight[b] (= 2j+1);
+ * the library cuts it into chunks of the length it would use for a Krylov vector of that size (1024 / 2048 /
+ * 8192 elements below 1 Mi / below 4 Mi / above).  Reductions run in a fixed order (bit-identical results).
+ *   fh_vec_wdot:            result = sum_b weight_b sum conj(x) y                       (F-6; one launch)
+ *   fh_vec_lanczos_update:  the three-term recurrence on UNNORMALISED Krylov vectors u_j = b_j v_j:
+ *                           w <- (w - (a_raw / bj2) u_j) / sqrt(bj2) - sqrt(bj2 / bjm2) u_prev,  *norm2_out = <w,w>;
+ *                           bj2 <= 0 means b_j = 1, uprev_dev NULL or bjm2 <= 0 drops the u_prev term; a norm below
+ *                           tol gives a zero reciprocal (happy breakdown)
+ *   fh_vec_lincomb:         y = sum_j coef_j V[j * stride + .]  (coef = m complex numbers as 2m doubles, m <= 32)
+ *   fh_copy_blocks:         dst[dst_off + r ld_dst + c] (or [c ld_dst + r] if transpose) = scale * src[src_off + r ld_src + c]
+ * All pointers named _dev are device pointers; the other arrays are host arrays of nblk entries. */
+int fh_vec_wdot(fh_ctx* ctx, int64_t n, int nblk, const int64_t* blk_len, const int32_t* blk_weight, const void* x_dev,
+                const void* y_dev, double* result);
+int fh_vec_lanczos_update(fh_ctx* ctx, int64_t n, int nblk, const int64_t* blk_len, const int32_t* blk_weight, double a_raw,
+                          double bj2, double bjm2, double tol, const void* uj_dev, const void* uprev_dev, void* w_dev,
+                          double* norm2_out);
+int fh_vec_lincomb(fh_ctx* ctx, int64_t n, int m, const double* coef, const void* V_dev, int64_t stride, void* y_dev);
+int fh_copy_blocks(fh_ctx* ctx, int nblk, const int64_t* src_off, const int64_t* dst_off, const int32_t* rows, const int32_t* cols,
+                   const int32_t* ld_src, const int32_t* ld_dst, const int32_t* transpose, const double* scale,
+                   const void* src_dev, void* dst_dev);
 /* HBM-bound kernels of the path timed in isolation on n_elems complex128
  * elements taken from the arena (FH_ENOMEM if (m + 3) * n_elems do not fit): gbs[0] weighted dot (one launch,
  * last CTA sums the partials), gbs[1] axpy, gbs[2] scale, gbs[3] m-vector linear combination, gbs[4] pack

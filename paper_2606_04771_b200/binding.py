@@ -47,6 +47,12 @@ _SIGS = {
     "mps_get_svals": (c_int, [c_void_p, c_int, P(c_int), c_void_p]),
     "fh_dmma_peak_tflops": (c_int, [c_void_p, c_int, P(c_dbl)]),
     "fh_vec_kernels_gbs": (c_int, [c_void_p, c_i64, c_int, c_int, P(c_dbl)]),
+    "fh_vec_wdot": (c_int, [c_void_p, c_i64, c_int, c_void_p, c_void_p, c_void_p, c_void_p, P(c_dbl)]),
+    "fh_vec_lanczos_update": (c_int, [c_void_p, c_i64, c_int, c_void_p, c_void_p, c_dbl, c_dbl, c_dbl, c_dbl, c_void_p,
+                                      c_void_p, c_void_p, P(c_dbl)]),
+    "fh_vec_lincomb": (c_int, [c_void_p, c_i64, c_int, c_void_p, c_void_p, c_i64, c_void_p]),
+    "fh_copy_blocks": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p,
+                               c_void_p, c_void_p]),
     "mps_drop_site": (c_int, [c_void_p, c_void_p, c_int]),
     "heff_apply_host": (c_int, [c_void_p, c_void_p, c_void_p]),
     "env_update_left": (c_int, [c_void_p, c_void_p, c_void_p, c_int]),
@@ -345,6 +351,33 @@ class Context:
     def heff_export(self, vec, blocks):
         """planned layout -> interchange format; CUDA tensors."""
         self.check(lib.heff_export(self.h, c_void_p(vec.data_ptr()), c_void_p(blocks.data_ptr())), "heff_export")
+
+    def fh_vec_wdot(self, blk_len, blk_weight, x, y):
+        bl, bw = np.ascontiguousarray(blk_len, dtype=np.int64), _i32(blk_weight)
+        r = (c_dbl * 2)()
+        self.check(lib.fh_vec_wdot(self.h, int(bl.sum()), len(bl), _np_ptr(bl), _np_ptr(bw), c_void_p(x.data_ptr()),
+                                   c_void_p(y.data_ptr()), r), "fh_vec_wdot")
+        return complex(r[0], r[1])
+
+    def fh_vec_lanczos_update(self, blk_len, blk_weight, a_raw, bj2, bjm2, tol, uj, uprev, w):
+        bl, bw = np.ascontiguousarray(blk_len, dtype=np.int64), _i32(blk_weight)
+        r = c_dbl()
+        self.check(lib.fh_vec_lanczos_update(self.h, int(bl.sum()), len(bl), _np_ptr(bl), _np_ptr(bw), a_raw, bj2, bjm2, tol,
+                                             c_void_p(uj.data_ptr()), c_void_p(uprev.data_ptr() if uprev is not None else 0),
+                                             c_void_p(w.data_ptr()), C.byref(r)), "fh_vec_lanczos_update")
+        return r.value
+
+    def fh_vec_lincomb(self, coef, V, stride, y):
+        c = np.ascontiguousarray(coef, dtype=np.complex128)
+        self.check(lib.fh_vec_lincomb(self.h, int(y.numel()), len(c), _np_ptr(c), c_void_p(V.data_ptr()), int(stride),
+                                      c_void_p(y.data_ptr())), "fh_vec_lincomb")
+
+    def fh_copy_blocks(self, src_off, dst_off, rows, cols, ld_src, ld_dst, transpose, scale, src, dst):
+        so, do = np.ascontiguousarray(src_off, dtype=np.int64), np.ascontiguousarray(dst_off, dtype=np.int64)
+        sc = np.ascontiguousarray(scale, dtype=np.float64)
+        arrs = [_i32(a) for a in (rows, cols, ld_src, ld_dst, transpose)]
+        self.check(lib.fh_copy_blocks(self.h, len(so), _np_ptr(so), _np_ptr(do), *[_np_ptr(a) for a in arrs], _np_ptr(sc),
+                                      c_void_p(src.data_ptr()), c_void_p(dst.data_ptr())), "fh_copy_blocks")
 
     def heff_flops(self):
         return int(lib.heff_flops(self.h))

@@ -1554,6 +1554,100 @@ int fh_vec_kernels_gbs(fh_ctx* ctx, int64_t n, int m, int reps, double* gbs) {
   })
 }
 
+// ---- the Lanczos vector kernels and the scaled block copy on caller-supplied data (H6, H8): what expm_lanczos,
+//      pack and unpack launch, with the chunk length the library would pick for a vector of n elements
+static VecChunk* upload_chunks(fh_ctx* ctx, int64_t n, int nblk, const int64_t* blk_len, const int32_t* blk_weight,
+                               int* nchunks, size_t extra_bytes) {
+  std::vector<VecChunk> ch;
+  const int cl = vec_chunk_len(n);
+  int64_t pos = 0;
+  for (int b = 0; b < nblk; ++b) {
+    FH_REQUIRE(blk_len[b] >= 0 && blk_weight[b] >= 0, FH_EINVAL, "vector kernels: bad block table");
+    for (int64_t s0 = 0; s0 < blk_len[b]; s0 += cl)
+      ch.push_back(VecChunk{pos + s0, (int)std::min<int64_t>(cl, blk_len[b] - s0), (float)blk_weight[b]});
+    pos += blk_len[b];
+  }
+  FH_REQUIRE(pos == n, FH_EINVAL, "vector kernels: block lengths do not add up to n");
+  ctx->pool_aux.reserve(ch.size() * (sizeof(VecChunk) + 16) + extra_bytes + 8192, ctx->stream);
+  *nchunks = (int)ch.size();
+  return upload(ctx->pool_aux, ch, ctx->stream);
+}
+
+int fh_vec_wdot(fh_ctx* ctx, int64_t n, int nblk, const int64_t* blk_len, const int32_t* blk_weight, const void* x_dev,
+                const void* y_dev, double* result) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && n > 0 && nblk > 0 && blk_len && blk_weight && x_dev && y_dev && result, FH_EINVAL, "fh_vec_wdot: bad argument");
+    int nch = 0;
+    VecChunk* d_ch = upload_chunks(ctx, n, nblk, blk_len, blk_weight, &nch, 0);
+    double* d_part = (double*)ctx->pool_aux.take((size_t)nch * 2 * sizeof(double));
+    double* d_res = (double*)ctx->pool_aux.take(2 * sizeof(double));
+    unsigned* d_cnt = (unsigned*)ctx->pool_aux.take(sizeof(unsigned));
+    FH_CUDA(cudaMemsetAsync(d_cnt, 0, sizeof(unsigned), ctx->stream));
+    launch_wdot_fused(d_ch, nch, (const cplx*)x_dev, (const cplx*)y_dev, d_part, d_res, d_cnt, ctx->stream, &ctx->launches);
+    ctx->ensure_pinned(2);
+    FH_CUDA(cudaMemcpyAsync(ctx->h_pinned, d_res, 2 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    FH_CUDA(cudaStreamSynchronize(ctx->stream));
+    result[0] = ctx->h_pinned[0];
+    result[1] = ctx->h_pinned[1];
+  })
+}
+
+int fh_vec_lanczos_update(fh_ctx* ctx, int64_t n, int nblk, const int64_t* blk_len, const int32_t* blk_weight, double a_raw,
+                          double bj2, double bjm2, double tol, const void* uj_dev, const void* uprev_dev, void* w_dev,
+                          double* norm2_out) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && n > 0 && nblk > 0 && blk_len && blk_weight && uj_dev && w_dev && norm2_out, FH_EINVAL,
+               "fh_vec_lanczos_update: bad argument");
+    int nch = 0;
+    VecChunk* d_ch = upload_chunks(ctx, n, nblk, blk_len, blk_weight, &nch, 0);
+    double* d_part = (double*)ctx->pool_aux.take((size_t)nch * 2 * sizeof(double));
+    double* d_sc = (double*)ctx->pool_aux.take(8 * sizeof(double));
+    unsigned* d_cnt = (unsigned*)ctx->pool_aux.take(sizeof(unsigned));
+    FH_CUDA(cudaMemsetAsync(d_cnt, 0, sizeof(unsigned), ctx->stream));
+    ctx->ensure_pinned(8);
+    ctx->h_pinned[0] = a_raw;
+    ctx->h_pinned[1] = bj2;
+    ctx->h_pinned[2] = bjm2;
+    FH_CUDA(cudaMemcpyAsync(d_sc, ctx->h_pinned, 3 * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    launch_lanczos_update(d_ch, nch, d_sc, bj2 > 0.0 ? d_sc + 1 : nullptr, (uprev_dev && bjm2 > 0.0) ? d_sc + 2 : nullptr, tol,
+                          (const cplx*)uj_dev, (const cplx*)uprev_dev, (cplx*)w_dev, d_part, d_sc + 4, d_cnt, ctx->stream,
+                          &ctx->launches);
+    FH_CUDA(cudaMemcpyAsync(ctx->h_pinned + 4, d_sc + 4, 2 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    FH_CUDA(cudaStreamSynchronize(ctx->stream));
+    *norm2_out = ctx->h_pinned[4];
+  })
+}
+
+int fh_vec_lincomb(fh_ctx* ctx, int64_t n, int m, const double* coef, const void* V_dev, int64_t stride, void* y_dev) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && n > 0 && m >= 1 && m <= 32 && coef && V_dev && y_dev && stride >= n, FH_EINVAL, "fh_vec_lincomb: bad argument");
+    std::vector<cplx> c(m);
+    for (int j = 0; j < m; ++j) c[j] = make_double2(coef[2 * j], coef[2 * j + 1]);
+    launch_lincomb(n, m, c.data(), (const cplx*)V_dev, stride, (cplx*)y_dev, ctx->stream, &ctx->launches);
+    FH_CUDA(cudaGetLastError());
+  })
+}
+
+int fh_copy_blocks(fh_ctx* ctx, int nblk, const int64_t* src_off, const int64_t* dst_off, const int32_t* rows, const int32_t* cols,
+                   const int32_t* ld_src, const int32_t* ld_dst, const int32_t* transpose, const double* scale,
+                   const void* src_dev, void* dst_dev) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && nblk > 0 && src_off && dst_off && rows && cols && ld_src && ld_dst && transpose && scale && src_dev &&
+                   dst_dev && src_dev != dst_dev,
+               FH_EINVAL, "fh_copy_blocks: bad argument");
+    std::vector<CopyBlk> cb(nblk);
+    for (int i = 0; i < nblk; ++i) {
+      FH_REQUIRE(rows[i] >= 0 && cols[i] >= 0 && ld_src[i] >= cols[i] && ld_dst[i] >= (transpose[i] ? rows[i] : cols[i]), FH_EINVAL,
+                 "fh_copy_blocks: bad block geometry");
+      cb[i] = CopyBlk{src_off[i], dst_off[i], rows[i], cols[i], ld_src[i], ld_dst[i], transpose[i] ? 1 : 0, 0, scale[i]};
+    }
+    ctx->pool_aux.reserve(cb.size() * sizeof(CopyBlk) + 4096, ctx->stream);
+    CopyBlk* d_cb = upload(ctx->pool_aux, cb, ctx->stream);
+    launch_copy_blocks(d_cb, nblk, (const cplx*)src_dev, (cplx*)dst_dev, ctx->stream, &ctx->launches);
+    FH_CUDA(cudaGetLastError());
+  })
+}
+
 // host-only helpers for the CPU test-suite (symmetry layer without a GPU)
 static fh::Stage g_host_st1, g_host_st2;
 

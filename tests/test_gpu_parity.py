@@ -7,7 +7,7 @@ import numpy as np
 import pytest
 
 import fh_inputs as fi
-from oracle import symm
+from oracle import symm, vecops
 from oracle import symm_tdvp as stv
 from oracle.dense_tdvp import lanczos_exp
 
@@ -858,6 +858,58 @@ def test_mid_size_jacobi_kernel_vs_vendor_svd(H, ctx, tmp_path):
     assert worst < 1e-11 and dobs < 1e-10, (worst, dobs)
     for h in (mps, a, b):
         ctx.mps_destroy(h)
+
+
+# ------------------------------------------------------------------ H6 / H8 kernels on their own
+@pytest.mark.parametrize("n", [300_001, 1_500_003, 4_700_011])
+def test_vector_kernels_and_block_copy_vs_oracle(H, ctx, n):
+    """H6 / H8 directly (not through a Lanczos run): weighted dot, the unnormalised three-term update with its fused
+    norm, the linear combination and the scaled block copy (plain and transposing) against oracle/vecops.py, on
+    vectors of 0.3, 1.5 and 4.7 Mi elements -- one in each chunk-length class of the library (1024 / 2048 / 8192) --
+    cut into ragged blocks (lengths 1 ... 200 000) with weights 1 ... 5."""
+    torch = _torch()
+    rng = np.random.default_rng(n)
+    lens, left = [], n
+    while left > 0:
+        k = int(min(left, rng.choice([1, 7, 1023, 1024, 1025, 8191, 8193, 50_000, 200_000])))
+        lens.append(k)
+        left -= k
+    wts = [int(rng.integers(1, 6)) for _ in lens]
+    x, y, w = (rng.standard_normal(n) + 1j * rng.standard_normal(n) for _ in range(3))
+    dx, dy = _dev(x), _dev(y)
+    ref = vecops.wdot(lens, wts, x, y)
+    got = ctx.fh_vec_wdot(lens, wts, dx, dy)
+    assert abs(got - ref) < 1e-12 * abs(ref) + 1e-9, (got, ref)
+    assert ctx.fh_vec_wdot(lens, wts, dx, dy) == got                      # fixed reduction order: same bits
+    for (bj2, bjm2, prev) in ((-1.0, -1.0, None), (2.5, -1.0, y), (2.5, 0.7, y)):
+        dw = _dev(w)
+        ru, rn = vecops.lanczos_update(lens, wts, 1.3, bj2, bjm2, 1e-12, x, prev, w)
+        gn = ctx.fh_vec_lanczos_update(lens, wts, 1.3, bj2, bjm2, 1e-12, dx, dy if prev is not None else None, dw)
+        assert np.abs(dw.cpu().numpy() - ru).max() < 1e-13 * np.abs(ru).max() and abs(gn / rn - 1) < 1e-12
+    m = 7
+    V = rng.standard_normal((m, n)) + 1j * rng.standard_normal((m, n))
+    coef = rng.standard_normal(m) + 1j * rng.standard_normal(m)
+    dV, dz = _dev(V), torch.empty(n, dtype=torch.complex128, device="cuda")
+    ctx.fh_vec_lincomb(coef, dV, n, dz)
+    rl = vecops.lincomb(coef, V)
+    assert np.abs(dz.cpu().numpy() - rl).max() < 1e-13 * np.abs(rl).max()
+    # block copies: ragged blocks out of a strided source into a strided destination, plain and transposed
+    blocks, so, do = [], 0, 0
+    for b in range(40):
+        r, c = int(rng.integers(1, 130)), int(rng.integers(1, 130))
+        ls, tr = c + int(rng.integers(0, 5)), int(b % 2)
+        ld = (r if tr else c) + int(rng.integers(0, 5))
+        blocks.append((so, do, r, c, ls, ld, tr, float(rng.uniform(0.5, 2.0))))
+        so += r * ls
+        do += (c if tr else r) * ld
+    assert so <= n and do <= n
+    dst_ref = np.zeros(n, dtype=complex)
+    vecops.copy_blocks(blocks, x, dst_ref)
+    ddst = torch.zeros(n, dtype=torch.complex128, device="cuda")
+    cols = list(zip(*blocks))
+    ctx.fh_copy_blocks(*cols, dx, ddst)
+    assert np.array_equal(ddst.cpu().numpy() == 0, dst_ref == 0)
+    assert np.abs(ddst.cpu().numpy() - dst_ref).max() < 1e-15 * np.abs(dst_ref).max() + 1e-300
 
 
 # ------------------------------------------------------------------ edge cases and errors
