@@ -27,8 +27,6 @@ NOMINAL_FP64_TF = 40.0      # B200 dense FP64 (tensor = vector) nominal, HGX B20
 NOMINAL_BF16_TF = 2250.0    # guide: 2.25 PFLOP/s dense bf16
 FALLBACK_BF16_TF = 1590.0   # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 FALLBACK_HBM_GBS = 6650.0
-# one ncu --set full capture of the default workload (profiles/r1_heff_apply_ncu.md), bytes per launch
-NCU_DRAM_BYTES_PER_LAUNCH = 0.5 * (16.202496e6 + 1.256704e6 + 36.604416e6 + 0.501760e6)
 
 
 def parse_args():
@@ -42,6 +40,9 @@ def parse_args():
     ap.add_argument("--s2-scale", default="1/6", help="num/den scale of Table S2 degeneracies")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-flush", action="store_true", help="do not flush L2 between timed applies")
+    ap.add_argument("--no-extra", action="store_true",
+                    help="skip the apply-only lines of the other configs (chi = 1024, Table S2 x 1/6, 16384, 24576) and "
+                         "the oracle timings on configs 1, 2, 5'")
     ap.add_argument("--no-sweep", action="store_true", help="skip the timed tdvp2_sweep (second half of the metric)")
     ap.add_argument("--sweep", action="store_true", help="(default on) time one full tdvp2_sweep at --sweep-chi")
     ap.add_argument("--sweep-chi", type=int, default=4096)
@@ -118,23 +119,46 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def cpu_oracle_setup(args):
-    """Oracle-side workload (bounded sample): same sector structure and theta; environments are
-    iid random blocks of the right shapes (timing does not depend on their values, and building
-    the canonical chain in pure Python would dominate the run)."""
+def oracle_central_bond(chi, L, c, profile, s2):
+    """Oracle-side twin of harness.build_central_bond (same seeded chain, every contraction by oracle/symm.py)."""
+    import fh_inputs as fi
+    from oracle import symm
+    dims = fi.chain_dims(chi, L, profile, s2)
+    W = [symm.mpo_reduced(i, 1.0, 4.0) for i in range(L)]
+    Le, Re = symm.boundary_left(), symm.boundary_right()
+    for i, A, dl, dr in fi.canonical_chain(chi, c, L, fi.SEED, dims=dims, weight=symm.canonical_weight):
+        if i < c:
+            Le = symm.env_update_left(Le, A, W[i])
+        elif i > c + 1:
+            Re = symm.env_update_right(Re, A, W[i])
+    return dims, Le, Re
+
+
+def cpu_oracle_setup(args, with_chain=None):
+    """Oracle-side workload.  chi <= 4096 (Gaussian profile): the environments are contracted by the oracle from
+    the same seeded canonical chain the library uses, so that its H_eff theta can also be compared with the
+    library's (the `parity` entry of the line).  Larger workloads: same sector structure and theta, iid random
+    environments of the right shapes (timing does not depend on their values) and a bounded sample of output
+    blocks."""
     import fh_inputs as fi
     from oracle import symm
     L, c = 60, 29
-    dims = fi.chain_dims(args.chi, L, args.profile, s2_scale(args))
-    dl, dr = dims[c], dims[c + 2]
-    Lk, Rk = fi.env_block_keys(dl, dl), fi.env_block_keys(dr, dr)
-    Le = fi.random_blocks(11, 1, Lk, {k: (dl[k[0]], dl[k[2]]) for k in Lk})
-    Re = fi.random_blocks(11, 2, Rk, {k: (dr[k[0]], dr[k[2]]) for k in Rk})
+    if with_chain is None:
+        with_chain = args.profile == "gaussian" and args.chi <= 4096
+    if with_chain:
+        dims, Le, Re = oracle_central_bond(args.chi, L, c, args.profile, s2_scale(args))
+        dl, dr = dims[c], dims[c + 2]
+    else:
+        dims = fi.chain_dims(args.chi, L, args.profile, s2_scale(args))
+        dl, dr = dims[c], dims[c + 2]
+        Lk, Rk = fi.env_block_keys(dl, dl), fi.env_block_keys(dr, dr)
+        Le = fi.random_blocks(11, 1, Lk, {k: (dl[k[0]], dl[k[2]]) for k in Lk})
+        Re = fi.random_blocks(11, 2, Rk, {k: (dr[k[0]], dr[k[2]]) for k in Rk})
     th = fi.theta_random(fi.SEED, c, dl, dr)
     W1, W2 = symm.mpo_reduced(c, 1.0, 4.0), symm.mpo_reduced(c + 1, 1.0, 4.0)
     st1, st2 = symm.heff2_tasks(sorted(Le), sorted(Re), sorted(th), W1, W2)
     flops = symm.heff2_flops(st1, st2, dl, dr)
-    # bound the sample to ~2 GFLOP of output blocks (whole apply when it is smaller)
+    # bound the sample to ~4 GFLOP of output blocks (whole apply when it is smaller)
     budget, sub2, acc = 4e9, {}, 0
     for k, segs in st2.items():
         sub2[k] = segs
@@ -146,15 +170,19 @@ def cpu_oracle_setup(args):
     sub1 = st1 if whole else {z: st1[z] for z in need}
     f1 = sum(8 * dl[ap] * dl[a] * dr[kk[4]] for z, segs in sub1.items() for (ap, w, a), kk, _ in segs)
     f2 = sum(8 * dl[z[0]] * dr[b] * dr[bp] for segs in sub2.values() for z, (bp, wr, b), _ in segs)
+    result = {}
 
     def step():
         Z = symm.run_stage(sub1, Le, th)
-        return symm.run_stage(sub2, Z, Re, "n", "t")
+        result["out"] = symm.run_stage(sub2, Z, Re, "n", "t")
+        return result["out"]
 
     sample = ("whole heff_apply" if whole else "%d of %d output blocks" % (len(sub2), len(st2))) + \
-        " (%.3g of %.3g GFLOP), task lists prebuilt, random environments of the same shapes" % (
-            (f1 + f2) * 1e-9, flops * 1e-9)
-    return step, f1 + f2, sample
+        " (%.3g of %.3g GFLOP), task lists prebuilt, %s" % (
+            (f1 + f2) * 1e-9, flops * 1e-9,
+            "environments contracted by the oracle from the seeded canonical chain" if with_chain
+            else "random environments of the same shapes")
+    return step, f1 + f2, sample, result, (whole and with_chain), th
 
 
 def cpu_cores():
@@ -166,22 +194,38 @@ def cpu_cores():
     return int(n)
 
 
-def time_oracle(args, steps, warmup):
-    step, flops, sample = cpu_oracle_setup(args)
+def time_oracle(args, steps, warmup, with_chain=None):
+    step, flops, sample, result, comparable, th = cpu_oracle_setup(args, with_chain)
     for _ in range(warmup):
         step()
     t0 = time.perf_counter()
     for _ in range(steps):
         step()
     dt = (time.perf_counter() - t0) / steps
-    return dict(value=flops / dt * 1e-9, unit="GFLOP/s", cores=cpu_cores(), kind="oracle", sample=sample), dt
+    cb = dict(value=flops / dt * 1e-9, unit="GFLOP/s", cores=cpu_cores(), kind="oracle", sample=sample)
+    return cb, dt, (result.get("out") if comparable else None), th
+
+
+def parity_vs_oracle(got_blocks, ref_blocks):
+    """Relative Frobenius error of the library's H_eff theta against the oracle's under the F-6 weighted norm,
+    globally and for the worst single block (north_star: <= 1e-11 per heff_apply)."""
+    num = den = worst = 0.0
+    for k, v in ref_blocks.items():
+        w = k[-1][1] + 1
+        d = np.linalg.norm(got_blocks[k] - v)
+        num += w * d * d
+        den += w * np.linalg.norm(v) ** 2
+        worst = max(worst, d / max(np.linalg.norm(v), 1e-300))
+    return {"rel_frobenius": float(np.sqrt(num / den)), "worst_block": float(worst), "blocks": len(ref_blocks),
+            "tolerance": 1e-11, "against": "oracle/symm.py heff2_apply on the same seeded chain, environments "
+            "contracted independently on each side"}
 
 
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    cb, dt = time_oracle(args, args.steps, args.warmup)
+    cb, dt, _, _ = time_oracle(args, args.steps, args.warmup)
     out = {"impl": "reference", "metric": "heff_apply_gflops", "value": cb["value"], "unit": "GFLOP/s",
            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3,
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "complex128 (f64)",
@@ -207,6 +251,89 @@ def max_over_ranks(values, device, world):
 def aggregate_gflops(flops_per_replica, steps, seconds, world):
     """Whole-job throughput of `world` independent replicas that each did `steps` applies."""
     return world * flops_per_replica * steps / seconds * 1e-9
+
+
+def profile_traffic():
+    """dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/): the line
+    'dram_bytes_per_launch: <number>' of the newest r*_heff_apply_ncu.md; None when there is none."""
+    import glob
+    import re
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_heff_apply_ncu.md")), reverse=True):
+        m = re.search(r"dram_bytes_per_launch:\s*([0-9.eE+]+)", open(path).read())
+        if m:
+            return float(m.group(1)), os.path.relpath(path, ROOT)
+    return None, None
+
+
+def time_apply_random_envs(H, fi, torch, chi, profile, s2, steps, peak_dmma, local):
+    """heff_apply on the central bond of the given workload with iid random environments of the right shapes
+    (env_set; timing does not depend on their values, and contracting a chi >= 16384 chain on the host would
+    take minutes).  Own context, so that `arena_peak_bytes` is this workload's."""
+    L, c = 60, 29
+    dims = fi.chain_dims(chi, L, profile, s2)
+    dl, dr = dims[c], dims[c + 2]
+    zest = 40.0 * sum(dl.values()) ** 2 * 16 / 1274.0 ** 2 * 1.2      # Z scales like chi_su2^2 (40 MB at 1274)
+    ctx = H.binding.Context(int(max(2 << 30, 6 * zest + (1 << 30))), device="cuda:%d" % local)
+    try:
+        mpo = ctx.fh_mpo_build(L, 1.0, 4.0)
+        mps = ctx.mps_create(L)
+        ctx.mps_set_bond(mps, c, dl)
+        ctx.mps_set_bond(mps, c + 2, dr)
+        for which, bond, d in ((0, c, dl), (1, c + 2, dr)):
+            keys = fi.env_block_keys(d, d)
+            E = fi.random_blocks(11, 1 + which, keys, {k: (d[k[0]], d[k[2]]) for k in keys})
+            labels = [[k[0][0], k[0][1], k[1], k[2][0], k[2][1]] for k in keys]
+            ctx.env_set(mps, which, bond, labels, np.concatenate([E[k].ravel() for k in keys]))
+            del E
+        ctx.heff_plan(mpo, mps, c, 2)
+        lab, dm, ne = ctx.heff_layout(2)
+        flops = ctx.heff_flops()
+        x = torch.randn(ne, dtype=torch.complex128, device="cuda:%d" % local) * (1.0 / np.sqrt(2.0 * ne))
+        y = torch.empty_like(x)
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device=x.device)
+        for _ in range(3):
+            ctx.heff_apply(x, y)
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        torch.cuda.synchronize()
+        clocks = ClockSampler(local)
+        for a, b in ev:
+            flush.zero_()
+            a.record()
+            ctx.heff_apply(x, y)
+            b.record()
+        torch.cuda.synchronize()
+        clk = clocks.stop()
+        t = sum(a.elapsed_time(b) for a, b in ev) * 1e-3 / steps
+        used, peak = ctx.fh_arena_stats()
+        return {"chi": chi, "profile": profile if profile == "gaussian" else "table_s2 x %d/%d" % s2,
+                "d_max": max(max(dl.values()), max(dr.values())), "theta_blocks": len(lab), "flop_per_apply": flops,
+                "ms_per_apply": t * 1e3, "gflops": flops / t * 1e-9, "frac_of_dmma_peak": flops / t * 1e-12 / peak_dmma,
+                "steps": steps, "arena_peak_bytes": int(peak), "theta_bytes": 16 * int(ne), "clocks": clk,
+                "environments": "iid random blocks (env_set)"}
+    finally:
+        ctx.close()
+
+
+def oracle_extra_timings():
+    """the oracle on configs 1, 2 and 5' (reported baselines, host cores)."""
+    from oracle import dense_tdvp as dtv
+    out = {}
+    t0 = time.perf_counter()
+    d = dtv.DenseTDVP(8, 1.0, 4.0, krylov_dim=10)
+    for _ in range(20):
+        d.step(0.05)
+    out["config1_dense_tdvp_L8_20_steps_seconds"] = time.perf_counter() - t0
+
+    class A:
+        pass
+    for tag, chi, prof, s2, chain in (("config2_chi1024", 1024, "gaussian", "1/1", True),
+                                      ("config5p_table_s2_x_1_6", 0, "table_s2", "1/6", False)):
+        a = A()
+        a.chi, a.profile, a.s2_scale = chi, prof, s2
+        cb, dt, _, _ = time_oracle(a, 2, 1, with_chain=chain)
+        out[tag] = {"gflops": cb["value"], "seconds_per_sample": dt, "sample": cb["sample"]}
+    out["cores"] = cpu_cores()
+    return out
 
 
 def run_ours(args):
@@ -294,8 +421,12 @@ def run_ours(args):
     t_dev, t_e2e, t_warm = max_over_ranks([t_dev, t_e2e, t_warm], x.device, world)
     if rank != 0:
         return
+    y_blocks = torch.empty_like(y)
+    ctx.heff_export(y, y_blocks)                     # planned layout -> canonical blocks, for the parity entry
+    got_blocks = H.unflatten(y_blocks.cpu().numpy(), lab, dm, H.theta_key)
     gf = aggregate_gflops(flops, args.steps, t_dev, world)
     per_gpu_tf = flops * args.steps / t_dev * 1e-12
+    traffic, traffic_src = profile_traffic()
     peak_rule = pk["bf16"] * NOMINAL_FP64_TF / NOMINAL_BF16_TF
     zbytes = 16 * sum(int(a_) * int(b_) for a_, b_ in dm)
     out = {
@@ -316,8 +447,9 @@ def run_ours(args):
                      "peak_rule_source": "%s bf16 %.1f TF x nominal fp64/bf16 %g/%g" % (
                          pk["source"], pk["bf16"], NOMINAL_FP64_TF, NOMINAL_BF16_TF),
                      "frac_l2_warm": flops * args.steps / t_warm * 1e-12 / peak_dmma,
-                     "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (chi == 4096 and args.profile == "gaussian") else None,
-                     "traffic_source": "profiles/r1_heff_apply_ncu.md: dram__bytes_read.sum + dram__bytes_write.sum, mean of the stage-1 and stage-2 launch (17.5 MB and 37.1 MB); algorithmic minimum 55 MB per launch pair / 2"},
+                     "traffic": traffic if (chi == 4096 and args.profile == "gaussian") else None,
+                     "traffic_source": ("%s: dram__bytes_read.sum + dram__bytes_write.sum, mean over the two launches of "
+                                        "one apply" % traffic_src) if traffic_src else None},
         "e2e": {"value": world * flops * args.steps / t_e2e * 1e-9, "unit": "GFLOP/s",
                 "h2d_bytes_per_step": zbytes, "d2h_bytes_per_step": zbytes, "api": "heff_apply_host (pinned host buffers)"},
         "gpu_launches": int(launches), "clocks": clk, "wall_seconds_timed_region": wall,
@@ -331,13 +463,41 @@ def run_ours(args):
                               "achieved": g, "frac": {k: v / pk["hbm"] for k, v in g.items()}}
     except H.binding.FhError as e:
         out["hbm_kernels"] = {"error": str(e)}
+    # library cross-check of the roofline denominator: cuBLAS FP64 GEMM 8192^3, burst (best of 5)
+    # and sustained (back to back for ~3 s)
+    try:
+        peaks64 = {}
+        for nm, cplx_, fl in (("dgemm", 0, 2.0 * 8192 ** 3), ("zgemm", 1, 8.0 * 8192 ** 3)):
+            burst = min(ctx.fh_cublas_gemm_seconds(8192, cplx_, 1) for _ in range(5))
+            reps = max(2, int(3.0 / burst))
+            sust = ctx.fh_cublas_gemm_seconds(8192, cplx_, reps)
+            peaks64["cublas_%s_8192_tflops_burst" % nm] = fl / burst * 1e-12
+            peaks64["cublas_%s_8192_tflops_sustained" % nm] = fl / sust * 1e-12
+        out["roofline"]["peak_cublas"] = peaks64
+        out["roofline"]["frac_of_cublas_zgemm_burst"] = per_gpu_tf / peaks64["cublas_zgemm_8192_tflops_burst"]
+    except H.binding.FhError as e:
+        out["roofline"]["peak_cublas"] = {"error": str(e)}
     if not args.no_sweep and world == 1:
         out["sweep"] = run_sweep(ctx, H, mpo, args)
-    if not args.no_cpu_baseline:
-        cb, _ = time_oracle(args, 3, 1)
-        out["cpu_baseline"] = cb
-    print(json.dumps(out))
     ctx.close()
+    if not args.no_extra and world == 1:
+        extra = []
+        for chi_x, prof_x, s2_x, st_x in ((1024, "gaussian", (1, 1), 20), (0, "table_s2", (1, 6), 10),
+                                          (16384, "gaussian", (1, 1), 5), (24576, "gaussian", (1, 1), 3)):
+            try:
+                extra.append(time_apply_random_envs(H, fi, torch, chi_x, prof_x, s2_x, st_x, peak_dmma, local))
+            except Exception as e:            # report, do not lose the headline line
+                extra.append({"chi": chi_x, "profile": prof_x, "error": "%s: %s" % (type(e).__name__, e)})
+        out["other_configs"] = extra
+    if not args.no_cpu_baseline:
+        cb, _, ref_blocks, th_o = time_oracle(args, 3, 1)
+        out["cpu_baseline"] = cb
+        if ref_blocks is not None:
+            assert all(np.array_equal(th[k], th_o[k]) for k in th)      # same seeded theta on both sides
+            out["parity"] = parity_vs_oracle(got_blocks, ref_blocks)
+        if not args.no_extra:
+            out["cpu_baseline_other_configs"] = oracle_extra_timings()
+    print(json.dumps(out))
 
 
 def run_sweep(ctx, H, mpo, args):
@@ -355,8 +515,14 @@ def run_sweep(ctx, H, mpo, args):
     torch.cuda.synchronize()
     sec = time.perf_counter() - t0
     tm = ctx.fh_get_timers()
+    tr = ctx.fh_get_traffic()
     st = ctx.tdvp2_last_stats()
     launches2 = ctx.fh_launch_count() - l0
+    in_sweep = {"vec_gbs": tr["vec_bytes"] / max(tm["vec"], 1e-12) * 1e-9, "pack_gbs": tr["pack_bytes"] / max(tm["pack"], 1e-12) * 1e-9,
+                "vec_bytes": tr["vec_bytes"], "pack_bytes": tr["pack_bytes"],
+                "note": "algorithmic bytes of the Lanczos vector kernels (H6) and of pack/unpack (H8) inside this sweep / "
+                        "their device seconds: vectors of 0.1-10 MB, launch- and latency-bound, unlike the 1 GiB "
+                        "vectors of hbm_kernels"}
     # NEXT-1: the one-site sweep on the same (now chi-saturated) MPS -- the paper's 4-10x lever
     ctx.fh_reset_timers()
     torch.cuda.synchronize()
@@ -389,7 +555,8 @@ def run_sweep(ctx, H, mpo, args):
     tm1s = ctx.fh_get_timers()
     cache = ctx.fh_plan_cache_stats(mps)
     ctx.mps_destroy(mps)
-    return {"chi": chi, "seconds": sec, "device_seconds_by_phase": tm, "stats": st, "launches": launches2,
+    return {"chi": chi, "seconds": sec, "device_seconds_by_phase": tm, "hbm_kernels_in_sweep": in_sweep, "stats": st,
+            "launches": launches2,
             "one_site": {"seconds": sec1, "device_seconds_by_phase": tm1, "chi_full": st1["chi_full"],
                          "launches": launches1, "speedup_vs_two_site": sec / sec1,
                          "seconds_task_lists_cached": steady, "seconds_cached_with_phase_events": sec1t,

@@ -242,6 +242,10 @@ int measure_global(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, double* no
 int fh_get_timers(const fh_ctx* ctx, double* sec_heff, double* sec_env, double* sec_svd,
                   double* sec_vec, double* sec_pack);
 int fh_reset_timers(fh_ctx* ctx);
+/* algorithmic bytes the HBM-bound phases moved since the last fh_reset_timers: vec = Lanczos vector kernels (H6:
+ * 32 n per dot, 64 n per three-term update, 16 (m+1) n per linear combination), pack = pack / unpack around the
+ * SVD (H8: 32 bytes per element + the zero fill).  With fh_get_timers: GB/s of those kernels inside a sweep. */
+int fh_get_traffic(const fh_ctx* ctx, int64_t* vec_bytes, int64_t* pack_bytes);
 /* on = 0: the library records no phase events any more (fh_get_timers then returns what was accumulated before);
  * on != 0 (the default at context creation) records them again.  An event record between two kernels of the
  * Lanczos loop costs about a microsecond of GPU time and keeps the next kernel from being set up while its

@@ -84,6 +84,7 @@ _SIGS = {
     "measure_global": (c_int, [c_void_p, c_void_p, c_void_p, P(c_dbl), P(c_dbl)]),
     "fh_get_timers": (c_int, [c_void_p, P(c_dbl), P(c_dbl), P(c_dbl), P(c_dbl), P(c_dbl)]),
     "fh_reset_timers": (c_int, [c_void_p]),
+    "fh_get_traffic": (c_int, [c_void_p, P(c_i64), P(c_i64)]),
     "fh_enable_timers": (c_int, [c_void_p, c_int]),
     "fh_launch_count": (c_i64, [c_void_p]),
     "fh_cublas_gemm_seconds": (c_int, [c_void_p, c_int, c_int, c_int, P(c_dbl)]),
@@ -401,6 +402,11 @@ class Context:
         self.check(lib.fh_factorization_stats(self.h, a), "fh_factorization_stats")
         return dict(jacobi_kernel=a[0], gesvdp=a[1], gesvd=a[2], gesvdp_rejected=a[3], qr=a[4], qr_kernel=a[5],
                     jacobi_mid_kernel=a[6])
+
+    def fh_get_traffic(self):
+        a, b = c_i64(0), c_i64(0)
+        self.check(lib.fh_get_traffic(self.h, C.byref(a), C.byref(b)), "fh_get_traffic")
+        return dict(vec_bytes=a.value, pack_bytes=b.value)
 
     def fh_enable_timers(self, on):
         self.check(lib.fh_enable_timers(self.h, 1 if on else 0), "fh_enable_timers")

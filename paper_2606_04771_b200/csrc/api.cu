@@ -528,6 +528,7 @@ int fh::expm_lanczos(fh_ctx* ctx, cplx* theta, double tau, int m, double tol, cp
   ctx->timer_begin(T_VEC);
   launch_wdot_fused(P.d_chunks, nch, theta, theta, P.d_partial, d_sc, P.d_counter, s, &ctx->launches);
   launch_scale_rsqrt_dev(n, d_sc, 0.0, theta, V, nullptr, s, &ctx->launches);
+  ctx->vec_bytes += 64 * n;
   ctx->timer_end();
   std::vector<double> alpha, beta;
   int k = 0;  // > 0 once the adaptive rule (or a breakdown seen by it) has fixed the dimension
@@ -539,6 +540,7 @@ int fh::expm_lanczos(fh_ctx* ctx, cplx* theta, double tau, int m, double tol, cp
     ctx->timer_end();
     ctx->timer_begin(T_VEC);
     launch_wdot_fused(P.d_chunks, nch, vj, w, P.d_partial, d_sc + 2 + 4 * j, P.d_counter, s, &ctx->launches);
+    ctx->vec_bytes += (32 + (j > 0 ? 64 : 48)) * n;
     launch_lanczos_update(P.d_chunks, nch, d_sc + 2 + 4 * j, j > 0 ? d_sc + 4 + 4 * (j - 1) : nullptr,
                           j > 1 ? d_sc + 4 + 4 * (j - 2) : nullptr, tol, vj, j > 0 ? V + (int64_t)(j - 1) * n : nullptr, w,
                           P.d_partial, d_sc + 4 + 4 * j, P.d_counter, s, &ctx->launches);
@@ -584,6 +586,7 @@ int fh::expm_lanczos(fh_ctx* ctx, cplx* theta, double tau, int m, double tol, cp
   }
   ctx->timer_begin(T_VEC);
   launch_lincomb(n, k, c.data(), V, n, theta, s, &ctx->launches);
+  ctx->vec_bytes += 16 * (int64_t)(k + 1) * n;
   ctx->timer_end();
   FH_CUDA(cudaGetLastError());
   ctx->krylov_calls += 1;
@@ -1413,7 +1416,14 @@ int fh_reset_timers(fh_ctx* ctx) {
     FH_REQUIRE(ctx != nullptr, FH_EINVAL, "fh_reset_timers: NULL context");
     ctx->timers_resolve();
     for (int i = 0; i < T_NCAT; ++i) ctx->sec[i] = 0.0;
+    ctx->vec_bytes = ctx->pack_bytes = 0;
   })
+}
+int fh_get_traffic(const fh_ctx* ctx, int64_t* vec_bytes, int64_t* pack_bytes) {
+  if (!ctx) return FH_EINVAL;
+  if (vec_bytes) *vec_bytes = ctx->vec_bytes;
+  if (pack_bytes) *pack_bytes = ctx->pack_bytes;
+  return FH_OK;
 }
 int fh_enable_timers(fh_ctx* ctx, int on) {
   FH_TRY(ctx, {

@@ -150,6 +150,10 @@ struct fh_ctx {
   fh::DevPool pool_aux;  // env updates, merge, pack, measure
   fh::DevPool pool_small;  // descriptors of the small-matrix SVD kernel
   int64_t launches = 0;
+  // algorithmic bytes of the HBM-bound phases since the last fh_reset_timers (H6: 32 n per dot, 64 n per three-term
+  // update, 16 (m + 1) n per linear combination; H8: 32 bytes per packed / unpacked element): with the phase
+  // timers they give the GB/s those kernels reach INSIDE a sweep
+  int64_t vec_bytes = 0, pack_bytes = 0;
   // pinned host scratch
   double* h_pinned = nullptr;  // 4096 doubles
   size_t h_pinned_n = 0;

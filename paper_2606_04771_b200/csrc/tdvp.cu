@@ -875,6 +875,7 @@ static void svd_split(fh_ctx* ctx, fh_mps* mps, int i, const BlockTensor& th, co
   ctx->pool_aux.reserve(blks.size() * sizeof(CopyBlk) + 4096, s);
   CopyBlk* d_blks = upload(ctx->pool_aux, blks, s);
   launch_copy_blocks(d_blks, (int)blks.size(), theta, buf, s, &ctx->launches);
+  ctx->pack_bytes += 16 * cplx_total + 32 * th.nelem;  // zero fill of the work matrices + the scaled copy
   ctx->timer_end();
 
   // ---- block-wise SVD (H9): vendor routine, timed separately
@@ -1007,6 +1008,7 @@ static void svd_split(fh_ctx* ctx, fh_mps* mps, int i, const BlockTensor& th, co
   CopyBlk* d_vb = upload(ctx->pool_aux, vb, s);
   launch_copy_blocks(d_ub, (int)ub.size(), buf, ctx->ptr(A1.base), s, &ctx->launches);
   launch_copy_blocks(d_vb, (int)vb.size(), buf, ctx->ptr(A2.base), s, &ctx->launches);
+  ctx->pack_bytes += 32 * (A1.nelem + A2.nelem);
   FH_CUDA(cudaGetLastError());
   ctx->timer_end();
   mps->A[i] = A1;
