@@ -60,10 +60,17 @@ def _counter_words(key):
     labels = _flatten(key)
     assert len(labels) <= 24
     words = [0, 0, 0]
+    if all(-128 <= int(v) < 128 for v in labels):
+        for i, v in enumerate(labels):
+            words[i // 8] |= (int(v) + 128) << (8 * (i % 8))
+        return words
+    # wide labels (the packed charges of the U(1) x U(1) mode): two bytes per label, top bit of the last word set
+    assert len(labels) <= 11
     for i, v in enumerate(labels):
-        b = int(v) + 128
-        assert 0 <= b < 256
-        words[i // 8] |= b << (8 * (i % 8))
+        b = int(v) + 32768
+        assert 0 <= b < 65536
+        words[i // 4] |= b << (16 * (i % 4))
+    words[2] |= 1 << 63
     return words
 
 

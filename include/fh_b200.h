@@ -71,6 +71,13 @@ const char* fh_last_error(const fh_ctx* ctx);
 #define FH_OPT_SVD_MID_MAXN 2
 #define FH_OPT_SVD_THREADS 3
 #define FH_OPT_SVD_SMALL_MAXN 4
+/*   FH_OPT_SYMMETRY      label algebra of every object created in the context afterwards: 0 =
+ *                        U(1)_spin x SU(2)_charge (default; the conventions at the top of this header), 1 = U(1) x U(1)
+ *                        (PAPER.md:59, 66, 296): labels (q, 0) with q = (N_up - N_dn) + 64 (N - k) on bond k, site
+ *                        states s = 0 |0>, 1 |up>, 2 |dn>, 3 |updn>; MPO bond states 0 = I, 1 = c+_up P, 2 = c+_dn P,
+ *                        3 = c_up P, 4 = c_dn P, 5 = final (W = 6), all recoupling coefficients 1, MPO of Eq. (1) as it
+ *                        stands.  Set it before fh_mpo_build / mps_create and do not change it while they live. */
+#define FH_OPT_SYMMETRY 5
 int fh_set_option(fh_ctx* ctx, int key, int value);
 /* bytes currently allocated / high-water mark in the arena */
 int fh_arena_stats(const fh_ctx* ctx, size_t* used_bytes, size_t* peak_bytes);
@@ -80,8 +87,8 @@ int fh_arena_stats(const fh_ctx* ctx, size_t* used_bytes, size_t* peak_bytes);
  * which equals Eq. (1) on the half-filled sector (reading A-2).  L even, 2 <= L <= 4096. */
 int fh_mpo_build(fh_ctx* ctx, int L, double t_h, double U, fh_mpo** out);
 void fh_mpo_destroy(fh_mpo* mpo);
-/* reduced MPO element table of one site: val[4][4][3][3] = W[w][w'][s'][s], rank2[4][4] = doubled
- * operator rank of (w,w') or -1 when the pair is absent. */
+/* reduced MPO element table of one site: val[6][6][4][4] = W[w][w'][s'][s], rank2[6][6] = doubled
+ * operator rank of (w,w') or -1 when the pair is absent (the SU(2) mode uses w < 4, s < 3). */
 int fh_mpo_get_site(const fh_mpo* mpo, int site, double* val, int32_t* rank2);
 
 /* ---- state -----------------------------------------------------------------------------
@@ -304,6 +311,8 @@ double fh_canonical_weight(int tjc, int tjb);
  *   coefR(c,s,b; k,r,k'; c',s',b') = (2b'+1)/(2c'+1) sqrt((2b+1)(2k'+1)(2c'+1)(2s'+1)) {c s b; k r k'; c' s' b'} */
 double fh_coef_left(int ta, int ts, int tc, int tk, int tr, int tkp, int tap, int tsp, int tcp);
 double fh_coef_right(int tc, int ts, int tb, int tk, int tr, int tkp, int tcp, int tsp, int tbp);
+/* label algebra fh_host_plan uses (host-only twin of FH_OPT_SYMMETRY): 0 = U(1) x SU(2), 1 = U(1) x U(1) */
+int fh_host_set_symmetry(int mode);
 /* Emit the task lists of an apply on `site` (nsite = 1 | 2; nsite = 0: the zero-site apply of one-site
  * TDVP on the bond whose bra-side dims are bl and ket-side dims br) from explicit tables: bl/br =
  * [n][3] (q,tj,d) of the left and right bond, Llab/Rlab = [nblk][5] canonical-order labels of the

@@ -33,6 +33,7 @@ _SIGS = {
     "fh_arena_stats": (c_int, [c_void_p, P(c_size_t), P(c_size_t)]),
     "fh_set_option": (c_int, [c_void_p, c_int, c_int]),
     "fh_canonical_weight": (c_dbl, [c_int, c_int]),
+    "fh_host_set_symmetry": (c_int, [c_int]),
     "fh_mpo_build": (c_int, [c_void_p, c_int, c_dbl, c_dbl, P(c_void_p)]),
     "fh_mpo_destroy": (None, [c_void_p]),
     "fh_mpo_get_site": (c_int, [c_void_p, c_int, c_void_p, c_void_p]),
@@ -206,8 +207,8 @@ class Context:
         return h
 
     def fh_mpo_get_site(self, mpo, site):
-        val = np.zeros((4, 4, 3, 3))
-        rank2 = np.zeros((4, 4), dtype=np.int32)
+        val = np.zeros((6, 6, 4, 4))
+        rank2 = np.zeros((6, 6), dtype=np.int32)
         self.check(lib.fh_mpo_get_site(mpo, site, _np_ptr(val), _np_ptr(rank2)), "fh_mpo_get_site")
         return val, rank2
 
@@ -466,7 +467,7 @@ class Context:
     def fh_launch_count(self):
         return int(lib.fh_launch_count(self.h))
 
-    OPT_GEMM_PATH, OPT_SVD_MID_MAXN, OPT_SVD_THREADS, OPT_SVD_SMALL_MAXN = 1, 2, 3, 4
+    OPT_GEMM_PATH, OPT_SVD_MID_MAXN, OPT_SVD_THREADS, OPT_SVD_SMALL_MAXN, OPT_SYMMETRY = 1, 2, 3, 4, 5
 
     def fh_set_option(self, key, value):
         self.check(lib.fh_set_option(self.h, int(key), int(value)), "fh_set_option")

@@ -234,7 +234,9 @@ void fh::prefetch_plan2(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int s
   if (site < 0 || site + 2 > mps->L || mps->Lenv[site].base < 0 || mps->Renv[site + 2].base < 0) return;
   PlanEmit* e = &ctx->prefetch;
   e->site = site;
-  ctx->prefetch_job = std::async(std::launch::async, [mpo, mps, site, e]() {
+  const SymMode* mode = ctx->sym;
+  ctx->prefetch_job = std::async(std::launch::async, [mpo, mps, site, e, mode]() {
+    SymScope scope(mode);
     e->Z.base = -1;
     emit_plan2(mpo, mps, site, e->vec, e->Z, e->st1, e->st2, e->chunks);
   });
@@ -252,6 +254,8 @@ void fh::prefetch_cancel(fh_ctx* ctx) {
 void fh::plan_heff(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, int nsite) {
   FH_REQUIRE(nsite == 1 || nsite == 2, FH_EINVAL, "heff_plan: nsite must be 1 or 2");
   FH_REQUIRE(site >= 0 && site + nsite <= mps->L, FH_EINVAL, "heff_plan: site out of range");
+  FH_REQUIRE(mpo->sym == ctx->sym && mps->sym == ctx->sym, FH_ESTATE,
+             "heff_plan: MPO / MPS were created under another FH_OPT_SYMMETRY than the context has now");
   const BlockTensor& Le = mps->Lenv[site];
   const BlockTensor& Re = mps->Renv[site + nsite];
   FH_REQUIRE(Le.base >= 0 && Re.base >= 0, FH_ESTATE, "heff_plan: environments of this bond are not built");
@@ -685,6 +689,7 @@ void fh::do_env_update_right(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int si
 // ============================================================================ C ABI
 #define FH_TRY(ctxptr, ...)                    \
   try {                                        \
+    fh::SymScope sym_scope__((ctxptr) ? (ctxptr)->sym : nullptr); \
     __VA_ARGS__;                               \
     return FH_OK;                              \
   } catch (const fh::FhError& e) {             \
@@ -784,6 +789,10 @@ int fh_set_option(fh_ctx* c, int key, int value) {
       if (value < 0 || value > 4096) return FH_EINVAL;
       c->opt_svd_small_maxn = value;
       return FH_OK;
+    case FH_OPT_SYMMETRY:
+      if (value < 0 || value > 1) return FH_EINVAL;
+      c->sym = value == 1 ? &SYM_U1U1 : &SYM_SU2;
+      return FH_OK;
     case FH_OPT_SVD_THREADS:
       if (value < 1 || value > 12) return FH_EINVAL;
       c->opt_svd_threads = value;
@@ -805,6 +814,7 @@ int fh_mpo_build(fh_ctx* ctx, int L, double t_h, double U, fh_mpo** out) {
     FH_REQUIRE(out != nullptr, FH_EINVAL, "fh_mpo_build: out is NULL");
     FH_REQUIRE(L >= 2 && L <= 4096 && L % 2 == 0, FH_EINVAL, "fh_mpo_build: L must be even, 2 <= L <= 4096");
     fh_mpo* m = new fh_mpo();
+    m->sym = ctx->sym;
     m->L = L;
     m->t_h = t_h;
     m->U = U;
@@ -820,8 +830,8 @@ int fh_mpo_get_site(const fh_mpo* mpo, int site, double* val, int32_t* rank2) {
   const MpoSite& W = mpo->site[site & 1];
   if (val) std::memcpy(val, W.val, sizeof(W.val));
   if (rank2)
-    for (int a = 0; a < 4; ++a)
-      for (int b = 0; b < 4; ++b) rank2[a * 4 + b] = W.rank2[a][b];
+    for (int a = 0; a < MAX_NW; ++a)
+      for (int b = 0; b < MAX_NW; ++b) rank2[a * MAX_NW + b] = W.rank2[a][b];
   return FH_OK;
 }
 
@@ -833,7 +843,7 @@ static void set_boundaries(fh_ctx* ctx, fh_mps* m) {
     ctx->free_tensor(E);
     E.clear();
     E.nlab = 5;
-    E.add(key_env(Sector{0, 0}, which == 0 ? 0 : 3, Sector{0, 0}), 1, 1);
+    E.add(key_env(Sector{0, 0}, which == 0 ? 0 : sym().nw - 1, Sector{0, 0}), 1, 1);
     E.finalize();
     ctx->alloc_tensor(E);
     FH_CUDA(cudaMemcpyAsync(ctx->ptr(E.base), &one, sizeof(cplx), cudaMemcpyHostToDevice, ctx->stream));
@@ -845,6 +855,7 @@ int mps_create(fh_ctx* ctx, int L, fh_mps** out) {
     FH_REQUIRE(ctx && out, FH_EINVAL, "mps_create: NULL argument");
     FH_REQUIRE(L >= 2 && L <= 4096 && L % 2 == 0, FH_EINVAL, "mps_create: L must be even, 2 <= L <= 4096");
     fh_mps* m = new fh_mps();
+    m->sym = ctx->sym;
     m->L = L;
     m->bond.resize(L + 1);
     m->A.resize(L);
@@ -879,7 +890,8 @@ int mps_init_neel(fh_ctx* ctx, const fh_mpo* mpo, int L, fh_mps** out) {
     const cplx one = make_double2(1.0, 0.0);
     int q = 0;
     for (int i = 0; i < L; ++i) {
-      const int s = (i % 2 == 0) ? 0 : 1;
+      const int up = sym().id == 1 ? 1 : 0;  // index of |up> among the site multiplets; |dn> follows it
+      const int s = (i % 2 == 0) ? up : up + 1;
       const int qn = q + SITE_Q[s];
       m->bond[i + 1].sec = {Sector{qn, 0}};
       m->bond[i + 1].d = {1};
@@ -980,7 +992,7 @@ int mps_load(fh_ctx* ctx, const fh_mpo* mpo, const char* path, fh_mps** out) {
         for (int32_t i = 0; i < n; ++i) {
           int32_t rec[3];
           get(rec, sizeof(rec));
-          FH_REQUIRE(rec[1] >= 0 && rec[1] <= 250 && rec[2] >= 1 && rec[0] >= -1000 && rec[0] <= 1000, FH_EINVAL,
+          FH_REQUIRE(rec[1] >= 0 && rec[1] <= 250 && rec[2] >= 1 && rec[0] >= -8000 && rec[0] <= 8000, FH_EINVAL,
                      "mps_load: bad sector record");
           if (i > 0) FH_REQUIRE(b.sec.back() < Sector({rec[0], rec[1]}), FH_EINVAL, "mps_load: sector labels not sorted");
           b.sec.push_back(Sector{rec[0], rec[1]});
@@ -1016,8 +1028,11 @@ int mps_set_bond(fh_ctx* ctx, fh_mps* mps, int bond, int n, const int32_t* q, co
     Bond b;
     for (int i = 0; i < n; ++i) {
       FH_REQUIRE(tj[i] >= 0 && tj[i] <= 250 && d[i] >= 1, FH_EINVAL, "mps_set_bond: 0 <= tj <= 250 and d >= 1 required");
-      FH_REQUIRE(q[i] >= -1000 && q[i] <= 1000, FH_EINVAL, "mps_set_bond: |q| <= 1000 required");
-      FH_REQUIRE(((q[i] + tj[i] - bond) & 1) == 0, FH_EINVAL, "mps_set_bond: parity rule q + 2j = bond (mod 2) violated");
+      FH_REQUIRE(q[i] >= -8000 && q[i] <= 8000, FH_EINVAL, "mps_set_bond: |q| <= 8000 required");
+      if (sym().id == 0)
+        FH_REQUIRE(((q[i] + tj[i] - bond) & 1) == 0, FH_EINVAL, "mps_set_bond: parity rule q + 2j = bond (mod 2) violated");
+      else
+        FH_REQUIRE(tj[i] == 0, FH_EINVAL, "mps_set_bond: U(1) x U(1) labels have tj = 0");
       if (i > 0) FH_REQUIRE(Sector({q[i - 1], tj[i - 1]}) < Sector({q[i], tj[i]}), FH_EINVAL, "mps_set_bond: labels must be sorted by (q, tj) and distinct");
       b.sec.push_back(Sector{q[i], tj[i]});
       b.d.push_back(d[i]);
@@ -1054,6 +1069,7 @@ static void export_layout(const BlockTensor& t, int nlab, int* nblk, int64_t* ne
 }
 
 int mps_site_layout(const fh_mps* mps, int site, int* nblk, int64_t* nelem, int32_t* labels, int32_t* dims) {
+  fh::SymScope sym_scope(mps ? mps->sym : nullptr);
   if (!mps || site < 0 || site >= mps->L) return FH_EINVAL;
   if (mps->A[site].base >= 0 || !mps->A[site].keys.empty()) {
     export_layout(mps->A[site], 5, nblk, nelem, labels, dims);
@@ -1148,7 +1164,7 @@ int env_set(fh_ctx* ctx, fh_mps* mps, int which, int bond, int nblk, const int32
       const int32_t* l = labels + 5 * i;
       const Sector xp{l[0], l[1]}, x{l[3], l[4]};
       const int w = l[2];
-      FH_REQUIRE(w >= 0 && w < 4 && b.find(xp) >= 0 && b.find(x) >= 0, FH_EINVAL, "env_set: label not in the bond table");
+      FH_REQUIRE(w >= 0 && w < sym().nw && b.find(xp) >= 0 && b.find(x) >= 0, FH_EINVAL, "env_set: label not in the bond table");
       FH_REQUIRE(xp.q == x.q + MPO_Q[w] && triangle(x.tj, MPO_TK[w], xp.tj), FH_EINVAL, "env_set: block violates the selection rule");
       const Key k = key_env(xp, w, x);
       if (i > 0) FH_REQUIRE(t.keys.back() < k, FH_EINVAL, "env_set: blocks must be in canonical order");
@@ -1388,7 +1404,7 @@ int measure_global(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, double* no
       if (i > 0) ctx->free_tensor(tmp.Lenv[i]);
     }
     BlockTensor& E = tmp.Lenv[mps->L];
-    const int is = E.find(key_env(Sector{0, 0}, 0, Sector{0, 0})), ie = E.find(key_env(Sector{0, 0}, 3, Sector{0, 0}));
+    const int is = E.find(key_env(Sector{0, 0}, 0, Sector{0, 0})), ie = E.find(key_env(Sector{0, 0}, sym().nw - 1, Sector{0, 0}));
     std::vector<cplx> h(E.nelem);
     FH_CUDA(cudaMemcpyAsync(h.data(), ctx->ptr(E.base), E.nelem * sizeof(cplx), cudaMemcpyDeviceToHost, ctx->stream));
     FH_CUDA(cudaStreamSynchronize(ctx->stream));
@@ -1661,9 +1677,17 @@ int fh_copy_blocks(fh_ctx* ctx, int nblk, const int64_t* src_off, const int64_t*
 // host-only helpers for the CPU test-suite (symmetry layer without a GPU)
 static fh::Stage g_host_st1, g_host_st2;
 
+static const fh::SymMode* g_host_sym = &fh::SYM_SU2;
+int fh_host_set_symmetry(int mode) {
+  if (mode < 0 || mode > 1) return FH_EINVAL;
+  g_host_sym = mode == 1 ? &fh::SYM_U1U1 : &fh::SYM_SU2;
+  return FH_OK;
+}
+
 int fh_host_plan(int site, int nsite, double t_h, double U, int nl, const int32_t* bl, int nr, const int32_t* br,
                  int nLblk, const int32_t* Llab, int nRblk, const int32_t* Rlab) {
   try {
+    fh::SymScope scope(g_host_sym);
     if ((nsite != 0 && nsite != 1 && nsite != 2) || !bl || !br || !Llab || !Rlab) return FH_EINVAL;
     Bond Bl, Br;
     for (int i = 0; i < nl; ++i) { Bl.sec.push_back(Sector{bl[3 * i], bl[3 * i + 1]}); Bl.d.push_back(bl[3 * i + 2]); }

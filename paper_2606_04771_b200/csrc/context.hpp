@@ -122,12 +122,14 @@ void sig_add(std::vector<int>& sig, double x);
 }  // namespace fh
 
 struct fh_mpo {
+  const fh::SymMode* sym = &fh::SYM_SU2;
   int L;
   double t_h, U;
   fh::MpoSite site[2];  // even / odd site parity
 };
 
 struct fh_mps {
+  const fh::SymMode* sym = &fh::SYM_SU2;  // label algebra the state was created under (FH_OPT_SYMMETRY at mps_create)
   int L;
   std::vector<fh::Bond> bond;                       // L+1
   std::vector<fh::BlockTensor> A, Lenv, Renv;       // L, L+1, L+1
@@ -190,6 +192,7 @@ struct fh_ctx {
   bool small_copied_armed = false;
   std::vector<char> small_desc_host;
   int device = 0;
+  const fh::SymMode* sym = &fh::SYM_SU2;  // fh_set_option(FH_OPT_SYMMETRY): the label algebra of every object of the context
   int opt_gemm_path = 0;      // fh_set_option: 0 auto, 1 warp units, 2 warp-specialised
   int opt_svd_mid_maxn = 128;
   int opt_svd_small_maxn = 4096;

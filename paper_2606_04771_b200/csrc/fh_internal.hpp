@@ -22,11 +22,32 @@ struct Sector {
   bool operator==(const Sector& o) const { return q == o.q && tj == o.tj; }
 };
 
-// (q, tj) of the site multiplets s = 0,1,2 and of the MPO bond multiplets w = S,P,M,F
-static const int SITE_Q[3] = {1, -1, 0};
-static const int SITE_TJ[3] = {0, 0, 1};
-static const int MPO_Q[4] = {0, 1, -1, 0};
-static const int MPO_TK[4] = {0, 1, 1, 0};
+// Symmetry mode: the labels (q, tj) of the site multiplets and of the MPO bond multiplets.
+//   SU2  (default): U(1)_spin x SU(2)_charge.  q = N_up - N_dn, tj = 2 T.  Site multiplets
+//        s = 0 (+1,0) |up>, 1 (-1,0) |dn>, 2 (0,1/2) {|0>, eps |updn>}; MPO bond multiplets S, P, M, F (W = 4).
+//   U1U1: U(1) x U(1), every multiplet one-dimensional (tj = 0, every
+//        recoupling coefficient 1).  The two additive charges are packed into the one integer label,
+//        q = (N_up - N_dn) + 64 (N - 1) per site (|N_up - N_dn| on a bond stays far below 32 for the chains in
+//        reach, so the packing is unique).  Site states s = 0 |0>, 1 |up>, 2 |dn>, 3 |updn> = c+_up c+_dn |0>;
+//        MPO bond states 0 = I, 1 = c+_up P, 2 = c+_dn P, 3 = c_up P, 4 = c_dn P, 5 = final (W = 6).
+struct SymMode {
+  int id;      // 0 SU2, 1 U1U1
+  int ns, nw;  // site multiplets, MPO bond multiplets (the last one closes the MPO)
+  int site_q[4], site_tj[4], mpo_q[6], mpo_tk[6];
+};
+const int MAX_NS = 4, MAX_NW = 6;
+extern const SymMode SYM_SU2, SYM_U1U1;
+// the mode of the calling thread: set for the duration of every API call from the context (SymScope)
+const SymMode& sym();
+struct SymScope {
+  const SymMode* prev;
+  explicit SymScope(const SymMode* m);
+  ~SymScope();
+};
+#define SITE_Q (fh::sym().site_q)
+#define SITE_TJ (fh::sym().site_tj)
+#define MPO_Q (fh::sym().mpo_q)
+#define MPO_TK (fh::sym().mpo_tk)
 
 inline bool triangle(int t1, int t2, int t3) {
   int lo = t1 > t2 ? t1 - t2 : t2 - t1;
@@ -80,8 +101,8 @@ struct BlockTensor {
 
 // reduced MPO of one site parity: val[w][w'][s'][s], rank2[w][w'] (-1 = absent)
 struct MpoSite {
-  double val[4][4][3][3];
-  int rank2[4][4];
+  double val[MAX_NW][MAX_NW][MAX_NS][MAX_NS];
+  int rank2[MAX_NW][MAX_NW];
 };
 
 // recoupling coefficients, closed forms (su2.cpp)

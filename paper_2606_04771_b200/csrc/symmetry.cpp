@@ -17,6 +17,14 @@
 
 namespace fh {
 
+// ----------------------------------------------------------------------------- symmetry modes
+const SymMode SYM_SU2 = {0, 3, 4, {1, -1, 0, 0}, {0, 0, 1, 0}, {0, 1, -1, 0, 0, 0}, {0, 1, 1, 0, 0, 0}};
+const SymMode SYM_U1U1 = {1, 4, 6, {-64, 1, -1, 64}, {0, 0, 0, 0}, {0, 65, 63, -65, -63, 0}, {0, 0, 0, 0, 0, 0}};
+static thread_local const SymMode* t_sym = &SYM_SU2;
+const SymMode& sym() { return *t_sym; }
+SymScope::SymScope(const SymMode* m) : prev(t_sym) { t_sym = m ? m : &SYM_SU2; }
+SymScope::~SymScope() { t_sym = prev; }
+
 // ----------------------------------------------------------------------------- Bond / BlockTensor
 int Bond::find(Sector s) const {
   auto it = std::lower_bound(sec.begin(), sec.end(), s);
@@ -117,8 +125,8 @@ static inline int fuse(Sector a, int s, Sector out[2]) {
 
 // column rank of the (s2, b) group inside a fused row panel: s2 in the order 0, 2, 1, then b by (q, tj)
 static inline int theta_col_rank(int s2, int bq, int btj) {
-  static const int perm[3] = {0, 2, 1};
-  return (perm[s2] << 22) + ((bq + 1024) << 11) + btj;
+  static const int perm[4] = {0, 2, 1, 3};  // SU2: s2 = 0, 2, 1; U1U1: plain order apart from that swap
+  return (perm[s2] << 24) + ((bq + 4096) << 11) + btj;
 }
 
 void layout_site(const Bond& bl, const Bond& br, BlockTensor& out) {
@@ -126,7 +134,7 @@ void layout_site(const Bond& bl, const Bond& br, BlockTensor& out) {
   out.nlab = 5;
   std::vector<std::pair<Key, std::pair<int, int>>> v;
   for (size_t ia = 0; ia < bl.sec.size(); ++ia)
-    for (int s = 0; s < 3; ++s) {
+    for (int s = 0; s < sym().ns; ++s) {
       Sector cs[2];
       int n = fuse(bl.sec[ia], s, cs);
       for (int j = 0; j < n; ++j) {
@@ -144,11 +152,11 @@ void layout_theta(const Bond& bl, const Bond& br, BlockTensor& out) {
   out.nlab = 8;
   std::vector<std::pair<Key, std::pair<int, int>>> v;
   for (size_t ia = 0; ia < bl.sec.size(); ++ia)
-    for (int s1 = 0; s1 < 3; ++s1) {
+    for (int s1 = 0; s1 < sym().ns; ++s1) {
       Sector cs[2];
       int nc = fuse(bl.sec[ia], s1, cs);
       for (int j = 0; j < nc; ++j)
-        for (int s2 = 0; s2 < 3; ++s2) {
+        for (int s2 = 0; s2 < sym().ns; ++s2) {
           Sector bs[2];
           int nb = fuse(cs[j], s2, bs);
           for (int l = 0; l < nb; ++l) {
@@ -183,12 +191,41 @@ void layout_theta(const Bond& bl, const Bond& br, BlockTensor& out) {
 
 // ----------------------------------------------------------------------------- reduced MPO (F-2, F-3)
 void mpo_site_table(int site, double t_h, double U, MpoSite& W) {
-  for (int a = 0; a < 4; ++a)
-    for (int b = 0; b < 4; ++b) {
+  for (int a = 0; a < MAX_NW; ++a)
+    for (int b = 0; b < MAX_NW; ++b) {
       W.rank2[a][b] = -1;
-      for (int i = 0; i < 3; ++i)
-        for (int j = 0; j < 3; ++j) W.val[a][b][i][j] = 0.0;
+      for (int i = 0; i < MAX_NS; ++i)
+        for (int j = 0; j < MAX_NS; ++j) W.val[a][b][i][j] = 0.0;
     }
+  if (sym().id == 1) {
+    // U(1) x U(1): Eq. (1) PAPER.md:26-30 literally.  Local states 0 |0>, 1 |up>, 2 |dn>, 3 |updn> = c+_up c+_dn |0>;
+    // Jordan-Wigner in mode order 1up, 1dn, 2up, ...:  c+_{i s} c_{i+1 s} = (c+_s P)_i (c_s)_{i+1},
+    // c+_{i+1 s} c_{i s} = -(c_s P)_i (c+_s)_{i+1} with P = (-1)^n, so that
+    //   row 0 (start): I, c+_up P, c+_dn P, c_up P, c_dn P, U n_up n_dn;  column 5 (close): -t c_up, -t c_dn, +t c+_up, +t c+_dn;  I.
+    // Non-zero elements <s'|op|s>: c+_up: (1,0) = 1, (3,2) = 1;  c+_dn: (2,0) = 1, (3,1) = -1;  c = transposes.
+    const double P[4] = {1.0, -1.0, -1.0, 1.0};
+    double cu[4][4] = {}, cd[4][4] = {};  // creation operators [s'][s]
+    cu[1][0] = 1.0;
+    cu[3][2] = 1.0;
+    cd[2][0] = 1.0;
+    cd[3][1] = -1.0;
+    for (int w = 0; w < 6; ++w) W.rank2[0][w] = 0;
+    for (int w = 1; w < 6; ++w) W.rank2[w][5] = 0;
+    for (int sp = 0; sp < 4; ++sp)
+      for (int s = 0; s < 4; ++s) {
+        W.val[0][0][sp][s] = W.val[5][5][sp][s] = sp == s ? 1.0 : 0.0;
+        W.val[0][1][sp][s] = cu[sp][s] * P[s];      // c+_up P
+        W.val[0][2][sp][s] = cd[sp][s] * P[s];      // c+_dn P
+        W.val[0][3][sp][s] = cu[s][sp] * P[s];      // c_up P
+        W.val[0][4][sp][s] = cd[s][sp] * P[s];      // c_dn P
+        W.val[1][5][sp][s] = -t_h * cu[s][sp];      // -t c_up
+        W.val[2][5][sp][s] = -t_h * cd[s][sp];      // -t c_dn
+        W.val[3][5][sp][s] = +t_h * cu[sp][s];      // +t c+_up
+        W.val[4][5][sp][s] = +t_h * cd[sp][s];      // +t c+_dn
+      }
+    W.val[0][5][3][3] = U;  // U n_up n_dn
+    return;
+  }
   const double eps = (site % 2 == 0) ? 1.0 : -1.0;  // eps_i = (-1)^i, 0-based (reading A-3)
   const double eps_prev = -eps;
   const double r2 = std::sqrt(2.0);
@@ -735,10 +772,10 @@ void left_contraction_tasks(const BlockTensor& Lenv, const BlockTensor& ket, con
       const Key& kk = ket.keys[ki];
       const int s = kk[2];
       const Sector c = key_sector(kk, 3);
-      for (int wp = 0; wp < 4; ++wp) {
+      for (int wp = 0; wp < sym().nw; ++wp) {
         const int tr = W.rank2[w][wp];
         if (tr < 0) continue;
-        for (int sp = 0; sp < 3; ++sp) {
+        for (int sp = 0; sp < sym().ns; ++sp) {
           const double wv = W.val[w][wp][sp][s];
           if (wv == 0.0) continue;
           Sector cps[2];
@@ -805,7 +842,7 @@ void emit_heff2(const BlockTensor& Lenv, const BlockTensor& Renv, const BlockTen
       const int wr = rk[2];
       const int tr = W2.rank2[wm][wr];
       if (tr < 0) continue;
-      for (int s2p = 0; s2p < 3; ++s2p) {
+      for (int s2p = 0; s2p < sym().ns; ++s2p) {
         const double wv = W2.val[wm][wr][s2p][s2];
         if (wv == 0.0) continue;
         const Key ok = key_theta(ap, s1p, cp, s2p, bp);
@@ -952,7 +989,7 @@ void emit_env_right(const BlockTensor& Renv, const BlockTensor& A, const MpoSite
         const Key& ak = A.keys[ai];  // c(0,1) s(2) b(3,4)
         const Sector c = key_sector(ak, 0);
         const int s = ak[2];
-        for (int w = 0; w < 4; ++w) {
+        for (int w = 0; w < sym().nw; ++w) {
           const int tr = W.rank2[w][wp];
           if (tr < 0) continue;
           const double wv = W.val[w][wp][sp][s];

@@ -1449,23 +1449,31 @@ void fh::measure_local_impl(fh_ctx* ctx, const fh_mps* mps, double* n_i, double*
     ctx->ensure_pinned(chunks.size() * 2 + 2);
     FH_CUDA(cudaMemcpyAsync(ctx->h_pinned, d_part, chunks.size() * 2 * sizeof(double), cudaMemcpyDeviceToHost, s));
     FH_CUDA(cudaStreamSynchronize(s));
-    double one_v = 0.0, sz = 0.0, pd = 0.0;
+    // expectation values of the diagonal one-site operators per site multiplet:
+    //   SU2  (s = up, dn, pair): S^z = (1/2, -1/2, 0), n_up n_dn = (0, 0, 1/2) (half of the pair projector), n = (1, 1, 1)
+    //        (the pair multiplet has <T^z> = 0 in a T_tot = 0 state, reading A-12);
+    //   U1U1 (s = 0, up, dn, updn): S^z = (0, 1/2, -1/2, 0), n_up n_dn = (0, 0, 0, 1), n = (0, 1, 1, 2)
+    static const double SZ[2][4] = {{0.5, -0.5, 0.0, 0.0}, {0.0, 0.5, -0.5, 0.0}};
+    static const double DO[2][4] = {{0.0, 0.0, 0.5, 0.0}, {0.0, 0.0, 0.0, 1.0}};
+    static const double NN[2][4] = {{1.0, 1.0, 1.0, 0.0}, {0.0, 1.0, 1.0, 2.0}};
+    const int md = sym().id;
+    double one_v = 0.0, sz = 0.0, pd = 0.0, nn = 0.0;
     for (size_t c = 0; c < chunks.size(); ++c) {
       const Key& k = A.keys[chunk_blk[c]];
       const double w = (k[4] + 1) * ctx->h_pinned[2 * c];
       one_v += w;
-      if (k[2] == 0) sz += 0.5 * w;
-      if (k[2] == 1) sz -= 0.5 * w;
-      if (k[2] == 2) pd += w;
+      sz += SZ[md][k[2]] * w;
+      pd += DO[md][k[2]] * w;
+      nn += NN[md][k[2]] * w;
     }
-    // <n_i> = <1 + 2 T^z_i> = (w_up + w_dn + 2 * w_pair / 2) / <psi|psi>: the pair multiplet has <T^z_i> = 0 in a
-    // T_tot = 0 state (A-12).  The numerator is this site's sum of multiplet weights, the denominator the norm from
-    // the complete left-to-right contraction (filled in below): the ratio is 1 only if the norm environments, the
-    // multiplet weights and the site tensors are consistent on every site.
-    n_i[i] = one_v;
+    // <n_i> = sum_s n_s w_s / <psi|psi>.  In the SU2 mode n_s = 1 for every multiplet (<n_i> = <1 + 2 T^z_i> and the
+    // pair multiplet has <T^z_i> = 0 in a T_tot = 0 state, A-12): the numerator is the site's sum of multiplet
+    // weights, the denominator the norm from the complete left-to-right contraction (filled in below), and the
+    // ratio is 1 only if norm environments, multiplet weights and site tensors are consistent on every site.
+    n_i[i] = nn;
     FH_REQUIRE(one_v > 0.0, FH_ESTATE, "measure_local: the state has zero weight on a site");
     sz_i[i] = sz / one_v;
-    docc_i[i] = 0.5 * pd / one_v;
+    docc_i[i] = pd / one_v;
     ctx->alloc.release(xoff, A.nelem);
     ctx->free_tensor(N);
     N = Nn;

@@ -860,6 +860,113 @@ def test_mid_size_jacobi_kernel_vs_vendor_svd(H, ctx, tmp_path):
         ctx.mps_destroy(h)
 
 
+# ------------------------------------------------------------------ NEXT-4: U(1) x U(1) mode
+@pytest.fixture()
+def actx(H):
+    c = H.binding.Context(2 << 30)
+    c.fh_set_option(c.OPT_SYMMETRY, 1)
+    yield c
+    c.close()
+
+
+def test_next4_abelian_env_and_apply_parity(H, actx):
+    """U(1) x U(1) mode (FH_OPT_SYMMETRY = 1): environments (H4, H5) along a random abelian
+    chain, the two-site apply on every bond and the one-site apply on every site against oracle/abelian.py
+    (pinned against the dense contractions), <= 1e-11; then the central bond of the abelian profile at chi = 4096
+    (the small-block stress case: 2012 blocks, d_max 148) on ALL output blocks with random environments."""
+    import fh_inputs.abelian as fab
+    from oracle import abelian as ab
+    ctx = actx
+    rng = np.random.default_rng(5)
+    L = 6
+    dims = [{k: min(v, int(rng.integers(1, 6))) for k, v in d.items()} for d in fab.chain_dims(10 ** 6, L)]
+    A = [{k: _rand(rng, dims[i][k[0]], dims[i + 1][k[2]]) for k in ab.site_keys(dims[i], dims[i + 1])} for i in range(L)]
+    W = ab.mpo_elements(1.0, 4.0)
+    Le, Re = [ab.boundary_left()], [None] * (L + 1)
+    for i in range(L):
+        Le.append(ab.env_update_left(Le[i], A[i], W))
+    Re[L] = ab.boundary_right()
+    for i in range(L - 1, -1, -1):
+        Re[i] = ab.env_update_right(Re[i + 1], A[i], W)
+    mpo = ctx.fh_mpo_build(L, 1.0, 4.0)
+    val, rank2 = ctx.fh_mpo_get_site(mpo, 1)
+    for (w, wp), M in W.items():
+        assert np.array_equal(val[w, wp], M) and rank2[w, wp] == 0          # the library's own W = 6 table
+    assert (rank2 >= 0).sum() == len(W)
+    mps = ctx.mps_create(L)
+    for i in range(L):
+        H.set_site(ctx, mps, i, A[i], dims[i], dims[i + 1])
+    for i in range(L):
+        ctx.env_update_left(mpo, mps, i)
+    for i in range(L - 1, -1, -1):
+        ctx.env_update_right(mpo, mps, i)
+    for which, ref in ((0, Le), (1, Re)):
+        for k in range(L + 1):
+            lab, dm, flat = ctx.env_get(mps, which, k)
+            got = H.unflatten(flat, lab, dm, env_key)
+            assert sorted(got) == sorted(ref[k]), (which, k)
+            assert rel_err(got, ref[k], weighted=False) < 1e-12, (which, k)
+    for i in range(L - 1):
+        th = {k: _rand(rng, dims[i][k[0]], dims[i + 2][k[4]]) for k in ab.theta_keys(dims[i], dims[i + 2])}
+        ctx.heff_plan(mpo, mps, i, 2)
+        assert rel_err(_apply_gpu(H, ctx, th, 2), ab.heff2_apply(Le[i], Re[i + 2], th, W, W), weighted=False) < TOL_APPLY
+    for i in range(L):
+        ctx.heff_plan(mpo, mps, i, 1)
+        assert rel_err(_apply_gpu(H, ctx, A[i], 1), ab.heff1_apply(Le[i], Re[i + 1], A[i], W), weighted=False) < TOL_APPLY
+    ctx.mps_destroy(mps)
+    # central bond at chi = 4096
+    Lc, c, chi = 60, 29, 4096
+    dl, dr = fab.profile(c, chi), fab.profile(c + 2, chi)
+    Lk, Rk = ab.env_keys(dl, dl), ab.env_keys(dr, dr)
+    Lenv = fi.random_blocks(9, 1, Lk, {k: (dl[k[0]], dl[k[2]]) for k in Lk})
+    Renv = fi.random_blocks(9, 2, Rk, {k: (dr[k[0]], dr[k[2]]) for k in Rk})
+    th = fab.theta_random(9, c, dl, dr)
+    mpo = ctx.fh_mpo_build(Lc, 1.0, 4.0)
+    mps = ctx.mps_create(Lc)
+    ctx.mps_set_bond(mps, c, dl)
+    ctx.mps_set_bond(mps, c + 2, dr)
+    for which, bond, keys, E in ((0, c, Lk, Lenv), (1, c + 2, Rk, Renv)):
+        labels = [[k[0][0], k[0][1], k[1], k[2][0], k[2][1]] for k in keys]
+        ctx.env_set(mps, which, bond, labels, np.concatenate([E[k].ravel() for k in keys]))
+    ctx.heff_plan(mpo, mps, c, 2)
+    st1, st2 = ab.heff2_tasks(Lk, Rk, sorted(th), W, W)
+    assert ctx.heff_flops() == ab.heff2_flops(st1, st2, dl, dr)
+    got = _apply_gpu(H, ctx, th, 2)
+    ref = symm.run_stage(st2, symm.run_stage(st1, Lenv, th), Renv, "n", "t")    # the pinned lists, executed
+    for k in th:
+        ref.setdefault(k, np.zeros_like(th[k]))
+    e, w = rel_err(got, ref, weighted=False), _per_block_worst(got, {k: v for k, v in ref.items() if np.any(v)})
+    print("abelian chi=4096: %d blocks, %.3g GFLOP, rel. Frobenius %.2e, worst block %.2e" % (len(th), ctx.heff_flops() * 1e-9, e, w))
+    assert e < TOL_APPLY and w < TOL_APPLY
+    ctx.mps_destroy(mps)
+
+
+def test_next4_abelian_tdvp_L8_vs_dense_oracle(H, actx):
+    """U(1) x U(1) two-site TDVP on the L = 8 Neel quench (config 1's problem) against the DENSE oracle O-D
+    (oracle/dense_tdvp.DenseTDVP, pinned against ED): untruncated, the symmetric and the dense algorithm are the
+    same computation, so n_up, n_dn, double occupancy agree to <= 1e-8 after every step (<n_i> is computed from
+    the occupation numbers of the four site states here, not fixed by the representation; it stays 1 by the
+    particle-hole symmetry of the quench); norm and energy (Eq. (1) as it stands) are conserved."""
+    from oracle import dense_tdvp as dtv
+    ctx = actx
+    L, dt, m = 8, 0.05, 10
+    ref = dtv.DenseTDVP(L, 1.0, 4.0, krylov_dim=m)
+    mpo = ctx.fh_mpo_build(L, 1.0, 4.0)
+    mps = ctx.mps_init_neel(mpo, L)
+    worst = 0.0
+    for step in range(12):
+        ref.step(dt)
+        ctx.tdvp2_sweep(mpo, mps, dt, krylov_dim=m, chi_max_full=256, eps_trunc=-1.0)
+        o, g = ref.observables(), ctx.measure_local(mps, L)
+        worst = max(worst, np.abs(g["sz"] - 0.5 * (o["n_up"] - o["n_dn"])).max(), np.abs(g["docc"] - o["docc"]).max(),
+                    np.abs(g["n"] - (o["n_up"] + o["n_dn"])).max())
+        gg = ctx.measure_global(mpo, mps)
+        assert abs(gg["norm2"] - 1) < 1e-10 and abs(gg["energy"]) < 1e-9       # <Neel|H|Neel> = 0 for Eq. (1)
+    print("abelian TDVP L=8 vs dense oracle: max observable difference %.1e, chi %s" % (worst, ctx.tdvp2_last_stats()["chi_full"]))
+    assert worst < 1e-8, worst
+    ctx.mps_destroy(mps)
+
+
 # ------------------------------------------------------------------ H6 / H8 kernels on their own
 @pytest.mark.parametrize("n", [300_001, 1_500_003, 4_700_011])
 def test_vector_kernels_and_block_copy_vs_oracle(H, ctx, n):

@@ -146,6 +146,39 @@ def test_zero_site_task_lists_match_oracle(binding):
     assert f1 + f2 == fl
 
 
+def test_abelian_mode_task_lists_bit_exact(binding):
+    """NEXT-4, U(1) x U(1) mode of the host layer (fh_host_set_symmetry(1)): W = 6 MPO, four site states, packed
+    charges.  Integer task tuples of both stages equal oracle/abelian.heff2_tasks bit for bit on the central bond
+    of the abelian profile (chi = 64, 1024), alpha = the MPO elements exactly, flops equal; the unit lists tile
+    every output once."""
+    import fh_inputs.abelian as fab
+    from oracle import abelian as ab
+    assert binding.lib.fh_host_set_symmetry(1) == 0
+    try:
+        for chi in (64, 1024):
+            dl, dr = fab.profile(29, chi), fab.profile(31, chi)
+            Lk, Rk = ab.env_keys(dl, dl), ab.env_keys(dr, dr)
+            assert Lk == fab.env_block_keys(dl, dl)
+            W = ab.mpo_elements(1.0, 4.0)
+            vk = ab.theta_keys(dl, dr)
+            st1, st2 = ab.heff2_tasks(Lk, Rk, vk, W, W)
+            o1 = symm.task_tuples(st1, list(st1), Lk, vk)
+            o2 = symm.task_tuples(st2, vk, list(st1), Rk)
+            (t1, a1, n1, f1), (t2, a2, n2, f2) = binding.fh_host_plan(29, 2, 1.0, 4.0, dl, dr, Lk, Rk)
+            assert n1 == len(st1) and n2 == len(vk)
+            assert t1.shape == o1[0].shape and (t1 == o1[0]).all() and t2.shape == o2[0].shape and (t2 == o2[0]).all()
+            assert (a1 == o1[1]).all() and (a2 == o2[1]).all()
+            assert f1 + f2 == ab.heff2_flops(st1, st2, dl, dr)
+            for stage in (1, 2):
+                units, outs, padded = binding.fh_host_get_units(stage)
+                cover = [np.zeros(((m + 7) // 8, (n + 7) // 8), dtype=np.int32) for m, n, _ in outs]
+                for o, m0, n0, mt, nt, steps in units:
+                    cover[o][m0 // 8:m0 // 8 + mt, n0 // 8:n0 // 8 + nt] += 1
+                assert all((cv == 1).all() for cv in cover)
+    finally:
+        binding.lib.fh_host_set_symmetry(0)
+
+
 def test_host_only_entry_points_refuse_null_handles(binding):
     """fh_plan_cache_stats / fh_plan_cache_limit / fh_enable_timers are host-only calls: without a GPU they can
     still be reached, and a NULL handle or a negative limit is FH_EINVAL (include/fh_b200.h), never a crash."""
