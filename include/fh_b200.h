@@ -293,6 +293,37 @@ int fh_vec_lincomb(fh_ctx* ctx, int64_t n, int m, const double* coef, const void
 int fh_copy_blocks(fh_ctx* ctx, int nblk, const int64_t* src_off, const int64_t* dst_off, const int32_t* rows, const int32_t* cols,
                    const int32_t* ld_src, const int32_t* ld_dst, const int32_t* transpose, const double* scale,
                    const void* src_dev, void* dst_dev);
+/* ---- the weighted inner product without any allocation ---------------------------------------------------------
+ * fh_vec_wdot_static computes what fh_vec_wdot computes,
+ *     result = sum_b blk_weight[b] * sum_{i in block b} conj(x_i) y_i          (F-6; the reduction of H6),
+ * for callers that may not call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid it).  It needs no context, calls no cudaMalloc / cudaFree / allocating library routine, does not
+ * synchronise and copies nothing to the host: two kernel launches on the caller's stream.
+ *   n, nblk            vector length in complex128 elements and number of blocks: 1 <= nblk <=
+ *                      FH_STATIC_MAX_BLOCKS, 1 <= n <= FH_STATIC_MAX_ELEMS; beyond that FH_EINVAL, nothing launched
+ *   blk_len_dev        DEVICE array of nblk int64 block lengths (>= 0, sum = n; a table that breaks this makes
+ *                      the result NaN + i NaN), blk_weight_dev DEVICE array of nblk int32 weights (2j+1)
+ *   x_dev, y_dev       DEVICE vectors of n complex128 (interleaved re, im); not written
+ *   result_dev         DEVICE, 2 doubles (re, im), written by the second kernel; owned by the caller
+ *   stream             the caller's cudaStream_t (NULL = the default stream)
+ * Its scratch memory (block prefix offsets, one partial sum per CTA, a retirement counter) is ONE file-scope
+ * device array of FH_STATIC_SCRATCH_BYTES bytes, which every GPU that loads the library holds until the process
+ * exits.  All calls share it and it keeps the last call's contents (each call clears what it needs cleared):
+ * calls that overlap on one GPU -- streams without an ordering between them, several host threads -- race on it;
+ * the caller orders them.  The sum is taken per CTA over contiguous 1024-element ranges (longer ones beyond 4 Mi
+ * elements) and then over the CTAs in index order: deterministic, and equal to fh_vec_wdot up to the rounding of a
+ * different summation order.
+ * fh_static_setup takes the device address of the array for the CURRENT device (cudaGetSymbolAddress, once per
+ * device); fh_vec_wdot_static calls it on first use on a device -- call it yourself before a graph capture
+ * starts.  fh_static_last_error: message of the last failed call of these two on the calling thread. */
+#define FH_STATIC_MAX_BLOCKS 16384
+#define FH_STATIC_MAX_ELEMS ((int64_t)1 << 32)
+#define FH_STATIC_SCRATCH_BYTES 196872
+int fh_static_setup(void);
+int fh_vec_wdot_static(int64_t n, int nblk, const int64_t* blk_len_dev, const int32_t* blk_weight_dev, const void* x_dev,
+                       const void* y_dev, double* result_dev, void* stream);
+const char* fh_static_last_error(void);
+
 /* HBM-bound kernels of the path timed in isolation on n_elems complex128
  * elements taken from the arena (FH_ENOMEM if (m + 3) * n_elems do not fit): gbs[0] weighted dot (one launch,
  * last CTA sums the partials), gbs[1] axpy, gbs[2] scale, gbs[3] m-vector linear combination, gbs[4] pack

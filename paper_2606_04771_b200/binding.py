@@ -49,6 +49,9 @@ _SIGS = {
     "fh_dmma_peak_tflops": (c_int, [c_void_p, c_int, P(c_dbl)]),
     "fh_vec_kernels_gbs": (c_int, [c_void_p, c_i64, c_int, c_int, P(c_dbl)]),
     "fh_vec_wdot": (c_int, [c_void_p, c_i64, c_int, c_void_p, c_void_p, c_void_p, c_void_p, P(c_dbl)]),
+    "fh_static_setup": (c_int, []),
+    "fh_vec_wdot_static": (c_int, [c_i64, c_int, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
+    "fh_static_last_error": (C.c_char_p, []),
     "fh_vec_lanczos_update": (c_int, [c_void_p, c_i64, c_int, c_void_p, c_void_p, c_dbl, c_dbl, c_dbl, c_dbl, c_void_p,
                                       c_void_p, c_void_p, P(c_dbl)]),
     "fh_vec_lincomb": (c_int, [c_void_p, c_i64, c_int, c_void_p, c_void_p, c_i64, c_void_p]),
@@ -119,6 +122,26 @@ def _i32(x):
 def fh_canonical_weight(c, b):
     """Metric of a right-canonical site tensor as the LIBRARY defines it (labels (q, tj))."""
     return lib.fh_canonical_weight(int(c[1]), int(b[1]))
+
+
+# ------------------------------------------------------------------ allocation-free entry point (no context)
+STATIC_MAX_BLOCKS, STATIC_MAX_ELEMS, STATIC_SCRATCH_BYTES = 16384, 1 << 32, 196872
+
+
+def fh_static_setup():
+    rc = lib.fh_static_setup()
+    if rc != 0:
+        raise FhError("fh_static_setup: rc=%d: %s" % (rc, lib.fh_static_last_error().decode()))
+
+
+def fh_vec_wdot_static(n, nblk, blk_len_dev, blk_weight_dev, x, y, result, stream=None):
+    """blk_len_dev (int64), blk_weight_dev (int32), x, y (complex128), result (2 float64): CUDA tensors; the call
+    only launches (no synchronisation): read `result` after synchronising the stream."""
+    rc = lib.fh_vec_wdot_static(int(n), int(nblk), c_void_p(blk_len_dev.data_ptr()), c_void_p(blk_weight_dev.data_ptr()),
+                                c_void_p(x.data_ptr()), c_void_p(y.data_ptr()), c_void_p(result.data_ptr()),
+                                c_void_p(stream if stream else 0))
+    if rc != 0:
+        raise FhError("fh_vec_wdot_static: rc=%d: %s" % (rc, lib.fh_static_last_error().decode()))
 
 
 def fh_coef_left(*t):
