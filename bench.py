@@ -268,19 +268,29 @@ def profile_traffic():
 def time_apply_random_envs(H, fi, torch, chi, profile, s2, steps, peak_dmma, local):
     """heff_apply on the central bond of the given workload with iid random environments of the right shapes
     (env_set; timing does not depend on their values, and contracting a chi >= 16384 chain on the host would
-    take minutes).  Own context, so that `arena_peak_bytes` is this workload's."""
+    take minutes).  Own context, so that `arena_peak_bytes` is this workload's.  profile "u1u1": the U(1) x U(1)
+    mode (NEXT-4) on fh_inputs.abelian's profile, the small-block stress case."""
     L, c = 60, 29
-    dims = fi.chain_dims(chi, L, profile, s2)
-    dl, dr = dims[c], dims[c + 2]
+    abelian = profile == "u1u1"
+    if abelian:
+        import fh_inputs.abelian as fab
+        dl, dr = fab.profile(c, chi, L), fab.profile(c + 2, chi, L)
+        env_keys = fab.env_block_keys
+    else:
+        dims = fi.chain_dims(chi, L, profile, s2)
+        dl, dr = dims[c], dims[c + 2]
+        env_keys = fi.env_block_keys
     zest = 40.0 * sum(dl.values()) ** 2 * 16 / 1274.0 ** 2 * 1.2      # Z scales like chi_su2^2 (40 MB at 1274)
     ctx = H.binding.Context(int(max(2 << 30, 6 * zest + (1 << 30))), device="cuda:%d" % local)
     try:
+        if abelian:
+            ctx.fh_set_option(ctx.OPT_SYMMETRY, 1)
         mpo = ctx.fh_mpo_build(L, 1.0, 4.0)
         mps = ctx.mps_create(L)
         ctx.mps_set_bond(mps, c, dl)
         ctx.mps_set_bond(mps, c + 2, dr)
         for which, bond, d in ((0, c, dl), (1, c + 2, dr)):
-            keys = fi.env_block_keys(d, d)
+            keys = env_keys(d, d)
             E = fi.random_blocks(11, 1 + which, keys, {k: (d[k[0]], d[k[2]]) for k in keys})
             labels = [[k[0][0], k[0][1], k[1], k[2][0], k[2][1]] for k in keys]
             ctx.env_set(mps, which, bond, labels, np.concatenate([E[k].ravel() for k in keys]))
@@ -305,7 +315,7 @@ def time_apply_random_envs(H, fi, torch, chi, profile, s2, steps, peak_dmma, loc
         clk = clocks.stop()
         t = sum(a.elapsed_time(b) for a, b in ev) * 1e-3 / steps
         used, peak = ctx.fh_arena_stats()
-        return {"chi": chi, "profile": profile if profile == "gaussian" else "table_s2 x %d/%d" % s2,
+        return {"chi": chi, "profile": profile if profile in ("gaussian", "u1u1") else "table_s2 x %d/%d" % s2,
                 "d_max": max(max(dl.values()), max(dr.values())), "theta_blocks": len(lab), "flop_per_apply": flops,
                 "ms_per_apply": t * 1e3, "gflops": flops / t * 1e-9, "frac_of_dmma_peak": flops / t * 1e-12 / peak_dmma,
                 "steps": steps, "arena_peak_bytes": int(peak), "theta_bytes": 16 * int(ne), "clocks": clk,
@@ -440,7 +450,8 @@ def run_ours(args):
                    "l2": "not flushed" if flush is None else "flushed between timed applies (256 MiB write, outside the event pairs)",
                    "parallelism": "replicas only (one GPU per problem, no collectives)", "setup_seconds": t_build},
         "value_l2_warm": world * flops * args.steps / t_warm * 1e-9,
-        "roofline": {"kernel": "grouped_zgemm_kernel (stage 1 + stage 2 launches of one apply)", "bound": "tensor",
+        "roofline": {"kernel": ("grouped_zgemm_kernel (stage 1 + stage 2 launches of one apply)" if launches == 2 * args.steps else
+                                "grouped_zgemm_ws_kernel (both stages of one apply in one launch)"), "bound": "tensor",
                      "achieved": per_gpu_tf, "peak": peak_dmma, "unit": "TFLOP/s", "frac": per_gpu_tf / peak_dmma,
                      "peak_source": "FP64 DMMA.8x8x4 issue peak measured in this run (fh_dmma_peak_tflops)",
                      "peak_rule": peak_rule, "frac_rule": per_gpu_tf / peak_rule,
@@ -482,7 +493,8 @@ def run_ours(args):
     ctx.close()
     if not args.no_extra and world == 1:
         extra = []
-        for chi_x, prof_x, s2_x, st_x in ((1024, "gaussian", (1, 1), 20), (0, "table_s2", (1, 6), 10),
+        for chi_x, prof_x, s2_x, st_x in ((1024, "gaussian", (1, 1), 20), (4096, "u1u1", (1, 1), 20),
+                                          (0, "table_s2", (1, 6), 10),
                                           (16384, "gaussian", (1, 1), 5), (24576, "gaussian", (1, 1), 3)):
             try:
                 extra.append(time_apply_random_envs(H, fi, torch, chi_x, prof_x, s2_x, st_x, peak_dmma, local))
