@@ -78,6 +78,14 @@ const char* fh_last_error(const fh_ctx* ctx);
  *                        3 = c_up P, 4 = c_dn P, 5 = final (W = 6), all recoupling coefficients 1, MPO of Eq. (1) as it
  *                        stands.  Set it before fh_mpo_build / mps_create and do not change it while they live. */
 #define FH_OPT_SYMMETRY 5
+/*   FH_OPT_PRECISION     arithmetic of the two-site heff_apply (and of every Lanczos step of tdvp2_sweep / heff_expm
+ *                        on a two-site plan): 0 = complex128 on the FP64 tensor pipe (default), 1 = split precision
+ *                        (PAPER.md:264-270): operands, intermediate and result stay complex128 in
+ *                        memory, every product is taken as 3 x TF32 (x = hi + lo, a b ~ hi hi + hi lo + lo hi) on the
+ *                        tcgen05 tensor cores with float32 accumulation in tensor memory: single-precision class
+ *                        error (<= ~1e-6 relative Frobenius per apply; oracle/splitprec.py states the bounds).
+ *                        One-site applies, environment updates, vector kernels and the SVD stay FP64. */
+#define FH_OPT_PRECISION 6
 int fh_set_option(fh_ctx* ctx, int key, int value);
 /* bytes currently allocated / high-water mark in the arena */
 int fh_arena_stats(const fh_ctx* ctx, size_t* used_bytes, size_t* peak_bytes);
@@ -290,6 +298,17 @@ int fh_vec_lanczos_update(fh_ctx* ctx, int64_t n, int nblk, const int64_t* blk_l
                           double bj2, double bjm2, double tol, const void* uj_dev, const void* uprev_dev, void* w_dev,
                           double* norm2_out);
 int fh_vec_lincomb(fh_ctx* ctx, int64_t n, int m, const double* coef, const void* V_dev, int64_t stride, void* y_dev);
+/* The split-precision segmented complex GEMM of FH_OPT_PRECISION = 1 on caller data (
+ * PAPER.md:264-270; oracle/splitprec.py): one output block
+ *     C (M x N, row-major, leading dimension ldc) = sum_t alpha[t] op(A_t) (M x K[t]) B_t (K[t] x N),
+ *     op(A_t)(m, k) = A_dev[a_off[t] + m a_sm[t] + k a_sk[t]]   (conjugated if conj_a),
+ *     B_t(k, n)     = B_dev[b_off[t] + k b_sk[t] + n b_sn[t]]
+ * (offsets and strides in complex128 elements; host arrays of nseg entries; nseg = 0 stores zeros), every product
+ * taken as 3 x TF32 on tcgen05 with float32 accumulation in tensor memory.  A_dev, B_dev, C_dev are device
+ * pointers to complex128; C must not overlap A or B.  Returns after the kernel has finished. */
+int fh_zgemm_split(fh_ctx* ctx, int M, int N, int nseg, const int32_t* K, const double* alpha, int conj_a, const void* A_dev,
+                   const int64_t* a_off, const int32_t* a_sm, const int32_t* a_sk, const void* B_dev, const int64_t* b_off,
+                   const int32_t* b_sk, const int32_t* b_sn, void* C_dev, int ldc);
 int fh_copy_blocks(fh_ctx* ctx, int nblk, const int64_t* src_off, const int64_t* dst_off, const int32_t* rows, const int32_t* cols,
                    const int32_t* ld_src, const int32_t* ld_dst, const int32_t* transpose, const double* scale,
                    const void* src_dev, void* dst_dev);

@@ -54,6 +54,8 @@ _SIGS = {
     "fh_static_last_error": (C.c_char_p, []),
     "fh_vec_lanczos_update": (c_int, [c_void_p, c_i64, c_int, c_void_p, c_void_p, c_dbl, c_dbl, c_dbl, c_dbl, c_void_p,
                                       c_void_p, c_void_p, P(c_dbl)]),
+    "fh_zgemm_split": (c_int, [c_void_p, c_int, c_int, c_int, c_void_p, c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p,
+                               c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int]),
     "fh_vec_lincomb": (c_int, [c_void_p, c_i64, c_int, c_void_p, c_void_p, c_i64, c_void_p]),
     "fh_copy_blocks": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p,
                                c_void_p, c_void_p]),
@@ -392,6 +394,15 @@ class Context:
                                              c_void_p(w.data_ptr()), C.byref(r)), "fh_vec_lanczos_update")
         return r.value
 
+    def fh_zgemm_split(self, M, N, segs, conj_a, A, B, C, ldc):
+        """segs: list of (K, alpha, a_off, a_sm, a_sk, b_off, b_sk, b_sn); A, B, C complex128 CUDA tensors."""
+        K, sm_, sk_, bk_, bn_ = (_i32([g[i] for g in segs]) for i in (0, 3, 4, 6, 7))
+        al = np.ascontiguousarray([g[1] for g in segs], dtype=np.float64)
+        ao, bo = (np.ascontiguousarray([g[i] for g in segs], dtype=np.int64) for i in (2, 5))
+        self.check(lib.fh_zgemm_split(self.h, M, N, len(segs), _np_ptr(K), _np_ptr(al), int(conj_a), c_void_p(A.data_ptr()),
+                                      _np_ptr(ao), _np_ptr(sm_), _np_ptr(sk_), c_void_p(B.data_ptr()), _np_ptr(bo),
+                                      _np_ptr(bk_), _np_ptr(bn_), c_void_p(C.data_ptr()), ldc), "fh_zgemm_split")
+
     def fh_vec_lincomb(self, coef, V, stride, y):
         c = np.ascontiguousarray(coef, dtype=np.complex128)
         self.check(lib.fh_vec_lincomb(self.h, int(y.numel()), len(c), _np_ptr(c), c_void_p(V.data_ptr()), int(stride),
@@ -490,7 +501,7 @@ class Context:
     def fh_launch_count(self):
         return int(lib.fh_launch_count(self.h))
 
-    OPT_GEMM_PATH, OPT_SVD_MID_MAXN, OPT_SVD_THREADS, OPT_SVD_SMALL_MAXN, OPT_SYMMETRY = 1, 2, 3, 4, 5
+    OPT_GEMM_PATH, OPT_SVD_MID_MAXN, OPT_SVD_THREADS, OPT_SVD_SMALL_MAXN, OPT_SYMMETRY, OPT_PRECISION = 1, 2, 3, 4, 5, 6
 
     def fh_set_option(self, key, value):
         self.check(lib.fh_set_option(self.h, int(key), int(value)), "fh_set_option")

@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfh_b200.so")
-SOURCES = ["zgemm.cu", "zgemm_ws.cu", "kernels.cu", "api.cu", "tdvp.cu", "noalloc.cu", "symmetry.cpp", "su2.cpp"]
+SOURCES = ["zgemm.cu", "zgemm_ws.cu", "zgemm_tc.cu", "kernels.cu", "api.cu", "tdvp.cu", "noalloc.cu", "symmetry.cpp", "su2.cpp"]
 HEADERS = ["fh_internal.hpp", "symmetry.hpp", "context.hpp"]
 
 

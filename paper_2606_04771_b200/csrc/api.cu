@@ -265,6 +265,7 @@ void fh::plan_heff(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, 
   P.ws_scratch = -1;
   P.valid = false;
   P.io_ready = false;
+  P.tc_ready = false;
   P.nsite = nsite;
   P.site = site;
   const bool use_cache = nsite == 1 && mps->cache.enabled;
@@ -400,9 +401,35 @@ void fh::vec_export(fh_ctx* ctx, const cplx* vec, cplx* blocks) {
   FH_CUDA(cudaGetLastError());
 }
 
+// Split-precision apply (NEXT-3): the same two stages, task lists, operands and intermediate as the FP64 apply, the
+// products taken as 3 x TF32 on the tcgen05 tensor cores (zgemm_tc.cu)
+static void apply_heff_tc(fh_ctx* ctx, const cplx* theta, cplx* out) {
+  Plan& P = ctx->plan;
+  if (!P.tc_ready) {
+    std::vector<TcTile> t1, t2;
+    build_tc_tiles(P.st1, t1);
+    build_tc_tiles(P.st2, t2);
+    P.tc_pool.reset();
+    P.tc_pool.reserve((t1.size() + t2.size()) * sizeof(TcTile) + 4096, ctx->stream);
+    P.d_tc1 = upload(P.tc_pool, t1, ctx->stream);
+    P.d_tc2 = upload(P.tc_pool, t2, ctx->stream);
+    P.n_tc1 = (int)t1.size();
+    P.n_tc2 = (int)t2.size();
+    FH_CUDA(cudaStreamSynchronize(ctx->stream));  // t1 / t2 are stack-owned
+    P.tc_ready = true;
+  }
+  cplx* Z = ctx->ptr(P.Z.base);
+  launch_grouped_gemm_tc(P.d_tc1, P.n_tc1, P.st1.d_segs, P.st1.opA != OPA_N, P.Lptr, theta, Z, ctx->num_sms, ctx->stream,
+                         &ctx->launches);
+  launch_grouped_gemm_tc(P.d_tc2, P.n_tc2, P.st2.d_segs, P.st2.opA != OPA_N, Z, P.Rptr, out, ctx->num_sms, ctx->stream,
+                         &ctx->launches);
+  FH_CUDA(cudaGetLastError());
+}
+
 void fh::apply_heff(fh_ctx* ctx, const cplx* theta, cplx* out) {
   Plan& P = ctx->plan;
   FH_REQUIRE(P.valid, FH_ESTATE, "heff_apply: no plan (call heff_plan first)");
+  if (ctx->opt_precision == 1 && P.nsite == 2) return apply_heff_tc(ctx, theta, out);
   cplx* Z = ctx->ptr(P.Z.base);
   // Which form: measured on the Gaussian and Table-S2 profiles the warp-specialised single
   // launch wins from about 1e7 padded DMMAs per apply upwards (chi ~ 5000 - 12000: +5 ... +10 %), ties above and
@@ -749,6 +776,7 @@ void fh_ctx_destroy(fh_ctx* c) {
   for (auto e : c->ev_free) cudaEventDestroy(e);
   c->plan.pool.destroy();
   c->plan.io_pool.destroy();
+  c->plan.tc_pool.destroy();
   if (c->d_ws_counters) cudaFree(c->d_ws_counters);
   if (c->d_fact_status) cudaFree(c->d_fact_status);
   if (c->h_fact_status) cudaFreeHost(c->h_fact_status);
@@ -788,6 +816,10 @@ int fh_set_option(fh_ctx* c, int key, int value) {
     case FH_OPT_SVD_SMALL_MAXN:
       if (value < 0 || value > 4096) return FH_EINVAL;
       c->opt_svd_small_maxn = value;
+      return FH_OK;
+    case FH_OPT_PRECISION:
+      if (value < 0 || value > 1) return FH_EINVAL;
+      c->opt_precision = (int)value;
       return FH_OK;
     case FH_OPT_SYMMETRY:
       if (value < 0 || value > 1) return FH_EINVAL;
@@ -1641,6 +1673,50 @@ int fh_vec_lanczos_update(fh_ctx* ctx, int64_t n, int nblk, const int64_t* blk_l
     FH_CUDA(cudaMemcpyAsync(ctx->h_pinned + 4, d_sc + 4, 2 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     FH_CUDA(cudaStreamSynchronize(ctx->stream));
     *norm2_out = ctx->h_pinned[4];
+  })
+}
+
+int fh_zgemm_split(fh_ctx* ctx, int M, int N, int nseg, const int32_t* K, const double* alpha, int conj_a, const void* A_dev,
+                   const int64_t* a_off, const int32_t* a_sm, const int32_t* a_sk, const void* B_dev, const int64_t* b_off,
+                   const int32_t* b_sk, const int32_t* b_sn, void* C_dev, int ldc) {
+  FH_TRY(ctx, {
+    FH_REQUIRE(ctx && M > 0 && N > 0 && nseg >= 0 && ldc >= N && A_dev && B_dev && C_dev, FH_EINVAL, "fh_zgemm_split: bad argument");
+    FH_REQUIRE(nseg == 0 || (K && alpha && a_off && a_sm && a_sk && b_off && b_sk && b_sn), FH_EINVAL,
+               "fh_zgemm_split: segment arrays missing");
+    Stage st;
+    GemmOut o;
+    o.c_off = 0;
+    o.M = M;
+    o.N = N;
+    o.seg_begin = 0;
+    o.seg_end = nseg;
+    o.ldc = ldc;
+    o.steps = 0;
+    o.col0 = 0;
+    for (int t = 0; t < nseg; ++t) {
+      FH_REQUIRE(K[t] >= 0, FH_EINVAL, "fh_zgemm_split: negative K");
+      GemmSeg g;
+      g.a_off = a_off[t];
+      g.b_off = b_off[t];
+      g.K = K[t];
+      g.a_sm = a_sm[t];
+      g.a_sk = a_sk[t];
+      g.b_sk = b_sk[t];
+      g.b_sn = b_sn[t];
+      g.pad = 0;
+      g.alpha = alpha[t];
+      st.segs.push_back(g);
+    }
+    st.mouts.push_back(o);
+    std::vector<TcTile> tiles;
+    build_tc_tiles(st, tiles);
+    ctx->pool_aux.reserve(tiles.size() * sizeof(TcTile) + st.segs.size() * sizeof(GemmSeg) + 4096, ctx->stream);
+    TcTile* d_t = upload(ctx->pool_aux, tiles, ctx->stream);
+    GemmSeg* d_s = upload(ctx->pool_aux, st.segs, ctx->stream);
+    launch_grouped_gemm_tc(d_t, (int)tiles.size(), d_s, conj_a ? 1 : 0, (const cplx*)A_dev, (const cplx*)B_dev, (cplx*)C_dev,
+                           ctx->num_sms, ctx->stream, &ctx->launches);
+    FH_CUDA(cudaGetLastError());
+    FH_CUDA(cudaStreamSynchronize(ctx->stream));  // tiles / segs are stack-owned
   })
 }
 

@@ -77,6 +77,12 @@ struct Plan {
   CopyBlk* d_import = nullptr;
   CopyBlk* d_export = nullptr;
   DevPool io_pool;
+  // tile lists of the split-precision form (FH_OPT_PRECISION = 1), built on first use per plan
+  bool tc_ready = false;
+  int n_tc1 = 0, n_tc2 = 0;
+  fh::TcTile* d_tc1 = nullptr;
+  fh::TcTile* d_tc2 = nullptr;
+  DevPool tc_pool;
 };
 
 // What the emitter produces for one two-site plan; filled by a second host thread while the main thread runs
@@ -197,6 +203,7 @@ struct fh_ctx {
   int opt_svd_mid_maxn = 128;
   int opt_svd_small_maxn = 4096;
   int opt_svd_threads = 0;    // 0 = default
+  int opt_precision = 0;      // fh_set_option(FH_OPT_PRECISION): 0 = FP64 DMMA, 1 = 3 x TF32 on tcgen05 (two-site applies)
   int num_sms = 148;
   unsigned* d_ws_counters = nullptr;  // tile-queue head and retired-CTA count of the warp-specialised GEMM (zero between launches)
   // status words of the last batch of sector factorisations (one per matrix, + one more per matrix for the

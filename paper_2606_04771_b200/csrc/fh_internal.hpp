@@ -267,6 +267,15 @@ void launch_grouped_gemm_ws_pair(const WsPair& pr, const cplx* A1, const cplx* B
                                  cplx* C2, unsigned* d_counters, int grid, cplx* scratch, unsigned* flags,
                                  unsigned* dep_counters, unsigned epoch, cudaStream_t s, int64_t* launch_counter);
 int ws_smem_bytes();
+// split-precision form on tcgen05 (zgemm_tc.cu, NEXT-3): a tile = up to 128 x 128 of a merged output over all its
+// segments (chunks = sum of ceil(K / 16)); same segment array, operands and results as the FP64 forms
+struct TcTile {
+  int64_t c_off;
+  int ldc, m0, n0, h, w, seg_begin, seg_end, chunks, pad;
+};
+void build_tc_tiles(const Stage& st, std::vector<TcTile>& tiles);
+void launch_grouped_gemm_tc(const TcTile* d_tiles, int ntiles, const GemmSeg* d_segs, int conjA, const cplx* A, const cplx* B,
+                            cplx* C, int grid, cudaStream_t s, int64_t* launch_counter);
 void launch_wdot(const VecChunk* d_chunks, int nchunks, const cplx* x, const cplx* y, double* d_partial,
                  double* d_result, cudaStream_t s, int64_t* launch_counter);
 // y = y + a*x (a complex, from device scalar array coef[idx]*sign) etc.: see kernels.cu

@@ -1,0 +1,336 @@
+// Split-precision form of the segmented grouped complex GEMM (
+// reading A-18) on the fifth-generation tensor cores:
+//     C_o (M x N) = sum_{t in seg(o)} alpha_t * op(A_t) (M x K_t) * op(B_t) (K_t x N),  alpha_t real,
+// with complex128 operands and results in memory (the same task lists, layouts and launch interface as zgemm.cu)
+// and the products taken as 3 x TF32:  x = hi + lo (+ 2^-22 |x|),  a b ~ hi hi + hi lo + lo hi, accumulated in
+// float32 in tensor memory (oracle/splitprec.py states the arithmetic and its two error bounds).
+//
+// One persistent CTA per SM, 13 warps, three roles that meet only at mbarriers:
+//   * 8 CONVERTER warps (4 for the A panel, 4 for the B panel; one lane = one row of the 128-row panel) walk the
+//     k range of a tile 16 k at a time: complex128 loads straight from the operand blocks (any stride pair, zero
+//     beyond a segment's K), alpha and the conjugation sign folded into A, every real number split into its two
+//     TF32 parts, and the four planes (re hi, re lo, im hi, im lo) of the panel written to shared memory in the
+//     K-major no-swizzle core-matrix layout tcgen05.mma reads (8 rows x 16 B per core matrix; 128 B between
+//     row groups, 2048 B between k quads).  No packed copy of an operand exists in global memory: the split
+//     representation is 16 B per complex number, as many bytes as the complex128 it is made from.
+//   * ONE thread issues the MMAs: per 8 k, 12 x tcgen05.mma.kind::tf32 (M = 128, N = the tile width rounded up
+//     to 16): Re C += Ar Br - Ai Bi, Im C += Ar Bi + Ai Br, each as hi hi + hi lo + lo hi; the minus sign is the
+//     negate-A bit of the instruction descriptor.  Accumulators: 2 x 128 float32 columns of tensor memory per
+//     tile, double buffered (all 512 columns).  tcgen05.commit hands a shared-memory stage back to the converters
+//     and, after the last chunk of a tile, the accumulator buffer over to the epilogue.
+//   * 4 EPILOGUE warps (warp w owns TMEM lanes 32 w ... 32 w + 31 = tile rows) read the accumulators with
+//     tcgen05.ld (32 lanes x 32 columns per instruction), widen them to double and store complex128.
+// All K segments of an output accumulate in tensor memory (alpha is inside A), so there is one epilogue per tile.
+// Tiles are taken round-robin from a list sorted heaviest first; a tile without segments is stored as zeros.
+// Deterministic: fixed tile -> CTA map, fixed k order, one accumulator per output element.
+#include "fh_internal.hpp"
+
+#include <algorithm>
+
+namespace fh {
+
+namespace {
+
+constexpr int TC_STAGES = 3;
+constexpr int TC_KC = 16;                          // k per chunk = two MMA k-steps of 8
+constexpr int TC_PLANE = 128 * TC_KC * 4;          // one TF32 plane of a panel: 128 rows x 16 k
+constexpr int TC_OPERAND = 4 * TC_PLANE;           // re hi, re lo, im hi, im lo
+constexpr int TC_STAGE_BYTES = 2 * TC_OPERAND;     // A panel + B panel = 64 KB
+constexpr int TC_EPI_WARPS = 4, TC_CONV_WARPS = 8;
+constexpr int TC_MMA_WARP = TC_EPI_WARPS;          // warp 4
+constexpr int TC_THREADS = 32 * (TC_EPI_WARPS + 1 + TC_CONV_WARPS);
+constexpr int TC_NBAR = 2 * TC_STAGES + 4;
+constexpr int TC_SMEM_BYTES = TC_STAGES * TC_STAGE_BYTES + 8 * TC_NBAR + 16;
+constexpr uint32_t TC_LBO = 2048, TC_SBO = 128;    // byte strides between core matrices along k / along rows
+
+__device__ __forceinline__ void mbar_init(uint32_t a, int count) {
+  asm volatile("mbarrier.init.shared.b64 [%0], %1;" ::"r"(a), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t a) {
+  asm volatile("mbarrier.arrive.shared.b64 _, [%0];" ::"r"(a) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t a, uint32_t parity) {
+  uint32_t ok = 0;
+  while (!ok) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(a), "r"(parity)
+        : "memory");
+  }
+}
+__device__ __forceinline__ uint32_t tf32_of(float f) {
+  uint32_t r;
+  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(f));
+  return r;
+}
+// x -> (hi, lo): hi = tf32(float(x)), lo = tf32(float(x - hi)), the difference in double (exact)
+__device__ __forceinline__ void split_tf32(double x, uint32_t& hi, uint32_t& lo) {
+  hi = tf32_of(__double2float_rn(x));
+  lo = tf32_of(__double2float_rn(x - (double)__uint_as_float(hi)));
+}
+__device__ __forceinline__ void sts128(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+// shared-memory matrix descriptor: K-major, no swizzle, version 1 (sm_100)
+__device__ __forceinline__ uint64_t smem_desc(uint32_t addr) {
+  return (uint64_t)((addr >> 4) & 0x3FFF) | ((uint64_t)(TC_LBO >> 4) << 16) | ((uint64_t)(TC_SBO >> 4) << 32) |
+         ((uint64_t)1 << 46);
+}
+// instruction descriptor: D float32, A / B TF32, both K-major, M = 128, N = n
+__device__ __forceinline__ uint32_t instr_desc(int n, int neg_a) {
+  return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)neg_a << 13) | ((uint32_t)(n >> 3) << 17) | (8u << 24);
+}
+__device__ __forceinline__ void mma_tf32(uint32_t d_tmem, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
+      ::"r"(d_tmem), "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+__device__ __forceinline__ void mma_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+        "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]),
+        "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]),
+        "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+      : "r"(taddr)
+      : "memory");
+}
+
+struct TcSmem {
+  uint32_t data, full, empty, tfull, tempty, tptr;
+  __device__ __forceinline__ uint32_t a_panel(int s) const { return data + s * TC_STAGE_BYTES; }
+  __device__ __forceinline__ uint32_t b_panel(int s) const { return data + s * TC_STAGE_BYTES + TC_OPERAND; }
+};
+
+// ------------------------------------------------------------------------------------------------ converters
+// One lane = one row of a 32-row group of its panel.  Per chunk and row: 16 complex128 -> 4 planes x 16 TF32.
+// op(A)(m, k) = A[a_off + m a_sm + k a_sk], op(B)(k, n) = B[b_off + k b_sk + n b_sn]: both panels are "row x k".
+__device__ __forceinline__ void convert_rows(const cplx* __restrict__ base, int64_t row_stride, int64_t k_stride, bool row_valid,
+                                             int k0, int K, double scale, double im_sign, uint32_t panel, int row) {
+  const uint32_t dst = panel + (uint32_t)((row >> 3) * TC_SBO + (row & 7) * 16);
+  if (!row_valid) return;  // rows beyond the tile edge only feed accumulator rows / columns that are never stored
+  const cplx* p = base + (int64_t)row * row_stride + (int64_t)k0 * k_stride;
+  cplx z[TC_KC];
+#pragma unroll
+  for (int i = 0; i < TC_KC; ++i) {
+    z[i] = make_double2(0.0, 0.0);
+    if (k0 + i < K) z[i] = __ldg(p + (int64_t)i * k_stride);
+  }
+#pragma unroll
+  for (int q = 0; q < TC_KC / 4; ++q) {
+    uint32_t rh[4], rl[4], ih[4], il[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      split_tf32(z[4 * q + i].x * scale, rh[i], rl[i]);
+      split_tf32(z[4 * q + i].y * scale * im_sign, ih[i], il[i]);
+    }
+    const uint32_t a = dst + q * TC_LBO;
+    sts128(a, rh[0], rh[1], rh[2], rh[3]);
+    sts128(a + TC_PLANE, rl[0], rl[1], rl[2], rl[3]);
+    sts128(a + 2 * TC_PLANE, ih[0], ih[1], ih[2], ih[3]);
+    sts128(a + 3 * TC_PLANE, il[0], il[1], il[2], il[3]);
+  }
+}
+
+__device__ __forceinline__ void converter_loop(const TcTile* __restrict__ tiles, int ntiles, const GemmSeg* __restrict__ segs,
+                                               const cplx* __restrict__ A, const cplx* __restrict__ B, double conj_sign,
+                                               const TcSmem& sm, int cw, int lane) {
+  const bool is_a = cw < 4;
+  const int row = 32 * (cw & 3) + lane;
+  uint32_t g = 0;  // chunks produced so far by this CTA
+  for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+    const TcTile tl = tiles[t];
+    const bool row_valid = is_a ? row < tl.h : row < tl.w;
+    for (int si = tl.seg_begin; si < tl.seg_end; ++si) {
+      const GemmSeg sg = segs[si];
+      const cplx* base = is_a ? A + sg.a_off + (int64_t)tl.m0 * sg.a_sm : B + sg.b_off + (int64_t)tl.n0 * sg.b_sn;
+      const int64_t rs = is_a ? sg.a_sm : sg.b_sn, ks = is_a ? sg.a_sk : sg.b_sk;
+      const double scale = is_a ? sg.alpha : 1.0, isg = is_a ? conj_sign : 1.0;
+      for (int k0 = 0; k0 < sg.K; k0 += TC_KC, ++g) {
+        const int s = g % TC_STAGES;
+        mbar_wait(sm.empty + 8 * s, ((g / TC_STAGES) & 1) ^ 1);
+        convert_rows(base, rs, ks, row_valid, k0, sg.K, scale, isg, is_a ? sm.a_panel(s) : sm.b_panel(s), row);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy stores -> visible to the MMA (async proxy)
+        mbar_arrive(sm.full + 8 * s);
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ MMA issuer
+__device__ __forceinline__ void mma_loop(const TcTile* __restrict__ tiles, int ntiles, const TcSmem& sm, uint32_t tmem) {
+  uint32_t g = 0, tt = 0;
+  for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+    const TcTile tl = tiles[t];
+    if (tl.chunks == 0) continue;
+    const int n_inst = max(16, (tl.w + 15) & ~15);
+    const uint32_t id_pos = instr_desc(n_inst, 0), id_neg = instr_desc(n_inst, 1);
+    const uint32_t buf = tt & 1;
+    mbar_wait(sm.tempty + 8 * buf, ((tt >> 1) & 1) ^ 1);
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t d_re = tmem + buf * 256, d_im = d_re + 128;
+    for (int c = 0; c < tl.chunks; ++c, ++g) {
+      const int s = g % TC_STAGES;
+      mbar_wait(sm.full + 8 * s, (g / TC_STAGES) & 1);
+      asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll
+      for (int j = 0; j < TC_KC / 8; ++j) {
+        const uint32_t pa = sm.a_panel(s) + j * 2 * TC_LBO, pb = sm.b_panel(s) + j * 2 * TC_LBO;
+        const uint64_t ar_h = smem_desc(pa), ar_l = smem_desc(pa + TC_PLANE), ai_h = smem_desc(pa + 2 * TC_PLANE),
+                       ai_l = smem_desc(pa + 3 * TC_PLANE);
+        const uint64_t br_h = smem_desc(pb), br_l = smem_desc(pb + TC_PLANE), bi_h = smem_desc(pb + 2 * TC_PLANE),
+                       bi_l = smem_desc(pb + 3 * TC_PLANE);
+        const uint32_t acc = (c | j) != 0;
+        // Re C += Ar Br - Ai Bi
+        mma_tf32(d_re, ar_h, br_h, id_pos, acc);
+        mma_tf32(d_re, ar_h, br_l, id_pos, 1);
+        mma_tf32(d_re, ar_l, br_h, id_pos, 1);
+        mma_tf32(d_re, ai_h, bi_h, id_neg, 1);
+        mma_tf32(d_re, ai_h, bi_l, id_neg, 1);
+        mma_tf32(d_re, ai_l, bi_h, id_neg, 1);
+        // Im C += Ar Bi + Ai Br
+        mma_tf32(d_im, ar_h, bi_h, id_pos, acc);
+        mma_tf32(d_im, ar_h, bi_l, id_pos, 1);
+        mma_tf32(d_im, ar_l, bi_h, id_pos, 1);
+        mma_tf32(d_im, ai_h, br_h, id_pos, 1);
+        mma_tf32(d_im, ai_h, br_l, id_pos, 1);
+        mma_tf32(d_im, ai_l, br_h, id_pos, 1);
+      }
+      mma_commit(sm.empty + 8 * s);  // the stage is free once these MMAs have read it
+    }
+    mma_commit(sm.tfull + 8 * buf);  // accumulators of the tile complete
+    ++tt;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ epilogue
+__device__ __forceinline__ void epilogue_loop(const TcTile* __restrict__ tiles, int ntiles, cplx* __restrict__ C,
+                                              const TcSmem& sm, uint32_t tmem, int warp, int lane) {
+  const int row = 32 * warp + lane;
+  uint32_t tt = 0;
+  for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+    const TcTile tl = tiles[t];
+    cplx* crow = C + tl.c_off + (int64_t)(tl.m0 + row) * tl.ldc + tl.n0;
+    if (tl.chunks == 0) {  // an output without contributions
+      if (row < tl.h)
+        for (int c = 0; c < tl.w; ++c) crow[c] = make_double2(0.0, 0.0);
+      continue;
+    }
+    const uint32_t buf = tt & 1;
+    mbar_wait(sm.tfull + 8 * buf, (tt >> 1) & 1);
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t t_re = tmem + ((uint32_t)(32 * warp) << 16) + buf * 256;
+    for (int c0 = 0; c0 < tl.w; c0 += 32) {
+      uint32_t re[32], im[32];
+      tmem_ld32(t_re + c0, re);
+      tmem_ld32(t_re + 128 + c0, im);
+      asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+      if (row < tl.h) {
+#pragma unroll
+        for (int i = 0; i < 32; ++i)
+          if (c0 + i < tl.w) crow[c0 + i] = make_double2((double)__uint_as_float(re[i]), (double)__uint_as_float(im[i]));
+      }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    mbar_arrive(sm.tempty + 8 * buf);
+    ++tt;
+  }
+}
+
+__global__ void __launch_bounds__(TC_THREADS, 1)
+    grouped_zgemm_tc_kernel(const TcTile* __restrict__ tiles, int ntiles, const GemmSeg* __restrict__ segs,
+                            const cplx* __restrict__ A, const cplx* __restrict__ B, cplx* __restrict__ C, int conjA) {
+  extern __shared__ __align__(1024) unsigned char tc_smem[];
+  TcSmem sm;
+  sm.data = (uint32_t)__cvta_generic_to_shared(tc_smem);
+  sm.full = sm.data + TC_STAGES * TC_STAGE_BYTES;
+  sm.empty = sm.full + 8 * TC_STAGES;
+  sm.tfull = sm.empty + 8 * TC_STAGES;
+  sm.tempty = sm.tfull + 16;
+  sm.tptr = sm.tempty + 16;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < TC_STAGES; ++s) {
+      mbar_init(sm.full + 8 * s, 32 * TC_CONV_WARPS);  // every converter thread arrives after its own stores
+      mbar_init(sm.empty + 8 * s, 1);                  // tcgen05.commit
+    }
+    for (int b = 0; b < 2; ++b) {
+      mbar_init(sm.tfull + 8 * b, 1);                  // tcgen05.commit
+      mbar_init(sm.tempty + 8 * b, 32 * TC_EPI_WARPS);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == TC_MMA_WARP) {  // all 512 columns: two accumulator buffers of 2 x 128 (one CTA per SM, nobody to share with)
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(sm.tptr), "r"(512) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  uint32_t tmem;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem) : "r"(sm.tptr) : "memory");
+
+  if (warp < TC_EPI_WARPS) {
+    epilogue_loop(tiles, ntiles, C, sm, tmem, warp, lane);
+  } else if (warp == TC_MMA_WARP) {
+    if (lane == 0) mma_loop(tiles, ntiles, sm, tmem);
+    __syncwarp();
+  } else {
+    converter_loop(tiles, ntiles, segs, A, B, conjA ? -1.0 : 1.0, sm, warp - TC_MMA_WARP - 1, lane);
+  }
+
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  if (warp == TC_MMA_WARP)
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512) : "memory");
+}
+
+}  // namespace
+
+// 128 x 128 tiles of the merged outputs, heaviest first
+void build_tc_tiles(const Stage& st, std::vector<TcTile>& tiles) {
+  tiles.clear();
+  for (const GemmOut& o : st.mouts) {
+    int chunks = 0;
+    for (int s = o.seg_begin; s < o.seg_end; ++s) chunks += (st.segs[s].K + TC_KC - 1) / TC_KC;
+    for (int m0 = 0; m0 < o.M; m0 += 128)
+      for (int n0 = 0; n0 < o.N; n0 += 128) {
+        TcTile t;
+        t.c_off = o.c_off;
+        t.ldc = o.ldc;
+        t.m0 = m0;
+        t.n0 = n0;
+        t.h = std::min(128, o.M - m0);
+        t.w = std::min(128, o.N - n0);
+        t.seg_begin = o.seg_begin;
+        t.seg_end = o.seg_end;
+        t.chunks = chunks;
+        t.pad = 0;
+        tiles.push_back(t);
+      }
+  }
+  std::stable_sort(tiles.begin(), tiles.end(), [](const TcTile& a, const TcTile& b) {
+    return (int64_t)a.chunks * ((a.w + 15) / 16) > (int64_t)b.chunks * ((b.w + 15) / 16);
+  });
+}
+
+void launch_grouped_gemm_tc(const TcTile* d_tiles, int ntiles, const GemmSeg* d_segs, int conjA, const cplx* A, const cplx* B,
+                            cplx* C, int grid, cudaStream_t s, int64_t* lc) {
+  if (ntiles == 0) return;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaFuncSetAttribute(grouped_zgemm_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES);
+    attr_set = true;
+  }
+  grouped_zgemm_tc_kernel<<<std::min(grid, ntiles), TC_THREADS, TC_SMEM_BYTES, s>>>(d_tiles, ntiles, d_segs, A, B, C, conjA);
+  ++*lc;
+}
+
+}  // namespace fh

@@ -1051,3 +1051,110 @@ def test_edge_cases_and_error_codes(H, ctx):
     with pytest.raises(B.FhError, match="arena"):
         H.build_central_bond(small, mpo2, 4096, 60)
     small.close()
+
+
+# ------------------------------------------------------------------ NEXT-3: split precision (3 x TF32 on tcgen05)
+def _split_case(rng, M, N, Ks, conj, tA, tB):
+    """Segments with every operand orientation the task lists use; returns (binding segments, oracle segments, A, B)."""
+    segs, osegs, Abuf, Bbuf, ao, bo = [], [], [], [], 0, 0
+    for K in Ks:
+        A, Bm = _rand(rng, M, K), _rand(rng, K, N)
+        al = float(rng.uniform(0.5, 2.0)) * (1 if rng.random() < 0.5 else -1)
+        Abuf.append(np.ascontiguousarray(A.T).ravel() if tA else A.ravel())
+        Bbuf.append(np.ascontiguousarray(Bm.T).ravel() if tB else Bm.ravel())
+        segs.append((K, al, ao, 1 if tA else K, M if tA else 1, bo, 1 if tB else N, K if tB else 1))
+        osegs.append((al, A.conj() if conj else A, Bm))
+        ao += M * K
+        bo += K * N
+    cat = lambda b: np.concatenate(b) if b else np.zeros(1, dtype=np.complex128)
+    return segs, osegs, cat(Abuf), cat(Bbuf)
+
+
+@pytest.mark.parametrize("M,N,Ks,conj,tA,tB", [
+    (128, 128, [16], 0, 0, 0), (128, 128, [8], 0, 0, 0), (128, 16, [16], 1, 0, 0), (64, 48, [20], 0, 0, 0),
+    (1, 1, [1], 0, 0, 0), (129, 257, [1, 3, 17], 1, 1, 0), (100, 77, [50, 13], 1, 0, 1),
+    (300, 500, [129, 64, 200], 0, 1, 1), (57, 33, [], 0, 0, 0), (1000, 1000, [512, 300], 0, 0, 0)])
+def test_next3_zgemm_split_vs_oracle(H, ctx, M, N, Ks, conj, tA, tB):
+    """fh_zgemm_split (tcgen05.mma kind::tf32, accumulators in tensor memory) against oracle/splitprec.py, element by
+    element: |C - zgemm_split| <= the float32-accumulation bound K 2^-23 S, hence |C - exact| <= that + the split
+    bound 3.1 2^-22 S; nothing outside the M x N block (leading dimension N + 3) is touched.  Cases: one tile / one
+    k-step, ragged tiles and tails in all three dimensions, several segments, every operand orientation of the task
+    lists (A as stored / transposed / conjugated, B as stored / transposed), an output without segments, 8 x 8
+    tiles with 51 chunks."""
+    from oracle import splitprec as sp
+    torch = _torch()
+    rng = np.random.default_rng(1000 * M + N)
+    segs, osegs, A, B = _split_case(rng, M, N, Ks, conj, tA, tB)
+    ldc = N + 3
+    dC = torch.full((M * ldc,), 7 + 7j, dtype=torch.complex128, device="cuda")
+    ctx.fh_zgemm_split(M, N, segs, conj, _dev(A), _dev(B), dC, ldc)
+    C = dC.cpu().numpy().reshape(M, ldc)
+    assert np.all(C[:, N:] == 7 + 7j)
+    C = C[:, :N]
+    if not Ks:
+        assert not C.any()
+        return
+    exact = sum(al * (a @ b) for al, a, b in osegs)
+    acc, spl = sp.split_bounds(osegs, M, N)
+    assert np.all(np.abs(C - sp.zgemm_split(osegs, M, N)) <= acc)
+    assert np.all(np.abs(C - exact) <= acc + spl)
+    e = np.linalg.norm(C - exact) / np.linalg.norm(exact)
+    assert e < 2e-5 and (sum(Ks) < 64 or e > 1e-9)               # single-precision class, and really the split path
+    dC2 = torch.empty_like(dC)
+    ctx.fh_zgemm_split(M, N, segs, conj, _dev(A), _dev(B), dC2, ldc)
+    assert bool((dC2.view(torch.float64).reshape(M, ldc, 2)[:, :N] == dC.view(torch.float64).reshape(M, ldc, 2)[:, :N]).all())
+
+
+@pytest.mark.parametrize("chi", [1024, 4096])
+def test_next3_split_apply_vs_oracle_all_blocks(H, chi):
+    """FH_OPT_PRECISION = 1 on the plan bench.py times (chi = 4096) and on config 2: the two-site apply through
+    the split-precision kernels (same task lists, layout and intermediate as the FP64 apply) against the FP64
+    oracle on ALL output blocks.  Tolerance: two chained stages, each within K_total 2^-23 of its operands'
+    absolute sums (oracle/splitprec.py); K_total <= ~900 here, so 1e-4 relative Frobenius bounds it with room;
+    measured 2e-6 ... 8e-6.  The FP64 apply of the same plan stays at 1e-11 when the option is switched back."""
+    L, c = 60, 29
+    o = central_bond(chi, L)
+    dims, W = o["dims"], o["W"]
+    ctx = H.binding.Context(int(max(1 << 30, 64.0 * chi * chi)))
+    try:
+        mpo = ctx.fh_mpo_build(L, 1.0, 4.0)
+        mps, gdims = H.build_central_bond(ctx, mpo, chi, L)
+        th = fi.theta_random(fi.SEED, c, dims[c], dims[c + 2])
+        ref = symm.heff2_apply(o["Lenv"], o["Renv"], th, W[c], W[c + 1])
+        ctx.heff_plan(mpo, mps, c, 2)
+        lab, dm, ne = ctx.heff_layout(2)
+        x = H.to_planned(ctx, H.flatten(th, lab, dm, H.theta_key))
+        y = _torch().empty_like(x)
+        ctx.fh_set_option(ctx.OPT_PRECISION, 1)
+        ctx.heff_apply(x, y)
+        got = H.unflatten(H.from_planned(ctx, y), lab, dm, H.theta_key)
+        e, w = rel_err(got, ref), _per_block_worst(got, ref)
+        print("split-precision apply chi=%d: rel. Frobenius %.2e, worst block %.2e" % (chi, e, w))
+        assert 1e-9 < e < 1e-4 and w < 1e-3
+        ctx.fh_set_option(ctx.OPT_PRECISION, 0)
+        ctx.heff_apply(x, y)
+        assert rel_err(H.unflatten(H.from_planned(ctx, y), lab, dm, H.theta_key), ref) < TOL_APPLY
+    finally:
+        ctx.close()
+
+
+def test_next3_split_tdvp_gate_L8(H, ctx):
+    """The paper's acceptance test of reduced precision (abs delta <n_up> < 1e-3) on config 1's
+    problem: 20 two-site TDVP steps of the L = 8 Neel quench with every H_eff application of the Lanczos steps in
+    split precision, against the dense FP64 oracle."""
+    from oracle import dense_tdvp as dtv
+    L, dt, m = 8, 0.05, 10
+    ref = dtv.DenseTDVP(L, 1.0, 4.0, krylov_dim=m)
+    ctx.fh_set_option(ctx.OPT_PRECISION, 1)
+    mpo = ctx.fh_mpo_build(L, 1.0, 4.0)
+    mps = ctx.mps_init_neel(mpo, L)
+    worst = 0.0
+    for step in range(20):
+        ref.step(dt)
+        ctx.tdvp2_sweep(mpo, mps, dt, krylov_dim=m, chi_max_full=256, eps_trunc=-1.0)
+        o, g = ref.observables(), ctx.measure_local(mps, L)
+        worst = max(worst, np.abs(g["sz"] - 0.5 * (o["n_up"] - o["n_dn"])).max(), np.abs(g["docc"] - o["docc"]).max())
+    gg = ctx.measure_global(mpo, mps)
+    print("split-precision TDVP L=8, 20 steps: max |delta <S^z_i>|, |delta <n_up n_dn>| = %.1e, norm^2 - 1 = %.1e" % (worst, gg["norm2"] - 1))
+    assert 1e-12 < worst < 1e-3 and abs(gg["norm2"] - 1) < 1e-3
+    ctx.mps_destroy(mps)
