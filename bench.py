@@ -315,7 +315,30 @@ def time_apply_random_envs(H, fi, torch, chi, profile, s2, steps, peak_dmma, loc
         clk = clocks.stop()
         t = sum(a.elapsed_time(b) for a, b in ev) * 1e-3 / steps
         used, peak = ctx.fh_arena_stats()
+        split = None
+        if max(max(dl.values()), max(dr.values())) >= 128 and not abelian:
+            # NEXT-3: the same apply with FH_OPT_PRECISION = 1 (3 x TF32 on tcgen05, zgemm_tc.cu), L2 flushed as above;
+            # the error is taken against the FP64 apply of this run (the oracle comparison lives in tests/)
+            y64 = y.clone()
+            ctx.fh_set_option(ctx.OPT_PRECISION, 1)
+            for _ in range(2):
+                ctx.heff_apply(x, y)
+            torch.cuda.synchronize()
+            for a, b in ev:
+                flush.zero_()
+                a.record()
+                ctx.heff_apply(x, y)
+                b.record()
+            torch.cuda.synchronize()
+            ts = sum(a.elapsed_time(b) for a, b in ev) * 1e-3 / steps
+            err = float((torch.linalg.norm(y - y64) / torch.linalg.norm(y64)).item())
+            ctx.fh_set_option(ctx.OPT_PRECISION, 0)
+            split = {"arithmetic": "3 x TF32 on tcgen05, float32 accumulation in tensor memory (FH_OPT_PRECISION = 1)",
+                     "ms_per_apply": ts * 1e3, "gflops_complex128_equivalent": flops / ts * 1e-9,
+                     "speedup_vs_fp64": t / ts, "rel_frobenius_vs_fp64_apply": err,
+                     "tf32_tflops_issued_lower_bound": 3.0 * flops / ts * 1e-12}
         return {"chi": chi, "profile": profile if profile in ("gaussian", "u1u1") else "table_s2 x %d/%d" % s2,
+                "split_precision": split,
                 "d_max": max(max(dl.values()), max(dr.values())), "theta_blocks": len(lab), "flop_per_apply": flops,
                 "ms_per_apply": t * 1e3, "gflops": flops / t * 1e-9, "frac_of_dmma_peak": flops / t * 1e-12 / peak_dmma,
                 "steps": steps, "arena_peak_bytes": int(peak), "theta_bytes": 16 * int(ne), "clocks": clk,

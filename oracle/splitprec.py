@@ -8,21 +8,24 @@ and PAPER.md:284-286 (S2.5) accepts the result when abs delta <n_46,up> < 1e-3. 
 matrix engine is the TF32 tensor core (1 sign, 8 exponent, 10 explicit mantissa bits), so the single-precision
 variant of the contraction is the standard "3 x TF32" split (reading A-18):
 
-    x  =  hi + lo + r,     hi = tf32(x),   lo = tf32(x - hi),   |r| <= 2^-22 |x|
+    x  =  hi + lo + r,     hi = round11(x),   lo = round11(x - hi),   |r| <= 2^-22 |x|
+    (round11: to 11 significant bits = the TF32 mantissa, nearest, ties away from zero, taken on the float64
+    value directly -- no intermediate float32 rounding; magnitudes below 2^-126 are flushed to zero)
     a b  ~  hi_a hi_b + hi_a lo_b + lo_a hi_b                    (lo_a lo_b <= 2^-22 |a b| is dropped)
 
 applied to the real and imaginary parts of alpha * op(A) and op(B) separately, the four real products of a
 complex product accumulated in single precision.  Every product of two TF32 numbers is exact in float32 (11 + 11
 significant bits), so the only rounding besides the split is the float32 accumulation, whose ORDER the hardware
 does not define.  The oracle therefore
-  * defines the split bit by bit (tf32_round: round to nearest, ties away from zero -- PTX cvt.rna.tf32.f32),
+  * defines the split bit by bit (round11 on the bit pattern of the double; tf32_round is the same rounding on
+    float32 input -- PTX cvt.rna.tf32.f32 -- and agrees with it on every float32 number),
   * evaluates the three-term product with float64 accumulation (zgemm_split): the value any accumulation order
     approaches, and
   * states the two bounds a kernel has to meet element by element (split_bounds):
         |C_kernel - zgemm_split|  <=  K_total 2^-23 S       (float32 accumulation, worst case, S below)
         |zgemm_split - C_exact|   <=  3.1 * 2^-22 S         (the split itself)
     with S = |alpha| (|Re A| + |Im A|) (|Re B| + |Im B|) summed over k.
-Functions: tf32_round, split_tf32, zgemm_split, split_bounds.
+Functions: tf32_round, round11, split_tf32, zgemm_split, split_bounds.
 """
 import numpy as np
 
@@ -41,13 +44,24 @@ def tf32_round(x):
     return out.view(np.float32).reshape(f.shape)
 
 
+def round11(x):
+    """float64 -> float64 with at most 11 significant bits: nearest, ties away from zero (add half a unit of the
+    11-bit mantissa -- bit 41 of the pattern -- and clear the 42 bits below; a carry out of the mantissa moves
+    into the exponent, as it must).  |result| < 2^-126 (not a normal float32) -> 0."""
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    bits = x.view(np.uint64)
+    r = ((bits + np.uint64(1 << 41)) & np.uint64(0xFFFFFC0000000000)).view(np.float64).reshape(x.shape).copy()
+    r[np.abs(r) < 2.0 ** -126] = 0.0
+    return r
+
+
 def split_tf32(x):
-    """x (float64) -> (hi, lo), both TF32-valued float32 arrays: hi = tf32(float32(x)), lo = tf32(float32(x - hi)),
-    the difference taken in float64 (exact: hi has 11 significant bits)."""
+    """x (float64) -> (hi, lo), both TF32-valued float32 arrays: hi = round11(x), lo = round11(x - hi), the
+    difference taken in float64 (exact: hi has 11 significant bits)."""
     x = np.asarray(x, dtype=np.float64)
-    hi = tf32_round(x.astype(np.float32))
-    lo = tf32_round((x - hi.astype(np.float64)).astype(np.float32))
-    return hi, lo
+    hi = round11(x)
+    lo = round11(x - hi)
+    return hi.astype(np.float32), lo.astype(np.float32)
 
 
 def _real3(ah, al, bh, bl):

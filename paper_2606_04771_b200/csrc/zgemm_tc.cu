@@ -2,7 +2,7 @@
 // reading A-18) on the fifth-generation tensor cores:
 //     C_o (M x N) = sum_{t in seg(o)} alpha_t * op(A_t) (M x K_t) * op(B_t) (K_t x N),  alpha_t real,
 // with complex128 operands and results in memory (the same task lists, layouts and launch interface as zgemm.cu)
-// and the products taken as 3 x TF32:  x = hi + lo (+ 2^-22 |x|),  a b ~ hi hi + hi lo + lo hi, accumulated in
+// and the products taken as 3 x TF32:  x = hi + lo (+ 2^-22 |x|; hi, lo = x and x - hi rounded to 11 significant bits),  a b ~ hi hi + hi lo + lo hi, accumulated in
 // float32 in tensor memory (oracle/splitprec.py states the arithmetic and its two error bounds).
 //
 // One persistent CTA per SM, 13 warps, three roles that meet only at mbarriers:
@@ -59,15 +59,22 @@ __device__ __forceinline__ void mbar_wait(uint32_t a, uint32_t parity) {
         : "memory");
   }
 }
-__device__ __forceinline__ uint32_t tf32_of(float f) {
-  uint32_t r;
-  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(f));
-  return r;
+// x -> (hi, lo), both TF32 numbers in float32 bit patterns, with integer arithmetic on the bits of the double
+// (F2F.F32.F64 runs at 8 per clock and SM on this part, measured; the integer pipe at 64+):
+//   round11(v): v rounded to 11 significant bits, ties away from zero = add half a unit (bit 41 of the double =
+//               bit 9 of its high word) and clear the 42 bits below; the low word plays no part;
+//   hi = round11(x), lo = round11(x - hi) (the difference is exact in double).
+// A double with <= 11 significant bits becomes a float32 by re-biasing the exponent (1023 -> 127) and moving the
+// 20 mantissa bits of the high word up by 3; magnitudes below 2^-126 become (sub)zero bits: max(., 0).
+__device__ __forceinline__ uint32_t round11_hiword(double v) { return ((uint32_t)__double2hiint(v) + 0x200u) & 0xFFFFFC00u; }
+__device__ __forceinline__ uint32_t f32_bits_of_hiword(uint32_t hw) {
+  const int e = max((int)(hw & 0x7FFFFFFFu) - 0x38000000, 0);
+  return ((uint32_t)e << 3) | (hw & 0x80000000u);
 }
-// x -> (hi, lo): hi = tf32(float(x)), lo = tf32(float(x - hi)), the difference in double (exact)
 __device__ __forceinline__ void split_tf32(double x, uint32_t& hi, uint32_t& lo) {
-  hi = tf32_of(__double2float_rn(x));
-  lo = tf32_of(__double2float_rn(x - (double)__uint_as_float(hi)));
+  const uint32_t hh = round11_hiword(x);
+  hi = f32_bits_of_hiword(hh);
+  lo = f32_bits_of_hiword(round11_hiword(x - __hiloint2double((int)hh, 0)));
 }
 __device__ __forceinline__ void sts128(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
   asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
@@ -112,8 +119,9 @@ struct TcSmem {
 // ------------------------------------------------------------------------------------------------ converters
 // One lane = one row of a 32-row group of its panel.  Per chunk and row: 16 complex128 -> 4 planes x 16 TF32.
 // op(A)(m, k) = A[a_off + m a_sm + k a_sk], op(B)(k, n) = B[b_off + k b_sk + n b_sn]: both panels are "row x k".
+template <bool IS_A>
 __device__ __forceinline__ void convert_rows(const cplx* __restrict__ base, int64_t row_stride, int64_t k_stride, bool row_valid,
-                                             int k0, int K, double scale, double im_sign, uint32_t panel, int row) {
+                                             int k0, int K, double scale, double im_scale, uint32_t panel, int row) {
   const uint32_t dst = panel + (uint32_t)((row >> 3) * TC_SBO + (row & 7) * 16);
   if (!row_valid) return;  // rows beyond the tile edge only feed accumulator rows / columns that are never stored
   const cplx* p = base + (int64_t)row * row_stride + (int64_t)k0 * k_stride;
@@ -128,8 +136,8 @@ __device__ __forceinline__ void convert_rows(const cplx* __restrict__ base, int6
     uint32_t rh[4], rl[4], ih[4], il[4];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-      split_tf32(z[4 * q + i].x * scale, rh[i], rl[i]);
-      split_tf32(z[4 * q + i].y * scale * im_sign, ih[i], il[i]);
+      split_tf32(IS_A ? z[4 * q + i].x * scale : z[4 * q + i].x, rh[i], rl[i]);
+      split_tf32(IS_A ? z[4 * q + i].y * im_scale : z[4 * q + i].y, ih[i], il[i]);
     }
     const uint32_t a = dst + q * TC_LBO;
     sts128(a, rh[0], rh[1], rh[2], rh[3]);
@@ -156,7 +164,8 @@ __device__ __forceinline__ void converter_loop(const TcTile* __restrict__ tiles,
       for (int k0 = 0; k0 < sg.K; k0 += TC_KC, ++g) {
         const int s = g % TC_STAGES;
         mbar_wait(sm.empty + 8 * s, ((g / TC_STAGES) & 1) ^ 1);
-        convert_rows(base, rs, ks, row_valid, k0, sg.K, scale, isg, is_a ? sm.a_panel(s) : sm.b_panel(s), row);
+        if (is_a) convert_rows<true>(base, rs, ks, row_valid, k0, sg.K, scale, scale * isg, sm.a_panel(s), row);
+        else convert_rows<false>(base, rs, ks, row_valid, k0, sg.K, 1.0, 1.0, sm.b_panel(s), row);
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy stores -> visible to the MMA (async proxy)
         mbar_arrive(sm.full + 8 * s);
       }

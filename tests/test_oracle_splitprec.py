@@ -27,8 +27,15 @@ def test_tf32_round_hand_worked_values():
     for x, want in cases.items():
         got = float(sp.tf32_round(np.float32(x)).reshape(-1)[0])
         assert got == want, (x, got, want)
-    r = sp.tf32_round(np.random.default_rng(1).standard_normal(4096).astype(np.float32))
+    f = np.random.default_rng(1).standard_normal(4096).astype(np.float32)
+    r = sp.tf32_round(f)
     assert np.all(r.view(np.uint32) & np.uint32(0x1FFF) == 0)          # 13 low mantissa bits are zero
+    # round11 (on doubles) is the same rounding: equal on every float32 number, hand-worked values included
+    assert np.array_equal(sp.round11(f.astype(np.float64)), r.astype(np.float64))
+    for x, want in cases.items():
+        assert float(sp.round11(np.array([x]))[0]) == want, x
+    assert float(sp.round11(np.array([1.0 + 2.0 ** -11 - 2.0 ** -40]))[0]) == 1.0          # just below the tie: down
+    assert float(sp.round11(np.array([2.0 ** -130]))[0]) == 0.0                          # below float32's normal range
 
 
 def test_split_remainder_bound_and_tf32_valued_parts():
@@ -38,8 +45,8 @@ def test_split_remainder_bound_and_tf32_valued_parts():
     for part in (hi, lo):
         assert part.dtype == np.float32 and np.all(part.view(np.uint32) & np.uint32(0x1FFF) == 0)
     r = x - hi.astype(np.float64) - lo.astype(np.float64)
-    assert np.all(np.abs(r) <= 2.0 ** -22 * (1 + 2.0 ** -10) * np.abs(x))
-    assert np.all(np.abs(x - hi) <= (2.0 ** -11 + 2.0 ** -23) * np.abs(x))
+    assert np.all(np.abs(r) <= 2.0 ** -22 * np.abs(x))
+    assert np.all(np.abs(x - hi) <= 2.0 ** -11 * np.abs(x))
     assert np.abs(r).max() > 2.0 ** -26 * np.abs(x).max() * 1e-3         # the remainder is really there (22, not 53 bits)
 
 
