@@ -406,23 +406,43 @@ void fh::vec_export(fh_ctx* ctx, const cplx* vec, cplx* blocks) {
 static void apply_heff_tc(fh_ctx* ctx, const cplx* theta, cplx* out) {
   Plan& P = ctx->plan;
   if (!P.tc_ready) {
+    // tile lists of both stages, and the static operand of each stage (stage 1: the left environment as op(A),
+    // stage 2: the right environment as op(B)) converted ONCE per plan into panel images that the kernel streams
+    // with bulk copies; the operand that changes with every apply (theta, Z) is converted inside the kernel
     std::vector<TcTile> t1, t2;
-    build_tc_tiles(P.st1, t1);
-    build_tc_tiles(P.st2, t2);
+    std::vector<int> cb1, cb2;
+    std::vector<int64_t> img1, img2;
+    std::vector<TcPackChunk> pc1, pc2;
+    build_tc_tiles(P.st1, ctx->num_sms, t1, cb1);
+    build_tc_tiles(P.st2, ctx->num_sms, t2, cb2);
+    const int64_t b1 = build_tc_static(P.st1, true, img1, pc1), b2 = build_tc_static(P.st2, false, img2, pc2);
     P.tc_pool.reset();
-    P.tc_pool.reserve((t1.size() + t2.size()) * sizeof(TcTile) + 4096, ctx->stream);
+    P.tc_pool.reserve((t1.size() + t2.size()) * sizeof(TcTile) + (img1.size() + img2.size()) * 8 + 8 * (size_t)ctx->num_sms + 2048 +
+                          (pc1.size() + pc2.size()) * sizeof(TcPackChunk) + (size_t)(b1 + b2) + 8192,
+                      ctx->stream);
     P.d_tc1 = upload(P.tc_pool, t1, ctx->stream);
     P.d_tc2 = upload(P.tc_pool, t2, ctx->stream);
+    P.d_tc_cb1 = upload(P.tc_pool, cb1, ctx->stream);
+    P.d_tc_cb2 = upload(P.tc_pool, cb2, ctx->stream);
+    P.d_tc_img1 = upload(P.tc_pool, img1, ctx->stream);
+    P.d_tc_img2 = upload(P.tc_pool, img2, ctx->stream);
+    TcPackChunk* d_pc1 = upload(P.tc_pool, pc1, ctx->stream);
+    TcPackChunk* d_pc2 = upload(P.tc_pool, pc2, ctx->stream);
+    P.tc_images1 = (unsigned char*)P.tc_pool.take((size_t)b1 + 256);
+    P.tc_images2 = (unsigned char*)P.tc_pool.take((size_t)b2 + 256);
     P.n_tc1 = (int)t1.size();
     P.n_tc2 = (int)t2.size();
-    FH_CUDA(cudaStreamSynchronize(ctx->stream));  // t1 / t2 are stack-owned
+    launch_tc_pack(d_pc1, (int)pc1.size(), P.Lptr, P.tc_images1, P.st1.opA != OPA_N, ctx->stream, &ctx->launches);
+    launch_tc_pack(d_pc2, (int)pc2.size(), P.Rptr, P.tc_images2, 0, ctx->stream, &ctx->launches);
+    FH_CUDA(cudaGetLastError());
+    FH_CUDA(cudaStreamSynchronize(ctx->stream));  // the host vectors are stack-owned
     P.tc_ready = true;
   }
   cplx* Z = ctx->ptr(P.Z.base);
-  launch_grouped_gemm_tc(P.d_tc1, P.n_tc1, P.st1.d_segs, P.st1.opA != OPA_N, P.Lptr, theta, Z, ctx->num_sms, ctx->stream,
-                         &ctx->launches);
-  launch_grouped_gemm_tc(P.d_tc2, P.n_tc2, P.st2.d_segs, P.st2.opA != OPA_N, Z, P.Rptr, out, ctx->num_sms, ctx->stream,
-                         &ctx->launches);
+  launch_grouped_gemm_tc(P.d_tc1, P.d_tc_cb1, ctx->num_sms, P.n_tc1, P.st1.d_segs, P.st1.opA != OPA_N, P.Lptr, theta, Z, ctx->stream,
+                         &ctx->launches, 1, P.d_tc_img1, P.tc_images1);
+  launch_grouped_gemm_tc(P.d_tc2, P.d_tc_cb2, ctx->num_sms, P.n_tc2, P.st2.d_segs, P.st2.opA != OPA_N, Z, P.Rptr, out, ctx->stream,
+                         &ctx->launches, 2, P.d_tc_img2, P.tc_images2);
   FH_CUDA(cudaGetLastError());
 }
 
@@ -1709,12 +1729,14 @@ int fh_zgemm_split(fh_ctx* ctx, int M, int N, int nseg, const int32_t* K, const 
     }
     st.mouts.push_back(o);
     std::vector<TcTile> tiles;
-    build_tc_tiles(st, tiles);
-    ctx->pool_aux.reserve(tiles.size() * sizeof(TcTile) + st.segs.size() * sizeof(GemmSeg) + 4096, ctx->stream);
+    std::vector<int> cb;
+    build_tc_tiles(st, ctx->num_sms, tiles, cb);
+    ctx->pool_aux.reserve(tiles.size() * sizeof(TcTile) + st.segs.size() * sizeof(GemmSeg) + cb.size() * 4 + 8192, ctx->stream);
     TcTile* d_t = upload(ctx->pool_aux, tiles, ctx->stream);
+    int* d_cb = upload(ctx->pool_aux, cb, ctx->stream);
     GemmSeg* d_s = upload(ctx->pool_aux, st.segs, ctx->stream);
-    launch_grouped_gemm_tc(d_t, (int)tiles.size(), d_s, conj_a ? 1 : 0, (const cplx*)A_dev, (const cplx*)B_dev, (cplx*)C_dev,
-                           ctx->num_sms, ctx->stream, &ctx->launches);
+    launch_grouped_gemm_tc(d_t, d_cb, ctx->num_sms, (int)tiles.size(), d_s, conj_a ? 1 : 0, (const cplx*)A_dev, (const cplx*)B_dev,
+                           (cplx*)C_dev, ctx->stream, &ctx->launches);
     FH_CUDA(cudaGetLastError());
     FH_CUDA(cudaStreamSynchronize(ctx->stream));  // tiles / segs are stack-owned
   })

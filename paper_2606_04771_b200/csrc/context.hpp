@@ -82,6 +82,12 @@ struct Plan {
   int n_tc1 = 0, n_tc2 = 0;
   fh::TcTile* d_tc1 = nullptr;
   fh::TcTile* d_tc2 = nullptr;
+  int* d_tc_cb1 = nullptr;                // first tile of every persistent CTA (tiles are dealt on the host)
+  int* d_tc_cb2 = nullptr;
+  int64_t* d_tc_img1 = nullptr;           // per segment: byte offset of its static operand's panel images
+  int64_t* d_tc_img2 = nullptr;
+  unsigned char* tc_images1 = nullptr;    // stage 1: left environment as op(A); stage 2: right environment as op(B)
+  unsigned char* tc_images2 = nullptr;
   DevPool tc_pool;
 };
 

@@ -273,9 +273,19 @@ struct TcTile {
   int64_t c_off;
   int ldc, m0, n0, h, w, seg_begin, seg_end, chunks, pad;
 };
-void build_tc_tiles(const Stage& st, std::vector<TcTile>& tiles);
-void launch_grouped_gemm_tc(const TcTile* d_tiles, int ntiles, const GemmSeg* d_segs, int conjA, const cplx* A, const cplx* B,
-                            cplx* C, int grid, cudaStream_t s, int64_t* launch_counter);
+void build_tc_tiles(const Stage& st, int grid, std::vector<TcTile>& tiles, std::vector<int>& cta_begin);
+// one 128-row x 16-k chunk of a static operand's panel images (zgemm_tc.cu): source element (row r, k) =
+// X[src_off + r rs + k ks], `rows` x `kleft` of it valid, image of 32 KB at byte dst_off
+struct TcPackChunk {
+  int64_t src_off, dst_off;
+  int rs, ks, rows, kleft;
+};
+int64_t build_tc_static(const Stage& st, bool a_side, std::vector<int64_t>& seg_img, std::vector<TcPackChunk>& chunks);
+void launch_tc_pack(const TcPackChunk* d_chunks, int nchunks, const cplx* X, unsigned char* images, int conj, cudaStream_t s,
+                    int64_t* launch_counter);
+void launch_grouped_gemm_tc(const TcTile* d_tiles, const int* d_cta_begin, int grid, int ntiles, const GemmSeg* d_segs, int conjA,
+                            const cplx* A, const cplx* B, cplx* C, cudaStream_t s, int64_t* launch_counter, int mode = 0,
+                            const int64_t* d_seg_img = nullptr, const unsigned char* images = nullptr);
 void launch_wdot(const VecChunk* d_chunks, int nchunks, const cplx* x, const cplx* y, double* d_partial,
                  double* d_result, cudaStream_t s, int64_t* launch_counter);
 // y = y + a*x (a complex, from device scalar array coef[idx]*sign) etc.: see kernels.cu

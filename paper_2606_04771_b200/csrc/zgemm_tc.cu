@@ -21,11 +21,13 @@
 //   * 4 EPILOGUE warps (warp w owns TMEM lanes 32 w ... 32 w + 31 = tile rows) read the accumulators with
 //     tcgen05.ld (32 lanes x 32 columns per instruction), widen them to double and store complex128.
 // All K segments of an output accumulate in tensor memory (alpha is inside A), so there is one epilogue per tile.
-// Tiles are taken round-robin from a list sorted heaviest first; a tile without segments is stored as zeros.
+// Tiles are dealt to the CTAs on the host (heaviest first to the least loaded); a tile without segments is stored as zeros.
 // Deterministic: fixed tile -> CTA map, fixed k order, one accumulator per output element.
 #include "fh_internal.hpp"
 
 #include <algorithm>
+#include <map>
+#include <tuple>
 
 namespace fh {
 
@@ -36,9 +38,9 @@ constexpr int TC_KC = 16;                          // k per chunk = two MMA k-st
 constexpr int TC_PLANE = 128 * TC_KC * 4;          // one TF32 plane of a panel: 128 rows x 16 k
 constexpr int TC_OPERAND = 4 * TC_PLANE;           // re hi, re lo, im hi, im lo
 constexpr int TC_STAGE_BYTES = 2 * TC_OPERAND;     // A panel + B panel = 64 KB
-constexpr int TC_EPI_WARPS = 4, TC_CONV_WARPS = 8;
+constexpr int TC_EPI_WARPS = 4, TC_CONV_WARPS = 16;
 constexpr int TC_MMA_WARP = TC_EPI_WARPS;          // warp 4
-constexpr int TC_THREADS = 32 * (TC_EPI_WARPS + 1 + TC_CONV_WARPS);
+constexpr int TC_THREADS = 32 * (TC_EPI_WARPS + 1 + TC_CONV_WARPS + 1);  // + the warp whose lane 0 issues the bulk copies
 constexpr int TC_NBAR = 2 * TC_STAGES + 4;
 constexpr int TC_SMEM_BYTES = TC_STAGES * TC_STAGE_BYTES + 8 * TC_NBAR + 16;
 constexpr uint32_t TC_LBO = 2048, TC_SBO = 128;    // byte strides between core matrices along k / along rows
@@ -117,55 +119,77 @@ struct TcSmem {
 };
 
 // ------------------------------------------------------------------------------------------------ converters
-// One lane = one row of a 32-row group of its panel.  Per chunk and row: 16 complex128 -> 4 planes x 16 TF32.
+// One thread = one row of its panel and NK of the chunk's 16 k: NK complex128 -> 4 planes x NK TF32.
 // op(A)(m, k) = A[a_off + m a_sm + k a_sk], op(B)(k, n) = B[b_off + k b_sk + n b_sn]: both panels are "row x k".
-template <bool IS_A>
-__device__ __forceinline__ void convert_rows(const cplx* __restrict__ base, int64_t row_stride, int64_t k_stride, bool row_valid,
-                                             int k0, int K, double scale, double im_scale, uint32_t panel, int row) {
-  const uint32_t dst = panel + (uint32_t)((row >> 3) * TC_SBO + (row & 7) * 16);
-  if (!row_valid) return;  // rows beyond the tile edge only feed accumulator rows / columns that are never stored
-  const cplx* p = base + (int64_t)row * row_stride + (int64_t)k0 * k_stride;
-  cplx z[TC_KC];
+// `dst` = address of (row, first k of this thread) in plane 0; generic address space: shared memory in the GEMM
+// kernel, global memory in the kernel that packs a static operand once per plan (same image either way).
+template <int NK, bool SCALE, bool TO_SHARED>
+__device__ __forceinline__ void convert_row(const cplx* __restrict__ p, int64_t k_stride, int k_left, double scale, double im_scale,
+                                            uint32_t dst_s, unsigned char* dst_g) {
+  cplx z[NK];
 #pragma unroll
-  for (int i = 0; i < TC_KC; ++i) {
+  for (int i = 0; i < NK; ++i) {
     z[i] = make_double2(0.0, 0.0);
-    if (k0 + i < K) z[i] = __ldg(p + (int64_t)i * k_stride);
+    if (i < k_left) z[i] = __ldg(p + (int64_t)i * k_stride);
   }
 #pragma unroll
-  for (int q = 0; q < TC_KC / 4; ++q) {
+  for (int q = 0; q < NK / 4; ++q) {
     uint32_t rh[4], rl[4], ih[4], il[4];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-      split_tf32(IS_A ? z[4 * q + i].x * scale : z[4 * q + i].x, rh[i], rl[i]);
-      split_tf32(IS_A ? z[4 * q + i].y * im_scale : z[4 * q + i].y, ih[i], il[i]);
+      split_tf32(SCALE ? z[4 * q + i].x * scale : z[4 * q + i].x, rh[i], rl[i]);
+      split_tf32(SCALE ? z[4 * q + i].y * im_scale : z[4 * q + i].y, ih[i], il[i]);
     }
-    const uint32_t a = dst + q * TC_LBO;
-    sts128(a, rh[0], rh[1], rh[2], rh[3]);
-    sts128(a + TC_PLANE, rl[0], rl[1], rl[2], rl[3]);
-    sts128(a + 2 * TC_PLANE, ih[0], ih[1], ih[2], ih[3]);
-    sts128(a + 3 * TC_PLANE, il[0], il[1], il[2], il[3]);
+    if (TO_SHARED) {
+      const uint32_t a = dst_s + q * TC_LBO;
+      sts128(a, rh[0], rh[1], rh[2], rh[3]);
+      sts128(a + TC_PLANE, rl[0], rl[1], rl[2], rl[3]);
+      sts128(a + 2 * TC_PLANE, ih[0], ih[1], ih[2], ih[3]);
+      sts128(a + 3 * TC_PLANE, il[0], il[1], il[2], il[3]);
+    } else {
+      unsigned char* a = dst_g + q * TC_LBO;
+      *reinterpret_cast<uint4*>(a) = make_uint4(rh[0], rh[1], rh[2], rh[3]);
+      *reinterpret_cast<uint4*>(a + TC_PLANE) = make_uint4(rl[0], rl[1], rl[2], rl[3]);
+      *reinterpret_cast<uint4*>(a + 2 * TC_PLANE) = make_uint4(ih[0], ih[1], ih[2], ih[3]);
+      *reinterpret_cast<uint4*>(a + 3 * TC_PLANE) = make_uint4(il[0], il[1], il[2], il[3]);
+    }
   }
 }
 
-__device__ __forceinline__ void converter_loop(const TcTile* __restrict__ tiles, int ntiles, const GemmSeg* __restrict__ segs,
+// MODE 0: both operands converted in the loop (4 + 4 warps, 16 k per thread), alpha folded into A.
+// MODE 1: A is STATIC (an environment: converted once per plan into panel images, streamed by cp.async.bulk), all
+//         8 converter warps work on B (8 k per thread) and fold alpha into it.
+// MODE 2: B is static, all 8 converter warps work on A and fold alpha (and the conjugation sign) into it.
+template <int MODE>
+__device__ __forceinline__ void converter_loop(const TcTile* __restrict__ tiles, const int* __restrict__ cta_begin, const GemmSeg* __restrict__ segs,
                                                const cplx* __restrict__ A, const cplx* __restrict__ B, double conj_sign,
-                                               const TcSmem& sm, int cw, int lane) {
-  const bool is_a = cw < 4;
-  const int row = 32 * (cw & 3) + lane;
+                                               const TcSmem& sm, int ct) {
+  const bool is_a = MODE == 0 ? ct < 256 : MODE == 2;
+  const int row = ct & 127;
+  const int kpart = MODE == 0 ? 8 * ((ct >> 7) & 1) : 4 * (ct >> 7);  // first k of this thread inside a chunk
   uint32_t g = 0;  // chunks produced so far by this CTA
-  for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+  for (int t = cta_begin[blockIdx.x], t_end = cta_begin[blockIdx.x + 1]; t < t_end; ++t) {
     const TcTile tl = tiles[t];
     const bool row_valid = is_a ? row < tl.h : row < tl.w;
     for (int si = tl.seg_begin; si < tl.seg_end; ++si) {
       const GemmSeg sg = segs[si];
-      const cplx* base = is_a ? A + sg.a_off + (int64_t)tl.m0 * sg.a_sm : B + sg.b_off + (int64_t)tl.n0 * sg.b_sn;
-      const int64_t rs = is_a ? sg.a_sm : sg.b_sn, ks = is_a ? sg.a_sk : sg.b_sk;
-      const double scale = is_a ? sg.alpha : 1.0, isg = is_a ? conj_sign : 1.0;
+      const cplx* base = is_a ? A + sg.a_off + (int64_t)(tl.m0 + row) * sg.a_sm : B + sg.b_off + (int64_t)(tl.n0 + row) * sg.b_sn;
+      const int64_t ks = is_a ? sg.a_sk : sg.b_sk;
+      const bool scaled = MODE == 0 ? is_a : true;
+      const double scale = scaled ? sg.alpha : 1.0, im_scale = scaled ? sg.alpha * (is_a ? conj_sign : 1.0) : 1.0;
       for (int k0 = 0; k0 < sg.K; k0 += TC_KC, ++g) {
         const int s = g % TC_STAGES;
         mbar_wait(sm.empty + 8 * s, ((g / TC_STAGES) & 1) ^ 1);
-        if (is_a) convert_rows<true>(base, rs, ks, row_valid, k0, sg.K, scale, scale * isg, sm.a_panel(s), row);
-        else convert_rows<false>(base, rs, ks, row_valid, k0, sg.K, 1.0, 1.0, sm.b_panel(s), row);
+        if (row_valid) {  // rows beyond the tile edge only feed accumulator rows / columns that are never stored
+          const uint32_t dst = (is_a ? sm.a_panel(s) : sm.b_panel(s)) + (uint32_t)(row * 16) + (uint32_t)(kpart >> 2) * TC_LBO;
+          const cplx* p = base + (int64_t)(k0 + kpart) * ks;
+          if (MODE == 0) {
+            if (is_a) convert_row<8, true, true>(p, ks, sg.K - k0 - kpart, scale, im_scale, dst, nullptr);
+            else convert_row<8, false, true>(p, ks, sg.K - k0 - kpart, 1.0, 1.0, dst, nullptr);
+          } else {
+            convert_row<4, true, true>(p, ks, sg.K - k0 - kpart, scale, im_scale, dst, nullptr);
+          }
+        }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy stores -> visible to the MMA (async proxy)
         mbar_arrive(sm.full + 8 * s);
       }
@@ -173,10 +197,37 @@ __device__ __forceinline__ void converter_loop(const TcTile* __restrict__ tiles,
   }
 }
 
+// MODE 1 / 2: one thread streams the static operand's panel images (32 KB per chunk, laid out exactly as the
+// shared-memory panel) with cp.async.bulk; the copy completes on the stage's full barrier (complete_tx).
+template <int MODE>
+__device__ __forceinline__ void bulk_loop(const TcTile* __restrict__ tiles, const int* __restrict__ cta_begin, const GemmSeg* __restrict__ segs,
+                                          const int64_t* __restrict__ seg_img, const unsigned char* __restrict__ images,
+                                          const TcSmem& sm) {
+  uint32_t g = 0;
+  for (int t = cta_begin[blockIdx.x], t_end = cta_begin[blockIdx.x + 1]; t < t_end; ++t) {
+    const TcTile tl = tiles[t];
+    const int rt = (MODE == 1 ? tl.m0 : tl.n0) >> 7;  // row tile of the static operand this output tile reads
+    for (int si = tl.seg_begin; si < tl.seg_end; ++si) {
+      const int K = segs[si].K;
+      const int nch = (K + TC_KC - 1) / TC_KC;
+      const unsigned char* src = images + seg_img[si] + (int64_t)rt * nch * TC_OPERAND;
+      for (int c = 0; c < nch; ++c, ++g, src += TC_OPERAND) {
+        const int s = g % TC_STAGES;
+        mbar_wait(sm.empty + 8 * s, ((g / TC_STAGES) & 1) ^ 1);
+        const uint32_t bar = sm.full + 8 * s, dst = MODE == 1 ? sm.a_panel(s) : sm.b_panel(s);
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(TC_OPERAND) : "memory");
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     ::"r"(dst), "l"(src), "r"(TC_OPERAND), "r"(bar)
+                     : "memory");
+      }
+    }
+  }
+}
+
 // ------------------------------------------------------------------------------------------------ MMA issuer
-__device__ __forceinline__ void mma_loop(const TcTile* __restrict__ tiles, int ntiles, const TcSmem& sm, uint32_t tmem) {
+__device__ __forceinline__ void mma_loop(const TcTile* __restrict__ tiles, const int* __restrict__ cta_begin, const TcSmem& sm, uint32_t tmem) {
   uint32_t g = 0, tt = 0;
-  for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+  for (int t = cta_begin[blockIdx.x], t_end = cta_begin[blockIdx.x + 1]; t < t_end; ++t) {
     const TcTile tl = tiles[t];
     if (tl.chunks == 0) continue;
     const int n_inst = max(16, (tl.w + 15) & ~15);
@@ -220,11 +271,11 @@ __device__ __forceinline__ void mma_loop(const TcTile* __restrict__ tiles, int n
 }
 
 // ------------------------------------------------------------------------------------------------ epilogue
-__device__ __forceinline__ void epilogue_loop(const TcTile* __restrict__ tiles, int ntiles, cplx* __restrict__ C,
+__device__ __forceinline__ void epilogue_loop(const TcTile* __restrict__ tiles, const int* __restrict__ cta_begin, cplx* __restrict__ C,
                                               const TcSmem& sm, uint32_t tmem, int warp, int lane) {
   const int row = 32 * warp + lane;
   uint32_t tt = 0;
-  for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+  for (int t = cta_begin[blockIdx.x], t_end = cta_begin[blockIdx.x + 1]; t < t_end; ++t) {
     const TcTile tl = tiles[t];
     cplx* crow = C + tl.c_off + (int64_t)(tl.m0 + row) * tl.ldc + tl.n0;
     if (tl.chunks == 0) {  // an output without contributions
@@ -253,9 +304,11 @@ __device__ __forceinline__ void epilogue_loop(const TcTile* __restrict__ tiles, 
   }
 }
 
+template <int MODE>
 __global__ void __launch_bounds__(TC_THREADS, 1)
-    grouped_zgemm_tc_kernel(const TcTile* __restrict__ tiles, int ntiles, const GemmSeg* __restrict__ segs,
-                            const cplx* __restrict__ A, const cplx* __restrict__ B, cplx* __restrict__ C, int conjA) {
+    grouped_zgemm_tc_kernel(const TcTile* __restrict__ tiles, const int* __restrict__ cta_begin, const GemmSeg* __restrict__ segs,
+                            const cplx* __restrict__ A, const cplx* __restrict__ B, cplx* __restrict__ C, int conjA,
+                            const int64_t* __restrict__ seg_img, const unsigned char* __restrict__ images) {
   extern __shared__ __align__(1024) unsigned char tc_smem[];
   TcSmem sm;
   sm.data = (uint32_t)__cvta_generic_to_shared(tc_smem);
@@ -267,7 +320,9 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
     for (int s = 0; s < TC_STAGES; ++s) {
-      mbar_init(sm.full + 8 * s, 32 * TC_CONV_WARPS);  // every converter thread arrives after its own stores
+      // every converter thread arrives after its own stores; with a static operand also the thread that starts
+      // the bulk copy (arrive.expect_tx; the bytes complete the phase)
+      mbar_init(sm.full + 8 * s, 32 * TC_CONV_WARPS + (MODE != 0 ? 1 : 0));
       mbar_init(sm.empty + 8 * s, 1);                  // tcgen05.commit
     }
     for (int b = 0; b < 2; ++b) {
@@ -287,12 +342,15 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem) : "r"(sm.tptr) : "memory");
 
   if (warp < TC_EPI_WARPS) {
-    epilogue_loop(tiles, ntiles, C, sm, tmem, warp, lane);
+    epilogue_loop(tiles, cta_begin, C, sm, tmem, warp, lane);
   } else if (warp == TC_MMA_WARP) {
-    if (lane == 0) mma_loop(tiles, ntiles, sm, tmem);
+    if (lane == 0) mma_loop(tiles, cta_begin, sm, tmem);
     __syncwarp();
+  } else if (warp <= TC_MMA_WARP + TC_CONV_WARPS) {
+    converter_loop<MODE>(tiles, cta_begin, segs, A, B, conjA ? -1.0 : 1.0, sm, (int)threadIdx.x - 32 * (TC_MMA_WARP + 1));
   } else {
-    converter_loop(tiles, ntiles, segs, A, B, conjA ? -1.0 : 1.0, sm, warp - TC_MMA_WARP - 1, lane);
+    if (MODE != 0 && lane == 0) bulk_loop<MODE>(tiles, cta_begin, segs, seg_img, images, sm);
+    __syncwarp();
   }
 
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -301,11 +359,24 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512) : "memory");
 }
 
+// Packs a static operand once per plan: one CTA per panel image chunk (128 rows x 16 k, 4 planes, 32 KB, zero padded),
+// one thread per row; no alpha (the converters of the other operand carry it), conjugation as the stage says.
+__global__ void __launch_bounds__(128) tc_pack_kernel(const TcPackChunk* __restrict__ chunks, const cplx* __restrict__ X,
+                                                      unsigned char* __restrict__ images, double im_sign) {
+  const TcPackChunk c = chunks[blockIdx.x];
+  const int row = threadIdx.x;
+  unsigned char* dst = images + c.dst_off + row * 16;
+  const cplx* p = X + c.src_off + (int64_t)row * c.rs;
+  convert_row<16, true, false>(p, c.ks, row < c.rows ? c.kleft : 0, 1.0, im_sign, 0u, dst);
+}
+
 }  // namespace
 
-// 128 x 128 tiles of the merged outputs, heaviest first
-void build_tc_tiles(const Stage& st, std::vector<TcTile>& tiles) {
-  tiles.clear();
+// 128 x 128 tiles of the merged outputs, dealt to `grid` persistent CTAs heaviest first to the least loaded CTA
+// (weight = chunks x a mix of the converter cost, which does not depend on the width, and the MMA cost, which
+// does); the tiles of CTA b are tiles[cta_begin[b] .. cta_begin[b + 1]), heaviest first
+void build_tc_tiles(const Stage& st, int grid, std::vector<TcTile>& tiles, std::vector<int>& cta_begin) {
+  std::vector<TcTile> all;
   for (const GemmOut& o : st.mouts) {
     int chunks = 0;
     for (int s = o.seg_begin; s < o.seg_end; ++s) chunks += (st.segs[s].K + TC_KC - 1) / TC_KC;
@@ -322,23 +393,95 @@ void build_tc_tiles(const Stage& st, std::vector<TcTile>& tiles) {
         t.seg_end = o.seg_end;
         t.chunks = chunks;
         t.pad = 0;
-        tiles.push_back(t);
+        all.push_back(t);
       }
   }
-  std::stable_sort(tiles.begin(), tiles.end(), [](const TcTile& a, const TcTile& b) {
-    return (int64_t)a.chunks * ((a.w + 15) / 16) > (int64_t)b.chunks * ((b.w + 15) / 16);
-  });
+  auto weight = [](const TcTile& t) { return (int64_t)t.chunks * (128 + ((t.w + 15) & ~15)) + 64; };
+  std::stable_sort(all.begin(), all.end(), [&](const TcTile& a, const TcTile& b) { return weight(a) > weight(b); });
+  grid = std::max(1, grid);
+  std::vector<std::vector<int>> mine(grid);
+  std::vector<std::pair<int64_t, int>> heap;  // (-load, cta): max-heap on -load = least loaded first
+  for (int b = 0; b < grid; ++b) heap.push_back({0, -b});
+  std::make_heap(heap.begin(), heap.end());
+  for (size_t i = 0; i < all.size(); ++i) {
+    std::pop_heap(heap.begin(), heap.end());
+    auto& top = heap.back();
+    mine[-top.second].push_back((int)i);
+    top.first -= weight(all[i]);
+    std::push_heap(heap.begin(), heap.end());
+  }
+  tiles.clear();
+  cta_begin.assign(grid + 1, 0);
+  for (int b = 0; b < grid; ++b) {
+    for (int i : mine[b]) tiles.push_back(all[i]);
+    cta_begin[b + 1] = (int)tiles.size();
+  }
 }
 
-void launch_grouped_gemm_tc(const TcTile* d_tiles, int ntiles, const GemmSeg* d_segs, int conjA, const cplx* A, const cplx* B,
-                            cplx* C, int grid, cudaStream_t s, int64_t* lc) {
+// Panel images of the static operand of a stage (a_side: op(A), else op(B)): one image per distinct operand region
+// (offset, strides, K, rows) -- segments that read the same environment block share it -- cut into row tiles of 128
+// and chunks of 16 k.  seg_img[s] = byte offset of the image of segment s; chunks = what tc_pack_kernel converts.
+int64_t build_tc_static(const Stage& st, bool a_side, std::vector<int64_t>& seg_img, std::vector<TcPackChunk>& chunks) {
+  struct Key {
+    int64_t off;
+    int rs, ks, K, rows;
+    bool operator<(const Key& o) const { return std::tie(off, rs, ks, K, rows) < std::tie(o.off, o.rs, o.ks, o.K, o.rows); }
+  };
+  std::map<Key, int64_t> seen;
+  seg_img.assign(st.segs.size(), 0);
+  chunks.clear();
+  int64_t bytes = 0;
+  for (const GemmOut& o : st.mouts)
+    for (int s = o.seg_begin; s < o.seg_end; ++s) {
+      const GemmSeg& g = st.segs[s];
+      const Key k{a_side ? g.a_off : g.b_off, a_side ? g.a_sm : g.b_sn, a_side ? g.a_sk : g.b_sk, g.K, a_side ? o.M : o.N};
+      auto it = seen.find(k);
+      if (it == seen.end()) {
+        it = seen.emplace(k, bytes).first;
+        const int nrt = (k.rows + 127) / 128, nch = (k.K + TC_KC - 1) / TC_KC;
+        for (int rt = 0; rt < nrt; ++rt)
+          for (int c = 0; c < nch; ++c) {
+            TcPackChunk pc;
+            pc.src_off = k.off + (int64_t)rt * 128 * k.rs + (int64_t)c * TC_KC * k.ks;
+            pc.dst_off = bytes;
+            pc.rs = k.rs;
+            pc.ks = k.ks;
+            pc.rows = std::min(128, k.rows - rt * 128);
+            pc.kleft = std::min(TC_KC, k.K - c * TC_KC);
+            chunks.push_back(pc);
+            bytes += TC_OPERAND;
+          }
+      }
+      seg_img[s] = it->second;
+    }
+  return bytes;
+}
+
+void launch_tc_pack(const TcPackChunk* d_chunks, int nchunks, const cplx* X, unsigned char* images, int conj, cudaStream_t s,
+                    int64_t* lc) {
+  if (nchunks == 0) return;
+  tc_pack_kernel<<<nchunks, 128, 0, s>>>(d_chunks, X, images, conj ? -1.0 : 1.0);
+  ++*lc;
+}
+
+// mode 0: both operands converted in the loop; 1: op(A) from panel images; 2: op(B) from panel images
+void launch_grouped_gemm_tc(const TcTile* d_tiles, const int* d_cta_begin, int grid, int ntiles, const GemmSeg* d_segs, int conjA,
+                            const cplx* A, const cplx* B, cplx* C, cudaStream_t s, int64_t* lc, int mode, const int64_t* d_seg_img,
+                            const unsigned char* images) {
   if (ntiles == 0) return;
   static bool attr_set = false;
   if (!attr_set) {
-    cudaFuncSetAttribute(grouped_zgemm_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES);
+    cudaFuncSetAttribute(grouped_zgemm_tc_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES);
+    cudaFuncSetAttribute(grouped_zgemm_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES);
+    cudaFuncSetAttribute(grouped_zgemm_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES);
     attr_set = true;
   }
-  grouped_zgemm_tc_kernel<<<std::min(grid, ntiles), TC_THREADS, TC_SMEM_BYTES, s>>>(d_tiles, ntiles, d_segs, A, B, C, conjA);
+  if (mode == 1)
+    grouped_zgemm_tc_kernel<1><<<grid, TC_THREADS, TC_SMEM_BYTES, s>>>(d_tiles, d_cta_begin, d_segs, A, B, C, conjA, d_seg_img, images);
+  else if (mode == 2)
+    grouped_zgemm_tc_kernel<2><<<grid, TC_THREADS, TC_SMEM_BYTES, s>>>(d_tiles, d_cta_begin, d_segs, A, B, C, conjA, d_seg_img, images);
+  else
+    grouped_zgemm_tc_kernel<0><<<grid, TC_THREADS, TC_SMEM_BYTES, s>>>(d_tiles, d_cta_begin, d_segs, A, B, C, conjA, nullptr, nullptr);
   ++*lc;
 }
 
