@@ -43,6 +43,9 @@ def parse_args():
     ap.add_argument("--precision", default="fp64", choices=["fp64", "split"],
                     help="split: run the main line's applies with FH_OPT_PRECISION = 1 (3 x TF32 on tcgen05; NEXT-3). "
                          "Not the headline metric: dtype and config say so; used for the ncu capture of that kernel")
+    ap.add_argument("--extra-chi", type=int, nargs="*", default=None,
+                    help="replace the default other_configs list by Gaussian-profile applies at these chi (e.g. 32768 49152: "
+                         "BASELINE config 5 sizes, minutes of host time to generate the environments)")
     ap.add_argument("--no-extra", action="store_true",
                     help="skip the apply-only lines of the other configs (chi = 1024, Table S2 x 1/6, 16384, 24576) and "
                          "the oracle timings on configs 1, 2, 5'")
@@ -283,8 +286,8 @@ def time_apply_random_envs(H, fi, torch, chi, profile, s2, steps, peak_dmma, loc
         dims = fi.chain_dims(chi, L, profile, s2)
         dl, dr = dims[c], dims[c + 2]
         env_keys = fi.env_block_keys
-    zest = 40.0 * sum(dl.values()) ** 2 * 16 / 1274.0 ** 2 * 1.2      # Z scales like chi_su2^2 (40 MB at 1274)
-    ctx = H.binding.Context(int(max(2 << 30, 6 * zest + (1 << 30))), device="cuda:%d" % local)
+    zest = 40e6 * (sum(dl.values()) / 1274.0) ** 2 * 1.5              # bytes of Z: scales like chi_su2^2 (40 MB at 1274)
+    ctx = H.binding.Context(int(min(150e9, max(2 << 30, 4 * zest + (1 << 30)))), device="cuda:%d" % local)
     try:
         if abelian:
             ctx.fh_set_option(ctx.OPT_SYMMETRY, 1)
@@ -524,9 +527,11 @@ def run_ours(args):
     ctx.close()
     if not args.no_extra and world == 1:
         extra = []
-        for chi_x, prof_x, s2_x, st_x in ((1024, "gaussian", (1, 1), 20), (4096, "u1u1", (1, 1), 20),
-                                          (0, "table_s2", (1, 6), 10),
-                                          (16384, "gaussian", (1, 1), 5), (24576, "gaussian", (1, 1), 3)):
+        todo = ((1024, "gaussian", (1, 1), 20), (4096, "u1u1", (1, 1), 20), (0, "table_s2", (1, 6), 10),
+                (16384, "gaussian", (1, 1), 5), (24576, "gaussian", (1, 1), 3))
+        if args.extra_chi is not None:
+            todo = tuple((cx, "gaussian", (1, 1), 3) for cx in args.extra_chi)
+        for chi_x, prof_x, s2_x, st_x in todo:
             try:
                 extra.append(time_apply_random_envs(H, fi, torch, chi_x, prof_x, s2_x, st_x, peak_dmma, local))
             except Exception as e:            # report, do not lose the headline line
