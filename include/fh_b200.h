@@ -376,6 +376,15 @@ int fh_host_get_tasks(int stage, int* ntask, int* nout, int32_t* tuples, double*
  * [M, N, steps] (int32[nout][3]); dmma_padded = DMMA.8x8x4 instructions the list issues.  Either array
  * pointer may be NULL to query the counts only. */
 int fh_host_get_units(int stage, int* nunit, int32_t* units, int* nout, int32_t* outs, int64_t* dmma_padded);
+/* Tile list of the split-precision kernel (zgemm_tc.cu, NEXT-3) for the same host plan and `grid` persistent CTAs:
+ * per tile [out, m0, n0, h, w, chunks] (int32[ntile][6]; out indexes the merged outputs of fh_host_get_units, a tile
+ * is h x w <= 128 x 128 elements of it, chunks = sum over its segments of ceil(K / 16)), in the order the kernel walks
+ * them: CTA b takes tiles cta_begin[b] .. cta_begin[b + 1] - 1 (int32[grid + 1]).  static_side 1 (op(A)) or 2 (op(B)):
+ * also the panel images of that operand: seg_img[s] = byte offset of the image segment s reads and seg_operand[s] =
+ * element offset of the operand block it is made from (int64 per segment; nseg = number of segments of the stage: the
+ * tasks; -1 for a segment of an output that was merged into its neighbour and is not read), nimage_chunks 32-KB chunks in image_bytes bytes; 0: skipped.  Pointers may be NULL. */
+int fh_host_get_tc_tiles(int stage, int grid, int static_side, int* ntile, int32_t* tiles, int32_t* cta_begin, int* nseg,
+                         int* nimage_chunks, int64_t* seg_img, int64_t* seg_operand, int64_t* image_bytes);
 
 #ifdef __cplusplus
 }

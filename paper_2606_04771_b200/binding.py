@@ -100,6 +100,8 @@ _SIGS = {
                              c_int, c_void_p]),
     "fh_host_get_tasks": (c_int, [c_int, P(c_int), P(c_int), c_void_p, c_void_p, P(c_i64)]),
     "fh_host_get_units": (c_int, [c_int, P(c_int), c_void_p, P(c_int), c_void_p, P(c_i64)]),
+    "fh_host_get_tc_tiles": (c_int, [c_int, c_int, c_int, P(c_int), c_void_p, c_void_p, P(c_int), P(c_int), c_void_p, c_void_p,
+                                     P(c_i64)]),
 }
 EXPORTS = sorted(_SIGS)
 for _name, (_res, _args) in _SIGS.items():
@@ -174,6 +176,22 @@ def fh_host_plan(site, nsite, t_h, U, dims_l, dims_r, L_keys, R_keys):
         lib.fh_host_get_tasks(stage, C.byref(nt), C.byref(no), _np_ptr(tup), _np_ptr(al), C.byref(fl))
         out.append((tup, al, no.value, fl.value))
     return out
+
+
+def fh_host_get_tc_tiles(stage, grid, static_side):
+    """(tiles int32[n,6], cta_begin int32[grid+1], seg_img int64[nseg], seg_operand int64[nseg], image chunks, image bytes)."""
+    nt, ns, nc, nb = c_int(), c_int(), c_int(), c_i64()
+    rc = lib.fh_host_get_tc_tiles(stage, grid, 0, C.byref(nt), None, None, C.byref(ns), None, None, None, None)
+    if rc != 0:
+        raise FhError("fh_host_get_tc_tiles failed: %d" % rc)
+    tiles = np.zeros((nt.value, 6), dtype=np.int32)
+    cb = np.zeros(grid + 1, dtype=np.int32)
+    img, opd = np.zeros(ns.value, dtype=np.int64), np.zeros(ns.value, dtype=np.int64)
+    rc = lib.fh_host_get_tc_tiles(stage, grid, static_side, C.byref(nt), _np_ptr(tiles), _np_ptr(cb), C.byref(ns), C.byref(nc),
+                                  _np_ptr(img), _np_ptr(opd), C.byref(nb))
+    if rc != 0:
+        raise FhError("fh_host_get_tc_tiles failed: %d" % rc)
+    return tiles, cb, img, opd, nc.value, nb.value
 
 
 def fh_host_get_units(stage):

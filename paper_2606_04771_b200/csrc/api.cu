@@ -1868,6 +1868,47 @@ int fh_host_get_units(int stage, int* nunit, int32_t* units, int* nout, int32_t*
   return FH_OK;
 }
 
+int fh_host_get_tc_tiles(int stage, int grid, int static_side, int* ntile, int32_t* tiles, int32_t* cta_begin, int* nseg,
+                         int* nimage_chunks, int64_t* seg_img, int64_t* seg_operand, int64_t* image_bytes) {
+  if ((stage != 1 && stage != 2) || grid < 1) return FH_EINVAL;
+  try {
+    const Stage& st = stage == 1 ? g_host_st1 : g_host_st2;
+    std::vector<TcTile> t;
+    std::vector<int> cb;
+    build_tc_tiles(st, grid, t, cb);
+    if (ntile) *ntile = (int)t.size();
+    if (nseg) *nseg = (int)st.segs.size();
+    if (tiles) {
+      std::map<int64_t, int> by_off;
+      for (size_t o = 0; o < st.mouts.size(); ++o) by_off[st.mouts[o].c_off] = (int)o;
+      for (size_t i = 0; i < t.size(); ++i) {
+        tiles[6 * i] = by_off.count(t[i].c_off) ? by_off[t[i].c_off] : -1;
+        tiles[6 * i + 1] = t[i].m0;
+        tiles[6 * i + 2] = t[i].n0;
+        tiles[6 * i + 3] = t[i].h;
+        tiles[6 * i + 4] = t[i].w;
+        tiles[6 * i + 5] = t[i].chunks;
+      }
+    }
+    if (cta_begin)
+      for (int b = 0; b <= grid; ++b) cta_begin[b] = cb[b];
+    if (static_side == 1 || static_side == 2) {
+      std::vector<int64_t> img;
+      std::vector<TcPackChunk> pc;
+      const int64_t bytes = build_tc_static(st, static_side == 1, img, pc);
+      if (nimage_chunks) *nimage_chunks = (int)pc.size();
+      if (image_bytes) *image_bytes = bytes;
+      if (seg_img)
+        for (size_t i = 0; i < img.size(); ++i) seg_img[i] = img[i];
+      if (seg_operand)
+        for (size_t i = 0; i < st.segs.size(); ++i) seg_operand[i] = static_side == 1 ? st.segs[i].a_off : st.segs[i].b_off;
+    }
+    return FH_OK;
+  } catch (...) {
+    return FH_EINVAL;
+  }
+}
+
 double fh_canonical_weight(int tjc, int tjb) { return std::sqrt((double)(tjb + 1) / (double)(tjc + 1)); }
 
 double fh_coef_left(int ta, int ts, int tc, int tk, int tr, int tkp, int tap, int tsp, int tcp) {

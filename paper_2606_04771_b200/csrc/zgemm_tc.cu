@@ -428,7 +428,7 @@ int64_t build_tc_static(const Stage& st, bool a_side, std::vector<int64_t>& seg_
     bool operator<(const Key& o) const { return std::tie(off, rs, ks, K, rows) < std::tie(o.off, o.rs, o.ks, o.K, o.rows); }
   };
   std::map<Key, int64_t> seen;
-  seg_img.assign(st.segs.size(), 0);
+  seg_img.assign(st.segs.size(), -1);  // segments of outputs that were merged into a neighbour are not read by any tile
   chunks.clear();
   int64_t bytes = 0;
   for (const GemmOut& o : st.mouts)

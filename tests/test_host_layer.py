@@ -125,6 +125,53 @@ def test_unit_lists_tile_every_output_exactly_once(binding, chi, profile):
         assert sum(int(cv.size) * 64 for cv in cover) < 4 * exact + 64 * len(outs) * 4
 
 
+@pytest.mark.parametrize("chi,grid", [(1024, 148), (4096, 148), (4096, 7)])
+def test_split_precision_tile_lists_and_panel_images(binding, chi, grid):
+    """Host side of the split-precision kernel (zgemm_tc.cu, NEXT-3): the 128 x 128 tiles cover every element of
+    every merged output exactly once and carry sum ceil(K / 16) chunks; the CTA ranges partition the list, each
+    CTA's tiles are in non-increasing weight order and the dealing is balanced to within one tile's weight of the
+    mean; the panel images of the static operand (stage 1: op(A), stage 2: op(B)) lie inside the image buffer, are
+    32-KB aligned, no image serves two operand blocks and segments that read the same block share one."""
+    L, c = 60, 29
+    dims = fi.chain_dims(chi, L, "gaussian", (1, 1))
+    dl, dr = dims[c], dims[c + 2]
+    Lk, Rk = sorted(fi.env_block_keys(dl, dl)), sorted(fi.env_block_keys(dr, dr))
+    binding.fh_host_plan(c, 2, 1.0, 4.0, dl, dr, Lk, Rk)
+    for stage in (1, 2):
+        _, outs, _ = binding.fh_host_get_units(stage)
+        tiles, cb, img, opd, nchunk, nbytes = binding.fh_host_get_tc_tiles(stage, grid, stage)
+        assert len(tiles) > 0 and (tiles[:, 0] >= 0).all()
+        cover = [np.zeros((m, n), dtype=np.int8) for m, n, _ in outs]
+        for o, m0, n0, h, w, ch in tiles:
+            M, N, _ = outs[o]
+            assert m0 % 128 == 0 and n0 % 128 == 0 and 1 <= h <= 128 and 1 <= w <= 128
+            assert h == min(128, M - m0) and w == min(128, N - n0)
+            cover[o][m0:m0 + h, n0:n0 + w] += 1
+        assert all((cv == 1).all() for cv in cover)
+        per_out = {}
+        for o, *_rest, ch in tiles:
+            per_out.setdefault(o, set()).add(int(ch))
+        assert all(len(v) == 1 for v in per_out.values())              # every tile of an output has that output's chunks
+        assert cb[0] == 0 and cb[-1] == len(tiles) and (np.diff(cb) >= 0).all() and len(cb) == grid + 1
+        wt = tiles[:, 5].astype(np.int64) * (128 + (tiles[:, 4] + 15) // 16 * 16) + 64
+        loads = np.array([wt[cb[b]:cb[b + 1]].sum() for b in range(grid)])
+        for b in range(grid):
+            seg = wt[cb[b]:cb[b + 1]]
+            assert (np.diff(seg) <= 0).all()
+        assert loads.max() - loads.min() <= wt.max()                   # greedy dealing: spread below one tile
+        used = img >= 0                                                  # -1: segment of an output merged into its neighbour
+        img, opd = img[used], opd[used]
+        assert nbytes == nchunk * 32768 and (img % 32768 == 0).all() and (img < nbytes).all() and used.sum() > 0
+        # an image serves one operand block only (segments that read the same block with the same extent share it;
+        # a block read as part of a wider merged operand has its own image), and images are shared at all
+        by_img = {}
+        assert len(img) == len(opd) > 0
+        for k, off in zip(opd.tolist(), img.tolist()):
+            by_img.setdefault(off, set()).add(k)
+        assert all(len(v) == 1 for v in by_img.values())
+        assert len(by_img) < len(img)
+
+
 def test_zero_site_task_lists_match_oracle(binding):
     """NEXT-1: the zero-site apply K C = sum_w L C R^T.  Integer task tuples of both stages equal the
     oracle's (oracle/symm.heff0_tasks) bit for bit, all coefficients are exactly 1, flops agree."""
