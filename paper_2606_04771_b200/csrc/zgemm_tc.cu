@@ -123,15 +123,16 @@ struct TcSmem {
 // op(A)(m, k) = A[a_off + m a_sm + k a_sk], op(B)(k, n) = B[b_off + k b_sk + n b_sn]: both panels are "row x k".
 // `dst` = address of (row, first k of this thread) in plane 0; generic address space: shared memory in the GEMM
 // kernel, global memory in the kernel that packs a static operand once per plan (same image either way).
-template <int NK, bool SCALE, bool TO_SHARED>
-__device__ __forceinline__ void convert_row(const cplx* __restrict__ p, int64_t k_stride, int k_left, double scale, double im_scale,
-                                            uint32_t dst_s, unsigned char* dst_g) {
-  cplx z[NK];
+template <int NK>
+__device__ __forceinline__ void load_row(const cplx* __restrict__ p, int64_t k_stride, int k_left, cplx (&z)[NK]) {
 #pragma unroll
   for (int i = 0; i < NK; ++i) {
     z[i] = make_double2(0.0, 0.0);
     if (i < k_left) z[i] = __ldg(p + (int64_t)i * k_stride);
   }
+}
+template <int NK, bool SCALE, bool TO_SHARED>
+__device__ __forceinline__ void convert_store(const cplx (&z)[NK], double scale, double im_scale, uint32_t dst_s, unsigned char* dst_g) {
 #pragma unroll
   for (int q = 0; q < NK / 4; ++q) {
     uint32_t rh[4], rl[4], ih[4], il[4];
@@ -156,10 +157,18 @@ __device__ __forceinline__ void convert_row(const cplx* __restrict__ p, int64_t 
   }
 }
 
-// MODE 0: both operands converted in the loop (4 + 4 warps, 16 k per thread), alpha folded into A.
+// MODE 0: both operands converted in the loop (8 + 8 warps, 8 k per thread), alpha folded into A.
 // MODE 1: A is STATIC (an environment: converted once per plan into panel images, streamed by cp.async.bulk), all
-//         8 converter warps work on B (8 k per thread) and fold alpha into it.
-// MODE 2: B is static, all 8 converter warps work on A and fold alpha (and the conjugation sign) into it.
+//         16 converter warps work on B (4 k per thread) and fold alpha into it.
+// MODE 2: B is static, all 16 converter warps work on A and fold alpha (and the conjugation sign) into it.
+template <int NK, bool SCALE, bool TO_SHARED>
+__device__ __forceinline__ void convert_row(const cplx* __restrict__ p, int64_t k_stride, int k_left, double scale, double im_scale,
+                                            uint32_t dst_s, unsigned char* dst_g) {
+  cplx z[NK];
+  load_row<NK>(p, k_stride, k_left, z);
+  convert_store<NK, SCALE, TO_SHARED>(z, scale, im_scale, dst_s, dst_g);
+}
+
 template <int MODE>
 __device__ __forceinline__ void converter_loop(const TcTile* __restrict__ tiles, const int* __restrict__ cta_begin, const GemmSeg* __restrict__ segs,
                                                const cplx* __restrict__ A, const cplx* __restrict__ B, double conj_sign,
@@ -177,17 +186,25 @@ __device__ __forceinline__ void converter_loop(const TcTile* __restrict__ tiles,
       const int64_t ks = is_a ? sg.a_sk : sg.b_sk;
       const bool scaled = MODE == 0 ? is_a : true;
       const double scale = scaled ? sg.alpha : 1.0, im_scale = scaled ? sg.alpha * (is_a ? conj_sign : 1.0) : 1.0;
+      // MODE 1 / 2: the loads of the next chunk of the segment are issued before this chunk is converted (and before the
+      // wait for its stage), so a thread's load latency overlaps its own conversion work
+      cplx zc[4], zn[4];
+      if (MODE != 0 && row_valid) load_row<4>(base + (int64_t)kpart * ks, ks, sg.K - kpart, zc);
       for (int k0 = 0; k0 < sg.K; k0 += TC_KC, ++g) {
         const int s = g % TC_STAGES;
+        if (MODE != 0 && row_valid && k0 + TC_KC < sg.K)
+          load_row<4>(base + (int64_t)(k0 + TC_KC + kpart) * ks, ks, sg.K - k0 - TC_KC - kpart, zn);
         mbar_wait(sm.empty + 8 * s, ((g / TC_STAGES) & 1) ^ 1);
         if (row_valid) {  // rows beyond the tile edge only feed accumulator rows / columns that are never stored
           const uint32_t dst = (is_a ? sm.a_panel(s) : sm.b_panel(s)) + (uint32_t)(row * 16) + (uint32_t)(kpart >> 2) * TC_LBO;
-          const cplx* p = base + (int64_t)(k0 + kpart) * ks;
           if (MODE == 0) {
+            const cplx* p = base + (int64_t)(k0 + kpart) * ks;
             if (is_a) convert_row<8, true, true>(p, ks, sg.K - k0 - kpart, scale, im_scale, dst, nullptr);
             else convert_row<8, false, true>(p, ks, sg.K - k0 - kpart, 1.0, 1.0, dst, nullptr);
           } else {
-            convert_row<4, true, true>(p, ks, sg.K - k0 - kpart, scale, im_scale, dst, nullptr);
+            convert_store<4, true, true>(zc, scale, im_scale, dst, nullptr);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) zc[i] = zn[i];
           }
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy stores -> visible to the MMA (async proxy)
