@@ -1158,3 +1158,59 @@ def test_next3_split_tdvp_gate_L8(H, ctx):
     print("split-precision TDVP L=8, 20 steps: max |delta <S^z_i>|, |delta <n_up n_dn>| = %.1e, norm^2 - 1 = %.1e" % (worst, gg["norm2"] - 1))
     assert 1e-12 < worst < 1e-3 and abs(gg["norm2"] - 1) < 1e-3
     ctx.mps_destroy(mps)
+
+
+@pytest.mark.parametrize("mode", ["su2", "u1u1"])
+def test_next3_split_apply_small_chains_both_modes(H, mode):
+    """FH_OPT_PRECISION = 1 on ragged tiny blocks (1 ... 11 columns: every 128 x 128 tile is mostly padding, many
+    outputs have no contribution at the chain ends) in both symmetry modes: the two-site apply on every bond of a
+    random L = 6 chain against the FP64 oracle, relative Frobenius <= 1e-5 (K_total <= ~60 here: measured ~1e-6),
+    while the one-site apply of the same context stays FP64 (<= 1e-11)."""
+    rng = np.random.default_rng(77)
+    L = 6
+    ctx = H.binding.Context(1 << 28)
+    try:
+        if mode == "u1u1":
+            import fh_inputs.abelian as fab
+            from oracle import abelian as ab
+            ctx.fh_set_option(ctx.OPT_SYMMETRY, 1)
+            dims = [{k: min(v, int(rng.integers(1, 12))) for k, v in d.items()} for d in fab.chain_dims(10 ** 6, L)]
+            A = [{k: _rand(rng, dims[i][k[0]], dims[i + 1][k[2]]) for k in ab.site_keys(dims[i], dims[i + 1])} for i in range(L)]
+            W = [ab.mpo_elements(1.0, 4.0)] * L
+            mod, left0, right0 = ab, ab.boundary_left(), ab.boundary_right()
+            tkeys = ab.theta_keys
+        else:
+            dims, A = _small_chain(rng, L, 11)
+            W = [symm.mpo_reduced(i, 1.0, 4.0) for i in range(L)]
+            mod, left0, right0 = symm, symm.boundary_left(), symm.boundary_right()
+            tkeys = symm.theta_keys
+        Le, Re = [left0], [None] * (L + 1)
+        for i in range(L):
+            Le.append(mod.env_update_left(Le[i], A[i], W[i]))
+        Re[L] = right0
+        for i in range(L - 1, -1, -1):
+            Re[i] = mod.env_update_right(Re[i + 1], A[i], W[i])
+        mpo = ctx.fh_mpo_build(L, 1.0, 4.0)
+        mps = ctx.mps_create(L)
+        for i in range(L):
+            H.set_site(ctx, mps, i, A[i], dims[i], dims[i + 1])
+        for i in range(L):
+            ctx.env_update_left(mpo, mps, i)
+        for i in range(L - 1, -1, -1):
+            ctx.env_update_right(mpo, mps, i)
+        ctx.fh_set_option(ctx.OPT_PRECISION, 1)
+        worst = 0.0
+        for i in range(L - 1):
+            th = {k: _rand(rng, dims[i][k[0]], dims[i + 2][k[4]]) for k in tkeys(dims[i], dims[i + 2])}
+            ref = mod.heff2_apply(Le[i], Re[i + 2], th, W[i], W[i + 1])
+            ctx.heff_plan(mpo, mps, i, 2)
+            e = rel_err(_apply_gpu(H, ctx, th, 2), ref, weighted=(mode == "su2"))
+            assert 1e-12 < e < 1e-5, (i, e)
+            worst = max(worst, e)
+        for i in range(L):
+            ref = mod.heff1_apply(Le[i], Re[i + 1], A[i], W[i])
+            ctx.heff_plan(mpo, mps, i, 1)
+            assert rel_err(_apply_gpu(H, ctx, A[i], 1), ref, weighted=(mode == "su2")) < TOL_APPLY, i
+        print("split-precision apply, small chain, %s: worst rel. Frobenius %.1e" % (mode, worst))
+    finally:
+        ctx.close()
