@@ -115,9 +115,10 @@ int mps_get_bond(const fh_mps* mps, int bond, int* n, int32_t* q, int32_t* tj, i
 int mps_site_layout(const fh_mps* mps, int site, int* nblk, int64_t* nelem, int32_t* labels,
                     int32_t* dims);
 /* Upload / download a whole site tensor: `data` holds the blocks back to back in planned block
- * order.  data_is_device != 0: device pointer (copied D2D on the context stream). */
+ * order.  data_is_device != 0: device pointer (copied D2D on the context stream).  The getters take the capacity
+ * of `data` in complex128 elements and return FH_EINVAL, copying nothing, when it is below the layout's nelem. */
 int mps_set_site(fh_ctx* ctx, fh_mps* mps, int site, const void* data, int data_is_device);
-int mps_get_site(fh_ctx* ctx, const fh_mps* mps, int site, void* data, int data_is_device);
+int mps_get_site(fh_ctx* ctx, const fh_mps* mps, int site, void* data, int64_t capacity_elems, int data_is_device);
 /* Checkpoint / resume for long runs (the paper's take up to 16 h).  mps_save writes the bond tables
  * and the site tensors of a state whose orthogonality centre is on site 0 (the state every sweep returns) to a
  * binary file (host byte order; header "FHMPS01", L, the tdvp_sweep_auto flag, per bond n x (q, 2j, d), per site
@@ -141,7 +142,7 @@ int env_update_right(fh_ctx* ctx, const fh_mpo* mpo, fh_mps* mps, int site);
  * labels[nblk][5] = (qx',tjx',w,qx,tjx), dims[nblk][2]. */
 int env_layout(const fh_mps* mps, int which, int bond, int* nblk, int64_t* nelem, int32_t* labels,
                int32_t* dims);
-int env_get(fh_ctx* ctx, const fh_mps* mps, int which, int bond, void* data, int data_is_device);
+int env_get(fh_ctx* ctx, const fh_mps* mps, int which, int bond, void* data, int64_t capacity_elems, int data_is_device);
 int env_set(fh_ctx* ctx, fh_mps* mps, int which, int bond, int nblk, const int32_t* labels,
             const void* data, int data_is_device);
 

@@ -44,7 +44,7 @@ _SIGS = {
     "mps_get_bond": (c_int, [c_void_p, c_int, P(c_int), c_void_p, c_void_p, c_void_p]),
     "mps_site_layout": (c_int, [c_void_p, c_int, P(c_int), P(c_i64), c_void_p, c_void_p]),
     "mps_set_site": (c_int, [c_void_p, c_void_p, c_int, c_void_p, c_int]),
-    "mps_get_site": (c_int, [c_void_p, c_void_p, c_int, c_void_p, c_int]),
+    "mps_get_site": (c_int, [c_void_p, c_void_p, c_int, c_void_p, c_i64, c_int]),
     "mps_get_svals": (c_int, [c_void_p, c_int, P(c_int), c_void_p]),
     "fh_dmma_peak_tflops": (c_int, [c_void_p, c_int, P(c_dbl)]),
     "fh_vec_kernels_gbs": (c_int, [c_void_p, c_i64, c_int, c_int, P(c_dbl)]),
@@ -64,7 +64,7 @@ _SIGS = {
     "env_update_left": (c_int, [c_void_p, c_void_p, c_void_p, c_int]),
     "env_update_right": (c_int, [c_void_p, c_void_p, c_void_p, c_int]),
     "env_layout": (c_int, [c_void_p, c_int, c_int, P(c_int), P(c_i64), c_void_p, c_void_p]),
-    "env_get": (c_int, [c_void_p, c_void_p, c_int, c_int, c_void_p, c_int]),
+    "env_get": (c_int, [c_void_p, c_void_p, c_int, c_int, c_void_p, c_i64, c_int]),
     "env_set": (c_int, [c_void_p, c_void_p, c_int, c_int, c_int, c_void_p, c_void_p, c_int]),
     "heff_plan": (c_int, [c_void_p, c_void_p, c_void_p, c_int, c_int]),
     "heff_layout": (c_int, [c_void_p, P(c_int), P(c_i64), c_void_p, c_void_p]),
@@ -309,7 +309,7 @@ class Context:
     def mps_get_site(self, mps, site):
         _, _, ne = self.mps_site_layout(mps, site)
         out = np.zeros(ne, dtype=np.complex128)
-        self.check(lib.mps_get_site(self.h, mps, site, _np_ptr(out), 0), "mps_get_site")
+        self.check(lib.mps_get_site(self.h, mps, site, _np_ptr(out), out.size, 0), "mps_get_site")
         return out
 
     def mps_get_svals(self, mps, bond):
@@ -361,7 +361,7 @@ class Context:
     def env_get(self, mps, which, bond):
         lab, dims, ne = self.env_layout(mps, which, bond)
         out = np.zeros(ne, dtype=np.complex128)
-        self.check(lib.env_get(self.h, mps, which, bond, _np_ptr(out), 0), "env_get")
+        self.check(lib.env_get(self.h, mps, which, bond, _np_ptr(out), out.size, 0), "env_get")
         return lab, dims, out
 
     def env_set(self, mps, which, bond, labels, data):

@@ -1147,11 +1147,12 @@ int mps_set_site(fh_ctx* ctx, fh_mps* mps, int site, const void* data, int is_de
   })
 }
 
-int mps_get_site(fh_ctx* ctx, const fh_mps* mps, int site, void* data, int is_dev) {
+int mps_get_site(fh_ctx* ctx, const fh_mps* mps, int site, void* data, int64_t capacity, int is_dev) {
   FH_TRY(ctx, {
     FH_REQUIRE(mps && site >= 0 && site < mps->L && data, FH_EINVAL, "mps_get_site: bad argument");
     const BlockTensor& t = mps->A[site];
     FH_REQUIRE(t.base >= 0, FH_ESTATE, "mps_get_site: site tensor not set");
+    FH_REQUIRE(capacity >= t.nelem, FH_EINVAL, "mps_get_site: buffer smaller than the site tensor (mps_site_layout gives nelem)");
     FH_CUDA(cudaMemcpyAsync(data, ctx->ptr(t.base), t.nelem * sizeof(cplx),
                             is_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, ctx->stream));
     FH_CUDA(cudaStreamSynchronize(ctx->stream));
@@ -1195,11 +1196,12 @@ int env_layout(const fh_mps* mps, int which, int bond, int* nblk, int64_t* nelem
   return FH_OK;
 }
 
-int env_get(fh_ctx* ctx, const fh_mps* mps, int which, int bond, void* data, int is_dev) {
+int env_get(fh_ctx* ctx, const fh_mps* mps, int which, int bond, void* data, int64_t capacity, int is_dev) {
   FH_TRY(ctx, {
     FH_REQUIRE(mps && bond >= 0 && bond <= mps->L && data && (which == 0 || which == 1), FH_EINVAL, "env_get: bad argument");
     const BlockTensor& t = which == 0 ? mps->Lenv[bond] : mps->Renv[bond];
     FH_REQUIRE(t.base >= 0, FH_ESTATE, "env_get: environment not built");
+    FH_REQUIRE(capacity >= t.nelem, FH_EINVAL, "env_get: buffer smaller than the environment (env_layout gives nelem)");
     FH_CUDA(cudaMemcpyAsync(data, ctx->ptr(t.base), t.nelem * sizeof(cplx),
                             is_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, ctx->stream));
     FH_CUDA(cudaStreamSynchronize(ctx->stream));

@@ -1040,6 +1040,13 @@ def test_edge_cases_and_error_codes(H, ctx):
     want = symm.heff2_apply(ref.Lenv[0], ref.Renv[2], th, ref.W[0], ref.W[1])
     got = _apply_gpu(H, ctx, th, 2)
     assert rel_err(got, want) < TOL_APPLY
+    # getters refuse a buffer smaller than the tensor instead of writing past it (capacity argument of the C ABI)
+    buf = np.zeros(64, dtype=np.complex128)
+    rc = B.lib.mps_get_site(ctx.h, mps, 0, buf.ctypes.data, 0, 0)
+    assert rc == -1 and b"smaller" in B.lib.fh_last_error(ctx.h) and not buf.any()
+    rc = B.lib.env_get(ctx.h, mps, 1, 1, buf.ctypes.data, 0, 0)
+    assert rc == -1 and b"smaller" in B.lib.fh_last_error(ctx.h)
+    assert B.lib.mps_get_site(ctx.h, mps, 0, buf.ctypes.data, 64, 0) == 0 and buf.any()
     with pytest.raises(B.FhError):
         ctx.heff_plan(mpo, mps, 1, 2)                 # bond out of range
     with pytest.raises(B.FhError):
