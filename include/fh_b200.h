@@ -57,8 +57,10 @@ const char* fh_last_error(const fh_ctx* ctx);
  *   FH_OPT_GEMM_PATH     which form of the grouped ZGEMM heff_apply uses for two-site plans: 0 = the library
  *                        chooses by the size of the plan (default), 1 = one warp-unit per one-warp CTA, two
  *                        launches (csrc/zgemm.cu), 2 = warp-specialised persistent kernel, both stages in one
- *                        launch (csrc/zgemm_ws.cu).  Same results to rounding (the k-split tiles of form 2 add
- *                        partial sums in another, fixed, order).
+ *                        launch (csrc/zgemm_ws.cu), 3 = the warp units of form 1 with both stages in ONE launch
+ *                        (stage-2 units wait on per-output counters; set it before heff_plan; bit-identical to
+ *                        form 1).  Same results to rounding (the k-split tiles of form 2 add partial sums in
+ *                        another, fixed, order).
  *   FH_OPT_SVD_MID_MAXN  widest sector matrix (columns) the library's own global-memory Jacobi kernel takes
  *                        instead of the vendor SVD, 0 .. 256 (default 128; 0 = none).
  *   FH_OPT_SVD_THREADS   host threads that drive the vendor SVD / QR routines, 1 .. 12 (default: cores - 1,

@@ -71,6 +71,9 @@ struct Plan {
   unsigned* d_ws_dep = nullptr;     // one counter per stage-1 output panel (cross-stage dependencies)
   unsigned ws_epoch = 0;
   WsPair pair;                      // joint tile queue of the two stages: one launch per apply
+  UnitPair upair;                   // the same for the warp-unit form (two-site plans)
+  unsigned* d_unit_dep = nullptr;   // one counter per stage-1 merged output
+  unsigned unit_epoch = 0;
   // interchange format <-> planned layout (heff_import / heff_export), built on first use per plan
   bool io_ready = false;
   int n_io = 0;
@@ -205,7 +208,7 @@ struct fh_ctx {
   std::vector<char> small_desc_host;
   int device = 0;
   const fh::SymMode* sym = &fh::SYM_SU2;  // fh_set_option(FH_OPT_SYMMETRY): the label algebra of every object of the context
-  int opt_gemm_path = 0;      // fh_set_option: 0 auto, 1 warp units, 2 warp-specialised
+  int opt_gemm_path = 0;      // fh_set_option: 0 auto, 1 warp units (two launches), 2 warp-specialised, 3 warp units (one launch)
   int opt_svd_mid_maxn = 128;
   int opt_svd_small_maxn = 4096;
   int opt_svd_threads = 0;    // 0 = default

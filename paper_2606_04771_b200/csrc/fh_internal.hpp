@@ -267,6 +267,29 @@ void launch_grouped_gemm_ws_pair(const WsPair& pr, const cplx* A1, const cplx* B
                                  cplx* C2, unsigned* d_counters, int grid, cplx* scratch, unsigned* flags,
                                  unsigned* dep_counters, unsigned epoch, cudaStream_t s, int64_t* launch_counter);
 int ws_smem_bytes();
+// warp-unit form with both stages in ONE launch (zgemm.cu): units of stage 1 then of stage 2, per unit its stage,
+// the stage-1 output it signals (stage 1) or its dependency list (stage 2)
+struct UnitLink {
+  int stage, sig, dep_begin, dep_count;
+};
+struct UnitPair {
+  std::vector<GemmUnit> units;
+  std::vector<GemmSeg> segs;
+  std::vector<UnitLink> link;
+  std::vector<int> dep_id;
+  std::vector<unsigned> dep_target;
+  int n1 = 0, n_dep_counters = 0, conj1 = 0, conj2 = 0;
+  GemmUnit* d_units = nullptr;
+  GemmSeg* d_segs = nullptr;
+  UnitLink* d_link = nullptr;
+  int* d_dep_id = nullptr;
+  unsigned* d_dep_target = nullptr;
+};
+void link_units(const Stage& st1, const Stage& st2, int mid_is_rhs2, UnitPair& out);
+// dep_counters: n_dep_counters unsigned, zero before the first launch; launch number `epoch` (1, 2, ...) raises
+// counter i to epoch * target_i
+void launch_grouped_gemm_pair(const UnitPair& pr, const cplx* A1, const cplx* B1, cplx* C1, const cplx* A2, const cplx* B2,
+                              cplx* C2, unsigned* dep_counters, unsigned epoch, cudaStream_t s, int64_t* launch_counter);
 // split-precision form on tcgen05 (zgemm_tc.cu, NEXT-3): a tile = up to 128 x 128 of a merged output over all its
 // segments (chunks = sum of ceil(K / 16)); same segment array, operands and results as the FP64 forms
 struct TcTile {

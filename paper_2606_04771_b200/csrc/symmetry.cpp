@@ -311,7 +311,7 @@ static void emit_units(Stage& st) {
       for (int j = 0; j < nu; ++j) {
         const int w = N8 / nu + (j < N8 % nu ? 1 : 0);
         UW x;
-        x.u = GemmUnit{o.c_off, o.ldc, o.M, o.N, o.seg_begin, o.seg_end, o.steps, m8 * 8, n8 * 8, h * 16 + w, 0,
+        x.u = GemmUnit{o.c_off, o.ldc, o.M, o.N, o.seg_begin, o.seg_end, o.steps, m8 * 8, n8 * 8, h * 16 + w, (int)oi,
                          o.seg_end > o.seg_begin ? st.segs[o.seg_begin] : GemmSeg{0, 0, 0, 0, 0, 0, 0, 0, 0.0}};
         x.work = (int64_t)h * w * std::max(1, o.steps);
         st.dmma_padded += 4 * (int64_t)h * w * o.steps;
@@ -582,6 +582,60 @@ void link_stages(const Stage& st1, const Stage& st2, int mid_is_rhs2, WsPair& pr
     t.dep_begin = dbeg[m];
     t.dep_count = dcnt[m];
     pr.tiles.push_back(t);
+  }
+}
+
+// The same for the warp-unit form: ONE launch whose grid is the stage-1 units followed by the stage-2 units (each
+// list heaviest first).  A stage-1 unit raises the counter of the merged output it tiles when its stores are
+// done; a stage-2 unit waits until every stage-1 output its segments read has collected one arrival per unit
+// that tiles it.  One-warp CTAs are dispatched in index order, so every stage-1 unit has started before a
+// stage-2 unit can occupy a warp slot: waiting cannot deadlock.
+void link_units(const Stage& st1, const Stage& st2, int mid_is_rhs2, UnitPair& pr) {
+  const int nseg1 = (int)st1.segs.size();
+  pr.segs = st1.segs;
+  pr.segs.insert(pr.segs.end(), st2.segs.begin(), st2.segs.end());
+  pr.n1 = (int)st1.units.size();
+  pr.n_dep_counters = (int)st1.mouts.size();
+  pr.conj1 = st1.opA != OPA_N;
+  pr.conj2 = st2.opA != OPA_N;
+  pr.units.clear();
+  pr.link.clear();
+  pr.dep_id.clear();
+  pr.dep_target.clear();
+  pr.units.reserve(st1.units.size() + st2.units.size());
+  std::vector<unsigned> tiled(st1.mouts.size(), 0);  // units per stage-1 merged output (GemmUnit::pad = its index)
+  for (const GemmUnit& u : st1.units) ++tiled[u.pad];
+  for (const GemmUnit& u : st1.units) {
+    pr.units.push_back(u);
+    pr.link.push_back(UnitLink{0, u.pad, 0, 0});
+  }
+  std::vector<std::vector<int>> deps(st2.mouts.size());
+  for (size_t o = 0; o < st2.outs.size(); ++o) {
+    const int m = st2.out_mout[o];
+    if (m < 0) continue;
+    for (int t = st2.outs[o].seg_begin; t < st2.outs[o].seg_end; ++t) {
+      const int z = mid_is_rhs2 ? st2.t_rhs[t] : st2.t_lhs[t];
+      const int zm = st1.out_mout[z];
+      if (zm >= 0) deps[m].push_back(zm);
+    }
+  }
+  std::vector<int> dbeg(deps.size(), 0), dcnt(deps.size(), 0);
+  for (size_t m = 0; m < deps.size(); ++m) {
+    std::sort(deps[m].begin(), deps[m].end());
+    deps[m].erase(std::unique(deps[m].begin(), deps[m].end()), deps[m].end());
+    dbeg[m] = (int)pr.dep_id.size();
+    dcnt[m] = (int)deps[m].size();
+    for (int zm : deps[m]) {
+      pr.dep_id.push_back(zm);
+      pr.dep_target.push_back(tiled[zm]);
+    }
+  }
+  for (const GemmUnit& u0 : st2.units) {
+    GemmUnit u = u0;
+    u.seg_begin += nseg1;
+    u.seg_end += nseg1;
+    pr.units.push_back(u);
+    pr.link.push_back(UnitLink{1, -1, dbeg[u0.pad], dcnt[u0.pad]});
   }
 }
 

@@ -256,8 +256,70 @@ __global__ void __launch_bounds__(32) grouped_zgemm_kernel(const GemmUnit* __res
   }
 }
 
+// Both stages of a two-stage contraction in one launch (UnitPair): block index = position in the joint unit list.
+__global__ void __launch_bounds__(32) grouped_zgemm_pair_kernel(const GemmUnit* __restrict__ units, int nunits,
+                                                                const GemmSeg* __restrict__ segs, const UnitLink* __restrict__ link,
+                                                                const cplx* __restrict__ A1, const cplx* __restrict__ B1,
+                                                                cplx* __restrict__ C1, const cplx* __restrict__ A2,
+                                                                const cplx* __restrict__ B2, cplx* __restrict__ C2, int conj1,
+                                                                int conj2, const int* __restrict__ dep_id,
+                                                                const unsigned* __restrict__ dep_target,
+                                                                unsigned* __restrict__ dep_cnt, unsigned epoch) {
+  __shared__ __align__(128) unsigned char ring_smem[RING_BYTES];
+  const int lane = threadIdx.x;
+  const int ui = blockIdx.x;
+  if (ui >= nunits) return;
+  pdl_launch_dependents();
+  const GemmUnit u = units[ui];
+  const UnitLink lk = link[ui];
+  pdl_wait();
+  const uint32_t ring = (uint32_t)__cvta_generic_to_shared(ring_smem);
+  const bool second = lk.stage != 0;
+  if (second) {  // wait for the stage-1 outputs this unit reads (lanes share the list; every lane must see the data)
+    for (int d = lk.dep_begin + lane; d < lk.dep_begin + lk.dep_count; d += 32) {
+      const unsigned want = dep_target[d] * epoch;
+      const unsigned* c = dep_cnt + dep_id[d];
+      unsigned v;
+      do {
+        asm volatile("ld.acquire.gpu.u32 %0, [%1];" : "=r"(v) : "l"(c) : "memory");
+      } while (v < want);
+    }
+    __syncwarp();
+    __threadfence();
+  }
+  const cplx* A = second ? A2 : A1;
+  const cplx* B = second ? B2 : B1;
+  cplx* C = second ? C2 : C1;
+  const double cs = (second ? conj2 : conj1) ? -1.0 : 1.0;
+  switch (u.shape) {
+#define FH_CASE(MT, NT)                                    \
+  case MT * 16 + NT:                                       \
+    run_unit<MT, NT>(u, segs, A, B, C, lane, cs, ring);    \
+    break;
+    FH_FOR_SHAPES(FH_CASE)
+#undef FH_CASE
+    default:
+      break;
+  }
+  if (!second) {  // this unit's part of its output is stored: publish it, then count
+    __threadfence();
+    __syncwarp();
+    if (lane == 0) atomicAdd(dep_cnt + lk.sig, 1u);
+  }
+}
+
 }  // namespace
 
+
+void launch_grouped_gemm_pair(const UnitPair& pr, const cplx* A1, const cplx* B1, cplx* C1, const cplx* A2, const cplx* B2,
+                              cplx* C2, unsigned* dep_counters, unsigned epoch, cudaStream_t s, int64_t* lc) {
+  const int n = (int)pr.units.size();
+  if (n == 0) return;
+  launch_pdl(PDL_GEMM_FIRST, grouped_zgemm_pair_kernel, n, 32, s, (const GemmUnit*)pr.d_units, n, (const GemmSeg*)pr.d_segs,
+             (const UnitLink*)pr.d_link, A1, B1, C1, A2, B2, C2, pr.conj1, pr.conj2, (const int*)pr.d_dep_id,
+             (const unsigned*)pr.d_dep_target, dep_counters, epoch);
+  ++*lc;
+}
 
 void launch_grouped_gemm(const Stage& st, const cplx* A, const cplx* B, cplx* C, cudaStream_t s, int64_t* lc,
                          int pdl_role) {

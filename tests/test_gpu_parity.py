@@ -213,7 +213,7 @@ def _per_block_worst(got, ref):
     return worst
 
 
-@pytest.mark.parametrize("chi,path", [(4096, 1), (4096, 2), (1024, 2)])
+@pytest.mark.parametrize("chi,path", [(4096, 1), (4096, 2), (1024, 2), (4096, 3)])
 def test_config3_full_size_all_blocks_both_gemm_forms(H, chi, path):
     """BASELINE config 3 (chi = 4096: the workload and plan bench.py times) and config 2 (chi = 1024), complete:
     the environments L_29, R_31 are contracted on both sides independently from the seeded canonical chain (29
@@ -221,7 +221,7 @@ def test_config3_full_size_all_blocks_both_gemm_forms(H, chi, path):
     the two-site apply (H1 + H2), of the one-site apply on site 30 (H3) and of one more right-environment update
     (H5) are compared with the oracle, per block and globally, relative Frobenius <= 1e-11.  `path` forces the
     form of the grouped ZGEMM heff_apply uses (fh_set_option): 1 = warp units, two launches; 2 = warp-specialised
-    single launch with cross-stage dependency counters and k-split tiles."""
+    single launch with cross-stage dependency counters and k-split tiles; 3 = warp units, both stages in one launch."""
     L, c = 60, 29
     o = central_bond(chi, L)
     dims, W = o["dims"], o["W"]
