@@ -62,7 +62,7 @@ const char* fh_last_error(const fh_ctx* ctx);
  *                        form 1).  Same results to rounding (the k-split tiles of form 2 add partial sums in
  *                        another, fixed, order).
  *   FH_OPT_SVD_MID_MAXN  widest sector matrix (columns) the library's own global-memory Jacobi kernel takes
- *                        instead of the vendor SVD, 0 .. 256 (default 128; 0 = none).
+ *                        instead of the vendor SVD, 0 .. 256 (default 100; 0 = none).
  *   FH_OPT_SVD_THREADS   host threads that drive the vendor SVD / QR routines, 1 .. 12 (default: cores - 1,
  *                        at most 12); takes effect before the first factorisation of the context.
  *   FH_OPT_SVD_SMALL_MAXN widest sector matrix (columns) the shared-memory Jacobi / Householder kernels take, provided
@@ -88,6 +88,14 @@ const char* fh_last_error(const fh_ctx* ctx);
  *                        error (<= ~1e-6 relative Frobenius per apply; oracle/splitprec.py states the bounds).
  *                        One-site applies, environment updates, vector kernels and the SVD stay FP64. */
 #define FH_OPT_PRECISION 6
+/*   FH_OPT_SVD_GRAM_MINN narrowest sector matrix (columns, 0 .. 65536; default 104; 0 = never) among those the vendor
+ *                        SVD would take that is factorised through its Gram matrix instead: G = B^H B, Hermitian
+ *                        eigendecomposition (cusolverDnZheevd), U = B V / sigma.  2.7 x faster per matrix at 600
+ *                        columns, and the largest sector matrix of a bond is the critical path of the SVD phase.
+ *                        Accurate for the singular values a chi-capped truncation keeps (error eps sigma_max^2 /
+ *                        sigma_i); a sector whose smallest KEPT singular value is below 3e-3 of its largest is redone
+ *                        by the vendor SVD before the bond is updated (fh_factorization_stats [7], [8]). */
+#define FH_OPT_SVD_GRAM_MINN 7
 int fh_set_option(fh_ctx* ctx, int key, int value);
 /* bytes currently allocated / high-water mark in the arena */
 int fh_arena_stats(const fh_ctx* ctx, size_t* used_bytes, size_t* peak_bytes);
@@ -195,8 +203,10 @@ int heff_expm_adaptive(fh_ctx* ctx, const void* theta_dev, void* out_dev, double
  * (n < 48, or redo of [3]), [3] gesvdp results rejected because it reported a perturbed spectrum,
  * [4] Householder QR by cusolverDnZgeqrf + Zungqr (one-site splits that do not fit shared memory), [5] Householder
  * QR by the library's own shared-memory kernel, [6] own global-memory Jacobi kernel (matrices above the
- * shared-memory route with at most 128 columns; it runs on a side stream beside the vendor routines). */
-int fh_factorization_stats(const fh_ctx* ctx, int64_t counts[7]);
+ * shared-memory route with at most 128 columns; it runs on a side stream beside the vendor routines), [7] Gram-matrix
+ * eigenvalue route (G = B^H B, cusolverDnZheevd, U = B V / sigma; FH_OPT_SVD_GRAM_MINN), [8] sectors of [7] redone by
+ * the vendor SVD because the truncation kept a singular value below 3e-3 of the sector's largest. */
+int fh_factorization_stats(const fh_ctx* ctx, int64_t counts[9]);
 /* Task-list cache of the one-site sweeps (H0).  One-site TDVP keeps every bond's sector table
  * (no SVD, bond dimension fixed), so tdvp1_sweep / tdvp_sweep_auto keep the task lists they emit in
  * host memory owned by the fh_mps and reuse an entry only when the labels and shapes of every tensor the emitter

@@ -451,10 +451,10 @@ class Context:
         return k.value
 
     def fh_factorization_stats(self):
-        a = (C.c_int64 * 7)()
+        a = (C.c_int64 * 9)()
         self.check(lib.fh_factorization_stats(self.h, a), "fh_factorization_stats")
         return dict(jacobi_kernel=a[0], gesvdp=a[1], gesvd=a[2], gesvdp_rejected=a[3], qr=a[4], qr_kernel=a[5],
-                    jacobi_mid_kernel=a[6])
+                    jacobi_mid_kernel=a[6], gram_eig=a[7], gram_redone=a[8])
 
     def fh_get_traffic(self):
         a, b = c_i64(0), c_i64(0)
@@ -519,7 +519,7 @@ class Context:
     def fh_launch_count(self):
         return int(lib.fh_launch_count(self.h))
 
-    OPT_GEMM_PATH, OPT_SVD_MID_MAXN, OPT_SVD_THREADS, OPT_SVD_SMALL_MAXN, OPT_SYMMETRY, OPT_PRECISION = 1, 2, 3, 4, 5, 6
+    OPT_GEMM_PATH, OPT_SVD_MID_MAXN, OPT_SVD_THREADS, OPT_SVD_SMALL_MAXN, OPT_SYMMETRY, OPT_PRECISION, OPT_SVD_GRAM_MINN = 1, 2, 3, 4, 5, 6, 7
 
     def fh_set_option(self, key, value):
         self.check(lib.fh_set_option(self.h, int(key), int(value)), "fh_set_option")

@@ -826,6 +826,7 @@ void fh_ctx_destroy(fh_ctx* c) {
     if (w.s) cudaStreamSynchronize(w.s);
     if (w.h) cusolverDnDestroy(w.h);
     if (w.params) cusolverDnDestroyParams(w.params);
+    if (w.cb) cublasDestroy(w.cb);
     if (w.dwork) cudaFree(w.dwork);
     if (w.d_info) cudaFree(w.d_info);
     if (w.done) cudaEventDestroy(w.done);
@@ -856,6 +857,10 @@ int fh_set_option(fh_ctx* c, int key, int value) {
     case FH_OPT_SVD_SMALL_MAXN:
       if (value < 0 || value > 4096) return FH_EINVAL;
       c->opt_svd_small_maxn = value;
+      return FH_OK;
+    case FH_OPT_SVD_GRAM_MINN:
+      if (value < 0 || value > 65536) return FH_EINVAL;
+      c->opt_svd_gram_minn = value;
       return FH_OK;
     case FH_OPT_PRECISION:
       if (value < 0 || value > 1) return FH_EINVAL;
@@ -1376,8 +1381,10 @@ int heff_expm_adaptive(fh_ctx* ctx, const void* theta_dev, void* out_dev, double
   return heff_expm_impl(ctx, theta_dev, out_dev, tau, krylov_dim, adapt_tol, k_used);
 }
 
-int fh_factorization_stats(const fh_ctx* ctx, int64_t counts[7]) {
+int fh_factorization_stats(const fh_ctx* ctx, int64_t counts[9]) {
   if (!ctx || !counts) return FH_EINVAL;
+  counts[7] = ctx->svd_count[3];
+  counts[8] = ctx->svd_gram_redone;
   counts[6] = ctx->svd_mid;
   counts[5] = ctx->qr_small;
   counts[0] = ctx->svd_small;

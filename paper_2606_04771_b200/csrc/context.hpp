@@ -1,5 +1,6 @@
 // Context, arena, device pools, plans (host side of libfh_b200).
 #pragma once
+#include <cublas_v2.h>
 #include <cusolverDn.h>
 
 #include <future>
@@ -191,6 +192,7 @@ struct fh_ctx {
   struct SvdWorker {
     cusolverDnHandle_t h = nullptr;
     cusolverDnParams_t params = nullptr;
+    cublasHandle_t cb = nullptr;          // Gram / back-multiplication GEMMs of the eigenvalue route (tdvp.cu, svd_one)
     cudaStream_t s = nullptr;
     void* dwork = nullptr;
     size_t dwork_bytes = 0;
@@ -209,9 +211,11 @@ struct fh_ctx {
   int device = 0;
   const fh::SymMode* sym = &fh::SYM_SU2;  // fh_set_option(FH_OPT_SYMMETRY): the label algebra of every object of the context
   int opt_gemm_path = 0;      // fh_set_option: 0 auto, 1 warp units (two launches), 2 warp-specialised, 3 warp units (one launch)
-  int opt_svd_mid_maxn = 128;
+  int opt_svd_mid_maxn = 100;
   int opt_svd_small_maxn = 4096;
   int opt_svd_threads = 0;    // 0 = default
+  int opt_svd_gram_minn = 104;  // fh_set_option(FH_OPT_SVD_GRAM_MINN): narrowest sector matrix (columns) of the vendor route that
+                                // goes through the Gram-matrix eigenvalue route (0 = never)
   int opt_precision = 0;      // fh_set_option(FH_OPT_PRECISION): 0 = FP64 DMMA, 1 = 3 x TF32 on tcgen05 (two-site applies)
   int num_sms = 148;
   unsigned* d_ws_counters = nullptr;  // tile-queue head and retired-CTA count of the warp-specialised GEMM (zero between launches)
@@ -221,7 +225,8 @@ struct fh_ctx {
   int* h_fact_status = nullptr;  // pinned
   int fact_status_cap = 0, fact_status_n = 0;
   bool fact_status_pending = false;
-  int64_t svd_count[3] = {0, 0, 0};  // gesvd, gesvdp, gesvdp fallbacks to gesvd
+  int64_t svd_count[4] = {0, 0, 0, 0};  // gesvd, gesvdp, gesvdp fallbacks to gesvd, Gram-matrix eigenvalue route
+  int64_t svd_gram_redone = 0;           // Gram-route sectors redone by the vendor SVD (a kept singular value too small)
   int64_t qr_small = 0;  // one-site splits done by small_qr_kernel
   int64_t svd_small = 0, qr_count = 0;  // sector matrices done by small_svd_kernel / by geqrf+ungqr
   int64_t krylov_calls = 0, krylov_vectors = 0;  // exponentials evaluated / Krylov vectors (= H_eff applies) used

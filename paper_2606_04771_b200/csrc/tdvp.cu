@@ -42,6 +42,7 @@ struct SectorSvd {
   std::vector<std::pair<Key, std::pair<int, int>>> rows;  // (a,s1) part: key{a.q,a.tj,s1}, (offset, dim)
   std::vector<std::pair<Key, std::pair<int, int>>> cols;  // (s2,b) part: key{s2,b.q,b.tj}
   int keep = 0;
+  bool gram = false;       // factorised by the Gram-matrix eigenvalue route (svd_one): checked after the truncation
   // QR mode (one-site split): column-major A (qm x qn) at m_off, tau at u_off, R written to r_dst
   int qm = 0, qn = 0, r_ld = 0, r_transpose = 0;
   cplx* r_dst = nullptr;
@@ -446,11 +447,29 @@ __global__ void __launch_bounds__(32 * SMALL_QR_MAX_WARPS) small_qr_kernel(const
 
 void worker_reserve(fh_ctx::SvdWorker& w, size_t bytes) {
   if (bytes <= w.dwork_bytes) return;
+  bytes = std::max<size_t>(bytes, (size_t)48 << 20);  // at least 48 MB: covers chi = 4096 without growing again
   FH_CUDA(cudaStreamSynchronize(w.s));
   if (w.dwork) FH_CUDA(cudaFree(w.dwork));
   w.dwork = nullptr;
   w.dwork_bytes = bytes + bytes / 2;
   FH_CUDA(cudaMalloc(&w.dwork, w.dwork_bytes));
+}
+
+// Gram-matrix eigenvalue route, last step: eigenpairs of G = B^H B (ascending, vectors in the columns of W) ->
+// singular values (descending), V^H (n x n, ld n) and Vs = V Sigma^-1 (n x n, ld n; zero columns where sigma = 0)
+__global__ void gram_finish_kernel(const cplx* __restrict__ W, const double* __restrict__ lam, int n, double* __restrict__ sv,
+                                   cplx* __restrict__ VT, cplx* __restrict__ Vs) {
+  const int64_t total = (int64_t)n * n;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x) {
+    const int j = (int)(e % n), i = (int)(e / n);  // component j of right singular vector i
+    const double l = lam[n - 1 - i];
+    const double sg = l > 0.0 ? sqrt(l) : 0.0;
+    const cplx v = W[j + (int64_t)(n - 1 - i) * n];
+    VT[i + (int64_t)j * n] = make_double2(v.x, -v.y);
+    const double r = sg > 0.0 ? 1.0 / sg : 0.0;
+    Vs[j + (int64_t)i * n] = make_double2(v.x * r, v.y * r);
+    if (j == 0) sv[i] = sg;
+  }
 }
 
 const int GESVDP_MIN_N = 48;  // below this the QR-iteration driver is as fast and has no conditioning caveat
@@ -460,12 +479,48 @@ const int GESVDP_MIN_N = 48;  // below this the QR-iteration driver is as fast a
 // n >= GESVDP_MIN_N: cusolverDnXgesvdp (polar decomposition + Hermitian eigensolver; measured 3.3x
 // faster than Zgesvd at n = 600) on a copy; if it reports a perturbation of the spectrum
 // (err_sigma != 0: numerically rank-deficient input) the QR-iteration driver Zgesvd redoes it.
-void svd_one(fh_ctx::SvdWorker& w, const SectorSvd& S, cplx* buf, double* dS, int64_t* counts, int* d_status) {
+//
+// Gram route (gram_minn > 0 and n >= gram_minn): G = B^H B (one ZGEMM), Hermitian eigendecomposition G = V Lambda V^H
+// (cusolverDnZheevd: 8 ms at n = 600 where gesvdp takes 23 ms, and the largest sector matrix of a bond is the
+// critical path of the whole SVD phase: the phase does not depend on the number of workers), sigma = sqrt(lambda),
+// U = B V Sigma^-1 (one ZGEMM).  Squaring the matrix costs accuracy for SMALL singular values only: sigma_i comes out
+// with an absolute error of eps sigma_max^2 / (2 sigma_i) and the columns of U are orthonormal to eps (sigma_max /
+// sigma_i)^2.  The caller therefore accepts the result of a sector only if every singular value the truncation KEEPS
+// is >= GRAM_SAFE_RATIO sigma_max of that sector, and sends the sector through the routes below otherwise
+// (svd_split).  In a chi-capped sweep the kept values of the large sectors are >= 1e-2 sigma_max.
+const double GRAM_SAFE_RATIO = 3e-3;  // U orthonormal to 1.2e-11, sigma to 2e-14 sigma_max
+void svd_one(fh_ctx::SvdWorker& w, SectorSvd& S, cplx* buf, double* dS, int64_t* counts, int* d_status, int gram_minn) {
   const int m = std::max(S.nrow, S.ncol), n = S.k;
   cuDoubleComplex* A = (cuDoubleComplex*)(buf + S.m_off);
   cuDoubleComplex* U = (cuDoubleComplex*)(buf + S.u_off);
   cuDoubleComplex* VT = (cuDoubleComplex*)(buf + S.vt_off);
   double* sv = dS + S.s_off;
+  S.gram = false;
+  if (gram_minn > 0 && n >= gram_minn) {
+    const size_t g_bytes = ((size_t)n * n * sizeof(cplx) + 255) / 256 * 256;
+    const size_t l_bytes = ((size_t)n * sizeof(double) + 255) / 256 * 256;
+    int lwork = 0;
+    FH_CUSOLVER(cusolverDnZheevd_bufferSize(w.h, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, n, nullptr, n, nullptr, &lwork));
+    worker_reserve(w, 2 * g_bytes + l_bytes + (size_t)lwork * sizeof(cuDoubleComplex) + 256);
+    char* base = (char*)w.dwork;
+    cuDoubleComplex* G = (cuDoubleComplex*)base;
+    cuDoubleComplex* Vs = (cuDoubleComplex*)(base + g_bytes);
+    double* lam = (double*)(base + 2 * g_bytes);
+    cuDoubleComplex* work = (cuDoubleComplex*)(base + 2 * g_bytes + l_bytes);
+    const cuDoubleComplex one = make_cuDoubleComplex(1.0, 0.0), zero = make_cuDoubleComplex(0.0, 0.0);
+    FH_REQUIRE(cublasZgemm(w.cb, CUBLAS_OP_C, CUBLAS_OP_N, n, n, m, &one, A, m, A, m, &zero, G, n) == CUBLAS_STATUS_SUCCESS,
+               FH_ECUDA, "svd: cublasZgemm (Gram matrix) failed");
+    FH_CUSOLVER(cusolverDnZheevd(w.h, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, n, G, n, lam, work, lwork, w.d_info));
+    const int64_t tot = (int64_t)n * n;
+    gram_finish_kernel<<<(int)std::min<int64_t>((tot + 255) / 256, 1184), 256, 0, w.s>>>((const cplx*)G, lam, n, sv, (cplx*)VT,
+                                                                                     (cplx*)Vs);
+    FH_REQUIRE(cublasZgemm(w.cb, CUBLAS_OP_N, CUBLAS_OP_N, m, n, n, &one, A, m, Vs, n, &zero, U, m) == CUBLAS_STATUS_SUCCESS,
+               FH_ECUDA, "svd: cublasZgemm (U = B V / sigma) failed");
+    FH_CUDA(cudaMemcpyAsync(d_status, w.d_info, sizeof(int), cudaMemcpyDeviceToDevice, w.s));
+    S.gram = true;
+    ++counts[3];
+    return;
+  }
   if (n >= GESVDP_MIN_N) {
     const size_t a_bytes = ((size_t)m * n * sizeof(cplx) + 255) / 256 * 256;
     const size_t v_bytes = ((size_t)n * n * sizeof(cplx) + 255) / 256 * 256;
@@ -534,7 +589,9 @@ const void* stage_small_desc(fh_ctx* ctx, const void* src, size_t bytes) {
 // counter; every worker has its own cuSOLVER handle, stream and workspace.  The main stream forks
 // into the worker streams and joins them again through events, so the phase timers on the main
 // stream cover the whole batch.
-void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* buf, double* dS, bool qr = false) {
+void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* buf, double* dS, bool qr = false,
+                     bool allow_gram = true) {
+  const int gram_minn = (allow_gram && !qr) ? ctx->opt_svd_gram_minn : 0;
   if (ctx->svd_workers.empty()) {
     int nw = (int)std::thread::hardware_concurrency() - 1;
     if (ctx->opt_svd_threads > 0) nw = ctx->opt_svd_threads;
@@ -545,6 +602,8 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
       FH_CUSOLVER(cusolverDnCreate(&w.h));
       FH_CUSOLVER(cusolverDnSetStream(w.h, w.s));
       FH_CUSOLVER(cusolverDnCreateParams(&w.params));
+      FH_REQUIRE(cublasCreate(&w.cb) == CUBLAS_STATUS_SUCCESS, FH_ECUDA, "cublasCreate failed");
+      cublasSetStream(w.cb, w.s);
       FH_CUDA(cudaMalloc((void**)&w.d_info, sizeof(int)));
       FH_CUDA(cudaEventCreateWithFlags(&w.done, cudaEventDisableTiming));
     }
@@ -578,7 +637,7 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
   size_t small_smem = 0, small_qr_smem = 0;
   int64_t mid_v_total = 0;
   // fh_set_option(FH_OPT_SVD_MID_MAXN): 0 sends every matrix above the shared-memory route to cuSOLVER;
-  // default 128: 64 column pairs per tournament round = two per warp of the 32-warp CTA
+  // default 100 since the Gram route exists (measured: sweep 4.00 s with 100 / 104, 4.19 s with 128 / 160)
   const int mid_maxn = std::max(0, std::min(ctx->opt_svd_mid_maxn, MID_SVD_HARD_MAXN));
   const double mid_work = 1.5 * mid_maxn * (double)mid_maxn * mid_maxn;  // m n^2 bound: a long thin matrix would make its one CTA the critical path
   const int small_maxn = ctx->opt_svd_small_maxn;  // fh_set_option(FH_OPT_SVD_SMALL_MAXN)
@@ -695,7 +754,7 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
   std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) { return cost(a) > cost(b); });
   std::atomic<int> next{0};
   std::vector<std::string> errs(nw);
-  std::vector<std::array<int64_t, 3>> counts(nw, std::array<int64_t, 3>{0, 0, 0});
+  std::vector<std::array<int64_t, 4>> counts(nw, std::array<int64_t, 4>{0, 0, 0, 0});
   auto body = [&](int wi) {
     try {
       FH_CUDA(cudaSetDevice(ctx->device));
@@ -704,7 +763,7 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
         const int i = next.fetch_add(1);
         if (i >= (int)idx.size()) break;
         if (qr) qr_one(w, *order[idx[i]], buf, d_status + idx[i], d_status + nord + idx[i]);
-        else svd_one(w, *order[idx[i]], buf, dS, counts[wi].data(), d_status + idx[i]);
+        else svd_one(w, *order[idx[i]], buf, dS, counts[wi].data(), d_status + idx[i], gram_minn);
       }
       FH_CUDA(cudaEventRecord(w.done, w.s));
     } catch (const std::exception& e) {
@@ -729,7 +788,7 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
       continue;
     }
     FH_CUDA(cudaStreamWaitEvent(ctx->stream, ctx->svd_workers[t].done, 0));
-    for (int k = 0; k < 3; ++k) ctx->svd_count[k] += counts[t][k];
+    for (int k = 0; k < 4; ++k) ctx->svd_count[k] += counts[t][k];
   }
   join_side();
   if (!first_err.empty()) throw FhError(FH_ECUDA, "sector SVD worker: " + first_err);
@@ -894,7 +953,26 @@ static void svd_split(fh_ctx* ctx, fh_mps* mps, int i, const BlockTensor& th, co
     sv.emplace_back(ctx->h_pinned + S->s_off, ctx->h_pinned + S->s_off + S->k);
     mult.push_back(S->c.tj + 1);
   }
-  const double disc = truncate_rule(sv, mult, prm->chi_max_full, prm->eps_trunc, keep);
+  double disc = truncate_rule(sv, mult, prm->chi_max_full, prm->eps_trunc, keep);
+  {
+    // sectors factorised through the Gram matrix are accepted only if every KEPT singular value is large enough for
+    // that route to be accurate (svd_one); the others are redone by the vendor SVD and the selection is repeated
+    std::vector<SectorSvd*> redo;
+    for (size_t x = 0; x < order.size(); ++x)
+      if (order[x]->gram && keep[x] > 0 && sv[x][keep[x] - 1] < GRAM_SAFE_RATIO * sv[x][0]) redo.push_back(order[x]);
+    if (!redo.empty()) {
+      ctx->timer_begin(T_SVD);
+      run_sector_svds(ctx, redo, buf, dS, false, false);
+      FH_CUDA(cudaMemcpyAsync(ctx->h_pinned, dS, dbl_total * sizeof(double), cudaMemcpyDeviceToHost, s));
+      FH_CUDA(cudaStreamSynchronize(s));
+      ctx->timer_end();
+      check_fact_status(ctx);
+      ctx->svd_gram_redone += (int64_t)redo.size();
+      for (size_t x = 0; x < order.size(); ++x)
+        sv[x].assign(ctx->h_pinned + order[x]->s_off, ctx->h_pinned + order[x]->s_off + order[x]->k);
+      disc = truncate_rule(sv, mult, prm->chi_max_full, prm->eps_trunc, keep);
+    }
+  }
   ctx->stat_disc = std::max(ctx->stat_disc, disc);
   Bond nb;
   for (size_t x = 0; x < order.size(); ++x) {

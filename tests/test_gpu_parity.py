@@ -440,7 +440,8 @@ def test_config1_neel_quench_L8_vs_oracle(H, ctx):
     ctx.mps_destroy(mps)
 
 
-@pytest.mark.parametrize("L,chi,route", [(12, 128, "default"), (14, 200, "default"), (12, 128, "mid"), (12, 128, "vendor")])
+@pytest.mark.parametrize("L,chi,route", [(12, 128, "default"), (14, 200, "default"), (12, 128, "mid"), (12, 128, "vendor"),
+                                         (12, 128, "gram"), (14, 200, "gram")])
 def test_config3_sweep_recipe_reduced_size_vs_oracle(H, ctx, L, chi, route):
     """The second half of BASELINE config 3 -- one tdvp2_sweep(0.05), m = 10, truncation back to chi by block-wise
     SVD, started from the seeded random canonical chain (the recipe bench.py times at L = 60,
@@ -452,10 +453,13 @@ def test_config3_sweep_recipe_reduced_size_vs_oracle(H, ctx, L, chi, route):
     then one tdvp1_sweep on the result (one-site splits by QR) against the oracle's step1.
     `route` sends the sector matrices of this small case through the factorisation routes that large bonds use
     (fh_set_option): "mid" = the global-memory Jacobi kernel and cusolver's geqrf/ungqr, "vendor" = cusolver's
-    gesvdp / gesvd and geqrf/ungqr; "default" = the shared-memory Jacobi and Householder kernels."""
+    gesvdp / gesvd and geqrf/ungqr; "default" = the shared-memory Jacobi and Householder kernels; "gram" = the
+    Gram-matrix eigenvalue route (G = B^H B, Zheevd, U = B V / sigma) for every matrix of at least 8 columns, with its
+    acceptance test on the kept singular values and the vendor redo of the sectors that fail it."""
     if route != "default":
         ctx.fh_set_option(ctx.OPT_SVD_SMALL_MAXN, 0)
         ctx.fh_set_option(ctx.OPT_SVD_MID_MAXN, 128 if route == "mid" else 0)
+    ctx.fh_set_option(ctx.OPT_SVD_GRAM_MINN, 8 if route == "gram" else 0)
     dims = fi.chain_dims(chi, L, "gaussian", (1, 1))
     sites = {}
     for i, A, dl, dr in fi.canonical_chain(chi, 0, L, fi.SEED, dims=dims, weight=symm.canonical_weight):
@@ -501,9 +505,42 @@ def test_config3_sweep_recipe_reduced_size_vs_oracle(H, ctx, L, chi, route):
         assert routes["jacobi_mid_kernel"] > 0 and routes["jacobi_kernel"] == 0 and f2["qr"] - f1["qr"] > 0
     if route == "vendor":
         assert routes["gesvdp"] + routes["gesvd"] > 0 and routes["jacobi_kernel"] == routes["jacobi_mid_kernel"] == 0
+        assert routes["gram_eig"] == 0
+    if route == "gram":
+        assert routes["gram_eig"] > 0 and routes["jacobi_kernel"] == routes["jacobi_mid_kernel"] == 0
+        assert routes["gram_redone"] < routes["gram_eig"]          # some sectors pass the acceptance test
     print("L=%d chi=%d sweep: sv %.1e s_max, obs %.1e / one-site %.1e, discarded %.3e (oracle %.3e); SVD routes %s; "
           "QR routes %s" % (L, chi, worst_sv, worst, worst1, st["max_discarded"], ref.max_discarded, routes,
                             {k: f2[k] - f1[k] for k in f2 if k.startswith("qr")}))
+    ctx.mps_destroy(mps)
+
+
+def test_gram_route_redone_when_small_singular_values_are_kept(H, ctx):
+    """The Gram-matrix eigenvalue route (FH_OPT_SVD_GRAM_MINN) squares the matrix and is accurate only for singular
+    values that are not small; the library accepts its result for a sector only if every KEPT value is >= 3e-3 of
+    the sector's largest and redoes the sector by the vendor SVD otherwise.  An UNtruncated quench keeps everything
+    (down to rule A-6's floor), so with the route forced on every matrix the redo must fire, and the run must still
+    agree with the dense oracle as the default routes do (config 1's problem, 8 steps: observables <= 1e-8,
+    norm to 1e-10)."""
+    from oracle import dense_tdvp as dtv
+    L, dt, m = 8, 0.05, 10
+    ctx.fh_set_option(ctx.OPT_SVD_SMALL_MAXN, 0)
+    ctx.fh_set_option(ctx.OPT_SVD_MID_MAXN, 0)
+    ctx.fh_set_option(ctx.OPT_SVD_GRAM_MINN, 2)
+    ref = dtv.DenseTDVP(L, 1.0, 4.0, krylov_dim=m)
+    mpo = ctx.fh_mpo_build(L, 1.0, 4.0)
+    mps = ctx.mps_init_neel(mpo, L)
+    worst = 0.0
+    for step in range(8):
+        ref.step(dt)
+        ctx.tdvp2_sweep(mpo, mps, dt, krylov_dim=m, chi_max_full=256, eps_trunc=-1.0)
+        o, g = ref.observables(), ctx.measure_local(mps, L)
+        worst = max(worst, np.abs(g["sz"] - 0.5 * (o["n_up"] - o["n_dn"])).max(), np.abs(g["docc"] - o["docc"]).max())
+    f = ctx.fh_factorization_stats()
+    gg = ctx.measure_global(mpo, mps)
+    print("Gram route forced, untruncated L=8 quench: obs %.1e, norm^2 - 1 %.1e, routes %s" % (worst, gg["norm2"] - 1, f))
+    assert f["gram_eig"] > 0 and f["gram_redone"] > 0 and f["jacobi_kernel"] == 0
+    assert worst < 1e-8 and abs(gg["norm2"] - 1) < 1e-10
     ctx.mps_destroy(mps)
 
 
