@@ -2,27 +2,34 @@
 // reading A-18) on the fifth-generation tensor cores:
 //     C_o (M x N) = sum_{t in seg(o)} alpha_t * op(A_t) (M x K_t) * op(B_t) (K_t x N),  alpha_t real,
 // with complex128 operands and results in memory (the same task lists, layouts and launch interface as zgemm.cu)
-// and the products taken as 3 x TF32:  x = hi + lo (+ 2^-22 |x|; hi, lo = x and x - hi rounded to 11 significant bits),  a b ~ hi hi + hi lo + lo hi, accumulated in
-// float32 in tensor memory (oracle/splitprec.py states the arithmetic and its two error bounds).
+// and the products taken as 3 x TF32:  x = hi + lo (+ 2^-22 |x|; hi, lo = x and x - hi rounded to 11 significant
+// bits),  a b ~ hi hi + hi lo + lo hi, accumulated in float32 in tensor memory (oracle/splitprec.py states the
+// arithmetic and its two error bounds).
 //
-// One persistent CTA per SM, 13 warps, three roles that meet only at mbarriers:
-//   * 8 CONVERTER warps (4 for the A panel, 4 for the B panel; one lane = one row of the 128-row panel) walk the
-//     k range of a tile 16 k at a time: complex128 loads straight from the operand blocks (any stride pair, zero
-//     beyond a segment's K), alpha and the conjugation sign folded into A, every real number split into its two
-//     TF32 parts, and the four planes (re hi, re lo, im hi, im lo) of the panel written to shared memory in the
-//     K-major no-swizzle core-matrix layout tcgen05.mma reads (8 rows x 16 B per core matrix; 128 B between
-//     row groups, 2048 B between k quads).  No packed copy of an operand exists in global memory: the split
-//     representation is 16 B per complex number, as many bytes as the complex128 it is made from.
+// One persistent CTA per SM, 22 warps, four roles that meet only at mbarriers:
+//   * The operand of a stage that does not change between applies (an environment: op(A) of stage 1, op(B) of
+//     stage 2) is converted ONCE per plan by tc_pack_kernel into PANEL IMAGES -- per 128-row tile and 16-k chunk
+//     the four TF32 planes (re hi, re lo, im hi, im lo) in exactly the shared-memory layout below, 32 KB, zero
+//     padded, one image per distinct block however many segments read it -- and ONE thread streams them into the
+//     ring with cp.async.bulk onto the stage's mbarrier (complete_tx).
+//   * 16 CONVERTER warps (one thread = one row of the 128-row panel and 4 of a chunk's 16 k) load the operand that
+//     changes with every apply as complex128 straight from its blocks (any stride pair, zero beyond a segment's K;
+//     the loads of the next chunk of the segment are in flight while the current one is converted), fold the
+//     segment's alpha (and the conjugation sign) into it, split every real number into its two TF32 parts, and
+//     write the four planes of the panel to shared memory in the K-major no-swizzle core-matrix layout
+//     tcgen05.mma reads (8 rows x 16 B per core matrix; 128 B between row groups, 2048 B between k quads).
+//     Without a static operand (fh_zgemm_split) 8 + 8 converter warps take the A and the B panel, alpha on A.
 //   * ONE thread issues the MMAs: per 8 k, 12 x tcgen05.mma.kind::tf32 (M = 128, N = the tile width rounded up
 //     to 16): Re C += Ar Br - Ai Bi, Im C += Ar Bi + Ai Br, each as hi hi + hi lo + lo hi; the minus sign is the
 //     negate-A bit of the instruction descriptor.  Accumulators: 2 x 128 float32 columns of tensor memory per
-//     tile, double buffered (all 512 columns).  tcgen05.commit hands a shared-memory stage back to the converters
-//     and, after the last chunk of a tile, the accumulator buffer over to the epilogue.
+//     tile, double buffered (all 512 columns).  tcgen05.commit hands a shared-memory stage (3 x 64 KB) back to the
+//     producers and, after the last chunk of a tile, the accumulator buffer over to the epilogue.
 //   * 4 EPILOGUE warps (warp w owns TMEM lanes 32 w ... 32 w + 31 = tile rows) read the accumulators with
 //     tcgen05.ld (32 lanes x 32 columns per instruction), widen them to double and store complex128.
-// All K segments of an output accumulate in tensor memory (alpha is inside A), so there is one epilogue per tile.
-// Tiles are dealt to the CTAs on the host (heaviest first to the least loaded); a tile without segments is stored as zeros.
-// Deterministic: fixed tile -> CTA map, fixed k order, one accumulator per output element.
+// All K segments of an output accumulate in tensor memory (alpha is inside the converted operand), so there is one
+// epilogue per tile.  Tiles are dealt to the CTAs on the host (heaviest first to the least loaded); a tile without
+// segments is stored as zeros.  Deterministic: fixed tile -> CTA map, fixed k order, one accumulator per output
+// element.  Measurements, ablations and what was tried and dropped: DESIGN.md 6.8, profiles/r2_zgemm_tc_ncu.md.
 #include "fh_internal.hpp"
 
 #include <algorithm>
