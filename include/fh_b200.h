@@ -96,6 +96,12 @@ const char* fh_last_error(const fh_ctx* ctx);
  *                        sigma_i); a sector whose smallest KEPT singular value is below 3e-3 of its largest is redone
  *                        by the vendor SVD before the bond is updated (fh_factorization_stats [7], [8]). */
 #define FH_OPT_SVD_GRAM_MINN 7
+/*   FH_OPT_SVD_GRAM_BATCH_MAXN widest Gram-route sector matrix (columns; default 256; 0 = none) whose eigenproblem is
+ *                        solved together with those of the other such sectors of the bond in ONE batched vendor call
+ *                        (cusolverDnXsyevBatched on Gram matrices padded to a common size) instead of one call per
+ *                        matrix: the vendor eigensolvers are chains of small dependent kernels and a bond's sixteen
+ *                        chains queue on the GPU front end; the batched solver walks one chain for all of them. */
+#define FH_OPT_SVD_GRAM_BATCH_MAXN 8
 int fh_set_option(fh_ctx* ctx, int key, int value);
 /* bytes currently allocated / high-water mark in the arena */
 int fh_arena_stats(const fh_ctx* ctx, size_t* used_bytes, size_t* peak_bytes);

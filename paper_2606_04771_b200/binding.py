@@ -519,7 +519,7 @@ class Context:
     def fh_launch_count(self):
         return int(lib.fh_launch_count(self.h))
 
-    OPT_GEMM_PATH, OPT_SVD_MID_MAXN, OPT_SVD_THREADS, OPT_SVD_SMALL_MAXN, OPT_SYMMETRY, OPT_PRECISION, OPT_SVD_GRAM_MINN = 1, 2, 3, 4, 5, 6, 7
+    OPT_GEMM_PATH, OPT_SVD_MID_MAXN, OPT_SVD_THREADS, OPT_SVD_SMALL_MAXN, OPT_SYMMETRY, OPT_PRECISION, OPT_SVD_GRAM_MINN, OPT_SVD_GRAM_BATCH_MAXN = 1, 2, 3, 4, 5, 6, 7, 8
 
     def fh_set_option(self, key, value):
         self.check(lib.fh_set_option(self.h, int(key), int(value)), "fh_set_option")

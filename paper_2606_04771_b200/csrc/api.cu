@@ -862,6 +862,10 @@ int fh_set_option(fh_ctx* c, int key, int value) {
       if (value < 0 || value > 65536) return FH_EINVAL;
       c->opt_svd_gram_minn = value;
       return FH_OK;
+    case FH_OPT_SVD_GRAM_BATCH_MAXN:
+      if (value < 0 || value > 65536) return FH_EINVAL;
+      c->opt_svd_gram_batch_maxn = value;
+      return FH_OK;
     case FH_OPT_PRECISION:
       if (value < 0 || value > 1) return FH_EINVAL;
       c->opt_precision = (int)value;

@@ -216,6 +216,7 @@ struct fh_ctx {
   int opt_svd_threads = 0;    // 0 = default
   int opt_svd_gram_minn = 104;  // fh_set_option(FH_OPT_SVD_GRAM_MINN): narrowest sector matrix (columns) of the vendor route that
                                 // goes through the Gram-matrix eigenvalue route (0 = never)
+  int opt_svd_gram_batch_maxn = 256;  // fh_set_option(FH_OPT_SVD_GRAM_BATCH_MAXN): widest Gram-route sector that joins the batched eigensolver call
   int opt_precision = 0;      // fh_set_option(FH_OPT_PRECISION): 0 = FP64 DMMA, 1 = 3 x TF32 on tcgen05 (two-site applies)
   int num_sms = 148;
   unsigned* d_ws_counters = nullptr;  // tile-queue head and retired-CTA count of the warp-specialised GEMM (zero between launches)

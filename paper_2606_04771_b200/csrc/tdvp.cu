@@ -472,6 +472,42 @@ __global__ void gram_finish_kernel(const cplx* __restrict__ W, const double* __r
   }
 }
 
+// Batched form of the Gram route (gram_batch below): the Gram matrix of a sector sits in the top-left n x n block of
+// an npad x npad slot (ld npad); this kernel, launched after the ZGEMM that wrote the block, clears the rest of the
+// slot and puts -(1 + trace G) on the padded diagonal: npad - n eigenvalues below every true one (>= 0), whose
+// eigenvectors are unit vectors of the padding, so the true eigenpairs are the LAST n of the ascending list.
+__global__ void gram_pad_kernel(cplx* __restrict__ G, int n, int npad) {
+  __shared__ double tr;
+  if (threadIdx.x < 32) {
+    double t = 0.0;
+    for (int i = threadIdx.x; i < n; i += 32) t += G[i + (int64_t)i * npad].x;
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    if (threadIdx.x == 0) tr = t;
+  }
+  __syncthreads();
+  const double pad = -(1.0 + tr);
+  const int64_t total = (int64_t)npad * npad;
+  for (int64_t e = threadIdx.x; e < total; e += blockDim.x) {
+    const int i = (int)(e % npad), j = (int)(e / npad);
+    if (i >= n || j >= n) G[e] = make_double2(i == j ? pad : 0.0, 0.0);
+  }
+}
+// as gram_finish_kernel, eigenpairs taken from an npad-wide slot (W: ld npad, lam: npad values, the last n are the sector's)
+__global__ void gram_finish_padded_kernel(const cplx* __restrict__ W, const double* __restrict__ lam, int n, int npad,
+                                          double* __restrict__ sv, cplx* __restrict__ VT, cplx* __restrict__ Vs) {
+  const int64_t total = (int64_t)n * n;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x) {
+    const int j = (int)(e % n), i = (int)(e / n);
+    const double l = lam[npad - 1 - i];
+    const double sg = l > 0.0 ? sqrt(l) : 0.0;
+    const cplx v = W[j + (int64_t)(npad - 1 - i) * npad];
+    VT[i + (int64_t)j * n] = make_double2(v.x, -v.y);
+    const double r = sg > 0.0 ? 1.0 / sg : 0.0;
+    Vs[j + (int64_t)i * n] = make_double2(v.x * r, v.y * r);
+    if (j == 0) sv[i] = sg;
+  }
+}
+
 const int GESVDP_MIN_N = 48;  // below this the QR-iteration driver is as fast and has no conditioning caveat
 
 // SVD of one sector matrix on worker w: column-major B (m x n, m >= n) at buf + m_off ->
@@ -554,6 +590,59 @@ void svd_one(fh_ctx::SvdWorker& w, SectorSvd& S, cplx* buf, double* dS, int64_t*
                                (int)(w.dwork_bytes / sizeof(cuDoubleComplex)), nullptr, w.d_info));
   FH_CUDA(cudaMemcpyAsync(d_status, w.d_info, sizeof(int), cudaMemcpyDeviceToDevice, w.s));
   ++counts[0];
+}
+
+// The Gram route for SEVERAL sectors at once: their Gram matrices, padded to a common size, go through ONE
+// cusolverDnXsyevBatched call.  Why: a vendor eigensolver is a chain of ~1500 small dependent kernels (4.3 ms alone at
+// n = 352), and sixteen chains side by side take 20 ms per bond whatever the number of host threads -- the GPU front
+// end is what they queue on; the batched solver walks ONE chain for all of them (1.7 / 9.5 / 19.7 ms for 16 matrices of
+// 128 / 224 / 352 columns, measured), so the mid-sized majority is taken out of the queue of the few largest.
+void gram_batch(fh_ctx::SvdWorker& w, const std::vector<SectorSvd*>& order, const std::vector<int>& gb, cplx* buf, double* dS,
+                int* d_status) {
+  const int nb = (int)gb.size();
+  int npad = 0;
+  for (int x : gb) npad = std::max(npad, order[x]->k);
+  npad = (npad + 31) / 32 * 32;
+  const size_t slot = (size_t)npad * npad;
+  const size_t g_bytes = (slot * nb * sizeof(cplx) + 255) / 256 * 256;
+  const size_t l_bytes = ((size_t)npad * nb * sizeof(double) + 255) / 256 * 256;
+  const size_t i_bytes = ((size_t)nb * sizeof(int) + 255) / 256 * 256;
+  size_t wd = 0, wh = 0;
+  FH_CUSOLVER(cusolverDnXsyevBatched_bufferSize(w.h, w.params, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, npad, CUDA_C_64F,
+                                                nullptr, npad, CUDA_R_64F, nullptr, CUDA_C_64F, &wd, &wh, nb));
+  worker_reserve(w, 2 * g_bytes + l_bytes + i_bytes + wd + 256);
+  if (w.hwork.size() < wh + 16) w.hwork.resize(wh + 16);
+  char* base = (char*)w.dwork;
+  cuDoubleComplex* G = (cuDoubleComplex*)base;
+  cuDoubleComplex* Vs = (cuDoubleComplex*)(base + g_bytes);
+  double* lam = (double*)(base + 2 * g_bytes);
+  int* info = (int*)(base + 2 * g_bytes + l_bytes);
+  void* ws = base + 2 * g_bytes + l_bytes + i_bytes;
+  const cuDoubleComplex one = make_cuDoubleComplex(1.0, 0.0), zero = make_cuDoubleComplex(0.0, 0.0);
+  for (int x = 0; x < nb; ++x) {
+    const SectorSvd& S = *order[gb[x]];
+    const int m = std::max(S.nrow, S.ncol), n = S.k;
+    const cuDoubleComplex* A = (const cuDoubleComplex*)(buf + S.m_off);
+    FH_REQUIRE(cublasZgemm(w.cb, CUBLAS_OP_C, CUBLAS_OP_N, n, n, m, &one, A, m, A, m, &zero, G + x * slot, npad) ==
+                   CUBLAS_STATUS_SUCCESS,
+               FH_ECUDA, "svd: cublasZgemm (Gram matrix, batched route) failed");
+    gram_pad_kernel<<<1, 1024, 0, w.s>>>((cplx*)(G + x * slot), n, npad);
+  }
+  FH_CUSOLVER(cusolverDnXsyevBatched(w.h, w.params, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, npad, CUDA_C_64F, G, npad,
+                                     CUDA_R_64F, lam, CUDA_C_64F, ws, wd, w.hwork.data(), wh, info, nb));
+  for (int x = 0; x < nb; ++x) {
+    SectorSvd& S = *order[gb[x]];
+    const int m = std::max(S.nrow, S.ncol), n = S.k;
+    const cuDoubleComplex* A = (const cuDoubleComplex*)(buf + S.m_off);
+    const int64_t tot = (int64_t)n * n;
+    gram_finish_padded_kernel<<<(int)std::min<int64_t>((tot + 255) / 256, 296), 256, 0, w.s>>>(
+        (const cplx*)(G + x * slot), lam + (size_t)x * npad, n, npad, dS + S.s_off, buf + S.vt_off, (cplx*)(Vs + x * slot));
+    FH_REQUIRE(cublasZgemm(w.cb, CUBLAS_OP_N, CUBLAS_OP_N, m, n, n, &one, A, m, Vs + x * slot, n, &zero,
+                           (cuDoubleComplex*)(buf + S.u_off), m) == CUBLAS_STATUS_SUCCESS,
+               FH_ECUDA, "svd: cublasZgemm (U = B V / sigma, batched route) failed");
+    FH_CUDA(cudaMemcpyAsync(d_status + gb[x], info + x, sizeof(int), cudaMemcpyDeviceToDevice, w.s));
+    S.gram = true;
+  }
 }
 
 // Householder QR of one sector matrix (one-site split, no truncation): geqrf, R copied out, ungqr in place.
@@ -752,6 +841,17 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
     return m * n * n;
   };
   std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) { return cost(a) > cost(b); });
+  // the mid-sized Gram-route sectors of the bond go through ONE batched eigensolver call on the last worker
+  std::vector<int> gb;
+  if (gram_minn > 0 && nw >= 2) {
+    std::vector<int> rest;
+    for (int i : idx) {
+      const int n = order[i]->k;
+      if (n >= gram_minn && n <= ctx->opt_svd_gram_batch_maxn) gb.push_back(i); else rest.push_back(i);
+    }
+    if (gb.size() >= 2) idx.swap(rest); else gb.clear();
+  }
+  const int nw_one = gb.empty() ? nw : nw - 1;  // workers that pull single matrices
   std::atomic<int> next{0};
   std::vector<std::string> errs(nw);
   std::vector<std::array<int64_t, 4>> counts(nw, std::array<int64_t, 4>{0, 0, 0, 0});
@@ -771,17 +871,35 @@ void run_sector_svds(fh_ctx* ctx, const std::vector<SectorSvd*>& order, cplx* bu
       if (errs[wi].empty()) errs[wi] = "unknown error";
     }
   };
-  const int nthreads = std::min<int>(nw, (int)idx.size());
-  if (nthreads <= 1) {
-    body(0);
-  } else {
+  const int nthreads = std::min<int>(nw_one, (int)idx.size());
+  auto batch_body = [&]() {
+    try {
+      FH_CUDA(cudaSetDevice(ctx->device));
+      fh_ctx::SvdWorker& w = ctx->svd_workers[nw - 1];
+      gram_batch(w, order, gb, buf, dS, d_status);
+      counts[nw - 1][3] += (int64_t)gb.size();
+      FH_CUDA(cudaEventRecord(w.done, w.s));
+    } catch (const std::exception& e) {
+      errs[nw - 1] = e.what();
+      if (errs[nw - 1].empty()) errs[nw - 1] = "unknown error";
+    }
+  };
+  {
     std::vector<std::thread> th;
-    for (int t = 0; t < nthreads; ++t) th.emplace_back(body, t);
+    if (!gb.empty()) th.emplace_back(batch_body);
+    if (nthreads <= 1 && gb.empty()) {
+      body(0);
+    } else {
+      for (int t = 0; t < std::max(1, nthreads); ++t) th.emplace_back(body, t);
+    }
     for (auto& t : th) t.join();
   }
   // join every stream that was forked before reporting a worker's failure: nothing may still run on them
   std::string first_err;
-  for (int t = 0; t < std::max(1, nthreads); ++t) {
+  std::vector<int> used;
+  for (int t = 0; t < std::max(1, nthreads); ++t) used.push_back(t);
+  if (!gb.empty()) used.push_back(nw - 1);
+  for (int t : used) {
     if (!errs[t].empty()) {
       if (first_err.empty()) first_err = errs[t];
       cudaStreamSynchronize(ctx->svd_workers[t].s);

@@ -441,7 +441,7 @@ def test_config1_neel_quench_L8_vs_oracle(H, ctx):
 
 
 @pytest.mark.parametrize("L,chi,route", [(12, 128, "default"), (14, 200, "default"), (12, 128, "mid"), (12, 128, "vendor"),
-                                         (12, 128, "gram"), (14, 200, "gram")])
+                                         (12, 128, "gram"), (14, 200, "gram"), (14, 200, "gram1")])
 def test_config3_sweep_recipe_reduced_size_vs_oracle(H, ctx, L, chi, route):
     """The second half of BASELINE config 3 -- one tdvp2_sweep(0.05), m = 10, truncation back to chi by block-wise
     SVD, started from the seeded random canonical chain (the recipe bench.py times at L = 60,
@@ -454,12 +454,16 @@ def test_config3_sweep_recipe_reduced_size_vs_oracle(H, ctx, L, chi, route):
     `route` sends the sector matrices of this small case through the factorisation routes that large bonds use
     (fh_set_option): "mid" = the global-memory Jacobi kernel and cusolver's geqrf/ungqr, "vendor" = cusolver's
     gesvdp / gesvd and geqrf/ungqr; "default" = the shared-memory Jacobi and Householder kernels; "gram" = the
-    Gram-matrix eigenvalue route (G = B^H B, Zheevd, U = B V / sigma) for every matrix of at least 8 columns, with its
-    acceptance test on the kept singular values and the vendor redo of the sectors that fail it."""
+    Gram-matrix eigenvalue route (G = B^H B, eigendecomposition, U = B V / sigma) for every matrix of at least 8
+    columns, the eigenproblems of a bond solved in one batched vendor call on Gram matrices padded to a common size
+    ("gram1": one Zheevd call per matrix), with its acceptance test on the kept singular values and the vendor redo of
+    the sectors that fail it."""
     if route != "default":
         ctx.fh_set_option(ctx.OPT_SVD_SMALL_MAXN, 0)
         ctx.fh_set_option(ctx.OPT_SVD_MID_MAXN, 128 if route == "mid" else 0)
-    ctx.fh_set_option(ctx.OPT_SVD_GRAM_MINN, 8 if route == "gram" else 0)
+    ctx.fh_set_option(ctx.OPT_SVD_GRAM_MINN, 8 if route.startswith("gram") else 0)
+    if route == "gram1":                                  # one eigensolver call per matrix instead of the batched call
+        ctx.fh_set_option(ctx.OPT_SVD_GRAM_BATCH_MAXN, 0)
     dims = fi.chain_dims(chi, L, "gaussian", (1, 1))
     sites = {}
     for i, A, dl, dr in fi.canonical_chain(chi, 0, L, fi.SEED, dims=dims, weight=symm.canonical_weight):
@@ -506,7 +510,7 @@ def test_config3_sweep_recipe_reduced_size_vs_oracle(H, ctx, L, chi, route):
     if route == "vendor":
         assert routes["gesvdp"] + routes["gesvd"] > 0 and routes["jacobi_kernel"] == routes["jacobi_mid_kernel"] == 0
         assert routes["gram_eig"] == 0
-    if route == "gram":
+    if route.startswith("gram"):
         assert routes["gram_eig"] > 0 and routes["jacobi_kernel"] == routes["jacobi_mid_kernel"] == 0
         assert routes["gram_redone"] < routes["gram_eig"]          # some sectors pass the acceptance test
     print("L=%d chi=%d sweep: sv %.1e s_max, obs %.1e / one-site %.1e, discarded %.3e (oracle %.3e); SVD routes %s; "
