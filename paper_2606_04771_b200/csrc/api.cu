@@ -251,6 +251,9 @@ void fh::prefetch_cancel(fh_ctx* ctx) {
   }
 }
 
+// padded DMMAs per apply between which the warp-specialised single launch is the faster form
+static const int64_t WS_MIN_DMMA = 10000000, WS_MAX_DMMA = 400000000;
+
 void fh::plan_heff(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, int nsite) {
   FH_REQUIRE(nsite == 1 || nsite == 2, FH_EINVAL, "heff_plan: nsite must be 1 or 2");
   FH_REQUIRE(site >= 0 && site + nsite <= mps->L, FH_EINVAL, "heff_plan: site out of range");
@@ -321,11 +324,23 @@ void fh::plan_heff(fh_ctx* ctx, const fh_mpo* mpo, const fh_mps* mps, int site, 
     }
   }
   ctx->alloc_tensor(P.Z);
+  // Tile queue of the warp-specialised form: only for the plans that will use it (FH_OPT_GEMM_PATH as it is NOW: set
+  // it before heff_plan).  Every other plan of a sweep (one-site, and two-site plans outside the window) skips
+  // the emission, the dependency lists and their upload.
+  P.pair = WsPair();
+  {
+    const int64_t dmma = P.st1.dmma_padded + P.st2.dmma_padded;
+    const bool want_ws = nsite == 2 && (ctx->opt_gemm_path == 2 || (ctx->opt_gemm_path == 0 && dmma >= WS_MIN_DMMA && dmma < WS_MAX_DMMA));
+    if (want_ws) {
+      emit_ws_tiles(P.st1);
+      emit_ws_tiles(P.st2);
+      link_stages(P.st1, P.st2, 0, P.pair);  // stage 2 reads the intermediate as its left operand
+    }
+  }
   P.ws_scratch_n = (int64_t)(P.st1.n_slots + P.st2.n_slots) * WS_SLOT_ELEMS;
   if (P.ws_scratch_n > 0) P.ws_scratch = ctx->alloc.alloc(P.ws_scratch_n);
   P.Lptr = ctx->ptr(Le.base);
   P.Rptr = ctx->ptr(Re.base);
-  link_stages(P.st1, P.st2, 0, P.pair);  // stage 2 reads the intermediate as its left operand
   P.upair = UnitPair();
   if (nsite == 2 && ctx->opt_gemm_path == 3) link_units(P.st1, P.st2, 0, P.upair);  // only on request: measured equal or slower
   const size_t upair_bytes = P.upair.units.size() * (sizeof(GemmUnit) + sizeof(UnitLink)) + P.upair.segs.size() * sizeof(GemmSeg) +
@@ -471,7 +486,7 @@ void fh::apply_heff(fh_ctx* ctx, const cplx* theta, cplx* out) {
   // at chi = 4096, and loses below (its start-up is longer than that of 148 x 8 one-warp CTAs).
   const int64_t dmma = P.st1.dmma_padded + P.st2.dmma_padded;
   const bool use_ws = P.nsite == 2 && !P.pair.tiles.empty() &&
-                      (ctx->opt_gemm_path == 2 || (ctx->opt_gemm_path == 0 && dmma >= 10000000 && dmma < 400000000));
+                      (ctx->opt_gemm_path == 2 || (ctx->opt_gemm_path == 0 && dmma >= WS_MIN_DMMA && dmma < WS_MAX_DMMA));
   if (use_ws) {
     ++P.ws_epoch;
     cplx* sc = P.ws_scratch >= 0 ? ctx->ptr(P.ws_scratch) : nullptr;

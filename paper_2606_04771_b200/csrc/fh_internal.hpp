@@ -262,6 +262,7 @@ struct WsPair {
   unsigned* d_dep_target = nullptr;
 };
 // which operand of stage 2 is stage 1's result: 0 = A (lhs), 1 = B (rhs)
+void emit_ws_tiles(Stage& st);  // tile list of one stage (call before link_stages)
 void link_stages(const Stage& st1, const Stage& st2, int mid_is_rhs2, WsPair& out);
 void launch_grouped_gemm_ws_pair(const WsPair& pr, const cplx* A1, const cplx* B1, cplx* C1, const cplx* A2, const cplx* B2,
                                  cplx* C2, unsigned* d_counters, int grid, cplx* scratch, unsigned* flags,

@@ -339,7 +339,7 @@ static void emit_units(Stage& st) {
 // chunk boundaries (16 k); all parts but the one that starts at k = 0 leave their accumulators in a scratch
 // slot, and that one adds them in slot order and stores the block (fixed order: deterministic).  In the queue
 // the parts of a tile come before its finishing part, so a finisher never waits for work not yet handed out.
-static void emit_tiles(Stage& st) {
+void emit_ws_tiles(Stage& st) {
   st.tiles.clear();
   st.n_slots = 0;
   st.mout_tiles.assign(st.mouts.size(), 0);
@@ -707,7 +707,10 @@ void finalize_stage(Stage& st, const BlockTensor& out, const BlockTensor& lhs, c
   if (t != nt) throw std::runtime_error("task list: tasks not sorted by output id");
   merge_outs(st, lhs.nelem, rhs.nelem);
   emit_units(st);
-  emit_tiles(st);
+  // the tile list of the warp-specialised form is emitted on demand (emit_ws_tiles): only two-site plans in its size
+  // window use it, and every stage of a sweep passes through here
+  st.tiles.clear();
+  st.n_slots = 0;
 }
 
 namespace {

@@ -1300,7 +1300,7 @@ static void plan_zero_site(fh_ctx* ctx, fh_mps* mps, int bond, const BlockTensor
   if (P.ws_scratch_n > 0) P.ws_scratch = ctx->alloc.alloc(P.ws_scratch_n);
   P.Lptr = ctx->ptr(Le.base);
   P.Rptr = ctx->ptr(Re.base);
-  link_stages(P.st1, P.st2, 0, P.pair);  // stage 2 reads the intermediate as its left operand
+  P.pair = WsPair();  // the zero-site apply always runs as warp units
   const size_t need = stage_bytes(P.st1) + stage_bytes(P.st2) + pair_bytes(P.pair) +
                       P.chunks.size() * (sizeof(VecChunk) + 16) + 8192;
   P.pool.reserve(need, ctx->stream);
