@@ -46,6 +46,9 @@ def parse_args():
     ap.add_argument("--extra-chi", type=int, nargs="*", default=None,
                     help="replace the default other_configs list by Gaussian-profile applies at these chi (e.g. 32768 49152: "
                          "BASELINE config 5 sizes, minutes of host time to generate the environments)")
+    ap.add_argument("--set-option", action="append", default=[], metavar="NAME=VALUE",
+                    help="fh_set_option on the main context before anything is planned, e.g. SVD_GRAM_MINN=0, "
+                         "SVD_GRAM_BATCH_MAXN=0, SVD_THREADS=6, GEMM_PATH=2 (names: binding.Context.OPT_*); recorded in config")
     ap.add_argument("--no-extra", action="store_true",
                     help="skip the apply-only lines of the other configs (chi = 1024, Table S2 x 1/6, 16384, 24576) and "
                          "the oracle timings on configs 1, 2, 5'")
@@ -396,6 +399,9 @@ def run_ours(args):
     sweep_need = 0.0 if args.no_sweep else 300.0 * args.sweep_chi * args.sweep_chi
     arena = int(min(160e9, max(16 << 30, 64.0 * chi * chi, sweep_need)))
     ctx = H.binding.Context(arena, device="cuda:%d" % local)
+    for kv in args.set_option:
+        name, val = kv.split("=")
+        ctx.fh_set_option(getattr(ctx, "OPT_" + name.upper()), int(val))
     mpo = ctx.fh_mpo_build(L, 1.0, 4.0)
     t_build = time.perf_counter()
     mps, dims = H.build_central_bond(ctx, mpo, chi, L, profile=args.profile, table_s2_scale=s2_scale(args))
@@ -481,7 +487,8 @@ def run_ours(args):
                    "d_max": max(max(dims[k].values()) for k in (c, c + 2)), "theta_blocks": len(lab),
                    "z_blocks": nz, "tasks": [len(t1), len(t2)], "flop_per_apply": flops, "theta_bytes": zbytes,
                    "l2": "not flushed" if flush is None else "flushed between timed applies (256 MiB write, outside the event pairs)",
-                   "parallelism": "replicas only (one GPU per problem, no collectives)", "setup_seconds": t_build},
+                   "parallelism": "replicas only (one GPU per problem, no collectives)", "setup_seconds": t_build,
+                   "options": list(args.set_option)},
         "value_l2_warm": world * flops * args.steps / t_warm * 1e-9,
         "roofline": {"kernel": ("grouped_zgemm_tc_kernel (split precision; the FP64 peak below is NOT its roofline)" if args.precision == "split" else
                                 "grouped_zgemm_kernel (stage 1 + stage 2 launches of one apply)" if launches == 2 * args.steps else
